@@ -1,0 +1,216 @@
+/*
+ * attn_jvp_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU statement of what the attention-JVP hot path computes,
+ * written from the paper's definitions (App. B, Eq. 42-44), NOT from
+ * Algorithm 1: the mask row, the scores s, the probabilities p and the score
+ * tangents ts are materialised explicitly for every query row; there is no
+ * tiling, no online softmax, no range list, no fusion.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  It shares no code,
+ * header, table or helper with paper_2606_25473_b200/ (the CUDA path), and the
+ * CUDA path never calls it.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): central finite differences
+ * of O along the tangent, brute-force dense masked attention written
+ * independently in numpy, torch.func.jvp / SDPA / logsumexp, closed forms,
+ * invariants and pair counts.  Every exported function below is pinned; none is
+ * "parity unpinned".
+ *
+ * Definitions followed (PAPER.md line : item):
+ *   842-844  Eq. 42  O = softmax(Q K^T / sqrt(d) + M) V,  M in {0,-inf}
+ *   846-848  Eq. 43  tS = (tQ K^T + Q tK^T) / sqrt(d)
+ *   851-854  masked entries: S = -inf, tS = 0 (the mask has no tangent)
+ *   862-864  Eq. 44  tO_a = sum_b p_ab tV_b + sum_b p_ab (tS_ab - sum_c p_ac tS_ac) V_b
+ *   945      L = m + log(l)  (log-sum-exp of the scaled, masked scores)
+ *   175-180  Eq. 8 / teacher-forcing mask over the packed [clean | noisy] sequence
+ *   882-886  generic mask = query groups with key-range lists
+ * Readings where the paper is silent are DESIGN.md R1 (both S and tS carry the
+ * scale), R4 (exact TF predicate), R6 (block index), R9 (row with no allowed
+ * key: O = 0, tO = 0, lse = -inf).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+enum { AJO_MASK_FULL = 0, AJO_MASK_BLOCK_CAUSAL = 1, AJO_MASK_TEACHER_FORCING = 2, AJO_MASK_RANGES = 3 };
+enum { AJO_F32 = 0, AJO_F64 = 1 };
+
+typedef struct {
+    int32_t kind;
+    int32_t block_len;       /* C: tokens per block (frame_len * chunk_frames)          */
+    int32_t num_blocks;      /* n: blocks (per half for TEACHER_FORCING)                */
+    int32_t first_block_len; /* C1: tokens in block 0; 0 means C                        */
+    /* AJO_MASK_RANGES only: group g owns query rows
+       [q_begin[g], q_end[g]) and may see keys in the union of
+       [k_begin[r], k_end[r]) for r in [range_offset[g], range_offset[g+1]).  */
+    int32_t num_groups;
+    const int32_t *q_begin, *q_end, *range_offset, *k_begin, *k_end;
+} ajo_mask;
+
+/* Block index of token x inside one half: blocks have length C1, C, C, ... (R6). */
+static int64_t ajo_block_of(const ajo_mask *m, int64_t x)
+{
+    int64_t c1 = m->first_block_len > 0 ? m->first_block_len : m->block_len;
+    if (x < c1) return 0;
+    return 1 + (x - c1) / m->block_len;
+}
+
+static int64_t ajo_half_len(const ajo_mask *m)
+{
+    int64_t c1 = m->first_block_len > 0 ? m->first_block_len : m->block_len;
+    return c1 + (int64_t)(m->num_blocks - 1) * m->block_len;
+}
+
+/* May query token a attend to key token b?  The plain predicate (R4). */
+int attn_jvp_oracle_allowed(const ajo_mask *m, int64_t a, int64_t b)
+{
+    switch (m->kind) {
+    case AJO_MASK_FULL:
+        return 1;
+    case AJO_MASK_BLOCK_CAUSAL:
+        /* block i attends blocks <= i */
+        return ajo_block_of(m, b) <= ajo_block_of(m, a);
+    case AJO_MASK_TEACHER_FORCING: {
+        /* packed sequence [clean | noisy] (Eq. 8) */
+        int64_t half = ajo_half_len(m);
+        int a_clean = a < half, b_clean = b < half;
+        if (a_clean) {
+            /* clean block i -> clean blocks <= i; clean never sees noisy */
+            if (!b_clean) return 0;
+            return ajo_block_of(m, b) <= ajo_block_of(m, a);
+        } else {
+            int64_t i = ajo_block_of(m, a - half);
+            /* noisy block i -> clean blocks < i, plus noisy block i itself */
+            if (b_clean) return ajo_block_of(m, b) < i;
+            return ajo_block_of(m, b - half) == i;
+        }
+    }
+    case AJO_MASK_RANGES:
+        for (int g = 0; g < m->num_groups; ++g) {
+            if (a < m->q_begin[g] || a >= m->q_end[g]) continue;
+            for (int r = m->range_offset[g]; r < m->range_offset[g + 1]; ++r)
+                if (b >= m->k_begin[r] && b < m->k_end[r]) return 1;
+        }
+        return 0;
+    default:
+        return 0;
+    }
+}
+
+/* Unmasked (query, key) pairs of one head, by counting the predicate. */
+int64_t attn_jvp_oracle_count_pairs(const ajo_mask *m, int64_t nq, int64_t nk)
+{
+    int64_t total = 0;
+#pragma omp parallel for schedule(static) reduction(+ : total)
+    for (int64_t a = 0; a < nq; ++a) {
+        int64_t c = 0;
+        for (int64_t b = 0; b < nk; ++b) c += attn_jvp_oracle_allowed(m, a, b);
+        total += c;
+    }
+    return total;
+}
+
+static inline double ajo_load(const void *p, int dtype, int64_t idx)
+{
+    return dtype == AJO_F64 ? ((const double *)p)[idx] : (double)((const float *)p)[idx];
+}
+
+/*
+ * One (batch, head) slice.  q, tq: [nq, d]; k, v, tk, tv: [nk, d]; rows contiguous
+ * with stride d; dtype says whether they hold float or double (values are widened
+ * exactly).  rows[0..nrows) lists the query rows to evaluate (NULL = rows 0..nrows-1).
+ * Outputs, all fp64: o, to: [nrows, d]; lse: [nrows].
+ * Returns 0, or -1 on a bad argument / allocation failure.
+ */
+int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d, double scale,
+                         int32_t dtype, const void *q, const void *k, const void *v,
+                         const void *tq, const void *tk, const void *tv,
+                         const int64_t *rows, int64_t nrows,
+                         double *o, double *to, double *lse)
+{
+    if (!mask || nq <= 0 || nk <= 0 || d <= 0 || nrows < 0) return -1;
+    if (dtype != AJO_F32 && dtype != AJO_F64) return -1;
+    int failed = 0;
+#pragma omp parallel
+    {
+        double *s = (double *)malloc(sizeof(double) * (size_t)nk);   /* scores, then p */
+        double *ts = (double *)malloc(sizeof(double) * (size_t)nk);  /* score tangents */
+        unsigned char *ok = (unsigned char *)malloc((size_t)nk);     /* mask row       */
+        double *qa = (double *)malloc(sizeof(double) * (size_t)d);
+        double *tqa = (double *)malloc(sizeof(double) * (size_t)d);
+        if (!s || !ts || !ok || !qa || !tqa) {
+#pragma omp atomic write
+            failed = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t i = 0; i < nrows; ++i) {
+                int64_t a = rows ? rows[i] : i;
+                double *oa = o + i * d, *toa = to + i * d;
+                for (int c = 0; c < d; ++c) { oa[c] = 0.0; toa[c] = 0.0; }
+                if (a < 0 || a >= nq) { lse[i] = NAN; continue; }
+                for (int c = 0; c < d; ++c) {
+                    qa[c] = ajo_load(q, dtype, a * d + c);
+                    tqa[c] = ajo_load(tq, dtype, a * d + c);
+                }
+                /* mask row, Eq. 42 scores, Eq. 43 score tangents */
+                double m = -INFINITY;
+                for (int64_t b = 0; b < nk; ++b) {
+                    ok[b] = (unsigned char)attn_jvp_oracle_allowed(mask, a, b);
+                    if (!ok[b]) { s[b] = -INFINITY; ts[b] = 0.0; continue; }
+                    double qk = 0.0, tqk = 0.0, qtk = 0.0;
+                    for (int c = 0; c < d; ++c) {
+                        double kb = ajo_load(k, dtype, b * d + c);
+                        double tkb = ajo_load(tk, dtype, b * d + c);
+                        qk += qa[c] * kb;
+                        tqk += tqa[c] * kb;
+                        qtk += qa[c] * tkb;
+                    }
+                    s[b] = scale * qk;
+                    ts[b] = scale * (tqk + qtk);
+                    if (s[b] > m) m = s[b];
+                }
+                if (m == -INFINITY) { lse[i] = -INFINITY; continue; } /* R9 */
+                /* masked softmax over the allowed keys */
+                double z = 0.0;
+                for (int64_t b = 0; b < nk; ++b) {
+                    s[b] = ok[b] ? exp(s[b] - m) : 0.0;
+                    z += s[b];
+                }
+                for (int64_t b = 0; b < nk; ++b) s[b] /= z; /* s now holds p_ab */
+                lse[i] = m + log(z);
+                /* mu = sum_c p_ac tS_ac */
+                double mu = 0.0;
+                for (int64_t b = 0; b < nk; ++b) mu += s[b] * ts[b];
+                /* O = sum p v;  Eq. 44 */
+                for (int64_t b = 0; b < nk; ++b) {
+                    if (!ok[b]) continue;
+                    double p = s[b], w = p * (ts[b] - mu);
+                    for (int c = 0; c < d; ++c) {
+                        double vb = ajo_load(v, dtype, b * d + c);
+                        double tvb = ajo_load(tv, dtype, b * d + c);
+                        oa[c] += p * vb;
+                        toa[c] += p * tvb + w * vb;
+                    }
+                }
+            }
+        }
+        free(s); free(ts); free(ok); free(qa); free(tqa);
+    }
+    return failed ? -1 : 0;
+}
+
+/* Threads an oracle call will use (reported by bench.py as cpu_baseline.cores). */
+int attn_jvp_oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,101 @@
+"""Seeded synthetic workloads (BASELINE.json `configs`) -- shapes and random draws only.
+
+This module holds NONE of the method's arithmetic: it names the five benchmark
+configurations, and draws Q, K, V, tQ, tK, tV from a seeded CPU generator.  Both the
+CUDA path's callers (tests, bench.py) and the oracle's callers use it, so the two
+sides see bit-identical inputs; neither side's arithmetic lives here.
+
+Recipe: one ``torch.Generator`` (CPU) seeded with
+``seed`` draws Q, K, V, tQ, tK, tV in that order as fp32 N(0,1) of shape [B,H,N,d];
+the tangents are multiplied by ``tangent_std``; everything is then cast to the config
+dtype (round-to-nearest-even).  The oracle receives the cast values widened to fp32.
+These tensors stand in for Wan2.1-1.3B activations, which are not
+available here.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Dict, List
+
+import torch
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    B: int
+    H: int
+    d: int
+    mask: str            # "teacher_forcing" | "block_causal" | "full"
+    frame_len: int       # L tokens per latent frame
+    num_frames: int      # F latent frames (per half for teacher forcing)
+    chunk_frames: int    # frames per block: 1 = frame-wise (c1-1), 3 = chunk-wise (c3-3)
+    dtype: str           # "bf16" | "fp32"
+    tangent_std: float
+    seed: int = 0
+
+    @property
+    def block_len(self) -> int:
+        return self.frame_len * self.chunk_frames
+
+    @property
+    def num_blocks(self) -> int:
+        assert self.num_frames % self.chunk_frames == 0
+        return self.num_frames // self.chunk_frames
+
+    @property
+    def N(self) -> int:
+        half = self.frame_len * self.num_frames
+        return 2 * half if self.mask == "teacher_forcing" else half
+
+    @property
+    def torch_dtype(self):
+        return torch.bfloat16 if self.dtype == "bf16" else torch.float32
+
+    @property
+    def unmasked_pairs_per_head(self) -> int:
+        """Size of the allowed set, from the shape alone (closed form; P6)."""
+        n, C = self.num_blocks, self.block_len
+        tri = n * (n + 1) // 2
+        if self.mask == "teacher_forcing":
+            return 2 * tri * C * C
+        if self.mask == "block_causal":
+            return tri * C * C
+        return self.N * self.N
+
+
+# BASELINE.json configs[0..4] (+ the full-mask control of configs[4]).
+WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
+    Workload("tiny_tf_fp32", 1, 2, 64, "teacher_forcing", 16, 3, 1, "fp32", 1.0),
+    Workload("wan13b_tf_framewise", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1),
+    Workload("wan13b_tf_chunkwise", 1, 12, 128, "teacher_forcing", 1560, 21, 3, "bf16", 0.1),
+    Workload("block_causal_b2", 2, 12, 128, "block_causal", 1560, 21, 1, "bf16", 0.1),
+    Workload("dit_large_tf_chunkwise", 1, 24, 128, "teacher_forcing", 3600, 16, 2, "bf16", 0.1),
+    Workload("dit_large_full", 1, 24, 128, "full", 3600, 32, 2, "bf16", 0.1),
+]}
+CONFIG_ORDER: List[str] = list(WORKLOADS)
+
+
+def scaled_down(w: Workload, frame_len: int, num_frames: int = 0, H: int = 0, B: int = 0) -> Workload:
+    """Same structure, smaller extent (parity cases the oracle finishes in seconds)."""
+    return Workload(f"{w.name}@L{frame_len}", B or w.B, H or w.H, w.d, w.mask, frame_len,
+                    num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed)
+
+
+def make_inputs(w: Workload, device: str = "cpu", pin: bool = False):
+    """Returns [q, k, v, tq, tk, tv], each [B, H, N, d] in the config dtype."""
+    g = torch.Generator(device="cpu")
+    g.manual_seed(w.seed)
+    shape = (w.B, w.H, w.N, w.d)
+    out = []
+    for i in range(6):
+        x = torch.randn(shape, generator=g, dtype=torch.float32)
+        if i >= 3:
+            x.mul_(w.tangent_std)
+        x = x.to(w.torch_dtype)
+        if device != "cpu":
+            x = x.to(device)
+        elif pin:
+            x = x.pin_memory()
+        out.append(x)
+    return out
