@@ -1,0 +1,160 @@
+/*
+ * attn_jvp.h -- C ABI of the B200 (sm_100a) fused attention + JVP library.
+ *
+ * One pass over Q, K, V and their tangents tQ, tK, tV returns
+ *     O   = softmax(mask(Q K^T * s)) V                         (Eq. 42)
+ *     tO  = sum_b p_ab tV_b + sum_b p_ab (tS_ab - sum_c p_ac tS_ac) V_b   (Eq. 44)
+ *     lse = log-sum-exp of the masked scaled scores             (Alg. 1 "L")
+ * with tS = (tQ K^T + Q tK^T) * s (Eq. 43); masked entries have S = -inf and
+ * tS = 0.  The computation is the online-softmax recurrence of PAPER.md:866-878
+ * (Alg. 1) under the sparse query-group / key-range mask of PAPER.md:880-886.
+ *
+ * Conventions
+ *  - All functions are extern "C", never throw, never synchronise the stream, and return an
+ *    aj_status; attn_jvp_last_error() gives a thread-local message for the last failure.
+ *  - The caller owns every tensor.  "device" pointers are CUDA device memory of the current
+ *    device; "host" pointers are ordinary (preferably pinned) host memory.
+ *  - Tensors are [B, H, N, d] with d contiguous; strides are in ELEMENTS (aj_tensor).
+ *  - Supported: d in {64, 128}; dtype AJ_FP32 (plain-FMA SIMT kernel, any supported d) and
+ *    AJ_BF16 (tcgen05/TMEM/TMA kernel for d = 128; SIMT kernel otherwise).  Anything else
+ *    returns AJ_ERR_UNSUPPORTED.  There is no CPU fallback.
+ *  - Inputs must be finite: masked-out tail keys are multiplied by an exact 0 (R15).
+ */
+#ifndef ATTN_JVP_H_
+#define ATTN_JVP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    AJ_OK = 0,
+    AJ_ERR_INVALID_ARG = -1, /* null pointer, bad shape, misaligned pointer/stride, bad descriptor */
+    AJ_ERR_UNSUPPORTED = -2, /* valid request this build has no kernel for (d, dtype)              */
+    AJ_ERR_CUDA = -3,        /* a CUDA runtime/driver call failed (message has the CUDA error)     */
+    AJ_ERR_OOM = -4          /* host or device allocation failed                                   */
+} aj_status;
+
+typedef enum { AJ_BF16 = 0, AJ_FP32 = 1 } aj_dtype;
+
+/* Mask kinds (PAPER.md:175-180 Eq. 8 teacher forcing; :155 block-causal; :886 dense; :882-886 ranges). */
+typedef enum {
+    AJ_MASK_FULL = 0,            /* every query sees every key                                          */
+    AJ_MASK_BLOCK_CAUSAL = 1,    /* block i sees blocks <= i                                             */
+    AJ_MASK_TEACHER_FORCING = 2, /* packed [clean | noisy]: clean i -> clean <= i; noisy i -> clean < i
+                                    and noisy i; nothing else                                             */
+    AJ_MASK_RANGES = 3           /* explicit query groups with key-range lists                            */
+} aj_mask_kind;
+
+/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA when (bf16, d = 128), else SIMT. */
+typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2 } aj_kernel;
+
+/*
+ * Mask descriptor = the paper's problem statement.  Structured kinds: a block is
+ * chunk_frames * frame_len tokens (frame-wise c1-1: chunk_frames = 1; chunk-wise c3-3: 3;
+ * PAPER.md:398); block 0 has first_chunk_frames frames if that is > 0.  num_frames counts latent
+ * frames per half; the sequence must be num_frames*frame_len tokens (twice that for
+ * TEACHER_FORCING, clean half first: PAPER.md:177).  AJ_MASK_RANGES: group g owns query rows
+ * [q_begin[g], q_end[g]) and sees keys in the union of [k_begin[r], k_end[r]) for
+ * r in [range_offset[g], range_offset[g+1]); groups must be disjoint, each group's ranges sorted
+ * and disjoint, everything inside [0,Nq) x [0,Nk) (else AJ_ERR_INVALID_ARG).  The arrays are HOST
+ * pointers and are copied by the call that receives the descriptor.  Rows in no group, or with an
+ * empty key list, get O = 0, tO = 0, lse = -inf.
+ */
+typedef struct {
+    int32_t kind;               /* aj_mask_kind */
+    int32_t frame_len;          /* L tokens per latent frame */
+    int32_t num_frames;         /* F frames (per half for TEACHER_FORCING) */
+    int32_t chunk_frames;       /* frames per block */
+    int32_t first_chunk_frames; /* 0 = same as chunk_frames */
+    int32_t num_groups;         /* AJ_MASK_RANGES only, as are the five arrays below */
+    const int32_t *q_begin, *q_end, *range_offset, *k_begin, *k_end;
+} aj_mask_desc;
+
+typedef struct {
+    int32_t B, H, Nq, Nk, d;
+    int32_t dtype; /* aj_dtype of q,k,v,tq,tk,tv,o,to; lse is always fp32 */
+    float scale;   /* softmax scale s applied to S and tS; 0 means 1/sqrt(d) */
+} aj_problem;
+
+/* A [B,H,N,d] tensor view: element strides, d contiguous. */
+typedef struct {
+    void *ptr;
+    int64_t stride_b, stride_h, stride_n;
+} aj_tensor;
+
+/* One unit of work: a query tile inside one query group, for one (b, h) ("tasks (g,i)"). */
+typedef struct {
+    int32_t b, h;
+    int32_t q_begin, q_rows;          /* query rows [q_begin, q_begin + q_rows) */
+    int32_t range_begin, range_count; /* its key ranges: schedule ranges [range_begin, +range_count) */
+    int32_t num_kv_tiles;             /* key tiles it streams (sum over ranges of ceil(len / tile_k)) */
+    int32_t group;                    /* index of its query group */
+} aj_task;
+
+typedef struct aj_schedule aj_schedule; /* host-only: groups, merged ranges, ordered task list */
+typedef struct aj_plan aj_plan;         /* schedule + its device copy + staging buffers       */
+
+/* ---- Host-side scheduler (no GPU needed): descriptor -> groups/ranges -> tile tasks (Alg. 1 input) ---- */
+
+/* Lowers `mask` to disjoint query groups with sorted, merged key ranges, cuts every group into query
+ * tiles of tile_q rows starting at the group start, and orders the tasks longest-first (ties: b, h,
+ * group, tile).  tile_q, tile_k > 0.  *out is owned by the caller (attn_jvp_schedule_destroy). */
+aj_status attn_jvp_schedule_create(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
+                                   int32_t tile_k, aj_schedule **out);
+aj_status attn_jvp_schedule_destroy(aj_schedule *sched);
+/* Any out pointer may be NULL. unmasked_pairs_per_head = sum over groups of rows * allowed keys. */
+aj_status attn_jvp_schedule_info(const aj_schedule *sched, int32_t *num_groups, int32_t *num_ranges,
+                                 int32_t *num_tasks, int64_t *unmasked_pairs_per_head);
+/* Copy out the lowered mask: q_begin, q_end [num_groups]; range_offset [num_groups + 1];
+ * k_begin, k_end [num_ranges]; tasks [num_tasks].  NULL pointers are skipped. */
+aj_status attn_jvp_schedule_get(const aj_schedule *sched, int32_t *q_begin, int32_t *q_end,
+                                int32_t *range_offset, int32_t *k_begin, int32_t *k_end, aj_task *tasks);
+
+/* ---- Plans and the forward call ---- */
+
+/* Validates the problem, builds the schedule for the kernel that will run and uploads it (one H2D copy,
+ * synchronous).  Needs a CUDA device.  Errors: INVALID_ARG, UNSUPPORTED, CUDA, OOM. */
+aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *mask, aj_plan **out);
+aj_status attn_jvp_plan_destroy(aj_plan *plan);
+aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_head, int32_t *num_tasks);
+/* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
+ * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged. */
+aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
+/* Which kernel attn_jvp_fwd will launch (aj_kernel, never AUTO) and how many kernel launches one
+ * attn_jvp_fwd call makes. */
+aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *launches_per_call);
+
+/*
+ * Enqueues the fused forward + JVP on `cuda_stream` (a cudaStream_t; NULL = default stream) and returns
+ * without waiting.  q, tq: [B,H,Nq,d]; k, v, tk, tv: [B,H,Nk,d]; o, to: [B,H,Nq,d] in the problem dtype;
+ * lse: contiguous fp32 [B,H,Nq] (may be NULL).  All DEVICE memory; inputs are only read.  Pointers must be
+ * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
+ * A plan must not be used by two streams at the same time (it owns a device work counter).
+ */
+aj_status attn_jvp_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v,
+                       const aj_tensor *tq, const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o,
+                       const aj_tensor *to, float *lse, void *cuda_stream);
+
+/*
+ * Same computation on HOST buffers: contiguous [B,H,N,d] arrays in the problem dtype (lse fp32
+ * [B,H,Nq], may be NULL).  Copies the six inputs to plan-owned device staging buffers (allocated on
+ * first use), runs attn_jvp_fwd, copies o, to, lse back, all asynchronously on `cuda_stream`; the
+ * caller synchronises the stream before reading the outputs.  Pinned host memory is needed for the
+ * copies to overlap; pageable memory works but is staged by the runtime.
+ */
+aj_status attn_jvp_fwd_host(aj_plan *plan, const void *q, const void *k, const void *v, const void *tq,
+                            const void *tk, const void *tv, void *o, void *to, float *lse,
+                            void *cuda_stream);
+
+/* Message for the most recent non-OK status returned to this thread ("" if none). Never NULL. */
+const char *attn_jvp_last_error(void);
+/* Library version string, e.g. "attn_jvp 0.1 (sm_100a)". */
+const char *attn_jvp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ATTN_JVP_H_ */

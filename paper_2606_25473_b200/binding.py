@@ -1,0 +1,212 @@
+"""ctypes binding of libattn_jvp.so: same names as include/attn_jvp.h, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; nothing here computes.
+There is no fallback: if the shared library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence, Tuple
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libattn_jvp.so")
+
+AJ_OK, AJ_ERR_INVALID_ARG, AJ_ERR_UNSUPPORTED, AJ_ERR_CUDA, AJ_ERR_OOM = 0, -1, -2, -3, -4
+AJ_BF16, AJ_FP32 = 0, 1
+AJ_MASK_FULL, AJ_MASK_BLOCK_CAUSAL, AJ_MASK_TEACHER_FORCING, AJ_MASK_RANGES = 0, 1, 2, 3
+AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA = 0, 1, 2
+
+_I32P = ctypes.POINTER(ctypes.c_int32)
+
+
+class aj_mask_desc(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("frame_len", ctypes.c_int32), ("num_frames", ctypes.c_int32),
+                ("chunk_frames", ctypes.c_int32), ("first_chunk_frames", ctypes.c_int32),
+                ("num_groups", ctypes.c_int32), ("q_begin", _I32P), ("q_end", _I32P),
+                ("range_offset", _I32P), ("k_begin", _I32P), ("k_end", _I32P)]
+
+
+class aj_problem(ctypes.Structure):
+    _fields_ = [("B", ctypes.c_int32), ("H", ctypes.c_int32), ("Nq", ctypes.c_int32), ("Nk", ctypes.c_int32),
+                ("d", ctypes.c_int32), ("dtype", ctypes.c_int32), ("scale", ctypes.c_float)]
+
+
+class aj_tensor(ctypes.Structure):
+    _fields_ = [("ptr", ctypes.c_void_p), ("stride_b", ctypes.c_int64), ("stride_h", ctypes.c_int64),
+                ("stride_n", ctypes.c_int64)]
+
+
+class aj_task(ctypes.Structure):
+    _fields_ = [("b", ctypes.c_int32), ("h", ctypes.c_int32), ("q_begin", ctypes.c_int32), ("q_rows", ctypes.c_int32),
+                ("range_begin", ctypes.c_int32), ("range_count", ctypes.c_int32), ("num_kv_tiles", ctypes.c_int32),
+                ("group", ctypes.c_int32)]
+
+
+class AttnJvpError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"attn_jvp status {status}: {message}")
+        self.status = status
+
+
+# Every symbol include/attn_jvp.h declares (tests check that the library exports all of them).
+SYMBOLS = [
+    "attn_jvp_schedule_create", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get",
+    "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel",
+    "attn_jvp_plan_kernel", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
+]
+
+_lib = None
+
+
+def lib():
+    """Loads libattn_jvp.so or raises: there is no non-CUDA path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_25473_b200.build` "
+                              "(or __graft_entry__.build()); this package has no fallback path")
+        l = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64p = ctypes.c_void_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int64)
+        l.attn_jvp_schedule_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
+        l.attn_jvp_schedule_destroy.argtypes = [vp]
+        l.attn_jvp_schedule_info.argtypes = [vp, _I32P, _I32P, _I32P, i64p]
+        l.attn_jvp_schedule_get.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P, ctypes.POINTER(aj_task)]
+        l.attn_jvp_plan_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), ctypes.POINTER(vp)]
+        l.attn_jvp_plan_destroy.argtypes = [vp]
+        l.attn_jvp_plan_info.argtypes = [vp, i64p, _I32P]
+        l.attn_jvp_plan_set_kernel.argtypes = [vp, i32]
+        l.attn_jvp_plan_kernel.argtypes = [vp, _I32P, _I32P]
+        l.attn_jvp_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp]
+        l.attn_jvp_fwd_host.argtypes = [vp] * 11
+        for name in SYMBOLS:
+            getattr(l, name).restype = ctypes.c_int
+        l.attn_jvp_last_error.restype = ctypes.c_char_p
+        l.attn_jvp_last_error.argtypes = []
+        l.attn_jvp_version.restype = ctypes.c_char_p
+        l.attn_jvp_version.argtypes = []
+        _lib = l
+    return _lib
+
+
+def _check(status: int):
+    if status != AJ_OK:
+        raise AttnJvpError(status, lib().attn_jvp_last_error().decode())
+
+
+def attn_jvp_last_error() -> str:
+    return lib().attn_jvp_last_error().decode()
+
+
+def attn_jvp_version() -> str:
+    return lib().attn_jvp_version().decode()
+
+
+def make_problem(B: int, H: int, Nq: int, Nk: int, d: int, dtype: int, scale: float = 0.0) -> aj_problem:
+    return aj_problem(B, H, Nq, Nk, d, dtype, scale)
+
+
+def make_mask(kind: int, frame_len: int = 0, num_frames: int = 0, chunk_frames: int = 1, first_chunk_frames: int = 0,
+              groups: Optional[Sequence[Tuple[int, int, Sequence[Tuple[int, int]]]]] = None):
+    """Returns (aj_mask_desc, keepalive).  `groups` = [(q_begin, q_end, [(k_begin, k_end), ...]), ...] for AJ_MASK_RANGES."""
+    m = aj_mask_desc(kind, frame_len, num_frames, chunk_frames, first_chunk_frames, 0, None, None, None, None, None)
+    keep = []
+    if groups is not None:
+        ng = len(groups)
+        qb = (ctypes.c_int32 * max(ng, 1))(*[g[0] for g in groups])
+        qe = (ctypes.c_int32 * max(ng, 1))(*[g[1] for g in groups])
+        off, kb, ke = [0], [], []
+        for g in groups:
+            for (a, b) in g[2]:
+                kb.append(a)
+                ke.append(b)
+            off.append(len(kb))
+        offa = (ctypes.c_int32 * len(off))(*off)
+        kba = (ctypes.c_int32 * max(len(kb), 1))(*kb)
+        kea = (ctypes.c_int32 * max(len(ke), 1))(*ke)
+        m.num_groups = ng
+        m.q_begin, m.q_end, m.range_offset = qb, qe, offa
+        m.k_begin, m.k_end = kba, kea
+        keep = [qb, qe, offa, kba, kea]
+    return m, keep
+
+
+# ---- host-side scheduler -------------------------------------------------------------------------------------------
+def attn_jvp_schedule_create(problem: aj_problem, mask: aj_mask_desc, tile_q: int, tile_k: int) -> ctypes.c_void_p:
+    out = ctypes.c_void_p()
+    _check(lib().attn_jvp_schedule_create(ctypes.byref(problem), ctypes.byref(mask), tile_q, tile_k, ctypes.byref(out)))
+    return out
+
+
+def attn_jvp_schedule_destroy(sched) -> None:
+    _check(lib().attn_jvp_schedule_destroy(sched))
+
+
+def attn_jvp_schedule_info(sched):
+    """-> (num_groups, num_ranges, num_tasks, unmasked_pairs_per_head)"""
+    a, b, c, d = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int64()
+    _check(lib().attn_jvp_schedule_info(sched, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d)))
+    return a.value, b.value, c.value, d.value
+
+
+def attn_jvp_schedule_get(sched):
+    """-> dict(q_begin, q_end, range_offset, k_begin, k_end: lists; tasks: list of aj_task)"""
+    ng, nr, nt, _ = attn_jvp_schedule_info(sched)
+    qb, qe = (ctypes.c_int32 * max(ng, 1))(), (ctypes.c_int32 * max(ng, 1))()
+    off = (ctypes.c_int32 * (ng + 1))()
+    kb, ke = (ctypes.c_int32 * max(nr, 1))(), (ctypes.c_int32 * max(nr, 1))()
+    tasks = (aj_task * max(nt, 1))()
+    _check(lib().attn_jvp_schedule_get(sched, qb, qe, off, kb, ke, tasks))
+    return dict(q_begin=list(qb)[:ng], q_end=list(qe)[:ng], range_offset=list(off), k_begin=list(kb)[:nr],
+                k_end=list(ke)[:nr], tasks=[tasks[i] for i in range(nt)])
+
+
+# ---- plans and the forward call ------------------------------------------------------------------------------------
+def attn_jvp_plan_create(problem: aj_problem, mask: aj_mask_desc) -> ctypes.c_void_p:
+    out = ctypes.c_void_p()
+    _check(lib().attn_jvp_plan_create(ctypes.byref(problem), ctypes.byref(mask), ctypes.byref(out)))
+    return out
+
+
+def attn_jvp_plan_destroy(plan) -> None:
+    _check(lib().attn_jvp_plan_destroy(plan))
+
+
+def attn_jvp_plan_info(plan):
+    """-> (unmasked_pairs_per_head, num_tasks)"""
+    a, b = ctypes.c_int64(), ctypes.c_int32()
+    _check(lib().attn_jvp_plan_info(plan, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
+
+
+def attn_jvp_plan_set_kernel(plan, kernel: int) -> None:
+    _check(lib().attn_jvp_plan_set_kernel(plan, kernel))
+
+
+def attn_jvp_plan_kernel(plan):
+    """-> (kernel, launches_per_call)"""
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib().attn_jvp_plan_kernel(plan, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
+
+
+def _tensor(t) -> aj_tensor:
+    """torch [B,H,N,d] tensor (d contiguous) -> aj_tensor view."""
+    if t.dim() != 4 or t.stride(3) != 1:
+        raise ValueError("expected a [B, H, N, d] tensor with contiguous d")
+    return aj_tensor(t.data_ptr(), t.stride(0), t.stride(1), t.stride(2))
+
+
+def attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
+    """Device tensors (torch.cuda); enqueues on `stream` (a cudaStream_t handle, 0 = default) and returns."""
+    ts = [_tensor(x) for x in (q, k, v, tq, tk, tv, o, to)]
+    _check(lib().attn_jvp_fwd(plan, *[ctypes.byref(x) for x in ts], None if lse is None else lse.data_ptr(), stream))
+
+
+def attn_jvp_fwd_host(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
+    """Host tensors (contiguous [B,H,N,d], ideally pinned); copies + kernel are enqueued on `stream`."""
+    for x in (q, k, v, tq, tk, tv, o, to):
+        if x.is_cuda or not x.is_contiguous():
+            raise ValueError("attn_jvp_fwd_host expects contiguous host tensors")
+    _check(lib().attn_jvp_fwd_host(plan, *[x.data_ptr() for x in (q, k, v, tq, tk, tv, o, to)],
+                                   None if lse is None else lse.data_ptr(), stream))

@@ -1,0 +1,270 @@
+// C-ABI entry points that need CUDA: plans and the forward call (include/attn_jvp.h).
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "internal.hpp"
+#include "kernels.hpp"
+
+struct aj_plan {
+    aj_problem problem;       // scale resolved (never 0)
+    aj_mask_desc mask;        // arrays below back the pointers for AJ_MASK_RANGES
+    std::vector<int32_t> m_qb, m_qe, m_off, m_kb, m_ke;
+    int32_t kernel = AJ_KERNEL_SIMT;
+    aj_schedule *sched = nullptr;
+    int32_t num_tasks = 0;
+    int device = 0, num_sms = 0;
+    // device copies of the schedule
+    aj_task *d_tasks = nullptr;
+    int32_t *d_kb = nullptr, *d_ke = nullptr, *d_counters = nullptr;
+    // staging for attn_jvp_fwd_host
+    void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    void *d_out[2] = {nullptr, nullptr};
+    float *d_lse = nullptr;
+};
+
+namespace {
+
+using aj::fail;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// The driver entry point is looked up at run time so that the library links against cudart only and loads
+// on machines without a driver (the CPU build box).
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+aj_status cuda_fail(cudaError_t e, const char *what) {
+    return fail(AJ_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+void free_device(aj_plan *p) {
+    cudaFree(p->d_tasks); cudaFree(p->d_kb); cudaFree(p->d_ke);
+    p->d_tasks = nullptr; p->d_kb = p->d_ke = nullptr;
+}
+
+bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
+
+// (Re)build the schedule for `kernel` and upload it.
+aj_status install_schedule(aj_plan *p, int32_t kernel) {
+    const int tq = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
+    const int tk = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+    aj_schedule *s = nullptr;
+    if (aj_status st = attn_jvp_schedule_create(&p->problem, &p->mask, tq, tk, &s)) return st;
+    const size_t nt = s->tasks.size(), nr = s->low.ranges.size();
+    std::vector<int32_t> kb(nr), ke(nr);
+    for (size_t r = 0; r < nr; ++r) { kb[r] = s->low.ranges[r].k_begin; ke[r] = s->low.ranges[r].k_end; }
+    aj_task *d_tasks = nullptr;
+    int32_t *d_kb = nullptr, *d_ke = nullptr;
+    cudaError_t e = cudaMalloc(&d_tasks, std::max<size_t>(nt, 1) * sizeof(aj_task));
+    if (e == cudaSuccess) e = cudaMalloc(&d_kb, std::max<size_t>(nr, 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&d_ke, std::max<size_t>(nr, 1) * sizeof(int32_t));
+    if (e == cudaSuccess && nt) e = cudaMemcpy(d_tasks, s->tasks.data(), nt * sizeof(aj_task), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nr) e = cudaMemcpy(d_kb, kb.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nr) e = cudaMemcpy(d_ke, ke.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke);
+        attn_jvp_schedule_destroy(s);
+        return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
+    }
+    free_device(p);
+    attn_jvp_schedule_destroy(p->sched);
+    p->sched = s; p->kernel = kernel; p->num_tasks = (int32_t)nt;
+    p->d_tasks = d_tasks; p->d_kb = d_kb; p->d_ke = d_ke;
+    return AJ_OK;
+}
+
+aj_status check_tensor(const aj_tensor *t, const char *name, int d, int elem_bytes) {
+    if (!t || !t->ptr) return fail(AJ_ERR_INVALID_ARG, std::string(name) + " is NULL");
+    if ((uintptr_t)t->ptr % 16 != 0) return fail(AJ_ERR_INVALID_ARG, std::string(name) + ": pointer must be 16-byte aligned");
+    if (t->stride_n < d || t->stride_n % 8 || t->stride_h % 8 || t->stride_b % 8 || t->stride_h < 0 || t->stride_b < 0)
+        return fail(AJ_ERR_INVALID_ARG, std::string(name) + ": strides must be multiples of 8 elements with stride_n >= d");
+    (void)elem_bytes;
+    return AJ_OK;
+}
+
+aj_status encode_map(CUtensorMap *map, const aj_tensor &t, const aj_problem &p, int64_t n_rows, int box_rows) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    // dims innermost first: d, N, H, B.  A size-1 dimension still needs a legal (16-byte multiple) stride.
+    cuuint64_t dims[4] = {(cuuint64_t)p.d, (cuuint64_t)n_rows, (cuuint64_t)p.H, (cuuint64_t)p.B};
+    auto bytes = [](int64_t elems) { return (cuuint64_t)std::max<int64_t>(elems, 8) * 2; };
+    cuuint64_t strides[3] = {bytes(t.stride_n), bytes(t.stride_h), bytes(t.stride_b)};
+    cuuint32_t box[4] = {64, (cuuint32_t)box_rows, 1, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, t.ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r));
+    return AJ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *mask, aj_plan **out) {
+    if (!out) return fail(AJ_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (aj_status st = aj::check_problem(problem)) return st;
+    if (!mask) return fail(AJ_ERR_INVALID_ARG, "mask is NULL");
+    if (problem->d != 64 && problem->d != 128) return fail(AJ_ERR_UNSUPPORTED, "d must be 64 or 128");
+    aj_plan *p = new (std::nothrow) aj_plan();
+    if (!p) return fail(AJ_ERR_OOM, "out of host memory");
+    aj_status st = AJ_OK;
+    try {
+        p->problem = *problem;
+        if (p->problem.scale == 0.0f) p->problem.scale = 1.0f / std::sqrt((float)problem->d);
+        p->mask = *mask;
+        if (mask->kind == AJ_MASK_RANGES && mask->num_groups > 0) {
+            if (!mask->q_begin || !mask->q_end || !mask->range_offset) { delete p; return fail(AJ_ERR_INVALID_ARG, "ranges mask: null group arrays"); }
+            const int ng = mask->num_groups, nr = mask->range_offset[ng];
+            if (nr < 0 || (nr > 0 && (!mask->k_begin || !mask->k_end))) { delete p; return fail(AJ_ERR_INVALID_ARG, "ranges mask: null range arrays"); }
+            p->m_qb.assign(mask->q_begin, mask->q_begin + ng);
+            p->m_qe.assign(mask->q_end, mask->q_end + ng);
+            p->m_off.assign(mask->range_offset, mask->range_offset + ng + 1);
+            p->m_kb.assign(mask->k_begin, mask->k_begin + nr);
+            p->m_ke.assign(mask->k_end, mask->k_end + nr);
+            p->mask.q_begin = p->m_qb.data(); p->mask.q_end = p->m_qe.data(); p->mask.range_offset = p->m_off.data();
+            p->mask.k_begin = p->m_kb.data(); p->mask.k_end = p->m_ke.data();
+        }
+        cudaError_t e = cudaGetDevice(&p->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
+        if (e != cudaSuccess) { delete p; return cuda_fail(e, "no usable CUDA device"); }
+        e = cudaMalloc(&p->d_counters, 4 * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
+        if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
+        st = install_schedule(p, umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT);
+    } catch (const std::bad_alloc &) {
+        st = fail(AJ_ERR_OOM, "out of host memory");
+    }
+    if (st != AJ_OK) { attn_jvp_plan_destroy(p); return st; }
+    *out = p;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_destroy(aj_plan *p) {
+    if (!p) return AJ_OK;
+    free_device(p);
+    cudaFree(p->d_counters);
+    for (void *x : p->d_in) cudaFree(x);
+    for (void *x : p->d_out) cudaFree(x);
+    cudaFree(p->d_lse);
+    attn_jvp_schedule_destroy(p->sched);
+    delete p;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_info(const aj_plan *p, int64_t *pairs, int32_t *num_tasks) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (pairs) *pairs = p->sched->low.pairs_per_head;
+    if (num_tasks) *num_tasks = p->num_tasks;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (kernel == AJ_KERNEL_AUTO) kernel = umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT;
+    if (kernel != AJ_KERNEL_SIMT && kernel != AJ_KERNEL_UMMA) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
+    if (kernel == AJ_KERNEL_UMMA && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernel needs bf16 and d = 128");
+    if (kernel == p->kernel) return AJ_OK;
+    return install_schedule(p, kernel);
+}
+
+aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launches) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (kernel) *kernel = p->kernel;
+    if (launches) *launches = p->num_tasks > 0 ? 1 : 0;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
+                       const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
+                       void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    const aj_problem &pr = p->problem;
+    const int eb = pr.dtype == AJ_BF16 ? 2 : 4;
+    const aj_tensor *ts[8] = {q, k, v, tq, tk, tv, o, to};
+    const char *names[8] = {"q", "k", "v", "tq", "tk", "tv", "o", "to"};
+    for (int i = 0; i < 8; ++i)
+        if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
+    if (lse && (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: pointer must be 4-byte aligned");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (p->num_tasks == 0) return AJ_OK;
+    cudaError_t e;
+    if (p->kernel == AJ_KERNEL_UMMA) {
+        aj::UmmaParams prm;
+        std::memset(&prm, 0, sizeof(prm));
+        aj_status st;
+        if ((st = encode_map(&prm.tm_q, *q, pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&prm.tm_tq, *tq, pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&prm.tm_k, *k, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_tk, *tk, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_v, *v, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_tv, *tv, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        prm.o = *o; prm.to = *to; prm.lse = lse;
+        prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke; prm.counters = p->d_counters;
+        prm.num_tasks = p->num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
+        prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
+        e = aj::launch_umma(prm, std::min(p->num_sms, p->num_tasks), stream);
+    } else {
+        aj::SimtParams prm;
+        prm.q = *q; prm.k = *k; prm.v = *v; prm.tq = *tq; prm.tk = *tk; prm.tv = *tv; prm.o = *o; prm.to = *to;
+        prm.lse = lse; prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke;
+        prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
+        e = aj::launch_simt(prm, pr.dtype, pr.d, p->num_tasks, stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
+    return AJ_OK;
+}
+
+aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *tq, const void *tk,
+                            const void *tv, void *o, void *to, float *lse, void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    const void *in[6] = {q, k, v, tq, tk, tv};
+    for (const void *x : in) if (!x) return fail(AJ_ERR_INVALID_ARG, "a host input pointer is NULL");
+    if (!o || !to) return fail(AJ_ERR_INVALID_ARG, "a host output pointer is NULL");
+    const aj_problem &pr = p->problem;
+    const size_t eb = pr.dtype == AJ_BF16 ? 2 : 4;
+    const size_t nq_bytes = (size_t)pr.B * pr.H * pr.Nq * pr.d * eb, nk_bytes = (size_t)pr.B * pr.H * pr.Nk * pr.d * eb;
+    const size_t lse_bytes = (size_t)pr.B * pr.H * pr.Nq * sizeof(float);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i)
+        if (!p->d_in[i]) e = cudaMalloc(&p->d_in[i], (i == 0 || i == 3) ? nq_bytes : nk_bytes);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i)
+        if (!p->d_out[i]) e = cudaMalloc(&p->d_out[i], nq_bytes);
+    if (e == cudaSuccess && !p->d_lse) e = cudaMalloc(&p->d_lse, lse_bytes);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for staging") : cuda_fail(e, "staging allocation");
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i)
+        e = cudaMemcpyAsync(p->d_in[i], in[i], (i == 0 || i == 3) ? nq_bytes : nk_bytes, cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "host-to-device copy");
+    aj_tensor t[8];
+    for (int i = 0; i < 8; ++i) {
+        const int64_t n = (i == 0 || i == 3 || i >= 6) ? pr.Nq : pr.Nk;
+        t[i].ptr = i < 6 ? p->d_in[i] : p->d_out[i - 6];
+        t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = (int64_t)pr.H * n * pr.d;
+    }
+    if (aj_status st = attn_jvp_fwd(p, &t[0], &t[1], &t[2], &t[3], &t[4], &t[5], &t[6], &t[7], p->d_lse, stream)) return st;
+    e = cudaMemcpyAsync(o, p->d_out[0], nq_bytes, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(to, p->d_out[1], nq_bytes, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess && lse) e = cudaMemcpyAsync(lse, p->d_lse, lse_bytes, cudaMemcpyDeviceToHost, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "device-to-host copy");
+    return AJ_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,37 @@
+// Internal declarations shared by the host-side pieces of libattn_jvp (not part of the ABI).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "attn_jvp.h"
+
+namespace aj {
+
+// Thread-local error message behind attn_jvp_last_error().
+void set_error(const std::string &msg);
+aj_status fail(aj_status st, const std::string &msg);
+const char *last_error_cstr();
+aj_status check_problem(const aj_problem *p);
+
+struct KeyRange { int32_t k_begin, k_end; };
+
+// The lowered mask: disjoint query groups, each with sorted, disjoint, merged key ranges.
+struct Lowered {
+    std::vector<int32_t> q_begin, q_end, range_offset;  // range_offset has num_groups + 1 entries
+    std::vector<KeyRange> ranges;
+    int64_t pairs_per_head = 0;
+};
+
+aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out);
+void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k,
+                 std::vector<aj_task> &tasks);
+
+}  // namespace aj
+
+struct aj_schedule {
+    aj_problem problem;
+    int32_t tile_q, tile_k;
+    aj::Lowered low;
+    std::vector<aj_task> tasks;
+};

@@ -1,0 +1,43 @@
+// Kernel launch interfaces (internal).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "attn_jvp.h"
+
+namespace aj {
+
+constexpr int SIMT_TILE_Q = 16;
+constexpr int SIMT_TILE_K = 32;
+constexpr int UMMA_TILE_Q = 128;  // B_r: query rows per task = UMMA M
+constexpr int UMMA_TILE_K = 64;   // B_c: keys per streamed tile
+
+struct SimtParams {
+    aj_tensor q, k, v, tq, tk, tv, o, to;
+    float *lse;
+    const aj_task *tasks;
+    const int32_t *k_begin, *k_end;
+    int32_t H, Nq;
+    float scale;
+};
+
+cudaError_t launch_simt(const SimtParams &prm, int dtype, int d, int num_tasks, cudaStream_t stream);
+
+// bf16, d = 128, tcgen05 + TMEM + TMA (kernel_umma_sm100.cu)
+struct UmmaParams {
+    CUtensorMap tm_q, tm_tq;    // box {64, 128, 1, 1} over [B, H, Nq, d], SWIZZLE_128B
+    CUtensorMap tm_k, tm_tk, tm_v, tm_tv;  // box {64, 64, 1, 1} over [B, H, Nk, d], SWIZZLE_128B
+    aj_tensor o, to;
+    float *lse;
+    const aj_task *tasks;
+    const int32_t *k_begin, *k_end;
+    int32_t *counters;          // [0] next task, [1] CTAs finished (both 0 between launches)
+    int32_t num_tasks, H, Nq;
+    float scale_log2;           // s * log2(e)
+    float scale;                // s
+};
+
+size_t umma_smem_bytes();
+cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream);
+
+}  // namespace aj

@@ -1,0 +1,230 @@
+// Mask descriptor -> query groups / key ranges -> ordered tile tasks (host, integers only).
+//
+// "The custom mask is represented as a set of query groups and their admissible key
+// ranges ... The kernel launches tasks (g, i), where i is a query tile inside Q_g.  Each task streams only
+// the key ranges in K_g."  Teacher forcing (Eq. 8) and block-causal masks become "a small
+// number of full query-key rectangles"; dense attention is one group with one range.
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "internal.hpp"
+
+namespace aj {
+
+static thread_local std::string g_error;
+
+void set_error(const std::string &msg) { g_error = msg; }
+aj_status fail(aj_status st, const std::string &msg) {
+    g_error = msg;
+    return st;
+}
+const char *last_error_cstr() { return g_error.c_str(); }
+
+// Block boundaries of one half: [0, C1, C1 + C, C1 + 2C, ...] (R6).
+static aj_status block_bounds(const aj_mask_desc &m, std::vector<int64_t> &b) {
+    if (m.frame_len <= 0 || m.num_frames <= 0 || m.chunk_frames <= 0 || m.first_chunk_frames < 0)
+        return fail(AJ_ERR_INVALID_ARG, "mask: frame_len, num_frames, chunk_frames must be > 0");
+    int64_t first = m.first_chunk_frames > 0 ? m.first_chunk_frames : m.chunk_frames;
+    if (first > m.num_frames || (m.num_frames - first) % m.chunk_frames != 0)
+        return fail(AJ_ERR_INVALID_ARG, "mask: num_frames is not first_chunk_frames + k * chunk_frames");
+    b.clear();
+    b.push_back(0);
+    for (int64_t f = first; f <= m.num_frames; f += m.chunk_frames) b.push_back(f * m.frame_len);
+    return AJ_OK;
+}
+
+static void push_group(Lowered &out, int64_t q0, int64_t q1, std::initializer_list<KeyRange> rs) {
+    out.q_begin.push_back((int32_t)q0);
+    out.q_end.push_back((int32_t)q1);
+    for (const KeyRange &r : rs) {
+        if (r.k_end <= r.k_begin) continue;
+        // merge with the previous range of this group when they touch
+        if ((int32_t)out.ranges.size() > out.range_offset.back() && out.ranges.back().k_end == r.k_begin)
+            out.ranges.back().k_end = r.k_end;
+        else
+            out.ranges.push_back(r);
+    }
+    out.range_offset.push_back((int32_t)out.ranges.size());
+}
+
+aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
+    out = Lowered();
+    out.range_offset.push_back(0);
+    std::vector<int64_t> bb;
+    switch (m.kind) {
+    case AJ_MASK_FULL:
+        push_group(out, 0, p.Nq, {KeyRange{0, p.Nk}});
+        break;
+    case AJ_MASK_BLOCK_CAUSAL: {
+        if (aj_status st = block_bounds(m, bb)) return st;
+        if (p.Nq != bb.back() || p.Nk != bb.back())
+            return fail(AJ_ERR_INVALID_ARG, "block-causal mask: Nq and Nk must equal num_frames * frame_len");
+        for (size_t i = 0; i + 1 < bb.size(); ++i)  // block i sees blocks <= i
+            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1]}});
+        break;
+    }
+    case AJ_MASK_TEACHER_FORCING: {
+        if (aj_status st = block_bounds(m, bb)) return st;
+        const int64_t half = bb.back();
+        if (p.Nq != 2 * half || p.Nk != 2 * half)
+            return fail(AJ_ERR_INVALID_ARG, "teacher-forcing mask: Nq and Nk must equal 2 * num_frames * frame_len");
+        for (size_t i = 0; i + 1 < bb.size(); ++i)  // clean block i -> clean blocks <= i
+            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1]}});
+        for (size_t i = 0; i + 1 < bb.size(); ++i)  // noisy block i -> clean blocks < i, noisy block i
+            push_group(out, half + bb[i], half + bb[i + 1],
+                       {KeyRange{0, (int32_t)bb[i]}, KeyRange{(int32_t)(half + bb[i]), (int32_t)(half + bb[i + 1])}});
+        break;
+    }
+    case AJ_MASK_RANGES: {
+        if (m.num_groups < 0 || (m.num_groups > 0 && (!m.q_begin || !m.q_end || !m.range_offset)))
+            return fail(AJ_ERR_INVALID_ARG, "ranges mask: null group arrays");
+        if (m.num_groups > 0 && m.range_offset[0] != 0)
+            return fail(AJ_ERR_INVALID_ARG, "ranges mask: range_offset[0] must be 0");
+        std::vector<std::pair<int32_t, int32_t>> rows;
+        for (int g = 0; g < m.num_groups; ++g) {
+            int32_t q0 = m.q_begin[g], q1 = m.q_end[g];
+            if (q0 < 0 || q1 > p.Nq || q0 >= q1)
+                return fail(AJ_ERR_INVALID_ARG, "ranges mask: query group outside [0, Nq) or empty");
+            int32_t r0 = m.range_offset[g], r1 = m.range_offset[g + 1];
+            if (r1 < r0) return fail(AJ_ERR_INVALID_ARG, "ranges mask: range_offset must be non-decreasing");
+            if (r1 > r0 && (!m.k_begin || !m.k_end)) return fail(AJ_ERR_INVALID_ARG, "ranges mask: null range arrays");
+            out.q_begin.push_back(q0);
+            out.q_end.push_back(q1);
+            int32_t prev_end = 0;
+            for (int r = r0; r < r1; ++r) {
+                int32_t k0 = m.k_begin[r], k1 = m.k_end[r];
+                if (k0 < 0 || k1 > p.Nk || k0 >= k1 || k0 < prev_end)
+                    return fail(AJ_ERR_INVALID_ARG, "ranges mask: key ranges must be non-empty, sorted, disjoint, inside [0, Nk)");
+                if (r > r0 && out.ranges.back().k_end == k0) out.ranges.back().k_end = k1;
+                else out.ranges.push_back(KeyRange{k0, k1});
+                prev_end = k1;
+            }
+            out.range_offset.push_back((int32_t)out.ranges.size());
+            rows.emplace_back(q0, q1);
+        }
+        std::sort(rows.begin(), rows.end());
+        for (size_t i = 1; i < rows.size(); ++i)
+            if (rows[i].first < rows[i - 1].second)
+                return fail(AJ_ERR_INVALID_ARG, "ranges mask: query groups overlap");
+        // rows in no group become key-less groups so that every output row is written (O = 0, tO = 0, lse = -inf)
+        int32_t next = 0;
+        rows.emplace_back(p.Nq, p.Nq);
+        for (const auto &qr : rows) {
+            if (qr.first > next) push_group(out, next, qr.first, {});
+            next = std::max(next, qr.second);
+        }
+        break;
+    }
+    default:
+        return fail(AJ_ERR_INVALID_ARG, "mask: unknown kind");
+    }
+    out.pairs_per_head = 0;
+    for (size_t g = 0; g < out.q_begin.size(); ++g) {
+        int64_t keys = 0;
+        for (int r = out.range_offset[g]; r < out.range_offset[g + 1]; ++r)
+            keys += out.ranges[r].k_end - out.ranges[r].k_begin;
+        out.pairs_per_head += keys * (int64_t)(out.q_end[g] - out.q_begin[g]);
+    }
+    return AJ_OK;
+}
+
+void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k,
+                 std::vector<aj_task> &tasks) {
+    tasks.clear();
+    for (int32_t b = 0; b < p.B; ++b)
+        for (int32_t h = 0; h < p.H; ++h)
+            for (size_t g = 0; g < low.q_begin.size(); ++g) {
+                int32_t r0 = low.range_offset[g], r1 = low.range_offset[g + 1];
+                int32_t kv_tiles = 0;
+                for (int r = r0; r < r1; ++r)
+                    kv_tiles += (low.ranges[r].k_end - low.ranges[r].k_begin + tile_k - 1) / tile_k;
+                // query tiles start at the group start (R8); the last one may be partial
+                for (int32_t q = low.q_begin[g]; q < low.q_end[g]; q += tile_q) {
+                    aj_task t;
+                    t.b = b; t.h = h; t.q_begin = q;
+                    t.q_rows = std::min(tile_q, low.q_end[g] - q);
+                    t.range_begin = r0; t.range_count = r1 - r0;
+                    t.num_kv_tiles = kv_tiles; t.group = (int32_t)g;
+                    tasks.push_back(t);
+                }
+            }
+    // Longest-first so that the persistent CTAs finish together; ties keep (b, h, group, tile) order so that
+    // tasks streaming the same keys of the same head run at the same time and share them in L2.
+    std::stable_sort(tasks.begin(), tasks.end(),
+                     [](const aj_task &x, const aj_task &y) { return x.num_kv_tiles > y.num_kv_tiles; });
+}
+
+}  // namespace aj
+
+namespace aj {
+
+aj_status check_problem(const aj_problem *p) {
+    if (!p) return aj::fail(AJ_ERR_INVALID_ARG, "problem is NULL");
+    if (p->B <= 0 || p->H <= 0 || p->Nq <= 0 || p->Nk <= 0 || p->d <= 0)
+        return aj::fail(AJ_ERR_INVALID_ARG, "problem: B, H, Nq, Nk, d must be > 0");
+    if (p->dtype != AJ_BF16 && p->dtype != AJ_FP32) return aj::fail(AJ_ERR_INVALID_ARG, "problem: unknown dtype");
+    if (!(p->scale >= 0.0f) || p->scale > 1e30f) return aj::fail(AJ_ERR_INVALID_ARG, "problem: scale must be finite and >= 0");
+    return AJ_OK;
+}
+
+}  // namespace aj
+
+extern "C" {
+
+aj_status attn_jvp_schedule_create(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
+                                   int32_t tile_k, aj_schedule **out) {
+    if (!out) return aj::fail(AJ_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (aj_status st = aj::check_problem(problem)) return st;
+    if (!mask) return aj::fail(AJ_ERR_INVALID_ARG, "mask is NULL");
+    if (tile_q <= 0 || tile_k <= 0) return aj::fail(AJ_ERR_INVALID_ARG, "tile_q and tile_k must be > 0");
+    aj_schedule *s = new (std::nothrow) aj_schedule();
+    if (!s) return aj::fail(AJ_ERR_OOM, "out of host memory");
+    try {
+        s->problem = *problem; s->tile_q = tile_q; s->tile_k = tile_k;
+        aj_status st = aj::lower_mask(*problem, *mask, s->low);
+        if (st != AJ_OK) { delete s; return st; }
+        aj::build_tasks(*problem, s->low, tile_q, tile_k, s->tasks);
+    } catch (const std::bad_alloc &) {
+        delete s;
+        return aj::fail(AJ_ERR_OOM, "out of host memory");
+    }
+    *out = s;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_destroy(aj_schedule *sched) {
+    delete sched;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_info(const aj_schedule *s, int32_t *num_groups, int32_t *num_ranges,
+                                 int32_t *num_tasks, int64_t *pairs) {
+    if (!s) return aj::fail(AJ_ERR_INVALID_ARG, "schedule is NULL");
+    if (num_groups) *num_groups = (int32_t)s->low.q_begin.size();
+    if (num_ranges) *num_ranges = (int32_t)s->low.ranges.size();
+    if (num_tasks) *num_tasks = (int32_t)s->tasks.size();
+    if (pairs) *pairs = s->low.pairs_per_head;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_get(const aj_schedule *s, int32_t *q_begin, int32_t *q_end, int32_t *range_offset,
+                                int32_t *k_begin, int32_t *k_end, aj_task *tasks) {
+    if (!s) return aj::fail(AJ_ERR_INVALID_ARG, "schedule is NULL");
+    const aj::Lowered &l = s->low;
+    if (q_begin) std::copy(l.q_begin.begin(), l.q_begin.end(), q_begin);
+    if (q_end) std::copy(l.q_end.begin(), l.q_end.end(), q_end);
+    if (range_offset) std::copy(l.range_offset.begin(), l.range_offset.end(), range_offset);
+    for (size_t r = 0; r < l.ranges.size(); ++r) {
+        if (k_begin) k_begin[r] = l.ranges[r].k_begin;
+        if (k_end) k_end[r] = l.ranges[r].k_end;
+    }
+    if (tasks) std::copy(s->tasks.begin(), s->tasks.end(), tasks);
+    return AJ_OK;
+}
+
+const char *attn_jvp_last_error(void) { return aj::last_error_cstr(); }
+const char *attn_jvp_version(void) { return "attn_jvp 0.1 (sm_100a)"; }
+
+}  // extern "C"
