@@ -1,0 +1,106 @@
+"""Shared by the `-m gpu` tests: run a workload through the C ABI, run the oracle, pick rows to compare."""
+import numpy as np
+import torch
+
+import oracle
+from helpers import oracle_mask, widen, max_norm_err
+from paper_2606_25473_b200 import binding as aj
+from paper_2606_25473_b200.workloads import Workload, make_inputs
+
+# BASELINE.json north_star tolerances, max|err| / max|ref| per tensor
+TOL = {"bf16": dict(o=1e-2, to=1e-2, lse=1e-3), "fp32": dict(o=1e-4, to=1e-4, lse=1e-4)}
+
+
+def mask_kind(w: Workload) -> int:
+    return {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL,
+            "full": aj.AJ_MASK_FULL}[w.mask]
+
+
+def make_plan(w: Workload, kernel: int = aj.AJ_KERNEL_AUTO, scale: float = 0.0):
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32, scale)
+    mask, keep = aj.make_mask(mask_kind(w), w.frame_len, w.num_frames, w.chunk_frames)
+    plan = aj.attn_jvp_plan_create(prob, mask)
+    if kernel != aj.AJ_KERNEL_AUTO:
+        aj.attn_jvp_plan_set_kernel(plan, kernel)
+    return plan
+
+
+def run_gpu(w: Workload, inputs_cpu, kernel: int = aj.AJ_KERNEL_AUTO, plan=None):
+    """-> (o, to, lse) on the CPU.  Outputs start as NaN so that an unwritten row fails the comparison."""
+    own = plan is None
+    if own:
+        plan = make_plan(w, kernel)
+    dev = [x.cuda() for x in inputs_cpu]
+    o = torch.full_like(dev[0], float("nan"))
+    to = torch.full_like(dev[0], float("nan"))
+    lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    if own:
+        aj.attn_jvp_plan_destroy(plan)
+    return o.cpu(), to.cpu(), lse.cpu()
+
+
+def run_oracle(w: Workload, inputs_cpu, rows_by_head=None):
+    """rows_by_head: {(b, h): int64 rows} or None for every row of every head.
+    -> {(b, h): (rows, o, to, lse)} in fp64."""
+    om = oracle_mask(w)
+    scale = 1.0 / np.sqrt(w.d)
+    out = {}
+    for b in range(w.B):
+        for h in range(w.H):
+            if rows_by_head is not None and (b, h) not in rows_by_head:
+                continue
+            rows = None if rows_by_head is None else np.asarray(rows_by_head[(b, h)], dtype=np.int64)
+            args = [widen(x[b, h]) for x in inputs_cpu]
+            o, to, lse = oracle.attn_jvp_head(om, *args, scale, rows)
+            out[(b, h)] = (np.arange(w.N) if rows is None else rows, o, to, lse)
+    return out
+
+
+def compare(w: Workload, gpu, ref, tol=None):
+    """Max-normalised error per tensor over all compared rows (R11)."""
+    tol = tol or TOL[w.dtype]
+    o, to, lse = gpu
+    got = {"o": [], "to": [], "lse": []}
+    want = {"o": [], "to": [], "lse": []}
+    for (b, h), (rows, ro, rto, rlse) in ref.items():
+        got["o"].append(o[b, h, rows].double().numpy()); want["o"].append(ro)
+        got["to"].append(to[b, h, rows].double().numpy()); want["to"].append(rto)
+        got["lse"].append(lse[b, h, rows].double().numpy()); want["lse"].append(rlse)
+    errs = {}
+    for key in got:
+        g, r = np.concatenate(got[key]), np.concatenate(want[key])
+        assert np.all(np.isfinite(g)), f"{w.name}: non-finite or unwritten {key}"
+        errs[key] = max_norm_err(g, r)
+    for key in errs:
+        assert errs[key] <= tol[key], f"{w.name}: {key} error {errs[key]:.3e} > {tol[key]:.1e} (all: {errs})"
+    return errs
+
+
+def sample_rows(w: Workload, per_head_groups: int = 4, random_per_group: int = 2, tile_q: int = 128):
+    """Deterministic row subset for full-size configs: for every (b, h) a rotating choice of query groups
+    (every group is hit by some head), and inside each group its first and last row, the rows on both sides
+    of the first and the last query-tile boundary, and seeded random rows."""
+    C, n = w.block_len, w.num_blocks
+    if w.mask == "full":
+        groups = [(0, w.N)]
+    elif w.mask == "block_causal":
+        groups = [(i * C, (i + 1) * C) for i in range(n)]
+    else:
+        groups = [(i * C, (i + 1) * C) for i in range(2 * n)]
+    rng = np.random.default_rng(1234)
+    out = {}
+    idx = 0
+    for b in range(w.B):
+        for h in range(w.H):
+            rows = []
+            for j in range(min(per_head_groups, len(groups))):
+                q0, q1 = groups[(idx + j * max(1, len(groups) // per_head_groups)) % len(groups)]
+                last_tile = q0 + ((q1 - q0 - 1) // tile_q) * tile_q
+                cand = [q0, q1 - 1, q0 + tile_q - 1, q0 + tile_q, last_tile - 1, last_tile]
+                cand += list(rng.integers(q0, q1, size=random_per_group))
+                rows += [int(r) for r in cand if q0 <= r < q1]
+            out[(b, h)] = np.unique(np.asarray(rows, dtype=np.int64))
+            idx += 1
+    return out

@@ -1,0 +1,248 @@
+"""`-m gpu`: the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Tolerances are BASELINE.json's: bf16 path max|err|/max|ref| <= 1e-2 on O and tO, <= 1e-3 on lse; fp32 path <= 1e-4.
+Small cases compare every row of every head and span several query/key tiles with ragged tails; the
+full-size configs (the launch configuration bench.py times) compare a deterministic row sample.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from gpu_common import TOL, compare, make_plan, run_gpu, run_oracle, sample_rows
+from helpers import widen, max_norm_err
+from paper_2606_25473_b200 import binding as aj
+from paper_2606_25473_b200 import build as aj_build
+from paper_2606_25473_b200.workloads import WORKLOADS, Workload, make_inputs, scaled_down
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _ready():
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    aj_build.build_library()
+    oracle.build()
+
+
+# ---------------------------------------------------------------------------------------- config 1 (fp32 path)
+def test_config1_tiny_tf_fp32_every_row():
+    w = WORKLOADS["tiny_tf_fp32"]
+    x = make_inputs(w)
+    plan = make_plan(w)
+    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_SIMT, 1)
+    assert aj.attn_jvp_plan_info(plan)[0] == 3072
+    gpu = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    errs = compare(w, gpu, run_oracle(w, x))
+    assert max(errs.values()) < 1e-5          # plain fp32 FMA lands ~3e-7 (R14)
+
+
+@pytest.mark.parametrize("mask,L,F,cf,d", [
+    ("teacher_forcing", 50, 3, 1, 64), ("teacher_forcing", 37, 4, 2, 128), ("block_causal", 45, 3, 1, 128),
+    ("full", 70, 2, 1, 64)])
+def test_simt_fp32_ragged(mask, L, F, cf, d):
+    w = Workload(f"simt_{mask}", 2, 2, d, mask, L, F, cf, "fp32", 1.0, seed=3)
+    x = make_inputs(w)
+    compare(w, run_gpu(w, x), run_oracle(w, x))
+
+
+def test_simt_runs_bf16_inputs():
+    w = Workload("simt_bf16", 1, 2, 128, "teacher_forcing", 40, 3, 1, "bf16", 0.1, seed=5)
+    x = make_inputs(w)
+    compare(w, run_gpu(w, x, kernel=aj.AJ_KERNEL_SIMT), run_oracle(w, x))
+
+
+# ---------------------------------------------------------------------------------------- tcgen05 path, small
+SMALL_UMMA = [
+    # several 128-row query tiles and 64-key tiles, every group and range with a ragged tail
+    Workload("tf_frame_L200", 1, 2, 128, "teacher_forcing", 200, 3, 1, "bf16", 0.1, seed=0),
+    Workload("tf_chunk_L100", 1, 2, 128, "teacher_forcing", 100, 6, 3, "bf16", 0.1, seed=1),
+    Workload("bc_L137_B2", 2, 2, 128, "block_causal", 137, 4, 1, "bf16", 0.1, seed=2),
+    Workload("full_N517", 1, 3, 128, "full", 517, 1, 1, "bf16", 0.1, seed=3),
+    Workload("tf_L8", 1, 1, 128, "teacher_forcing", 8, 2, 1, "bf16", 0.1, seed=4),          # all tiles partial
+    Workload("tf_L64x5", 1, 1, 128, "teacher_forcing", 64, 5, 1, "bf16", 0.1, seed=5),      # exact key tiles
+    Workload("tf_L1560_F2", 1, 1, 128, "teacher_forcing", 1560, 2, 1, "bf16", 0.1, seed=6),  # the real frame length
+]
+
+
+@pytest.mark.parametrize("w", SMALL_UMMA, ids=lambda w: w.name)
+def test_umma_small_every_row(w):
+    x = make_inputs(w)
+    plan = make_plan(w)
+    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA, 1)
+    gpu = run_gpu(w, x, plan=plan)
+    gpu2 = run_gpu(w, x, plan=plan)            # the plan re-arms its work counter: a second launch must agree
+    aj.attn_jvp_plan_destroy(plan)
+    compare(w, gpu, run_oracle(w, x))
+    for a, b in zip(gpu, gpu2):
+        assert torch.equal(a, b)
+
+
+def test_umma_large_unit_variance_tangents():
+    # tangents as large as the primals, peaked scores (|s| up to ~4*sqrt(d)/sqrt(d)): exercises the lazy rescale
+    w = Workload("tf_peaked", 1, 2, 128, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=11)
+    x = make_inputs(w)
+    x[0] = (x[0].float() * 4.0).to(torch.bfloat16)
+    compare(w, run_gpu(w, x), run_oracle(w, x))
+
+
+def test_umma_zero_tangents_give_exact_zero():
+    w = SMALL_UMMA[0]
+    x = make_inputs(w)
+    for i in (3, 4, 5):
+        x[i].zero_()
+    o, to, lse = run_gpu(w, x)
+    assert torch.count_nonzero(to) == 0
+    ref = run_oracle(w, x)
+    compare(w, (o, to, lse), ref, tol=dict(o=1e-2, to=1e-2, lse=1e-3))
+
+
+def test_umma_masked_keys_have_no_effect():
+    w = SMALL_UMMA[0]                       # TF: the first noisy block sees only itself
+    x = make_inputs(w)
+    base = run_gpu(w, x)
+    half, C = w.N // 2, w.block_len
+    y = [t.clone() for t in x]
+    for i in (1, 2, 4, 5):                  # K, V, tK, tV of every key the first noisy block may not see
+        y[i][:, :, :half] = 7.0
+        y[i][:, :, half + C:] = -3.0
+    pert = run_gpu(w, y)
+    rows = slice(half, half + C)
+    for a, b in zip(base, pert):
+        assert torch.equal(a[:, :, rows], b[:, :, rows])
+
+
+def test_umma_strided_views():
+    # [B, N, H, d] storage viewed as [B, H, N, d] (what a projection layer produces), outputs likewise
+    w = SMALL_UMMA[0]
+    x = make_inputs(w)
+    dev = [t.cuda().permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3) for t in x]
+    assert not dev[0].is_contiguous()
+    o = torch.full((w.B, w.N, w.H, w.d), float("nan"), dtype=torch.bfloat16, device="cuda").permute(0, 2, 1, 3)
+    to = torch.full_like(o, float("nan"))
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    plan = make_plan(w)
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+    ref = run_gpu(w, x)
+    assert torch.equal(o.cpu(), ref[0]) and torch.equal(to.cpu(), ref[1]) and torch.equal(lse.cpu(), ref[2])
+
+
+def test_umma_matches_simt_kernel_on_bf16():
+    w = SMALL_UMMA[1]
+    x = make_inputs(w)
+    a = run_gpu(w, x, kernel=aj.AJ_KERNEL_UMMA)
+    b = run_gpu(w, x, kernel=aj.AJ_KERNEL_SIMT)
+    for u, v, tol in zip(a, b, (1e-2, 1e-2, 1e-3)):
+        assert max_norm_err(u.double().numpy(), v.double().numpy()) <= tol
+
+
+# ---------------------------------------------------------------------------------------- generic ranges, edge cases
+@pytest.mark.parametrize("dtype,d", [("fp32", 64), ("bf16", 128)])
+def test_ranges_mask_uncovered_rows_and_nq_ne_nk(dtype, d):
+    Nq, Nk = 300, 421
+    groups = [(0, 130, [(3, 70), (70, 131), (200, 421)]), (150, 290, [(64, 65)]), (290, 300, [])]
+    tdt = torch.bfloat16 if dtype == "bf16" else torch.float32
+    g = torch.Generator().manual_seed(9)
+    q, tq = [torch.randn((1, 2, Nq, d), generator=g).to(tdt) for _ in range(2)]
+    k, v, tk, tv = [torch.randn((1, 2, Nk, d), generator=g).to(tdt) for _ in range(4)]
+    prob = aj.make_problem(1, 2, Nq, Nk, d, aj.AJ_BF16 if dtype == "bf16" else aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+    plan = aj.attn_jvp_plan_create(prob, mask)
+    o = torch.full((1, 2, Nq, d), float("nan"), dtype=tdt, device="cuda")
+    to = torch.full_like(o, float("nan"))
+    lse = torch.full((1, 2, Nq), float("nan"), dtype=torch.float32, device="cuda")
+    aj.attn_jvp_fwd(plan, q.cuda(), k.cuda(), v.cuda(), tq.cuda(), tk.cuda(), tv.cuda(), o, to, lse, 0)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+    o, to, lse = o.cpu(), to.cpu(), lse.cpu()
+    om = oracle.ranges_mask(groups)
+    covered = np.r_[0:130, 150:290]
+    empty = np.r_[130:150, 290:300]
+    tol = TOL[dtype]
+    for h in range(2):
+        ro, rto, rlse = oracle.attn_jvp_head(om, widen(q[0, h]), widen(k[0, h]), widen(v[0, h]), widen(tq[0, h]),
+                                             widen(tk[0, h]), widen(tv[0, h]), 1.0 / np.sqrt(d), covered)
+        assert max_norm_err(o[0, h, covered].double().numpy(), ro) <= tol["o"]
+        assert max_norm_err(to[0, h, covered].double().numpy(), rto) <= tol["to"]
+        assert max_norm_err(lse[0, h, covered].double().numpy(), rlse) <= tol["lse"]
+        # rows in no group or with no key: O = 0, tO = 0, lse = -inf (R9)
+        assert torch.count_nonzero(o[0, h, empty]) == 0 and torch.count_nonzero(to[0, h, empty]) == 0
+        assert torch.all(torch.isneginf(lse[0, h, empty]))
+
+
+def test_lse_may_be_null_and_custom_scale():
+    w = SMALL_UMMA[4]
+    x = make_inputs(w)
+    plan = make_plan(w, scale=0.05)
+    dev = [t.cuda() for t in x]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    aj.attn_jvp_fwd(plan, *dev, o, to, None, 0)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+    om = oracle.teacher_forcing_mask(w.block_len, w.num_blocks)
+    ro, rto, _ = oracle.attn_jvp_head(om, *[widen(t[0, 0]) for t in x], 0.05)
+    assert max_norm_err(o.cpu()[0, 0].double().numpy(), ro) <= 1e-2
+    assert max_norm_err(to.cpu()[0, 0].double().numpy(), rto) <= 1e-2
+
+
+def test_fwd_host_matches_device_path():
+    w = SMALL_UMMA[0]
+    x = make_inputs(w, pin=True)
+    plan = make_plan(w)
+    o = torch.empty_like(x[0]).pin_memory()
+    to = torch.empty_like(x[0]).pin_memory()
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
+    aj.attn_jvp_fwd_host(plan, *x, o, to, lse, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    ref = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    assert torch.equal(o, ref[0]) and torch.equal(to, ref[1]) and torch.equal(lse, ref[2])
+
+
+def test_fwd_argument_errors():
+    w = SMALL_UMMA[4]
+    plan = make_plan(w)
+    dev = [t.cuda() for t in make_inputs(w)]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    with pytest.raises(aj.AttnJvpError) as e:                      # misaligned pointer
+        bad = torch.empty(dev[0].numel() + 8, dtype=torch.bfloat16, device="cuda")[1:1 + dev[0].numel()].view_as(dev[0])
+        aj.attn_jvp_fwd(plan, bad, *dev[1:], o, to, None, 0)
+    assert e.value.status == aj.AJ_ERR_INVALID_ARG
+    with pytest.raises(aj.AttnJvpError) as e:                      # stride_n < d
+        aj.attn_jvp_fwd(plan, dev[0].as_strided(dev[0].shape, (0, 0, 64, 1)), *dev[1:], o, to, None, 0)
+    assert e.value.status == aj.AJ_ERR_INVALID_ARG
+    assert aj.lib().attn_jvp_fwd(plan, None, None, None, None, None, None, None, None, None, None) == aj.AJ_ERR_INVALID_ARG
+    with pytest.raises(aj.AttnJvpError) as e:                      # the tcgen05 kernel does not cover fp32
+        p32 = make_plan(WORKLOADS["tiny_tf_fp32"])
+        try:
+            aj.attn_jvp_plan_set_kernel(p32, aj.AJ_KERNEL_UMMA)
+        finally:
+            aj.attn_jvp_plan_destroy(p32)
+    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    aj.attn_jvp_plan_destroy(plan)
+    torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------- configs 2-5 at full size
+FULL = ["wan13b_tf_framewise", "wan13b_tf_chunkwise", "block_causal_b2", "dit_large_tf_chunkwise", "dit_large_full"]
+
+
+@pytest.mark.parametrize("name", FULL)
+def test_full_size_config_sampled_rows(name):
+    w = WORKLOADS[name]
+    x = make_inputs(w)
+    plan = make_plan(w)
+    pairs, ntasks = aj.attn_jvp_plan_info(plan)
+    assert pairs == w.unmasked_pairs_per_head
+    gpu = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    per_head = 2 if w.N > 100000 else 3
+    rows = sample_rows(w, per_head_groups=per_head, random_per_group=2)
+    errs = compare(w, gpu, run_oracle(w, x, rows))
+    print(f"{name}: rows/head={len(next(iter(rows.values())))} errs={errs}")
+    # properties that hold at any size: every output written and finite, lse within [min s, max s + ln N]
+    for t in gpu:
+        assert torch.isfinite(t.float()).all()

@@ -1,0 +1,195 @@
+"""Host-side logic of the CUDA library, no GPU: library exports, mask lowering, tile tasks, error codes.
+
+The lowered mask (query groups + key ranges) and the task rectangles are rasterised and
+compared bit for bit with the oracle's token-by-token predicate (the two share no code).
+"""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from helpers import oracle_mask
+from paper_2606_25473_b200 import binding as aj
+from paper_2606_25473_b200 import build as aj_build
+from paper_2606_25473_b200.workloads import WORKLOADS, Workload
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    aj_build.build_library()
+
+
+def _kind(w: Workload) -> int:
+    return {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL,
+            "full": aj.AJ_MASK_FULL}[w.mask]
+
+
+def _schedule(w: Workload, tile_q: int, tile_k: int):
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32)
+    mask, keep = aj.make_mask(_kind(w), w.frame_len, w.num_frames, w.chunk_frames)
+    s = aj.attn_jvp_schedule_create(prob, mask, tile_q, tile_k)
+    info = aj.attn_jvp_schedule_info(s)
+    got = aj.attn_jvp_schedule_get(s)
+    aj.attn_jvp_schedule_destroy(s)
+    return info, got
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "attn_jvp.h")).read()
+    declared = set(re.findall(r"\b(attn_jvp_[a-z_]+)\s*\(", header))
+    assert declared == set(aj.SYMBOLS)
+    lib = ctypes.CDLL(aj.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert "sm_100a" in aj.attn_jvp_version()
+
+
+def test_struct_layouts_match_header():
+    assert ctypes.sizeof(aj.aj_task) == 32
+    assert ctypes.sizeof(aj.aj_problem) == 28
+    assert ctypes.sizeof(aj.aj_tensor) == 32
+    assert ctypes.sizeof(aj.aj_mask_desc) == 24 + 5 * ctypes.sizeof(ctypes.c_void_p)
+
+
+@pytest.mark.parametrize("mask,L,F,cf", [
+    ("teacher_forcing", 16, 3, 1), ("teacher_forcing", 10, 6, 3), ("teacher_forcing", 7, 4, 2),
+    ("block_causal", 16, 3, 1), ("block_causal", 9, 6, 2), ("full", 13, 5, 1)])
+@pytest.mark.parametrize("tile_q,tile_k", [(16, 32), (8, 4), (128, 64)])
+def test_task_rectangles_cover_the_mask_exactly_once(oracle, mask, L, F, cf, tile_q, tile_k):
+    w = Workload("t", 1, 1, 64, mask, L, F, cf, "fp32", 1.0)
+    (ng, nr, nt, pairs), got = _schedule(w, tile_q, tile_k)
+    want = oracle.dense_mask(oracle_mask(w), w.N, w.N)
+    cover = np.zeros((w.N, w.N), dtype=np.int32)
+    rows_seen = np.zeros(w.N, dtype=np.int32)
+    for t in got["tasks"]:
+        assert 0 < t.q_rows <= tile_q
+        g = t.group
+        assert got["q_begin"][g] <= t.q_begin and t.q_begin + t.q_rows <= got["q_end"][g]
+        assert (t.q_begin - got["q_begin"][g]) % tile_q == 0          # tiles start at the group start (R8)
+        assert (t.range_begin, t.range_begin + t.range_count) == (got["range_offset"][g], got["range_offset"][g + 1])
+        tiles = 0
+        for r in range(t.range_begin, t.range_begin + t.range_count):
+            k0, k1 = got["k_begin"][r], got["k_end"][r]
+            cover[t.q_begin:t.q_begin + t.q_rows, k0:k1] += 1
+            tiles += -(-(k1 - k0) // tile_k)
+        assert tiles == t.num_kv_tiles
+        rows_seen[t.q_begin:t.q_begin + t.q_rows] += 1
+    assert np.array_equal(cover, want.astype(np.int32))              # every unmasked pair once, no masked pair
+    assert np.all(rows_seen == 1)                                    # every output row is written by one task
+    assert pairs == int(want.sum()) == w.unmasked_pairs_per_head
+    kv = [t.num_kv_tiles for t in got["tasks"]]
+    assert kv == sorted(kv, reverse=True)                            # longest first
+
+
+def test_ranges_are_sorted_disjoint_and_merged():
+    w = Workload("t", 1, 1, 64, "teacher_forcing", 8, 4, 1, "fp32", 1.0)
+    _, got = _schedule(w, 16, 32)
+    off = got["range_offset"]
+    for g in range(len(got["q_begin"])):
+        rs = [(got["k_begin"][r], got["k_end"][r]) for r in range(off[g], off[g + 1])]
+        for (a0, a1), (b0, b1) in zip(rs, rs[1:]):
+            assert a1 < b0                                           # touching ranges were merged
+    # noisy block 0 sees no clean keys: one range only; clean groups always have exactly one
+    n = 4
+    assert off[n + 1] - off[n] == 1
+    assert all(off[g + 1] - off[g] == 1 for g in range(n))
+
+
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_full_size_configs_counts(name):
+    w = WORKLOADS[name]
+    (ng, nr, nt, pairs), _ = _schedule(w, 128, 64)
+    assert pairs == w.unmasked_pairs_per_head
+    tiles_per_block = -(-w.block_len // 128)
+    groups = {"teacher_forcing": 2 * w.num_blocks, "block_causal": w.num_blocks, "full": 1}[w.mask]
+    assert ng == groups
+    if w.mask == "full":
+        assert nt == w.B * w.H * -(-w.N // 128)
+    else:
+        assert nt == w.B * w.H * groups * tiles_per_block
+
+
+def test_generic_ranges_and_uncovered_rows(oracle):
+    groups = [(4, 20, [(0, 5), (5, 9), (30, 40)]), (24, 31, [(2, 3)]), (33, 40, [])]
+    prob = aj.make_problem(1, 1, 40, 48, 64, aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+    s = aj.attn_jvp_schedule_create(prob, mask, 8, 4)
+    ng, nr, nt, pairs = aj.attn_jvp_schedule_info(s)
+    got = aj.attn_jvp_schedule_get(s)
+    aj.attn_jvp_schedule_destroy(s)
+    want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
+    cover = np.zeros((40, 48), dtype=np.int32)
+    rows_seen = np.zeros(40, dtype=np.int32)
+    for t in got["tasks"]:
+        for r in range(t.range_begin, t.range_begin + t.range_count):
+            cover[t.q_begin:t.q_begin + t.q_rows, got["k_begin"][r]:got["k_end"][r]] += 1
+        rows_seen[t.q_begin:t.q_begin + t.q_rows] += 1
+    assert np.array_equal(cover, want.astype(np.int32))
+    assert np.all(rows_seen == 1)          # rows in no group become key-less tasks (O = 0, tO = 0, lse = -inf)
+    assert pairs == int(want.sum())
+    assert (0, 9) in list(zip(got["k_begin"], got["k_end"]))   # (0,5)+(5,9) merged
+
+
+def test_first_chunk_frames(oracle):
+    prob = aj.make_problem(1, 1, 2 * 7 * 5, 2 * 7 * 5, 64, aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 5, 7, 3, first_chunk_frames=1)
+    s = aj.attn_jvp_schedule_create(prob, mask, 4, 4)
+    got = aj.attn_jvp_schedule_get(s)
+    _, _, _, pairs = aj.attn_jvp_schedule_info(s)
+    aj.attn_jvp_schedule_destroy(s)
+    om = oracle.teacher_forcing_mask(15, 3, first_block_len=5)
+    want = oracle.dense_mask(om, 70, 70)
+    cover = np.zeros((70, 70), dtype=np.int32)
+    for t in got["tasks"]:
+        for r in range(t.range_begin, t.range_begin + t.range_count):
+            cover[t.q_begin:t.q_begin + t.q_rows, got["k_begin"][r]:got["k_end"][r]] += 1
+    assert np.array_equal(cover, want.astype(np.int32))
+    assert pairs == int(want.sum())
+
+
+def _expect(status, fn, *args):
+    with pytest.raises(aj.AttnJvpError) as e:
+        fn(*args)
+    assert e.value.status == status
+    assert aj.attn_jvp_last_error() != ""
+
+
+def test_schedule_error_codes():
+    ok_prob = aj.make_problem(1, 1, 96, 96, 64, aj.AJ_FP32)
+    tf, _ = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 16, 3, 1)
+    bad = aj.AJ_ERR_INVALID_ARG
+    _expect(bad, aj.attn_jvp_schedule_create, aj.make_problem(1, 1, 95, 96, 64, aj.AJ_FP32), tf, 16, 32)   # Nq mismatch
+    _expect(bad, aj.attn_jvp_schedule_create, aj.make_problem(0, 1, 96, 96, 64, aj.AJ_FP32), tf, 16, 32)
+    _expect(bad, aj.attn_jvp_schedule_create, aj.make_problem(1, 1, 96, 96, 64, 7), tf, 16, 32)            # dtype
+    _expect(bad, aj.attn_jvp_schedule_create, ok_prob, tf, 0, 32)
+    m, _ = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 16, 3, 2)                                              # 3 % 2
+    _expect(bad, aj.attn_jvp_schedule_create, ok_prob, m, 16, 32)
+    m, _ = aj.make_mask(9, 16, 3, 1)
+    _expect(bad, aj.attn_jvp_schedule_create, ok_prob, m, 16, 32)
+    for groups in ([(0, 10, [(0, 4)]), (5, 12, [(0, 4)])],          # overlapping query groups
+                   [(0, 10, [(4, 8), (0, 2)])],                     # unsorted ranges
+                   [(0, 10, [(0, 5), (4, 8)])],                     # overlapping ranges
+                   [(0, 10, [(0, 97)])],                            # outside Nk
+                   [(0, 97, [(0, 4)])],                             # outside Nq
+                   [(5, 5, [(0, 4)])]):                             # empty group
+        m, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+        _expect(bad, aj.attn_jvp_schedule_create, ok_prob, m, 16, 32)
+    # NULL out pointer / NULL problem go through the raw ABI
+    lib = aj.lib()
+    assert lib.attn_jvp_schedule_create(None, ctypes.byref(tf), 16, 32, ctypes.byref(ctypes.c_void_p())) == bad
+    assert lib.attn_jvp_schedule_create(ctypes.byref(ok_prob), ctypes.byref(tf), 16, 32, None) == bad
+    assert lib.attn_jvp_schedule_info(None, None, None, None, None) == bad
+    assert lib.attn_jvp_schedule_destroy(None) == aj.AJ_OK
+
+
+def test_plan_create_without_gpu_fails_loudly():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    tf, _ = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 16, 3, 1)
+    _expect(aj.AJ_ERR_CUDA, aj.attn_jvp_plan_create, aj.make_problem(1, 1, 96, 96, 64, aj.AJ_FP32), tf)
+    _expect(aj.AJ_ERR_UNSUPPORTED, aj.attn_jvp_plan_create, aj.make_problem(1, 1, 96, 96, 32, aj.AJ_FP32), tf)
