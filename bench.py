@@ -1,0 +1,364 @@
+#!/usr/bin/env python
+"""Benchmark of the fused attention-JVP hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+A step = one pass of the whole hot path (schedule already planned; one `attn_jvp_fwd` call = one kernel launch)
+over one batch of synthetic input of the BASELINE.json configs[1] shape (Wan2.1-1.3B-shaped frame-wise
+teacher-forcing JVP).  Prints ONE JSON line (rank 0).  FLOP convention: 12*d flop per unmasked (query, key)
+pair (six length-d contractions); padded tile area, masked pairs and the softmax are
+not counted.  N > 1: every rank runs its own head shard (B, H heads each; Ulysses-style head sharding,
+PAPER.md:318) with no data-path collective -> "scaling": "weak".
+
+`--impl reference` times the fp64 CPU oracle (oracle/, as it stands) on the host cores on a bounded row sample
+of the same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_2606_25473_b200.workloads import WORKLOADS, Workload, make_inputs
+
+METRIC = "attention-JVP TFLOPS (unmasked pairs)"
+UNIT = "TFLOP/s"
+DEFAULT_WORKLOAD = "wan13b_tf_framewise"
+FALLBACK_PEAKS = {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_gbs": 6650.0}   # B200_PROFILING.md
+
+
+def flops_per_call(w: Workload) -> float:
+    return 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H
+
+
+def allowed_keys_per_row(w: Workload, rows: np.ndarray) -> np.ndarray:
+    """Size of a row's allowed key set from the block structure (accounting only, for the CPU sample)."""
+    C, n = w.block_len, w.num_blocks
+    if w.mask == "full":
+        return np.full(rows.shape, w.N, dtype=np.int64)
+    blk = (rows // C) % n          # clean block i and noisy block i both see (i + 1) * C keys
+    return (blk + 1) * C
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def recorded_traffic(workload: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, if any."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    best = None
+    with open(path) as f:
+        for line in f:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) >= 3 and parts[0] == workload:
+                try:
+                    best = float(parts[2])
+                except ValueError:
+                    pass
+    return best
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    REASONS = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu_index = gpu_index
+        self.proc = None
+        self.out = None
+
+    def start(self):
+        try:
+            self.out = tempfile.TemporaryFile(mode="w+")
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=self.out, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return res
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.out.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        for line in self.out.read().splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(self.REASONS, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        self.out.close()
+        if sm:
+            # "under load" = samples in the upper half of the power range (skips idle samples at the edges)
+            thr = 0.5 * (max(power) + min(power))
+            loaded = [c for c, p in zip(sm, power) if p >= thr] or sm
+            res.update(sm_mhz=statistics.median(loaded), sm_max_mhz=max(smax), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=max(power))
+        return res
+
+
+# ----------------------------------------------------------------------------------------------- CPU oracle legs
+def time_oracle_sample(w: Workload, inputs, budget_s: float, seed: int = 0):
+    """Runs the oracle as it stands on a seeded uniform row sample of head (0, 0) sized to ~budget_s seconds.
+    -> (TFLOP/s under the 12*d convention, seconds, rows, cores)."""
+    import oracle
+    oracle.build()
+    om = {"teacher_forcing": oracle.teacher_forcing_mask, "block_causal": oracle.block_causal_mask}.get(w.mask)
+    om = om(w.block_len, w.num_blocks) if om else oracle.full_mask()
+    args = [x[0, 0].float().numpy() for x in inputs]
+    scale = 1.0 / float(np.sqrt(w.d))
+    rng = np.random.default_rng(seed)
+    pilot = np.sort(rng.integers(0, w.N, size=64))
+    t0 = time.perf_counter()
+    oracle.attn_jvp_head(om, *args, scale, pilot)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    nrows = int(min(max(64, budget_s / dt * 64), 4 * w.N))
+    rows = np.sort(rng.integers(0, w.N, size=nrows))
+    t0 = time.perf_counter()
+    oracle.attn_jvp_head(om, *args, scale, rows)
+    dt = time.perf_counter() - t0
+    flops = 12.0 * w.d * float(allowed_keys_per_row(w, rows).sum())
+    return flops / dt / 1e12, dt, nrows, oracle.num_threads()
+
+
+def run_reference(args, w: Workload):
+    """--impl reference: the oracle on the host cores; each step is a bounded row sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    inputs = make_inputs(w)
+    steps, warmup = args.steps, args.warmup
+    budget = min(6.0, 150.0 / (steps + warmup))
+    for i in range(warmup):
+        time_oracle_sample(w, inputs, budget, seed=100 + i)
+    tot_flops, tot_s, tot_rows, cores = 0.0, 0.0, 0, 1
+    for i in range(steps):
+        tf, dt, nrows, cores = time_oracle_sample(w, inputs, budget, seed=i)
+        tot_flops += tf * 1e12 * dt
+        tot_s += dt
+        tot_rows += nrows
+    value = tot_flops / tot_s / 1e12
+    sample = f"{tot_rows // steps} uniformly sampled query rows of head (0,0) per step, all their allowed keys"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warmup, "ms_per_step": 1e3 * tot_s / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "tokens_per_s": tot_rows / tot_s, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w: Workload):
+    return {"workload": w.name, "B": w.B, "H": w.H, "d": w.d, "N": w.N, "mask": w.mask, "frame_len": w.frame_len,
+            "num_frames": w.num_frames, "chunk_frames": w.chunk_frames, "input_dtype": w.dtype,
+            "unmasked_pairs_per_head": w.unmasked_pairs_per_head, "flop_convention": "12*d per unmasked pair",
+            "l2": "no flush: the six inputs (%.2f GB) are larger than the 126 MB L2" %
+                  (6 * w.B * w.H * w.N * w.d * (2 if w.dtype == "bf16" else 4) / 1e9)}
+
+
+# ----------------------------------------------------------------------------------------------- distributed glue
+def dist_setup(n_gpus: int):
+    """One process per GPU (torchrun env).  -> (rank, world, local_rank, initialised)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+        return rank, world, local, True
+    if n_gpus > 1:
+        raise SystemExit("bench.py --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")
+    return 0, 1, 0, False
+
+
+def aggregate(elapsed_ms: float, units: float, initialised: bool, device: str = "cpu"):
+    """Whole-job numbers: time = max over ranks, units = sum over ranks (no data-path collective anywhere else)."""
+    if not initialised:
+        return elapsed_ms, units
+    import torch.distributed as dist
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def barrier(initialised: bool):
+    if initialised:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+# ----------------------------------------------------------------------------------------------- the CUDA arm
+def run_cuda(args, w: Workload):
+    from paper_2606_25473_b200 import binding as aj
+
+    rank, world, local, inited = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the attention-JVP path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    stream = torch.cuda.current_stream()
+    kind = {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL,
+            "full": aj.AJ_MASK_FULL}[w.mask]
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32)
+    mask, keep = aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames)
+    t0 = time.perf_counter()
+    plan = aj.attn_jvp_plan_create(prob, mask)
+    plan_ms = 1e3 * (time.perf_counter() - t0)
+    kernel, launches_per_call = aj.attn_jvp_plan_kernel(plan)
+    pairs, num_tasks = aj.attn_jvp_plan_info(plan)
+    assert pairs == w.unmasked_pairs_per_head
+
+    # every rank draws its own head shard (seed + rank): weak scaling, no exchange
+    wr = Workload(w.name, w.B, w.H, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std,
+                  w.seed + rank)
+    host = make_inputs(wr, pin=True)
+    devin = [x.to(dev, non_blocking=True) for x in host]
+    o, to = torch.empty_like(devin[0]), torch.empty_like(devin[0])
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device=dev)
+    h_o, h_to = torch.empty_like(host[0]).pin_memory(), torch.empty_like(host[0]).pin_memory()
+    h_lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
+    torch.cuda.synchronize()
+    flops = flops_per_call(w)
+    K, W = args.steps, args.warmup
+
+    def step_device():
+        aj.attn_jvp_fwd(plan, *devin, o, to, lse, stream.cuda_stream)
+
+    def step_host():
+        aj.attn_jvp_fwd_host(plan, *host, h_o, h_to, h_lse, stream.cuda_stream)
+        stream.synchronize()                  # the user reads the result after every step
+
+    # ---- device-resident timing: events on the launching stream, barrier + synchronize on both sides
+    for _ in range(W):
+        step_device()
+    torch.cuda.synchronize()
+    barrier(inited)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    torch.cuda.synchronize()
+    ev[0].record(stream)
+    for i in range(K):
+        step_device()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    barrier(inited)
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[K])
+    per_launch = [ev[i].elapsed_time(ev[i + 1]) for i in range(K)]
+    total_ms_all, flops_all = aggregate(total_ms, flops * K, inited, dev)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the six inputs + kernel + D2H of O, tO, lse
+    for _ in range(min(W, 3)):
+        step_host()
+    torch.cuda.synchronize()
+    barrier(inited)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(K):
+        step_host()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(inited)
+    e2e_ms_all, e2e_flops_all = aggregate(e0.elapsed_time(e1), flops * K, inited, dev)
+    h2d = sum(x.numel() * x.element_size() for x in host)
+    d2h = h_o.numel() * h_o.element_size() * 2 + h_lse.numel() * 4
+
+    aj.attn_jvp_plan_destroy(plan)
+    if rank != 0:
+        return
+    peaks, peak_src = load_peaks()
+    value = flops_all / (total_ms_all * 1e-3) / 1e12
+    avg_launch_ms = total_ms / K
+    achieved = flops / (avg_launch_ms * 1e-3) / 1e12
+    peak = float(peaks.get("bf16_tflops", FALLBACK_PEAKS["bf16_tflops"]))
+    sustained = float(peaks.get("bf16_tflops_sustained", FALLBACK_PEAKS["bf16_tflops_sustained"]))
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": total_ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "config": workload_config(w),
+        "tokens_per_s": world * w.B * w.N / (total_ms_all / K * 1e-3),
+        "kernel": {1: "simt_fp32", 2: "tcgen05_umma"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
+        "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
+        "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "api": "attn_jvp_fwd_host (pinned host buffers, copies inside the timed region)"},
+        "gpu_launches": K * launches_per_call,
+        "clocks": clocks,
+        "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                     "traffic": recorded_traffic(w.name), "peak_source": f"{peak_src} bf16_tflops (burst cuBLAS GEMM)",
+                     "frac_of_sustained": achieved / sustained, "frac_of_nominal_2250": achieved / 2250.0,
+                     "kernel": "attn_jvp_umma_kernel" if kernel == 2 else "attn_jvp_simt_kernel",
+                     "flops_per_launch": flops},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        tf, dt, nrows, cores = time_oracle_sample(w, host, args.cpu_budget_s)
+        line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{nrows} uniformly sampled query rows of head (0,0), all their allowed "
+                                          f"keys, {dt:.1f} s", "extrapolated_full_config_s": flops / (tf * 1e12)}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(WORKLOADS))
+    ap.add_argument("--cpu-budget-s", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    w = WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_cuda(args, w)
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
