@@ -149,6 +149,14 @@ aj_status attn_jvp_fwd_host(aj_plan *plan, const void *q, const void *k, const v
                             const void *tk, const void *tv, void *o, void *to, float *lse,
                             void *cuda_stream);
 
+/*
+ * Device-side health of the plan's last launches: synchronises the device, then *code = 0 if every
+ * attn_jvp_fwd on this plan ran to completion, else a non-zero internal code (a pipeline wait of the
+ * tcgen05 kernel timed out and the launch was abandoned: its outputs are garbage).  Resets the code.
+ * Returns AJ_ERR_CUDA if the device itself reports an error.
+ */
+aj_status attn_jvp_plan_device_status(aj_plan *plan, int32_t *code);
+
 /* Message for the most recent non-OK status returned to this thread ("" if none). Never NULL. */
 const char *attn_jvp_last_error(void);
 /* Library version string, e.g. "attn_jvp 0.1 (sm_100a)". */

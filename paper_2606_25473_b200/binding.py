@@ -53,7 +53,7 @@ class AttnJvpError(RuntimeError):
 SYMBOLS = [
     "attn_jvp_schedule_create", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel",
-    "attn_jvp_plan_kernel", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
+    "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
 ]
 
 _lib = None
@@ -77,6 +77,7 @@ def lib():
         l.attn_jvp_plan_info.argtypes = [vp, i64p, _I32P]
         l.attn_jvp_plan_set_kernel.argtypes = [vp, i32]
         l.attn_jvp_plan_kernel.argtypes = [vp, _I32P, _I32P]
+        l.attn_jvp_plan_device_status.argtypes = [vp, _I32P]
         l.attn_jvp_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp]
         l.attn_jvp_fwd_host.argtypes = [vp] * 11
         for name in SYMBOLS:
@@ -188,6 +189,13 @@ def attn_jvp_plan_kernel(plan):
     a, b = ctypes.c_int32(), ctypes.c_int32()
     _check(lib().attn_jvp_plan_kernel(plan, ctypes.byref(a), ctypes.byref(b)))
     return a.value, b.value
+
+
+def attn_jvp_plan_device_status(plan) -> int:
+    """Synchronises the device; 0 if every launch of the plan completed, else the kernel's abort code."""
+    a = ctypes.c_int32()
+    _check(lib().attn_jvp_plan_device_status(plan, ctypes.byref(a)))
+    return a.value
 
 
 def _tensor(t) -> aj_tensor:

@@ -192,6 +192,15 @@ aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launc
     return AJ_OK;
 }
 
+aj_status attn_jvp_plan_device_status(aj_plan *p, int32_t *code) {
+    if (!p || !code) return fail(AJ_ERR_INVALID_ARG, "plan or code is NULL");
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(code, p->d_counters + 2, sizeof(int32_t), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && *code != 0) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
+    if (e != cudaSuccess) return cuda_fail(e, "device status");
+    return AJ_OK;
+}
+
 aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
                        const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
                        void *cuda_stream) {

@@ -12,11 +12,17 @@
 //
 // CTA = 8 warps, persistent, one CTA per SM:
 //   warp 0      TMA producer (one lane): task fetch, Q/tQ tile, ring of {K,tK} / {V,tV} half-stages
-//   warp 1      MMA issuer (one lane): QK(j+1) is issued before PV(j) so the tensor pipe never waits on softmax
+//   warp 1      MMA issuer (whole warp runs the loop so every descriptor stays in uniform registers, one elected
+//               lane issues): QK(j+1) is issued before PV(j) so the tensor pipe never waits on softmax
 //   warp 2      TMEM allocator
 //   warps 4-7   softmax + tangent weights + lazy rescale + epilogue; thread = one query row (TMEM lane)
 // TMEM columns (fp32): O [0,128) | T [128,256) | S0 [256,320) tS0 [320,384) | S1 [384,448) tS1 [448,512);
 // P~ and H~ (bf16, 32 columns each) overwrite the first half of their S / tS buffer.
+// The six contractions of a tile are four MMA shapes (operands adjacent in shared memory / TMEM):
+//   [S | tS]  = Q [K ; tK]^T   (N = 128)      tS += tQ K^T      (N = 64)       -- 2 x 8 instructions (K = 16 each)
+//   [O | T]  += P~ [V | tV]    (N = 256)      T  += H~ V        (N = 128)      -- 2 x 4 instructions
+// which cuts the operand bytes read from shared memory per tile from 192 KB to 160 KB (the 128 B/clk shared-memory
+// port, not the tensor pipe, bounds the N = 64 shapes) and the issue count from 36 to 24.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -48,7 +54,7 @@ constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
 enum {
     BAR_Q_FULL = 0, BAR_Q_EMPTY,
     BAR_KV_FULL, BAR_KV_EMPTY = BAR_KV_FULL + NSTAGE,
-    BAR_S_FULL = BAR_KV_EMPTY + NSTAGE, BAR_P_FULL = BAR_S_FULL + 2, BAR_PV_DONE = BAR_P_FULL + 2,
+    BAR_S_FULL = BAR_KV_EMPTY + NSTAGE, BAR_P_FULL = BAR_S_FULL + 2, BAR_H_FULL = BAR_P_FULL + 2, BAR_PV_DONE = BAR_H_FULL + 2,
     BAR_TASK_FULL = BAR_PV_DONE + 2, BAR_TASK_EMPTY = BAR_TASK_FULL + 2, NUM_BARS = BAR_TASK_EMPTY + 2
 };
 
@@ -73,24 +79,35 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug prints where it is stuck and makes every role leave instead of hanging the GPU.
-__device__ __forceinline__ bool mbar_wait(uint32_t bar0, int idx, uint32_t parity, volatile int *abort_flag) {
-    const uint32_t bar = bar0 + 8u * idx;
-    if (mbar_try_wait(bar, parity)) return true;
+// Bounded wait.  A protocol bug must never hang the GPU: after ~2 s the waiter reports where it is stuck, raises the
+// CTA-wide abort flag and the error word the host reads back; from then on every wait of the CTA returns at once, so
+// all roles run off the end of their (now meaningless) work and the kernel ends.
+__device__ __noinline__ void mbar_wait_slow(uint32_t bar, int idx, uint32_t parity, volatile int *abort_flag, int32_t *err) {
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0xff) == 0) {
-            if (*abort_flag) return false;
+        if ((++spins & 0x3f) == 0) {
+            if (*abort_flag) return;
             if (clock64() - t0 > 4000000000LL) {
                 printf("attn_jvp umma: timeout block %d thread %d barrier %d parity %u\n", blockIdx.x, threadIdx.x, idx, parity);
                 *abort_flag = 1;
-                return false;
+                atomicExch(err, 1 + idx);
+                return;
             }
         }
     }
-    return true;
 }
+struct Waiter {
+    uint32_t bars;
+    volatile int *abort_flag;
+    int32_t *err;
+    __device__ __forceinline__ void operator()(int idx, uint32_t parity) const {
+        const uint32_t bar = bars + 8u * idx;
+        if (mbar_try_wait(bar, parity)) return;
+        if (mbar_try_wait(bar, parity)) return;
+        mbar_wait_slow(bar, idx, parity, abort_flag, err);
+    }
+};
 
 // ---- TMA ------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2, int c3) {
@@ -105,28 +122,43 @@ __device__ __forceinline__ void prefetch_tmap(const CUtensorMap *map) {
 // ---- tcgen05 --------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ bool elect_one() {
+    uint32_t p;
+    asm volatile("{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\tselp.b32 %0, 1, 0, q;\n\t}" : "=r"(p));
+    return p != 0;
+}
+// A value every lane of the (converged) warp holds, moved to a uniform register (CREDUX writes UR).
+__device__ __forceinline__ uint32_t warp_uniform(uint32_t v) { return __reduce_max_sync(0xffffffffu, v); }
+
+// Shared-memory matrix descriptors (PTX ISA "tcgen05 shared memory descriptor"): start address, leading / stride
+// byte offsets in 16-byte units, descriptor version 1 (bit 46), 128-byte swizzle (value 2 in bits 61-63).  The low
+// word (address and LBO) changes per instruction, the high word is a constant per operand kind.
+constexpr uint32_t desc_hi(uint32_t sbo_bytes) { return ((sbo_bytes >> 4) & 0x3FFF) | (1u << 14) | (2u << 29); }
+constexpr uint32_t desc_lo_lbo(uint32_t lbo_bytes) { return ((lbo_bytes >> 4) & 0x3FFF) << 16; }
 // D[tmem] (+)= A[smem] * B[smem]
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi, uint32_t idesc, uint32_t accum) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
+        "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %6, 0;\n\t"
+        "mov.b64 da, {%1, %2};\n\tmov.b64 db, {%3, %4};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accum) : "memory");
 }
 // D[tmem] (+)= A[tmem] * B[smem]
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc, uint32_t accum) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
+        "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+        "mov.b64 db, {%2, %3};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accum) : "memory");
 }
 
 #define AJ_R8(r, o) "=r"(r[o + 0]), "=r"(r[o + 1]), "=r"(r[o + 2]), "=r"(r[o + 3]), "=r"(r[o + 4]), "=r"(r[o + 5]), "=r"(r[o + 6]), "=r"(r[o + 7])
 #define AJ_I8(r, o) "r"(r[o + 0]), "r"(r[o + 1]), "r"(r[o + 2]), "r"(r[o + 3]), "r"(r[o + 4]), "r"(r[o + 5]), "r"(r[o + 6]), "r"(r[o + 7])
+#define AJ_P8(r, o) "+r"(r[o + 0]), "+r"(r[o + 1]), "+r"(r[o + 2]), "+r"(r[o + 3]), "+r"(r[o + 4]), "+r"(r[o + 5]), "+r"(r[o + 6]), "+r"(r[o + 7])
 
 // 32 lanes x 32 consecutive fp32 columns: thread t of the warp gets lane (taddr.lane + t).
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
@@ -136,6 +168,14 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
         : AJ_R8(r, 0), AJ_R8(r, 8), AJ_R8(r, 16), AJ_R8(r, 24) : "r"(taddr) : "memory");
 }
+// tcgen05.wait::ld that also names the loaded registers, so no use of them can be scheduled above the wait.
+__device__ __forceinline__ void tc_wait_ld(uint32_t (&r)[32]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : AJ_P8(r, 0), AJ_P8(r, 8), AJ_P8(r, 16), AJ_P8(r, 24)::"memory");
+}
+__device__ __forceinline__ void tc_wait_ld(uint32_t (&a)[32], uint32_t (&b)[32]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : AJ_P8(a, 0), AJ_P8(a, 8), AJ_P8(a, 16), AJ_P8(a, 24), AJ_P8(b, 0), AJ_P8(b, 8), AJ_P8(b, 16), AJ_P8(b, 24)::"memory");
+}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x32.b32 [%32], "
@@ -143,13 +183,14 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
         "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
         ::AJ_I8(r, 0), AJ_I8(r, 8), AJ_I8(r, 16), AJ_I8(r, 24), "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15};"
-        ::AJ_I8(r, 0), AJ_I8(r, 8), "r"(taddr) : "memory");
-}
 
+// ---- fp32 helpers: packed pairs (FFMA2 / FMUL2 / FADD2 halve the issue slots of the softmax role) -----------------
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ uint64_t pack2(uint32_t lo, uint32_t hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi)); return r; }
+__device__ __forceinline__ void unpack2(uint64_t v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) { uint64_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ uint64_t fmul2(uint64_t a, uint64_t b) { uint64_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) { uint64_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ float ex2(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -162,19 +203,18 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     return r;
 }
 
-// Shared-memory matrix descriptors (PTX ISA "tcgen05 shared memory descriptor"): start address, leading / stride
-// byte offsets in 16-byte units, descriptor version 1 (bit 46), 128-byte swizzle (value 2 in bits 61-63).
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46) | (2ull << 61);
-}
 // Instruction descriptor for kind::f16: D fp32 (bits 4-5 = 1), A and B bf16 (bits 7-9, 10-12 = 1), B major (bit 16),
 // N >> 3 (bits 17-22), M >> 4 (bits 24-28).
 constexpr uint32_t make_idesc(int n, bool b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BR >> 4) << 24);
 }
-constexpr uint32_t IDESC_QK = make_idesc(BC, false);  // 128 x 64 x 16, A and B K-major
-constexpr uint32_t IDESC_PV = make_idesc(D, true);    // 128 x 128 x 16, A from TMEM, B (V) MN-major
+constexpr uint32_t IDESC_QK2 = make_idesc(2 * BC, false);  // 128 x 128 x 16: [S | tS] = Q [K ; tK]^T, A and B K-major
+constexpr uint32_t IDESC_QK1 = make_idesc(BC, false);      // 128 x  64 x 16: tS += tQ K^T
+constexpr uint32_t IDESC_PV2 = make_idesc(2 * D, true);    // 128 x 256 x 16: [O | T] += P~ [V | tV], A from TMEM, B MN-major
+constexpr uint32_t IDESC_PV1 = make_idesc(D, true);        // 128 x 128 x 16: T += H~ V
+constexpr uint32_t DESC_HI = desc_hi(1024);                // 8-row (K-major) / 8-key (MN-major) groups are 1024 B apart
+constexpr uint32_t LBO_K = desc_lo_lbo(16);                // K-major with 128 B swizzle: unused, canonical value
+constexpr uint32_t LBO_V = desc_lo_lbo(KVHALF_BYTES);      // MN-major: 64-column blocks [V h0 | V h1 | tV h0 | tV h1] 8 KB apart
 
 // Walks the key tiles of a task in order: ranges [rb, rb + rc), each cut into BC-key tiles from its start.
 struct TileCursor {
@@ -207,7 +247,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
     Shared *sh = reinterpret_cast<Shared *>(smem_raw + (tiles - raw) + SMEM_TILES);
     const uint32_t sQ = tiles, sTQ = tiles + Q_BYTES, sRing = tiles + 2 * Q_BYTES;
     const uint32_t bars = smem_u32(sh->bars);
-    volatile int *abort_flag = &sh->abort_flag;
+    const Waiter wait{bars, &sh->abort_flag, prm.counters + 2};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
@@ -217,9 +257,10 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
         for (int i = 0; i < 2; ++i) {
             mbar_init(bars + 8 * (BAR_S_FULL + i), 1);
             mbar_init(bars + 8 * (BAR_P_FULL + i), 128);
+            mbar_init(bars + 8 * (BAR_H_FULL + i), 128);
             mbar_init(bars + 8 * (BAR_PV_DONE + i), 1);
             mbar_init(bars + 8 * (BAR_TASK_FULL + i), 1);
-            mbar_init(bars + 8 * (BAR_TASK_EMPTY + i), 5);   // MMA lane + one lane of each softmax warp
+            mbar_init(bars + 8 * (BAR_TASK_EMPTY + i), 5);   // MMA warp + one lane of each softmax warp
         }
         sh->abort_flag = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -243,7 +284,8 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             int task_id = blockIdx.x;
             for (uint32_t t = 0;; ++t) {
                 const int ts = t & 1;
-                if (!mbar_wait(bars, BAR_TASK_EMPTY + ts, ((t >> 1) & 1) ^ 1, abort_flag)) break;
+                wait(BAR_TASK_EMPTY + ts, ((t >> 1) & 1) ^ 1);
+                if (sh->abort_flag) task_id = prm.num_tasks;
                 sh->task_id[ts] = task_id;
                 mbar_arrive(bars + 8 * (BAR_TASK_FULL + ts));
                 if (task_id >= prm.num_tasks) break;
@@ -251,7 +293,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 task_id = atomicAdd(&prm.counters[0], 1) + gridDim.x;
                 if (task.num_kv_tiles == 0) continue;
                 // Q_i, tQ_i: two 64-column swizzle blocks each
-                if (!mbar_wait(bars, BAR_Q_EMPTY, (nq & 1) ^ 1, abort_flag)) break;
+                wait(BAR_Q_EMPTY, (nq & 1) ^ 1);
                 mbar_expect_tx(bars + 8 * BAR_Q_FULL, 2 * Q_BYTES);
                 tma_load_4d(sQ, &prm.tm_q, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
                 tma_load_4d(sQ + QHALF_BYTES, &prm.tm_q, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
@@ -259,145 +301,151 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 tma_load_4d(sTQ + QHALF_BYTES, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
                 ++nq;
                 // ring order = MMA consumption order: KtK(0), KtK(1), VtV(0), KtK(2), VtV(1), ...
+                // {K,tK} slot: [K h0 | tK h0 | K h1 | tK h1] so that [K ; tK] is one 128-row B operand per 64-column half;
+                // {V,tV} slot: [V h0 | V h1 | tV h0 | tV h1] so that [V | tV] is one 256-column B operand.   (8 KB each)
                 TileCursor ck, cv;
                 ck.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
                 cv = ck;
                 const int n = task.num_kv_tiles;
-                auto push = [&](bool is_k) -> bool {
+                auto push = [&](bool is_k) {
                     const uint32_t slot = ring % NSTAGE;
-                    if (!mbar_wait(bars, BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1, abort_flag)) return false;
+                    wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                     const uint32_t dst = sRing + slot * SLOT_BYTES, full = bars + 8 * (BAR_KV_FULL + slot);
                     mbar_expect_tx(full, SLOT_BYTES);
                     TileCursor &c = is_k ? ck : cv;
                     const CUtensorMap *m0 = is_k ? &prm.tm_k : &prm.tm_v, *m1 = is_k ? &prm.tm_tk : &prm.tm_tv;
+                    const uint32_t o_m0h1 = is_k ? 2 * KVHALF_BYTES : KVHALF_BYTES, o_m1h0 = is_k ? KVHALF_BYTES : 2 * KVHALF_BYTES;
                     const int row = c.key_row();
                     tma_load_4d(dst, m0, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + KVHALF_BYTES, m0, full, 64, row, task.h, task.b);
-                    tma_load_4d(dst + KV_BYTES, m1, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + KV_BYTES + KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
+                    tma_load_4d(dst + o_m0h1, m0, full, 64, row, task.h, task.b);
+                    tma_load_4d(dst + o_m1h0, m1, full, 0, row, task.h, task.b);
+                    tma_load_4d(dst + 3 * KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
                     c.next();
                     ++ring;
-                    return true;
                 };
-                bool ok = push(true);
-                for (int j = 0; j < n && ok; ++j) {
-                    if (j + 1 < n) ok = push(true);
-                    if (ok) ok = push(false);
+                push(true);
+                for (int j = 0; j < n; ++j) {
+                    if (j + 1 < n) push(true);
+                    push(false);
                 }
-                if (!ok) break;
             }
             // the last CTA to run out of work re-arms the counters for the next launch
-            if (!*abort_flag) {
-                const int done = atomicAdd(&prm.counters[1], 1);
-                if (done == (int)gridDim.x - 1) { prm.counters[0] = 0; prm.counters[1] = 0; __threadfence(); }
-            }
+            const int done = atomicAdd(&prm.counters[1], 1);
+            if (done == (int)gridDim.x - 1) { prm.counters[0] = 0; prm.counters[1] = 0; __threadfence(); }
         }
     } else if (warp == 1) {
         // ================================================= MMA issuer ============================================
-        if (lane == 0) {
-            uint32_t ring = 0, nq = 0, g = 0;   // g = tiles issued so far (selects S/tS buffer and barrier phase)
-            for (uint32_t t = 0;; ++t) {
-                const int ts = t & 1;
-                if (!mbar_wait(bars, BAR_TASK_FULL + ts, (t >> 1) & 1, abort_flag)) break;
-                const int task_id = sh->task_id[ts];
-                mbar_arrive(bars + 8 * (BAR_TASK_EMPTY + ts));
-                if (task_id >= prm.num_tasks) break;
-                const int n = prm.tasks[task_id].num_kv_tiles;
-                if (n == 0) continue;
-                if (!mbar_wait(bars, BAR_Q_FULL, nq & 1, abort_flag)) break;
-                ++nq;
-                tc_fence_after();
-                bool ok = true;
-                auto issue_qk = [&](uint32_t gj) -> bool {
-                    const uint32_t slot = ring % NSTAGE;
-                    if (!mbar_wait(bars, BAR_KV_FULL + slot, (ring / NSTAGE) & 1, abort_flag)) return false;
-                    tc_fence_after();
-                    const uint32_t sK = sRing + slot * SLOT_BYTES, sTK = sK + KV_BYTES;
-                    const uint32_t tS_ = tmem + TM_S0 + (gj & 1) * TM_SBUF, tTS_ = tmem + TM_TS0 + (gj & 1) * TM_SBUF;
+        // Every lane runs the control flow (so ring / tile counters and descriptors are warp-uniform and live in
+        // uniform registers); the elected lane alone issues tcgen05.mma / tcgen05.commit.
+        const bool leader = elect_one();
+        const uint32_t q_lo = ((sQ >> 4) & 0x3FFF) | LBO_K, tq_lo = ((sTQ >> 4) & 0x3FFF) | LBO_K;
+        uint32_t ring = 0, nq = 0, g = 0;   // g = tiles issued so far (selects S/tS buffer and barrier phase)
+        auto issue_qk = [&](uint32_t gj) {
+            const uint32_t slot = ring % NSTAGE;
+            wait(BAR_KV_FULL + slot, (ring / NSTAGE) & 1);
+            tc_fence_after();
+            const uint32_t k_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_K;
+            const uint32_t tS_ = tmem + TM_S0 + (gj & 1) * TM_SBUF, tTS_ = tS_ + (TM_TS0 - TM_S0);
+            if (leader) {
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        const uint32_t qoff = (ks >> 2) * QHALF_BYTES + (ks & 3) * 32;
-                        const uint32_t koff = (ks >> 2) * KVHALF_BYTES + (ks & 3) * 32;
-                        const uint64_t dq = make_desc(sQ + qoff, 16, 1024), dtq = make_desc(sTQ + qoff, 16, 1024);
-                        const uint64_t dk = make_desc(sK + koff, 16, 1024), dtk = make_desc(sTK + koff, 16, 1024);
-                        mma_ss(tS_, dq, dk, IDESC_QK, ks > 0);        // S  = Q K^T
-                        mma_ss(tTS_, dtq, dk, IDESC_QK, ks > 0);      // tS = tQ K^T
-                        mma_ss(tTS_, dq, dtk, IDESC_QK, 1);           //    + Q tK^T
-                    }
-                    tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
-                    tc_commit(bars + 8 * (BAR_S_FULL + (gj & 1)));
-                    ++ring;
-                    return true;
-                };
-                if (!issue_qk(g)) break;
-                for (int j = 0; j < n; ++j) {
-                    const uint32_t gj = g + j;
-                    if (j + 1 < n) { if (!issue_qk(gj + 1)) { ok = false; break; } }
-                    else tc_commit(bars + 8 * BAR_Q_EMPTY);           // every QK of this task has been issued
-                    if (!mbar_wait(bars, BAR_P_FULL + (gj & 1), (gj >> 1) & 1, abort_flag)) { ok = false; break; }
-                    const uint32_t slot = ring % NSTAGE;
-                    if (!mbar_wait(bars, BAR_KV_FULL + slot, (ring / NSTAGE) & 1, abort_flag)) { ok = false; break; }
-                    tc_fence_after();
-                    const uint32_t sV = sRing + slot * SLOT_BYTES, sTV = sV + KV_BYTES;
-                    const uint32_t tP = tmem + TM_S0 + (gj & 1) * TM_SBUF, tH = tmem + TM_TS0 + (gj & 1) * TM_SBUF;
-#pragma unroll
-                    for (int ks = 0; ks < BC / 16; ++ks) {
-                        // V tile in smem: key row r at r*128 bytes inside each 64-column block; blocks 8 KB apart.
-                        const uint64_t dv = make_desc(sV + ks * 2048, KVHALF_BYTES, 1024);
-                        const uint64_t dtv = make_desc(sTV + ks * 2048, KVHALF_BYTES, 1024);
-                        const uint32_t acc = (j > 0 || ks > 0) ? 1u : 0u;
-                        mma_ts(tmem + TM_O, tP + ks * 8, dv, IDESC_PV, acc);     // O += P~ V
-                        mma_ts(tmem + TM_T, tP + ks * 8, dtv, IDESC_PV, acc);    // T += P~ tV
-                        mma_ts(tmem + TM_T, tH + ks * 8, dv, IDESC_PV, 1);       // T += H~ V
-                    }
-                    tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
-                    tc_commit(bars + 8 * (BAR_PV_DONE + (gj & 1)));
-                    ++ring;
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
+                    const uint32_t koff = ((ks >> 2) * 2 * KVHALF_BYTES + (ks & 3) * 32) >> 4;
+                    mma_ss(tS_, q_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK2, ks > 0);   // [S | tS] = Q [K ; tK]^T
+                    mma_ss(tTS_, tq_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK1, 1);      // tS += tQ K^T
                 }
-                if (!ok) break;
-                g += n;
+                tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
+                tc_commit(bars + 8 * (BAR_S_FULL + (gj & 1)));
             }
+            __syncwarp();
+            ++ring;
+        };
+        for (uint32_t t = 0;; ++t) {
+            const int ts = t & 1;
+            wait(BAR_TASK_FULL + ts, (t >> 1) & 1);
+            const int task_id = (int)warp_uniform((uint32_t)sh->task_id[ts] | (sh->abort_flag ? 0x40000000u : 0u));
+            if (leader) mbar_arrive(bars + 8 * (BAR_TASK_EMPTY + ts));
+            if (task_id >= prm.num_tasks) break;
+            const int n = (int)warp_uniform((uint32_t)prm.tasks[task_id].num_kv_tiles);
+            if (n == 0) continue;
+            wait(BAR_Q_FULL, nq & 1);
+            ++nq;
+            tc_fence_after();
+            issue_qk(g);
+            for (int j = 0; j < n; ++j) {
+                const uint32_t gj = g + j, b = gj & 1;
+                if (j + 1 < n) issue_qk(gj + 1);
+                else if (leader) tc_commit(bars + 8 * BAR_Q_EMPTY);   // every QK of this task has been issued
+                const uint32_t slot = ring % NSTAGE;
+                // V tile in smem: key row r at r*128 bytes inside each 64-column block; 16-key K steps are 2 KB apart.
+                const uint32_t v_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_V;
+                const uint32_t tP = tmem + TM_S0 + b * TM_SBUF, tH = tP + (TM_TS0 - TM_S0);
+                const uint32_t acc = j > 0 ? 1u : 0u;
+                wait(BAR_P_FULL + b, (gj >> 1) & 1);
+                wait(BAR_KV_FULL + slot, (ring / NSTAGE) & 1);
+                tc_fence_after();
+                if (leader) {
+#pragma unroll
+                    for (int ks = 0; ks < BC / 16; ++ks)    // [O | T] += P~ [V | tV]
+                        mma_ts(tmem + TM_O, tP + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV2, acc | (ks > 0));
+                }
+                __syncwarp();
+                wait(BAR_H_FULL + b, (gj >> 1) & 1);
+                tc_fence_after();
+                if (leader) {
+#pragma unroll
+                    for (int ks = 0; ks < BC / 16; ++ks)    // T += H~ V
+                        mma_ts(tmem + TM_T, tH + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV1, 1);
+                    tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
+                    tc_commit(bars + 8 * (BAR_PV_DONE + b));
+                }
+                __syncwarp();
+                ++ring;
+            }
+            g += n;
         }
     } else if (warp >= 4) {
         // ================================================= softmax / tangent weights / epilogue ==================
         const int row = threadIdx.x - 128;                       // query row inside the tile = TMEM lane
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const float sl2 = prm.scale_log2, sc = prm.scale;
+        const uint64_t sl2_2 = pack2(sl2, sl2), sc_2 = pack2(sc, sc);
         uint32_t g = 0;
         for (uint32_t t = 0;; ++t) {
             const int ts = t & 1;
-            if (!mbar_wait(bars, BAR_TASK_FULL + ts, (t >> 1) & 1, abort_flag)) break;
+            wait(BAR_TASK_FULL + ts, (t >> 1) & 1);
             const int task_id = sh->task_id[ts];
             __syncwarp();
             if (lane == 0) mbar_arrive(bars + 8 * (BAR_TASK_EMPTY + ts));
-            if (task_id >= prm.num_tasks) break;
+            if (task_id >= prm.num_tasks || sh->abort_flag) break;
             const aj_task task = prm.tasks[task_id];
             const int n = task.num_kv_tiles;
-            float m_ref = 0.f, l = 0.f, r = 0.f;
+            float m_ref = 0.f;
+            uint64_t l2[2] = {0ull, 0ull}, r2[2] = {0ull, 0ull};   // 4 partial sums each of l = sum P~ and r = sum H~
             TileCursor cur;
             cur.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
-            bool ok = true;
             for (int j = 0; j < n; ++j, cur.next()) {
                 const uint32_t gj = g + j, b = gj & 1;
-                const uint32_t tS_ = tmem + lane_base + TM_S0 + b * TM_SBUF, tTS_ = tmem + lane_base + TM_TS0 + b * TM_SBUF;
-                if (!mbar_wait(bars, BAR_S_FULL + b, (gj >> 1) & 1, abort_flag)) { ok = false; break; }
+                const uint32_t tS_ = tmem + lane_base + TM_S0 + b * TM_SBUF, tTS_ = tS_ + (TM_TS0 - TM_S0);
+                wait(BAR_S_FULL + b, (gj >> 1) & 1);
                 tc_fence_after();
-                uint32_t su[2][32];
+                uint32_t su[2][32], tu[2][32];
                 tmem_ld32(tS_, su[0]);
                 tmem_ld32(tS_ + 32, su[1]);
-                tc_wait_ld();
-                float s[BC];
-#pragma unroll
-                for (int c = 0; c < BC; ++c) s[c] = __uint_as_float(su[c >> 5][c & 31]);
+                tc_wait_ld(su[0], su[1]);
+                tmem_ld32(tTS_, tu[0]);                            // in flight while P~ is computed
+                tmem_ld32(tTS_ + 32, tu[1]);
                 const int valid = cur.valid();
                 if (valid < BC) {                                 // tile-valid mask: S = -inf
 #pragma unroll
-                    for (int c = 0; c < BC; ++c) if (c >= valid) s[c] = -INFINITY;
+                    for (int c = 0; c < BC; ++c) if (c >= valid) su[c >> 5][c & 31] = 0xff800000u;
                 }
-                float mx = s[0];
+                float mx[4];
 #pragma unroll
-                for (int c = 1; c < BC; ++c) mx = fmaxf(mx, s[c]);
-                const float cand = mx * sl2;
+                for (int i = 0; i < 4; ++i) mx[i] = __uint_as_float(su[0][i]);
+#pragma unroll
+                for (int c = 4; c < BC; ++c) mx[c & 3] = fmaxf(mx[c & 3], __uint_as_float(su[c >> 5][c & 31]));
+                const float cand = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * sl2;
                 if (j == 0) {
                     m_ref = cand;
                 } else {
@@ -405,53 +453,62 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     if (__any_sync(0xffffffffu, need)) {
                         // e^{m - m_new} applied to O, T (= A + B), l, r; needs PV(j-1) finished
                         const uint32_t gp = gj - 1;
-                        if (!mbar_wait(bars, BAR_PV_DONE + (gp & 1), (gp >> 1) & 1, abort_flag)) { ok = false; break; }
+                        wait(BAR_PV_DONE + (gp & 1), (gp >> 1) & 1);
                         tc_fence_after();
                         const float f = need ? ex2(m_ref - cand) : 1.f;
 #pragma unroll 1
                         for (int cb = 0; cb < 256; cb += 32) {
                             uint32_t a[32];
                             tmem_ld32(tmem + lane_base + cb, a);
-                            tc_wait_ld();
+                            tc_wait_ld(a);
 #pragma unroll
                             for (int c = 0; c < 32; ++c) a[c] = __float_as_uint(__uint_as_float(a[c]) * f);
                             tmem_st32(tmem + lane_base + cb, a);
                         }
-                        l *= f; r *= f;
+                        const uint64_t f2 = pack2(f, f);
+                        l2[0] = fmul2(l2[0], f2); l2[1] = fmul2(l2[1], f2);
+                        r2[0] = fmul2(r2[0], f2); r2[1] = fmul2(r2[1], f2);
                         if (need) m_ref = cand;
                     }
                 }
                 // P~ = exp2(S*s*log2e - m_ref); l += rowsum
+                const uint64_t negm2 = pack2(-m_ref, -m_ref);
+                float p[BC];
+                {
+                    uint32_t pk[32];
 #pragma unroll
-                for (int c = 0; c < BC; ++c) { s[c] = ex2(fmaf(s[c], sl2, -m_ref)); l += s[c]; }
-#pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int c = 0; c < 16; ++c) pk[c] = pack_bf16(s[hh * 32 + 2 * c], s[hh * 32 + 2 * c + 1]);
-                    tmem_st16(tS_ + hh * 16, pk);
-                }
-                // H~ = P~ o (s * tS); r += rowsum (PAPER.md:932-936).  Masked columns have P~ = 0, so H~ = 0.
-#pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    uint32_t tu[32];
-                    tmem_ld32(tTS_ + hh * 32, tu);
-                    tc_wait_ld();
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int c = 0; c < 16; ++c) {
-                        const float h0 = s[hh * 32 + 2 * c] * (__uint_as_float(tu[2 * c]) * sc);
-                        const float h1 = s[hh * 32 + 2 * c + 1] * (__uint_as_float(tu[2 * c + 1]) * sc);
-                        r += h0; r += h1;
-                        pk[c] = pack_bf16(h0, h1);
+                    for (int c = 0; c < BC / 2; ++c) {
+                        const uint64_t x = ffma2(pack2(su[c >> 4][(2 * c) & 31], su[c >> 4][(2 * c + 1) & 31]), sl2_2, negm2);
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        p[2 * c] = ex2(x0); p[2 * c + 1] = ex2(x1);
+                        l2[c & 1] = fadd2(l2[c & 1], pack2(p[2 * c], p[2 * c + 1]));
+                        pk[c] = pack_bf16(p[2 * c], p[2 * c + 1]);
                     }
-                    tmem_st16(tTS_ + hh * 16, pk);
+                    tmem_st32(tS_, pk);
                 }
                 tc_wait_st();
                 tc_fence_before();
                 mbar_arrive(bars + 8 * (BAR_P_FULL + b));
+                // H~ = P~ o (s * tS); r += rowsum (PAPER.md:932-936).  Masked columns have P~ = 0, so H~ = 0.
+                tc_wait_ld(tu[0], tu[1]);
+                {
+                    uint32_t hk[32];
+#pragma unroll
+                    for (int c = 0; c < BC / 2; ++c) {
+                        const uint64_t tsc = fmul2(pack2(tu[c >> 4][(2 * c) & 31], tu[c >> 4][(2 * c + 1) & 31]), sc_2);
+                        const uint64_t h = fmul2(pack2(p[2 * c], p[2 * c + 1]), tsc);
+                        r2[c & 1] = fadd2(r2[c & 1], h);
+                        float h0, h1;
+                        unpack2(h, h0, h1);
+                        hk[c] = pack_bf16(h0, h1);
+                    }
+                    tmem_st32(tTS_, hk);
+                }
+                tc_wait_st();
+                tc_fence_before();
+                mbar_arrive(bars + 8 * (BAR_H_FULL + b));
             }
-            if (!ok) break;
             // ---- epilogue (Eq. 45) ----
             const bool store = row < task.q_rows;
             const int64_t grow = task.q_begin + row;
@@ -467,16 +524,20 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             }
             {
                 const uint32_t gl = g + n - 1;
-                if (!mbar_wait(bars, BAR_PV_DONE + (gl & 1), (gl >> 1) & 1, abort_flag)) break;
+                wait(BAR_PV_DONE + (gl & 1), (gl >> 1) & 1);
                 tc_fence_after();
             }
+            float la, lb, lc, ld, ra, rb, rc, rd;
+            unpack2(l2[0], la, lb); unpack2(l2[1], lc, ld);
+            unpack2(r2[0], ra, rb); unpack2(r2[1], rc, rd);
+            const float l = (la + lb) + (lc + ld), r = (ra + rb) + (rc + rd);
             const float inv = 1.f / l, rl = r * inv;
 #pragma unroll 1
             for (int cb = 0; cb < D; cb += 32) {
                 uint32_t ao[32], at[32];
                 tmem_ld32(tmem + lane_base + TM_O + cb, ao);
                 tmem_ld32(tmem + lane_base + TM_T + cb, at);
-                tc_wait_ld();
+                tc_wait_ld(ao, at);
                 if (store) {
 #pragma unroll
                     for (int v4 = 0; v4 < 4; ++v4) {

@@ -36,6 +36,7 @@ def run_gpu(w: Workload, inputs_cpu, kernel: int = aj.AJ_KERNEL_AUTO, plan=None)
     lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")
     aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0, "the kernel abandoned a launch (pipeline wait timed out)"
     if own:
         aj.attn_jvp_plan_destroy(plan)
     return o.cpu(), to.cpu(), lse.cpu()
