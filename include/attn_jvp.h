@@ -85,13 +85,25 @@ typedef struct {
     int64_t stride_b, stride_h, stride_n;
 } aj_tensor;
 
-/* One unit of work: a query tile inside one query group, for one (b, h) ("tasks (g,i)"). */
+/*
+ * How query rows are cut into tiles.  PER_GROUP: tiles start at each query group's first row, so every row of a
+ * tile sees the same keys ("i is a query tile inside Q_g").  PACKED: tiles lie on a global grid of
+ * tile_q rows ("Split Q into query tiles"); a tile that straddles groups streams the union of
+ * their key ranges and every entry carries the interval of tile rows that may see it (the other rows are masked,
+ * PAPER.md:909-914).  Same results; PACKED wastes no rows at group ends.
+ */
+typedef enum { AJ_TILING_PER_GROUP = 0, AJ_TILING_PACKED = 1 } aj_tiling;
+
+/* One unit of work: a query tile for one (b, h) ("tasks (g,i)").  Its keys are the schedule ENTRIES
+ * [range_begin, range_begin + range_count): entry e = keys [k_begin[e], k_end[e]) seen by tile rows
+ * [row_begin[e], row_end[e]) (relative to q_begin).  PER_GROUP: entries are the lowered key ranges (same indices as
+ * attn_jvp_schedule_get) with rows [0, tile_q). */
 typedef struct {
     int32_t b, h;
     int32_t q_begin, q_rows;          /* query rows [q_begin, q_begin + q_rows) */
-    int32_t range_begin, range_count; /* its key ranges: schedule ranges [range_begin, +range_count) */
-    int32_t num_kv_tiles;             /* key tiles it streams (sum over ranges of ceil(len / tile_k)) */
-    int32_t group;                    /* index of its query group */
+    int32_t range_begin, range_count; /* its entries */
+    int32_t num_kv_tiles;             /* key tiles it streams (sum over entries of ceil(len / tile_k)) */
+    int32_t group;                    /* PER_GROUP: index of its query group; PACKED: -1 */
 } aj_task;
 
 typedef struct aj_schedule aj_schedule; /* host-only: groups, merged ranges, ordered task list */
@@ -104,6 +116,9 @@ typedef struct aj_plan aj_plan;         /* schedule + its device copy + staging 
  * group, tile).  tile_q, tile_k > 0.  *out is owned by the caller (attn_jvp_schedule_destroy). */
 aj_status attn_jvp_schedule_create(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
                                    int32_t tile_k, aj_schedule **out);
+/* Same with an explicit aj_tiling (attn_jvp_schedule_create = AJ_TILING_PER_GROUP).  tile_q < 32768. */
+aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
+                                         int32_t tile_k, int32_t tiling, aj_schedule **out);
 aj_status attn_jvp_schedule_destroy(aj_schedule *sched);
 /* Any out pointer may be NULL. unmasked_pairs_per_head = sum over groups of rows * allowed keys. */
 aj_status attn_jvp_schedule_info(const aj_schedule *sched, int32_t *num_groups, int32_t *num_ranges,
@@ -112,6 +127,11 @@ aj_status attn_jvp_schedule_info(const aj_schedule *sched, int32_t *num_groups, 
  * k_begin, k_end [num_ranges]; tasks [num_tasks].  NULL pointers are skipped. */
 aj_status attn_jvp_schedule_get(const aj_schedule *sched, int32_t *q_begin, int32_t *q_end,
                                 int32_t *range_offset, int32_t *k_begin, int32_t *k_end, aj_task *tasks);
+
+/* Copy out the entries the tasks index: k_begin, k_end, row_begin, row_end [num_entries].  NULL pointers are
+ * skipped (call once with only num_entries to size the arrays). */
+aj_status attn_jvp_schedule_entries(const aj_schedule *sched, int32_t *num_entries, int32_t *k_begin,
+                                    int32_t *k_end, int32_t *row_begin, int32_t *row_end);
 
 /* ---- Plans and the forward call ---- */
 
@@ -123,6 +143,9 @@ aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_he
 /* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
  * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged. */
 aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
+/* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernel, PER_GROUP for the SIMT kernel (which
+ * supports nothing else: AJ_ERR_UNSUPPORTED).  Rebuilds and re-uploads the schedule; results do not change. */
+aj_status attn_jvp_plan_set_tiling(aj_plan *plan, int32_t tiling);
 /* Which kernel attn_jvp_fwd will launch (aj_kernel, never AUTO) and how many kernel launches one
  * attn_jvp_fwd call makes. */
 aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *launches_per_call);

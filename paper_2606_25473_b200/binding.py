@@ -16,6 +16,7 @@ AJ_OK, AJ_ERR_INVALID_ARG, AJ_ERR_UNSUPPORTED, AJ_ERR_CUDA, AJ_ERR_OOM = 0, -1, 
 AJ_BF16, AJ_FP32 = 0, 1
 AJ_MASK_FULL, AJ_MASK_BLOCK_CAUSAL, AJ_MASK_TEACHER_FORCING, AJ_MASK_RANGES = 0, 1, 2, 3
 AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA = 0, 1, 2
+AJ_TILING_PER_GROUP, AJ_TILING_PACKED = 0, 1
 
 _I32P = ctypes.POINTER(ctypes.c_int32)
 
@@ -51,8 +52,8 @@ class AttnJvpError(RuntimeError):
 
 # Every symbol include/attn_jvp.h declares (tests check that the library exports all of them).
 SYMBOLS = [
-    "attn_jvp_schedule_create", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get",
-    "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel",
+    "attn_jvp_schedule_create", "attn_jvp_schedule_create_tiled", "attn_jvp_schedule_entries", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get",
+    "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
 ]
 
@@ -69,6 +70,8 @@ def lib():
         l = ctypes.CDLL(LIB_PATH)
         vp, i32, i64p = ctypes.c_void_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int64)
         l.attn_jvp_schedule_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
+        l.attn_jvp_schedule_create_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
+        l.attn_jvp_schedule_entries.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P]
         l.attn_jvp_schedule_destroy.argtypes = [vp]
         l.attn_jvp_schedule_info.argtypes = [vp, _I32P, _I32P, _I32P, i64p]
         l.attn_jvp_schedule_get.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P, ctypes.POINTER(aj_task)]
@@ -76,6 +79,7 @@ def lib():
         l.attn_jvp_plan_destroy.argtypes = [vp]
         l.attn_jvp_plan_info.argtypes = [vp, i64p, _I32P]
         l.attn_jvp_plan_set_kernel.argtypes = [vp, i32]
+        l.attn_jvp_plan_set_tiling.argtypes = [vp, i32]
         l.attn_jvp_plan_kernel.argtypes = [vp, _I32P, _I32P]
         l.attn_jvp_plan_device_status.argtypes = [vp, _I32P]
         l.attn_jvp_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp]
@@ -139,6 +143,21 @@ def attn_jvp_schedule_create(problem: aj_problem, mask: aj_mask_desc, tile_q: in
     return out
 
 
+def attn_jvp_schedule_create_tiled(problem: aj_problem, mask: aj_mask_desc, tile_q: int, tile_k: int, tiling: int) -> ctypes.c_void_p:
+    out = ctypes.c_void_p()
+    _check(lib().attn_jvp_schedule_create_tiled(ctypes.byref(problem), ctypes.byref(mask), tile_q, tile_k, tiling, ctypes.byref(out)))
+    return out
+
+
+def attn_jvp_schedule_entries(sched):
+    """-> dict(k_begin, k_end, row_begin, row_end: lists), the entries aj_task.range_begin / range_count index"""
+    n = ctypes.c_int32()
+    _check(lib().attn_jvp_schedule_entries(sched, ctypes.byref(n), None, None, None, None))
+    arrs = [(ctypes.c_int32 * max(n.value, 1))() for _ in range(4)]
+    _check(lib().attn_jvp_schedule_entries(sched, ctypes.byref(n), *arrs))
+    return dict(zip(("k_begin", "k_end", "row_begin", "row_end"), (list(a)[:n.value] for a in arrs)))
+
+
 def attn_jvp_schedule_destroy(sched) -> None:
     _check(lib().attn_jvp_schedule_destroy(sched))
 
@@ -182,6 +201,10 @@ def attn_jvp_plan_info(plan):
 
 def attn_jvp_plan_set_kernel(plan, kernel: int) -> None:
     _check(lib().attn_jvp_plan_set_kernel(plan, kernel))
+
+
+def attn_jvp_plan_set_tiling(plan, tiling: int) -> None:
+    _check(lib().attn_jvp_plan_set_tiling(plan, tiling))
 
 
 def attn_jvp_plan_kernel(plan):

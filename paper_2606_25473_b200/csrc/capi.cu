@@ -16,12 +16,14 @@ struct aj_plan {
     aj_mask_desc mask;        // arrays below back the pointers for AJ_MASK_RANGES
     std::vector<int32_t> m_qb, m_qe, m_off, m_kb, m_ke;
     int32_t kernel = AJ_KERNEL_SIMT;
+    int32_t tiling = AJ_TILING_PER_GROUP;
     aj_schedule *sched = nullptr;
     int32_t num_tasks = 0;
     int device = 0, num_sms = 0;
     // device copies of the schedule
     aj_task *d_tasks = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr, *d_counters = nullptr;
+    uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
     // staging for attn_jvp_fwd_host
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void *d_out[2] = {nullptr, nullptr};
@@ -54,38 +56,46 @@ aj_status cuda_fail(cudaError_t e, const char *what) {
 }
 
 void free_device(aj_plan *p) {
-    cudaFree(p->d_tasks); cudaFree(p->d_kb); cudaFree(p->d_ke);
-    p->d_tasks = nullptr; p->d_kb = p->d_ke = nullptr;
+    cudaFree(p->d_tasks); cudaFree(p->d_kb); cudaFree(p->d_ke); cudaFree(p->d_rows);
+    p->d_tasks = nullptr; p->d_kb = p->d_ke = nullptr; p->d_rows = nullptr;
 }
 
 bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
 
-// (Re)build the schedule for `kernel` and upload it.
-aj_status install_schedule(aj_plan *p, int32_t kernel) {
+// The tcgen05 kernel tiles queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
+int32_t default_tiling(int32_t kernel) { return kernel == AJ_KERNEL_UMMA ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
+
+// (Re)build the schedule for `kernel` / `tiling` and upload it.
+aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     const int tq = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
     const int tk = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+    if (kernel == AJ_KERNEL_SIMT && tiling != AJ_TILING_PER_GROUP)
+        return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
     aj_schedule *s = nullptr;
-    if (aj_status st = attn_jvp_schedule_create(&p->problem, &p->mask, tq, tk, &s)) return st;
-    const size_t nt = s->tasks.size(), nr = s->low.ranges.size();
-    std::vector<int32_t> kb(nr), ke(nr);
-    for (size_t r = 0; r < nr; ++r) { kb[r] = s->low.ranges[r].k_begin; ke[r] = s->low.ranges[r].k_end; }
+    if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, tq, tk, tiling, &s)) return st;
+    const size_t nt = s->tasks.size(), nr = s->entries.size();
+    std::vector<uint32_t> rows(nr);
+    for (size_t r = 0; r < nr; ++r) rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16);
     aj_task *d_tasks = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr;
+    uint32_t *d_rows = nullptr;
     cudaError_t e = cudaMalloc(&d_tasks, std::max<size_t>(nt, 1) * sizeof(aj_task));
     if (e == cudaSuccess) e = cudaMalloc(&d_kb, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_ke, std::max<size_t>(nr, 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&d_rows, std::max<size_t>(nr, 1) * sizeof(uint32_t));
     if (e == cudaSuccess && nt) e = cudaMemcpy(d_tasks, s->tasks.data(), nt * sizeof(aj_task), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && nr) e = cudaMemcpy(d_kb, kb.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && nr) e = cudaMemcpy(d_ke, ke.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nr) e = cudaMemcpy(d_kb, s->entries.k_begin.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nr) e = cudaMemcpy(d_ke, s->entries.k_end.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nr) e = cudaMemcpy(d_rows, rows.data(), nr * sizeof(uint32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
-        cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke);
+        cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke); cudaFree(d_rows);
         attn_jvp_schedule_destroy(s);
         return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
     }
     free_device(p);
     attn_jvp_schedule_destroy(p->sched);
-    p->sched = s; p->kernel = kernel; p->num_tasks = (int32_t)nt;
-    p->d_tasks = d_tasks; p->d_kb = d_kb; p->d_ke = d_ke;
+    p->sched = s; p->kernel = kernel; p->tiling = tiling; p->num_tasks = (int32_t)nt;
+    p->d_tasks = d_tasks; p->d_kb = d_kb; p->d_ke = d_ke; p->d_rows = d_rows;
     return AJ_OK;
 }
 
@@ -148,7 +158,8 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         e = cudaMalloc(&p->d_counters, 4 * sizeof(int32_t));
         if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
-        st = install_schedule(p, umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT);
+        const int32_t kernel = umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT;
+        st = install_schedule(p, kernel, default_tiling(kernel));
     } catch (const std::bad_alloc &) {
         st = fail(AJ_ERR_OOM, "out of host memory");
     }
@@ -182,7 +193,14 @@ aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
     if (kernel != AJ_KERNEL_SIMT && kernel != AJ_KERNEL_UMMA) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
     if (kernel == AJ_KERNEL_UMMA && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernel needs bf16 and d = 128");
     if (kernel == p->kernel) return AJ_OK;
-    return install_schedule(p, kernel);
+    return install_schedule(p, kernel, default_tiling(kernel));
+}
+
+aj_status attn_jvp_plan_set_tiling(aj_plan *p, int32_t tiling) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (tiling != AJ_TILING_PER_GROUP && tiling != AJ_TILING_PACKED) return fail(AJ_ERR_INVALID_ARG, "unknown tiling");
+    if (tiling == p->tiling) return AJ_OK;
+    return install_schedule(p, p->kernel, tiling);
 }
 
 aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launches) {
@@ -226,7 +244,7 @@ aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k,
         if ((st = encode_map(&prm.tm_v, *v, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
         if ((st = encode_map(&prm.tm_tv, *tv, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
         prm.o = *o; prm.to = *to; prm.lse = lse;
-        prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke; prm.counters = p->d_counters;
+        prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke; prm.rows = p->d_rows; prm.counters = p->d_counters;
         prm.num_tasks = p->num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
         prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
         e = aj::launch_umma(prm, std::min(p->num_sms, p->num_tasks), stream);

@@ -23,15 +23,27 @@ struct Lowered {
     int64_t pairs_per_head = 0;
 };
 
+// What the tasks index (aj_task::range_begin / range_count): key ranges with the rows of the query tile that see them.
+struct Entries {
+    std::vector<int32_t> k_begin, k_end, row_begin, row_end;  // rows relative to the task's q_begin
+    size_t size() const { return k_begin.size(); }
+};
+
 aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out);
-void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k,
+// Per-group tiling: entries = the lowered ranges, every row of a tile sees every entry of its task.
+void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
                  std::vector<aj_task> &tasks);
+// Packed tiling: query tiles on a global grid; a tile that straddles query groups streams the
+// union of their key ranges, each with the interval of its rows that may see it.
+void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
+                        std::vector<aj_task> &tasks);
 
 }  // namespace aj
 
 struct aj_schedule {
     aj_problem problem;
-    int32_t tile_q, tile_k;
+    int32_t tile_q, tile_k, tiling;
     aj::Lowered low;
+    aj::Entries entries;
     std::vector<aj_task> tasks;
 };

@@ -49,6 +49,7 @@ constexpr int NTHREADS = 256;
 
 constexpr uint32_t TM_O = 0, TM_T = 128, TM_S0 = 256, TM_TS0 = 320, TM_SBUF = 128;  // S1 = S0 + 128, ...
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
+constexpr float M_UNSET = -1.0e30f;        // reference max of a row that has not met an unmasked key yet (finite on purpose)
 
 // Barrier indices inside the shared barrier array.
 enum {
@@ -216,7 +217,7 @@ constexpr uint32_t DESC_HI = desc_hi(1024);                // 8-row (K-major) / 
 constexpr uint32_t LBO_K = desc_lo_lbo(16);                // K-major with 128 B swizzle: unused, canonical value
 constexpr uint32_t LBO_V = desc_lo_lbo(KVHALF_BYTES);      // MN-major: 64-column blocks [V h0 | V h1 | tV h0 | tV h1] 8 KB apart
 
-// Walks the key tiles of a task in order: ranges [rb, rb + rc), each cut into BC-key tiles from its start.
+// Walks the key tiles of a task in order: schedule entries [rb, rb + rc), each cut into BC-key tiles from its start.
 struct TileCursor {
     const int32_t *kb, *ke;
     int r, rend, k, kend;
@@ -226,6 +227,7 @@ struct TileCursor {
     }
     __device__ int key_row() const { return k; }
     __device__ int valid() const { return min(BC, kend - k); }
+    __device__ int entry() const { return r; }
     __device__ void next() {
         k += BC;
         if (k >= kend) { ++r; if (r < rend) { k = kb[r]; kend = ke[r]; } }
@@ -420,13 +422,19 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             if (task_id >= prm.num_tasks || sh->abort_flag) break;
             const aj_task task = prm.tasks[task_id];
             const int n = task.num_kv_tiles;
-            float m_ref = 0.f;
+            float m_ref = M_UNSET;
             uint64_t l2[2] = {0ull, 0ull}, r2[2] = {0ull, 0ull};   // 4 partial sums each of l = sum P~ and r = sum H~
             TileCursor cur;
             cur.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
+            int cur_entry = -1, row_lo = 0, row_hi = 0;
             for (int j = 0; j < n; ++j, cur.next()) {
                 const uint32_t gj = g + j, b = gj & 1;
                 const uint32_t tS_ = tmem + lane_base + TM_S0 + b * TM_SBUF, tTS_ = tS_ + (TM_TS0 - TM_S0);
+                if (cur.entry() != cur_entry) {                    // rows of this tile that may see the entry's keys
+                    cur_entry = cur.entry();
+                    const uint32_t rr = prm.rows[cur_entry];
+                    row_lo = (int)(rr & 0xffffu); row_hi = (int)(rr >> 16);
+                }
                 wait(BAR_S_FULL + b, (gj >> 1) & 1);
                 tc_fence_after();
                 uint32_t su[2][32], tu[2][32];
@@ -435,8 +443,9 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 tc_wait_ld(su[0], su[1]);
                 tmem_ld32(tTS_, tu[0]);                            // in flight while P~ is computed
                 tmem_ld32(tTS_ + 32, tu[1]);
-                const int valid = cur.valid();
-                if (valid < BC) {                                 // tile-valid mask: S = -inf
+                // tile-valid mask: S = -inf past the entry's last key and on rows outside its row interval
+                const int valid = (row >= row_lo && row < row_hi) ? cur.valid() : 0;
+                if (valid < BC) {
 #pragma unroll
                     for (int c = 0; c < BC; ++c) if (c >= valid) su[c >> 5][c & 31] = 0xff800000u;
                 }
@@ -446,16 +455,17 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
 #pragma unroll
                 for (int c = 4; c < BC; ++c) mx[c & 3] = fmaxf(mx[c & 3], __uint_as_float(su[c >> 5][c & 31]));
                 const float cand = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * sl2;
-                if (j == 0) {
-                    m_ref = cand;
-                } else {
+                {
+                    // Lazy reference max (PAPER.md:922-927 applied only when needed).  A row whose reference is still
+                    // unset has O = T = l = r = 0 exactly, so it adopts the tile max with nothing to rescale.
                     const bool need = cand > m_ref + RESCALE_THRESHOLD;
-                    if (__any_sync(0xffffffffu, need)) {
-                        // e^{m - m_new} applied to O, T (= A + B), l, r (PAPER.md:922-927); needs PV(j-1) finished
+                    const bool fresh = m_ref == M_UNSET;
+                    if (__any_sync(0xffffffffu, need && !fresh)) {
+                        // e^{m - m_new} applied to O, T (= A + B), l, r; needs PV(j-1) finished
                         const uint32_t gp = gj - 1;
                         wait(BAR_PV_DONE + (gp & 1), (gp >> 1) & 1);
                         tc_fence_after();
-                        const float f = need ? ex2(m_ref - cand) : 1.f;
+                        const float f = (need && !fresh) ? ex2(m_ref - cand) : 1.f;
 #pragma unroll 1
                         for (int cb = 0; cb < 256; cb += 32) {
                             uint32_t a[32];
@@ -468,8 +478,8 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                         const uint64_t f2 = pack2(f, f);
                         l2[0] = fmul2(l2[0], f2); l2[1] = fmul2(l2[1], f2);
                         r2[0] = fmul2(r2[0], f2); r2[1] = fmul2(r2[1], f2);
-                        if (need) m_ref = cand;
                     }
+                    if (need) m_ref = cand;
                 }
                 // P~ = exp2(S*s*log2e - m_ref); l += rowsum
                 const uint64_t negm2 = pack2(-m_ref, -m_ref);
@@ -531,7 +541,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             unpack2(l2[0], la, lb); unpack2(l2[1], lc, ld);
             unpack2(r2[0], ra, rb); unpack2(r2[1], rc, rd);
             const float l = (la + lb) + (lc + ld), r = (ra + rb) + (rc + rd);
-            const float inv = 1.f / l, rl = r * inv;
+            const float inv = l > 0.f ? 1.f / l : 0.f, rl = r * inv;   // l = 0: the row saw no key (O = 0, tO = 0, lse = -inf)
 #pragma unroll 1
             for (int cb = 0; cb < D; cb += 32) {
                 uint32_t ao[32], at[32];
@@ -557,7 +567,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 }
             }
             if (store && prm.lse)
-                prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = (m_ref + log2f(l)) * 0.6931471805599453f;
+                prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = l > 0.f ? (m_ref + log2f(l)) * 0.6931471805599453f : -INFINITY;
             tc_fence_before();
             g += n;
         }

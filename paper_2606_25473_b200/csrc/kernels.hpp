@@ -30,8 +30,9 @@ struct UmmaParams {
     aj_tensor o, to;
     float *lse;
     const aj_task *tasks;
-    const int32_t *k_begin, *k_end;
-    int32_t *counters;          // [0] next task, [1] CTAs finished (both 0 between launches)
+    const int32_t *k_begin, *k_end;   // schedule entries: keys [k_begin[e], k_end[e]) ...
+    const uint32_t *rows;             // ... seen by tile rows [rows[e] & 0xffff, rows[e] >> 16)
+    int32_t *counters;          // [0] next task, [1] CTAs finished (both 0 between launches), [2] abort code
     int32_t num_tasks, H, Nq;
     float scale_log2;           // s * log2(e)
     float scale;                // s

@@ -129,9 +129,21 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
     return AJ_OK;
 }
 
-void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k,
+static void order_tasks(std::vector<aj_task> &tasks) {
+    // Longest-first so that the persistent CTAs finish together; ties keep (b, h, group/tile) order so that
+    // tasks streaming the same keys of the same head run at the same time and share them in L2.
+    std::stable_sort(tasks.begin(), tasks.end(),
+                     [](const aj_task &x, const aj_task &y) { return x.num_kv_tiles > y.num_kv_tiles; });
+}
+
+void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
                  std::vector<aj_task> &tasks) {
     tasks.clear();
+    ent = Entries();
+    for (const KeyRange &r : low.ranges) {
+        ent.k_begin.push_back(r.k_begin); ent.k_end.push_back(r.k_end);
+        ent.row_begin.push_back(0); ent.row_end.push_back(tile_q);
+    }
     for (int32_t b = 0; b < p.B; ++b)
         for (int32_t h = 0; h < p.H; ++h)
             for (size_t g = 0; g < low.q_begin.size(); ++g) {
@@ -149,10 +161,86 @@ void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_
                     tasks.push_back(t);
                 }
             }
-    // Longest-first so that the persistent CTAs finish together; ties keep (b, h, group, tile) order so that
-    // tasks streaming the same keys of the same head run at the same time and share them in L2.
-    std::stable_sort(tasks.begin(), tasks.end(),
-                     [](const aj_task &x, const aj_task &y) { return x.num_kv_tiles > y.num_kv_tiles; });
+    order_tasks(tasks);
+}
+
+void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
+                        std::vector<aj_task> &tasks) {
+    tasks.clear();
+    ent = Entries();
+    const size_t ng = low.q_begin.size();
+    std::vector<size_t> order(ng);                     // groups in row order (they are disjoint)
+    for (size_t g = 0; g < ng; ++g) order[g] = g;
+    std::sort(order.begin(), order.end(), [&](size_t a, size_t b) { return low.q_begin[a] < low.q_begin[b]; });
+    struct Run { int32_t lo, hi; };
+    struct TileInfo { int32_t q_begin, q_rows, ent_begin, ent_count, kv_tiles; };
+    std::vector<TileInfo> tiles;
+    size_t first = 0;                                  // first group (in row order) that may reach this tile
+    std::vector<int32_t> cuts;
+    std::vector<Run> runs, prev_runs;
+    for (int32_t t0 = 0; t0 < p.Nq; t0 += tile_q) {
+        const int32_t t1 = std::min(p.Nq, t0 + tile_q);
+        while (first < ng && low.q_end[order[first]] <= t0) ++first;
+        size_t last = first;                           // groups [first, last) intersect rows [t0, t1)
+        while (last < ng && low.q_begin[order[last]] < t1) ++last;
+        cuts.clear();
+        for (size_t i = first; i < last; ++i) {
+            const size_t g = order[i];
+            for (int r = low.range_offset[g]; r < low.range_offset[g + 1]; ++r) {
+                cuts.push_back(low.ranges[r].k_begin);
+                cuts.push_back(low.ranges[r].k_end);
+            }
+        }
+        std::sort(cuts.begin(), cuts.end());
+        cuts.erase(std::unique(cuts.begin(), cuts.end()), cuts.end());
+        TileInfo ti{t0, t1 - t0, (int32_t)ent.size(), 0, 0};
+        size_t open_begin = ent.size();                // entries of the key interval being extended
+        prev_runs.clear();
+        int32_t prev_end = -1;
+        for (size_t c = 0; c + 1 < cuts.size(); ++c) {
+            const int32_t a = cuts[c], bnd = cuts[c + 1];
+            // rows of the tile that see keys [a, bnd): union over the groups whose ranges cover it, as maximal runs
+            runs.clear();
+            for (size_t i = first; i < last; ++i) {
+                const size_t g = order[i];
+                bool covered = false;
+                for (int r = low.range_offset[g]; r < low.range_offset[g + 1] && !covered; ++r)
+                    covered = low.ranges[r].k_begin <= a && bnd <= low.ranges[r].k_end;
+                if (!covered) continue;
+                const int32_t lo = std::max(low.q_begin[g], t0) - t0, hi = std::min(low.q_end[g], t1) - t0;
+                if (!runs.empty() && runs.back().hi == lo) runs.back().hi = hi;
+                else runs.push_back(Run{lo, hi});
+            }
+            if (runs.empty()) { prev_runs.clear(); prev_end = -1; continue; }
+            bool same = prev_end == a && runs.size() == prev_runs.size();
+            for (size_t i = 0; same && i < runs.size(); ++i) same = runs[i].lo == prev_runs[i].lo && runs[i].hi == prev_runs[i].hi;
+            if (same) {                                // same rows as the interval before and adjacent keys: extend
+                for (size_t e = open_begin; e < ent.size(); ++e) ent.k_end[e] = bnd;
+            } else {
+                open_begin = ent.size();
+                for (const Run &r : runs) {
+                    ent.k_begin.push_back(a); ent.k_end.push_back(bnd);
+                    ent.row_begin.push_back(r.lo); ent.row_end.push_back(r.hi);
+                }
+            }
+            prev_runs = runs;
+            prev_end = bnd;
+        }
+        ti.ent_count = (int32_t)ent.size() - ti.ent_begin;
+        for (int32_t e = ti.ent_begin; e < ti.ent_begin + ti.ent_count; ++e)
+            ti.kv_tiles += (ent.k_end[e] - ent.k_begin[e] + tile_k - 1) / tile_k;
+        tiles.push_back(ti);
+    }
+    for (int32_t b = 0; b < p.B; ++b)
+        for (int32_t h = 0; h < p.H; ++h)
+            for (const TileInfo &ti : tiles) {
+                aj_task t;
+                t.b = b; t.h = h; t.q_begin = ti.q_begin; t.q_rows = ti.q_rows;
+                t.range_begin = ti.ent_begin; t.range_count = ti.ent_count;
+                t.num_kv_tiles = ti.kv_tiles; t.group = -1;
+                tasks.push_back(t);
+            }
+    order_tasks(tasks);
 }
 
 }  // namespace aj
@@ -174,18 +262,26 @@ extern "C" {
 
 aj_status attn_jvp_schedule_create(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
                                    int32_t tile_k, aj_schedule **out) {
+    return attn_jvp_schedule_create_tiled(problem, mask, tile_q, tile_k, AJ_TILING_PER_GROUP, out);
+}
+
+aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
+                                         int32_t tile_k, int32_t tiling, aj_schedule **out) {
     if (!out) return aj::fail(AJ_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
     if (aj_status st = aj::check_problem(problem)) return st;
     if (!mask) return aj::fail(AJ_ERR_INVALID_ARG, "mask is NULL");
     if (tile_q <= 0 || tile_k <= 0) return aj::fail(AJ_ERR_INVALID_ARG, "tile_q and tile_k must be > 0");
+    if (tiling != AJ_TILING_PER_GROUP && tiling != AJ_TILING_PACKED) return aj::fail(AJ_ERR_INVALID_ARG, "unknown tiling");
+    if (tile_q > 32767) return aj::fail(AJ_ERR_INVALID_ARG, "tile_q must be < 32768");
     aj_schedule *s = new (std::nothrow) aj_schedule();
     if (!s) return aj::fail(AJ_ERR_OOM, "out of host memory");
     try {
-        s->problem = *problem; s->tile_q = tile_q; s->tile_k = tile_k;
+        s->problem = *problem; s->tile_q = tile_q; s->tile_k = tile_k; s->tiling = tiling;
         aj_status st = aj::lower_mask(*problem, *mask, s->low);
         if (st != AJ_OK) { delete s; return st; }
-        aj::build_tasks(*problem, s->low, tile_q, tile_k, s->tasks);
+        if (tiling == AJ_TILING_PACKED) aj::build_tasks_packed(*problem, s->low, tile_q, tile_k, s->entries, s->tasks);
+        else aj::build_tasks(*problem, s->low, tile_q, tile_k, s->entries, s->tasks);
     } catch (const std::bad_alloc &) {
         delete s;
         return aj::fail(AJ_ERR_OOM, "out of host memory");
@@ -221,6 +317,18 @@ aj_status attn_jvp_schedule_get(const aj_schedule *s, int32_t *q_begin, int32_t 
         if (k_end) k_end[r] = l.ranges[r].k_end;
     }
     if (tasks) std::copy(s->tasks.begin(), s->tasks.end(), tasks);
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_entries(const aj_schedule *s, int32_t *num_entries, int32_t *k_begin, int32_t *k_end,
+                                    int32_t *row_begin, int32_t *row_end) {
+    if (!s) return aj::fail(AJ_ERR_INVALID_ARG, "schedule is NULL");
+    const aj::Entries &e = s->entries;
+    if (num_entries) *num_entries = (int32_t)e.size();
+    if (k_begin) std::copy(e.k_begin.begin(), e.k_begin.end(), k_begin);
+    if (k_end) std::copy(e.k_end.begin(), e.k_end.end(), k_end);
+    if (row_begin) std::copy(e.row_begin.begin(), e.row_begin.end(), row_begin);
+    if (row_end) std::copy(e.row_end.begin(), e.row_end.end(), row_end);
     return AJ_OK;
 }
 

@@ -79,6 +79,24 @@ def test_umma_small_every_row(w):
         assert torch.equal(a, b)
 
 
+@pytest.mark.parametrize("w", SMALL_UMMA[:4] + SMALL_UMMA[6:], ids=lambda w: w.name)
+def test_umma_per_group_and_packed_tilings_agree(w):
+    # PACKED (default: global 128-row grid, straddling tiles carry row intervals) vs PER_GROUP
+    x = make_inputs(w)
+    ref = run_oracle(w, x)
+    plan = make_plan(w)
+    packed = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_set_tiling(plan, aj.AJ_TILING_PER_GROUP)
+    per_group = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_set_tiling(plan, aj.AJ_TILING_PACKED)
+    packed2 = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    compare(w, packed, ref)
+    compare(w, per_group, ref)
+    for a, b in zip(packed, packed2):
+        assert torch.equal(a, b)
+
+
 def test_umma_large_unit_variance_tangents():
     # tangents as large as the primals, peaked scores (|s| up to ~4*sqrt(d)/sqrt(d)): exercises the lazy rescale
     w = Workload("tf_peaked", 1, 2, 128, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=11)

@@ -193,3 +193,76 @@ def test_plan_create_without_gpu_fails_loudly():
     tf, _ = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 16, 3, 1)
     _expect(aj.AJ_ERR_CUDA, aj.attn_jvp_plan_create, aj.make_problem(1, 1, 96, 96, 64, aj.AJ_FP32), tf)
     _expect(aj.AJ_ERR_UNSUPPORTED, aj.attn_jvp_plan_create, aj.make_problem(1, 1, 96, 96, 32, aj.AJ_FP32), tf)
+
+
+# ---------------------------------------------------------------------------------------------- packed tiling
+def _packed(prob, mask, tile_q, tile_k):
+    s = aj.attn_jvp_schedule_create_tiled(prob, mask, tile_q, tile_k, aj.AJ_TILING_PACKED)
+    info = aj.attn_jvp_schedule_info(s)
+    got = aj.attn_jvp_schedule_get(s)
+    ent = aj.attn_jvp_schedule_entries(s)
+    aj.attn_jvp_schedule_destroy(s)
+    return info, got, ent
+
+
+def _check_packed(want, Nq, info, got, ent, tile_q, tile_k, heads=1):
+    """Every unmasked pair is covered by exactly one (entry, row interval) of exactly one task; no masked pair."""
+    cover = np.zeros(want.shape, dtype=np.int32)
+    rows_seen = np.zeros(Nq, dtype=np.int32)
+    for t in got["tasks"]:
+        if (t.b, t.h) != (0, 0):
+            continue
+        assert t.group == -1 and t.q_begin % tile_q == 0 and t.q_rows == min(tile_q, Nq - t.q_begin)
+        tiles = 0
+        for e in range(t.range_begin, t.range_begin + t.range_count):
+            k0, k1, r0, r1 = ent["k_begin"][e], ent["k_end"][e], ent["row_begin"][e], ent["row_end"][e]
+            assert 0 <= r0 < r1 <= t.q_rows and k0 < k1
+            cover[t.q_begin + r0:t.q_begin + r1, k0:k1] += 1
+            tiles += -(-(k1 - k0) // tile_k)
+        assert tiles == t.num_kv_tiles
+        rows_seen[t.q_begin:t.q_begin + t.q_rows] += 1
+    assert np.array_equal(cover, want.astype(np.int32))
+    assert np.all(rows_seen == 1)
+    assert info[3] == int(want.sum())
+    assert len(got["tasks"]) == heads * -(-Nq // tile_q)
+    kv = [t.num_kv_tiles for t in got["tasks"]]
+    assert kv == sorted(kv, reverse=True)
+
+
+@pytest.mark.parametrize("mask,L,F,cf", [
+    ("teacher_forcing", 16, 3, 1), ("teacher_forcing", 10, 6, 3), ("teacher_forcing", 7, 4, 2),
+    ("block_causal", 16, 3, 1), ("block_causal", 9, 6, 2), ("full", 13, 5, 1), ("teacher_forcing", 3, 5, 1)])
+@pytest.mark.parametrize("tile_q,tile_k", [(16, 32), (8, 4), (128, 64), (5, 3)])
+def test_packed_tiles_cover_the_mask_exactly_once(oracle, mask, L, F, cf, tile_q, tile_k):
+    w = Workload("t", 1, 2, 64, mask, L, F, cf, "fp32", 1.0)
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_FP32)
+    kind = {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL, "full": aj.AJ_MASK_FULL}[mask]
+    m, keep = aj.make_mask(kind, L, F, cf)
+    info, got, ent = _packed(prob, m, tile_q, tile_k)
+    want = oracle.dense_mask(oracle_mask(w), w.N, w.N)
+    _check_packed(want, w.N, info, got, ent, tile_q, tile_k, heads=2)
+
+
+def test_packed_generic_ranges_with_gaps_and_split_row_runs(oracle):
+    # groups 0 and 2 share keys (30,40) but group 1 between them does not: rows that see them are not one interval
+    groups = [(4, 9, [(0, 5), (5, 9), (30, 40)]), (9, 13, [(2, 3)]), (13, 20, [(30, 40), (44, 48)]), (33, 40, [])]
+    prob = aj.make_problem(1, 1, 40, 48, 64, aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+    want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
+    for tile_q, tile_k in [(8, 4), (16, 8), (64, 64), (3, 5)]:
+        info, got, ent = _packed(prob, mask, tile_q, tile_k)
+        _check_packed(want, 40, info, got, ent, tile_q, tile_k)
+
+
+def test_packed_tiling_wastes_fewer_tile_rows_on_config_2():
+    w = WORKLOADS["wan13b_tf_framewise"]
+    prob = aj.make_problem(1, 1, w.N, w.N, w.d, aj.AJ_BF16)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, w.frame_len, w.num_frames, w.chunk_frames)
+    per_group = aj.attn_jvp_schedule_create(prob, m, 128, 64)
+    pg = aj.attn_jvp_schedule_get(per_group)
+    aj.attn_jvp_schedule_destroy(per_group)
+    info, got, ent = _packed(prob, m, 128, 64)
+    area = lambda tasks: sum(t.num_kv_tiles for t in tasks) * 128 * 64
+    eff_pg, eff_pk = w.unmasked_pairs_per_head / area(pg["tasks"]), w.unmasked_pairs_per_head / area(got["tasks"])
+    assert 0.93 < eff_pg < 0.94 and eff_pk > 0.975, (eff_pg, eff_pk)
+    assert len(got["tasks"]) == 512            # 65520 rows / 128
