@@ -48,8 +48,10 @@ typedef enum {
     AJ_MASK_RANGES = 3           /* explicit query groups with key-range lists                            */
 } aj_mask_kind;
 
-/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA when (bf16, d = 128), else SIMT. */
-typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2 } aj_kernel;
+/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA when (bf16, d = 128), else SIMT.
+ * UMMA: one CTA per 128-row query tile (tcgen05.mma.cta_group::1).  UMMA_PAIR: a CTA pair per 256-row query tile
+ * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile). */
+typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2, AJ_KERNEL_UMMA_PAIR = 3 } aj_kernel;
 
 /*
  * Mask descriptor = the paper's problem statement.  Structured kinds: a block is

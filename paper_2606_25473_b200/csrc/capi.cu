@@ -24,6 +24,8 @@ struct aj_plan {
     aj_task *d_tasks = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr, *d_counters = nullptr;
     uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
+    int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
+    int32_t num_pairs = 0;
     // staging for attn_jvp_fwd_host
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void *d_out[2] = {nullptr, nullptr};
@@ -57,18 +59,45 @@ aj_status cuda_fail(cudaError_t e, const char *what) {
 
 void free_device(aj_plan *p) {
     cudaFree(p->d_tasks); cudaFree(p->d_kb); cudaFree(p->d_ke); cudaFree(p->d_rows);
+    cudaFree(p->d_pair_off); cudaFree(p->d_pair_ids);
     p->d_tasks = nullptr; p->d_kb = p->d_ke = nullptr; p->d_rows = nullptr;
+    p->d_pair_off = p->d_pair_ids = nullptr; p->num_pairs = 0;
 }
 
 bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
 
-// The tcgen05 kernel tiles queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
-int32_t default_tiling(int32_t kernel) { return kernel == AJ_KERNEL_UMMA ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
+bool is_umma(int32_t kernel) { return kernel == AJ_KERNEL_UMMA || kernel == AJ_KERNEL_UMMA_PAIR; }
+int32_t auto_kernel(const aj_problem &p) { return umma_covers(p) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT; }
+
+// The tcgen05 kernels tile queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
+int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
+
+// Longest-processing-time-first assignment of the (already longest-first) tasks to `num_pairs` CTA pairs: every task
+// goes to the pair with the least work so far, so the pairs finish within one shortest task of each other.  A task's
+// cost is its pair-steps (two key tiles each) plus a constant for its Q load and epilogue.
+void assign_pairs(const std::vector<aj_task> &tasks, int num_pairs, std::vector<int32_t> &off, std::vector<int32_t> &ids) {
+    std::vector<std::vector<int32_t>> lists(num_pairs);
+    std::vector<std::pair<int64_t, int>> heap;            // (-load, -pair): max-heap picks the least loaded, lowest pair
+    for (int i = 0; i < num_pairs; ++i) heap.emplace_back(0, -i);
+    std::make_heap(heap.begin(), heap.end());
+    for (size_t t = 0; t < tasks.size(); ++t) {
+        std::pop_heap(heap.begin(), heap.end());
+        auto &top = heap.back();
+        lists[-top.second].push_back((int32_t)t);
+        top.first -= (tasks[t].num_kv_tiles + 1) / 2 + 1;
+        std::push_heap(heap.begin(), heap.end());
+    }
+    off.assign(1, 0);
+    ids.clear();
+    for (const auto &l : lists) { ids.insert(ids.end(), l.begin(), l.end()); off.push_back((int32_t)ids.size()); }
+}
 
 // (Re)build the schedule for `kernel` / `tiling` and upload it.
 aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
-    const int tq = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
-    const int tk = kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+    const int tq = kernel == AJ_KERNEL_UMMA_PAIR ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
+    const int tk = is_umma(kernel) ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+    if (kernel == AJ_KERNEL_UMMA_PAIR && tiling != AJ_TILING_PACKED)
+        return fail(AJ_ERR_UNSUPPORTED, "the CTA-pair tcgen05 kernel only supports packed tiling");
     if (kernel == AJ_KERNEL_SIMT && tiling != AJ_TILING_PER_GROUP)
         return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
     aj_schedule *s = nullptr;
@@ -76,10 +105,20 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r) rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16);
+    std::vector<int32_t> pair_off, pair_ids;
+    int num_pairs = 0;
+    if (kernel == AJ_KERNEL_UMMA_PAIR) {
+        num_pairs = (int)std::min<size_t>(std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
+        assign_pairs(s->tasks, num_pairs, pair_off, pair_ids);
+    }
     aj_task *d_tasks = nullptr;
-    int32_t *d_kb = nullptr, *d_ke = nullptr;
+    int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr;
     uint32_t *d_rows = nullptr;
     cudaError_t e = cudaMalloc(&d_tasks, std::max<size_t>(nt, 1) * sizeof(aj_task));
+    if (e == cudaSuccess && num_pairs) e = cudaMalloc(&d_pair_off, pair_off.size() * sizeof(int32_t));
+    if (e == cudaSuccess && num_pairs) e = cudaMalloc(&d_pair_ids, std::max<size_t>(pair_ids.size(), 1) * sizeof(int32_t));
+    if (e == cudaSuccess && num_pairs) e = cudaMemcpy(d_pair_off, pair_off.data(), pair_off.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && num_pairs && !pair_ids.empty()) e = cudaMemcpy(d_pair_ids, pair_ids.data(), pair_ids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&d_kb, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_ke, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_rows, std::max<size_t>(nr, 1) * sizeof(uint32_t));
@@ -88,7 +127,7 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     if (e == cudaSuccess && nr) e = cudaMemcpy(d_ke, s->entries.k_end.data(), nr * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && nr) e = cudaMemcpy(d_rows, rows.data(), nr * sizeof(uint32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
-        cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke); cudaFree(d_rows);
+        cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke); cudaFree(d_rows); cudaFree(d_pair_off); cudaFree(d_pair_ids);
         attn_jvp_schedule_destroy(s);
         return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
     }
@@ -96,6 +135,7 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     attn_jvp_schedule_destroy(p->sched);
     p->sched = s; p->kernel = kernel; p->tiling = tiling; p->num_tasks = (int32_t)nt;
     p->d_tasks = d_tasks; p->d_kb = d_kb; p->d_ke = d_ke; p->d_rows = d_rows;
+    p->d_pair_off = d_pair_off; p->d_pair_ids = d_pair_ids; p->num_pairs = num_pairs;
     return AJ_OK;
 }
 
@@ -158,7 +198,7 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         e = cudaMalloc(&p->d_counters, 4 * sizeof(int32_t));
         if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
-        const int32_t kernel = umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT;
+        const int32_t kernel = auto_kernel(p->problem);
         st = install_schedule(p, kernel, default_tiling(kernel));
     } catch (const std::bad_alloc &) {
         st = fail(AJ_ERR_OOM, "out of host memory");
@@ -189,9 +229,9 @@ aj_status attn_jvp_plan_info(const aj_plan *p, int64_t *pairs, int32_t *num_task
 
 aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
-    if (kernel == AJ_KERNEL_AUTO) kernel = umma_covers(p->problem) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT;
-    if (kernel != AJ_KERNEL_SIMT && kernel != AJ_KERNEL_UMMA) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
-    if (kernel == AJ_KERNEL_UMMA && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernel needs bf16 and d = 128");
+    if (kernel == AJ_KERNEL_AUTO) kernel = auto_kernel(p->problem);
+    if (kernel != AJ_KERNEL_SIMT && !is_umma(kernel)) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
+    if (is_umma(kernel) && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernels need bf16 and d = 128");
     if (kernel == p->kernel) return AJ_OK;
     return install_schedule(p, kernel, default_tiling(kernel));
 }
@@ -233,7 +273,7 @@ aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k,
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (p->num_tasks == 0) return AJ_OK;
     cudaError_t e;
-    if (p->kernel == AJ_KERNEL_UMMA) {
+    if (is_umma(p->kernel)) {
         aj::UmmaParams prm;
         std::memset(&prm, 0, sizeof(prm));
         aj_status st;
@@ -247,7 +287,9 @@ aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k,
         prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke; prm.rows = p->d_rows; prm.counters = p->d_counters;
         prm.num_tasks = p->num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
         prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
-        e = aj::launch_umma(prm, std::min(p->num_sms, p->num_tasks), stream);
+        prm.pair_off = p->d_pair_off; prm.pair_ids = p->d_pair_ids;
+        e = p->kernel == AJ_KERNEL_UMMA_PAIR ? aj::launch_umma_pair(prm, p->num_pairs, stream)
+                                             : aj::launch_umma(prm, std::min(p->num_sms, p->num_tasks), stream);
     } else {
         aj::SimtParams prm;
         prm.q = *q; prm.k = *k; prm.v = *v; prm.tq = *tq; prm.tk = *tk; prm.tv = *tv; prm.o = *o; prm.to = *to;

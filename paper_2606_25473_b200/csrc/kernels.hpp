@@ -11,6 +11,7 @@ constexpr int SIMT_TILE_Q = 16;
 constexpr int SIMT_TILE_K = 32;
 constexpr int UMMA_TILE_Q = 128;  // B_r: query rows per task = UMMA M
 constexpr int UMMA_TILE_K = 64;   // B_c: keys per streamed tile
+constexpr int UMMA_PAIR_TILE_Q = 256;  // query rows per task of the CTA-pair kernel (UMMA M = 256 over two SMs)
 
 struct SimtParams {
     aj_tensor q, k, v, tq, tk, tv, o, to;
@@ -33,6 +34,7 @@ struct UmmaParams {
     const int32_t *k_begin, *k_end;   // schedule entries: keys [k_begin[e], k_end[e]) ...
     const uint32_t *rows;             // ... seen by tile rows [rows[e] & 0xffff, rows[e] >> 16)
     int32_t *counters;          // [0] next task, [1] CTAs finished (both 0 between launches), [2] abort code
+    const int32_t *pair_off, *pair_ids;   // CTA-pair kernel: pair p runs tasks pair_ids[pair_off[p] .. pair_off[p+1])
     int32_t num_tasks, H, Nq;
     float scale_log2;           // s * log2(e)
     float scale;                // s
@@ -40,5 +42,9 @@ struct UmmaParams {
 
 size_t umma_smem_bytes();
 cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream);
+
+// bf16, d = 128, CTA pairs: tcgen05.mma.cta_group::2 with M = 256 (kernel_umma_pair_sm100.cu)
+size_t umma_pair_smem_bytes();
+cudaError_t launch_umma_pair(const UmmaParams &prm, int num_pairs, cudaStream_t stream);
 
 }  // namespace aj
