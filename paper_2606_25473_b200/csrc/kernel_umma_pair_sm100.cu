@@ -72,7 +72,7 @@ constexpr uint32_t LBO_CANON = desc_lo_lbo(16);            // single 64-column b
 __device__ __noinline__ void pair_wait_slow(uint32_t bar, int idx, uint32_t parity, volatile int *abort_flag, int32_t *err) {
     const long long t0 = clock64();
     uint32_t spins = 0;
-    while (!mbar_try_wait_cluster(bar, parity)) {
+    while (!mbar_try_wait(bar, parity)) {
         if ((++spins & 0x3f) == 0) {
             if (*abort_flag) return;
             if (clock64() - t0 > 4000000000LL) {
@@ -90,8 +90,8 @@ struct PairWaiter {
     int32_t *err;
     __device__ __forceinline__ void operator()(int idx, uint32_t parity) const {
         const uint32_t bar = bars + 8u * idx;
-        if (mbar_try_wait_cluster(bar, parity)) return;
-        if (mbar_try_wait_cluster(bar, parity)) return;
+        if (mbar_try_wait(bar, parity)) return;
+        if (mbar_try_wait(bar, parity)) return;
         pair_wait_slow(bar, idx, parity, abort_flag, err);
     }
 };
@@ -338,20 +338,22 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             TileCursor cur;
             cur.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
             const int np = (n + 1) >> 1;
+            int cur_entry = -1;
+            bool sees = false;                                   // this row is inside the current entry's row interval
             for (int p = 0; p < np; ++p, ++gp) {
                 // columns of the two tiles this row may see: inside the entry's keys and row interval
                 int valid[2];
                 {
                     const Tile t0 = cur.get();
                     cur.next();
-                    const uint32_t rr0 = prm.rows[t0.entry];
-                    valid[0] = (prow >= (int)(rr0 & 0xffffu) && prow < (int)(rr0 >> 16)) ? t0.valid : 0;
+                    if (t0.entry != cur_entry) { cur_entry = t0.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)(rr >> 16); }
+                    valid[0] = sees ? t0.valid : 0;
                     valid[1] = 0;
                     if (2 * p + 1 < n) {
                         const Tile t1 = cur.get();
                         cur.next();
-                        const uint32_t rr1 = prm.rows[t1.entry];
-                        valid[1] = (prow >= (int)(rr1 & 0xffffu) && prow < (int)(rr1 >> 16)) ? t1.valid : 0;
+                        if (t1.entry != cur_entry) { cur_entry = t1.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)(rr >> 16); }
+                        valid[1] = sees ? t1.valid : 0;
                     }
                 }
                 wait(BAR_S_FULL, gp & 1);
