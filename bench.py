@@ -317,7 +317,7 @@ def run_cuda(args, w: Workload):
         "ms_per_step": total_ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "config": workload_config(w),
         "tokens_per_s": world * w.B * w.N / (total_ms_all / K * 1e-3),
-        "kernel": {1: "simt_fp32", 2: "tcgen05_umma"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
+        "kernel": {1: "simt_fp32", 2: "tcgen05_umma", 3: "tcgen05_umma_cta_pair"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
         "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
         "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -327,7 +327,7 @@ def run_cuda(args, w: Workload):
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": recorded_traffic(w.name), "peak_source": f"{peak_src} bf16_tflops (burst cuBLAS GEMM)",
                      "frac_of_sustained": achieved / sustained, "frac_of_nominal_2250": achieved / 2250.0,
-                     "kernel": "attn_jvp_umma_kernel" if kernel == 2 else "attn_jvp_simt_kernel",
+                     "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
                      "flops_per_launch": flops},
     }
     if world == 1 and not args.no_cpu_baseline:

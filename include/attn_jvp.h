@@ -48,7 +48,7 @@ typedef enum {
     AJ_MASK_RANGES = 3           /* explicit query groups with key-range lists                            */
 } aj_mask_kind;
 
-/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA when (bf16, d = 128), else SIMT.
+/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA_PAIR when (bf16, d = 128), else SIMT.
  * UMMA: one CTA per 128-row query tile (tcgen05.mma.cta_group::1).  UMMA_PAIR: a CTA pair per 256-row query tile
  * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile). */
 typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2, AJ_KERNEL_UMMA_PAIR = 3 } aj_kernel;
@@ -135,6 +135,14 @@ aj_status attn_jvp_schedule_get(const aj_schedule *sched, int32_t *q_begin, int3
 aj_status attn_jvp_schedule_entries(const aj_schedule *sched, int32_t *num_entries, int32_t *k_begin,
                                     int32_t *k_end, int32_t *row_begin, int32_t *row_end);
 
+/* Static assignment of the tasks to num_workers persistent workers (the CTA-pair kernel's SM pairs; PAPER.md:897
+ * "parallel over tasks"): tasks are taken (b, h)-major, longest first inside a head, and each goes to the worker that
+ * is free first under the cost model ceil(num_kv_tiles / 2) + 1.  worker_offset [num_workers + 1], task_ids
+ * [num_tasks] (indices into the task list of attn_jvp_schedule_get): worker w runs
+ * task_ids[worker_offset[w] .. worker_offset[w+1]) in order.  Every task appears exactly once. */
+aj_status attn_jvp_schedule_assign(const aj_schedule *sched, int32_t num_workers, int32_t *worker_offset,
+                                   int32_t *task_ids);
+
 /* ---- Plans and the forward call ---- */
 
 /* Validates the problem, builds the schedule for the kernel that will run and uploads it (one H2D copy,
@@ -145,8 +153,8 @@ aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_he
 /* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
  * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged. */
 aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
-/* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernel, PER_GROUP for the SIMT kernel (which
- * supports nothing else: AJ_ERR_UNSUPPORTED).  Rebuilds and re-uploads the schedule; results do not change. */
+/* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernels, PER_GROUP for the SIMT kernel; the SIMT
+ * kernel supports only PER_GROUP and the CTA-pair kernel only PACKED (AJ_ERR_UNSUPPORTED otherwise).  Rebuilds and re-uploads the schedule; results do not change. */
 aj_status attn_jvp_plan_set_tiling(aj_plan *plan, int32_t tiling);
 /* Which kernel attn_jvp_fwd will launch (aj_kernel, never AUTO) and how many kernel launches one
  * attn_jvp_fwd call makes. */

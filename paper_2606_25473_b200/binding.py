@@ -52,7 +52,7 @@ class AttnJvpError(RuntimeError):
 
 # Every symbol include/attn_jvp.h declares (tests check that the library exports all of them).
 SYMBOLS = [
-    "attn_jvp_schedule_create", "attn_jvp_schedule_create_tiled", "attn_jvp_schedule_entries", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get",
+    "attn_jvp_schedule_create", "attn_jvp_schedule_create_tiled", "attn_jvp_schedule_entries", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get", "attn_jvp_schedule_assign",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
 ]
@@ -72,6 +72,7 @@ def lib():
         l.attn_jvp_schedule_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_create_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_entries.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P]
+        l.attn_jvp_schedule_assign.argtypes = [vp, i32, _I32P, _I32P]
         l.attn_jvp_schedule_destroy.argtypes = [vp]
         l.attn_jvp_schedule_info.argtypes = [vp, _I32P, _I32P, _I32P, i64p]
         l.attn_jvp_schedule_get.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P, ctypes.POINTER(aj_task)]
@@ -156,6 +157,15 @@ def attn_jvp_schedule_entries(sched):
     arrs = [(ctypes.c_int32 * max(n.value, 1))() for _ in range(4)]
     _check(lib().attn_jvp_schedule_entries(sched, ctypes.byref(n), *arrs))
     return dict(zip(("k_begin", "k_end", "row_begin", "row_end"), (list(a)[:n.value] for a in arrs)))
+
+
+def attn_jvp_schedule_assign(sched, num_workers: int):
+    """-> (worker_offset [num_workers + 1], task_ids [num_tasks]) as lists"""
+    nt = attn_jvp_schedule_info(sched)[2]
+    off = (ctypes.c_int32 * (max(num_workers, 0) + 1))()
+    ids = (ctypes.c_int32 * max(nt, 1))()
+    _check(lib().attn_jvp_schedule_assign(sched, num_workers, off, ids))
+    return list(off), list(ids)[:nt]
 
 
 def attn_jvp_schedule_destroy(sched) -> None:

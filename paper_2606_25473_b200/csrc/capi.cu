@@ -67,30 +67,11 @@ void free_device(aj_plan *p) {
 bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
 
 bool is_umma(int32_t kernel) { return kernel == AJ_KERNEL_UMMA || kernel == AJ_KERNEL_UMMA_PAIR; }
-int32_t auto_kernel(const aj_problem &p) { return umma_covers(p) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT; }
+int32_t auto_kernel(const aj_problem &p) { return umma_covers(p) ? AJ_KERNEL_UMMA_PAIR : AJ_KERNEL_SIMT; }
 
 // The tcgen05 kernels tile queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
 int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
 
-// Longest-processing-time-first assignment of the (already longest-first) tasks to `num_pairs` CTA pairs: every task
-// goes to the pair with the least work so far, so the pairs finish within one shortest task of each other.  A task's
-// cost is its pair-steps (two key tiles each) plus a constant for its Q load and epilogue.
-void assign_pairs(const std::vector<aj_task> &tasks, int num_pairs, std::vector<int32_t> &off, std::vector<int32_t> &ids) {
-    std::vector<std::vector<int32_t>> lists(num_pairs);
-    std::vector<std::pair<int64_t, int>> heap;            // (-load, -pair): max-heap picks the least loaded, lowest pair
-    for (int i = 0; i < num_pairs; ++i) heap.emplace_back(0, -i);
-    std::make_heap(heap.begin(), heap.end());
-    for (size_t t = 0; t < tasks.size(); ++t) {
-        std::pop_heap(heap.begin(), heap.end());
-        auto &top = heap.back();
-        lists[-top.second].push_back((int32_t)t);
-        top.first -= (tasks[t].num_kv_tiles + 1) / 2 + 1;
-        std::push_heap(heap.begin(), heap.end());
-    }
-    off.assign(1, 0);
-    ids.clear();
-    for (const auto &l : lists) { ids.insert(ids.end(), l.begin(), l.end()); off.push_back((int32_t)ids.size()); }
-}
 
 // (Re)build the schedule for `kernel` / `tiling` and upload it.
 aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
@@ -109,7 +90,7 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     int num_pairs = 0;
     if (kernel == AJ_KERNEL_UMMA_PAIR) {
         num_pairs = (int)std::min<size_t>(std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
-        assign_pairs(s->tasks, num_pairs, pair_off, pair_ids);
+        aj::assign_workers(s->tasks, num_pairs, pair_off, pair_ids);
     }
     aj_task *d_tasks = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr;

@@ -38,6 +38,10 @@ void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_
 void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
                         std::vector<aj_task> &tasks);
 
+// Static list scheduling of tasks onto persistent workers (the CTA pairs of the cta_group::2 kernel): off has
+// num_workers + 1 entries, worker w runs tasks ids[off[w] .. off[w+1]) in that order.
+void assign_workers(const std::vector<aj_task> &tasks, int num_workers, std::vector<int32_t> &off, std::vector<int32_t> &ids);
+
 }  // namespace aj
 
 struct aj_schedule {

@@ -243,6 +243,36 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
     order_tasks(tasks);
 }
 
+// Static list scheduling of the tasks onto `num_pairs` workers (CTA pairs): the tasks are taken head by head ((b, h) major,
+// longest first inside a head) and each goes to the pair that is free first under the cost model (pair-steps plus a
+// constant for the Q load and epilogue).  All pairs therefore stream the K/V of the same head at the same time (one
+// head's K, tK, V, tV stay in L2), heads overlap only at their boundaries, and because the last head ends with its
+// shortest tasks the pairs finish within about one short task of each other.
+void assign_workers(const std::vector<aj_task> &tasks, int num_pairs, std::vector<int32_t> &off, std::vector<int32_t> &ids) {
+    std::vector<int32_t> order(tasks.size());
+    for (size_t t = 0; t < tasks.size(); ++t) order[t] = (int32_t)t;
+    std::stable_sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
+        const aj_task &a = tasks[x], &c = tasks[y];
+        if (a.b != c.b) return a.b < c.b;
+        if (a.h != c.h) return a.h < c.h;
+        return a.num_kv_tiles > c.num_kv_tiles;
+    });
+    std::vector<std::vector<int32_t>> lists(num_pairs);
+    std::vector<std::pair<int64_t, int>> heap;            // (-busy-until, -pair): max-heap picks the pair free first
+    for (int i = 0; i < num_pairs; ++i) heap.emplace_back(0, -i);
+    std::make_heap(heap.begin(), heap.end());
+    for (int32_t t : order) {
+        std::pop_heap(heap.begin(), heap.end());
+        auto &top = heap.back();
+        lists[-top.second].push_back(t);
+        top.first -= (tasks[t].num_kv_tiles + 1) / 2 + 1;
+        std::push_heap(heap.begin(), heap.end());
+    }
+    off.assign(1, 0);
+    ids.clear();
+    for (const auto &l : lists) { ids.insert(ids.end(), l.begin(), l.end()); off.push_back((int32_t)ids.size()); }
+}
+
 }  // namespace aj
 
 namespace aj {
@@ -329,6 +359,20 @@ aj_status attn_jvp_schedule_entries(const aj_schedule *s, int32_t *num_entries, 
     if (k_end) std::copy(e.k_end.begin(), e.k_end.end(), k_end);
     if (row_begin) std::copy(e.row_begin.begin(), e.row_begin.end(), row_begin);
     if (row_end) std::copy(e.row_end.begin(), e.row_end.end(), row_end);
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_assign(const aj_schedule *s, int32_t num_workers, int32_t *worker_offset, int32_t *task_ids) {
+    if (!s) return aj::fail(AJ_ERR_INVALID_ARG, "schedule is NULL");
+    if (num_workers <= 0 || !worker_offset || !task_ids) return aj::fail(AJ_ERR_INVALID_ARG, "num_workers must be > 0 and the output arrays non-NULL");
+    try {
+        std::vector<int32_t> off, ids;
+        aj::assign_workers(s->tasks, num_workers, off, ids);
+        std::copy(off.begin(), off.end(), worker_offset);
+        std::copy(ids.begin(), ids.end(), task_ids);
+    } catch (const std::bad_alloc &) {
+        return aj::fail(AJ_ERR_OOM, "out of host memory");
+    }
     return AJ_OK;
 }
 

@@ -66,11 +66,25 @@ SMALL_UMMA = [
 ]
 
 
+UMMA_KERNELS = [aj.AJ_KERNEL_UMMA_PAIR, aj.AJ_KERNEL_UMMA]     # cta_group::2 pairs (the default) and the single-CTA kernel
+KERNEL_IDS = {aj.AJ_KERNEL_UMMA_PAIR: "pair", aj.AJ_KERNEL_UMMA: "single"}
+
+
+def test_default_kernel_for_bf16_d128_is_the_cta_pair_kernel():
+    plan = make_plan(SMALL_UMMA[0])
+    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA_PAIR, 1)
+    with pytest.raises(aj.AttnJvpError) as e:                      # 256-row pair tiles exist only on the packed grid
+        aj.attn_jvp_plan_set_tiling(plan, aj.AJ_TILING_PER_GROUP)
+    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    aj.attn_jvp_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("kernel", UMMA_KERNELS, ids=KERNEL_IDS.get)
 @pytest.mark.parametrize("w", SMALL_UMMA, ids=lambda w: w.name)
-def test_umma_small_every_row(w):
+def test_umma_small_every_row(w, kernel):
     x = make_inputs(w)
-    plan = make_plan(w)
-    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA, 1)
+    plan = make_plan(w, kernel)
+    assert aj.attn_jvp_plan_kernel(plan) == (kernel, 1)
     gpu = run_gpu(w, x, plan=plan)
     gpu2 = run_gpu(w, x, plan=plan)            # the plan re-arms its work counter: a second launch must agree
     aj.attn_jvp_plan_destroy(plan)
@@ -84,7 +98,7 @@ def test_umma_per_group_and_packed_tilings_agree(w):
     # PACKED (default: global 128-row grid, straddling tiles carry row intervals) vs PER_GROUP
     x = make_inputs(w)
     ref = run_oracle(w, x)
-    plan = make_plan(w)
+    plan = make_plan(w, aj.AJ_KERNEL_UMMA)
     packed = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_set_tiling(plan, aj.AJ_TILING_PER_GROUP)
     per_group = run_gpu(w, x, plan=plan)
@@ -97,12 +111,25 @@ def test_umma_per_group_and_packed_tilings_agree(w):
         assert torch.equal(a, b)
 
 
-def test_umma_large_unit_variance_tangents():
+@pytest.mark.parametrize("kernel", UMMA_KERNELS, ids=KERNEL_IDS.get)
+def test_umma_large_unit_variance_tangents(kernel):
     # tangents as large as the primals, peaked scores (|s| up to ~4*sqrt(d)/sqrt(d)): exercises the lazy rescale
     w = Workload("tf_peaked", 1, 2, 128, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=11)
     x = make_inputs(w)
     x[0] = (x[0].float() * 4.0).to(torch.bfloat16)
-    compare(w, run_gpu(w, x), run_oracle(w, x))
+    compare(w, run_gpu(w, x, kernel=kernel), run_oracle(w, x))
+
+
+@pytest.mark.parametrize("kernel", UMMA_KERNELS, ids=KERNEL_IDS.get)
+def test_umma_growing_scores_force_rescales_late_in_the_stream(kernel):
+    # key norms grow along the sequence, so the running max keeps moving by more than the lazy threshold (2^8) long
+    # after the first tiles: the accumulator rescale must happen mid-stream, several times per row
+    w = Workload("full_growing", 1, 2, 128, "full", 1100, 1, 1, "bf16", 0.5, seed=13)
+    x = make_inputs(w)
+    ramp = torch.linspace(0.2, 9.0, w.N).view(1, 1, w.N, 1)
+    x[1] = (x[1].float() * ramp).to(torch.bfloat16)
+    x[0] = (x[0].float() * 3.0).to(torch.bfloat16)
+    compare(w, run_gpu(w, x, kernel=kernel), run_oracle(w, x))
 
 
 def test_umma_zero_tangents_give_exact_zero():
@@ -148,10 +175,11 @@ def test_umma_strided_views():
     assert torch.equal(o.cpu(), ref[0]) and torch.equal(to.cpu(), ref[1]) and torch.equal(lse.cpu(), ref[2])
 
 
-def test_umma_matches_simt_kernel_on_bf16():
+@pytest.mark.parametrize("kernel", UMMA_KERNELS, ids=KERNEL_IDS.get)
+def test_umma_matches_simt_kernel_on_bf16(kernel):
     w = SMALL_UMMA[1]
     x = make_inputs(w)
-    a = run_gpu(w, x, kernel=aj.AJ_KERNEL_UMMA)
+    a = run_gpu(w, x, kernel=kernel)
     b = run_gpu(w, x, kernel=aj.AJ_KERNEL_SIMT)
     for u, v, tol in zip(a, b, (1e-2, 1e-2, 1e-3)):
         assert max_norm_err(u.double().numpy(), v.double().numpy()) <= tol
@@ -248,17 +276,19 @@ def test_fwd_argument_errors():
 FULL = ["wan13b_tf_framewise", "wan13b_tf_chunkwise", "block_causal_b2", "dit_large_tf_chunkwise", "dit_large_full"]
 
 
-@pytest.mark.parametrize("name", FULL)
-def test_full_size_config_sampled_rows(name):
+@pytest.mark.parametrize("name,kernel", [(n, aj.AJ_KERNEL_AUTO) for n in FULL] + [("wan13b_tf_framewise", aj.AJ_KERNEL_UMMA)],
+                         ids=lambda v: v if isinstance(v, str) else {0: "default", 2: "single"}[v])
+def test_full_size_config_sampled_rows(name, kernel):
     w = WORKLOADS[name]
     x = make_inputs(w)
-    plan = make_plan(w)
+    plan = make_plan(w, kernel)
+    assert aj.attn_jvp_plan_kernel(plan)[0] == (aj.AJ_KERNEL_UMMA_PAIR if kernel == aj.AJ_KERNEL_AUTO else kernel)
     pairs, ntasks = aj.attn_jvp_plan_info(plan)
     assert pairs == w.unmasked_pairs_per_head
     gpu = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_destroy(plan)
     per_head = 2 if w.N > 100000 else 3
-    rows = sample_rows(w, per_head_groups=per_head, random_per_group=2)
+    rows = sample_rows(w, per_head_groups=per_head, random_per_group=2, tile_q=256 if kernel == aj.AJ_KERNEL_AUTO else 128)
     errs = compare(w, gpu, run_oracle(w, x, rows))
     print(f"{name}: rows/head={len(next(iter(rows.values())))} errs={errs}")
     # properties that hold at any size: every output written and finite, lse within [min s, max s + ln N]

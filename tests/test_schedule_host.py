@@ -232,7 +232,7 @@ def _check_packed(want, Nq, info, got, ent, tile_q, tile_k, heads=1):
 @pytest.mark.parametrize("mask,L,F,cf", [
     ("teacher_forcing", 16, 3, 1), ("teacher_forcing", 10, 6, 3), ("teacher_forcing", 7, 4, 2),
     ("block_causal", 16, 3, 1), ("block_causal", 9, 6, 2), ("full", 13, 5, 1), ("teacher_forcing", 3, 5, 1)])
-@pytest.mark.parametrize("tile_q,tile_k", [(16, 32), (8, 4), (128, 64), (5, 3)])
+@pytest.mark.parametrize("tile_q,tile_k", [(16, 32), (8, 4), (128, 64), (5, 3), (256, 64)])
 def test_packed_tiles_cover_the_mask_exactly_once(oracle, mask, L, F, cf, tile_q, tile_k):
     w = Workload("t", 1, 2, 64, mask, L, F, cf, "fp32", 1.0)
     prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_FP32)
@@ -266,3 +266,43 @@ def test_packed_tiling_wastes_fewer_tile_rows_on_config_2():
     eff_pg, eff_pk = w.unmasked_pairs_per_head / area(pg["tasks"]), w.unmasked_pairs_per_head / area(got["tasks"])
     assert 0.93 < eff_pg < 0.94 and eff_pk > 0.975, (eff_pg, eff_pk)
     assert len(got["tasks"]) == 512            # 65520 rows / 128
+
+
+# ---------------------------------------------------------------------------------------------- CTA-pair kernel schedule
+def test_pair_tiling_256_rows_on_config_2_and_worker_assignment():
+    """The cta_group::2 kernel's schedule: packed 256-row tiles, tasks assigned head by head to 74 SM pairs."""
+    w = WORKLOADS["wan13b_tf_framewise"]
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, w.frame_len, w.num_frames, w.chunk_frames)
+    s = aj.attn_jvp_schedule_create_tiled(prob, m, 256, 64, aj.AJ_TILING_PACKED)
+    tasks = aj.attn_jvp_schedule_get(s)["tasks"]
+    nt = len(tasks)
+    assert nt == w.H * 256                       # 65520 rows / 256
+    # executed tile area (pair-steps cover two 64-key tiles; an odd tail pays for a masked tile) vs counted pairs
+    area = sum(((t.num_kv_tiles + 1) // 2) * 2 for t in tasks) * 256 * 64
+    assert w.H * w.unmasked_pairs_per_head / area > 0.965
+    workers = 74
+    off, ids = aj.attn_jvp_schedule_assign(s, workers)
+    aj.attn_jvp_schedule_destroy(s)
+    assert off[0] == 0 and off[-1] == nt and sorted(ids) == list(range(nt))      # every task exactly once
+    cost = lambda t: (t.num_kv_tiles + 1) // 2 + 1
+    loads = [sum(cost(tasks[i]) for i in ids[off[k]:off[k + 1]]) for k in range(workers)]
+    assert max(loads) - min(loads) <= max(cost(t) for t in tasks)
+    assert max(loads) <= 1.01 * sum(loads) / workers                            # tail under 1 %
+    # head-major: the heads a worker visits never go backwards, so all workers stream the same head's K/V together
+    for k in range(workers):
+        heads = [tasks[i].h for i in ids[off[k]:off[k + 1]]]
+        assert heads == sorted(heads)
+
+
+@pytest.mark.parametrize("workers", [1, 3, 7])
+def test_worker_assignment_small_and_errors(workers):
+    prob = aj.make_problem(2, 2, 96, 96, 64, aj.AJ_FP32)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, 16, 3, 1)
+    s = aj.attn_jvp_schedule_create_tiled(prob, m, 16, 8, aj.AJ_TILING_PACKED)
+    nt = aj.attn_jvp_schedule_info(s)[2]
+    off, ids = aj.attn_jvp_schedule_assign(s, workers)
+    assert len(off) == workers + 1 and off[-1] == nt and sorted(ids) == list(range(nt))
+    assert aj.lib().attn_jvp_schedule_assign(s, 0, None, None) == aj.AJ_ERR_INVALID_ARG
+    assert aj.lib().attn_jvp_schedule_assign(None, 2, None, None) == aj.AJ_ERR_INVALID_ARG
+    aj.attn_jvp_schedule_destroy(s)
