@@ -17,19 +17,27 @@ struct aj_plan {
     std::vector<int32_t> m_qb, m_qe, m_off, m_kb, m_ke;
     int32_t kernel = AJ_KERNEL_SIMT;
     int32_t tiling = AJ_TILING_PER_GROUP;
-    aj_schedule *sched = nullptr;
-    int32_t num_tasks = 0;
     int device = 0, num_sms = 0;
-    // device copies of the schedule
-    aj_task *d_tasks = nullptr;
-    int32_t *d_kb = nullptr, *d_ke = nullptr, *d_counters = nullptr;
-    uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
-    int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
-    int32_t num_pairs = 0;
-    // staging for attn_jvp_fwd_host
+    int32_t *d_counters = nullptr;
+    // A schedule and its device copy.  `full` covers all B x H heads (attn_jvp_fwd); `head` is the same mask for ONE
+    // (b, h) (built on first use by attn_jvp_fwd_host, which launches head by head while the copies of the
+    // neighbouring heads are in flight).
+    struct DevSchedule {
+        aj_schedule *sched = nullptr;
+        int32_t num_tasks = 0;
+        aj_task *d_tasks = nullptr;
+        int32_t *d_kb = nullptr, *d_ke = nullptr;
+        uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
+        int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
+        int32_t num_pairs = 0;
+    } full, head;
+    // attn_jvp_fwd_host: device staging buffers, copy streams, one event per head and direction
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void *d_out[2] = {nullptr, nullptr};
     float *d_lse = nullptr;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> ev_in, ev_k;
+    cudaEvent_t ev_begin = nullptr, ev_end = nullptr;
 };
 
 namespace {
@@ -57,11 +65,11 @@ aj_status cuda_fail(cudaError_t e, const char *what) {
     return fail(AJ_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 
-void free_device(aj_plan *p) {
-    cudaFree(p->d_tasks); cudaFree(p->d_kb); cudaFree(p->d_ke); cudaFree(p->d_rows);
-    cudaFree(p->d_pair_off); cudaFree(p->d_pair_ids);
-    p->d_tasks = nullptr; p->d_kb = p->d_ke = nullptr; p->d_rows = nullptr;
-    p->d_pair_off = p->d_pair_ids = nullptr; p->num_pairs = 0;
+void free_schedule(aj_plan::DevSchedule &ds) {
+    cudaFree(ds.d_tasks); cudaFree(ds.d_kb); cudaFree(ds.d_ke); cudaFree(ds.d_rows);
+    cudaFree(ds.d_pair_off); cudaFree(ds.d_pair_ids);
+    attn_jvp_schedule_destroy(ds.sched);
+    ds = aj_plan::DevSchedule();
 }
 
 bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
@@ -73,8 +81,9 @@ int32_t auto_kernel(const aj_problem &p) { return umma_covers(p) ? AJ_KERNEL_UMM
 int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
 
 
-// (Re)build the schedule for `kernel` / `tiling` and upload it.
-aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
+// Build the schedule of `prob` (the plan's problem, or one head of it) for `kernel` / `tiling` and upload it into `ds`
+// (left unchanged on failure).
+aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int32_t tiling, aj_plan::DevSchedule &ds) {
     const int tq = kernel == AJ_KERNEL_UMMA_PAIR ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
     const int tk = is_umma(kernel) ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
     if (kernel == AJ_KERNEL_UMMA_PAIR && tiling != AJ_TILING_PACKED)
@@ -82,7 +91,7 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     if (kernel == AJ_KERNEL_SIMT && tiling != AJ_TILING_PER_GROUP)
         return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
     aj_schedule *s = nullptr;
-    if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, tq, tk, tiling, &s)) return st;
+    if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tq, tk, tiling, &s)) return st;
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r) rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16);
@@ -112,11 +121,18 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
         attn_jvp_schedule_destroy(s);
         return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
     }
-    free_device(p);
-    attn_jvp_schedule_destroy(p->sched);
-    p->sched = s; p->kernel = kernel; p->tiling = tiling; p->num_tasks = (int32_t)nt;
-    p->d_tasks = d_tasks; p->d_kb = d_kb; p->d_ke = d_ke; p->d_rows = d_rows;
-    p->d_pair_off = d_pair_off; p->d_pair_ids = d_pair_ids; p->num_pairs = num_pairs;
+    free_schedule(ds);
+    ds.sched = s; ds.num_tasks = (int32_t)nt;
+    ds.d_tasks = d_tasks; ds.d_kb = d_kb; ds.d_ke = d_ke; ds.d_rows = d_rows;
+    ds.d_pair_off = d_pair_off; ds.d_pair_ids = d_pair_ids; ds.num_pairs = num_pairs;
+    return AJ_OK;
+}
+
+// (Re)build the plan's schedule for `kernel` / `tiling`; the per-head schedule is rebuilt on its next use.
+aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
+    if (aj_status st = build_schedule(p, p->problem, kernel, tiling, p->full)) return st;
+    free_schedule(p->head);
+    p->kernel = kernel; p->tiling = tiling;
     return AJ_OK;
 }
 
@@ -191,20 +207,26 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
 
 aj_status attn_jvp_plan_destroy(aj_plan *p) {
     if (!p) return AJ_OK;
-    free_device(p);
+    free_schedule(p->full);
+    free_schedule(p->head);
     cudaFree(p->d_counters);
     for (void *x : p->d_in) cudaFree(x);
     for (void *x : p->d_out) cudaFree(x);
     cudaFree(p->d_lse);
-    attn_jvp_schedule_destroy(p->sched);
+    for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
+    for (cudaEvent_t e : p->ev_k) cudaEventDestroy(e);
+    if (p->ev_begin) cudaEventDestroy(p->ev_begin);
+    if (p->ev_end) cudaEventDestroy(p->ev_end);
+    if (p->s_in) cudaStreamDestroy(p->s_in);
+    if (p->s_out) cudaStreamDestroy(p->s_out);
     delete p;
     return AJ_OK;
 }
 
 aj_status attn_jvp_plan_info(const aj_plan *p, int64_t *pairs, int32_t *num_tasks) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
-    if (pairs) *pairs = p->sched->low.pairs_per_head;
-    if (num_tasks) *num_tasks = p->num_tasks;
+    if (pairs) *pairs = p->full.sched->low.pairs_per_head;
+    if (num_tasks) *num_tasks = p->full.num_tasks;
     return AJ_OK;
 }
 
@@ -227,7 +249,7 @@ aj_status attn_jvp_plan_set_tiling(aj_plan *p, int32_t tiling) {
 aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launches) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
     if (kernel) *kernel = p->kernel;
-    if (launches) *launches = p->num_tasks > 0 ? 1 : 0;
+    if (launches) *launches = p->full.num_tasks > 0 ? 1 : 0;
     return AJ_OK;
 }
 
@@ -240,6 +262,50 @@ aj_status attn_jvp_plan_device_status(aj_plan *p, int32_t *code) {
     return AJ_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// One kernel launch over the tasks of `ds`, which were built for a [B, H] problem (the plan's, or B = H = 1 with the
+// tensor views already moved to the head they address).
+aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int32_t B, int32_t H, const aj_tensor *const ts[8],
+                          float *lse, cudaStream_t stream) {
+    aj_problem pr = p->problem;
+    pr.B = B; pr.H = H;
+    if (ds.num_tasks == 0) return AJ_OK;
+    cudaError_t e;
+    if (is_umma(p->kernel)) {
+        aj::UmmaParams prm;
+        std::memset(&prm, 0, sizeof(prm));
+        aj_status st;
+        if ((st = encode_map(&prm.tm_q, *ts[0], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&prm.tm_tq, *ts[3], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&prm.tm_k, *ts[1], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_tk, *ts[4], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_v, *ts[2], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_tv, *ts[5], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        prm.o = *ts[6]; prm.to = *ts[7]; prm.lse = lse;
+        prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke; prm.rows = ds.d_rows; prm.counters = p->d_counters;
+        prm.num_tasks = ds.num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
+        prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
+        prm.pair_off = ds.d_pair_off; prm.pair_ids = ds.d_pair_ids;
+        e = p->kernel == AJ_KERNEL_UMMA_PAIR ? aj::launch_umma_pair(prm, ds.num_pairs, stream)
+                                             : aj::launch_umma(prm, std::min(p->num_sms, ds.num_tasks), stream);
+    } else {
+        aj::SimtParams prm;
+        prm.q = *ts[0]; prm.k = *ts[1]; prm.v = *ts[2]; prm.tq = *ts[3]; prm.tk = *ts[4]; prm.tv = *ts[5]; prm.o = *ts[6]; prm.to = *ts[7];
+        prm.lse = lse; prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke;
+        prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
+        e = aj::launch_simt(prm, pr.dtype, pr.d, ds.num_tasks, stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
+    return AJ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
                        const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
                        void *cuda_stream) {
@@ -251,35 +317,7 @@ aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k,
     for (int i = 0; i < 8; ++i)
         if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
     if (lse && (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: pointer must be 4-byte aligned");
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    if (p->num_tasks == 0) return AJ_OK;
-    cudaError_t e;
-    if (is_umma(p->kernel)) {
-        aj::UmmaParams prm;
-        std::memset(&prm, 0, sizeof(prm));
-        aj_status st;
-        if ((st = encode_map(&prm.tm_q, *q, pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&prm.tm_tq, *tq, pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&prm.tm_k, *k, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tk, *tk, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_v, *v, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tv, *tv, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        prm.o = *o; prm.to = *to; prm.lse = lse;
-        prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke; prm.rows = p->d_rows; prm.counters = p->d_counters;
-        prm.num_tasks = p->num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
-        prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
-        prm.pair_off = p->d_pair_off; prm.pair_ids = p->d_pair_ids;
-        e = p->kernel == AJ_KERNEL_UMMA_PAIR ? aj::launch_umma_pair(prm, p->num_pairs, stream)
-                                             : aj::launch_umma(prm, std::min(p->num_sms, p->num_tasks), stream);
-    } else {
-        aj::SimtParams prm;
-        prm.q = *q; prm.k = *k; prm.v = *v; prm.tq = *tq; prm.tk = *tk; prm.tv = *tv; prm.o = *o; prm.to = *to;
-        prm.lse = lse; prm.tasks = p->d_tasks; prm.k_begin = p->d_kb; prm.k_end = p->d_ke;
-        prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
-        e = aj::launch_simt(prm, pr.dtype, pr.d, p->num_tasks, stream);
-    }
-    if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
-    return AJ_OK;
+    return launch_schedule(p, p->full, pr.B, pr.H, ts, lse, (cudaStream_t)cuda_stream);
 }
 
 aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *tq, const void *tk,
@@ -290,8 +328,10 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
     if (!o || !to) return fail(AJ_ERR_INVALID_ARG, "a host output pointer is NULL");
     const aj_problem &pr = p->problem;
     const size_t eb = pr.dtype == AJ_BF16 ? 2 : 4;
-    const size_t nq_bytes = (size_t)pr.B * pr.H * pr.Nq * pr.d * eb, nk_bytes = (size_t)pr.B * pr.H * pr.Nk * pr.d * eb;
-    const size_t lse_bytes = (size_t)pr.B * pr.H * pr.Nq * sizeof(float);
+    const int nheads = pr.B * pr.H;
+    const size_t hq_bytes = (size_t)pr.Nq * pr.d * eb, hk_bytes = (size_t)pr.Nk * pr.d * eb;   // one head of a tensor
+    const size_t nq_bytes = hq_bytes * nheads, nk_bytes = hk_bytes * nheads;
+    const size_t lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSuccess;
     for (int i = 0; i < 6 && e == cudaSuccess; ++i)
@@ -300,20 +340,59 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
         if (!p->d_out[i]) e = cudaMalloc(&p->d_out[i], nq_bytes);
     if (e == cudaSuccess && !p->d_lse) e = cudaMalloc(&p->d_lse, lse_bytes);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for staging") : cuda_fail(e, "staging allocation");
-    for (int i = 0; i < 6 && e == cudaSuccess; ++i)
-        e = cudaMemcpyAsync(p->d_in[i], in[i], (i == 0 || i == 3) ? nq_bytes : nk_bytes, cudaMemcpyHostToDevice, stream);
-    if (e != cudaSuccess) return cuda_fail(e, "host-to-device copy");
-    aj_tensor t[8];
-    for (int i = 0; i < 8; ++i) {
-        const int64_t n = (i == 0 || i == 3 || i >= 6) ? pr.Nq : pr.Nk;
-        t[i].ptr = i < 6 ? p->d_in[i] : p->d_out[i - 6];
-        t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = (int64_t)pr.H * n * pr.d;
+    if (!p->s_in) {
+        e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_begin, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_end, cudaEventDisableTiming);
+        p->ev_in.assign(nheads, nullptr); p->ev_k.assign(nheads, nullptr);
+        for (int i = 0; i < nheads && e == cudaSuccess; ++i) {
+            e = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_k[i], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "copy streams / events");
     }
-    if (aj_status st = attn_jvp_fwd(p, &t[0], &t[1], &t[2], &t[3], &t[4], &t[5], &t[6], &t[7], p->d_lse, stream)) return st;
-    e = cudaMemcpyAsync(o, p->d_out[0], nq_bytes, cudaMemcpyDeviceToHost, stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(to, p->d_out[1], nq_bytes, cudaMemcpyDeviceToHost, stream);
-    if (e == cudaSuccess && lse) e = cudaMemcpyAsync(lse, p->d_lse, lse_bytes, cudaMemcpyDeviceToHost, stream);
-    if (e != cudaSuccess) return cuda_fail(e, "device-to-host copy");
+    if (!p->head.sched) {
+        aj_problem one = p->problem;
+        one.B = 1; one.H = 1;
+        if (aj_status st = build_schedule(p, one, p->kernel, p->tiling, p->head)) return st;
+    }
+    // Heads are independent: head i's six slices go up on the copy-in stream, its kernel runs on the
+    // caller's stream as soon as they have landed, and its O, tO, lse come back on the copy-out stream, so the copies
+    // of heads i+1 and i-1 overlap the kernel of head i.  The caller's stream finally waits for the last D2H copy.
+    e = cudaEventRecord(p->ev_begin, stream);                       // earlier work on `stream` may still use the staging buffers
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_in, p->ev_begin, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_begin, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
+    for (int hd = 0; hd < nheads; ++hd) {
+        for (int i = 0; i < 6 && e == cudaSuccess; ++i) {
+            const size_t hb = (i == 0 || i == 3) ? hq_bytes : hk_bytes;
+            e = cudaMemcpyAsync((char *)p->d_in[i] + hd * hb, (const char *)in[i] + hd * hb, hb, cudaMemcpyHostToDevice, p->s_in);
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(p->ev_in[hd], p->s_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_in[hd], 0);
+        if (e != cudaSuccess) return cuda_fail(e, "host-to-device copy");
+        aj_tensor t[8];
+        const aj_tensor *ts[8];
+        for (int i = 0; i < 8; ++i) {
+            const bool is_q = i == 0 || i == 3 || i >= 6;
+            const int64_t n = is_q ? pr.Nq : pr.Nk;
+            t[i].ptr = (char *)(i < 6 ? p->d_in[i] : p->d_out[i - 6]) + hd * (is_q ? hq_bytes : hk_bytes);
+            t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = n * pr.d;
+            ts[i] = &t[i];
+        }
+        if (aj_status st = launch_schedule(p, p->head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq, stream)) return st;
+        e = cudaEventRecord(p->ev_k[hd], stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync((char *)o + hd * hq_bytes, (char *)p->d_out[0] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
+        if (e == cudaSuccess) e = cudaMemcpyAsync((char *)to + hd * hq_bytes, (char *)p->d_out[1] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
+        if (e == cudaSuccess && lse)
+            e = cudaMemcpyAsync(lse + (size_t)hd * pr.Nq, p->d_lse + (size_t)hd * pr.Nq, pr.Nq * sizeof(float), cudaMemcpyDeviceToHost, p->s_out);
+        if (e != cudaSuccess) return cuda_fail(e, "device-to-host copy");
+    }
+    e = cudaEventRecord(p->ev_end, p->s_out);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_end, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
     return AJ_OK;
 }
 

@@ -234,18 +234,31 @@ def test_lse_may_be_null_and_custom_scale():
     assert max_norm_err(to.cpu()[0, 0].double().numpy(), rto) <= 1e-2
 
 
-def test_fwd_host_matches_device_path():
-    w = SMALL_UMMA[0]
+@pytest.mark.parametrize("w", [SMALL_UMMA[0], SMALL_UMMA[2], WORKLOADS["tiny_tf_fp32"]], ids=lambda w: w.name)
+def test_fwd_host_matches_device_path(w):
+    # attn_jvp_fwd_host launches head by head (copies of the neighbouring heads in flight): same bits as one launch
     x = make_inputs(w, pin=True)
     plan = make_plan(w)
-    o = torch.empty_like(x[0]).pin_memory()
-    to = torch.empty_like(x[0]).pin_memory()
-    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
-    aj.attn_jvp_fwd_host(plan, *x, o, to, lse, torch.cuda.current_stream().cuda_stream)
-    torch.cuda.synchronize()
+    o = torch.full_like(x[0], float("nan")).pin_memory()
+    to = torch.full_like(x[0], float("nan")).pin_memory()
+    lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32).pin_memory()
     ref = run_gpu(w, x, plan=plan)
+    for _ in range(2):                                  # the second call reuses the staging buffers and events
+        aj.attn_jvp_fwd_host(plan, *x, o, to, lse, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert torch.equal(o, ref[0]) and torch.equal(to, ref[1]) and torch.equal(lse, ref[2])
+        o.fill_(float("nan")); to.fill_(float("nan")); lse.fill_(float("nan"))
+    aj.attn_jvp_fwd_host(plan, *x, o, to, None, 0)      # default stream, no lse
+    torch.cuda.synchronize()
+    assert torch.equal(o, ref[0]) and torch.equal(to, ref[1]) and torch.isnan(lse).all()
+    if w.dtype == "bf16":                               # switching the kernel rebuilds the per-head schedule too
+        aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA)
+        ref1 = run_gpu(w, x, plan=plan)
+        aj.attn_jvp_fwd_host(plan, *x, o, to, lse, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert torch.equal(o, ref1[0]) and torch.equal(to, ref1[1]) and torch.equal(lse, ref1[2])
+    assert aj.attn_jvp_plan_device_status(plan) == 0
     aj.attn_jvp_plan_destroy(plan)
-    assert torch.equal(o, ref[0]) and torch.equal(to, ref[1]) and torch.equal(lse, ref[2])
 
 
 def test_fwd_argument_errors():
