@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 import numpy as np
 import torch
 
-from paper_2606_25473_b200.workloads import WORKLOADS, Workload, make_inputs
+from paper_2606_25473_b200.workloads import EXTRA_WORKLOADS, WORKLOADS, Workload, make_inputs
 
 METRIC = "attention-JVP TFLOPS (unmasked pairs)"
 UNIT = "TFLOP/s"
@@ -39,8 +39,19 @@ DEFAULT_WORKLOAD = "wan13b_tf_framewise"
 FALLBACK_PEAKS = {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_gbs": 6650.0}   # B200_PROFILING.md
 
 
+def pair_classes(w: Workload):
+    """Unmasked pairs per head needing 2 / 4 / 6 length-d contractions (accounting only).  Dense tangents: all 6.
+    Zero clean tangents: clean x clean pairs need S and P V only, noisy x clean pairs also tQ K^T and H V."""
+    if not w.clean_tangent_zero:
+        return [0, 0, w.unmasked_pairs_per_head]
+    n, C = w.num_blocks, w.block_len
+    return [n * (n + 1) // 2 * C * C, n * (n - 1) // 2 * C * C, n * C * C]
+
+
 def flops_per_call(w: Workload) -> float:
-    return 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H
+    """2*d flop per contraction per unmasked pair: 12*d per pair with dense tangents (the BASELINE.json convention)."""
+    c = pair_classes(w)
+    return 2.0 * w.d * (2 * c[0] + 4 * c[1] + 6 * c[2]) * w.B * w.H
 
 
 def allowed_keys_per_row(w: Workload, rows: np.ndarray) -> np.ndarray:
@@ -185,7 +196,10 @@ def run_reference(args, w: Workload):
 def workload_config(w: Workload):
     return {"workload": w.name, "B": w.B, "H": w.H, "d": w.d, "N": w.N, "mask": w.mask, "frame_len": w.frame_len,
             "num_frames": w.num_frames, "chunk_frames": w.chunk_frames, "input_dtype": w.dtype,
-            "unmasked_pairs_per_head": w.unmasked_pairs_per_head, "flop_convention": "12*d per unmasked pair",
+            "unmasked_pairs_per_head": w.unmasked_pairs_per_head,
+            "tangent_zero": "clean" if w.clean_tangent_zero else "none",
+            "flop_convention": ("2*d per contraction actually needed per unmasked pair (2, 4 or 6 of them: zero clean tangents)"
+                                if w.clean_tangent_zero else "12*d per unmasked pair"),
             "l2": "no flush: the six inputs (%.2f GB) are larger than the 126 MB L2" %
                   (6 * w.B * w.H * w.N * w.d * (2 if w.dtype == "bf16" else 4) / 1e9)}
 
@@ -238,17 +252,18 @@ def run_cuda(args, w: Workload):
     kind = {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL,
             "full": aj.AJ_MASK_FULL}[w.mask]
     prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32)
-    mask, keep = aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames)
+    mask, keep = aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames,
+                              tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE)
     t0 = time.perf_counter()
     plan = aj.attn_jvp_plan_create(prob, mask)
     plan_ms = 1e3 * (time.perf_counter() - t0)
     kernel, launches_per_call = aj.attn_jvp_plan_kernel(plan)
     pairs, num_tasks = aj.attn_jvp_plan_info(plan)
-    assert pairs == w.unmasked_pairs_per_head
+    assert pairs == w.unmasked_pairs_per_head and aj.attn_jvp_plan_pair_classes(plan) == pair_classes(w)
 
     # every rank draws its own head shard (seed + rank): weak scaling, no exchange
     wr = Workload(w.name, w.B, w.H, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std,
-                  w.seed + rank)
+                  w.seed + rank, w.clean_tangent_zero)
     host = make_inputs(wr, pin=True)
     devin = [x.to(dev, non_blocking=True) for x in host]
     o, to = torch.empty_like(devin[0]), torch.empty_like(devin[0])
@@ -330,6 +345,8 @@ def run_cuda(args, w: Workload):
                      "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
                      "flops_per_launch": flops},
     }
+    if w.clean_tangent_zero:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
+        line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
     if world == 1 and not args.no_cpu_baseline:
         tf, dt, nrows, cores = time_oracle_sample(w, host, args.cpu_budget_s)
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -344,12 +361,12 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(WORKLOADS))
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(WORKLOADS) + list(EXTRA_WORKLOADS))
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    w = WORKLOADS[args.workload]
+    w = {**WORKLOADS, **EXTRA_WORKLOADS}[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -48,6 +48,18 @@ typedef enum {
     AJ_MASK_RANGES = 3           /* explicit query groups with key-range lists                            */
 } aj_mask_kind;
 
+/* Structural zeros among the tangents: a PROMISE by the caller that lets the kernel skip contractions whose operand is
+ * identically zero ("The tangent of the clean context is zero" in every TF-sCM call, and clean rows see
+ * only clean keys, so their tangents stay zero in every layer).  The results are those of the dense computation on the
+ * same data; data that breaks the promise gives undefined tO.
+ *   DENSE      no promise (6 contractions per unmasked pair)
+ *   CLEAN_ZERO TEACHER_FORCING: tQ, tK, tV rows of the clean half are zero -> clean x clean pairs need 2 of the 6
+ *              contractions (S, P V), noisy x clean pairs 4 (no Q tK^T, no P tV), and tO of the clean rows is written as 0.
+ *              RANGES: per-group / per-range flags (q_tangent_zero, k_tangent_zero) say the same.
+ *   NONE       no tangents at all: plain masked attention forward (O, lse); tq, tk, tv, to may be NULL in attn_jvp_fwd
+ *              (a non-NULL `to` is filled with zeros).  This is the cached-prefix forward of PAPER.md:324-328. */
+typedef enum { AJ_TANGENT_DENSE = 0, AJ_TANGENT_CLEAN_ZERO = 1, AJ_TANGENT_NONE = 2 } aj_tangent_zero;
+
 /* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA_PAIR when (bf16, d = 128), else SIMT.
  * UMMA: one CTA per 128-row query tile (tcgen05.mma.cta_group::1).  UMMA_PAIR: a CTA pair per 256-row query tile
  * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile). */
@@ -71,8 +83,13 @@ typedef struct {
     int32_t num_frames;         /* F frames (per half for TEACHER_FORCING) */
     int32_t chunk_frames;       /* frames per block */
     int32_t first_chunk_frames; /* 0 = same as chunk_frames */
-    int32_t num_groups;         /* AJ_MASK_RANGES only, as are the five arrays below */
+    int32_t num_groups;         /* AJ_MASK_RANGES only, as are the arrays below */
+    int32_t tangent_zero;       /* aj_tangent_zero */
     const int32_t *q_begin, *q_end, *range_offset, *k_begin, *k_end;
+    /* AJ_MASK_RANGES with AJ_TANGENT_CLEAN_ZERO: non-zero = the tQ rows of group g / the tK, tV rows of range r are all
+     * zero; [num_groups] / [range_offset[num_groups]]; NULL = no flag set.  Overlapping key ranges of different groups
+     * must agree. */
+    const int32_t *q_tangent_zero, *k_tangent_zero;
 } aj_mask_desc;
 
 typedef struct {
@@ -106,7 +123,12 @@ typedef struct {
     int32_t range_begin, range_count; /* its entries */
     int32_t num_kv_tiles;             /* key tiles it streams (sum over entries of ceil(len / tile_k)) */
     int32_t group;                    /* PER_GROUP: index of its query group; PACKED: -1 */
+    int32_t flags;                    /* AJ_TASK_* */
 } aj_task;
+
+/* aj_task::flags.  PRIMAL_ONLY: tQ of every row and tK, tV of every key of the task are structurally zero: the task needs
+ * only S = Q K^T and O += P V (tO = 0). */
+enum { AJ_TASK_PRIMAL_ONLY = 1 };
 
 typedef struct aj_schedule aj_schedule; /* host-only: groups, merged ranges, ordered task list */
 typedef struct aj_plan aj_plan;         /* schedule + its device copy + staging buffers       */
@@ -135,9 +157,16 @@ aj_status attn_jvp_schedule_get(const aj_schedule *sched, int32_t *q_begin, int3
 aj_status attn_jvp_schedule_entries(const aj_schedule *sched, int32_t *num_entries, int32_t *k_begin,
                                     int32_t *k_end, int32_t *row_begin, int32_t *row_end);
 
+/* Per entry: non-zero = the tK, tV rows of its keys are structurally zero (aj_tangent_zero).  [num_entries]. */
+aj_status attn_jvp_schedule_entry_flags(const aj_schedule *sched, int32_t *key_tangent_zero);
+/* Unmasked pairs per head by the number of contractions they need: pairs[0] need 2 (tQ row and tK, tV key zero),
+ * pairs[1] need 4 (only the key's tangents zero), pairs[2] need all 6.  Sums to unmasked_pairs_per_head. */
+aj_status attn_jvp_schedule_pair_classes(const aj_schedule *sched, int64_t pairs[3]);
+
 /* Static assignment of the tasks to num_workers persistent workers (the CTA-pair kernel's SM pairs; PAPER.md:897
  * "parallel over tasks"): tasks are taken (b, h)-major, longest first inside a head, and each goes to the worker that
- * is free first under the cost model ceil(num_kv_tiles / 2) + 1.  worker_offset [num_workers + 1], task_ids
+ * is free first under a cost model (a constant per task plus, per pair of key tiles, a weight that depends on how many
+ * contractions the pair needs).  worker_offset [num_workers + 1], task_ids
  * [num_tasks] (indices into the task list of attn_jvp_schedule_get): worker w runs
  * task_ids[worker_offset[w] .. worker_offset[w+1]) in order.  Every task appears exactly once. */
 aj_status attn_jvp_schedule_assign(const aj_schedule *sched, int32_t num_workers, int32_t *worker_offset,
@@ -150,6 +179,8 @@ aj_status attn_jvp_schedule_assign(const aj_schedule *sched, int32_t num_workers
 aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *mask, aj_plan **out);
 aj_status attn_jvp_plan_destroy(aj_plan *plan);
 aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_head, int32_t *num_tasks);
+/* attn_jvp_schedule_pair_classes of the plan's mask. */
+aj_status attn_jvp_plan_pair_classes(const aj_plan *plan, int64_t pairs[3]);
 /* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
  * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged. */
 aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
@@ -166,10 +197,18 @@ aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *la
  * lse: contiguous fp32 [B,H,Nq] (may be NULL).  All DEVICE memory; inputs are only read.  Pointers must be
  * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
  * A plan must not be used by two streams at the same time (it owns a device work counter).
+ * Plans whose mask says AJ_TANGENT_NONE accept NULL for tq, tk, tv and to (CTA-pair tcgen05 kernel only; the other
+ * kernels return AJ_ERR_UNSUPPORTED for NULL tangents).
  */
 aj_status attn_jvp_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v,
                        const aj_tensor *tq, const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o,
                        const aj_tensor *to, float *lse, void *cuda_stream);
+
+/* Masked attention forward without tangents: attn_jvp_fwd(plan, q, k, v, NULL, NULL, NULL, o, NULL, lse, stream) on a plan
+ * whose mask says AJ_TANGENT_NONE (else AJ_ERR_INVALID_ARG).  q: [B,H,Nq,d], k, v: [B,H,Nk,d] (Nq != Nk allowed: the
+ * current chunk against the cached prefix). */
+aj_status attn_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o,
+                   float *lse, void *cuda_stream);
 
 /*
  * Same computation on HOST buffers: contiguous [B,H,N,d] arrays in the problem dtype (lse fp32
@@ -192,7 +231,7 @@ aj_status attn_jvp_plan_device_status(aj_plan *plan, int32_t *code);
 
 /* Message for the most recent non-OK status returned to this thread ("" if none). Never NULL. */
 const char *attn_jvp_last_error(void);
-/* Library version string, e.g. "attn_jvp 0.1 (sm_100a)". */
+/* Library version string, e.g. "attn_jvp 0.2 (sm_100a)". */
 const char *attn_jvp_version(void);
 
 #ifdef __cplusplus

@@ -17,6 +17,8 @@ AJ_BF16, AJ_FP32 = 0, 1
 AJ_MASK_FULL, AJ_MASK_BLOCK_CAUSAL, AJ_MASK_TEACHER_FORCING, AJ_MASK_RANGES = 0, 1, 2, 3
 AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA, AJ_KERNEL_UMMA_PAIR = 0, 1, 2, 3
 AJ_TILING_PER_GROUP, AJ_TILING_PACKED = 0, 1
+AJ_TANGENT_DENSE, AJ_TANGENT_CLEAN_ZERO, AJ_TANGENT_NONE = 0, 1, 2
+AJ_TASK_PRIMAL_ONLY = 1
 
 _I32P = ctypes.POINTER(ctypes.c_int32)
 
@@ -24,8 +26,9 @@ _I32P = ctypes.POINTER(ctypes.c_int32)
 class aj_mask_desc(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int32), ("frame_len", ctypes.c_int32), ("num_frames", ctypes.c_int32),
                 ("chunk_frames", ctypes.c_int32), ("first_chunk_frames", ctypes.c_int32),
-                ("num_groups", ctypes.c_int32), ("q_begin", _I32P), ("q_end", _I32P),
-                ("range_offset", _I32P), ("k_begin", _I32P), ("k_end", _I32P)]
+                ("num_groups", ctypes.c_int32), ("tangent_zero", ctypes.c_int32), ("q_begin", _I32P), ("q_end", _I32P),
+                ("range_offset", _I32P), ("k_begin", _I32P), ("k_end", _I32P),
+                ("q_tangent_zero", _I32P), ("k_tangent_zero", _I32P)]
 
 
 class aj_problem(ctypes.Structure):
@@ -41,7 +44,7 @@ class aj_tensor(ctypes.Structure):
 class aj_task(ctypes.Structure):
     _fields_ = [("b", ctypes.c_int32), ("h", ctypes.c_int32), ("q_begin", ctypes.c_int32), ("q_rows", ctypes.c_int32),
                 ("range_begin", ctypes.c_int32), ("range_count", ctypes.c_int32), ("num_kv_tiles", ctypes.c_int32),
-                ("group", ctypes.c_int32)]
+                ("group", ctypes.c_int32), ("flags", ctypes.c_int32)]
 
 
 class AttnJvpError(RuntimeError):
@@ -53,6 +56,7 @@ class AttnJvpError(RuntimeError):
 # Every symbol include/attn_jvp.h declares (tests check that the library exports all of them).
 SYMBOLS = [
     "attn_jvp_schedule_create", "attn_jvp_schedule_create_tiled", "attn_jvp_schedule_entries", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get", "attn_jvp_schedule_assign",
+    "attn_jvp_schedule_entry_flags", "attn_jvp_schedule_pair_classes", "attn_jvp_plan_pair_classes", "attn_fwd",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
 ]
@@ -73,6 +77,10 @@ def lib():
         l.attn_jvp_schedule_create_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_entries.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P]
         l.attn_jvp_schedule_assign.argtypes = [vp, i32, _I32P, _I32P]
+        l.attn_jvp_schedule_entry_flags.argtypes = [vp, _I32P]
+        l.attn_jvp_schedule_pair_classes.argtypes = [vp, i64p]
+        l.attn_jvp_plan_pair_classes.argtypes = [vp, i64p]
+        l.attn_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 4 + [vp, vp]
         l.attn_jvp_schedule_destroy.argtypes = [vp]
         l.attn_jvp_schedule_info.argtypes = [vp, _I32P, _I32P, _I32P, i64p]
         l.attn_jvp_schedule_get.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P, ctypes.POINTER(aj_task)]
@@ -113,9 +121,13 @@ def make_problem(B: int, H: int, Nq: int, Nk: int, d: int, dtype: int, scale: fl
 
 
 def make_mask(kind: int, frame_len: int = 0, num_frames: int = 0, chunk_frames: int = 1, first_chunk_frames: int = 0,
-              groups: Optional[Sequence[Tuple[int, int, Sequence[Tuple[int, int]]]]] = None):
-    """Returns (aj_mask_desc, keepalive).  `groups` = [(q_begin, q_end, [(k_begin, k_end), ...]), ...] for AJ_MASK_RANGES."""
-    m = aj_mask_desc(kind, frame_len, num_frames, chunk_frames, first_chunk_frames, 0, None, None, None, None, None)
+              groups: Optional[Sequence[Tuple[int, int, Sequence[Tuple[int, int]]]]] = None,
+              tangent_zero: int = AJ_TANGENT_DENSE, q_tangent_zero: Optional[Sequence[int]] = None,
+              k_tangent_zero: Optional[Sequence[int]] = None):
+    """Returns (aj_mask_desc, keepalive).  `groups` = [(q_begin, q_end, [(k_begin, k_end), ...]), ...] for AJ_MASK_RANGES;
+    q_tangent_zero [len(groups)] / k_tangent_zero [total ranges] are its AJ_TANGENT_CLEAN_ZERO flags."""
+    m = aj_mask_desc(kind, frame_len, num_frames, chunk_frames, first_chunk_frames, 0, tangent_zero,
+                     None, None, None, None, None, None, None)
     keep = []
     if groups is not None:
         ng = len(groups)
@@ -134,6 +146,14 @@ def make_mask(kind: int, frame_len: int = 0, num_frames: int = 0, chunk_frames: 
         m.q_begin, m.q_end, m.range_offset = qb, qe, offa
         m.k_begin, m.k_end = kba, kea
         keep = [qb, qe, offa, kba, kea]
+        if q_tangent_zero is not None:
+            qz = (ctypes.c_int32 * max(ng, 1))(*q_tangent_zero)
+            m.q_tangent_zero = qz
+            keep.append(qz)
+        if k_tangent_zero is not None:
+            kz = (ctypes.c_int32 * max(len(kb), 1))(*k_tangent_zero)
+            m.k_tangent_zero = kz
+            keep.append(kz)
     return m, keep
 
 
@@ -157,6 +177,22 @@ def attn_jvp_schedule_entries(sched):
     arrs = [(ctypes.c_int32 * max(n.value, 1))() for _ in range(4)]
     _check(lib().attn_jvp_schedule_entries(sched, ctypes.byref(n), *arrs))
     return dict(zip(("k_begin", "k_end", "row_begin", "row_end"), (list(a)[:n.value] for a in arrs)))
+
+
+def attn_jvp_schedule_entry_flags(sched):
+    """-> key_tangent_zero per entry (list of 0/1)"""
+    n = ctypes.c_int32()
+    _check(lib().attn_jvp_schedule_entries(sched, ctypes.byref(n), None, None, None, None))
+    arr = (ctypes.c_int32 * max(n.value, 1))()
+    _check(lib().attn_jvp_schedule_entry_flags(sched, arr))
+    return list(arr)[:n.value]
+
+
+def attn_jvp_schedule_pair_classes(sched):
+    """-> [pairs needing 2, 4, 6 contractions] per head"""
+    arr = (ctypes.c_int64 * 3)()
+    _check(lib().attn_jvp_schedule_pair_classes(sched, arr))
+    return list(arr)
 
 
 def attn_jvp_schedule_assign(sched, num_workers: int):
@@ -209,6 +245,13 @@ def attn_jvp_plan_info(plan):
     return a.value, b.value
 
 
+def attn_jvp_plan_pair_classes(plan):
+    """-> [pairs needing 2, 4, 6 contractions] per head"""
+    arr = (ctypes.c_int64 * 3)()
+    _check(lib().attn_jvp_plan_pair_classes(plan, arr))
+    return list(arr)
+
+
 def attn_jvp_plan_set_kernel(plan, kernel: int) -> None:
     _check(lib().attn_jvp_plan_set_kernel(plan, kernel))
 
@@ -239,9 +282,17 @@ def _tensor(t) -> aj_tensor:
 
 
 def attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
-    """Device tensors (torch.cuda); enqueues on `stream` (a cudaStream_t handle, 0 = default) and returns."""
-    ts = [_tensor(x) for x in (q, k, v, tq, tk, tv, o, to)]
-    _check(lib().attn_jvp_fwd(plan, *[ctypes.byref(x) for x in ts], None if lse is None else lse.data_ptr(), stream))
+    """Device tensors (torch.cuda); enqueues on `stream` (a cudaStream_t handle, 0 = default) and returns.
+    tq, tk, tv, to may be None on AJ_TANGENT_NONE plans."""
+    ts = [None if x is None else _tensor(x) for x in (q, k, v, tq, tk, tv, o, to)]
+    _check(lib().attn_jvp_fwd(plan, *[None if x is None else ctypes.byref(x) for x in ts],
+                              None if lse is None else lse.data_ptr(), stream))
+
+
+def attn_fwd(plan, q, k, v, o, lse=None, stream: int = 0) -> None:
+    """Masked attention forward without tangents (AJ_TANGENT_NONE plans): O and lse only."""
+    ts = [_tensor(x) for x in (q, k, v, o)]
+    _check(lib().attn_fwd(plan, *[ctypes.byref(x) for x in ts], None if lse is None else lse.data_ptr(), stream))
 
 
 def attn_jvp_fwd_host(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:

@@ -14,7 +14,7 @@
 struct aj_plan {
     aj_problem problem;       // scale resolved (never 0)
     aj_mask_desc mask;        // arrays below back the pointers for AJ_MASK_RANGES
-    std::vector<int32_t> m_qb, m_qe, m_off, m_kb, m_ke;
+    std::vector<int32_t> m_qb, m_qe, m_off, m_kb, m_ke, m_qtz, m_ktz;
     int32_t kernel = AJ_KERNEL_SIMT;
     int32_t tiling = AJ_TILING_PER_GROUP;
     int device = 0, num_sms = 0;
@@ -94,12 +94,13 @@ aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int
     if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tq, tk, tiling, &s)) return st;
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
-    for (size_t r = 0; r < nr; ++r) rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16);
+    for (size_t r = 0; r < nr; ++r)   // row_begin | row_end << 16 (both < 32768) | key-tangents-zero << 31
+        rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16) | (s->entries.k_tz[r] ? 0x80000000u : 0u);
     std::vector<int32_t> pair_off, pair_ids;
     int num_pairs = 0;
     if (kernel == AJ_KERNEL_UMMA_PAIR) {
         num_pairs = (int)std::min<size_t>(std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
-        aj::assign_workers(s->tasks, num_pairs, pair_off, pair_ids);
+        aj::assign_workers(s->tasks, s->entries, s->tile_k, num_pairs, pair_off, pair_ids);
     }
     aj_task *d_tasks = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr;
@@ -188,6 +189,10 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
             p->m_ke.assign(mask->k_end, mask->k_end + nr);
             p->mask.q_begin = p->m_qb.data(); p->mask.q_end = p->m_qe.data(); p->mask.range_offset = p->m_off.data();
             p->mask.k_begin = p->m_kb.data(); p->mask.k_end = p->m_ke.data();
+            if (mask->q_tangent_zero) { p->m_qtz.assign(mask->q_tangent_zero, mask->q_tangent_zero + ng); p->mask.q_tangent_zero = p->m_qtz.data(); }
+            if (mask->k_tangent_zero) { p->m_ktz.assign(mask->k_tangent_zero, mask->k_tangent_zero + nr); p->mask.k_tangent_zero = p->m_ktz.data(); }
+        } else {
+            p->mask.q_tangent_zero = p->mask.k_tangent_zero = nullptr;
         }
         cudaError_t e = cudaGetDevice(&p->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
@@ -228,6 +233,11 @@ aj_status attn_jvp_plan_info(const aj_plan *p, int64_t *pairs, int32_t *num_task
     if (pairs) *pairs = p->full.sched->low.pairs_per_head;
     if (num_tasks) *num_tasks = p->full.num_tasks;
     return AJ_OK;
+}
+
+aj_status attn_jvp_plan_pair_classes(const aj_plan *p, int64_t pairs[3]) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    return attn_jvp_schedule_pair_classes(p->full.sched, pairs);
 }
 
 aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
@@ -274,17 +284,23 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
     pr.B = B; pr.H = H;
     if (ds.num_tasks == 0) return AJ_OK;
     cudaError_t e;
+    // AJ_TANGENT_NONE plans may leave tq, tk, tv, to NULL: every task is primal-only and never touches them (the tensor
+    // maps of the absent tangents alias the primals so that they stay valid)
+    const bool no_tangents = !ts[3] || !ts[4] || !ts[5] || !ts[7];
+    if (no_tangents && p->kernel != AJ_KERNEL_UMMA_PAIR)
+        return fail(AJ_ERR_UNSUPPORTED, "NULL tangents need the CTA-pair tcgen05 kernel (bf16, d = 128)");
     if (is_umma(p->kernel)) {
         aj::UmmaParams prm;
         std::memset(&prm, 0, sizeof(prm));
         aj_status st;
         if ((st = encode_map(&prm.tm_q, *ts[0], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&prm.tm_tq, *ts[3], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&prm.tm_tq, *(ts[3] ? ts[3] : ts[0]), pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
         if ((st = encode_map(&prm.tm_k, *ts[1], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tk, *ts[4], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&prm.tm_tk, *(ts[4] ? ts[4] : ts[1]), pr, pr.Nk, aj::UMMA_TILE_K))) return st;
         if ((st = encode_map(&prm.tm_v, *ts[2], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tv, *ts[5], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        prm.o = *ts[6]; prm.to = *ts[7]; prm.lse = lse;
+        if ((st = encode_map(&prm.tm_tv, *(ts[5] ? ts[5] : ts[2]), pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        prm.o = *ts[6]; prm.lse = lse;
+        if (ts[7]) prm.to = *ts[7];
         prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke; prm.rows = ds.d_rows; prm.counters = p->d_counters;
         prm.num_tasks = ds.num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
         prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
@@ -314,10 +330,21 @@ aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k,
     const int eb = pr.dtype == AJ_BF16 ? 2 : 4;
     const aj_tensor *ts[8] = {q, k, v, tq, tk, tv, o, to};
     const char *names[8] = {"q", "k", "v", "tq", "tk", "tv", "o", "to"};
-    for (int i = 0; i < 8; ++i)
+    const bool may_omit = p->mask.tangent_zero == AJ_TANGENT_NONE;
+    for (int i = 0; i < 8; ++i) {
+        const bool tangent = (i >= 3 && i <= 5) || i == 7;
+        if (tangent && may_omit && !ts[i]) continue;
         if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
+    }
     if (lse && (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: pointer must be 4-byte aligned");
     return launch_schedule(p, p->full, pr.B, pr.H, ts, lse, (cudaStream_t)cuda_stream);
+}
+
+aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o, float *lse,
+                   void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (p->mask.tangent_zero != AJ_TANGENT_NONE) return fail(AJ_ERR_INVALID_ARG, "attn_fwd needs a plan whose mask says AJ_TANGENT_NONE");
+    return attn_jvp_fwd(p, q, k, v, nullptr, nullptr, nullptr, o, nullptr, lse, cuda_stream);
 }
 
 aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *tq, const void *tk,

@@ -14,18 +14,21 @@ aj_status fail(aj_status st, const std::string &msg);
 const char *last_error_cstr();
 aj_status check_problem(const aj_problem *p);
 
-struct KeyRange { int32_t k_begin, k_end; };
+struct KeyRange { int32_t k_begin, k_end; int32_t tz = 0; /* tK, tV rows of these keys are structurally zero */ };
 
 // The lowered mask: disjoint query groups, each with sorted, disjoint, merged key ranges.
 struct Lowered {
     std::vector<int32_t> q_begin, q_end, range_offset;  // range_offset has num_groups + 1 entries
     std::vector<KeyRange> ranges;
+    std::vector<int32_t> q_tz;                          // per group: its tQ rows are structurally zero
     int64_t pairs_per_head = 0;
+    int64_t pair_class[3] = {0, 0, 0};                  // pairs needing 2 / 4 / 6 contractions (sum = pairs_per_head)
 };
 
 // What the tasks index (aj_task::range_begin / range_count): key ranges with the rows of the query tile that see them.
 struct Entries {
     std::vector<int32_t> k_begin, k_end, row_begin, row_end;  // rows relative to the task's q_begin
+    std::vector<int32_t> k_tz;                                // tK, tV of the entry's keys are structurally zero
     size_t size() const { return k_begin.size(); }
 };
 
@@ -40,7 +43,8 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
 
 // Static list scheduling of tasks onto persistent workers (the CTA pairs of the cta_group::2 kernel): off has
 // num_workers + 1 entries, worker w runs tasks ids[off[w] .. off[w+1]) in that order.
-void assign_workers(const std::vector<aj_task> &tasks, int num_workers, std::vector<int32_t> &off, std::vector<int32_t> &ids);
+void assign_workers(const std::vector<aj_task> &tasks, const Entries &ent, int32_t tile_k, int num_workers,
+                    std::vector<int32_t> &off, std::vector<int32_t> &ids);
 
 }  // namespace aj
 

@@ -17,6 +17,15 @@
 // Roles per CTA (8 warps): warp 0 TMA producer, warp 1 MMA issuer (CTA 0 only), warp 2 TMEM allocator, warps 4-7
 // softmax / tangent weights / rescale / epilogue (thread = query row = TMEM lane).  Tasks are assigned to pairs by the
 // host (longest-processing-time first), so there is no device-side work queue.
+//
+// Structural-zero tangents (aj_tangent_zero; "The tangent of the clean context is zero"):
+//   key-zero pair-step (both tiles' tK, tV are zero, schedule entry flag): tK, tV are not loaded, Q tK^T and P~ tV are not
+//     issued: 32 MMAs instead of 48.  The producer decides per pair-step and tells the MMA warp through `slot_kz`.
+//   primal-only task (AJ_TASK_PRIMAL_ONLY: tQ of its rows is zero too): only S = Q K^T and O += P~ V (16 MMAs per
+//     pair-step); the tS columns of TMEM become a second S buffer, so that S(p+2) is computed while the softmax of
+//     pair-step p+1 runs (the classic two-stage forward-attention pipeline); tO of its rows is written as 0.
+// Barrier phases are counted per barrier set: c_s (S_FULL, P_FULL), c_ts (TS_FULL, H_FULL), c_pv (PV_DONE); every role
+// walks the same task list, so the counts agree.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -117,6 +126,8 @@ struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
     int abort_flag;
+    int slot_kz[NSTAGE];   // leader CTA: the pair-step whose {K, tK} sits in the slot has zero key tangents (set by the
+                           // producer before it arms KV_FULL[slot], read by the MMA warp after its wait)
 };
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
@@ -170,46 +181,61 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
-                // Q_i, tQ_i: this CTA's 128 rows, two 64-column swizzle blocks each
+                const bool primal = (task.flags & AJ_TASK_PRIMAL_ONLY) != 0;
+                // Q_i, tQ_i: this CTA's 128 rows, two 64-column swizzle blocks each (no tQ if it is zero)
                 wait(BAR_Q_EMPTY, (nq & 1) ^ 1);
                 const uint32_t qfull = lead_bars + 8 * BAR_Q_FULL;
-                if (rank == 0) mbar_expect_tx(bars + 8 * BAR_Q_FULL, 4 * Q_BYTES);
+                if (rank == 0) mbar_expect_tx(bars + 8 * BAR_Q_FULL, primal ? 2 * Q_BYTES : 4 * Q_BYTES);
                 const int qrow = task.q_begin + BR * (int)rank;
                 tma_load_4d_pair(sQ, &prm.tm_q, qfull, 0, qrow, task.h, task.b);
                 tma_load_4d_pair(sQ + QHALF_BYTES, &prm.tm_q, qfull, 64, qrow, task.h, task.b);
-                tma_load_4d_pair(sTQ, &prm.tm_tq, qfull, 0, qrow, task.h, task.b);
-                tma_load_4d_pair(sTQ + QHALF_BYTES, &prm.tm_tq, qfull, 64, qrow, task.h, task.b);
+                if (!primal) {
+                    tma_load_4d_pair(sTQ, &prm.tm_tq, qfull, 0, qrow, task.h, task.b);
+                    tma_load_4d_pair(sTQ + QHALF_BYTES, &prm.tm_tq, qfull, 64, qrow, task.h, task.b);
+                }
                 ++nq;
                 TileCursor cur;
                 cur.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
                 const int np = (n + 1) >> 1;
+                int flag_entry = -1;
+                bool flag = false;                         // tK, tV of the entry's keys are structurally zero
+                auto entry_kz = [&](int e) { if (e != flag_entry) { flag_entry = e; flag = (prm.rows[e] >> 31) != 0; } return flag; };
                 for (int p = 0; p < np; ++p) {
                     const Tile t0 = cur.get();
                     cur.next();
                     Tile t1 = t0;                          // odd tail: the second tile is a fully masked copy of the first
-                    if (2 * p + 1 < n) { t1 = cur.get(); cur.next(); }
+                    bool kz = primal || entry_kz(t0.entry);
+                    if (2 * p + 1 < n) { t1 = cur.get(); cur.next(); kz = kz && (primal || entry_kz(t1.entry)); }
+                    const uint32_t slot_tx = kz ? SLOT_BYTES : 2 * SLOT_BYTES;   // bytes of both CTAs
                     {   // {K, tK} of this CTA's tile: [K h0 | K h1 | tK h0 | tK h1]
                         const uint32_t slot = ring % NSTAGE;
                         wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                         const uint32_t dst = sRing + slot * SLOT_BYTES, full = lead_bars + 8 * (BAR_KV_FULL + slot);
-                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES);
+                        if (rank == 0) {
+                            ((volatile int *)sh->slot_kz)[slot] = kz ? 1 : 0;
+                            mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), slot_tx);
+                        }
                         const int row = rank ? t1.key_row : t0.key_row;
                         tma_load_4d_pair(dst, &prm.tm_k, full, 0, row, task.h, task.b);
                         tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_k, full, 64, row, task.h, task.b);
-                        tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_tk, full, 0, row, task.h, task.b);
-                        tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_tk, full, 64, row, task.h, task.b);
+                        if (!kz) {
+                            tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_tk, full, 0, row, task.h, task.b);
+                            tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_tk, full, 64, row, task.h, task.b);
+                        }
                         ++ring;
                     }
                     {   // this CTA's column half of {V, tV} of both tiles: [V(j0) | tV(j0) | V(j1) | tV(j1)]
                         const uint32_t slot = ring % NSTAGE;
                         wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                         const uint32_t dst = sRing + slot * SLOT_BYTES, full = lead_bars + 8 * (BAR_KV_FULL + slot);
-                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES);
+                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), slot_tx);
                         const int col = 64 * (int)rank;
                         tma_load_4d_pair(dst, &prm.tm_v, full, col, t0.key_row, task.h, task.b);
-                        tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_tv, full, col, t0.key_row, task.h, task.b);
                         tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_v, full, col, t1.key_row, task.h, task.b);
-                        tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_tv, full, col, t1.key_row, task.h, task.b);
+                        if (!kz) {
+                            tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_tv, full, col, t0.key_row, task.h, task.b);
+                            tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_tv, full, col, t1.key_row, task.h, task.b);
+                        }
                         ++ring;
                     }
                 }
@@ -221,20 +247,79 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
         if (rank == 0) {
             const bool leader = elect_one();
             const uint32_t q_lo = ((sQ >> 4) & 0x3FFF) | LBO_CANON, tq_lo = ((sTQ >> 4) & 0x3FFF) | LBO_CANON;
-            uint32_t ring = 0, nq = 0, gp = 0;   // gp = pair-steps issued so far (barrier phases)
+            uint32_t ring = 0, nq = 0, c_s = 0, c_ts = 0;   // ring items consumed; uses of the S / tS barrier sets
             for (int it = list_begin; it < list_end; ++it) {
-                const int n = (int)warp_uniform((uint32_t)prm.tasks[prm.pair_ids[it]].num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
+                const aj_task &tk = prm.tasks[prm.pair_ids[it]];
+                const int n = (int)warp_uniform((uint32_t)tk.num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
                 if (n <= 0) continue;
+                const bool primal = warp_uniform((uint32_t)tk.flags & AJ_TASK_PRIMAL_ONLY) != 0;
                 wait(BAR_Q_FULL, nq & 1);
                 ++nq;
                 tc_fence_after();
                 const int np = (n + 1) >> 1;
-                // QK of pair-step p: [S | S] first (softmax starts on it), then [tS | tS]
+                if (primal) {
+                    // ---- primal-only task: S double-buffered in the S and tS columns; ring items: K(p) = base + 2p, V(p) = base + 2p + 1
+                    const uint32_t base = ring;
+                    ring += 2 * (uint32_t)np;
+                    auto issue_S = [&](int p) {
+                        const uint32_t item = base + 2 * (uint32_t)p, slot = item % NSTAGE;
+                        wait(BAR_KV_FULL + slot, (item / NSTAGE) & 1);
+                        tc_fence_after();
+                        const uint32_t k_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
+                        const uint32_t tS = tmem + ((p & 1) ? TM_TS : TM_S);
+                        if (leader) {
+#pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks) {   // [S(j0) | S(j1)] = Q [K(j0) ; K(j1)]^T
+                                const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
+                                const uint32_t koff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
+                                mma_ss_pair(tS, q_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK, ks > 0);
+                            }
+                            tc_commit_pair(bars + 8 * ((p & 1) ? BAR_TS_FULL : BAR_S_FULL), 3);
+                            tc_commit_pair(bars + 8 * (BAR_KV_EMPTY + slot), 3);
+                            if (p + 1 == np) tc_commit_pair(bars + 8 * BAR_Q_EMPTY, 3);
+                        }
+                        __syncwarp();
+                    };
+                    issue_S(0);
+                    if (np > 1) issue_S(1);
+                    for (int p = 0; p < np; ++p) {
+                        const uint32_t item = base + 2 * (uint32_t)p + 1, vslot = item % NSTAGE;
+                        wait(BAR_KV_FULL + vslot, (item / NSTAGE) & 1);
+                        const uint32_t v_lo = (((sRing + vslot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
+                        const int buf = p & 1;
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            const uint32_t vi_lo = v_lo + ((2 * i * BLK_BYTES) >> 4);
+                            const uint32_t tP = tmem + (buf ? TM_TS : TM_S) + i * BC;
+                            const uint32_t acc = (p > 0 || i > 0) ? 1u : 0u;
+                            wait((buf ? BAR_H_FULL : BAR_P_FULL) + i, (buf ? c_ts : c_s) & 1);
+                            tc_fence_after();
+                            if (leader) {
+#pragma unroll
+                                for (int ks = 0; ks < BC / 16; ++ks)    // O += P~ V
+                                    mma_ts_pair(tmem + TM_O, tP + ks * 8, vi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, acc | (ks > 0));
+                            }
+                            __syncwarp();
+                        }
+                        if (leader) {
+                            tc_commit_pair(bars + 8 * (BAR_KV_EMPTY + vslot), 3);
+                            tc_commit_pair(bars + 8 * BAR_PV_DONE, 3);
+                        }
+                        __syncwarp();
+                        if (buf) ++c_ts; else ++c_s;
+                        if (p + 2 < np) issue_S(p + 2);       // overwrites P~(p): the pipe executes in order
+                    }
+                    continue;
+                }
+                // ---- general task.  QK of pair-step p: [S | S] first (softmax starts on it), then [tS | tS]
                 uint32_t kslot = 0, k_lo = 0;
+                bool kz_next = false;                    // key tangents of the pair-step whose S was issued last are zero
+                uint32_t t_acc = 0;                      // T has been written in this task
                 auto issue_s = [&]() {
                     kslot = ring % NSTAGE;
                     wait(BAR_KV_FULL + kslot, (ring / NSTAGE) & 1);
                     tc_fence_after();
+                    kz_next = warp_uniform((uint32_t)((volatile int *)sh->slot_kz)[kslot]) != 0;
                     k_lo = (((sRing + kslot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
                     if (leader) {
 #pragma unroll
@@ -251,17 +336,20 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 auto issue_ts = [&](bool last) {
                     const uint32_t tk_lo = k_lo + ((2 * BLK_BYTES) >> 4);
                     if (leader) {
+                        if (!kz_next) {
 #pragma unroll
-                        for (int ks = 0; ks < D / 16; ++ks) {   // [tS(j0) | tS(j1)] = Q [tK ; tK]^T + tQ [K ; K]^T
-                            const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
-                            const uint32_t koff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
-                            mma_ss_pair(tmem + TM_TS, q_lo + qoff, DESC_HI, tk_lo + koff, DESC_HI, IDESC_QK, ks > 0);
+                            for (int ks = 0; ks < D / 16; ++ks) {   // [tS(j0) | tS(j1)] = Q [tK ; tK]^T + tQ [K ; K]^T  (Eq. 43)
+                                const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
+                                const uint32_t koff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
+                                mma_ss_pair(tmem + TM_TS, q_lo + qoff, DESC_HI, tk_lo + koff, DESC_HI, IDESC_QK, ks > 0);
+                            }
                         }
+                        const uint32_t acc0 = kz_next ? 0u : 1u;    // tK = 0: tS = tQ K^T alone
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks) {
                             const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
                             const uint32_t koff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
-                            mma_ss_pair(tmem + TM_TS, tq_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK, 1);
+                            mma_ss_pair(tmem + TM_TS, tq_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK, acc0 | (ks > 0));
                         }
                         tc_commit_pair(bars + 8 * BAR_TS_FULL, 3);
                         tc_commit_pair(bars + 8 * (BAR_KV_EMPTY + kslot), 3);
@@ -271,10 +359,11 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 };
                 issue_s();
                 issue_ts(np == 1);
-                for (int p = 0; p < np; ++p, ++gp) {
+                for (int p = 0; p < np; ++p, ++c_s, ++c_ts) {
                     // Issue order P~(j0), P~(j1), S of the NEXT pair-step, H~(j0), H~(j1), tS of the next pair-step: the
                     // tensor pipe executes in order, so S(p+1) may overwrite P~(p) and tS(p+1) may overwrite H~(p), and
                     // the softmax of step p+1 runs while the pipe does the H~ MMAs and tS(p+1).
+                    const bool kz = kz_next;                // this pair-step: tV = 0, so T += P~ tV is skipped
                     const uint32_t vslot = ring % NSTAGE;
                     wait(BAR_KV_FULL + vslot, (ring / NSTAGE) & 1);
                     ++ring;
@@ -285,16 +374,19 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                         const uint32_t vi_lo = v_lo + ((2 * i * BLK_BYTES) >> 4), tvi_lo = vi_lo + (BLK_BYTES >> 4);
                         const uint32_t tP = tmem + TM_S + i * BC;
                         const uint32_t acc = (p > 0 || i > 0) ? 1u : 0u;
-                        wait(BAR_P_FULL + i, gp & 1);
+                        wait(BAR_P_FULL + i, c_s & 1);
                         tc_fence_after();
                         if (leader) {
 #pragma unroll
                             for (int ks = 0; ks < BC / 16; ++ks)    // O += P~ V
                                 mma_ts_pair(tmem + TM_O, tP + ks * 8, vi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, acc | (ks > 0));
+                            if (!kz) {
 #pragma unroll
-                            for (int ks = 0; ks < BC / 16; ++ks)    // T += P~ tV
-                                mma_ts_pair(tmem + TM_T, tP + ks * 8, tvi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, acc | (ks > 0));
+                                for (int ks = 0; ks < BC / 16; ++ks)    // T += P~ tV
+                                    mma_ts_pair(tmem + TM_T, tP + ks * 8, tvi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, t_acc | (ks > 0));
+                            }
                         }
+                        if (!kz) t_acc = 1;
                         __syncwarp();
                     }
                     if (p + 1 < np) issue_s();
@@ -302,13 +394,14 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     for (int i = 0; i < 2; ++i) {
                         const uint32_t vi_lo = v_lo + ((2 * i * BLK_BYTES) >> 4);
                         const uint32_t tH = tmem + TM_TS + i * BC;
-                        wait(BAR_H_FULL + i, gp & 1);
+                        wait(BAR_H_FULL + i, c_ts & 1);
                         tc_fence_after();
                         if (leader) {
 #pragma unroll
                             for (int ks = 0; ks < BC / 16; ++ks)    // T += H~ V
-                                mma_ts_pair(tmem + TM_T, tH + ks * 8, vi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, 1);
+                                mma_ts_pair(tmem + TM_T, tH + ks * 8, vi_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV, t_acc | (ks > 0));
                         }
+                        t_acc = 1;
                         __syncwarp();
                     }
                     if (leader) {
@@ -328,11 +421,12 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
         const float sl2 = prm.scale_log2, sc = prm.scale;
         const uint64_t sl2_2 = pack2(sl2, sl2), sc_2 = pack2(sc, sc);
         const uint32_t p_full = lead_bars + 8 * BAR_P_FULL, h_full = lead_bars + 8 * BAR_H_FULL;
-        uint32_t gp = 0;
+        uint32_t c_s = 0, c_ts = 0, c_pv = 0;                    // uses of the S / tS barrier sets, pair-steps (PV_DONE)
         for (int it = list_begin; it < list_end; ++it) {
             if (sh->abort_flag) break;
             const aj_task task = prm.tasks[prm.pair_ids[it]];
             const int n = task.num_kv_tiles;
+            const bool primal = (task.flags & AJ_TASK_PRIMAL_ONLY) != 0;
             float m_ref = M_UNSET;
             uint64_t l2[2] = {0ull, 0ull}, r2[2] = {0ull, 0ull};   // 4 partial sums each of l = sum P~ and r = sum H~
             TileCursor cur;
@@ -340,29 +434,32 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             const int np = (n + 1) >> 1;
             int cur_entry = -1;
             bool sees = false;                                   // this row is inside the current entry's row interval
-            for (int p = 0; p < np; ++p, ++gp) {
+            for (int p = 0; p < np; ++p, ++c_pv) {
                 // columns of the two tiles this row may see: inside the entry's keys and row interval
                 int valid[2];
                 {
                     const Tile t0 = cur.get();
                     cur.next();
-                    if (t0.entry != cur_entry) { cur_entry = t0.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)(rr >> 16); }
+                    if (t0.entry != cur_entry) { cur_entry = t0.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)((rr >> 16) & 0x7fffu); }
                     valid[0] = sees ? t0.valid : 0;
                     valid[1] = 0;
                     if (2 * p + 1 < n) {
                         const Tile t1 = cur.get();
                         cur.next();
-                        if (t1.entry != cur_entry) { cur_entry = t1.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)(rr >> 16); }
+                        if (t1.entry != cur_entry) { cur_entry = t1.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)((rr >> 16) & 0x7fffu); }
                         valid[1] = sees ? t1.valid : 0;
                     }
                 }
-                wait(BAR_S_FULL, gp & 1);
+                // primal-only tasks alternate between the S columns (even pair-steps) and the tS columns (odd) as S buffer
+                const bool alt = primal && (p & 1);
+                const uint32_t tm_s = alt ? TM_TS : TM_S;
+                wait(alt ? BAR_TS_FULL : BAR_S_FULL, (alt ? c_ts : c_s) & 1);
                 tc_fence_after();
                 uint32_t su[2][2][32];
-                tmem_ld32(tmem + lane_base + TM_S, su[0][0]);
-                tmem_ld32(tmem + lane_base + TM_S + 32, su[0][1]);
-                tmem_ld32(tmem + lane_base + TM_S + 64, su[1][0]);
-                tmem_ld32(tmem + lane_base + TM_S + 96, su[1][1]);
+                tmem_ld32(tmem + lane_base + tm_s, su[0][0]);
+                tmem_ld32(tmem + lane_base + tm_s + 32, su[0][1]);
+                tmem_ld32(tmem + lane_base + tm_s + 64, su[1][0]);
+                tmem_ld32(tmem + lane_base + tm_s + 96, su[1][1]);
                 tc_wait_ld(su[0][0], su[0][1]);
                 tc_wait_ld(su[1][0], su[1][1]);
 #pragma unroll
@@ -384,11 +481,12 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     const bool fresh = m_ref == M_UNSET;
                     if (__any_sync(0xffffffffu, need && !fresh)) {
                         // e^{m - m_new} applied to O, T (= A + B), l, r; every MMA of the previous pair-step must be complete
-                        wait(BAR_PV_DONE, (gp - 1) & 1);
+                        wait(BAR_PV_DONE, (c_pv - 1) & 1);
                         tc_fence_after();
                         const float f = (need && !fresh) ? ex2(m_ref - cand) : 1.f;
+                        const int ncols = primal ? 128 : 256;          // a primal-only task has no T
 #pragma unroll 1
-                        for (int cb = 0; cb < 256; cb += 32) {
+                        for (int cb = 0; cb < ncols; cb += 32) {
                             uint32_t a[32];
                             tmem_ld32(tmem + lane_base + cb, a);
                             tc_wait_ld(a);
@@ -404,6 +502,7 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 }
                 // P~ = exp2(S*s*log2e - m_ref); l += rowsum.  The bf16 pairs stay in registers for H~.
                 const uint64_t negm2 = pack2(-m_ref, -m_ref);
+                const uint32_t p_arrive = alt ? h_full : p_full;
                 uint32_t pk[2][32];
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
@@ -416,15 +515,19 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                         l2[c & 1] = fadd2(l2[c & 1], pack2(p0, p1));
                         pk[i][c] = pack_bf16(p0, p1);
                     }
-                    tmem_st32(tmem + lane_base + TM_S + i * BC, pk[i]);
+                    tmem_st32(tmem + lane_base + tm_s + i * BC, pk[i]);
                     tc_wait_st();
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(p_full + 8 * i);
+                    if (lane == 0) mbar_arrive_cluster(p_arrive + 8 * i);
+                }
+                if (primal) {                                    // no tS, no H~: the other buffer's S is next
+                    if (alt) ++c_ts; else ++c_s;
+                    continue;
                 }
                 // H~ = P~ o (s * tS); r += rowsum.  P~ is the bf16 value the MMAs see; masked columns
                 // have P~ = 0, so H~ = 0.
-                wait(BAR_TS_FULL, gp & 1);
+                wait(BAR_TS_FULL, c_ts & 1);
                 tc_fence_after();
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
@@ -447,48 +550,73 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(h_full + 8 * i);
                 }
+                ++c_s;
+                ++c_ts;
             }
             // ---- epilogue (Eq. 45) ----
             const bool store = prow < task.q_rows;
             const int64_t grow = task.q_begin + prow;
             __nv_bfloat16 *op = (__nv_bfloat16 *)prm.o.ptr + task.b * prm.o.stride_b + task.h * prm.o.stride_h + grow * prm.o.stride_n;
-            __nv_bfloat16 *tp = (__nv_bfloat16 *)prm.to.ptr + task.b * prm.to.stride_b + task.h * prm.to.stride_h + grow * prm.to.stride_n;
+            __nv_bfloat16 *tp = prm.to.ptr ? (__nv_bfloat16 *)prm.to.ptr + task.b * prm.to.stride_b + task.h * prm.to.stride_h + grow * prm.to.stride_n : nullptr;
             if (n == 0) {                                         // no key: O = 0, tO = 0, lse = -inf (R9)
                 if (store) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
-                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; ((uint4 *)tp)[c] = z; }
+                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; if (tp) ((uint4 *)tp)[c] = z; }
                     if (prm.lse) prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = -INFINITY;
                 }
                 continue;
             }
-            wait(BAR_PV_DONE, (gp - 1) & 1);
+            wait(BAR_PV_DONE, (c_pv - 1) & 1);
             tc_fence_after();
             float la, lb, lc, ld, ra, rb, rc, rd;
             unpack2(l2[0], la, lb); unpack2(l2[1], lc, ld);
             unpack2(r2[0], ra, rb); unpack2(r2[1], rc, rd);
             const float l = (la + lb) + (lc + ld), r = (ra + rb) + (rc + rd);
             const float inv = l > 0.f ? 1.f / l : 0.f, rl = r * inv;   // l = 0: the row saw no key (O = 0, tO = 0, lse = -inf)
+            if (primal) {
+                // every tangent the task touches is zero: tO = 0 exactly (written only if the caller passed `to`)
 #pragma unroll 1
-            for (int cb = 0; cb < D; cb += 32) {
-                uint32_t ao[32], at[32];
-                tmem_ld32(tmem + lane_base + TM_O + cb, ao);
-                tmem_ld32(tmem + lane_base + TM_T + cb, at);
-                tc_wait_ld(ao, at);
-                if (store) {
+                for (int cb = 0; cb < D; cb += 32) {
+                    uint32_t ao[32];
+                    tmem_ld32(tmem + lane_base + TM_O + cb, ao);
+                    tc_wait_ld(ao);
+                    if (store) {
 #pragma unroll
-                    for (int v4 = 0; v4 < 4; ++v4) {
-                        uint32_t wo[4], wt[4];
+                        for (int v4 = 0; v4 < 4; ++v4) {
+                            uint32_t wo[4];
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            const int c = v4 * 8 + 2 * e;
-                            const float o0 = __uint_as_float(ao[c]) * inv, o1 = __uint_as_float(ao[c + 1]) * inv;
-                            const float t0 = fmaf(__uint_as_float(at[c]), inv, -rl * o0);
-                            const float t1 = fmaf(__uint_as_float(at[c + 1]), inv, -rl * o1);
-                            wo[e] = pack_bf16(o0, o1);
-                            wt[e] = pack_bf16(t0, t1);
+                            for (int e = 0; e < 4; ++e) {
+                                const int c = v4 * 8 + 2 * e;
+                                wo[e] = pack_bf16(__uint_as_float(ao[c]) * inv, __uint_as_float(ao[c + 1]) * inv);
+                            }
+                            *(uint4 *)(op + cb + v4 * 8) = make_uint4(wo[0], wo[1], wo[2], wo[3]);
+                            if (tp) *(uint4 *)(tp + cb + v4 * 8) = make_uint4(0, 0, 0, 0);
                         }
-                        *(uint4 *)(op + cb + v4 * 8) = make_uint4(wo[0], wo[1], wo[2], wo[3]);
-                        *(uint4 *)(tp + cb + v4 * 8) = make_uint4(wt[0], wt[1], wt[2], wt[3]);
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int cb = 0; cb < D; cb += 32) {
+                    uint32_t ao[32], at[32];
+                    tmem_ld32(tmem + lane_base + TM_O + cb, ao);
+                    tmem_ld32(tmem + lane_base + TM_T + cb, at);
+                    tc_wait_ld(ao, at);
+                    if (store) {
+#pragma unroll
+                        for (int v4 = 0; v4 < 4; ++v4) {
+                            uint32_t wo[4], wt[4];
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const int c = v4 * 8 + 2 * e;
+                                const float o0 = __uint_as_float(ao[c]) * inv, o1 = __uint_as_float(ao[c + 1]) * inv;
+                                const float t0 = fmaf(__uint_as_float(at[c]), inv, -rl * o0);
+                                const float t1 = fmaf(__uint_as_float(at[c + 1]), inv, -rl * o1);
+                                wo[e] = pack_bf16(o0, o1);
+                                wt[e] = pack_bf16(t0, t1);
+                            }
+                            *(uint4 *)(op + cb + v4 * 8) = make_uint4(wo[0], wo[1], wo[2], wo[3]);
+                            *(uint4 *)(tp + cb + v4 * 8) = make_uint4(wt[0], wt[1], wt[2], wt[3]);
+                        }
                     }
                 }
             }

@@ -291,7 +291,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 if (cur.entry() != cur_entry) {                    // rows of this tile that may see the entry's keys
                     cur_entry = cur.entry();
                     const uint32_t rr = prm.rows[cur_entry];
-                    row_lo = (int)(rr & 0xffffu); row_hi = (int)(rr >> 16);
+                    row_lo = (int)(rr & 0xffffu); row_hi = (int)((rr >> 16) & 0x7fffu);   // bit 31: key-tangents-zero flag (CTA-pair kernel)
                 }
                 wait(BAR_S_FULL + b, (gj >> 1) & 1);
                 tc_fence_after();

@@ -34,13 +34,14 @@ static aj_status block_bounds(const aj_mask_desc &m, std::vector<int64_t> &b) {
     return AJ_OK;
 }
 
-static void push_group(Lowered &out, int64_t q0, int64_t q1, std::initializer_list<KeyRange> rs) {
+static void push_group(Lowered &out, int64_t q0, int64_t q1, std::initializer_list<KeyRange> rs, int32_t q_tz = 0) {
     out.q_begin.push_back((int32_t)q0);
     out.q_end.push_back((int32_t)q1);
+    out.q_tz.push_back(q_tz);
     for (const KeyRange &r : rs) {
         if (r.k_end <= r.k_begin) continue;
-        // merge with the previous range of this group when they touch
-        if ((int32_t)out.ranges.size() > out.range_offset.back() && out.ranges.back().k_end == r.k_begin)
+        // merge with the previous range of this group when they touch (and promise the same about their tangents)
+        if ((int32_t)out.ranges.size() > out.range_offset.back() && out.ranges.back().k_end == r.k_begin && out.ranges.back().tz == r.tz)
             out.ranges.back().k_end = r.k_end;
         else
             out.ranges.push_back(r);
@@ -52,16 +53,23 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
     out = Lowered();
     out.range_offset.push_back(0);
     std::vector<int64_t> bb;
+    const int32_t tzk = m.tangent_zero;
+    if (tzk != AJ_TANGENT_DENSE && tzk != AJ_TANGENT_CLEAN_ZERO && tzk != AJ_TANGENT_NONE)
+        return fail(AJ_ERR_INVALID_ARG, "mask: unknown tangent_zero");
+    if (tzk == AJ_TANGENT_CLEAN_ZERO && m.kind != AJ_MASK_TEACHER_FORCING && m.kind != AJ_MASK_RANGES)
+        return fail(AJ_ERR_INVALID_ARG, "mask: AJ_TANGENT_CLEAN_ZERO needs a teacher-forcing or ranges mask");
+    const int32_t all0 = tzk == AJ_TANGENT_NONE ? 1 : 0;       // every tangent is zero
+    const int32_t clean0 = tzk != AJ_TANGENT_DENSE ? 1 : 0;    // the clean half's tangents are zero
     switch (m.kind) {
     case AJ_MASK_FULL:
-        push_group(out, 0, p.Nq, {KeyRange{0, p.Nk}});
+        push_group(out, 0, p.Nq, {KeyRange{0, p.Nk, all0}}, all0);
         break;
     case AJ_MASK_BLOCK_CAUSAL: {
         if (aj_status st = block_bounds(m, bb)) return st;
         if (p.Nq != bb.back() || p.Nk != bb.back())
             return fail(AJ_ERR_INVALID_ARG, "block-causal mask: Nq and Nk must equal num_frames * frame_len");
         for (size_t i = 0; i + 1 < bb.size(); ++i)  // block i sees blocks <= i
-            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1]}});
+            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1], all0}}, all0);
         break;
     }
     case AJ_MASK_TEACHER_FORCING: {
@@ -70,10 +78,10 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
         if (p.Nq != 2 * half || p.Nk != 2 * half)
             return fail(AJ_ERR_INVALID_ARG, "teacher-forcing mask: Nq and Nk must equal 2 * num_frames * frame_len");
         for (size_t i = 0; i + 1 < bb.size(); ++i)  // clean block i -> clean blocks <= i
-            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1]}});
+            push_group(out, bb[i], bb[i + 1], {KeyRange{0, (int32_t)bb[i + 1], clean0}}, clean0);
         for (size_t i = 0; i + 1 < bb.size(); ++i)  // noisy block i -> clean blocks < i, noisy block i
             push_group(out, half + bb[i], half + bb[i + 1],
-                       {KeyRange{0, (int32_t)bb[i]}, KeyRange{(int32_t)(half + bb[i]), (int32_t)(half + bb[i + 1])}});
+                       {KeyRange{0, (int32_t)bb[i], clean0}, KeyRange{(int32_t)(half + bb[i]), (int32_t)(half + bb[i + 1]), all0}}, all0);
         break;
     }
     case AJ_MASK_RANGES: {
@@ -91,13 +99,15 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
             if (r1 > r0 && (!m.k_begin || !m.k_end)) return fail(AJ_ERR_INVALID_ARG, "ranges mask: null range arrays");
             out.q_begin.push_back(q0);
             out.q_end.push_back(q1);
+            out.q_tz.push_back(all0 || (tzk == AJ_TANGENT_CLEAN_ZERO && m.q_tangent_zero && m.q_tangent_zero[g]) ? 1 : 0);
             int32_t prev_end = 0;
             for (int r = r0; r < r1; ++r) {
                 int32_t k0 = m.k_begin[r], k1 = m.k_end[r];
                 if (k0 < 0 || k1 > p.Nk || k0 >= k1 || k0 < prev_end)
                     return fail(AJ_ERR_INVALID_ARG, "ranges mask: key ranges must be non-empty, sorted, disjoint, inside [0, Nk)");
-                if (r > r0 && out.ranges.back().k_end == k0) out.ranges.back().k_end = k1;
-                else out.ranges.push_back(KeyRange{k0, k1});
+                const int32_t tz = all0 || (tzk == AJ_TANGENT_CLEAN_ZERO && m.k_tangent_zero && m.k_tangent_zero[r]) ? 1 : 0;
+                if (r > r0 && out.ranges.back().k_end == k0 && out.ranges.back().tz == tz) out.ranges.back().k_end = k1;
+                else out.ranges.push_back(KeyRange{k0, k1, tz});
                 prev_end = k1;
             }
             out.range_offset.push_back((int32_t)out.ranges.size());
@@ -111,7 +121,7 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
         int32_t next = 0;
         rows.emplace_back(p.Nq, p.Nq);
         for (const auto &qr : rows) {
-            if (qr.first > next) push_group(out, next, qr.first, {});
+            if (qr.first > next) push_group(out, next, qr.first, {}, 1);
             next = std::max(next, qr.second);
         }
         break;
@@ -121,10 +131,12 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
     }
     out.pairs_per_head = 0;
     for (size_t g = 0; g < out.q_begin.size(); ++g) {
-        int64_t keys = 0;
-        for (int r = out.range_offset[g]; r < out.range_offset[g + 1]; ++r)
-            keys += out.ranges[r].k_end - out.ranges[r].k_begin;
-        out.pairs_per_head += keys * (int64_t)(out.q_end[g] - out.q_begin[g]);
+        const int64_t rows = out.q_end[g] - out.q_begin[g];
+        for (int r = out.range_offset[g]; r < out.range_offset[g + 1]; ++r) {
+            const int64_t pairs = rows * (int64_t)(out.ranges[r].k_end - out.ranges[r].k_begin);
+            out.pairs_per_head += pairs;
+            out.pair_class[!out.ranges[r].tz ? 2 : out.q_tz[g] ? 0 : 1] += pairs;
+        }
     }
     return AJ_OK;
 }
@@ -143,14 +155,18 @@ void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_
     for (const KeyRange &r : low.ranges) {
         ent.k_begin.push_back(r.k_begin); ent.k_end.push_back(r.k_end);
         ent.row_begin.push_back(0); ent.row_end.push_back(tile_q);
+        ent.k_tz.push_back(r.tz);
     }
     for (int32_t b = 0; b < p.B; ++b)
         for (int32_t h = 0; h < p.H; ++h)
             for (size_t g = 0; g < low.q_begin.size(); ++g) {
                 int32_t r0 = low.range_offset[g], r1 = low.range_offset[g + 1];
                 int32_t kv_tiles = 0;
-                for (int r = r0; r < r1; ++r)
+                bool primal = low.q_tz[g] != 0;
+                for (int r = r0; r < r1; ++r) {
                     kv_tiles += (low.ranges[r].k_end - low.ranges[r].k_begin + tile_k - 1) / tile_k;
+                    primal = primal && low.ranges[r].tz;
+                }
                 // query tiles start at the group start (R8); the last one may be partial
                 for (int32_t q = low.q_begin[g]; q < low.q_end[g]; q += tile_q) {
                     aj_task t;
@@ -158,6 +174,7 @@ void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_
                     t.q_rows = std::min(tile_q, low.q_end[g] - q);
                     t.range_begin = r0; t.range_count = r1 - r0;
                     t.num_kv_tiles = kv_tiles; t.group = (int32_t)g;
+                    t.flags = primal ? AJ_TASK_PRIMAL_ONLY : 0;
                     tasks.push_back(t);
                 }
             }
@@ -173,7 +190,7 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
     for (size_t g = 0; g < ng; ++g) order[g] = g;
     std::sort(order.begin(), order.end(), [&](size_t a, size_t b) { return low.q_begin[a] < low.q_begin[b]; });
     struct Run { int32_t lo, hi; };
-    struct TileInfo { int32_t q_begin, q_rows, ent_begin, ent_count, kv_tiles; };
+    struct TileInfo { int32_t q_begin, q_rows, ent_begin, ent_count, kv_tiles, flags; };
     std::vector<TileInfo> tiles;
     size_t first = 0;                                  // first group (in row order) that may reach this tile
     std::vector<int32_t> cuts;
@@ -193,26 +210,30 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
         }
         std::sort(cuts.begin(), cuts.end());
         cuts.erase(std::unique(cuts.begin(), cuts.end()), cuts.end());
-        TileInfo ti{t0, t1 - t0, (int32_t)ent.size(), 0, 0};
+        TileInfo ti{t0, t1 - t0, (int32_t)ent.size(), 0, 0, 0};
         size_t open_begin = ent.size();                // entries of the key interval being extended
         prev_runs.clear();
-        int32_t prev_end = -1;
+        int32_t prev_end = -1, prev_tz = -1;
+        bool primal = true;                            // tQ of every row and tK, tV of every key are structurally zero
+        for (size_t i = first; i < last; ++i) primal = primal && low.q_tz[order[i]];
         for (size_t c = 0; c + 1 < cuts.size(); ++c) {
             const int32_t a = cuts[c], bnd = cuts[c + 1];
             // rows of the tile that see keys [a, bnd): union over the groups whose ranges cover it, as maximal runs
             runs.clear();
+            int32_t tz = 1;                            // zero only if every covering range says so
             for (size_t i = first; i < last; ++i) {
                 const size_t g = order[i];
                 bool covered = false;
                 for (int r = low.range_offset[g]; r < low.range_offset[g + 1] && !covered; ++r)
-                    covered = low.ranges[r].k_begin <= a && bnd <= low.ranges[r].k_end;
+                    if ((covered = low.ranges[r].k_begin <= a && bnd <= low.ranges[r].k_end)) tz = tz && low.ranges[r].tz;
                 if (!covered) continue;
                 const int32_t lo = std::max(low.q_begin[g], t0) - t0, hi = std::min(low.q_end[g], t1) - t0;
                 if (!runs.empty() && runs.back().hi == lo) runs.back().hi = hi;
                 else runs.push_back(Run{lo, hi});
             }
             if (runs.empty()) { prev_runs.clear(); prev_end = -1; continue; }
-            bool same = prev_end == a && runs.size() == prev_runs.size();
+            primal = primal && tz;
+            bool same = prev_end == a && prev_tz == tz && runs.size() == prev_runs.size();
             for (size_t i = 0; same && i < runs.size(); ++i) same = runs[i].lo == prev_runs[i].lo && runs[i].hi == prev_runs[i].hi;
             if (same) {                                // same rows as the interval before and adjacent keys: extend
                 for (size_t e = open_begin; e < ent.size(); ++e) ent.k_end[e] = bnd;
@@ -221,11 +242,14 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
                 for (const Run &r : runs) {
                     ent.k_begin.push_back(a); ent.k_end.push_back(bnd);
                     ent.row_begin.push_back(r.lo); ent.row_end.push_back(r.hi);
+                    ent.k_tz.push_back(tz);
                 }
             }
             prev_runs = runs;
             prev_end = bnd;
+            prev_tz = tz;
         }
+        ti.flags = primal ? AJ_TASK_PRIMAL_ONLY : 0;
         ti.ent_count = (int32_t)ent.size() - ti.ent_begin;
         for (int32_t e = ti.ent_begin; e < ti.ent_begin + ti.ent_count; ++e)
             ti.kv_tiles += (ent.k_end[e] - ent.k_begin[e] + tile_k - 1) / tile_k;
@@ -237,25 +261,49 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
                 aj_task t;
                 t.b = b; t.h = h; t.q_begin = ti.q_begin; t.q_rows = ti.q_rows;
                 t.range_begin = ti.ent_begin; t.range_count = ti.ent_count;
-                t.num_kv_tiles = ti.kv_tiles; t.group = -1;
+                t.num_kv_tiles = ti.kv_tiles; t.group = -1; t.flags = ti.flags;
                 tasks.push_back(t);
             }
     order_tasks(tasks);
 }
 
+// Cost of a task on a CTA pair in units of a tenth of a full pair-step (two key tiles, all 6 contractions = 48 MMAs):
+// a pair-step whose keys have zero tangents runs 32 MMAs, a primal-only one 16 (but is bound by the exponentials of
+// its softmax, not by the MMAs); the constant covers the Q load and the epilogue.
+static int64_t task_cost(const aj_task &t, const Entries &ent, int32_t tile_k) {
+    constexpr int64_t W_FULL = 10, W_KEYZERO = 7, W_PRIMAL = 5, W_TASK = 10;
+    const int64_t steps = (t.num_kv_tiles + 1) / 2;
+    if (t.flags & AJ_TASK_PRIMAL_ONLY) return W_TASK + W_PRIMAL * steps;
+    int64_t cost = W_TASK, tile = 0;
+    bool step_tz = true;
+    for (int32_t e = t.range_begin; e < t.range_begin + t.range_count; ++e) {
+        const int64_t n = (ent.k_end[e] - ent.k_begin[e] + tile_k - 1) / tile_k;
+        const bool tz = !ent.k_tz.empty() && ent.k_tz[e];
+        for (int64_t i = 0; i < n; ++i, ++tile) {
+            if ((tile & 1) == 0) step_tz = tz;
+            else { step_tz = step_tz && tz; cost += step_tz ? W_KEYZERO : W_FULL; }
+        }
+    }
+    if (tile & 1) cost += step_tz ? W_KEYZERO : W_FULL;
+    return cost;
+}
+
 // Static list scheduling of the tasks onto `num_pairs` workers (CTA pairs): the tasks are taken head by head ((b, h) major,
-// longest first inside a head) and each goes to the pair that is free first under the cost model (pair-steps plus a
-// constant for the Q load and epilogue).  All pairs therefore stream the K/V of the same head at the same time (one
+// most expensive first inside a head) and each goes to the pair that is free first under the cost model above.
+// All pairs therefore stream the K/V of the same head at the same time (one
 // head's K, tK, V, tV stay in L2), heads overlap only at their boundaries, and because the last head ends with its
 // shortest tasks the pairs finish within about one short task of each other.
-void assign_workers(const std::vector<aj_task> &tasks, int num_pairs, std::vector<int32_t> &off, std::vector<int32_t> &ids) {
+void assign_workers(const std::vector<aj_task> &tasks, const Entries &ent, int32_t tile_k, int num_pairs,
+                    std::vector<int32_t> &off, std::vector<int32_t> &ids) {
+    std::vector<int64_t> cost(tasks.size());
+    for (size_t t = 0; t < tasks.size(); ++t) cost[t] = task_cost(tasks[t], ent, tile_k);
     std::vector<int32_t> order(tasks.size());
     for (size_t t = 0; t < tasks.size(); ++t) order[t] = (int32_t)t;
     std::stable_sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
         const aj_task &a = tasks[x], &c = tasks[y];
         if (a.b != c.b) return a.b < c.b;
         if (a.h != c.h) return a.h < c.h;
-        return a.num_kv_tiles > c.num_kv_tiles;
+        return cost[x] > cost[y];
     });
     std::vector<std::vector<int32_t>> lists(num_pairs);
     std::vector<std::pair<int64_t, int>> heap;            // (-busy-until, -pair): max-heap picks the pair free first
@@ -265,7 +313,7 @@ void assign_workers(const std::vector<aj_task> &tasks, int num_pairs, std::vecto
         std::pop_heap(heap.begin(), heap.end());
         auto &top = heap.back();
         lists[-top.second].push_back(t);
-        top.first -= (tasks[t].num_kv_tiles + 1) / 2 + 1;
+        top.first -= cost[t];
         std::push_heap(heap.begin(), heap.end());
     }
     off.assign(1, 0);
@@ -362,12 +410,24 @@ aj_status attn_jvp_schedule_entries(const aj_schedule *s, int32_t *num_entries, 
     return AJ_OK;
 }
 
+aj_status attn_jvp_schedule_entry_flags(const aj_schedule *s, int32_t *key_tangent_zero) {
+    if (!s || !key_tangent_zero) return aj::fail(AJ_ERR_INVALID_ARG, "schedule or output is NULL");
+    std::copy(s->entries.k_tz.begin(), s->entries.k_tz.end(), key_tangent_zero);
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_pair_classes(const aj_schedule *s, int64_t pairs[3]) {
+    if (!s || !pairs) return aj::fail(AJ_ERR_INVALID_ARG, "schedule or output is NULL");
+    for (int i = 0; i < 3; ++i) pairs[i] = s->low.pair_class[i];
+    return AJ_OK;
+}
+
 aj_status attn_jvp_schedule_assign(const aj_schedule *s, int32_t num_workers, int32_t *worker_offset, int32_t *task_ids) {
     if (!s) return aj::fail(AJ_ERR_INVALID_ARG, "schedule is NULL");
     if (num_workers <= 0 || !worker_offset || !task_ids) return aj::fail(AJ_ERR_INVALID_ARG, "num_workers must be > 0 and the output arrays non-NULL");
     try {
         std::vector<int32_t> off, ids;
-        aj::assign_workers(s->tasks, num_workers, off, ids);
+        aj::assign_workers(s->tasks, s->entries, s->tile_k, num_workers, off, ids);
         std::copy(off.begin(), off.end(), worker_offset);
         std::copy(ids.begin(), ids.end(), task_ids);
     } catch (const std::bad_alloc &) {
@@ -377,6 +437,6 @@ aj_status attn_jvp_schedule_assign(const aj_schedule *s, int32_t num_workers, in
 }
 
 const char *attn_jvp_last_error(void) { return aj::last_error_cstr(); }
-const char *attn_jvp_version(void) { return "attn_jvp 0.1 (sm_100a)"; }
+const char *attn_jvp_version(void) { return "attn_jvp 0.2 (sm_100a)"; }
 
 }  // extern "C"

@@ -33,6 +33,7 @@ class Workload:
     dtype: str           # "bf16" | "fp32"
     tangent_std: float
     seed: int = 0
+    clean_tangent_zero: bool = False   # teacher forcing: tQ, tK, tV rows of the clean half are zero
 
     @property
     def block_len(self) -> int:
@@ -75,11 +76,18 @@ WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
 ]}
 CONFIG_ORDER: List[str] = list(WORKLOADS)
 
+# SURVEY.md section 8(f) "next" rows, measured separately from the BASELINE.json configs.
+# N1: the real TF-sCM call: "The tangent of the clean context is zero" -> configs[1] with zero clean tangents.
+EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
+    Workload("wan13b_tf_framewise_cleanzero", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, True),
+    Workload("wan13b_tf_chunkwise_cleanzero", 1, 12, 128, "teacher_forcing", 1560, 21, 3, "bf16", 0.1, 0, True),
+]}
+
 
 def scaled_down(w: Workload, frame_len: int, num_frames: int = 0, H: int = 0, B: int = 0) -> Workload:
     """Same structure, smaller extent (parity cases the oracle finishes in seconds)."""
     return Workload(f"{w.name}@L{frame_len}", B or w.B, H or w.H, w.d, w.mask, frame_len,
-                    num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed)
+                    num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed, w.clean_tangent_zero)
 
 
 def make_inputs(w: Workload, device: str = "cpu", pin: bool = False):
@@ -92,6 +100,9 @@ def make_inputs(w: Workload, device: str = "cpu", pin: bool = False):
         x = torch.randn(shape, generator=g, dtype=torch.float32)
         if i >= 3:
             x.mul_(w.tangent_std)
+            if w.clean_tangent_zero:
+                assert w.mask == "teacher_forcing"
+                x[:, :, :w.N // 2] = 0.0          # the packed sequence is [clean | noisy]
         x = x.to(w.torch_dtype)
         if device != "cpu":
             x = x.to(device)

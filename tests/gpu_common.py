@@ -16,9 +16,12 @@ def mask_kind(w: Workload) -> int:
             "full": aj.AJ_MASK_FULL}[w.mask]
 
 
-def make_plan(w: Workload, kernel: int = aj.AJ_KERNEL_AUTO, scale: float = 0.0):
+def make_plan(w: Workload, kernel: int = aj.AJ_KERNEL_AUTO, scale: float = 0.0, tangent_zero=None):
+    """tangent_zero: an aj_tangent_zero promise; default = what the workload's data guarantees."""
     prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32, scale)
-    mask, keep = aj.make_mask(mask_kind(w), w.frame_len, w.num_frames, w.chunk_frames)
+    if tangent_zero is None:
+        tangent_zero = aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE
+    mask, keep = aj.make_mask(mask_kind(w), w.frame_len, w.num_frames, w.chunk_frames, tangent_zero=tangent_zero)
     plan = aj.attn_jvp_plan_create(prob, mask)
     if kernel != aj.AJ_KERNEL_AUTO:
         aj.attn_jvp_plan_set_kernel(plan, kernel)

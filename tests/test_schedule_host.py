@@ -40,7 +40,7 @@ def _schedule(w: Workload, tile_q: int, tile_k: int):
 
 def test_library_exports_every_declared_symbol():
     header = open(os.path.join(ROOT, "include", "attn_jvp.h")).read()
-    declared = set(re.findall(r"\b(attn_jvp_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(attn_(?:jvp_)?[a-z_]+)\s*\(", header))
     assert declared == set(aj.SYMBOLS)
     lib = ctypes.CDLL(aj.LIB_PATH)
     for name in declared:
@@ -49,10 +49,10 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(aj.aj_task) == 32
+    assert ctypes.sizeof(aj.aj_task) == 36
     assert ctypes.sizeof(aj.aj_problem) == 28
     assert ctypes.sizeof(aj.aj_tensor) == 32
-    assert ctypes.sizeof(aj.aj_mask_desc) == 24 + 5 * ctypes.sizeof(ctypes.c_void_p)
+    assert ctypes.sizeof(aj.aj_mask_desc) == 32 + 7 * ctypes.sizeof(ctypes.c_void_p)
 
 
 @pytest.mark.parametrize("mask,L,F,cf", [
@@ -306,3 +306,100 @@ def test_worker_assignment_small_and_errors(workers):
     assert aj.lib().attn_jvp_schedule_assign(s, 0, None, None) == aj.AJ_ERR_INVALID_ARG
     assert aj.lib().attn_jvp_schedule_assign(None, 2, None, None) == aj.AJ_ERR_INVALID_ARG
     aj.attn_jvp_schedule_destroy(s)
+
+
+# ---------------------------------------------------------------------------------------------- structural-zero tangents
+def _classes_by_brute_force(want, q_zero, k_zero):
+    """Pairs needing 2 / 4 / 6 contractions from the rasterised mask and per-token zero-tangent flags."""
+    qz, kz = np.asarray(q_zero, bool)[:, None], np.asarray(k_zero, bool)[None, :]
+    return [int((want & qz & kz).sum()), int((want & ~qz & kz).sum()), int((want & ~kz).sum())]
+
+
+@pytest.mark.parametrize("L,F,cf", [(16, 3, 1), (10, 6, 3), (7, 4, 2), (3, 5, 1)])
+@pytest.mark.parametrize("tile_q,tile_k", [(16, 32), (8, 4), (256, 64), (5, 3)])
+def test_clean_zero_flags_follow_the_clean_half(oracle, L, F, cf, tile_q, tile_k):
+    """AJ_TANGENT_CLEAN_ZERO on a teacher-forcing mask: an entry is flagged iff all its keys are clean, a
+    task is primal-only iff all its rows are clean; the mask itself does not change."""
+    w = Workload("t", 1, 1, 64, "teacher_forcing", L, F, cf, "fp32", 1.0)
+    half = w.N // 2
+    prob = aj.make_problem(1, 1, w.N, w.N, w.d, aj.AJ_FP32)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, L, F, cf, tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO)
+    want = oracle.dense_mask(oracle_mask(w), w.N, w.N)
+    clean = np.arange(w.N) < half
+    for tiling in (aj.AJ_TILING_PACKED, aj.AJ_TILING_PER_GROUP):
+        s = aj.attn_jvp_schedule_create_tiled(prob, m, tile_q, tile_k, tiling)
+        info, got, ent = aj.attn_jvp_schedule_info(s), aj.attn_jvp_schedule_get(s), aj.attn_jvp_schedule_entries(s)
+        flags, classes = aj.attn_jvp_schedule_entry_flags(s), aj.attn_jvp_schedule_pair_classes(s)
+        aj.attn_jvp_schedule_destroy(s)
+        if tiling == aj.AJ_TILING_PACKED:
+            _check_packed(want, w.N, info, got, ent, tile_q, tile_k)
+        assert classes == _classes_by_brute_force(want, clean, clean) and sum(classes) == info[3]
+        for t in got["tasks"]:
+            all_clean = t.q_begin + t.q_rows <= half
+            assert bool(t.flags & aj.AJ_TASK_PRIMAL_ONLY) == all_clean
+            for e in range(t.range_begin, t.range_begin + t.range_count):
+                assert bool(flags[e]) == (ent["k_end"][e] <= half)     # no entry mixes clean and noisy keys
+                assert ent["k_end"][e] <= half or ent["k_begin"][e] >= half
+
+
+def test_tangent_none_marks_everything_and_dense_marks_nothing():
+    for kind, args in [(aj.AJ_MASK_TEACHER_FORCING, (16, 3, 1)), (aj.AJ_MASK_BLOCK_CAUSAL, (16, 6, 2)), (aj.AJ_MASK_FULL, ())]:
+        prob = aj.make_problem(1, 2, 96, 96, 64, aj.AJ_FP32)
+        for tz, want_flag in [(aj.AJ_TANGENT_NONE, 1), (aj.AJ_TANGENT_DENSE, 0)]:
+            m, keep = aj.make_mask(kind, *args, tangent_zero=tz)
+            s = aj.attn_jvp_schedule_create_tiled(prob, m, 32, 16, aj.AJ_TILING_PACKED)
+            pairs = aj.attn_jvp_schedule_info(s)[3]
+            assert all(f == want_flag for f in aj.attn_jvp_schedule_entry_flags(s))
+            assert all((t.flags & aj.AJ_TASK_PRIMAL_ONLY) == want_flag for t in aj.attn_jvp_schedule_get(s)["tasks"])
+            assert aj.attn_jvp_schedule_pair_classes(s) == ([pairs, 0, 0] if want_flag else [0, 0, pairs])
+            aj.attn_jvp_schedule_destroy(s)
+    bc, _ = aj.make_mask(aj.AJ_MASK_BLOCK_CAUSAL, 16, 6, 2, tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO)   # no clean half
+    _expect(aj.AJ_ERR_INVALID_ARG, aj.attn_jvp_schedule_create, aj.make_problem(1, 1, 96, 96, 64, aj.AJ_FP32), bc, 16, 32)
+    bad, _ = aj.make_mask(aj.AJ_MASK_FULL, tangent_zero=5)
+    _expect(aj.AJ_ERR_INVALID_ARG, aj.attn_jvp_schedule_create, aj.make_problem(1, 1, 96, 96, 64, aj.AJ_FP32), bad, 16, 32)
+
+
+def test_ranges_mask_with_per_group_and_per_range_zero_flags(oracle):
+    # keys [0, 20) have zero tangents; groups 0 and 1 have zero tQ.  Adjacent ranges with different flags must not merge.
+    groups = [(0, 12, [(0, 10), (10, 20)]), (12, 20, [(0, 20), (20, 30)]), (20, 40, [(5, 20), (20, 25), (30, 48)])]
+    qz, kz = [1, 1, 0], [1, 1, 1, 0, 1, 0, 0]
+    prob = aj.make_problem(1, 1, 40, 48, 64, aj.AJ_FP32)
+    m, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups, tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO, q_tangent_zero=qz, k_tangent_zero=kz)
+    want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
+    q_zero, k_zero = np.arange(40) < 20, np.arange(48) < 20
+    for tile_q, tile_k in [(8, 4), (16, 8), (64, 64), (3, 5)]:
+        s = aj.attn_jvp_schedule_create_tiled(prob, m, tile_q, tile_k, aj.AJ_TILING_PACKED)
+        info, got, ent = aj.attn_jvp_schedule_info(s), aj.attn_jvp_schedule_get(s), aj.attn_jvp_schedule_entries(s)
+        flags, classes = aj.attn_jvp_schedule_entry_flags(s), aj.attn_jvp_schedule_pair_classes(s)
+        aj.attn_jvp_schedule_destroy(s)
+        _check_packed(want, 40, info, got, ent, tile_q, tile_k)
+        assert classes == _classes_by_brute_force(want, q_zero, k_zero)
+        for t in got["tasks"]:
+            es = range(t.range_begin, t.range_begin + t.range_count)
+            for e in es:
+                assert bool(flags[e]) == (ent["k_end"][e] <= 20)
+            assert bool(t.flags & aj.AJ_TASK_PRIMAL_ONLY) == (t.q_begin + t.q_rows <= 20 and all(flags[e] for e in es))
+    # the flags are ignored unless the descriptor says CLEAN_ZERO
+    m2, keep2 = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups, q_tangent_zero=qz, k_tangent_zero=kz)
+    s = aj.attn_jvp_schedule_create_tiled(prob, m2, 8, 4, aj.AJ_TILING_PACKED)
+    assert not any(aj.attn_jvp_schedule_entry_flags(s))
+    aj.attn_jvp_schedule_destroy(s)
+
+
+def test_worker_assignment_weights_cheaper_pair_steps_on_config_2_clean_zero():
+    w = WORKLOADS["wan13b_tf_framewise"]
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, w.frame_len, w.num_frames, w.chunk_frames, tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO)
+    s = aj.attn_jvp_schedule_create_tiled(prob, m, 256, 64, aj.AJ_TILING_PACKED)
+    tasks = aj.attn_jvp_schedule_get(s)["tasks"]
+    n, C = w.num_blocks, w.block_len
+    assert aj.attn_jvp_schedule_pair_classes(s) == [n * (n + 1) // 2 * C * C, n * (n - 1) // 2 * C * C, n * C * C]
+    assert sum(1 for t in tasks if t.flags & aj.AJ_TASK_PRIMAL_ONLY) == w.H * (w.N // 2 // 256)    # 127 all-clean tiles per head
+    off, ids = aj.attn_jvp_schedule_assign(s, 74)
+    aj.attn_jvp_schedule_destroy(s)
+    assert sorted(ids) == list(range(len(tasks)))
+    # primal-only tasks cost about half a full task per pair-step, so a worker's share of key tiles is no longer equal:
+    # workers holding more primal-only tasks stream more tiles
+    tiles = [sum(tasks[i].num_kv_tiles for i in ids[off[k]:off[k + 1]]) for k in range(74)]
+    primal = [sum(tasks[i].num_kv_tiles for i in ids[off[k]:off[k + 1]] if tasks[i].flags & 1) for k in range(74)]
+    assert np.corrcoef(tiles, primal)[0, 1] > 0.5
