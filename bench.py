@@ -42,6 +42,8 @@ FALLBACK_PEAKS = {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_g
 def pair_classes(w: Workload):
     """Unmasked pairs per head needing 2 / 4 / 6 length-d contractions (accounting only).  Dense tangents: all 6.
     Zero clean tangents: clean x clean pairs need S and P V only, noisy x clean pairs also tQ K^T and H V."""
+    if w.no_tangents:
+        return [w.unmasked_pairs_per_head, 0, 0]
     if not w.clean_tangent_zero:
         return [0, 0, w.unmasked_pairs_per_head]
     n, C = w.num_blocks, w.block_len
@@ -152,12 +154,12 @@ def time_oracle_sample(w: Workload, inputs, budget_s: float, seed: int = 0):
     args = [x[0, 0].float().numpy() for x in inputs]
     scale = 1.0 / float(np.sqrt(w.d))
     rng = np.random.default_rng(seed)
-    pilot = np.sort(rng.integers(0, w.N, size=64))
+    pilot = np.sort(rng.integers(0, w.num_queries, size=64))
     t0 = time.perf_counter()
     oracle.attn_jvp_head(om, *args, scale, pilot)
     dt = max(time.perf_counter() - t0, 1e-6)
-    nrows = int(min(max(64, budget_s / dt * 64), 4 * w.N))
-    rows = np.sort(rng.integers(0, w.N, size=nrows))
+    nrows = int(min(max(64, budget_s / dt * 64), 4 * w.num_queries))
+    rows = np.sort(rng.integers(0, w.num_queries, size=nrows))
     t0 = time.perf_counter()
     oracle.attn_jvp_head(om, *args, scale, rows)
     dt = time.perf_counter() - t0
@@ -197,8 +199,10 @@ def workload_config(w: Workload):
     return {"workload": w.name, "B": w.B, "H": w.H, "d": w.d, "N": w.N, "mask": w.mask, "frame_len": w.frame_len,
             "num_frames": w.num_frames, "chunk_frames": w.chunk_frames, "input_dtype": w.dtype,
             "unmasked_pairs_per_head": w.unmasked_pairs_per_head,
-            "tangent_zero": "clean" if w.clean_tangent_zero else "none",
-            "flop_convention": ("2*d per contraction actually needed per unmasked pair (2, 4 or 6 of them: zero clean tangents)"
+            "Nq": w.num_queries,
+            "tangents": "none (forward only)" if w.no_tangents else "zero on the clean half" if w.clean_tangent_zero else "dense",
+            "flop_convention": ("4*d per unmasked pair (S and P V only)" if w.no_tangents else
+                                "2*d per contraction actually needed per unmasked pair (2, 4 or 6 of them: zero clean tangents)"
                                 if w.clean_tangent_zero else "12*d per unmasked pair"),
             "l2": "no flush: the six inputs (%.2f GB) are larger than the 126 MB L2" %
                   (6 * w.B * w.H * w.N * w.d * (2 if w.dtype == "bf16" else 4) / 1e9)}
@@ -251,9 +255,9 @@ def run_cuda(args, w: Workload):
     stream = torch.cuda.current_stream()
     kind = {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL,
             "full": aj.AJ_MASK_FULL}[w.mask]
-    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32)
-    mask, keep = aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames,
-                              tangent_zero=aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE)
+    prob = aj.make_problem(w.B, w.H, w.num_queries, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32)
+    tz = aj.AJ_TANGENT_NONE if w.no_tangents else aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE
+    mask, keep = aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames, tangent_zero=tz)
     t0 = time.perf_counter()
     plan = aj.attn_jvp_plan_create(prob, mask)
     plan_ms = 1e3 * (time.perf_counter() - t0)
@@ -263,13 +267,16 @@ def run_cuda(args, w: Workload):
 
     # every rank draws its own head shard (seed + rank): weak scaling, no exchange
     wr = Workload(w.name, w.B, w.H, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std,
-                  w.seed + rank, w.clean_tangent_zero)
-    host = make_inputs(wr, pin=True)
-    devin = [x.to(dev, non_blocking=True) for x in host]
-    o, to = torch.empty_like(devin[0]), torch.empty_like(devin[0])
-    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device=dev)
-    h_o, h_to = torch.empty_like(host[0]).pin_memory(), torch.empty_like(host[0]).pin_memory()
-    h_lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
+                  w.seed + rank, w.clean_tangent_zero, w.no_tangents, w.Nq)
+    host_all = make_inputs(wr, pin=True)
+    host = host_all[:3] + [None, None, None] if w.no_tangents else host_all   # the forward-only call takes no tangents
+    devin = [None if x is None else x.to(dev, non_blocking=True) for x in host]
+    o = torch.empty_like(devin[0])
+    to = None if w.no_tangents else torch.empty_like(devin[0])
+    lse = torch.empty((w.B, w.H, w.num_queries), dtype=torch.float32, device=dev)
+    h_o = torch.empty_like(host[0]).pin_memory()
+    h_to = None if w.no_tangents else torch.empty_like(host[0]).pin_memory()
+    h_lse = torch.empty((w.B, w.H, w.num_queries), dtype=torch.float32).pin_memory()
     torch.cuda.synchronize()
     flops = flops_per_call(w)
     K, W = args.steps, args.warmup
@@ -315,8 +322,8 @@ def run_cuda(args, w: Workload):
     torch.cuda.synchronize()
     barrier(inited)
     e2e_ms_all, e2e_flops_all = aggregate(e0.elapsed_time(e1), flops * K, inited, dev)
-    h2d = sum(x.numel() * x.element_size() for x in host)
-    d2h = h_o.numel() * h_o.element_size() * 2 + h_lse.numel() * 4
+    h2d = sum(x.numel() * x.element_size() for x in host if x is not None)
+    d2h = h_o.numel() * h_o.element_size() * (1 if w.no_tangents else 2) + h_lse.numel() * 4
 
     aj.attn_jvp_plan_destroy(plan)
     if rank != 0:
@@ -331,7 +338,7 @@ def run_cuda(args, w: Workload):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "config": workload_config(w),
-        "tokens_per_s": world * w.B * w.N / (total_ms_all / K * 1e-3),
+        "tokens_per_s": world * w.B * w.num_queries / (total_ms_all / K * 1e-3),
         "kernel": {1: "simt_fp32", 2: "tcgen05_umma", 3: "tcgen05_umma_cta_pair"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
         "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
         "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
@@ -345,10 +352,10 @@ def run_cuda(args, w: Workload):
                      "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
                      "flops_per_launch": flops},
     }
-    if w.clean_tangent_zero:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
+    if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
     if world == 1 and not args.no_cpu_baseline:
-        tf, dt, nrows, cores = time_oracle_sample(w, host, args.cpu_budget_s)
+        tf, dt, nrows, cores = time_oracle_sample(w, host_all, args.cpu_budget_s)
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{nrows} uniformly sampled query rows of head (0,0), all their allowed "
                                           f"keys, {dt:.1f} s", "extrapolated_full_config_s": flops / (tf * 1e12)}

@@ -215,7 +215,9 @@ aj_status attn_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, 
  * [B,H,Nq], may be NULL).  Copies the six inputs to plan-owned device staging buffers (allocated on
  * first use), runs attn_jvp_fwd, copies o, to, lse back, all asynchronously on `cuda_stream`; the
  * caller synchronises the stream before reading the outputs.  Pinned host memory is needed for the
- * copies to overlap; pageable memory works but is staged by the runtime.
+ * copies to overlap; pageable memory works but is staged by the runtime.  The heads are processed one by one (copy-in,
+ * kernel and copy-out of neighbouring heads overlap on three streams).  AJ_TANGENT_NONE plans accept tq = tk = tv = to =
+ * NULL (all four): only q, k, v go up and o, lse come back.
  */
 aj_status attn_jvp_fwd_host(aj_plan *plan, const void *q, const void *k, const void *v, const void *tq,
                             const void *tk, const void *tv, void *o, void *to, float *lse,

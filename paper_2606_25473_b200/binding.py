@@ -296,9 +296,10 @@ def attn_fwd(plan, q, k, v, o, lse=None, stream: int = 0) -> None:
 
 
 def attn_jvp_fwd_host(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
-    """Host tensors (contiguous [B,H,N,d], ideally pinned); copies + kernel are enqueued on `stream`."""
+    """Host tensors (contiguous [B,H,N,d], ideally pinned); copies + kernel are enqueued on `stream`.
+    tq, tk, tv, to may be None on AJ_TANGENT_NONE plans."""
     for x in (q, k, v, tq, tk, tv, o, to):
-        if x.is_cuda or not x.is_contiguous():
+        if x is not None and (x.is_cuda or not x.is_contiguous()):
             raise ValueError("attn_jvp_fwd_host expects contiguous host tensors")
-    _check(lib().attn_jvp_fwd_host(plan, *[x.data_ptr() for x in (q, k, v, tq, tk, tv, o, to)],
+    _check(lib().attn_jvp_fwd_host(plan, *[None if x is None else x.data_ptr() for x in (q, k, v, tq, tk, tv, o, to)],
                                    None if lse is None else lse.data_ptr(), stream))

@@ -351,8 +351,9 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
                             const void *tv, void *o, void *to, float *lse, void *cuda_stream) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
     const void *in[6] = {q, k, v, tq, tk, tv};
-    for (const void *x : in) if (!x) return fail(AJ_ERR_INVALID_ARG, "a host input pointer is NULL");
-    if (!o || !to) return fail(AJ_ERR_INVALID_ARG, "a host output pointer is NULL");
+    const bool no_tangents = p->mask.tangent_zero == AJ_TANGENT_NONE && !tq && !tk && !tv && !to;   // forward only
+    for (int i = 0; i < (no_tangents ? 3 : 6); ++i) if (!in[i]) return fail(AJ_ERR_INVALID_ARG, "a host input pointer is NULL");
+    if (!o || (!to && !no_tangents)) return fail(AJ_ERR_INVALID_ARG, "a host output pointer is NULL");
     const aj_problem &pr = p->problem;
     const size_t eb = pr.dtype == AJ_BF16 ? 2 : 4;
     const int nheads = pr.B * pr.H;
@@ -361,9 +362,9 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
     const size_t lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSuccess;
-    for (int i = 0; i < 6 && e == cudaSuccess; ++i)
+    for (int i = 0; i < (no_tangents ? 3 : 6) && e == cudaSuccess; ++i)
         if (!p->d_in[i]) e = cudaMalloc(&p->d_in[i], (i == 0 || i == 3) ? nq_bytes : nk_bytes);
-    for (int i = 0; i < 2 && e == cudaSuccess; ++i)
+    for (int i = 0; i < (no_tangents ? 1 : 2) && e == cudaSuccess; ++i)
         if (!p->d_out[i]) e = cudaMalloc(&p->d_out[i], nq_bytes);
     if (e == cudaSuccess && !p->d_lse) e = cudaMalloc(&p->d_lse, lse_bytes);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for staging") : cuda_fail(e, "staging allocation");
@@ -392,7 +393,7 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_begin, 0);
     if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
     for (int hd = 0; hd < nheads; ++hd) {
-        for (int i = 0; i < 6 && e == cudaSuccess; ++i) {
+        for (int i = 0; i < (no_tangents ? 3 : 6) && e == cudaSuccess; ++i) {
             const size_t hb = (i == 0 || i == 3) ? hq_bytes : hk_bytes;
             e = cudaMemcpyAsync((char *)p->d_in[i] + hd * hb, (const char *)in[i] + hd * hb, hb, cudaMemcpyHostToDevice, p->s_in);
         }
@@ -406,13 +407,14 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
             const int64_t n = is_q ? pr.Nq : pr.Nk;
             t[i].ptr = (char *)(i < 6 ? p->d_in[i] : p->d_out[i - 6]) + hd * (is_q ? hq_bytes : hk_bytes);
             t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = n * pr.d;
-            ts[i] = &t[i];
+            ts[i] = (no_tangents && ((i >= 3 && i <= 5) || i == 7)) ? nullptr : &t[i];
         }
         if (aj_status st = launch_schedule(p, p->head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq, stream)) return st;
         e = cudaEventRecord(p->ev_k[hd], stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync((char *)o + hd * hq_bytes, (char *)p->d_out[0] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
-        if (e == cudaSuccess) e = cudaMemcpyAsync((char *)to + hd * hq_bytes, (char *)p->d_out[1] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
+        if (e == cudaSuccess && !no_tangents)
+            e = cudaMemcpyAsync((char *)to + hd * hq_bytes, (char *)p->d_out[1] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
         if (e == cudaSuccess && lse)
             e = cudaMemcpyAsync(lse + (size_t)hd * pr.Nq, p->d_lse + (size_t)hd * pr.Nq, pr.Nq * sizeof(float), cudaMemcpyDeviceToHost, p->s_out);
         if (e != cudaSuccess) return cuda_fail(e, "device-to-host copy");

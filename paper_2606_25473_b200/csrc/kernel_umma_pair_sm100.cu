@@ -122,6 +122,50 @@ struct TileCursor {
     }
 };
 
+// The softmax role's view of a task's key stream: how many columns of the next tile this thread's row sees
+// (inside the entry's key range and the entry's row interval).  The next entry is fetched when the
+// current one is entered, so that crossing into it costs no memory latency.
+struct RowCursor {
+    const int32_t *kb, *ke;
+    const uint32_t *rows;
+    int r, rend, prow;
+    int rem;             // keys left in the current entry
+    bool sees;           // this row is inside the current entry's row interval
+    int nkb, nke;        // the next entry as loaded (decoded only when it is entered, so the loads stay in flight)
+    uint32_t nrr;
+    __device__ __forceinline__ void fetch_next() {
+        if (r + 1 < rend) { nkb = kb[r + 1]; nke = ke[r + 1]; nrr = rows[r + 1]; }
+        else { nkb = 0; nke = 0; nrr = 0; }
+    }
+    __device__ __forceinline__ void advance() {
+        ++r;
+        rem = nke - nkb;
+        sees = prow >= (int)(nrr & 0xffffu) && prow < (int)((nrr >> 16) & 0x7fffu);
+        fetch_next();
+    }
+    __device__ __forceinline__ void init(const int32_t *k_begin, const int32_t *k_end, const uint32_t *row_iv, int rb, int rc, int row) {
+        kb = k_begin; ke = k_end; rows = row_iv; r = rb - 2; rend = rb + rc; prow = row;
+        nkb = 0; nke = 0; nrr = 0;
+        advance();           // r = rb - 1: fetches entry rb
+        advance();           // r = rb: current = entry rb, next = entry rb + 1
+    }
+    // columns of the next tile this row sees; consumes the tile
+    __device__ __forceinline__ int tile() {
+        const int v = sees ? min(BC, rem) : 0;
+        rem -= BC;
+        if (rem <= 0) advance();
+        return v;
+    }
+    // both tiles of a pair-step that lies inside the current entry
+    __device__ __forceinline__ bool pair_inside() const { return rem >= 2 * BC; }
+    __device__ __forceinline__ int pair() {
+        const int v = sees ? BC : 0;
+        rem -= 2 * BC;
+        if (rem <= 0) advance();
+        return v;
+    }
+};
+
 struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
@@ -319,7 +363,6 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     kslot = ring % NSTAGE;
                     wait(BAR_KV_FULL + kslot, (ring / NSTAGE) & 1);
                     tc_fence_after();
-                    kz_next = warp_uniform((uint32_t)((volatile int *)sh->slot_kz)[kslot]) != 0;
                     k_lo = (((sRing + kslot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
                     if (leader) {
 #pragma unroll
@@ -331,6 +374,8 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                         tc_commit_pair(bars + 8 * BAR_S_FULL, 3);
                     }
                     __syncwarp();
+                    // read after the S MMAs are on their way: only tS and the P~ tV MMAs of this pair-step depend on it
+                    kz_next = warp_uniform((uint32_t)((volatile int *)sh->slot_kz)[kslot]) != 0;
                     ++ring;
                 };
                 auto issue_ts = [&](bool last) {
@@ -429,26 +474,17 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             const bool primal = (task.flags & AJ_TASK_PRIMAL_ONLY) != 0;
             float m_ref = M_UNSET;
             uint64_t l2[2] = {0ull, 0ull}, r2[2] = {0ull, 0ull};   // 4 partial sums each of l = sum P~ and r = sum H~
-            TileCursor cur;
-            cur.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
+            RowCursor cur;
+            cur.init(prm.k_begin, prm.k_end, prm.rows, task.range_begin, task.range_count, prow);
             const int np = (n + 1) >> 1;
-            int cur_entry = -1;
-            bool sees = false;                                   // this row is inside the current entry's row interval
             for (int p = 0; p < np; ++p, ++c_pv) {
                 // columns of the two tiles this row may see: inside the entry's keys and row interval
                 int valid[2];
-                {
-                    const Tile t0 = cur.get();
-                    cur.next();
-                    if (t0.entry != cur_entry) { cur_entry = t0.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)((rr >> 16) & 0x7fffu); }
-                    valid[0] = sees ? t0.valid : 0;
-                    valid[1] = 0;
-                    if (2 * p + 1 < n) {
-                        const Tile t1 = cur.get();
-                        cur.next();
-                        if (t1.entry != cur_entry) { cur_entry = t1.entry; const uint32_t rr = prm.rows[cur_entry]; sees = prow >= (int)(rr & 0xffffu) && prow < (int)((rr >> 16) & 0x7fffu); }
-                        valid[1] = sees ? t1.valid : 0;
-                    }
+                if (cur.pair_inside()) {
+                    valid[0] = valid[1] = cur.pair();
+                } else {
+                    valid[0] = cur.tile();
+                    valid[1] = 2 * p + 1 < n ? cur.tile() : 0;
                 }
                 // primal-only tasks alternate between the S columns (even pair-steps) and the tS columns (odd) as S buffer
                 const bool alt = primal && (p & 1);
@@ -468,6 +504,22 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
 #pragma unroll
                         for (int c = 0; c < BC; ++c) if (c >= valid[i]) su[i][c >> 5][c & 31] = 0xff800000u;
                     }
+                // P~ = exp2(S*s*log2e - m_ref); l += rowsum (PAPER.md:919-920).  The bf16 pairs stay in registers for H~.
+                uint32_t pk[2][32];
+                uint64_t ls[2];                                   // this tile's contribution to l (committed once m_ref is settled)
+                auto exp_tile = [&](int i, float mref) {
+                    const uint64_t negm2 = pack2(-mref, -mref);
+                    ls[0] = 0ull; ls[1] = 0ull;
+#pragma unroll
+                    for (int c = 0; c < BC / 2; ++c) {
+                        const uint64_t x = ffma2(pack2(su[i][c >> 4][(2 * c) & 31], su[i][c >> 4][(2 * c + 1) & 31]), sl2_2, negm2);
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        const float p0 = ex2(x0), p1 = ex2(x1);
+                        ls[c & 1] = fadd2(ls[c & 1], pack2(p0, p1));
+                        pk[i][c] = pack_bf16(p0, p1);
+                    }
+                };
                 float mx[4];
 #pragma unroll
                 for (int k = 0; k < 4; ++k) mx[k] = __uint_as_float(su[0][0][k]);
@@ -475,46 +527,50 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 for (int c = 4; c < 2 * BC; ++c) mx[c & 3] = fmaxf(mx[c & 3], __uint_as_float(su[c >> 6][(c >> 5) & 1][c & 31]));
                 const float cand = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * sl2;
                 {
-                    // Lazy reference max (PAPER.md:922-927 applied only when needed), once per pair-step.  A row whose
-                    // reference is still unset has O = T = l = r = 0 exactly: it adopts the max with nothing to rescale.
+                    // Lazy reference max (PAPER.md:922-927 applied only when needed), once per pair-step: it moves only when
+                    // the pair-step's max exceeds it by 2^8 (first pair-step of a task; later only for growing scores).
+                    // A row whose reference is still unset has O = T = l = r = 0 exactly: it adopts the max with nothing
+                    // to rescale.
                     const bool need = cand > m_ref + RESCALE_THRESHOLD;
-                    const bool fresh = m_ref == M_UNSET;
-                    if (__any_sync(0xffffffffu, need && !fresh)) {
-                        // e^{m - m_new} applied to O, T (= A + B), l, r; every MMA of the previous pair-step must be complete
-                        wait(BAR_PV_DONE, (c_pv - 1) & 1);
-                        tc_fence_after();
-                        const float f = (need && !fresh) ? ex2(m_ref - cand) : 1.f;
-                        const int ncols = primal ? 128 : 256;          // a primal-only task has no T
+                    if (__any_sync(0xffffffffu, need)) {
+                        const bool fresh = m_ref == M_UNSET;
+                        if (__any_sync(0xffffffffu, need && !fresh)) {
+                            // e^{m - m_new} applied to O, T (= A + B), l, r; every MMA of the previous pair-step must be complete
+                            wait(BAR_PV_DONE, (c_pv - 1) & 1);
+                            tc_fence_after();
+                            const float f = (need && !fresh) ? ex2(m_ref - cand) : 1.f;
+                            const int ncols = primal ? 128 : 256;          // a primal-only task has no T
 #pragma unroll 1
-                        for (int cb = 0; cb < ncols; cb += 32) {
-                            uint32_t a[32];
-                            tmem_ld32(tmem + lane_base + cb, a);
-                            tc_wait_ld(a);
+                            for (int cb = 0; cb < ncols; cb += 32) {
+                                uint32_t a[32];
+                                tmem_ld32(tmem + lane_base + cb, a);
+                                tc_wait_ld(a);
 #pragma unroll
-                            for (int c = 0; c < 32; ++c) a[c] = __float_as_uint(__uint_as_float(a[c]) * f);
-                            tmem_st32(tmem + lane_base + cb, a);
+                                for (int c = 0; c < 32; ++c) a[c] = __float_as_uint(__uint_as_float(a[c]) * f);
+                                tmem_st32(tmem + lane_base + cb, a);
+                            }
+                            const uint64_t f2 = pack2(f, f);
+                            l2[0] = fmul2(l2[0], f2); l2[1] = fmul2(l2[1], f2);
+                            r2[0] = fmul2(r2[0], f2); r2[1] = fmul2(r2[1], f2);
                         }
-                        const uint64_t f2 = pack2(f, f);
-                        l2[0] = fmul2(l2[0], f2); l2[1] = fmul2(l2[1], f2);
-                        r2[0] = fmul2(r2[0], f2); r2[1] = fmul2(r2[1], f2);
+                        if (need) m_ref = cand;
                     }
-                    if (need) m_ref = cand;
                 }
-                // P~ = exp2(S*s*log2e - m_ref); l += rowsum (PAPER.md:919-920).  The bf16 pairs stay in registers for H~.
-                const uint64_t negm2 = pack2(-m_ref, -m_ref);
                 const uint32_t p_arrive = alt ? h_full : p_full;
-                uint32_t pk[2][32];
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
-#pragma unroll
-                    for (int c = 0; c < BC / 2; ++c) {
-                        const uint64_t x = ffma2(pack2(su[i][c >> 4][(2 * c) & 31], su[i][c >> 4][(2 * c + 1) & 31]), sl2_2, negm2);
-                        float x0, x1;
-                        unpack2(x, x0, x1);
-                        const float p0 = ex2(x0), p1 = ex2(x1);
-                        l2[c & 1] = fadd2(l2[c & 1], pack2(p0, p1));
-                        pk[i][c] = pack_bf16(p0, p1);
+                    // tile j1's exponentials must not be hoisted above tile j0's store and arrive (the P~ MMAs of j0 run
+                    // under them): the reference passes through an opaque, ordered asm
+                    float m_i = m_ref;
+                    if (i == 1) {
+                        // (ptxas would otherwise schedule all 128 MUFUs in front of the first tcgen05.st: tile j1's
+                        // reference is made to depend on a shared-memory load that follows the arrive in program order)
+                        uint32_t z;
+                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(smem_u32(&sh->abort_flag)) : "memory");
+                        m_i = z ? M_UNSET : m_ref;
                     }
+                    exp_tile(i, m_i);
+                    l2[0] = fadd2(l2[0], ls[0]); l2[1] = fadd2(l2[1], ls[1]);
                     tmem_st32(tmem + lane_base + tm_s + i * BC, pk[i]);
                     tc_wait_st();
                     tc_fence_before();

@@ -34,6 +34,8 @@ class Workload:
     tangent_std: float
     seed: int = 0
     clean_tangent_zero: bool = False   # teacher forcing: tQ, tK, tV rows of the clean half are zero
+    no_tangents: bool = False          # plain masked attention forward: tQ = tK = tV = 0 (no JVP at inference)
+    Nq: int = 0                        # full mask only: query rows when they differ from the keys (current chunk x cached prefix)
 
     @property
     def block_len(self) -> int:
@@ -50,6 +52,10 @@ class Workload:
         return 2 * half if self.mask == "teacher_forcing" else half
 
     @property
+    def num_queries(self) -> int:
+        return self.Nq or self.N
+
+    @property
     def torch_dtype(self):
         return torch.bfloat16 if self.dtype == "bf16" else torch.float32
 
@@ -62,7 +68,7 @@ class Workload:
             return 2 * tri * C * C
         if self.mask == "block_causal":
             return tri * C * C
-        return self.N * self.N
+        return self.num_queries * self.N
 
 
 # BASELINE.json configs[0..4] (+ the full-mask control of configs[4]).
@@ -81,25 +87,30 @@ CONFIG_ORDER: List[str] = list(WORKLOADS)
 EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     Workload("wan13b_tf_framewise_cleanzero", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, True),
     Workload("wan13b_tf_chunkwise_cleanzero", 1, 12, 128, "teacher_forcing", 1560, 21, 3, "bf16", 0.1, 0, True),
+    # N3: attention without tangents.  The teacher-forcing / diffusion-forcing packed forward of the non-JVP stages
+    # (PAPER.md:180), and the rollout shape: one chunk of queries against the cached prefix plus itself.
+    Workload("wan13b_tf_framewise_fwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.0, 0, False, True),
+    Workload("wan13b_chunk_vs_prefix_fwd", 8, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
 ]}
 
 
 def scaled_down(w: Workload, frame_len: int, num_frames: int = 0, H: int = 0, B: int = 0) -> Workload:
     """Same structure, smaller extent (parity cases the oracle finishes in seconds)."""
     return Workload(f"{w.name}@L{frame_len}", B or w.B, H or w.H, w.d, w.mask, frame_len,
-                    num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed, w.clean_tangent_zero)
+                    num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed, w.clean_tangent_zero,
+                    w.no_tangents, 0)
 
 
 def make_inputs(w: Workload, device: str = "cpu", pin: bool = False):
-    """Returns [q, k, v, tq, tk, tv], each [B, H, N, d] in the config dtype."""
+    """Returns [q, k, v, tq, tk, tv]: q, tq [B, H, Nq, d], the rest [B, H, N, d], in the config dtype."""
     g = torch.Generator(device="cpu")
     g.manual_seed(w.seed)
-    shape = (w.B, w.H, w.N, w.d)
     out = []
     for i in range(6):
+        shape = (w.B, w.H, w.num_queries if i in (0, 3) else w.N, w.d)
         x = torch.randn(shape, generator=g, dtype=torch.float32)
         if i >= 3:
-            x.mul_(w.tangent_std)
+            x.mul_(0.0 if w.no_tangents else w.tangent_std)
             if w.clean_tangent_zero:
                 assert w.mask == "teacher_forcing"
                 x[:, :, :w.N // 2] = 0.0          # the packed sequence is [clean | noisy] (PAPER.md:177)

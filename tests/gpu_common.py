@@ -18,9 +18,10 @@ def mask_kind(w: Workload) -> int:
 
 def make_plan(w: Workload, kernel: int = aj.AJ_KERNEL_AUTO, scale: float = 0.0, tangent_zero=None):
     """tangent_zero: an aj_tangent_zero promise; default = what the workload's data guarantees."""
-    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32, scale)
+    prob = aj.make_problem(w.B, w.H, w.num_queries, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32, scale)
     if tangent_zero is None:
-        tangent_zero = aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE
+        tangent_zero = (aj.AJ_TANGENT_NONE if w.no_tangents else
+                        aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE)
     mask, keep = aj.make_mask(mask_kind(w), w.frame_len, w.num_frames, w.chunk_frames, tangent_zero=tangent_zero)
     plan = aj.attn_jvp_plan_create(prob, mask)
     if kernel != aj.AJ_KERNEL_AUTO:
@@ -36,8 +37,12 @@ def run_gpu(w: Workload, inputs_cpu, kernel: int = aj.AJ_KERNEL_AUTO, plan=None)
     dev = [x.cuda() for x in inputs_cpu]
     o = torch.full_like(dev[0], float("nan"))
     to = torch.full_like(dev[0], float("nan"))
-    lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")
-    aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream)
+    lse = torch.full((w.B, w.H, w.num_queries), float("nan"), dtype=torch.float32, device="cuda")
+    if w.no_tangents:                      # forward only: no tangent goes in, none comes out (tO = 0 by definition)
+        aj.attn_fwd(plan, *dev[:3], o, lse, torch.cuda.current_stream().cuda_stream)
+        to.zero_()
+    else:
+        aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     assert aj.attn_jvp_plan_device_status(plan) == 0, "the kernel abandoned a launch (pipeline wait timed out)"
     if own:
@@ -58,7 +63,7 @@ def run_oracle(w: Workload, inputs_cpu, rows_by_head=None):
             rows = None if rows_by_head is None else np.asarray(rows_by_head[(b, h)], dtype=np.int64)
             args = [widen(x[b, h]) for x in inputs_cpu]
             o, to, lse = oracle.attn_jvp_head(om, *args, scale, rows)
-            out[(b, h)] = (np.arange(w.N) if rows is None else rows, o, to, lse)
+            out[(b, h)] = (np.arange(w.num_queries) if rows is None else rows, o, to, lse)
     return out
 
 
@@ -88,7 +93,7 @@ def sample_rows(w: Workload, per_head_groups: int = 4, random_per_group: int = 2
     of the first and the last query-tile boundary, and seeded random rows."""
     C, n = w.block_len, w.num_blocks
     if w.mask == "full":
-        groups = [(0, w.N)]
+        groups = [(0, w.num_queries)]
     elif w.mask == "block_causal":
         groups = [(i * C, (i + 1) * C) for i in range(n)]
     else:

@@ -189,15 +189,18 @@ def test_null_tangents_are_rejected_unless_the_plan_says_none():
 
 # ---------------------------------------------------------------------------------------- full size (what bench.py times)
 @pytest.mark.parametrize("name", list(EXTRA_WORKLOADS))
-def test_clean_zero_full_size_sampled_rows(name):
+def test_extra_workloads_full_size_sampled_rows(name):
     w = EXTRA_WORKLOADS[name]
     x = make_inputs(w)
     plan = make_plan(w)
     gpu = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_destroy(plan)
     rows = sample_rows(w, per_head_groups=3, random_per_group=2, tile_q=256)
+    if w.B * w.H > 24:                       # keep the oracle's share to seconds: every fourth (b, h)
+        rows = {bh: r for i, (bh, r) in enumerate(rows.items()) if i % 4 == 0}
     errs = compare(w, gpu, run_oracle(w, x, rows))
     print(f"{name}: errs={errs}")
-    assert torch.count_nonzero(gpu[1][:, :, :w.N // 2]) == 0
+    if w.clean_tangent_zero:
+        assert torch.count_nonzero(gpu[1][:, :, :w.N // 2]) == 0
     for t in gpu:
         assert torch.isfinite(t.float()).all()
