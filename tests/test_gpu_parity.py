@@ -307,3 +307,27 @@ def test_full_size_config_sampled_rows(name, kernel):
     # properties that hold at any size: every output written and finite, lse within [min s, max s + ln N]
     for t in gpu:
         assert torch.isfinite(t.float()).all()
+
+
+# ---------------------------------------------------------------------------------------- Ulysses wrapper on one GPU
+def test_ulysses_wrapper_with_the_cuda_local_op_world_size_1():
+    """The N4 plumbing with the production local op (NCCL, one rank = one GPU: the exchanges are identities here; the
+    multi-rank layout is covered by the gloo test): same bits as the direct call."""
+    import torch.distributed as dist
+    from paper_2606_25473_b200 import ulysses
+    w = SMALL_UMMA[0]
+    x = make_inputs(w)
+    plan = make_plan(w)
+    ref = run_gpu(w, x, plan=plan)
+    own = not dist.is_initialized()
+    if own:
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29517", rank=0, world_size=1)
+    try:
+        o, to, lse = ulysses.ulysses_attn_jvp(ulysses.local_attn_jvp(plan, torch.cuda.current_stream().cuda_stream),
+                                              *[t.cuda() for t in x])
+        torch.cuda.synchronize()
+    finally:
+        if own:
+            dist.destroy_process_group()
+    aj.attn_jvp_plan_destroy(plan)
+    assert torch.equal(o.cpu(), ref[0]) and torch.equal(to.cpu(), ref[1]) and torch.equal(lse.cpu(), ref[2])
