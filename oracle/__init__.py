@@ -62,6 +62,10 @@ def _load():
             ctypes.POINTER(_CMask), ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_double,
             ctypes.c_int32] + [ctypes.c_void_p] * 6 + [
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.attn_jvp_oracle_bwd.restype = ctypes.c_int
+        lib.attn_jvp_oracle_bwd.argtypes = [
+            ctypes.POINTER(_CMask), ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int32] + \
+            [ctypes.c_void_p] * 4 + [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64] + [ctypes.c_void_p] * 3
         lib.attn_jvp_oracle_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -185,3 +189,33 @@ def attn_jvp(mask: Mask, q, k, v, tq, tk, tv, scale: float, rows: Optional[np.nd
     to = np.stack([np.stack([outs[b][h][1] for h in range(H)]) for b in range(B)])
     lse = np.stack([np.stack([outs[b][h][2] for h in range(H)]) for b in range(B)])
     return o, to, lse
+
+
+def attn_bwd_head(mask: Mask, q, k, v, dout, scale: float, rows: Optional[np.ndarray] = None,
+                  keys: Optional[np.ndarray] = None):
+    """Primal backward of one (batch, head) slice: q, dout [Nq, d]; k, v [Nk, d] (float32 or float64 numpy).
+
+    Returns (dq [R, d], dk [Kn, d], dv [Kn, d]) in float64 for the requested query rows / keys (all if None).
+    """
+    lib = _load()
+    dt = np.float64 if q.dtype == np.float64 else np.float32
+    arrs = [np.ascontiguousarray(x, dtype=dt) for x in (q, k, v, dout)]
+    nq, d = arrs[0].shape
+    nk = arrs[1].shape[0]
+    assert arrs[3].shape == (nq, d) and arrs[2].shape == (nk, d)
+    rows_arr = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    keys_arr = None if keys is None else np.ascontiguousarray(keys, dtype=np.int64)
+    nrows = nq if rows_arr is None else rows_arr.shape[0]
+    nkeys = nk if keys_arr is None else keys_arr.shape[0]
+    dq = np.empty((nrows, d), dtype=np.float64)
+    dk = np.empty((nkeys, d), dtype=np.float64)
+    dv = np.empty((nkeys, d), dtype=np.float64)
+    cm, keep = mask._c()
+    rc = lib.attn_jvp_oracle_bwd(
+        ctypes.byref(cm), nq, nk, d, float(scale), 1 if dt == np.float64 else 0, *[x.ctypes.data for x in arrs],
+        None if rows_arr is None else rows_arr.ctypes.data, nrows,
+        None if keys_arr is None else keys_arr.ctypes.data, nkeys,
+        dq.ctypes.data, dk.ctypes.data, dv.ctypes.data)
+    if rc != 0:
+        raise RuntimeError("attn_jvp_oracle_bwd failed")
+    return dq, dk, dv

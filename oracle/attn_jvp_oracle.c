@@ -15,7 +15,8 @@
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): central finite differences
  * of O along the tangent, brute-force dense masked attention written
  * independently in numpy, torch.func.jvp / SDPA / logsumexp, closed forms,
- * invariants and pair counts.  Every exported function below is pinned; none is
+ * invariants and pair counts; the backward (attn_jvp_oracle_bwd) is pinned by torch.autograd, finite differences of
+ * <O, dO> and invariants (tests/test_oracle_bwd_pins.py).  Every exported function below is pinned; none is
  * "parity unpinned".
  *
  * Definitions followed (PAPER.md line : item):
@@ -202,6 +203,107 @@ int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d
         }
         free(s); free(ts); free(ok); free(qa); free(tqa);
     }
+    return failed ? -1 : 0;
+}
+
+/*
+ * Primal backward: the vector-Jacobian product of Eq. 42.  The paper gives no formula for it; it
+ * only says the student's gradient flows through the ordinary primal path (Eq. 19) and that the forward
+ * returns L for it.  This is the textbook VJP of O = softmax(S + M) V, S = scale * Q K^T, written out
+ * with every row of P materialised:
+ *     dV_b = sum_a p_ab dO_a
+ *     dP_ab = <dO_a, v_b>,  delta_a = sum_b p_ab dP_ab,  dS_ab = p_ab (dP_ab - delta_a)     (softmax Jacobian)
+ *     dQ_a = scale * sum_b dS_ab k_b,   dK_b = scale * sum_a dS_ab q_a
+ * over the allowed pairs only (masked entries have p = 0 and the mask has no gradient).  Rows with no allowed key
+ * contribute nothing and get dQ = 0.
+ * Pass 1 runs over query rows (p row materialised; dQ, and lse_a, delta_a kept), pass 2 over keys (dK, dV), each
+ * parallel over its own outputs so that no two threads add into the same element.
+ * q, dout: [nq, d]; k, v: [nk, d].  rows / keys list the query rows / keys whose gradients are wanted (NULL = all);
+ * dq: [nrows, d]; dk, dv: [nkeys, d], all fp64.  Pins: torch.autograd, finite differences of <O, dO>, invariants
+ * (tests/test_oracle_bwd_pins.py).
+ */
+int attn_jvp_oracle_bwd(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d, double scale, int32_t dtype,
+                        const void *q, const void *k, const void *v, const void *dout,
+                        const int64_t *rows, int64_t nrows, const int64_t *keys, int64_t nkeys,
+                        double *dq, double *dk, double *dv)
+{
+    if (!mask || nq <= 0 || nk <= 0 || d <= 0 || nrows < 0 || nkeys < 0) return -1;
+    if (dtype != AJO_F32 && dtype != AJO_F64) return -1;
+    double *lse = (double *)malloc(sizeof(double) * (size_t)nq);
+    double *delta = (double *)malloc(sizeof(double) * (size_t)nq);
+    int64_t *slot = (int64_t *)malloc(sizeof(int64_t) * (size_t)nq);   /* where row a's dQ goes, or -1 */
+    if (!lse || !delta || !slot) { free(lse); free(delta); free(slot); return -1; }
+    for (int64_t a = 0; a < nq; ++a) slot[a] = rows ? -1 : (a < nrows ? a : -1);
+    if (rows) for (int64_t i = 0; i < nrows; ++i) if (rows[i] >= 0 && rows[i] < nq) slot[rows[i]] = i;
+    for (int64_t i = 0; i < nrows * d; ++i) dq[i] = 0.0;
+    int failed = 0;
+#pragma omp parallel
+    {
+        double *p = (double *)malloc(sizeof(double) * (size_t)nk);    /* scores, then p_ab */
+        double *dp = (double *)malloc(sizeof(double) * (size_t)nk);   /* dP_ab             */
+        unsigned char *ok = (unsigned char *)malloc((size_t)nk);
+        if (!p || !dp || !ok) {
+#pragma omp atomic write
+            failed = 1;
+        } else {
+            /* pass 1: every query row (lse and delta of all rows are needed by pass 2) */
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t a = 0; a < nq; ++a) {
+                double m = -INFINITY;
+                for (int64_t b = 0; b < nk; ++b) {
+                    ok[b] = (unsigned char)attn_jvp_oracle_allowed(mask, a, b);
+                    if (!ok[b]) { p[b] = -INFINITY; dp[b] = 0.0; continue; }
+                    double qk = 0.0, dov = 0.0;
+                    for (int c = 0; c < d; ++c) {
+                        qk += ajo_load(q, dtype, a * d + c) * ajo_load(k, dtype, b * d + c);
+                        dov += ajo_load(dout, dtype, a * d + c) * ajo_load(v, dtype, b * d + c);
+                    }
+                    p[b] = scale * qk;
+                    dp[b] = dov;
+                    if (p[b] > m) m = p[b];
+                }
+                if (m == -INFINITY) { lse[a] = -INFINITY; delta[a] = 0.0; continue; }
+                double z = 0.0;
+                for (int64_t b = 0; b < nk; ++b) { p[b] = ok[b] ? exp(p[b] - m) : 0.0; z += p[b]; }
+                for (int64_t b = 0; b < nk; ++b) p[b] /= z;
+                lse[a] = m + log(z);
+                double dl = 0.0;
+                for (int64_t b = 0; b < nk; ++b) dl += p[b] * dp[b];
+                delta[a] = dl;
+                if (slot[a] < 0) continue;
+                double *dqa = dq + slot[a] * d;
+                for (int64_t b = 0; b < nk; ++b) {
+                    if (!ok[b]) continue;
+                    double ds = p[b] * (dp[b] - dl);
+                    for (int c = 0; c < d; ++c) dqa[c] += scale * ds * ajo_load(k, dtype, b * d + c);
+                }
+            }
+            /* pass 2: the requested keys */
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t j = 0; j < nkeys; ++j) {
+                int64_t b = keys ? keys[j] : j;
+                double *dkb = dk + j * d, *dvb = dv + j * d;
+                for (int c = 0; c < d; ++c) { dkb[c] = 0.0; dvb[c] = 0.0; }
+                if (b < 0 || b >= nk) continue;
+                for (int64_t a = 0; a < nq; ++a) {
+                    if (!attn_jvp_oracle_allowed(mask, a, b) || lse[a] == -INFINITY) continue;
+                    double qk = 0.0, dov = 0.0;
+                    for (int c = 0; c < d; ++c) {
+                        qk += ajo_load(q, dtype, a * d + c) * ajo_load(k, dtype, b * d + c);
+                        dov += ajo_load(dout, dtype, a * d + c) * ajo_load(v, dtype, b * d + c);
+                    }
+                    double pab = exp(scale * qk - lse[a]);
+                    double ds = pab * (dov - delta[a]);
+                    for (int c = 0; c < d; ++c) {
+                        dvb[c] += pab * ajo_load(dout, dtype, a * d + c);
+                        dkb[c] += scale * ds * ajo_load(q, dtype, a * d + c);
+                    }
+                }
+            }
+        }
+        free(p); free(dp); free(ok);
+    }
+    free(lse); free(delta); free(slot);
     return failed ? -1 : 0;
 }
 
