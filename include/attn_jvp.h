@@ -143,6 +143,12 @@ aj_status attn_jvp_schedule_create(const aj_problem *problem, const aj_mask_desc
 /* Same with an explicit aj_tiling (attn_jvp_schedule_create = AJ_TILING_PER_GROUP).  tile_q < 32768. */
 aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_q,
                                          int32_t tile_k, int32_t tiling, aj_schedule **out);
+/* The same mask seen from the KEYS (primal backward, dK and dV): "query groups" of the result are maximal key intervals
+ * seen by the same rows, their "key ranges" are the sorted, merged query-row ranges that see them (keys no row sees
+ * become range-less groups); tasks are tiles of tile_keys keys (per-group tiling) that stream their rows in tiles of
+ * tile_rows.  attn_jvp_schedule_get / _info read it like any schedule, with the roles swapped. */
+aj_status attn_jvp_schedule_create_transposed(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
+                                              int32_t tile_rows, aj_schedule **out);
 aj_status attn_jvp_schedule_destroy(aj_schedule *sched);
 /* Any out pointer may be NULL. unmasked_pairs_per_head = sum over groups of rows * allowed keys. */
 aj_status attn_jvp_schedule_info(const aj_schedule *sched, int32_t *num_groups, int32_t *num_ranges,
@@ -209,6 +215,21 @@ aj_status attn_jvp_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor 
  * current chunk against the cached prefix). */
 aj_status attn_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o,
                    float *lse, void *cuda_stream);
+
+/*
+ * Primal backward under the plan's mask (Eq. 19: the student's gradient flows through
+ * the ordinary primal path, for which the forward returns L): the vector-Jacobian product of Eq. 42,
+ *     dV_b = sum_a p_ab dO_a,  dS_ab = p_ab (<dO_a, v_b> - <dO_a, O_a>),  dQ_a = s sum_b dS_ab k_b,  dK_b = s sum_a dS_ab q_a
+ * with p_ab = exp(s <q_a, k_b> - lse_a) over the unmasked pairs.  q, o, dout, dq: [B,H,Nq,d]; k, v, dk, dv: [B,H,Nk,d]
+ * in the problem dtype; lse: contiguous fp32 [B,H,Nq] as written by attn_jvp_fwd / attn_fwd on the same q, k, v.  All
+ * DEVICE memory, same alignment rules as attn_jvp_fwd.  Every element of dq, dk, dv is written (0 for rows without
+ * keys and keys no row sees).  Enqueues three kernels on `cuda_stream`; the first call on a plan also builds and
+ * uploads the backward schedules (synchronous host work) and allocates a [B,H,Nq] fp32 workspace.
+ * This round: plain-FMA fp32 arithmetic for both dtypes (a correct first path, not a tensor-core kernel).
+ */
+aj_status attn_bwd(aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o,
+                   const float *lse, const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv,
+                   void *cuda_stream);
 
 /*
  * Same computation on HOST buffers: contiguous [B,H,N,d] arrays in the problem dtype (lse fp32

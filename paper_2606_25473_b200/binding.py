@@ -56,7 +56,7 @@ class AttnJvpError(RuntimeError):
 # Every symbol include/attn_jvp.h declares (tests check that the library exports all of them).
 SYMBOLS = [
     "attn_jvp_schedule_create", "attn_jvp_schedule_create_tiled", "attn_jvp_schedule_entries", "attn_jvp_schedule_destroy", "attn_jvp_schedule_info", "attn_jvp_schedule_get", "attn_jvp_schedule_assign",
-    "attn_jvp_schedule_entry_flags", "attn_jvp_schedule_pair_classes", "attn_jvp_plan_pair_classes", "attn_fwd",
+    "attn_jvp_schedule_create_transposed", "attn_jvp_schedule_entry_flags", "attn_jvp_schedule_pair_classes", "attn_jvp_plan_pair_classes", "attn_fwd", "attn_bwd",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
 ]
@@ -75,12 +75,14 @@ def lib():
         vp, i32, i64p = ctypes.c_void_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int64)
         l.attn_jvp_schedule_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_create_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
+        l.attn_jvp_schedule_create_transposed.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_entries.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P]
         l.attn_jvp_schedule_assign.argtypes = [vp, i32, _I32P, _I32P]
         l.attn_jvp_schedule_entry_flags.argtypes = [vp, _I32P]
         l.attn_jvp_schedule_pair_classes.argtypes = [vp, i64p]
         l.attn_jvp_plan_pair_classes.argtypes = [vp, i64p]
         l.attn_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 4 + [vp, vp]
+        l.attn_bwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 4 + [vp] + [ctypes.POINTER(aj_tensor)] * 4 + [vp]
         l.attn_jvp_schedule_destroy.argtypes = [vp]
         l.attn_jvp_schedule_info.argtypes = [vp, _I32P, _I32P, _I32P, i64p]
         l.attn_jvp_schedule_get.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P, ctypes.POINTER(aj_task)]
@@ -167,6 +169,12 @@ def attn_jvp_schedule_create(problem: aj_problem, mask: aj_mask_desc, tile_q: in
 def attn_jvp_schedule_create_tiled(problem: aj_problem, mask: aj_mask_desc, tile_q: int, tile_k: int, tiling: int) -> ctypes.c_void_p:
     out = ctypes.c_void_p()
     _check(lib().attn_jvp_schedule_create_tiled(ctypes.byref(problem), ctypes.byref(mask), tile_q, tile_k, tiling, ctypes.byref(out)))
+    return out
+
+
+def attn_jvp_schedule_create_transposed(problem: aj_problem, mask: aj_mask_desc, tile_keys: int, tile_rows: int) -> ctypes.c_void_p:
+    out = ctypes.c_void_p()
+    _check(lib().attn_jvp_schedule_create_transposed(ctypes.byref(problem), ctypes.byref(mask), tile_keys, tile_rows, ctypes.byref(out)))
     return out
 
 
@@ -293,6 +301,13 @@ def attn_fwd(plan, q, k, v, o, lse=None, stream: int = 0) -> None:
     """Masked attention forward without tangents (AJ_TANGENT_NONE plans): O and lse only."""
     ts = [_tensor(x) for x in (q, k, v, o)]
     _check(lib().attn_fwd(plan, *[ctypes.byref(x) for x in ts], None if lse is None else lse.data_ptr(), stream))
+
+
+def attn_bwd(plan, q, k, v, o, lse, dout, dq, dk, dv, stream: int = 0) -> None:
+    """Primal backward: device tensors; lse is the forward's fp32 [B,H,Nq]; writes dq, dk, dv."""
+    a = [_tensor(x) for x in (q, k, v, o)]
+    b = [_tensor(x) for x in (dout, dq, dk, dv)]
+    _check(lib().attn_bwd(plan, *[ctypes.byref(x) for x in a], lse.data_ptr(), *[ctypes.byref(x) for x in b], stream))
 
 
 def attn_jvp_fwd_host(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:

@@ -30,7 +30,8 @@ struct aj_plan {
         uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
         int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
         int32_t num_pairs = 0;
-    } full, head;
+    } full, head, bwd_q, bwd_k;   // bwd_*: SIMT-tiled schedules of the primal backward (rows x key ranges, keys x row ranges)
+    float *d_delta = nullptr;     // [B, H, Nq] workspace of attn_bwd
     // attn_jvp_fwd_host: device staging buffers, copy streams, one event per head and direction
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void *d_out[2] = {nullptr, nullptr};
@@ -83,6 +84,8 @@ int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACK
 
 // Build the schedule of `prob` (the plan's problem, or one head of it) for `kernel` / `tiling` and upload it into `ds`
 // (left unchanged on failure).
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds);
+
 aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int32_t tiling, aj_plan::DevSchedule &ds) {
     const int tq = kernel == AJ_KERNEL_UMMA_PAIR ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
     const int tk = is_umma(kernel) ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
@@ -92,6 +95,11 @@ aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int
         return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
     aj_schedule *s = nullptr;
     if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tq, tk, tiling, &s)) return st;
+    return upload_schedule(p, s, kernel, ds);
+}
+
+// Uploads `s` (owned by `ds` afterwards; destroyed on failure, `ds` then unchanged).
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds) {
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r)   // row_begin | row_end << 16 (both < 32768) | key-tangents-zero << 31
@@ -214,6 +222,9 @@ aj_status attn_jvp_plan_destroy(aj_plan *p) {
     if (!p) return AJ_OK;
     free_schedule(p->full);
     free_schedule(p->head);
+    free_schedule(p->bwd_q);
+    free_schedule(p->bwd_k);
+    cudaFree(p->d_delta);
     cudaFree(p->d_counters);
     for (void *x : p->d_in) cudaFree(x);
     for (void *x : p->d_out) cudaFree(x);
@@ -345,6 +356,42 @@ aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, con
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
     if (p->mask.tangent_zero != AJ_TANGENT_NONE) return fail(AJ_ERR_INVALID_ARG, "attn_fwd needs a plan whose mask says AJ_TANGENT_NONE");
     return attn_jvp_fwd(p, q, k, v, nullptr, nullptr, nullptr, o, nullptr, lse, cuda_stream);
+}
+
+aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o, const float *lse,
+                   const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv, void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    const aj_problem &pr = p->problem;
+    const int eb = pr.dtype == AJ_BF16 ? 2 : 4;
+    const aj_tensor *ts[8] = {q, k, v, o, dout, dq, dk, dv};
+    const char *names[8] = {"q", "k", "v", "o", "dout", "dq", "dk", "dv"};
+    for (int i = 0; i < 8; ++i)
+        if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
+    if (!lse || (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: NULL or misaligned");
+    // first use: the two SIMT-tiled schedules (query tiles x key ranges; key tiles x row ranges) and the delta workspace
+    if (!p->bwd_q.sched) {
+        aj_schedule *s = nullptr;
+        if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, aj::SIMT_TILE_Q, aj::SIMT_TILE_K, AJ_TILING_PER_GROUP, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_q)) return st;
+    }
+    if (!p->bwd_k.sched) {
+        aj_schedule *s = nullptr;
+        if (aj_status st = attn_jvp_schedule_create_transposed(&p->problem, &p->mask, aj::SIMT_TILE_Q, aj::SIMT_TILE_K, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_k)) return st;
+    }
+    if (!p->d_delta) {
+        cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
+    }
+    aj::BwdParams prm;
+    prm.q = *q; prm.k = *k; prm.v = *v; prm.o = *o; prm.dout = *dout; prm.dq = *dq; prm.dk = *dk; prm.dv = *dv;
+    prm.lse = lse; prm.delta = p->d_delta;
+    prm.q_tasks = p->bwd_q.d_tasks; prm.q_kb = p->bwd_q.d_kb; prm.q_ke = p->bwd_q.d_ke;
+    prm.k_tasks = p->bwd_k.d_tasks; prm.k_rb = p->bwd_k.d_kb; prm.k_re = p->bwd_k.d_ke;
+    prm.B = pr.B; prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
+    cudaError_t e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, p->bwd_q.num_tasks, p->bwd_k.num_tasks, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
+    return AJ_OK;
 }
 
 aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *tq, const void *tk,

@@ -33,6 +33,8 @@ struct Entries {
 };
 
 aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out);
+// The lowered mask with the roles of queries and keys swapped (primal backward: dK, dV are accumulated per key tile).
+void transpose_lowered(const aj_problem &p, const Lowered &low, Lowered &out);
 // Per-group tiling: entries = the lowered ranges, every row of a tile sees every entry of its task.
 void build_tasks(const aj_problem &p, const Lowered &low, int32_t tile_q, int32_t tile_k, Entries &ent,
                  std::vector<aj_task> &tasks);

@@ -24,6 +24,19 @@ struct SimtParams {
 
 cudaError_t launch_simt(const SimtParams &prm, int dtype, int d, int num_tasks, cudaStream_t stream);
 
+// Primal backward, plain FMA (kernel_simt_bwd.cu): a delta kernel, a dQ kernel over q_tasks and a dK/dV kernel over
+// k_tasks (the transposed schedule: key tiles with the row ranges that see them)
+struct BwdParams {
+    aj_tensor q, k, v, o, dout, dq, dk, dv;
+    const float *lse;                 // [B, H, Nq] from the forward
+    float *delta;                     // [B, H, Nq] workspace: <dO_a, O_a>
+    const aj_task *q_tasks; const int32_t *q_kb, *q_ke;   // query tiles and their key ranges
+    const aj_task *k_tasks; const int32_t *k_rb, *k_re;   // key tiles and their row ranges
+    int32_t B, H, Nq;
+    float scale;
+};
+cudaError_t launch_bwd_simt(const BwdParams &prm, int dtype, int d, int num_q_tasks, int num_k_tasks, cudaStream_t stream);
+
 // bf16, d = 128, tcgen05 + TMEM + TMA (kernel_umma_sm100.cu)
 struct UmmaParams {
     CUtensorMap tm_q, tm_tq;    // box {64, 128, 1, 1} over [B, H, Nq, d], SWIZZLE_128B

@@ -141,6 +141,47 @@ aj_status lower_mask(const aj_problem &p, const aj_mask_desc &m, Lowered &out) {
     return AJ_OK;
 }
 
+// The mask seen from the keys (for dK, dV of the primal backward): key groups = maximal key intervals seen by the same
+// set of rows, each with the sorted, merged row ranges that see it.  In `out` the roles are swapped: q_* are key
+// intervals and `ranges` are query-row ranges.  Keys no row sees become range-less groups (their dK, dV are 0).
+void transpose_lowered(const aj_problem &p, const Lowered &low, Lowered &out) {
+    out = Lowered();
+    out.range_offset.push_back(0);
+    const size_t ng = low.q_begin.size();
+    std::vector<size_t> order(ng);
+    for (size_t g = 0; g < ng; ++g) order[g] = g;
+    std::sort(order.begin(), order.end(), [&](size_t a, size_t b) { return low.q_begin[a] < low.q_begin[b]; });
+    std::vector<int32_t> cuts{0, p.Nk};
+    for (const KeyRange &r : low.ranges) { cuts.push_back(r.k_begin); cuts.push_back(r.k_end); }
+    std::sort(cuts.begin(), cuts.end());
+    cuts.erase(std::unique(cuts.begin(), cuts.end()), cuts.end());
+    std::vector<KeyRange> rows, prev;
+    for (size_t c = 0; c + 1 < cuts.size(); ++c) {
+        const int32_t a = cuts[c], b = cuts[c + 1];
+        rows.clear();
+        for (size_t i = 0; i < ng; ++i) {
+            const size_t g = order[i];
+            bool covered = false;
+            for (int r = low.range_offset[g]; r < low.range_offset[g + 1] && !covered; ++r)
+                covered = low.ranges[r].k_begin <= a && b <= low.ranges[r].k_end;
+            if (!covered || low.q_end[g] <= low.q_begin[g]) continue;
+            if (!rows.empty() && rows.back().k_end == low.q_begin[g]) rows.back().k_end = low.q_end[g];
+            else rows.push_back(KeyRange{low.q_begin[g], low.q_end[g], 0});
+        }
+        bool same = !out.q_begin.empty() && out.q_end.back() == a && rows.size() == prev.size();
+        for (size_t i = 0; same && i < rows.size(); ++i) same = rows[i].k_begin == prev[i].k_begin && rows[i].k_end == prev[i].k_end;
+        if (same) { out.q_end.back() = b; continue; }       // same rows as the interval before: extend it
+        out.q_begin.push_back(a);
+        out.q_end.push_back(b);
+        out.q_tz.push_back(0);
+        out.ranges.insert(out.ranges.end(), rows.begin(), rows.end());
+        out.range_offset.push_back((int32_t)out.ranges.size());
+        prev = rows;
+    }
+    out.pairs_per_head = low.pairs_per_head;
+    out.pair_class[2] = low.pairs_per_head;
+}
+
 static void order_tasks(std::vector<aj_task> &tasks) {
     // Longest-first so that the persistent CTAs finish together; ties keep (b, h, group/tile) order so that
     // tasks streaming the same keys of the same head run at the same time and share them in L2.
@@ -360,6 +401,32 @@ aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mas
         if (st != AJ_OK) { delete s; return st; }
         if (tiling == AJ_TILING_PACKED) aj::build_tasks_packed(*problem, s->low, tile_q, tile_k, s->entries, s->tasks);
         else aj::build_tasks(*problem, s->low, tile_q, tile_k, s->entries, s->tasks);
+    } catch (const std::bad_alloc &) {
+        delete s;
+        return aj::fail(AJ_ERR_OOM, "out of host memory");
+    }
+    *out = s;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_schedule_create_transposed(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
+                                              int32_t tile_rows, aj_schedule **out) {
+    if (!out) return aj::fail(AJ_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (aj_status st = aj::check_problem(problem)) return st;
+    if (!mask) return aj::fail(AJ_ERR_INVALID_ARG, "mask is NULL");
+    if (tile_keys <= 0 || tile_rows <= 0 || tile_keys > 32767) return aj::fail(AJ_ERR_INVALID_ARG, "tile sizes must be > 0 (tile_keys < 32768)");
+    aj_schedule *s = new (std::nothrow) aj_schedule();
+    if (!s) return aj::fail(AJ_ERR_OOM, "out of host memory");
+    try {
+        aj::Lowered low;
+        aj_status st = aj::lower_mask(*problem, *mask, low);
+        if (st != AJ_OK) { delete s; return st; }
+        s->problem = *problem;
+        std::swap(s->problem.Nq, s->problem.Nk);           // the tasks' "query rows" are keys
+        s->tile_q = tile_keys; s->tile_k = tile_rows; s->tiling = AJ_TILING_PER_GROUP;
+        aj::transpose_lowered(*problem, low, s->low);
+        aj::build_tasks(s->problem, s->low, tile_keys, tile_rows, s->entries, s->tasks);
     } catch (const std::bad_alloc &) {
         delete s;
         return aj::fail(AJ_ERR_OOM, "out of host memory");

@@ -403,3 +403,59 @@ def test_worker_assignment_weights_cheaper_pair_steps_on_config_2_clean_zero():
     tiles = [sum(tasks[i].num_kv_tiles for i in ids[off[k]:off[k + 1]]) for k in range(74)]
     primal = [sum(tasks[i].num_kv_tiles for i in ids[off[k]:off[k + 1]] if tasks[i].flags & 1) for k in range(74)]
     assert np.corrcoef(tiles, primal)[0, 1] > 0.5
+
+
+# ---------------------------------------------------------------------------------------------- transposed (backward) schedule
+def _check_transposed(want, prob, mask, tile_keys, tile_rows):
+    """Key-tile tasks with row ranges cover the TRANSPOSE of the mask exactly once; every key belongs to one task."""
+    s = aj.attn_jvp_schedule_create_transposed(prob, mask, tile_keys, tile_rows)
+    ng, nr, nt, pairs = aj.attn_jvp_schedule_info(s)
+    got = aj.attn_jvp_schedule_get(s)
+    aj.attn_jvp_schedule_destroy(s)
+    Nq, Nk = want.shape
+    cover = np.zeros((Nk, Nq), dtype=np.int32)
+    keys_seen = np.zeros(Nk, dtype=np.int32)
+    for t in got["tasks"]:
+        if (t.b, t.h) != (0, 0):
+            continue
+        assert 0 < t.q_rows <= tile_keys
+        tiles = 0
+        for r in range(t.range_begin, t.range_begin + t.range_count):
+            r0, r1 = got["k_begin"][r], got["k_end"][r]
+            cover[t.q_begin:t.q_begin + t.q_rows, r0:r1] += 1
+            tiles += -(-(r1 - r0) // tile_rows)
+        assert tiles == t.num_kv_tiles
+        keys_seen[t.q_begin:t.q_begin + t.q_rows] += 1
+    assert np.array_equal(cover, want.T.astype(np.int32))
+    assert np.all(keys_seen == 1)
+    assert pairs == int(want.sum())
+    off = got["range_offset"]
+    for g in range(ng):                                      # row ranges of a key group: sorted, disjoint, merged
+        rs = [(got["k_begin"][r], got["k_end"][r]) for r in range(off[g], off[g + 1])]
+        for (a0, a1), (b0, b1) in zip(rs, rs[1:]):
+            assert a1 < b0
+    return ng
+
+
+@pytest.mark.parametrize("mask,L,F,cf", [
+    ("teacher_forcing", 16, 3, 1), ("teacher_forcing", 10, 6, 3), ("teacher_forcing", 7, 4, 2),
+    ("block_causal", 16, 3, 1), ("block_causal", 9, 6, 2), ("full", 13, 5, 1)])
+@pytest.mark.parametrize("tile_keys,tile_rows", [(16, 32), (8, 4), (5, 3)])
+def test_transposed_schedule_covers_the_transposed_mask_exactly_once(oracle, mask, L, F, cf, tile_keys, tile_rows):
+    w = Workload("t", 1, 2, 64, mask, L, F, cf, "fp32", 1.0)
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_FP32)
+    m, keep = aj.make_mask(_kind(w), L, F, cf)
+    want = oracle.dense_mask(oracle_mask(w), w.N, w.N)
+    ng = _check_transposed(want, prob, m, tile_keys, tile_rows)
+    n = w.num_blocks
+    # teacher forcing: clean key block j is seen by clean blocks >= j and noisy blocks > j; noisy key block j by itself
+    assert ng == {"teacher_forcing": 2 * n, "block_causal": n, "full": 1}[mask]
+
+
+def test_transposed_schedule_of_generic_ranges_with_unseen_keys(oracle):
+    groups = [(4, 9, [(0, 5), (5, 9), (30, 40)]), (9, 13, [(2, 3)]), (13, 20, [(30, 40), (44, 48)]), (33, 40, [])]
+    prob = aj.make_problem(1, 1, 40, 48, 64, aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+    want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
+    for tk, tr in [(8, 4), (16, 8), (3, 5)]:
+        _check_transposed(want, prob, mask, tk, tr)
