@@ -52,6 +52,8 @@ def pair_classes(w: Workload):
 
 def flops_per_call(w: Workload) -> float:
     """2*d flop per contraction per unmasked pair: 12*d per pair with dense tangents (the BASELINE.json convention)."""
+    if w.backward:      # five contractions per pair: S recomputed, dP = dO V^T, dV += P^T dO, dK += dS^T Q, dQ += dS K
+        return 10.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H
     c = pair_classes(w)
     return 2.0 * w.d * (2 * c[0] + 4 * c[1] + 6 * c[2]) * w.B * w.H
 
@@ -201,7 +203,9 @@ def workload_config(w: Workload):
             "unmasked_pairs_per_head": w.unmasked_pairs_per_head,
             "Nq": w.num_queries,
             "tangents": "none (forward only)" if w.no_tangents else "zero on the clean half" if w.clean_tangent_zero else "dense",
-            "flop_convention": ("4*d per unmasked pair (S and P V only)" if w.no_tangents else
+            "pass": "primal backward (attn_bwd)" if w.backward else "forward",
+            "flop_convention": ("10*d per unmasked pair (S, dP, dV, dK, dQ)" if w.backward else
+                                "4*d per unmasked pair (S and P V only)" if w.no_tangents else
                                 "2*d per contraction actually needed per unmasked pair (2, 4 or 6 of them: zero clean tangents)"
                                 if w.clean_tangent_zero else "12*d per unmasked pair"),
             "l2": "no flush: the six inputs (%.2f GB) are larger than the 126 MB L2" %
@@ -267,7 +271,7 @@ def run_cuda(args, w: Workload):
 
     # every rank draws its own head shard (seed + rank): weak scaling, no exchange
     wr = Workload(w.name, w.B, w.H, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std,
-                  w.seed + rank, w.clean_tangent_zero, w.no_tangents, w.Nq)
+                  w.seed + rank, w.clean_tangent_zero, w.no_tangents, w.Nq, w.backward)
     host_all = make_inputs(wr, pin=True)
     host = host_all[:3] + [None, None, None] if w.no_tangents else host_all   # the forward-only call takes no tangents
     devin = [None if x is None else x.to(dev, non_blocking=True) for x in host]
@@ -287,6 +291,31 @@ def run_cuda(args, w: Workload):
     def step_host():
         aj.attn_jvp_fwd_host(plan, *host, h_o, h_to, h_lse, stream.cuda_stream)
         stream.synchronize()                  # the user reads the result after every step
+
+    if w.backward:
+        # the step is attn_bwd on the forward's O and lse (computed once, outside the timed region); end to end = the
+        # six device inputs of attn_bwd copied up from pinned host memory, the call, dQ, dK, dV copied back
+        step_device()
+        g = torch.Generator().manual_seed(1000 + rank)
+        h_bwd = [host[0], host[1], host[2], o.cpu().pin_memory(),
+                 torch.randn(host[0].shape, generator=g).to(host[0].dtype).pin_memory()]
+        h_lse_in = lse.cpu().pin_memory()
+        d_bwd = [x.to(dev) for x in h_bwd]
+        dq, dk, dv = torch.empty_like(devin[0]), torch.empty_like(devin[1]), torch.empty_like(devin[1])
+        h_grads = [torch.empty_like(host[0]).pin_memory(), torch.empty_like(host[1]).pin_memory(), torch.empty_like(host[1]).pin_memory()]
+        d_lse_in = torch.empty_like(lse)
+
+        def step_device():
+            aj.attn_bwd(plan, d_bwd[0], d_bwd[1], d_bwd[2], d_bwd[3], lse, d_bwd[4], dq, dk, dv, stream.cuda_stream)
+
+        def step_host():
+            for dst, src in zip(d_bwd, h_bwd):
+                dst.copy_(src, non_blocking=True)
+            d_lse_in.copy_(h_lse_in, non_blocking=True)
+            aj.attn_bwd(plan, d_bwd[0], d_bwd[1], d_bwd[2], d_bwd[3], d_lse_in, d_bwd[4], dq, dk, dv, stream.cuda_stream)
+            for dst, src in zip(h_grads, (dq, dk, dv)):
+                dst.copy_(src, non_blocking=True)
+            stream.synchronize()
 
     # ---- device-resident timing: events on the launching stream, barrier + synchronize on both sides
     for _ in range(W):
@@ -324,6 +353,10 @@ def run_cuda(args, w: Workload):
     e2e_ms_all, e2e_flops_all = aggregate(e0.elapsed_time(e1), flops * K, inited, dev)
     h2d = sum(x.numel() * x.element_size() for x in host if x is not None)
     d2h = h_o.numel() * h_o.element_size() * (1 if w.no_tangents else 2) + h_lse.numel() * 4
+    if w.backward:
+        h2d = sum(x.numel() * x.element_size() for x in h_bwd) + h_lse_in.numel() * 4
+        d2h = sum(x.numel() * x.element_size() for x in h_grads)
+        launches_per_call = 3               # delta, dQ, dK/dV kernels
 
     aj.attn_jvp_plan_destroy(plan)
     if rank != 0:
@@ -343,7 +376,8 @@ def run_cuda(args, w: Workload):
         "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
         "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "api": "attn_jvp_fwd_host (pinned host buffers, copies inside the timed region)"},
+                "api": ("attn_bwd between torch copies from/to pinned host buffers (copies inside the timed region)" if w.backward
+                        else "attn_jvp_fwd_host (pinned host buffers, copies inside the timed region)")},
         "gpu_launches": K * launches_per_call,
         "clocks": clocks,
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
@@ -352,9 +386,18 @@ def run_cuda(args, w: Workload):
                      "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
                      "flops_per_launch": flops},
     }
+    if w.backward:
+        # the first backward path is plain fp32 FMA: bound by the FP32 pipe, 148 SMs x 128 lanes x 2 flop x max SM clock
+        # (DESIGN.md section 6d); the three kernels of a step are timed together (dK/dV and dQ dominate, about 60 % / 40 %)
+        alu_peak = 148 * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        line["kernel"] = "simt_fp32_backward"
+        line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                            "traffic": recorded_traffic(w.name), "peak_source": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz",
+                            "kernel": "attn_bwd_simt_kernel (dQ and dK/dV instances) + attn_bwd_delta_kernel",
+                            "flops_per_launch": flops, "frac_of_bf16_tensor_peak": achieved / peak}
     if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and not w.backward:   # (the timed oracle leg is the forward oracle)
         tf, dt, nrows, cores = time_oracle_sample(w, host_all, args.cpu_budget_s)
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{nrows} uniformly sampled query rows of head (0,0), all their allowed "

@@ -36,6 +36,7 @@ class Workload:
     clean_tangent_zero: bool = False   # teacher forcing: tQ, tK, tV rows of the clean half are zero
     no_tangents: bool = False          # plain masked attention forward: tQ = tK = tV = 0 (no JVP at inference)
     Nq: int = 0                        # full mask only: query rows when they differ from the keys (current chunk x cached prefix)
+    backward: bool = False             # the step is the primal backward (dQ, dK, dV from dO, O, lse), not the forward
 
     @property
     def block_len(self) -> int:
@@ -91,6 +92,8 @@ EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     # (PAPER.md:180), and the rollout shape: one chunk of queries against the cached prefix plus itself.
     Workload("wan13b_tf_framewise_fwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.0, 0, False, True),
     Workload("wan13b_chunk_vs_prefix_fwd", 8, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
+    # N2: the primal backward of configs[1] (first correct path: fp32 FMA kernels), two heads to keep a step short
+    Workload("wan13b_tf_framewise_bwd", 1, 2, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
 ]}
 
 
@@ -98,7 +101,7 @@ def scaled_down(w: Workload, frame_len: int, num_frames: int = 0, H: int = 0, B:
     """Same structure, smaller extent (parity cases the oracle finishes in seconds)."""
     return Workload(f"{w.name}@L{frame_len}", B or w.B, H or w.H, w.d, w.mask, frame_len,
                     num_frames or w.num_frames, w.chunk_frames, w.dtype, w.tangent_std, w.seed, w.clean_tangent_zero,
-                    w.no_tangents, 0)
+                    w.no_tangents, 0, w.backward)
 
 
 def make_inputs(w: Workload, device: str = "cpu", pin: bool = False):
