@@ -622,6 +622,10 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 }
                 continue;
             }
+            // A parity wait is only meaningful one phase at a time.  General task: tS of the last pair-step was consumed, and
+            // the pipe produced it after the MMAs of the pair-step before, so only the last phase can be open.  Primal-only
+            // task: S of the last pair-step (np - 1) only proves pair-step np - 3 complete, so np - 2 is waited for first.
+            if (primal && np >= 2) wait(BAR_PV_DONE, (c_pv - 2) & 1);
             wait(BAR_PV_DONE, (c_pv - 1) & 1);
             tc_fence_after();
             float la, lb, lc, ld, ra, rb, rc, rd;
