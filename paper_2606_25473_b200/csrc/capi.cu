@@ -141,6 +141,8 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
 aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     if (aj_status st = build_schedule(p, p->problem, kernel, tiling, p->full)) return st;
     free_schedule(p->head);
+    free_schedule(p->bwd_q);      // their tile sizes follow the kernel family
+    free_schedule(p->bwd_k);
     p->kernel = kernel; p->tiling = tiling;
     return AJ_OK;
 }
@@ -368,29 +370,61 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     for (int i = 0; i < 8; ++i)
         if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
     if (!lse || (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: NULL or misaligned");
-    // first use: the two SIMT-tiled schedules (query tiles x key ranges; key tiles x row ranges) and the delta workspace
+    // bf16, d = 128 (unless the plan was forced to the SIMT kernels): tcgen05 passes; otherwise plain-FMA kernels
+    const bool umma = umma_covers(pr) && p->kernel != AJ_KERNEL_SIMT;
+    const int tile_s = umma ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q, tile_m = umma ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+    // first use: the two schedules (query tiles x key ranges; key tiles x row ranges) and the delta workspace
     if (!p->bwd_q.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, aj::SIMT_TILE_Q, aj::SIMT_TILE_K, AJ_TILING_PER_GROUP, &s)) return st;
+        if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, tile_s, tile_m, AJ_TILING_PER_GROUP, &s)) return st;
         if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_q)) return st;
     }
     if (!p->bwd_k.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_transposed(&p->problem, &p->mask, aj::SIMT_TILE_Q, aj::SIMT_TILE_K, &s)) return st;
+        if (aj_status st = attn_jvp_schedule_create_transposed(&p->problem, &p->mask, tile_s, tile_m, &s)) return st;
         if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_k)) return st;
     }
     if (!p->d_delta) {
         cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
     }
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
     aj::BwdParams prm;
     prm.q = *q; prm.k = *k; prm.v = *v; prm.o = *o; prm.dout = *dout; prm.dq = *dq; prm.dk = *dk; prm.dv = *dv;
     prm.lse = lse; prm.delta = p->d_delta;
     prm.q_tasks = p->bwd_q.d_tasks; prm.q_kb = p->bwd_q.d_kb; prm.q_ke = p->bwd_q.d_ke;
     prm.k_tasks = p->bwd_k.d_tasks; prm.k_rb = p->bwd_k.d_kb; prm.k_re = p->bwd_k.d_ke;
     prm.B = pr.B; prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
-    cudaError_t e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, p->bwd_q.num_tasks, p->bwd_k.num_tasks, (cudaStream_t)cuda_stream);
-    if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
+    cudaError_t e;
+    if (!umma) {
+        e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, p->bwd_q.num_tasks, p->bwd_k.num_tasks, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
+        return AJ_OK;
+    }
+    e = aj::launch_bwd_delta(prm, pr.dtype, pr.d, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "backward delta kernel launch");
+    for (int pass = 0; pass < 2; ++pass) {
+        const bool keys = pass == 1;
+        const aj_plan::DevSchedule &ds = keys ? p->bwd_k : p->bwd_q;
+        aj::BwdUmmaParams up;
+        std::memset(&up, 0, sizeof(up));
+        aj_status st;
+        // stationary operands (128-row boxes) and streamed operands (64-row boxes) of the pass
+        const aj_tensor *a1 = keys ? k : q, *a2 = keys ? v : dout, *b1 = keys ? q : k, *b2 = keys ? dout : v;
+        const int64_t na = keys ? pr.Nk : pr.Nq, nb = keys ? pr.Nq : pr.Nk;
+        if ((st = encode_map(&up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(&up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(&up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+        up.out1 = keys ? *dk : *dq;
+        up.out2 = *dv;
+        up.lse = lse; up.delta = p->d_delta;
+        up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.err = p->d_counters + 2;
+        up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
+        up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
+        e = aj::launch_bwd_umma(up, keys, std::min(p->num_sms, ds.num_tasks), stream);
+        if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
+    }
     return AJ_OK;
 }
 

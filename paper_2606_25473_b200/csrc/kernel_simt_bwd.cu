@@ -171,6 +171,17 @@ cudaError_t launch_t(const BwdParams &prm, int num_q_tasks, int num_k_tasks, cud
 
 }  // namespace
 
+cudaError_t launch_bwd_delta(const BwdParams &prm, int dtype, int d, cudaStream_t stream) {
+    const int64_t rows = (int64_t)prm.B * prm.H * prm.Nq;
+    const unsigned grid = (unsigned)((rows + 3) / 4);
+    if (dtype == AJ_BF16 && d == 128) attn_bwd_delta_kernel<__nv_bfloat16, 128><<<grid, 128, 0, stream>>>(prm);
+    else if (dtype == AJ_BF16 && d == 64) attn_bwd_delta_kernel<__nv_bfloat16, 64><<<grid, 128, 0, stream>>>(prm);
+    else if (dtype == AJ_FP32 && d == 128) attn_bwd_delta_kernel<float, 128><<<grid, 128, 0, stream>>>(prm);
+    else if (dtype == AJ_FP32 && d == 64) attn_bwd_delta_kernel<float, 64><<<grid, 128, 0, stream>>>(prm);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_bwd_simt(const BwdParams &prm, int dtype, int d, int num_q_tasks, int num_k_tasks, cudaStream_t stream) {
     if (dtype == AJ_FP32 && d == 64) return launch_t<float, 64>(prm, num_q_tasks, num_k_tasks, stream);
     if (dtype == AJ_FP32 && d == 128) return launch_t<float, 128>(prm, num_q_tasks, num_k_tasks, stream);

@@ -1,0 +1,343 @@
+// bf16 primal backward of masked attention for sm_100a: TMA -> shared-memory ring -> tcgen05.mma with
+// TMEM accumulators.  Same formulas as kernel_simt_bwd.cu (the VJP of Eq. 42):
+//     p_ab = exp(s <q_a, k_b> - lse_a),  dP_ab = <dO_a, v_b>,  dS_ab = p_ab (dP_ab - delta_a),  delta_a = <dO_a, O_a>
+//     dQ_a = s sum_b dS_ab k_b ;   dK_b = s sum_a dS_ab q_a ;   dV_b = sum_a p_ab dO_a
+// Two passes of ONE kernel, because the two are the same computation with the roles swapped:
+//   a CTA keeps 128 STATIONARY rows (A1, A2) in shared memory and streams 64-row tiles (B1, B2) of the other side:
+//     X  = A1 B1^T,  Y = A2 B2^T            2 x 8 MMAs (M128 N64 K16), A and B from shared memory   -> TMEM
+//     W  = exp2(X s log2e - lse log2e),  Z = W o (Y - delta)         softmax warps, thread = stationary row = TMEM lane
+//     acc1 += Z B1   (and acc2 += W B2)     4 (+4) MMAs (M128 N128 K16), A = bf16 Z / W in TMEM, B MN-major
+//   KEYS = false: stationary = query rows (A1 = Q, A2 = dO), streamed = keys (B1 = K, B2 = V): acc1 = dQ / s; lse and
+//                 delta belong to the thread's own row.
+//   KEYS = true:  stationary = keys (A1 = K, A2 = V), streamed = query rows (B1 = Q, B2 = dO): X = S^T, Y = dP^T,
+//                 acc1 = dK / s, acc2 = dV; lse and delta belong to the COLUMNS and are staged in shared memory per tile.
+//                 The tasks come from the transposed schedule (key tiles with the row ranges that see them).
+// S and dP are therefore computed twice (7 contractions instead of the minimal 5) in exchange for no atomics and no
+// cross-CTA reduction of dQ.  X/Y are double-buffered in TMEM (acc1 128 | acc2 128 | X0 Y0 X1 Y1 64 columns each), so
+// the MMAs of tile j + 1 run under the softmax of tile j.  Roles (8 warps): warp 0 TMA producer, warp 1 MMA issuer,
+// warp 2 TMEM allocator, warps 4-7 softmax / epilogue.  Tasks are dealt round-robin (task list is longest-first).
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+
+#include "kernels.hpp"
+#include "umma_ptx.cuh"
+
+namespace aj {
+
+namespace {
+
+using namespace ptx;
+
+constexpr int BR = UMMA_TILE_Q;        // 128 stationary rows
+constexpr int BC = UMMA_TILE_K;        // 64 streamed rows per tile
+constexpr int D = 128;
+constexpr int NSTAGE = 4;              // ring slots of 32 KB: [B1 h0 | B1 h1 | B2 h0 | B2 h1]
+constexpr uint32_t A_BYTES = BR * D * 2;           // 32 KB
+constexpr uint32_t AHALF_BYTES = BR * 64 * 2;      // one 64-column swizzle block of a stationary operand: 16 KB
+constexpr uint32_t BHALF_BYTES = BC * 64 * 2;      // 8 KB
+constexpr uint32_t SLOT_BYTES = 4 * BHALF_BYTES;   // 32 KB
+constexpr uint32_t SMEM_TILES = 2 * A_BYTES + NSTAGE * SLOT_BYTES;  // 192 KB
+constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 2048 /*struct Shared*/;
+constexpr int NTHREADS = 256;
+
+constexpr uint32_t TM_ACC1 = 0, TM_ACC2 = 128, TM_X0 = 256, TM_Y0 = 320, TM_BUF = 128;   // X1 = X0 + 128, Y1 = Y0 + 128
+
+enum {
+    BAR_A_FULL = 0, BAR_A_EMPTY,
+    BAR_B_FULL, BAR_B_EMPTY = BAR_B_FULL + NSTAGE,
+    BAR_X_FULL = BAR_B_EMPTY + NSTAGE,      // x2: X, Y of the buffer complete
+    BAR_W_FULL = BAR_X_FULL + 2,            // x2: Z (and W) stored by the four softmax warps
+    BAR_ACC_DONE = BAR_W_FULL + 2,          // every MMA into acc1 / acc2 of the tile is complete (one phase per tile)
+    NUM_BARS
+};
+
+constexpr uint32_t make_idesc(int n, bool b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BR >> 4) << 24);
+}
+constexpr uint32_t IDESC_XY = make_idesc(BC, false);     // 128 x  64 x 16, A and B K-major
+constexpr uint32_t IDESC_ACC = make_idesc(D, true);      // 128 x 128 x 16, A from TMEM, B MN-major
+constexpr uint32_t DESC_HI = desc_hi(1024);
+constexpr uint32_t LBO_K = desc_lo_lbo(16);              // K-major with 128 B swizzle: unused, canonical value
+constexpr uint32_t LBO_MN = desc_lo_lbo(BHALF_BYTES);    // MN-major: the two 64-column blocks of a streamed operand are 8 KB apart
+
+struct Shared {
+    uint64_t bars[NUM_BARS];
+    uint32_t tmem_base;
+    int abort_flag;
+    float stage[2][2][BC];     // KEYS pass: [buffer][0 = lse * log2e (+inf past the range end), 1 = delta][streamed row]
+};
+static_assert(sizeof(Shared) <= 2048, "struct Shared outgrew its reservation");
+
+// Walks the streamed tiles of a task: its ranges [rb, rb + rc), each cut into BC-row tiles from its start.
+struct TileCursor {
+    const int32_t *b, *e;
+    int r, rend, m, mend;
+    __device__ void init(const int32_t *begin, const int32_t *end, int rb, int rc) {
+        b = begin; e = end; r = rb; rend = rb + rc;
+        if (r < rend) { m = b[r]; mend = e[r]; } else { m = 0; mend = 0; }
+    }
+    __device__ int row() const { return m; }
+    __device__ int valid() const { return min(BC, mend - m); }
+    __device__ void next() {
+        m += BC;
+        if (m >= mend) { ++r; if (r < rend) { m = b[r]; mend = e[r]; } }
+    }
+};
+
+template <bool KEYS>
+__global__ void __launch_bounds__(NTHREADS, 1)
+attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t tiles = (raw + 1023u) & ~1023u;
+    Shared *sh = reinterpret_cast<Shared *>(smem_raw + (tiles - raw) + SMEM_TILES);
+    const uint32_t sA1 = tiles, sA2 = tiles + A_BYTES, sRing = tiles + 2 * A_BYTES;
+    const uint32_t bars = smem_u32(sh->bars);
+    const Waiter wait{bars, &sh->abort_flag, prm.err};
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bars + 8 * BAR_A_FULL, 1);
+        mbar_init(bars + 8 * BAR_A_EMPTY, 1);
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bars + 8 * (BAR_B_FULL + i), 1); mbar_init(bars + 8 * (BAR_B_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(bars + 8 * (BAR_X_FULL + i), 1); mbar_init(bars + 8 * (BAR_W_FULL + i), 4); }
+        mbar_init(bars + 8 * BAR_ACC_DONE, 1);
+        sh->abort_flag = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh->tmem_base)), "r"(512u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sh->tmem_base;
+
+    if (warp == 0) {
+        // ================================================= TMA producer ==========================================
+        if (lane == 0) {
+            prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_b1); prefetch_tmap(&prm.tm_b2);
+            uint32_t ring = 0, na = 0;
+            for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
+                const aj_task task = prm.tasks[t];
+                const int n = task.num_kv_tiles;
+                if (n == 0 || sh->abort_flag) continue;
+                wait(BAR_A_EMPTY, (na & 1) ^ 1);
+                const uint32_t afull = bars + 8 * BAR_A_FULL;
+                mbar_expect_tx(afull, 2 * A_BYTES);
+                tma_load_4d(sA1, &prm.tm_a1, afull, 0, task.q_begin, task.h, task.b);
+                tma_load_4d(sA1 + AHALF_BYTES, &prm.tm_a1, afull, 64, task.q_begin, task.h, task.b);
+                tma_load_4d(sA2, &prm.tm_a2, afull, 0, task.q_begin, task.h, task.b);
+                tma_load_4d(sA2 + AHALF_BYTES, &prm.tm_a2, afull, 64, task.q_begin, task.h, task.b);
+                ++na;
+                TileCursor cur;
+                cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
+                for (int j = 0; j < n; ++j, cur.next(), ++ring) {
+                    const uint32_t slot = ring % NSTAGE;
+                    wait(BAR_B_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
+                    const uint32_t dst = sRing + slot * SLOT_BYTES, full = bars + 8 * (BAR_B_FULL + slot);
+                    mbar_expect_tx(full, SLOT_BYTES);
+                    const int row = cur.row();
+                    tma_load_4d(dst, &prm.tm_b1, full, 0, row, task.h, task.b);
+                    tma_load_4d(dst + BHALF_BYTES, &prm.tm_b1, full, 64, row, task.h, task.b);
+                    tma_load_4d(dst + 2 * BHALF_BYTES, &prm.tm_b2, full, 0, row, task.h, task.b);
+                    tma_load_4d(dst + 3 * BHALF_BYTES, &prm.tm_b2, full, 64, row, task.h, task.b);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================================================= MMA issuer ============================================
+        // Every lane runs the control flow (counters and descriptors stay warp-uniform), one elected lane issues.
+        const bool leader = elect_one();
+        const uint32_t a1_lo = ((sA1 >> 4) & 0x3FFF) | LBO_K, a2_lo = ((sA2 >> 4) & 0x3FFF) | LBO_K;
+        uint32_t ring = 0, na = 0, g = 0;   // g = tiles issued so far (selects the X/Y buffer and the barrier phases)
+        auto issue_xy = [&](uint32_t gj, uint32_t item) {
+            const uint32_t slot = item % NSTAGE;
+            wait(BAR_B_FULL + slot, (item / NSTAGE) & 1);
+            tc_fence_after();
+            const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_K, b2_lo = b1_lo + ((2 * BHALF_BYTES) >> 4);
+            const uint32_t tX = tmem + TM_X0 + (gj & 1) * TM_BUF, tY = tmem + TM_Y0 + (gj & 1) * TM_BUF;
+            if (leader) {
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t aoff = ((ks >> 2) * AHALF_BYTES + (ks & 3) * 32) >> 4;
+                    const uint32_t boff = ((ks >> 2) * BHALF_BYTES + (ks & 3) * 32) >> 4;
+                    mma_ss(tX, a1_lo + aoff, DESC_HI, b1_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // X = A1 B1^T  (S or S^T)
+                    mma_ss(tY, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // Y = A2 B2^T  (dP or dP^T)
+                }
+                tc_commit(bars + 8 * (BAR_X_FULL + (gj & 1)));
+            }
+            __syncwarp();
+        };
+        for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
+            const int n = (int)warp_uniform((uint32_t)prm.tasks[t].num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
+            if (n <= 0) continue;
+            wait(BAR_A_FULL, na & 1);
+            ++na;
+            tc_fence_after();
+            issue_xy(g, ring);
+            for (int j = 0; j < n; ++j) {
+                const uint32_t gj = g + j, b = gj & 1, item = ring + j, slot = item % NSTAGE;
+                if (j + 1 < n) issue_xy(gj + 1, item + 1);
+                else if (leader) tc_commit(bars + 8 * BAR_A_EMPTY);      // every X, Y of this task has been issued
+                // streamed tile as MN-major B operand: row r at r*128 bytes inside each 64-column block, 16-row K steps 2 KB apart
+                const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_MN, b2_lo = b1_lo + ((2 * BHALF_BYTES) >> 4);
+                const uint32_t tW = tmem + TM_X0 + b * TM_BUF, tZ = tmem + TM_Y0 + b * TM_BUF;
+                const uint32_t acc = j > 0 ? 1u : 0u;
+                wait(BAR_W_FULL + b, (gj >> 1) & 1);
+                tc_fence_after();
+                if (leader) {
+#pragma unroll
+                    for (int ks = 0; ks < BC / 16; ++ks)        // acc1 += Z B1   (dQ += dS K | dK += dS^T Q)
+                        mma_ts(tmem + TM_ACC1, tZ + ks * 8, b1_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
+                    if (KEYS) {
+#pragma unroll
+                        for (int ks = 0; ks < BC / 16; ++ks)    // acc2 += W B2   (dV += P^T dO)
+                            mma_ts(tmem + TM_ACC2, tW + ks * 8, b2_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
+                    }
+                    tc_commit(bars + 8 * (BAR_B_EMPTY + slot));
+                    tc_commit(bars + 8 * BAR_ACC_DONE);
+                }
+                __syncwarp();
+            }
+            g += n;
+            ring += n;
+        }
+    } else if (warp >= 4) {
+        // ================================================= exp / dS / epilogue (thread = stationary row = TMEM lane) ==
+        const int row = threadIdx.x - 128;
+        const int st = threadIdx.x - 128;                          // staging duty in the KEYS pass: 0..63 lse, 64..127 delta
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const float sl2 = prm.scale_log2;
+        constexpr float LOG2E = 1.4426950408889634f;
+        uint32_t g = 0;
+        for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
+            if (sh->abort_flag) break;
+            const aj_task task = prm.tasks[t];
+            const int n = task.num_kv_tiles;
+            const bool store = row < task.q_rows;
+            const int64_t grow = task.q_begin + row;
+            const float *lse = prm.lse + ((int64_t)task.b * prm.H + task.h) * prm.Nq;
+            const float *del = prm.delta + ((int64_t)task.b * prm.H + task.h) * prm.Nq;
+            // dQ pass: this thread's own row (rows past the group's end are computed on neighbouring data and never stored;
+            // a row without keys has lse = -inf and belongs to a task without tiles)
+            float my_l2 = 0.f, my_del = 0.f;
+            if (!KEYS && store) { my_l2 = lse[grow] * LOG2E; my_del = del[grow]; }
+            TileCursor cur;
+            cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
+            for (int j = 0; j < n; ++j, cur.next()) {
+                const uint32_t gj = g + j, b = gj & 1;
+                const uint32_t tX = tmem + lane_base + TM_X0 + b * TM_BUF, tY = tmem + lane_base + TM_Y0 + b * TM_BUF;
+                const int valid = cur.valid();
+                if (KEYS) {
+                    // lse (in log2 units; +inf past the range end, so that W = 0 there) and delta of the 64 streamed rows
+                    const int c = st & (BC - 1);
+                    const bool ok = c < valid;
+                    const int64_t qrow = cur.row() + c;
+                    sh->stage[b][st >> 6][c] = st < BC ? (ok ? lse[qrow] * LOG2E : INFINITY) : (ok ? del[qrow] : 0.f);
+                    named_bar_sync(1, 128);
+                }
+                wait(BAR_X_FULL + b, (gj >> 1) & 1);
+                tc_fence_after();
+                uint32_t xu[2][32], yu[2][32];
+                tmem_ld32(tX, xu[0]);
+                tmem_ld32(tX + 32, xu[1]);
+                tmem_ld32(tY, yu[0]);
+                tmem_ld32(tY + 32, yu[1]);
+                tc_wait_ld(xu[0], xu[1]);
+                tc_wait_ld(yu[0], yu[1]);
+                uint32_t wk[32], zk[32];
+#pragma unroll
+                for (int c = 0; c < BC; c += 2) {
+                    float l0, l1, d0, d1;
+                    if (KEYS) {
+                        l0 = sh->stage[b][0][c]; l1 = sh->stage[b][0][c + 1];
+                        d0 = sh->stage[b][1][c]; d1 = sh->stage[b][1][c + 1];
+                    } else {
+                        l0 = c < valid ? my_l2 : INFINITY; l1 = c + 1 < valid ? my_l2 : INFINITY;
+                        d0 = my_del; d1 = my_del;
+                    }
+                    // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
+                    const float w0 = ex2(fmaf(__uint_as_float(xu[c >> 5][c & 31]), sl2, -l0));
+                    const float w1 = ex2(fmaf(__uint_as_float(xu[c >> 5][(c + 1) & 31]), sl2, -l1));
+                    const float z0 = w0 * (__uint_as_float(yu[c >> 5][c & 31]) - d0);
+                    const float z1 = w1 * (__uint_as_float(yu[c >> 5][(c + 1) & 31]) - d1);
+                    wk[c >> 1] = pack_bf16(w0, w1);
+                    zk[c >> 1] = pack_bf16(z0, z1);
+                }
+                if (KEYS) tmem_st32(tX, wk);
+                tmem_st32(tY, zk);
+                tc_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bars + 8 * (BAR_W_FULL + b));
+            }
+            // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV ----
+            __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
+            __nv_bfloat16 *o2 = KEYS ? (__nv_bfloat16 *)prm.out2.ptr + task.b * prm.out2.stride_b + task.h * prm.out2.stride_h + grow * prm.out2.stride_n : nullptr;
+            if (n == 0) {                                           // a row without keys / a key no row sees: zeros
+                if (store) {
+                    const uint4 z = make_uint4(0, 0, 0, 0);
+                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
+                }
+                continue;
+            }
+            // the last two tiles' MMAs, one barrier phase at a time (X of the last tile only proves tile n - 3 complete)
+            if (n >= 2) wait(BAR_ACC_DONE, (g + n - 2) & 1);
+            wait(BAR_ACC_DONE, (g + n - 1) & 1);
+            tc_fence_after();
+            g += n;
+#pragma unroll 1
+            for (int cb = 0; cb < D; cb += 32) {
+                uint32_t a1[32], a2[32];
+                tmem_ld32(tmem + lane_base + TM_ACC1 + cb, a1);
+                if (KEYS) tmem_ld32(tmem + lane_base + TM_ACC2 + cb, a2);
+                if (KEYS) tc_wait_ld(a1, a2); else tc_wait_ld(a1);
+                if (store) {
+#pragma unroll
+                    for (int v4 = 0; v4 < 4; ++v4) {
+                        uint32_t w1[4], w2[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const int c = v4 * 8 + 2 * e;
+                            w1[e] = pack_bf16(__uint_as_float(a1[c]) * prm.scale, __uint_as_float(a1[c + 1]) * prm.scale);
+                            if (KEYS) w2[e] = pack_bf16(__uint_as_float(a2[c]), __uint_as_float(a2[c + 1]));
+                        }
+                        *(uint4 *)(o1 + cb + v4 * 8) = make_uint4(w1[0], w1[1], w1[2], w1[3]);
+                        if (KEYS) *(uint4 *)(o2 + cb + v4 * 8) = make_uint4(w2[0], w2[1], w2[2], w2[3]);
+                    }
+                }
+            }
+            tc_fence_before();
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream) {
+    if (grid <= 0 || prm.num_tasks <= 0) return cudaSuccess;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(attn_bwd_umma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(attn_bwd_umma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    if (keys) attn_bwd_umma_kernel<true><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
+    else attn_bwd_umma_kernel<false><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
+    return cudaGetLastError();
+}
+
+}  // namespace aj

@@ -37,6 +37,22 @@ struct BwdParams {
 };
 cudaError_t launch_bwd_simt(const BwdParams &prm, int dtype, int d, int num_q_tasks, int num_k_tasks, cudaStream_t stream);
 
+// Primal backward on tcgen05 (kernel_umma_bwd_sm100.cu; bf16, d = 128): one pass with query tiles stationary (dQ),
+// one with key tiles stationary (dK, dV).  a1, a2: stationary operands (box {64, 128}); b1, b2: streamed (box {64, 64}).
+struct BwdUmmaParams {
+    CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2;
+    aj_tensor out1, out2;             // dQ | dK, dV
+    const float *lse, *delta;         // [B, H, Nq]
+    const aj_task *tasks;
+    const int32_t *r_begin, *r_end;   // the tasks' streamed ranges
+    int32_t *err;                     // abort code word of the plan
+    int32_t num_tasks, H, Nq;
+    float scale, scale_log2;
+};
+cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream);
+// delta kernel of kernel_simt_bwd.cu alone (shared by both backward paths)
+cudaError_t launch_bwd_delta(const BwdParams &prm, int dtype, int d, cudaStream_t stream);
+
 // bf16, d = 128, tcgen05 + TMEM + TMA (kernel_umma_sm100.cu)
 struct UmmaParams {
     CUtensorMap tm_q, tm_tq;    // box {64, 128, 1, 1} over [B, H, Nq, d], SWIZZLE_128B

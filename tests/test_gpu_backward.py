@@ -30,11 +30,12 @@ def _dout(w: Workload, seed=99):
     return torch.randn((w.B, w.H, w.num_queries, w.d), generator=g).to(w.torch_dtype)
 
 
-def run_fwd_bwd(w: Workload, x, dout, plan=None):
-    """-> (dq, dk, dv) on the CPU; the gradients start as NaN so that an unwritten element fails the comparison."""
+def run_fwd_bwd(w: Workload, x, dout, plan=None, kernel=aj.AJ_KERNEL_AUTO):
+    """-> (dq, dk, dv) on the CPU; the gradients start as NaN so that an unwritten element fails the comparison.
+    kernel = AJ_KERNEL_SIMT forces the plain-FMA forward and backward kernels on bf16 inputs."""
     own = plan is None
     if own:
-        plan = make_plan(w)
+        plan = make_plan(w, kernel)
     q, k, v, tq, tk, tv = [t.cuda() for t in x]
     o, to = torch.empty_like(q), torch.empty_like(q)
     lse = torch.empty((w.B, w.H, w.num_queries), dtype=torch.float32, device="cuda")
@@ -43,6 +44,7 @@ def run_fwd_bwd(w: Workload, x, dout, plan=None):
     dk, dv = torch.full_like(k, float("nan")), torch.full_like(k, float("nan"))
     aj.attn_bwd(plan, q, k, v, o, lse, dout.cuda(), dq, dk, dv, 0)
     torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0, "a backward kernel abandoned its launch (pipeline wait timed out)"
     if own:
         aj.attn_jvp_plan_destroy(plan)
     return dq.cpu(), dk.cpu(), dv.cpu()
@@ -80,6 +82,13 @@ SMALL = [
     Workload("bwd_tf_bf16", 1, 2, 128, "teacher_forcing", 200, 3, 1, "bf16", 0.1, seed=4),      # forward = CTA-pair tcgen05 kernel
     Workload("bwd_bc_bf16_B2", 2, 2, 128, "block_causal", 137, 4, 1, "bf16", 0.1, seed=5),
     Workload("bwd_tf_bf16_d64", 1, 2, 64, "teacher_forcing", 50, 3, 1, "bf16", 0.1, seed=6),
+    # tcgen05 backward (bf16, d = 128): several 128-row stationary tiles and 64-row streamed tiles, ragged everywhere
+    Workload("bwd_tf_chunk_bf16", 1, 2, 128, "teacher_forcing", 100, 6, 3, "bf16", 0.1, seed=7),
+    Workload("bwd_full_bf16_N517", 1, 3, 128, "full", 517, 1, 1, "bf16", 0.1, seed=8),
+    Workload("bwd_tf_bf16_L8", 1, 1, 128, "teacher_forcing", 8, 2, 1, "bf16", 0.1, seed=9),          # every tile partial
+    Workload("bwd_tf_bf16_L64x5", 1, 1, 128, "teacher_forcing", 64, 5, 1, "bf16", 0.1, seed=10),     # exact streamed tiles
+    Workload("bwd_tf_bf16_L1560_F2", 1, 1, 128, "teacher_forcing", 1560, 2, 1, "bf16", 0.1, seed=11),
+    Workload("bwd_tf_bf16_unit", 1, 2, 128, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=12),      # unit-variance dO-scale tangents irrelevant; peaked scores below
 ]
 
 
@@ -98,13 +107,28 @@ def test_backward_small_every_element(w):
         assert max(errs.values()) < 2e-5
 
 
-def test_backward_ranges_mask_unseen_keys_and_keyless_rows():
+def test_backward_bf16_tcgen05_and_simt_paths_agree():
+    w = SMALL[4]
+    x = make_inputs(w)
+    x[0] = (x[0].float() * 3.0).to(torch.bfloat16)          # peaked scores: p spans many orders of magnitude
+    dout = _dout(w)
+    a = run_fwd_bwd(w, x, dout)
+    b = run_fwd_bwd(w, x, dout, kernel=aj.AJ_KERNEL_SIMT)
+    check(w, x, dout, a)
+    check(w, x, dout, b)
+    for u, v in zip(a, b):
+        assert max_norm_err(u.double().numpy(), v.double().numpy()) <= 1e-2
+
+
+@pytest.mark.parametrize("dtype", ["fp32", "bf16"])
+def test_backward_ranges_mask_unseen_keys_and_keyless_rows(dtype):
     Nq, Nk, d = 300, 421, 128
     groups = [(0, 130, [(3, 70), (70, 131), (200, 400)]), (150, 290, [(64, 65)]), (290, 300, [])]
     g = torch.Generator().manual_seed(9)
-    q, dout = [torch.randn((1, 2, Nq, d), generator=g) for _ in range(2)]
-    k, v = [torch.randn((1, 2, Nk, d), generator=g) for _ in range(2)]
-    prob = aj.make_problem(1, 2, Nq, Nk, d, aj.AJ_FP32)
+    tdt = torch.bfloat16 if dtype == "bf16" else torch.float32
+    q, dout = [torch.randn((1, 2, Nq, d), generator=g).to(tdt) for _ in range(2)]
+    k, v = [torch.randn((1, 2, Nk, d), generator=g).to(tdt) for _ in range(2)]
+    prob = aj.make_problem(1, 2, Nq, Nk, d, aj.AJ_BF16 if dtype == "bf16" else aj.AJ_FP32)
     mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
     plan = aj.attn_jvp_plan_create(prob, mask)
     dev = [t.cuda() for t in (q, k, v)]
@@ -116,13 +140,14 @@ def test_backward_ranges_mask_unseen_keys_and_keyless_rows():
     dk, dv = torch.full_like(dev[1], float("nan")), torch.full_like(dev[1], float("nan"))
     aj.attn_bwd(plan, *dev, o, lse, dout.cuda(), dq, dk, dv, 0)
     torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
     aj.attn_jvp_plan_destroy(plan)
     om = oracle.ranges_mask(groups)
     for h in range(2):
         rq, rk, rv = oracle.attn_bwd_head(om, widen(q[0, h]), widen(k[0, h]), widen(v[0, h]), widen(dout[0, h]), 1.0 / np.sqrt(d))
-        assert max_norm_err(dq[0, h].cpu().double().numpy(), rq) <= 1e-4
-        assert max_norm_err(dk[0, h].cpu().double().numpy(), rk) <= 1e-4
-        assert max_norm_err(dv[0, h].cpu().double().numpy(), rv) <= 1e-4
+        assert max_norm_err(dq[0, h].cpu().double().numpy(), rq) <= TOL[dtype]
+        assert max_norm_err(dk[0, h].cpu().double().numpy(), rk) <= TOL[dtype]
+        assert max_norm_err(dv[0, h].cpu().double().numpy(), rv) <= TOL[dtype]
     unseen = np.r_[0:3, 131:200, 400:421]                    # keys no row sees: exact zeros, and written
     keyless = np.r_[130:150, 290:300]
     assert torch.count_nonzero(dk[0, :, unseen]) == 0 and torch.count_nonzero(dv[0, :, unseen]) == 0
