@@ -387,14 +387,12 @@ def run_cuda(args, w: Workload):
                      "flops_per_launch": flops},
     }
     if w.backward:
-        # the first backward path is plain fp32 FMA: bound by the FP32 pipe, 148 SMs x 128 lanes x 2 flop x max SM clock
-        # (DESIGN.md section 6d); the three kernels of a step are timed together (dK/dV and dQ dominate, about 60 % / 40 %)
-        alu_peak = 148 * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-        line["kernel"] = "simt_fp32_backward"
-        line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                            "traffic": recorded_traffic(w.name), "peak_source": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz",
-                            "kernel": "attn_bwd_simt_kernel (dQ and dK/dV instances) + attn_bwd_delta_kernel",
-                            "flops_per_launch": flops, "frac_of_bf16_tensor_peak": achieved / peak}
+        # three kernels per step, timed together: delta (HBM-bound, small), the dQ pass and the dK/dV pass of the tcgen05
+        # backward kernel (bf16, d = 128).  The 10*d convention counts the minimal five contractions;
+        # the two-pass kernel executes seven (S and dP are recomputed in the second pass).
+        line["kernel"] = "tcgen05_backward_two_pass" if (w.dtype == "bf16" and w.d == 128) else "simt_fp32_backward"
+        line["roofline"].update(kernel="attn_bwd_umma_kernel<false> (dQ) + attn_bwd_umma_kernel<true> (dK, dV) + attn_bwd_delta_kernel",
+                                executed_over_counted_contractions=7.0 / 5.0)
     if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
     if world == 1 and not args.no_cpu_baseline and not w.backward:   # (the timed oracle leg is the forward oracle)

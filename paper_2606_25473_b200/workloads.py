@@ -92,8 +92,8 @@ EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     # (PAPER.md:180), and the rollout shape: one chunk of queries against the cached prefix plus itself.
     Workload("wan13b_tf_framewise_fwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.0, 0, False, True),
     Workload("wan13b_chunk_vs_prefix_fwd", 8, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
-    # N2: the primal backward of configs[1] (first correct path: fp32 FMA kernels), two heads to keep a step short
-    Workload("wan13b_tf_framewise_bwd", 1, 2, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
+    # N2: the primal backward of configs[1]
+    Workload("wan13b_tf_framewise_bwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
 ]}
 
 
