@@ -84,7 +84,7 @@ int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACK
 
 // Build the schedule of `prob` (the plan's problem, or one head of it) for `kernel` / `tiling` and upload it into `ds`
 // (left unchanged on failure).
-aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds);
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers = 0);
 
 aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int32_t tiling, aj_plan::DevSchedule &ds) {
     const int tq = kernel == AJ_KERNEL_UMMA_PAIR ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
@@ -99,15 +99,16 @@ aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int
 }
 
 // Uploads `s` (owned by `ds` afterwards; destroyed on failure, `ds` then unchanged).
-aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds) {
+// workers > 0: also assign the tasks to that many persistent workers (head-major lists, see assign_workers).
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers) {
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r)   // row_begin | row_end << 16 (both < 32768) | key-tangents-zero << 31
         rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16) | (s->entries.k_tz[r] ? 0x80000000u : 0u);
     std::vector<int32_t> pair_off, pair_ids;
     int num_pairs = 0;
-    if (kernel == AJ_KERNEL_UMMA_PAIR) {
-        num_pairs = (int)std::min<size_t>(std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
+    if (kernel == AJ_KERNEL_UMMA_PAIR || workers > 0) {
+        num_pairs = (int)std::min<size_t>(workers > 0 ? workers : std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
         aj::assign_workers(s->tasks, s->entries, s->tile_k, num_pairs, pair_off, pair_ids);
     }
     aj_task *d_tasks = nullptr;
@@ -377,12 +378,12 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     if (!p->bwd_q.sched) {
         aj_schedule *s = nullptr;
         if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, tile_s, tile_m, AJ_TILING_PER_GROUP, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_q)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_q, umma ? p->num_sms : 0)) return st;
     }
     if (!p->bwd_k.sched) {
         aj_schedule *s = nullptr;
         if (aj_status st = attn_jvp_schedule_create_transposed(&p->problem, &p->mask, tile_s, tile_m, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_k)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_k, umma ? p->num_sms : 0)) return st;
     }
     if (!p->d_delta) {
         cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
@@ -420,9 +421,10 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
         up.out2 = *dv;
         up.lse = lse; up.delta = p->d_delta;
         up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.err = p->d_counters + 2;
+        up.cta_off = ds.d_pair_off; up.cta_ids = ds.d_pair_ids;
         up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
         up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
-        e = aj::launch_bwd_umma(up, keys, std::min(p->num_sms, ds.num_tasks), stream);
+        e = aj::launch_bwd_umma(up, keys, ds.num_pairs, stream);
         if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
     }
     return AJ_OK;

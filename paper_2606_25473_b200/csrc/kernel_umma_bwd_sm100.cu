@@ -15,7 +15,8 @@
 // S and dP are therefore computed twice (7 contractions instead of the minimal 5) in exchange for no atomics and no
 // cross-CTA reduction of dQ.  X/Y are double-buffered in TMEM (acc1 128 | acc2 128 | X0 Y0 X1 Y1 64 columns each), so
 // the MMAs of tile j + 1 run under the softmax of tile j.  Roles (8 warps): warp 0 TMA producer, warp 1 MMA issuer,
-// warp 2 TMEM allocator, warps 4-7 softmax / epilogue.  Tasks are dealt round-robin (task list is longest-first).
+// warp 2 TMEM allocator, warps 4-7 softmax / epilogue.  Tasks are assigned to the CTAs by the host, head by head and most
+// expensive first (assign_workers), so that all CTAs stream the same head's operands through L2 at the same time.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -66,7 +67,7 @@ struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
     int abort_flag;
-    float stage[2][2][BC];     // KEYS pass: [buffer][0 = lse * log2e (+inf past the range end), 1 = delta][streamed row]
+    alignas(16) float stage[2][2][BC];     // KEYS pass: [buffer][0 = lse * log2e (+inf past the range end), 1 = delta][streamed row]
 };
 static_assert(sizeof(Shared) <= 2048, "struct Shared outgrew its reservation");
 
@@ -97,6 +98,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
     const uint32_t bars = smem_u32(sh->bars);
     const Waiter wait{bars, &sh->abort_flag, prm.err};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int list_begin = prm.cta_off[blockIdx.x], list_end = prm.cta_off[blockIdx.x + 1];
 
     if (threadIdx.x == 0) {
         mbar_init(bars + 8 * BAR_A_FULL, 1);
@@ -122,8 +124,8 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
         if (lane == 0) {
             prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_b1); prefetch_tmap(&prm.tm_b2);
             uint32_t ring = 0, na = 0;
-            for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
-                const aj_task task = prm.tasks[t];
+            for (int it = list_begin; it < list_end; ++it) {
+                const aj_task task = prm.tasks[prm.cta_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
                 wait(BAR_A_EMPTY, (na & 1) ^ 1);
@@ -173,8 +175,8 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
             }
             __syncwarp();
         };
-        for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
-            const int n = (int)warp_uniform((uint32_t)prm.tasks[t].num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
+        for (int it = list_begin; it < list_end; ++it) {
+            const int n = (int)warp_uniform((uint32_t)prm.tasks[prm.cta_ids[it]].num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
             if (n <= 0) continue;
             wait(BAR_A_FULL, na & 1);
             ++na;
@@ -215,9 +217,9 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
         const float sl2 = prm.scale_log2;
         constexpr float LOG2E = 1.4426950408889634f;
         uint32_t g = 0;
-        for (int t = blockIdx.x; t < prm.num_tasks; t += gridDim.x) {
+        for (int it = list_begin; it < list_end; ++it) {
             if (sh->abort_flag) break;
-            const aj_task task = prm.tasks[t];
+            const aj_task task = prm.tasks[prm.cta_ids[it]];
             const int n = task.num_kv_tiles;
             const bool store = row < task.q_rows;
             const int64_t grow = task.q_begin + row;
@@ -250,24 +252,37 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 tmem_ld32(tY + 32, yu[1]);
                 tc_wait_ld(xu[0], xu[1]);
                 tc_wait_ld(yu[0], yu[1]);
-                uint32_t wk[32], zk[32];
+                if (!KEYS && valid < BC) {                          // past the range end: S = -inf, so W = Z = 0
 #pragma unroll
-                for (int c = 0; c < BC; c += 2) {
-                    float l0, l1, d0, d1;
+                    for (int c = 0; c < BC; ++c) if (c >= valid) xu[c >> 5][c & 31] = 0xff800000u;
+                }
+                uint32_t wk[32], zk[32];
+                const uint64_t sl2_2 = pack2(sl2, sl2), myl_2 = pack2(-my_l2, -my_l2), myd_2 = pack2(-my_del, -my_del);
+#pragma unroll
+                for (int c4 = 0; c4 < BC; c4 += 4) {
+                    uint64_t nl[2], nd[2];                          // -lse * log2e and -delta of columns c4 .. c4 + 3
                     if (KEYS) {
-                        l0 = sh->stage[b][0][c]; l1 = sh->stage[b][0][c + 1];
-                        d0 = sh->stage[b][1][c]; d1 = sh->stage[b][1][c + 1];
+                        const float4 l4 = *reinterpret_cast<const float4 *>(&sh->stage[b][0][c4]);
+                        const float4 d4 = *reinterpret_cast<const float4 *>(&sh->stage[b][1][c4]);
+                        nl[0] = pack2(-l4.x, -l4.y); nl[1] = pack2(-l4.z, -l4.w);
+                        nd[0] = pack2(-d4.x, -d4.y); nd[1] = pack2(-d4.z, -d4.w);
                     } else {
-                        l0 = c < valid ? my_l2 : INFINITY; l1 = c + 1 < valid ? my_l2 : INFINITY;
-                        d0 = my_del; d1 = my_del;
+                        nl[0] = nl[1] = myl_2; nd[0] = nd[1] = myd_2;
                     }
-                    // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
-                    const float w0 = ex2(fmaf(__uint_as_float(xu[c >> 5][c & 31]), sl2, -l0));
-                    const float w1 = ex2(fmaf(__uint_as_float(xu[c >> 5][(c + 1) & 31]), sl2, -l1));
-                    const float z0 = w0 * (__uint_as_float(yu[c >> 5][c & 31]) - d0);
-                    const float z1 = w1 * (__uint_as_float(yu[c >> 5][(c + 1) & 31]) - d1);
-                    wk[c >> 1] = pack_bf16(w0, w1);
-                    zk[c >> 1] = pack_bf16(z0, z1);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int c = c4 + 2 * h;
+                        // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
+                        const uint64_t x = ffma2(pack2(xu[c >> 5][c & 31], xu[c >> 5][(c + 1) & 31]), sl2_2, nl[h]);
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        const float w0 = ex2(x0), w1 = ex2(x1);
+                        const uint64_t z = fmul2(pack2(w0, w1), fadd2(pack2(yu[c >> 5][c & 31], yu[c >> 5][(c + 1) & 31]), nd[h]));
+                        float z0, z1;
+                        unpack2(z, z0, z1);
+                        wk[c >> 1] = pack_bf16(w0, w1);
+                        zk[c >> 1] = pack_bf16(z0, z1);
+                    }
                 }
                 if (KEYS) tmem_st32(tX, wk);
                 tmem_st32(tY, zk);

@@ -45,6 +45,7 @@ struct BwdUmmaParams {
     const float *lse, *delta;         // [B, H, Nq]
     const aj_task *tasks;
     const int32_t *r_begin, *r_end;   // the tasks' streamed ranges
+    const int32_t *cta_off, *cta_ids; // CTA c runs tasks cta_ids[cta_off[c] .. cta_off[c+1]) (head-major, host-assigned)
     int32_t *err;                     // abort code word of the plan
     int32_t num_tasks, H, Nq;
     float scale, scale_log2;
