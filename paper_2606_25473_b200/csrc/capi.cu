@@ -417,6 +417,7 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
         if ((st = encode_map(&up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
         if ((st = encode_map(&up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
         if ((st = encode_map(&up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+        up.a1 = *a1; up.a2 = *a2; up.Na = (int32_t)na;
         up.out1 = keys ? *dk : *dq;
         up.out2 = *dv;
         up.lse = lse; up.delta = p->d_delta;

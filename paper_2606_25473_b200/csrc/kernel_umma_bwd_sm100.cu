@@ -14,8 +14,10 @@
 //                 The tasks come from the transposed schedule (key tiles with the row ranges that see them).
 // S and dP are therefore computed twice (7 contractions instead of the minimal 5) in exchange for no atomics and no
 // cross-CTA reduction of dQ.  X/Y are double-buffered in TMEM (acc1 128 | acc2 128 | X0 Y0 X1 Y1 64 columns each), so
-// the MMAs of tile j + 1 run under the softmax of tile j.  Roles (8 warps): warp 0 TMA producer, warp 1 MMA issuer,
-// warp 2 TMEM allocator, warps 4-7 softmax / epilogue.  Tasks are assigned to the CTAs by the host, head by head and most
+// the MMAs of tile j + 1 run under the exp / dS work of tile j.  Roles (12 warps): warp 0 TMA producer, warp 1 MMA issuer,
+// warp 2 TMEM allocator, warps 4-7 and 8-11 two exp / dS / epilogue warpgroups that take ALTERNATE tiles (tile = TMEM
+// buffer = warpgroup; the tiles are independent, there is no running max), so that one tile's MUFU-bound exponentials
+// run under the other's TMEM loads, packs, stores and barrier round trips.  Tasks are assigned to the CTAs by the host, head by head and most
 // expensive first (assign_workers), so that all CTAs stream the same head's operands through L2 at the same time.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -41,17 +43,21 @@ constexpr uint32_t BHALF_BYTES = BC * 64 * 2;      // 8 KB
 constexpr uint32_t SLOT_BYTES = 4 * BHALF_BYTES;   // 32 KB
 constexpr uint32_t SMEM_TILES = 2 * A_BYTES + NSTAGE * SLOT_BYTES;  // 192 KB
 constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 2048 /*struct Shared*/;
-constexpr int NTHREADS = 256;
+constexpr int NTHREADS = 384;               // warps 0-3: TMA / MMA / TMEM alloc / idle; warps 4-7 and 8-11: exp / dS warpgroups 0, 1
 
 constexpr uint32_t TM_ACC1 = 0, TM_ACC2 = 128, TM_X0 = 256, TM_Y0 = 320, TM_BUF = 128;   // X1 = X0 + 128, Y1 = Y0 + 128
+// dQ pass: there is no acc2, and its 128 columns hold the stationary operands themselves as bf16 A operands (64 columns
+// each): the X / Y MMAs then read A from TMEM, which takes their 4 KB per instruction off the shared-memory port (the
+// port, not the tensor pipe, bounds the N = 64 shared-memory-operand form: 6 KB per 32 clk of math at 128 B/clk).
+constexpr uint32_t TM_A1 = 128, TM_A2 = 192;
 
 enum {
     BAR_A_FULL = 0, BAR_A_EMPTY,
     BAR_B_FULL, BAR_B_EMPTY = BAR_B_FULL + NSTAGE,
     BAR_X_FULL = BAR_B_EMPTY + NSTAGE,      // x2: X, Y of the buffer complete
     BAR_W_FULL = BAR_X_FULL + 2,            // x2: Z (and W) stored by the four softmax warps
-    BAR_ACC_DONE = BAR_W_FULL + 2,          // every MMA into acc1 / acc2 of the tile is complete (one phase per tile)
-    NUM_BARS
+    BAR_ACC_DONE = BAR_W_FULL + 2,          // x2 (by TMEM buffer): every MMA up to and including the tile's is complete
+    NUM_BARS = BAR_ACC_DONE + 2
 };
 
 constexpr uint32_t make_idesc(int n, bool b_mn_major) {
@@ -101,11 +107,12 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
     const int list_begin = prm.cta_off[blockIdx.x], list_end = prm.cta_off[blockIdx.x + 1];
 
     if (threadIdx.x == 0) {
-        mbar_init(bars + 8 * BAR_A_FULL, 1);
+        mbar_init(bars + 8 * BAR_A_FULL, KEYS ? 1 : 8);     // TMA transaction | one arrive per exp / dS warp (rows stored to TMEM)
         mbar_init(bars + 8 * BAR_A_EMPTY, 1);
         for (int i = 0; i < NSTAGE; ++i) { mbar_init(bars + 8 * (BAR_B_FULL + i), 1); mbar_init(bars + 8 * (BAR_B_EMPTY + i), 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(bars + 8 * (BAR_X_FULL + i), 1); mbar_init(bars + 8 * (BAR_W_FULL + i), 4); }
         mbar_init(bars + 8 * BAR_ACC_DONE, 1);
+        mbar_init(bars + 8 * (BAR_ACC_DONE + 1), 1);
         sh->abort_flag = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -128,14 +135,16 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 const aj_task task = prm.tasks[prm.cta_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
-                wait(BAR_A_EMPTY, (na & 1) ^ 1);
-                const uint32_t afull = bars + 8 * BAR_A_FULL;
-                mbar_expect_tx(afull, 2 * A_BYTES);
-                tma_load_4d(sA1, &prm.tm_a1, afull, 0, task.q_begin, task.h, task.b);
-                tma_load_4d(sA1 + AHALF_BYTES, &prm.tm_a1, afull, 64, task.q_begin, task.h, task.b);
-                tma_load_4d(sA2, &prm.tm_a2, afull, 0, task.q_begin, task.h, task.b);
-                tma_load_4d(sA2 + AHALF_BYTES, &prm.tm_a2, afull, 64, task.q_begin, task.h, task.b);
-                ++na;
+                if (KEYS) {
+                    wait(BAR_A_EMPTY, (na & 1) ^ 1);
+                    const uint32_t afull = bars + 8 * BAR_A_FULL;
+                    mbar_expect_tx(afull, 2 * A_BYTES);
+                    tma_load_4d(sA1, &prm.tm_a1, afull, 0, task.q_begin, task.h, task.b);
+                    tma_load_4d(sA1 + AHALF_BYTES, &prm.tm_a1, afull, 64, task.q_begin, task.h, task.b);
+                    tma_load_4d(sA2, &prm.tm_a2, afull, 0, task.q_begin, task.h, task.b);
+                    tma_load_4d(sA2 + AHALF_BYTES, &prm.tm_a2, afull, 64, task.q_begin, task.h, task.b);
+                    ++na;
+                }
                 TileCursor cur;
                 cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
                 for (int j = 0; j < n; ++j, cur.next(), ++ring) {
@@ -168,8 +177,13 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 for (int ks = 0; ks < D / 16; ++ks) {
                     const uint32_t aoff = ((ks >> 2) * AHALF_BYTES + (ks & 3) * 32) >> 4;
                     const uint32_t boff = ((ks >> 2) * BHALF_BYTES + (ks & 3) * 32) >> 4;
-                    mma_ss(tX, a1_lo + aoff, DESC_HI, b1_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // X = A1 B1^T  (S or S^T)
-                    mma_ss(tY, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // Y = A2 B2^T  (dP or dP^T)
+                    if (KEYS) {
+                        mma_ss(tX, a1_lo + aoff, DESC_HI, b1_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // X = A1 B1^T  (S^T)
+                        mma_ss(tY, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // Y = A2 B2^T  (dP^T)
+                    } else {
+                        mma_ts(tX, tmem + TM_A1 + ks * 8, b1_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // S  = Q K^T, Q from TMEM
+                        mma_ts(tY, tmem + TM_A2 + ks * 8, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);   // dP = dO V^T
+                    }
                 }
                 tc_commit(bars + 8 * (BAR_X_FULL + (gj & 1)));
             }
@@ -202,7 +216,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                             mma_ts(tmem + TM_ACC2, tW + ks * 8, b2_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
                     }
                     tc_commit(bars + 8 * (BAR_B_EMPTY + slot));
-                    tc_commit(bars + 8 * BAR_ACC_DONE);
+                    tc_commit(bars + 8 * (BAR_ACC_DONE + b));
                 }
                 __syncwarp();
             }
@@ -211,8 +225,9 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
         }
     } else if (warp >= 4) {
         // ================================================= exp / dS / epilogue (thread = stationary row = TMEM lane) ==
-        const int row = threadIdx.x - 128;
-        const int st = threadIdx.x - 128;                          // staging duty in the KEYS pass: 0..63 lse, 64..127 delta
+        const int wg = (warp - 4) >> 2;                            // takes the tiles whose TMEM buffer is wg
+        const int row = (threadIdx.x - 128) & (BR - 1);
+        const int st = row;                                        // staging duty in the KEYS pass: 0..63 lse, 64..127 delta
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const float sl2 = prm.scale_log2;
         constexpr float LOG2E = 1.4426950408889634f;
@@ -229,85 +244,125 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
             // a row without keys has lse = -inf and belongs to a task without tiles)
             float my_l2 = 0.f, my_del = 0.f;
             if (!KEYS && store) { my_l2 = lse[grow] * LOG2E; my_del = del[grow]; }
-            TileCursor cur;
+            if (!KEYS && n > 0) {
+                // This thread's row of Q (warpgroup 0) or dO (warpgroup 1) as a bf16 A operand in TMEM (16 elements = 8
+                // columns per MMA K step).  The previous task's MMAs are complete (its epilogue waited for them).
+                const bool in = grow < prm.Na;
+                const aj_tensor &src = wg ? prm.a2 : prm.a1;
+                const uint4 *rowp = (const uint4 *)((const __nv_bfloat16 *)src.ptr + task.b * src.stride_b + task.h * src.stride_h + grow * src.stride_n);
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+                    uint32_t ra[32];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const uint4 u = in ? rowp[half * 8 + i] : make_uint4(0, 0, 0, 0);
+                        ra[4 * i] = u.x; ra[4 * i + 1] = u.y; ra[4 * i + 2] = u.z; ra[4 * i + 3] = u.w;
+                    }
+                    tmem_st32(tmem + lane_base + (wg ? TM_A2 : TM_A1) + 32 * half, ra);
+                }
+                tc_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bars + 8 * BAR_A_FULL);
+            }
+            TileCursor cur, pf;                                    // pf runs ahead: the next tile of this warpgroup
             cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
-            for (int j = 0; j < n; ++j, cur.next()) {
-                const uint32_t gj = g + j, b = gj & 1;
+            if (((g & 1) != (uint32_t)wg) && n > 0) cur.next();    // first tile of this warpgroup
+            const int j0 = ((g & 1) != (uint32_t)wg) ? 1 : 0;
+            pf = cur;
+            // KEYS pass: lse (in log2 units; +inf past the range end, so that W = 0 there) or delta of streamed row st & 63,
+            // fetched one tile of this warpgroup ahead so that the global-memory latency is off the tile's critical path
+            auto fetch = [&](const TileCursor &c) -> float {
+                const int cc = st & (BC - 1);
+                const bool ok = cc < c.valid();
+                const int64_t qrow = c.row() + cc;
+                return st < BC ? (ok ? lse[qrow] * LOG2E : INFINITY) : (ok ? del[qrow] : 0.f);
+            };
+            float pre = 0.f;
+            if (KEYS && j0 < n) pre = fetch(pf);
+            for (int j = j0; j < n; j += 2) {
+                const uint32_t gj = g + j, b = (uint32_t)wg;
                 const uint32_t tX = tmem + lane_base + TM_X0 + b * TM_BUF, tY = tmem + lane_base + TM_Y0 + b * TM_BUF;
                 const int valid = cur.valid();
                 if (KEYS) {
-                    // lse (in log2 units; +inf past the range end, so that W = 0 there) and delta of the 64 streamed rows
-                    const int c = st & (BC - 1);
-                    const bool ok = c < valid;
-                    const int64_t qrow = cur.row() + c;
-                    sh->stage[b][st >> 6][c] = st < BC ? (ok ? lse[qrow] * LOG2E : INFINITY) : (ok ? del[qrow] : 0.f);
-                    named_bar_sync(1, 128);
+                    sh->stage[b][st >> 6][st & (BC - 1)] = pre;
+                    if (j + 2 < n) { pf.next(); pf.next(); pre = fetch(pf); }
+                    named_bar_sync(1 + wg, 128);
                 }
                 wait(BAR_X_FULL + b, (gj >> 1) & 1);
                 tc_fence_after();
-                uint32_t xu[2][32], yu[2][32];
-                tmem_ld32(tX, xu[0]);
-                tmem_ld32(tX + 32, xu[1]);
-                tmem_ld32(tY, yu[0]);
-                tmem_ld32(tY + 32, yu[1]);
-                tc_wait_ld(xu[0], xu[1]);
-                tc_wait_ld(yu[0], yu[1]);
-                if (!KEYS && valid < BC) {                          // past the range end: S = -inf, so W = Z = 0
-#pragma unroll
-                    for (int c = 0; c < BC; ++c) if (c >= valid) xu[c >> 5][c & 31] = 0xff800000u;
-                }
-                uint32_t wk[32], zk[32];
                 const uint64_t sl2_2 = pack2(sl2, sl2), myl_2 = pack2(-my_l2, -my_l2), myd_2 = pack2(-my_del, -my_del);
 #pragma unroll
-                for (int c4 = 0; c4 < BC; c4 += 4) {
-                    uint64_t nl[2], nd[2];                          // -lse * log2e and -delta of columns c4 .. c4 + 3
-                    if (KEYS) {
-                        const float4 l4 = *reinterpret_cast<const float4 *>(&sh->stage[b][0][c4]);
-                        const float4 d4 = *reinterpret_cast<const float4 *>(&sh->stage[b][1][c4]);
-                        nl[0] = pack2(-l4.x, -l4.y); nl[1] = pack2(-l4.z, -l4.w);
-                        nd[0] = pack2(-d4.x, -d4.y); nd[1] = pack2(-d4.z, -d4.w);
-                    } else {
-                        nl[0] = nl[1] = myl_2; nd[0] = nd[1] = myd_2;
-                    }
+                for (int half = 0; half < 2; ++half) {              // 32 columns at a time (register budget of 384 threads)
+                    uint32_t xu[32], yu[32];
+                    tmem_ld32(tX + 32 * half, xu);
+                    tmem_ld32(tY + 32 * half, yu);
+                    tc_wait_ld(xu, yu);
+                    if (!KEYS && valid < BC) {                      // past the range end: S = -inf, so W = Z = 0
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int c = c4 + 2 * h;
-                        // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
-                        const uint64_t x = ffma2(pack2(xu[c >> 5][c & 31], xu[c >> 5][(c + 1) & 31]), sl2_2, nl[h]);
-                        float x0, x1;
-                        unpack2(x, x0, x1);
-                        const float w0 = ex2(x0), w1 = ex2(x1);
-                        const uint64_t z = fmul2(pack2(w0, w1), fadd2(pack2(yu[c >> 5][c & 31], yu[c >> 5][(c + 1) & 31]), nd[h]));
-                        float z0, z1;
-                        unpack2(z, z0, z1);
-                        wk[c >> 1] = pack_bf16(w0, w1);
-                        zk[c >> 1] = pack_bf16(z0, z1);
+                        for (int c = 0; c < 32; ++c) if (32 * half + c >= valid) xu[c] = 0xff800000u;
                     }
+                    uint32_t wk[16], zk[16];
+#pragma unroll
+                    for (int c4 = 0; c4 < 32; c4 += 4) {
+                        uint64_t nl[2], nd[2];                      // -lse * log2e and -delta of four columns
+                        if (KEYS) {
+                            const float4 l4 = *reinterpret_cast<const float4 *>(&sh->stage[b][0][32 * half + c4]);
+                            const float4 d4 = *reinterpret_cast<const float4 *>(&sh->stage[b][1][32 * half + c4]);
+                            nl[0] = pack2(-l4.x, -l4.y); nl[1] = pack2(-l4.z, -l4.w);
+                            nd[0] = pack2(-d4.x, -d4.y); nd[1] = pack2(-d4.z, -d4.w);
+                        } else {
+                            nl[0] = nl[1] = myl_2; nd[0] = nd[1] = myd_2;
+                        }
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int c = c4 + 2 * h;
+                            // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
+                            const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl[h]);
+                            float x0, x1;
+                            unpack2(x, x0, x1);
+                            const float w0 = ex2(x0), w1 = ex2(x1);
+                            const uint64_t z = fmul2(pack2(w0, w1), fadd2(pack2(yu[c], yu[c + 1]), nd[h]));
+                            float z0, z1;
+                            unpack2(z, z0, z1);
+                            wk[c >> 1] = pack_bf16(w0, w1);
+                            zk[c >> 1] = pack_bf16(z0, z1);
+                        }
+                    }
+                    // W / Z (bf16 pairs) go to columns [16 half, 16 half + 16) of the X / Y buffer: fp32 columns that have
+                    // already been read (half 0 read [0, 32))
+                    if (KEYS) tmem_st16(tX + 16 * half, wk);
+                    tmem_st16(tY + 16 * half, zk);
                 }
-                if (KEYS) tmem_st32(tX, wk);
-                tmem_st32(tY, zk);
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bars + 8 * (BAR_W_FULL + b));
+                cur.next(); cur.next();
             }
-            // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV ----
+            // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one 64-column half ----
             __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
             __nv_bfloat16 *o2 = KEYS ? (__nv_bfloat16 *)prm.out2.ptr + task.b * prm.out2.stride_b + task.h * prm.out2.stride_h + grow * prm.out2.stride_n : nullptr;
             if (n == 0) {                                           // a row without keys / a key no row sees: zeros
                 if (store) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
-                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
+                    for (int c = 8 * wg; c < 8 * wg + 8; ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
                 }
                 continue;
             }
-            // the last two tiles' MMAs, one barrier phase at a time (X of the last tile only proves tile n - 3 complete)
-            if (n >= 2) wait(BAR_ACC_DONE, (g + n - 2) & 1);
-            wait(BAR_ACC_DONE, (g + n - 1) & 1);
+            // A parity wait is sound only if the barrier is known to be at most one phase away.  Each warpgroup waits on ITS
+            // buffer's barrier for ITS last tile jl: it consumed X(jl), which the in-order pipe produced after the MMAs of
+            // tile jl - 2 (the previous phase of that barrier), and tile jl + 2 does not exist.  Once both have passed,
+            // every tile of the task is complete.
+            {
+                const int jl = ((g + n - 1) & 1) == (uint32_t)wg ? n - 1 : n - 2;
+                if (jl >= 0) wait(BAR_ACC_DONE + wg, ((g + jl) >> 1) & 1);
+            }
+            named_bar_sync(3, 256);
             tc_fence_after();
             g += n;
 #pragma unroll 1
-            for (int cb = 0; cb < D; cb += 32) {
+            for (int cb = 64 * wg; cb < 64 * wg + 64; cb += 32) {
                 uint32_t a1[32], a2[32];
                 tmem_ld32(tmem + lane_base + TM_ACC1 + cb, a1);
                 if (KEYS) tmem_ld32(tmem + lane_base + TM_ACC2 + cb, a2);
@@ -328,6 +383,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 }
             }
             tc_fence_before();
+            named_bar_sync(3, 256);          // the accumulators and the A columns are free only when both warpgroups are done
         }
     }
 

@@ -556,6 +556,10 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                         if (need) m_ref = cand;
                     }
                 }
+                // Last pair-step of a primal-only task: S(p) only proves the MMAs of pair-step p - 2 complete (the pipe produced
+                // it after them); the MMAs of p - 1 are waited for HERE, while those of p cannot have started (they need this
+                // thread's P~), so that the epilogue's wait for pair-step p finds the barrier exactly one phase away.
+                if (primal && p + 1 == np && np >= 2) wait(BAR_PV_DONE, (c_pv - 1) & 1);
                 const uint32_t p_arrive = alt ? h_full : p_full;
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
@@ -622,10 +626,9 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 }
                 continue;
             }
-            // A parity wait is only meaningful one phase at a time.  General task: tS of the last pair-step was consumed, and
-            // the pipe produced it after the MMAs of the pair-step before, so only the last phase can be open.  Primal-only
-            // task: S of the last pair-step (np - 1) only proves pair-step np - 3 complete, so np - 2 is waited for first.
-            if (primal && np >= 2) wait(BAR_PV_DONE, (c_pv - 2) & 1);
+            // A parity wait is sound only if the barrier is known to be at most one phase away.  General task: tS of the last
+            // pair-step was consumed, and the pipe produced it after the MMAs of the pair-step before.  Primal-only task:
+            // the last pair-step waited for the one before it ahead of handing over its P~ (see there).
             wait(BAR_PV_DONE, (c_pv - 1) & 1);
             tc_fence_after();
             float la, lb, lc, ld, ra, rb, rc, rd;

@@ -42,6 +42,8 @@ cudaError_t launch_bwd_simt(const BwdParams &prm, int dtype, int d, int num_q_ta
 struct BwdUmmaParams {
     CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2;
     aj_tensor out1, out2;             // dQ | dK, dV
+    aj_tensor a1, a2;                 // dQ pass: Q and dO again as plain views (their rows go to TMEM, not to shared memory)
+    int32_t Na;                       // rows of the stationary tensors
     const float *lse, *delta;         // [B, H, Nq]
     const aj_task *tasks;
     const int32_t *r_begin, *r_end;   // the tasks' streamed ranges

@@ -192,6 +192,14 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
         ::AJ_I8(r, 0), AJ_I8(r, 8), AJ_I8(r, 16), AJ_I8(r, 24), "r"(taddr) : "memory");
 }
 
+// 32 lanes x 16 columns
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15};"
+        ::AJ_I8(r, 0), AJ_I8(r, 8), "r"(taddr) : "memory");
+}
+
 // ---- fp32 helpers: packed pairs (FFMA2 / FMUL2 / FADD2 halve the issue slots of the softmax role) -----------------
 __device__ __forceinline__ uint64_t pack2(float lo, float hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ uint64_t pack2(uint32_t lo, uint32_t hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi)); return r; }
