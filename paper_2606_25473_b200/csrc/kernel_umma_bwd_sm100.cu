@@ -15,9 +15,8 @@
 // S and dP are therefore computed twice (7 contractions instead of the minimal 5) in exchange for no atomics and no
 // cross-CTA reduction of dQ.  X/Y are double-buffered in TMEM (acc1 128 | acc2 128 | X0 Y0 X1 Y1 64 columns each), so
 // the MMAs of tile j + 1 run under the exp / dS work of tile j.  Roles (12 warps): warp 0 TMA producer, warp 1 MMA issuer,
-// warp 2 TMEM allocator, warps 4-7 and 8-11 two exp / dS / epilogue warpgroups that take ALTERNATE tiles (tile = TMEM
-// buffer = warpgroup; the tiles are independent, there is no running max), so that one tile's MUFU-bound exponentials
-// run under the other's TMEM loads, packs, stores and barrier round trips.  Tasks are assigned to the CTAs by the host, head by head and most
+// warp 2 TMEM allocator, warps 4-7 and 8-11 two exp / dS / epilogue warpgroups that each take 32 of a tile's 64 streamed
+// rows (the columns are independent: there is no running max), which halves the X -> W latency that sets the tile period.  Tasks are assigned to the CTAs by the host, head by head and most
 // expensive first (assign_workers), so that all CTAs stream the same head's operands through L2 at the same time.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -110,7 +109,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
         mbar_init(bars + 8 * BAR_A_FULL, KEYS ? 1 : 8);     // TMA transaction | one arrive per exp / dS warp (rows stored to TMEM)
         mbar_init(bars + 8 * BAR_A_EMPTY, 1);
         for (int i = 0; i < NSTAGE; ++i) { mbar_init(bars + 8 * (BAR_B_FULL + i), 1); mbar_init(bars + 8 * (BAR_B_EMPTY + i), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(bars + 8 * (BAR_X_FULL + i), 1); mbar_init(bars + 8 * (BAR_W_FULL + i), 4); }
+        for (int i = 0; i < 2; ++i) { mbar_init(bars + 8 * (BAR_X_FULL + i), 1); mbar_init(bars + 8 * (BAR_W_FULL + i), 8); }
         mbar_init(bars + 8 * BAR_ACC_DONE, 1);
         mbar_init(bars + 8 * (BAR_ACC_DONE + 1), 1);
         sh->abort_flag = 0;
@@ -208,12 +207,14 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 tc_fence_after();
                 if (leader) {
 #pragma unroll
+                    // bf16 Z / W of streamed rows [32 h, 32 h + 32) sit in columns [32 h, 32 h + 16) of the Y / X buffer
+                    // (each exp / dS warpgroup writes inside the fp32 columns it has read)
                     for (int ks = 0; ks < BC / 16; ++ks)        // acc1 += Z B1   (dQ += dS K | dK += dS^T Q)
-                        mma_ts(tmem + TM_ACC1, tZ + ks * 8, b1_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
+                        mma_ts(tmem + TM_ACC1, tZ + (ks >> 1) * 32 + (ks & 1) * 8, b1_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
                     if (KEYS) {
 #pragma unroll
                         for (int ks = 0; ks < BC / 16; ++ks)    // acc2 += W B2   (dV += P^T dO)
-                            mma_ts(tmem + TM_ACC2, tW + ks * 8, b2_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
+                            mma_ts(tmem + TM_ACC2, tW + (ks >> 1) * 32 + (ks & 1) * 8, b2_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (ks > 0));
                     }
                     tc_commit(bars + 8 * (BAR_B_EMPTY + slot));
                     tc_commit(bars + 8 * (BAR_ACC_DONE + b));
@@ -265,14 +266,16 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bars + 8 * BAR_A_FULL);
             }
-            TileCursor cur, pf;                                    // pf runs ahead: the next tile of this warpgroup
+            // Both warpgroups work on every tile: warpgroup h takes streamed rows (columns) [32 h, 32 h + 32), which halves
+            // the latency between "X, Y complete" and "W, Z stored" -- with two TMEM buffers that latency, not the
+            // throughput, sets the tile period.  In the KEYS pass the warpgroup whose index equals the tile's buffer
+            // stages lse / delta of the tile's 64 streamed rows, fetched one of ITS tiles (two tiles) ahead.
+            TileCursor cur, pf;
             cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
-            if (((g & 1) != (uint32_t)wg) && n > 0) cur.next();    // first tile of this warpgroup
-            const int j0 = ((g & 1) != (uint32_t)wg) ? 1 : 0;
             pf = cur;
-            // KEYS pass: lse (in log2 units; +inf past the range end, so that W = 0 there) or delta of streamed row st & 63,
-            // fetched one tile of this warpgroup ahead so that the global-memory latency is off the tile's critical path
-            auto fetch = [&](const TileCursor &c) -> float {
+            const int j0 = ((g & 1) != (uint32_t)wg) ? 1 : 0;      // first tile this warpgroup stages
+            if (j0 == 1 && n > 1) pf.next();
+            auto fetch = [&](const TileCursor &c) -> float {       // lse in log2 units (+inf past the range end: W = 0) or delta
                 const int cc = st & (BC - 1);
                 const bool ok = cc < c.valid();
                 const int64_t qrow = c.row() + cc;
@@ -280,65 +283,62 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
             };
             float pre = 0.f;
             if (KEYS && j0 < n) pre = fetch(pf);
-            for (int j = j0; j < n; j += 2) {
-                const uint32_t gj = g + j, b = (uint32_t)wg;
-                const uint32_t tX = tmem + lane_base + TM_X0 + b * TM_BUF, tY = tmem + lane_base + TM_Y0 + b * TM_BUF;
+            for (int j = 0; j < n; ++j, cur.next()) {
+                const uint32_t gj = g + j, b = gj & 1;
+                const uint32_t tX = tmem + lane_base + TM_X0 + b * TM_BUF + 32 * wg, tY = tmem + lane_base + TM_Y0 + b * TM_BUF + 32 * wg;
                 const int valid = cur.valid();
                 if (KEYS) {
-                    sh->stage[b][st >> 6][st & (BC - 1)] = pre;
-                    if (j + 2 < n) { pf.next(); pf.next(); pre = fetch(pf); }
-                    named_bar_sync(1 + wg, 128);
+                    if (b == (uint32_t)wg) {
+                        sh->stage[b][st >> 6][st & (BC - 1)] = pre;
+                        if (j + 2 < n) { pf.next(); pf.next(); pre = fetch(pf); }
+                    }
+                    named_bar_sync(1 + b, 256);
                 }
                 wait(BAR_X_FULL + b, (gj >> 1) & 1);
                 tc_fence_after();
                 const uint64_t sl2_2 = pack2(sl2, sl2), myl_2 = pack2(-my_l2, -my_l2), myd_2 = pack2(-my_del, -my_del);
+                uint32_t xu[32], yu[32];
+                tmem_ld32(tX, xu);
+                tmem_ld32(tY, yu);
+                tc_wait_ld(xu, yu);
+                if (!KEYS && valid < BC) {                          // past the range end: S = -inf, so W = Z = 0
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {              // 32 columns at a time (register budget of 384 threads)
-                    uint32_t xu[32], yu[32];
-                    tmem_ld32(tX + 32 * half, xu);
-                    tmem_ld32(tY + 32 * half, yu);
-                    tc_wait_ld(xu, yu);
-                    if (!KEYS && valid < BC) {                      // past the range end: S = -inf, so W = Z = 0
-#pragma unroll
-                        for (int c = 0; c < 32; ++c) if (32 * half + c >= valid) xu[c] = 0xff800000u;
-                    }
-                    uint32_t wk[16], zk[16];
-#pragma unroll
-                    for (int c4 = 0; c4 < 32; c4 += 4) {
-                        uint64_t nl[2], nd[2];                      // -lse * log2e and -delta of four columns
-                        if (KEYS) {
-                            const float4 l4 = *reinterpret_cast<const float4 *>(&sh->stage[b][0][32 * half + c4]);
-                            const float4 d4 = *reinterpret_cast<const float4 *>(&sh->stage[b][1][32 * half + c4]);
-                            nl[0] = pack2(-l4.x, -l4.y); nl[1] = pack2(-l4.z, -l4.w);
-                            nd[0] = pack2(-d4.x, -d4.y); nd[1] = pack2(-d4.z, -d4.w);
-                        } else {
-                            nl[0] = nl[1] = myl_2; nd[0] = nd[1] = myd_2;
-                        }
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int c = c4 + 2 * h;
-                            // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
-                            const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl[h]);
-                            float x0, x1;
-                            unpack2(x, x0, x1);
-                            const float w0 = ex2(x0), w1 = ex2(x1);
-                            const uint64_t z = fmul2(pack2(w0, w1), fadd2(pack2(yu[c], yu[c + 1]), nd[h]));
-                            float z0, z1;
-                            unpack2(z, z0, z1);
-                            wk[c >> 1] = pack_bf16(w0, w1);
-                            zk[c >> 1] = pack_bf16(z0, z1);
-                        }
-                    }
-                    // W / Z (bf16 pairs) go to columns [16 half, 16 half + 16) of the X / Y buffer: fp32 columns that have
-                    // already been read (half 0 read [0, 32))
-                    if (KEYS) tmem_st16(tX + 16 * half, wk);
-                    tmem_st16(tY + 16 * half, zk);
+                    for (int c = 0; c < 32; ++c) if (32 * wg + c >= valid) xu[c] = 0xff800000u;
                 }
+                uint32_t wk[16], zk[16];
+#pragma unroll
+                for (int c4 = 0; c4 < 32; c4 += 4) {
+                    uint64_t nl[2], nd[2];                          // -lse * log2e and -delta of four columns
+                    if (KEYS) {
+                        const float4 l4 = *reinterpret_cast<const float4 *>(&sh->stage[b][0][32 * wg + c4]);
+                        const float4 d4 = *reinterpret_cast<const float4 *>(&sh->stage[b][1][32 * wg + c4]);
+                        nl[0] = pack2(-l4.x, -l4.y); nl[1] = pack2(-l4.z, -l4.w);
+                        nd[0] = pack2(-d4.x, -d4.y); nd[1] = pack2(-d4.z, -d4.w);
+                    } else {
+                        nl[0] = nl[1] = myl_2; nd[0] = nd[1] = myd_2;
+                    }
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int c = c4 + 2 * h;
+                        // W = exp(S - lse) = p_ab (PAPER.md:842-844 with the forward's L, :945); Z = W (dP - delta)
+                        const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl[h]);
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        const float w0 = ex2(x0), w1 = ex2(x1);
+                        const uint64_t z = fmul2(pack2(w0, w1), fadd2(pack2(yu[c], yu[c + 1]), nd[h]));
+                        float z0, z1;
+                        unpack2(z, z0, z1);
+                        wk[c >> 1] = pack_bf16(w0, w1);
+                        zk[c >> 1] = pack_bf16(z0, z1);
+                    }
+                }
+                // bf16 W / Z over the first 16 of the 32 fp32 columns this thread has just read
+                if (KEYS) tmem_st16(tX, wk);
+                tmem_st16(tY, zk);
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bars + 8 * (BAR_W_FULL + b));
-                cur.next(); cur.next();
             }
             // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one 64-column half ----
             __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
@@ -350,15 +350,10 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 }
                 continue;
             }
-            // A parity wait is sound only if the barrier is known to be at most one phase away.  Each warpgroup waits on ITS
-            // buffer's barrier for ITS last tile jl: it consumed X(jl), which the in-order pipe produced after the MMAs of
-            // tile jl - 2 (the previous phase of that barrier), and tile jl + 2 does not exist.  Once both have passed,
-            // every tile of the task is complete.
-            {
-                const int jl = ((g + n - 1) & 1) == (uint32_t)wg ? n - 1 : n - 2;
-                if (jl >= 0) wait(BAR_ACC_DONE + wg, ((g + jl) >> 1) & 1);
-            }
-            named_bar_sync(3, 256);
+            // A parity wait is sound only if the barrier is known to be at most one phase away: this thread consumed X of the
+            // last tile, which the in-order pipe produced after the MMAs of tile n - 3 (the previous phase of that buffer's
+            // barrier), and the next phase needs this thread's next hand-over.
+            wait(BAR_ACC_DONE + ((g + n - 1) & 1), ((g + n - 1) >> 1) & 1);
             tc_fence_after();
             g += n;
 #pragma unroll 1
