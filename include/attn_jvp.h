@@ -223,9 +223,11 @@ aj_status attn_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, 
  * with p_ab = exp(s <q_a, k_b> - lse_a) over the unmasked pairs.  q, o, dout, dq: [B,H,Nq,d]; k, v, dk, dv: [B,H,Nk,d]
  * in the problem dtype; lse: contiguous fp32 [B,H,Nq] as written by attn_jvp_fwd / attn_fwd on the same q, k, v.  All
  * DEVICE memory, same alignment rules as attn_jvp_fwd.  Every element of dq, dk, dv is written (0 for rows without
- * keys and keys no row sees).  Enqueues three kernels on `cuda_stream`; the first call on a plan also builds and
- * uploads the backward schedules (synchronous host work) and allocates a [B,H,Nq] fp32 workspace.
- * This round: plain-FMA fp32 arithmetic for both dtypes (a correct first path, not a tensor-core kernel).
+ * keys and keys no row sees).  Enqueues three kernels on `cuda_stream` (delta = <dO, O>; a pass with query tiles
+ * stationary for dQ; a pass with key tiles stationary, on the transposed schedule, for dK and dV -- no atomics); the
+ * first call on a plan also builds and uploads the two backward schedules (synchronous host work) and allocates a
+ * [B,H,Nq] fp32 workspace.  bf16 with d = 128: tcgen05 / TMEM / TMA kernel (bf16 P and dS operands, fp32 accumulation);
+ * anything else, or a plan forced to AJ_KERNEL_SIMT: plain fp32 FMA kernels.
  */
 aj_status attn_bwd(aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o,
                    const float *lse, const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv,

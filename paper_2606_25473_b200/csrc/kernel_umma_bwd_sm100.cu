@@ -3,8 +3,9 @@
 //     p_ab = exp(s <q_a, k_b> - lse_a),  dP_ab = <dO_a, v_b>,  dS_ab = p_ab (dP_ab - delta_a),  delta_a = <dO_a, O_a>
 //     dQ_a = s sum_b dS_ab k_b ;   dK_b = s sum_a dS_ab q_a ;   dV_b = sum_a p_ab dO_a
 // Two passes of ONE kernel, because the two are the same computation with the roles swapped:
-//   a CTA keeps 128 STATIONARY rows (A1, A2) in shared memory and streams 64-row tiles (B1, B2) of the other side:
-//     X  = A1 B1^T,  Y = A2 B2^T            2 x 8 MMAs (M128 N64 K16), A and B from shared memory   -> TMEM
+//   a CTA keeps 128 STATIONARY rows (A1, A2; in shared memory, or in TMEM in the dQ pass) and streams 64-row tiles (B1, B2)
+//   of the other side:
+//     X  = A1 B1^T,  Y = A2 B2^T            2 x 8 MMAs (M128 N64 K16), B from shared memory          -> TMEM
 //     W  = exp2(X s log2e - lse log2e),  Z = W o (Y - delta)         softmax warps, thread = stationary row = TMEM lane
 //     acc1 += Z B1   (and acc2 += W B2)     4 (+4) MMAs (M128 N128 K16), A = bf16 Z / W in TMEM, B MN-major
 //   KEYS = false: stationary = query rows (A1 = Q, A2 = dO), streamed = keys (B1 = K, B2 = V): acc1 = dQ / s; lse and
@@ -16,8 +17,8 @@
 // cross-CTA reduction of dQ.  X/Y are double-buffered in TMEM (acc1 128 | acc2 128 | X0 Y0 X1 Y1 64 columns each), so
 // the MMAs of tile j + 1 run under the exp / dS work of tile j.  Roles (12 warps): warp 0 TMA producer, warp 1 MMA issuer,
 // warp 2 TMEM allocator, warps 4-7 and 8-11 two exp / dS / epilogue warpgroups that each take 32 of a tile's 64 streamed
-// rows (the columns are independent: there is no running max), which halves the X -> W latency that sets the tile period.  Tasks are assigned to the CTAs by the host, head by head and most
-// expensive first (assign_workers), so that all CTAs stream the same head's operands through L2 at the same time.
+// rows (the columns are independent: there is no running max).  Tasks are assigned to the CTAs by the host, head by head
+// and most expensive first (assign_workers), so that all CTAs stream the same head's operands through L2 at the same time.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
