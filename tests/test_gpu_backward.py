@@ -154,6 +154,24 @@ def test_backward_ranges_mask_unseen_keys_and_keyless_rows(dtype):
     assert torch.count_nonzero(dq[0, :, keyless]) == 0
 
 
+def test_forward_only_plan_feeds_the_backward():
+    # the non-JVP stages: attn_fwd on an AJ_TANGENT_NONE plan, then attn_bwd on the same plan
+    w = Workload("fwdbwd_bc", 1, 2, 128, "block_causal", 150, 4, 1, "bf16", 0.0, 21, False, True)
+    x = make_inputs(w)
+    dout = _dout(w)
+    plan = make_plan(w)
+    q, k, v = [t.cuda() for t in x[:3]]
+    o = torch.empty_like(q)
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    aj.attn_fwd(plan, q, k, v, o, lse, 0)
+    dq, dk, dv = torch.full_like(q, float("nan")), torch.full_like(q, float("nan")), torch.full_like(q, float("nan"))
+    aj.attn_bwd(plan, q, k, v, o, lse, dout.cuda(), dq, dk, dv, 0)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    check(w, x, dout, (dq.cpu(), dk.cpu(), dv.cpu()))
+
+
 def test_backward_strided_views_and_argument_errors():
     w = SMALL[4]
     x = make_inputs(w)
