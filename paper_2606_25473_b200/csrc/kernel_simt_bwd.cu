@@ -7,8 +7,8 @@
 //     dQ_a = scale sum_b dS_ab k_b          one CTA per query tile, streaming the key ranges of its group
 //     dV_b = sum_a p_ab dO_a,  dK_b = scale sum_a dS_ab q_a      one CTA per KEY tile, streaming the row ranges that
 //                                                                  see it (the transposed schedule), so no atomics
-// This is the first correct path for N2 (same schedule machinery, fp32 arithmetic for both input dtypes); it is not
-// a tensor-core kernel.
+// These kernels serve fp32 inputs, d = 64 and plans forced to AJ_KERNEL_SIMT (fp32 arithmetic for both input dtypes), and
+// the delta kernel serves both backward paths; bf16 with d = 128 runs kernel_umma_bwd_sm100.cu (tcgen05).
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math_constants.h>
