@@ -8,10 +8,12 @@
  * with tS = (tQ K^T + Q tK^T) * s (Eq. 43); masked entries have S = -inf and
  * tS = 0.  The computation is the online-softmax recurrence of PAPER.md:866-878
  * (Alg. 1) under the sparse query-group / key-range mask of PAPER.md:880-886.
+ * Around that call: attn_fwd (the same without tangents, also for Nq != Nk), attn_bwd (the primal backward dQ, dK, dV
+ * that consumes lse), attn_jvp_fwd_host (host buffers, copies pipelined head by head), and the host-only scheduler.
  *
  * Conventions
- *  - All functions are extern "C", never throw, never synchronise the stream, and return an
- *    aj_status; attn_jvp_last_error() gives a thread-local message for the last failure.
+ *  - All functions are extern "C", never throw, never synchronise the stream (except plan creation / first-use
+ *    schedule uploads and attn_jvp_plan_device_status, as stated there), and return an aj_status; attn_jvp_last_error() gives a thread-local message for the last failure.
  *  - The caller owns every tensor.  "device" pointers are CUDA device memory of the current
  *    device; "host" pointers are ordinary (preferably pinned) host memory.
  *  - Tensors are [B, H, N, d] with d contiguous; strides are in ELEMENTS (aj_tensor).
