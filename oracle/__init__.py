@@ -62,6 +62,8 @@ def _load():
             ctypes.POINTER(_CMask), ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_double,
             ctypes.c_int32] + [ctypes.c_void_p] * 6 + [
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.attn_jvp_oracle_rows_tl.restype = ctypes.c_int
+        lib.attn_jvp_oracle_rows_tl.argtypes = lib.attn_jvp_oracle_rows.argtypes + [ctypes.c_void_p]
         lib.attn_jvp_oracle_bwd.restype = ctypes.c_int
         lib.attn_jvp_oracle_bwd.argtypes = [
             ctypes.POINTER(_CMask), ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int32] + \
@@ -146,11 +148,12 @@ def num_threads() -> int:
 
 
 def attn_jvp_head(mask: Mask, q, k, v, tq, tk, tv, scale: float,
-                  rows: Optional[np.ndarray] = None):
+                  rows: Optional[np.ndarray] = None, with_tlse: bool = False):
     """One (batch, head) slice: q, tq [Nq, d]; k, v, tk, tv [Nk, d] (float32 or float64 numpy).
 
     Returns (o [R, d], to [R, d], lse [R]) in float64 for the R requested rows
-    (all rows if ``rows`` is None).
+    (all rows if ``rows`` is None); with ``with_tlse`` also tlse [R], the tangent of lse
+    (sum_b p_ab tS_ab = r / l).
     """
     lib = _load()
     dt = np.float64 if q.dtype == np.float64 else np.float32
@@ -169,15 +172,16 @@ def attn_jvp_head(mask: Mask, q, k, v, tq, tk, tv, scale: float,
     o = np.empty((nrows, d), dtype=np.float64)
     to = np.empty((nrows, d), dtype=np.float64)
     lse = np.empty((nrows,), dtype=np.float64)
+    tlse = np.empty((nrows,), dtype=np.float64) if with_tlse else None
     cm, keep = mask._c()
-    rc = lib.attn_jvp_oracle_rows(
+    rc = lib.attn_jvp_oracle_rows_tl(
         ctypes.byref(cm), nq, nk, d, float(scale), 1 if dt == np.float64 else 0,
         *[x.ctypes.data for x in arrs],
         None if rows_arr is None else rows_arr.ctypes.data, nrows,
-        o.ctypes.data, to.ctypes.data, lse.ctypes.data)
+        o.ctypes.data, to.ctypes.data, lse.ctypes.data, None if tlse is None else tlse.ctypes.data)
     if rc != 0:
         raise RuntimeError("attn_jvp_oracle_rows failed")
-    return o, to, lse
+    return (o, to, lse, tlse) if with_tlse else (o, to, lse)
 
 
 def attn_jvp(mask: Mask, q, k, v, tq, tk, tv, scale: float, rows: Optional[np.ndarray] = None):

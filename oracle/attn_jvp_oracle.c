@@ -16,7 +16,8 @@
  * of O along the tangent, brute-force dense masked attention written
  * independently in numpy, torch.func.jvp / SDPA / logsumexp, closed forms,
  * invariants and pair counts; the backward (attn_jvp_oracle_bwd) is pinned by torch.autograd, finite differences of
- * <O, dO> and invariants (tests/test_oracle_bwd_pins.py).  Every exported function below is pinned; none is
+ * <O, dO> and invariants (tests/test_oracle_bwd_pins.py); the lse tangent (attn_jvp_oracle_rows_tl) by finite differences of
+ * lse, torch.func.jvp(logsumexp) and closed forms (test_oracle_pins.py "TL").  Every exported function below is pinned; none is
  * "parity unpinned".
  *
  * Definitions followed (PAPER.md line : item):
@@ -25,6 +26,8 @@
  *   851-854  masked entries: S = -inf, tS = 0 (the mask has no tangent)
  *   862-864  Eq. 44  tO_a = sum_b p_ab tV_b + sum_b p_ab (tS_ab - sum_c p_ac tS_ac) V_b
  *   945      L = m + log(l)  (log-sum-exp of the scaled, masked scores)
+ *   870-876  r = sum_b e^{s_ab - m} tS_ab, so r / l = sum_b p_ab tS_ab = mu_a: the tangent of L along the input
+ *            tangent (d/d eps of log sum exp(S + eps tS) = softmax-weighted mean of tS); output `tlse`
  *   175-180  Eq. 8 / teacher-forcing mask over the packed [clean | noisy] sequence
  *   882-886  generic mask = query groups with key-range lists
  * Readings where the paper is silent are DESIGN.md R1 (both S and tS carry the
@@ -126,14 +129,15 @@ static inline double ajo_load(const void *p, int dtype, int64_t idx)
  * One (batch, head) slice.  q, tq: [nq, d]; k, v, tk, tv: [nk, d]; rows contiguous
  * with stride d; dtype says whether they hold float or double (values are widened
  * exactly).  rows[0..nrows) lists the query rows to evaluate (NULL = rows 0..nrows-1).
- * Outputs, all fp64: o, to: [nrows, d]; lse: [nrows].
+ * Outputs, all fp64: o, to: [nrows, d]; lse: [nrows]; tlse: [nrows] or NULL (the tangent of lse, mu_a = sum_b p_ab
+ * tS_ab = the paper's r / l; 0 for a row with no allowed key).
  * Returns 0, or -1 on a bad argument / allocation failure.
  */
-int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d, double scale,
-                         int32_t dtype, const void *q, const void *k, const void *v,
-                         const void *tq, const void *tk, const void *tv,
-                         const int64_t *rows, int64_t nrows,
-                         double *o, double *to, double *lse)
+int attn_jvp_oracle_rows_tl(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d, double scale,
+                            int32_t dtype, const void *q, const void *k, const void *v,
+                            const void *tq, const void *tk, const void *tv,
+                            const int64_t *rows, int64_t nrows,
+                            double *o, double *to, double *lse, double *tlse)
 {
     if (!mask || nq <= 0 || nk <= 0 || d <= 0 || nrows < 0) return -1;
     if (dtype != AJO_F32 && dtype != AJO_F64) return -1;
@@ -148,12 +152,16 @@ int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d
         if (!s || !ts || !ok || !qa || !tqa) {
 #pragma omp atomic write
             failed = 1;
-        } else {
+        }
+        /* every thread reaches the worksharing loop or none does: the flag is read after a barrier */
+#pragma omp barrier
+        if (!failed) {
 #pragma omp for schedule(dynamic, 1)
             for (int64_t i = 0; i < nrows; ++i) {
                 int64_t a = rows ? rows[i] : i;
                 double *oa = o + i * d, *toa = to + i * d;
                 for (int c = 0; c < d; ++c) { oa[c] = 0.0; toa[c] = 0.0; }
+                if (tlse) tlse[i] = 0.0;
                 if (a < 0 || a >= nq) { lse[i] = NAN; continue; }
                 for (int c = 0; c < d; ++c) {
                     qa[c] = ajo_load(q, dtype, a * d + c);
@@ -188,6 +196,7 @@ int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d
                 /* mu = sum_c p_ac tS_ac */
                 double mu = 0.0;
                 for (int64_t b = 0; b < nk; ++b) mu += s[b] * ts[b];
+                if (tlse) tlse[i] = mu;
                 /* O = sum p v;  Eq. 44 */
                 for (int64_t b = 0; b < nk; ++b) {
                     if (!ok[b]) continue;
@@ -204,6 +213,16 @@ int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d
         free(s); free(ts); free(ok); free(qa); free(tqa);
     }
     return failed ? -1 : 0;
+}
+
+/* The same without the lse tangent (the original entry point). */
+int attn_jvp_oracle_rows(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d, double scale,
+                         int32_t dtype, const void *q, const void *k, const void *v,
+                         const void *tq, const void *tk, const void *tv,
+                         const int64_t *rows, int64_t nrows,
+                         double *o, double *to, double *lse)
+{
+    return attn_jvp_oracle_rows_tl(mask, nq, nk, d, scale, dtype, q, k, v, tq, tk, tv, rows, nrows, o, to, lse, NULL);
 }
 
 /*
@@ -245,7 +264,9 @@ int attn_jvp_oracle_bwd(const ajo_mask *mask, int64_t nq, int64_t nk, int32_t d,
         if (!p || !dp || !ok) {
 #pragma omp atomic write
             failed = 1;
-        } else {
+        }
+#pragma omp barrier
+        if (!failed) {
             /* pass 1: every query row (lse and delta of all rows are needed by pass 2) */
 #pragma omp for schedule(dynamic, 1)
             for (int64_t a = 0; a < nq; ++a) {

@@ -6,6 +6,7 @@ P3 library autodiff: torch.func.jvp through a 3-line dense attention; SDPA; torc
 P4 invariants (zero tangents, full mask, masked keys have no effect)
 P5 closed forms
 P6 pair counts against closed forms and tests/golden/pair_counts.txt
+TL the lse tangent (tlse = r / l): finite differences of lse, torch.func.jvp(logsumexp), closed forms
 """
 import os
 
@@ -310,6 +311,73 @@ def test_float32_inputs_are_widened_exactly(oracle):
     b = oracle.attn_jvp_head(m, *x64, 0.1)
     for p, r in zip(a, b):
         assert np.array_equal(p, r)
+
+
+# ----------------------------------------------------------------------------- TL: the lse tangent
+@pytest.mark.parametrize("kind", ["teacher_forcing", "block_causal", "full"])
+def test_tl_finite_differences_of_lse(oracle, kind):
+    n, C, d = 3, 16, 64
+    N = 2 * n * C if kind == "teacher_forcing" else n * C
+    mask = {"teacher_forcing": oracle.teacher_forcing_mask(C, n),
+            "block_causal": oracle.block_causal_mask(C, n), "full": oracle.full_mask()}[kind]
+    q, k, v, tq, tk, tv = [_rand((N, d), 200 + s) for s in range(6)]
+    scale = 1.0 / np.sqrt(d)
+    o, to, lse, tlse = oracle.attn_jvp_head(mask, q, k, v, tq, tk, tv, scale, with_tlse=True)
+    o3, to3, lse3 = oracle.attn_jvp_head(mask, q, k, v, tq, tk, tv, scale)
+    assert np.array_equal(o, o3) and np.array_equal(to, to3) and np.array_equal(lse, lse3)
+    h = 1e-4
+    z = np.zeros_like(q)
+    _, _, lp = oracle.attn_jvp_head(mask, q + h * tq, k + h * tk, v, z, z, z, scale)
+    _, _, lm = oracle.attn_jvp_head(mask, q - h * tq, k - h * tk, v, z, z, z, scale)
+    assert max_norm_err((lp - lm) / (2 * h), tlse) <= 1e-6
+
+
+def test_tl_autodiff_logsumexp(oracle):
+    w = WORKLOADS["tiny_tf_fp32"]
+    q, k, v, tq, tk, tv = [t.double() for t in make_inputs(w)]
+    scale = 1.0 / np.sqrt(w.d)
+    mask_t = torch.from_numpy(_tf_dense_mask(w.num_blocks, w.block_len))
+
+    def lse_fn(q_, k_):
+        s = torch.where(mask_t, (q_ @ k_.transpose(-1, -2)) * scale, torch.tensor(-float("inf"), dtype=q_.dtype))
+        return torch.logsumexp(s, dim=-1)
+
+    _, tl_ad = torch.func.jvp(lse_fn, (q, k), (tq, tk))
+    om = oracle_mask(w)
+    for h in range(w.H):
+        tl = oracle.attn_jvp_head(om, *[x[0, h].numpy() for x in (q, k, v, tq, tk, tv)], scale, with_tlse=True)[3]
+        assert np.max(np.abs(tl - tl_ad[0, h].numpy())) < 1e-13
+
+
+def test_tl_closed_forms(oracle):
+    n, C, d = 3, 4, 8
+    N = 2 * n * C
+    m = oracle.teacher_forcing_mask(C, n)
+    q, k, v, tq, tk, tv = [_rand((N, d), 210 + s) for s in range(6)]
+    z = np.zeros((N, d))
+    # one allowed key (C = 1): tlse = s (<tq, k> + <q, tk>)
+    q1, k1, v1, tq1, tk1, tv1 = [x[:2 * n] for x in (q, k, v, tq, tk, tv)]
+    tl = oracle.attn_jvp_head(oracle.teacher_forcing_mask(1, n), q1, k1, v1, tq1, tk1, tv1, 0.7, with_tlse=True)[3]
+    for a, b in [(0, 0), (n, n)]:
+        assert abs(tl[a] - 0.7 * (tq1[a] @ k1[b] + q1[a] @ tk1[b])) < 1e-14
+    # Q = tQ = 0: every tS is zero
+    assert np.all(oracle.attn_jvp_head(m, z, k, v, z, tk, tv, 0.3, with_tlse=True)[3] == 0.0)
+    # zero tangents: tlse = 0; tV never enters
+    assert np.all(oracle.attn_jvp_head(m, q, k, v, z, z, tv, 0.3, with_tlse=True)[3] == 0.0)
+    # a common vector u added to every tK row moves every tS_ab of row a by s <q_a, u>, hence tlse by the same
+    u = _rand((1, d), 8)
+    t0 = oracle.attn_jvp_head(m, q, k, v, tq, tk, tv, 0.3, with_tlse=True)[3]
+    t1 = oracle.attn_jvp_head(m, q, k, v, tq, tk + u, tv, 0.3, with_tlse=True)[3]
+    assert np.max(np.abs((t1 - t0) - 0.3 * (q @ u[0]))) < 1e-12
+    # rows without keys: 0 (R9)
+    x = [_rand((8, 4), 220 + s) for s in range(6)]
+    tl = oracle.attn_jvp_head(oracle.ranges_mask([(0, 4, [(0, 8)])]), *x, 0.5, with_tlse=True)[3]
+    assert np.all(tl[4:] == 0.0) and np.all(tl[:4] != 0.0)
+    # Eq. 44 can be written with it: tO = P tV + (P o tS) V - tlse * O
+    o, to, lse, tl = oracle.attn_jvp_head(oracle.full_mask(), q, k, v, tq, tk, tv, 0.3, with_tlse=True)
+    P = np.exp(0.3 * q @ k.T - lse[:, None])
+    tS = 0.3 * (tq @ k.T + q @ tk.T)
+    assert np.max(np.abs(to - (P @ tv + (P * tS) @ v - tl[:, None] * o))) < 1e-13
 
 
 # ----------------------------------------------------------------------------- P6
