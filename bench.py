@@ -10,6 +10,10 @@ pair (six length-d contractions); padded tile area, mas
 not counted.  N > 1: every rank runs its own head shard (B, H heads each; Ulysses-style head sharding,
 PAPER.md:318) with no data-path collective -> "scaling": "weak".
 
+`--ulysses`: the ranks hold SEQUENCE shards [B, H, N/P, d] of ONE problem; a step = packed all-to-all
+in per head group, the kernel on the rank's head shard, packed all-to-all out (paper_2606_25473_b200/ulysses.py), timed
+whole and in parts -> "scaling": "strong".  On a box without CUDA it is a dry run of the exchange (gloo, no kernel).
+
 `--impl reference` times the fp64 CPU oracle (oracle/, as it stands) on the host cores on a bounded row sample
 of the same workload; rank 0 only.
 """
@@ -76,20 +80,22 @@ def load_peaks():
 
 
 def recorded_traffic(workload: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, if any."""
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, if any, and where the figure
+    comes from (rows of profiles/dram_traffic.csv: workload, kernel / capture name, bytes): -> (bytes, source) or (None, None).
+    The last matching row wins; the source names it so that a capture older than the kernel is visible in the line."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
-        return None
-    best = None
+        return None, None
+    best, src = None, None
     with open(path) as f:
         for line in f:
             parts = [p.strip() for p in line.split(",")]
             if len(parts) >= 3 and parts[0] == workload:
                 try:
-                    best = float(parts[2])
+                    best, src = float(parts[2]), f"profiles/dram_traffic.csv: {parts[1]}"
                 except ValueError:
                     pass
-    return best
+    return best, src
 
 
 class ClockSampler:
@@ -148,7 +154,7 @@ class ClockSampler:
 # ----------------------------------------------------------------------------------------------- CPU oracle legs
 def time_oracle_sample(w: Workload, inputs, budget_s: float, seed: int = 0):
     """Runs the oracle as it stands on a seeded uniform row sample of head (0, 0) sized to ~budget_s seconds.
-    -> (TFLOP/s under the 12*d convention, seconds, rows, cores)."""
+    -> (TFLOP/s under the 12*d convention, seconds, number of rows, cores, (rows, o, to, lse) of the sample)."""
     import oracle
     oracle.build()
     om = {"teacher_forcing": oracle.teacher_forcing_mask, "block_causal": oracle.block_causal_mask}.get(w.mask)
@@ -163,10 +169,10 @@ def time_oracle_sample(w: Workload, inputs, budget_s: float, seed: int = 0):
     nrows = int(min(max(64, budget_s / dt * 64), 4 * w.num_queries))
     rows = np.sort(rng.integers(0, w.num_queries, size=nrows))
     t0 = time.perf_counter()
-    oracle.attn_jvp_head(om, *args, scale, rows)
+    ref = oracle.attn_jvp_head(om, *args, scale, rows)
     dt = time.perf_counter() - t0
     flops = 12.0 * w.d * float(allowed_keys_per_row(w, rows).sum())
-    return flops / dt / 1e12, dt, nrows, oracle.num_threads()
+    return flops / dt / 1e12, dt, nrows, oracle.num_threads(), (rows,) + tuple(ref)
 
 
 def run_reference(args, w: Workload):
@@ -181,7 +187,7 @@ def run_reference(args, w: Workload):
         time_oracle_sample(w, inputs, budget, seed=100 + i)
     tot_flops, tot_s, tot_rows, cores = 0.0, 0.0, 0, 1
     for i in range(steps):
-        tf, dt, nrows, cores = time_oracle_sample(w, inputs, budget, seed=i)
+        tf, dt, nrows, cores, _ = time_oracle_sample(w, inputs, budget, seed=i)
         tot_flops += tf * 1e12 * dt
         tot_s += dt
         tot_rows += nrows
@@ -303,18 +309,12 @@ def run_cuda(args, w: Workload):
         d_bwd = [x.to(dev) for x in h_bwd]
         dq, dk, dv = torch.empty_like(devin[0]), torch.empty_like(devin[1]), torch.empty_like(devin[1])
         h_grads = [torch.empty_like(host[0]).pin_memory(), torch.empty_like(host[1]).pin_memory(), torch.empty_like(host[1]).pin_memory()]
-        d_lse_in = torch.empty_like(lse)
 
         def step_device():
             aj.attn_bwd(plan, d_bwd[0], d_bwd[1], d_bwd[2], d_bwd[3], lse, d_bwd[4], dq, dk, dv, stream.cuda_stream)
 
         def step_host():
-            for dst, src in zip(d_bwd, h_bwd):
-                dst.copy_(src, non_blocking=True)
-            d_lse_in.copy_(h_lse_in, non_blocking=True)
-            aj.attn_bwd(plan, d_bwd[0], d_bwd[1], d_bwd[2], d_bwd[3], d_lse_in, d_bwd[4], dq, dk, dv, stream.cuda_stream)
-            for dst, src in zip(h_grads, (dq, dk, dv)):
-                dst.copy_(src, non_blocking=True)
+            aj.attn_bwd_host(plan, h_bwd[0], h_bwd[1], h_bwd[2], h_bwd[3], h_lse_in, h_bwd[4], *h_grads, stream.cuda_stream)
             stream.synchronize()
 
     # ---- device-resident timing: events on the launching stream, barrier + synchronize on both sides
@@ -358,10 +358,60 @@ def run_cuda(args, w: Workload):
         d2h = sum(x.numel() * x.element_size() for x in h_grads)
         launches_per_call = 3               # delta, dQ, dK/dV kernels
 
+    # ---- host cost of one enqueue: the time attn_jvp_fwd (attn_bwd) takes to return, median of 1000 calls on a SMALL problem
+    # of the same kernel family (so that the device drains faster than the host enqueues and the launch queue never blocks)
+    overhead_us = None
+    if rank == 0 and w.dtype == "bf16" and w.d == 128:
+        sw = Workload("overhead_probe", 1, 2, 128, "teacher_forcing", 128, 2, 1, "bf16", 0.1)
+        sp = aj.attn_jvp_plan_create(aj.make_problem(sw.B, sw.H, sw.N, sw.N, sw.d, aj.AJ_BF16),
+                                     aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, sw.frame_len, sw.num_frames, 1)[0])
+        sx = [t.to(dev) for t in make_inputs(sw)]
+        so, sto = torch.empty_like(sx[0]), torch.empty_like(sx[0])
+        sl = torch.empty((sw.B, sw.H, sw.N), dtype=torch.float32, device=dev)
+        sg = [torch.empty_like(sx[0]) for _ in range(3)]
+        aj.attn_jvp_fwd(sp, *sx, so, sto, sl, stream.cuda_stream)
+        aj.attn_bwd(sp, sx[0], sx[1], sx[2], so, sl, sx[3], *sg, stream.cuda_stream)
+        torch.cuda.synchronize()
+        ts_f, ts_b = [], []
+        for i in range(1000):
+            t0 = time.perf_counter_ns()
+            aj.attn_jvp_fwd(sp, *sx, so, sto, sl, stream.cuda_stream)
+            t1 = time.perf_counter_ns()
+            aj.attn_bwd(sp, sx[0], sx[1], sx[2], so, sl, sx[3], *sg, stream.cuda_stream)
+            t2 = time.perf_counter_ns()
+            ts_f.append((t1 - t0) / 1e3); ts_b.append((t2 - t1) / 1e3)
+            if i % 100 == 99:
+                torch.cuda.synchronize()
+        enc, hits = aj.attn_jvp_plan_tensor_map_stats(sp)
+        aj.attn_jvp_plan_destroy(sp)
+        overhead_us = {"attn_jvp_fwd": statistics.median(ts_f), "attn_bwd": statistics.median(ts_b),
+                       "how": "median host time of 1000 calls through the ctypes binding (marshalling included) on a "
+                              "2-head, 512-token problem of the same kernels", "tensor_maps_encoded": enc, "tensor_map_cache_hits": hits}
+
+    # ---- parity of what was just timed: the device outputs of head (0, 0) against the oracle rows of the cpu_baseline leg
+    parity = None
+    cpu_leg = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not w.backward:
+        step_device()
+        torch.cuda.synchronize()
+        tf, dt, nrows, cores, (rows, ro, rto, rlse) = time_oracle_sample(w, host_all, args.cpu_budget_s)
+        cpu_leg = (tf, dt, nrows, cores)
+        rsel = torch.from_numpy(rows).to(dev)
+
+        def nerr(got, ref):
+            den = float(np.max(np.abs(ref)))
+            return float(np.max(np.abs(got.double().cpu().numpy() - ref)) / (den if den > 0 else 1.0))
+
+        parity = {"rows": int(len(rows)), "head": [0, 0], "o": nerr(o[0, 0][rsel], ro), "lse": nerr(lse[0, 0][rsel], rlse),
+                  "to": None if w.no_tangents else nerr(to[0, 0][rsel], rto), "metric": "max|gpu - oracle| / max|oracle|",
+                  "tolerance": {"o": 1e-2, "to": 1e-2, "lse": 1e-3} if w.dtype == "bf16" else {"o": 1e-4, "to": 1e-4, "lse": 1e-4}}
+        parity["ok"] = all(parity[k] is None or parity[k] <= parity["tolerance"][k] for k in ("o", "to", "lse"))
+
     aj.attn_jvp_plan_destroy(plan)
     if rank != 0:
         return
     peaks, peak_src = load_peaks()
+    traffic, traffic_src = recorded_traffic(w.name)
     value = flops_all / (total_ms_all * 1e-3) / 1e12
     avg_launch_ms = total_ms / K
     achieved = flops / (avg_launch_ms * 1e-3) / 1e12
@@ -376,12 +426,12 @@ def run_cuda(args, w: Workload):
         "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
         "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "api": ("attn_bwd between torch copies from/to pinned host buffers (copies inside the timed region)" if w.backward
+                "api": ("attn_bwd_host (pinned host buffers, copies inside the timed region)" if w.backward
                         else "attn_jvp_fwd_host (pinned host buffers, copies inside the timed region)")},
         "gpu_launches": K * launches_per_call,
         "clocks": clocks,
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": recorded_traffic(w.name), "peak_source": f"{peak_src} bf16_tflops (burst cuBLAS GEMM)",
+                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": f"{peak_src} bf16_tflops (burst cuBLAS GEMM)",
                      "frac_of_sustained": achieved / sustained, "frac_of_nominal_2250": achieved / 2250.0,
                      "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
                      "flops_per_launch": flops},
@@ -395,12 +445,120 @@ def run_cuda(args, w: Workload):
                                 executed_over_counted_contractions=7.0 / 5.0)
     if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
-    if world == 1 and not args.no_cpu_baseline and not w.backward:   # (the timed oracle leg is the forward oracle)
-        tf, dt, nrows, cores = time_oracle_sample(w, host_all, args.cpu_budget_s)
+    if overhead_us is not None:
+        line["launch_overhead_us"] = overhead_us
+    if parity is not None:
+        line["parity"] = parity
+    if cpu_leg is not None:                                          # (the timed oracle leg is the forward oracle)
+        tf, dt, nrows, cores = cpu_leg
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{nrows} uniformly sampled query rows of head (0,0), all their allowed "
                                           f"keys, {dt:.1f} s", "extrapolated_full_config_s": flops / (tf * 1e12)}
     print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------- the Ulysses arm (8(f) N4)
+def run_ulysses(args, w: Workload):
+    """ONE problem of the workload's shape, sequence-sharded over the ranks: a step = per head group one
+    packed all-to-all in, the kernel on the rank's head shard, one packed all-to-all out.  Strong scaling: the whole job's
+    FLOPs over the max-over-ranks time.  Also timed in parts (exchange alone with a no-op local op; kernel alone on the
+    head shard).  Without CUDA: a dry run of the exchange on gloo with a no-op local op (no throughput is reported)."""
+    from paper_2606_25473_b200 import ulysses
+    import torch.distributed as dist
+
+    rank, world, local, inited = dist_setup(args.gpus)
+    cuda = torch.cuda.is_available()
+    if not inited:                                       # world size 1 still goes through the collective
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl" if cuda else "gloo", rank=0, world_size=1)
+    P, G = world, args.head_groups
+    if w.H % (P * G) or w.N % P or w.backward or w.Nq:
+        raise SystemExit(f"--ulysses needs H = {w.H} divisible by ranks x head groups = {P * G}, N divisible by {P}, a forward workload")
+    dev = f"cuda:{local}" if cuda else "cpu"
+    if cuda:
+        torch.cuda.set_device(local)
+    n, hg = w.N // P, w.H // (P * G)
+    # this rank's token shard of the SAME global tensors every rank would draw (seeded per tensor and rank: no rank ever
+    # materialises the 1.2 GB global problem just to slice it)
+    gen = torch.Generator().manual_seed(w.seed * 1000 + rank)
+    shard = []
+    for i in range(6):
+        x = torch.randn((w.B, w.H, n, w.d), generator=gen, dtype=torch.float32)
+        if i >= 3:
+            x.mul_(w.tangent_std)
+        shard.append(x.to(w.torch_dtype).to(dev))
+    esz = shard[0].element_size()
+    bytes_in = 6 * shard[0].numel() * esz * (P - 1) // P          # what leaves this rank per step and direction
+    bytes_out = 2 * shard[0].numel() * esz * (P - 1) // P
+    K, W = args.steps, max(args.warmup, 1)
+
+    def noop(g, q, k, v, tq, tk, tv):
+        return torch.empty_like(q), torch.empty_like(q), None
+
+    plan = None
+    if cuda:
+        from paper_2606_25473_b200 import binding as aj
+        kind = {"teacher_forcing": aj.AJ_MASK_TEACHER_FORCING, "block_causal": aj.AJ_MASK_BLOCK_CAUSAL, "full": aj.AJ_MASK_FULL}[w.mask]
+        tz = aj.AJ_TANGENT_CLEAN_ZERO if w.clean_tangent_zero else aj.AJ_TANGENT_DENSE
+        plan = aj.attn_jvp_plan_create(aj.make_problem(w.B, hg, w.N, w.N, w.d, aj.AJ_BF16 if w.dtype == "bf16" else aj.AJ_FP32),
+                                       aj.make_mask(kind, w.frame_len, w.num_frames, w.chunk_frames, tangent_zero=tz)[0])
+        stream = torch.cuda.current_stream()
+        local_op = ulysses.local_attn_jvp(plan, stream.cuda_stream)
+    else:
+        local_op = noop
+
+    def timed(fn):
+        for _ in range(W):
+            fn()
+        if cuda:
+            torch.cuda.synchronize()
+        dist.barrier()
+        if cuda:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(K):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / K
+        else:
+            t0 = time.perf_counter()
+            for _ in range(K):
+                fn()
+            ms = 1e3 * (time.perf_counter() - t0) / K
+        dist.barrier()
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    step_ms = timed(lambda: ulysses.ulysses_attn_jvp(local_op, *shard, head_groups=G))
+    comm_ms = timed(lambda: ulysses.ulysses_attn_jvp(noop, *shard, head_groups=G))
+    kernel_ms = None
+    if cuda:
+        hs = [torch.empty((w.B, hg, w.N, w.d), dtype=w.torch_dtype, device=dev).normal_() for _ in range(6)]
+        kernel_ms = timed(lambda: [local_op(g, *hs) for g in range(G)])
+        aj.attn_jvp_plan_destroy(plan)
+    dist.barrier()
+    if rank == 0:
+        flops = flops_per_call(w)
+        peaks, peak_src = load_peaks()
+        line = {"metric": METRIC, "value": flops / (step_ms * 1e-3) / 1e12 if cuda else None, "unit": UNIT, "n_gpus": world,
+                "steps": K, "warmup": W, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "mode": "ulysses",
+                "config": dict(workload_config(w), parallelism=f"ulysses cp{P}, {G} head group(s) per rank",
+                               tokens_per_rank=n, heads_per_rank=w.H // P),
+                "comm_ms": comm_ms, "kernel_ms": kernel_ms, "a2a_bytes_in_per_rank": bytes_in, "a2a_bytes_out_per_rank": bytes_out,
+                "overlap": None if kernel_ms is None else {"serial_ms": comm_ms + kernel_ms, "hidden_ms": comm_ms + kernel_ms - step_ms},
+                "collectives_per_step": 2 * G, "backend": dist.get_backend(), "dry_run": not cuda,
+                "gpu_launches": K * G if cuda else 0}
+        if cuda:
+            peak = float(peaks.get("bf16_tflops", FALLBACK_PEAKS["bf16_tflops"])) * world
+            line["roofline"] = {"bound": "tensor", "achieved": line["value"], "peak": peak, "unit": "TFLOP/s",
+                                "frac": line["value"] / peak, "traffic": None, "peak_source": f"{peak_src} bf16_tflops x {world} GPUs",
+                                "kernel": "attn_jvp_umma_pair_kernel + all_to_all_single"}
+        print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
 
 
 def main():
@@ -412,11 +570,16 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(WORKLOADS) + list(EXTRA_WORKLOADS))
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ulysses", action="store_true", help="sequence-sharded ranks with the all-to-all on both sides of the kernel")
+    ap.add_argument("--head-groups", type=int, default=2, help="--ulysses: head groups per rank (exchange / kernel pipelining)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     w = {**WORKLOADS, **EXTRA_WORKLOADS}[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
+    elif args.ulysses:
+        run_ulysses(args, w)
+        return
     else:
         run_cuda(args, w)
     if int(os.environ.get("WORLD_SIZE", "1")) > 1:

@@ -17,10 +17,19 @@
  *  - The caller owns every tensor.  "device" pointers are CUDA device memory of the current
  *    device; "host" pointers are ordinary (preferably pinned) host memory.
  *  - Tensors are [B, H, N, d] with d contiguous; strides are in ELEMENTS (aj_tensor).
- *  - Supported: d in {64, 128}; dtype AJ_FP32 (plain-FMA SIMT kernel, any supported d) and
- *    AJ_BF16 (tcgen05/TMEM/TMA kernel for d = 128; SIMT kernel otherwise).  Anything else
- *    returns AJ_ERR_UNSUPPORTED.  There is no CPU fallback.
+ *  - Supported: d in {64, 128}; dtype AJ_BF16 with d = 128 is the performance path (tcgen05 / TMEM / TMA kernels on
+ *    CTA pairs).  Everything else -- AJ_FP32 (any supported d; plain fp32 FMA for the 1e-4 tolerance, R14) and
+ *    AJ_BF16 with d = 64 -- runs the plain-FMA SIMT kernels: a CORRECTNESS path two to three orders of magnitude slower
+ *    (a few TFLOP/s; DESIGN.md section 7 has the measured figure), which attn_jvp_plan_kernel reports as AJ_KERNEL_SIMT.
+ *    Anything else returns AJ_ERR_UNSUPPORTED.  There is no CPU fallback.
  *  - Inputs must be finite: masked-out tail keys are multiplied by an exact 0 (R15).
+ *  - The CUDA device that is current when a plan is created owns the plan: every later call with that plan must be made
+ *    with the same device current (else AJ_ERR_INVALID_ARG).  Plans of different devices may live in one process.
+ *  - Input tensors may be broadcast over heads or batches with a zero stride on the SIMT kernels only (the tcgen05
+ *    kernels return AJ_ERR_UNSUPPORTED); output tensors never (AJ_ERR_INVALID_ARG).
+ *  - The enqueueing calls (attn_jvp_fwd, attn_jvp_fwd_tl, attn_fwd, and attn_bwd after its first call on a plan) make no
+ *    allocation and no synchronisation: they can be captured into a CUDA graph.  The plan caches the TMA
+ *    tensor maps it encodes per tensor argument and re-encodes one only when that argument's pointer or strides change.
  */
 #ifndef ATTN_JVP_H_
 #define ATTN_JVP_H_
@@ -190,7 +199,8 @@ aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_he
 /* attn_jvp_schedule_pair_classes of the plan's mask. */
 aj_status attn_jvp_plan_pair_classes(const aj_plan *plan, int64_t pairs[3]);
 /* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
- * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged. */
+ * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged; the single-CTA kernel also has no
+ * tangent-free mode (AJ_ERR_UNSUPPORTED on AJ_TANGENT_NONE plans). */
 aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
 /* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernels, PER_GROUP for the SIMT kernel; the SIMT
  * kernel supports only PER_GROUP and the CTA-pair kernel only PACKED (AJ_ERR_UNSUPPORTED otherwise).  Rebuilds and re-uploads the schedule; results do not change. */
@@ -205,12 +215,21 @@ aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *la
  * lse: contiguous fp32 [B,H,Nq] (may be NULL).  All DEVICE memory; inputs are only read.  Pointers must be
  * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
  * A plan must not be used by two streams at the same time (it owns a device work counter).
- * Plans whose mask says AJ_TANGENT_NONE accept NULL for tq, tk, tv and to (CTA-pair tcgen05 kernel only; the other
- * kernels return AJ_ERR_UNSUPPORTED for NULL tangents).
+ * Plans whose mask says AJ_TANGENT_NONE never read tq, tk, tv (they may be NULL), fill a non-NULL `to` with zeros and
+ * write O and lse only -- on every kernel that runs them (CTA-pair tcgen05, SIMT).
  */
 aj_status attn_jvp_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v,
                        const aj_tensor *tq, const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o,
                        const aj_tensor *to, float *lse, void *cuda_stream);
+
+/* attn_jvp_fwd that also returns the tangent of lse along the input tangents,
+ *     tlse_a = sum_b p_ab tS_ab = r_a / l_a        (r is the running sum the recurrence carries anyway)
+ * i.e. d/d eps of log sum_b exp(S_ab + eps tS_ab), which a layer-level JVP that consumes L needs.
+ * tlse: contiguous fp32 [B,H,Nq], DEVICE memory, or NULL (then identical to attn_jvp_fwd).  0 for rows without keys,
+ * for rows whose tangents are structurally zero, and on AJ_TANGENT_NONE plans. */
+aj_status attn_jvp_fwd_tl(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v,
+                          const aj_tensor *tq, const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o,
+                          const aj_tensor *to, float *lse, float *tlse, void *cuda_stream);
 
 /* Masked attention forward without tangents: attn_jvp_fwd(plan, q, k, v, NULL, NULL, NULL, o, NULL, lse, stream) on a plan
  * whose mask says AJ_TANGENT_NONE (else AJ_ERR_INVALID_ARG).  q: [B,H,Nq,d], k, v: [B,H,Nk,d] (Nq != Nk allowed: the
@@ -247,6 +266,20 @@ aj_status attn_bwd(aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const 
 aj_status attn_jvp_fwd_host(aj_plan *plan, const void *q, const void *k, const void *v, const void *tq,
                             const void *tk, const void *tv, void *o, void *to, float *lse,
                             void *cuda_stream);
+
+/*
+ * attn_bwd on HOST buffers (SURVEY.md 8(b) conventions as attn_jvp_fwd_host): contiguous [B,H,N,d] arrays in the problem
+ * dtype, lse contiguous fp32 [B,H,Nq].  Head by head: q, k, v, o, dout, lse go up on a copy-in stream, the head's three
+ * kernels run on `cuda_stream` as soon as they have landed, dq, dk, dv come back on a copy-out stream; `cuda_stream`
+ * finally waits for the last copy.  The caller synchronises the stream before reading the outputs.  Staging buffers,
+ * per-head schedules, copy streams and events are plan-owned and created on first use.
+ */
+aj_status attn_bwd_host(aj_plan *plan, const void *q, const void *k, const void *v, const void *o, const float *lse,
+                        const void *dout, void *dq, void *dk, void *dv, void *cuda_stream);
+
+/* How many TMA tensor maps the plan has encoded so far and how many calls found theirs in the plan's cache (either
+ * pointer may be NULL).  Steady-state calls on unchanged tensors encode nothing. */
+aj_status attn_jvp_plan_tensor_map_stats(const aj_plan *plan, int64_t *encodes, int64_t *hits);
 
 /*
  * Device-side health of the plan's last launches: synchronises the device, then *code = 0 if every

@@ -59,6 +59,7 @@ SYMBOLS = [
     "attn_jvp_schedule_create_transposed", "attn_jvp_schedule_entry_flags", "attn_jvp_schedule_pair_classes", "attn_jvp_plan_pair_classes", "attn_fwd", "attn_bwd",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
+    "attn_jvp_fwd_tl", "attn_bwd_host", "attn_jvp_plan_tensor_map_stats",
 ]
 
 _lib = None
@@ -95,6 +96,9 @@ def lib():
         l.attn_jvp_plan_device_status.argtypes = [vp, _I32P]
         l.attn_jvp_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp]
         l.attn_jvp_fwd_host.argtypes = [vp] * 11
+        l.attn_jvp_fwd_tl.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp, vp]
+        l.attn_bwd_host.argtypes = [vp] * 11
+        l.attn_jvp_plan_tensor_map_stats.argtypes = [vp, i64p, i64p]
         for name in SYMBOLS:
             getattr(l, name).restype = ctypes.c_int
         l.attn_jvp_last_error.restype = ctypes.c_char_p
@@ -236,14 +240,26 @@ def attn_jvp_schedule_get(sched):
 
 
 # ---- plans and the forward call ------------------------------------------------------------------------------------
+_PLANS = {}   # plan handle -> (B, H, Nq, Nk, d, dtype): what the tensors of a call must look like
+
+
 def attn_jvp_plan_create(problem: aj_problem, mask: aj_mask_desc) -> ctypes.c_void_p:
     out = ctypes.c_void_p()
     _check(lib().attn_jvp_plan_create(ctypes.byref(problem), ctypes.byref(mask), ctypes.byref(out)))
+    _PLANS[out.value] = (problem.B, problem.H, problem.Nq, problem.Nk, problem.d, problem.dtype)
     return out
 
 
 def attn_jvp_plan_destroy(plan) -> None:
+    _PLANS.pop(getattr(plan, "value", plan), None)
     _check(lib().attn_jvp_plan_destroy(plan))
+
+
+def attn_jvp_plan_tensor_map_stats(plan):
+    """-> (TMA tensor maps encoded so far, cache hits so far)"""
+    a, b = ctypes.c_int64(), ctypes.c_int64()
+    _check(lib().attn_jvp_plan_tensor_map_stats(plan, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def attn_jvp_plan_info(plan):
@@ -282,39 +298,93 @@ def attn_jvp_plan_device_status(plan) -> int:
     return a.value
 
 
-def _tensor(t) -> aj_tensor:
-    """torch [B,H,N,d] tensor (d contiguous) -> aj_tensor view."""
+def _torch_dtype(dtype: int):
+    import torch
+    return torch.bfloat16 if dtype == AJ_BF16 else torch.float32
+
+
+def _tensor(t, plan=None, name: str = "tensor", keys: bool = False, cuda: bool = True) -> aj_tensor:
+    """torch [B,H,N,d] tensor (d contiguous) -> aj_tensor view, checked against the plan's problem: the kernels index by
+    the plan's (B, H, N, d), so a wrong shape, dtype or device must fail here, not fault on the device."""
     if t.dim() != 4 or t.stride(3) != 1:
-        raise ValueError("expected a [B, H, N, d] tensor with contiguous d")
+        raise ValueError(f"{name}: expected a [B, H, N, d] tensor with contiguous d")
+    info = _PLANS.get(getattr(plan, "value", plan))
+    if info is not None:
+        B, H, Nq, Nk, d, dtype = info
+        want = (B, H, Nk if keys else Nq, d)
+        if tuple(t.shape) != want:
+            raise ValueError(f"{name}: shape {tuple(t.shape)} does not match the plan's {want}")
+        if t.dtype != _torch_dtype(dtype):
+            raise ValueError(f"{name}: dtype {t.dtype} does not match the plan's {_torch_dtype(dtype)}")
+        if t.is_cuda != cuda:
+            raise ValueError(f"{name}: expected a {'CUDA' if cuda else 'host'} tensor")
     return aj_tensor(t.data_ptr(), t.stride(0), t.stride(1), t.stride(2))
 
 
-def attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
+def _rowvec(x, plan, name: str, cuda: bool = True):
+    """lse-like argument: contiguous fp32 [B, H, Nq] (or None) -> pointer"""
+    if x is None:
+        return None
+    import torch
+    info = _PLANS.get(getattr(plan, "value", plan))
+    if x.dtype != torch.float32 or not x.is_contiguous() or x.is_cuda != cuda:
+        raise ValueError(f"{name}: expected a contiguous fp32 {'CUDA' if cuda else 'host'} tensor")
+    if info is not None and tuple(x.shape) != (info[0], info[1], info[2]):
+        raise ValueError(f"{name}: shape {tuple(x.shape)} does not match the plan's {(info[0], info[1], info[2])}")
+    return x.data_ptr()
+
+
+_FWD_NAMES = ("q", "k", "v", "tq", "tk", "tv", "o", "to")
+_FWD_KEYS = (False, True, True, False, True, True, False, False)
+
+
+def attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0, tlse=None) -> None:
     """Device tensors (torch.cuda); enqueues on `stream` (a cudaStream_t handle, 0 = default) and returns.
-    tq, tk, tv, to may be None on AJ_TANGENT_NONE plans."""
-    ts = [None if x is None else _tensor(x) for x in (q, k, v, tq, tk, tv, o, to)]
-    _check(lib().attn_jvp_fwd(plan, *[None if x is None else ctypes.byref(x) for x in ts],
-                              None if lse is None else lse.data_ptr(), stream))
+    tq, tk, tv, to may be None on AJ_TANGENT_NONE plans.  tlse: optional fp32 [B,H,Nq] for the tangent of lse."""
+    ts = [None if x is None else _tensor(x, plan, n, kk) for x, n, kk in zip((q, k, v, tq, tk, tv, o, to), _FWD_NAMES, _FWD_KEYS)]
+    args = [None if x is None else ctypes.byref(x) for x in ts]
+    if tlse is None:
+        _check(lib().attn_jvp_fwd(plan, *args, _rowvec(lse, plan, "lse"), stream))
+    else:
+        _check(lib().attn_jvp_fwd_tl(plan, *args, _rowvec(lse, plan, "lse"), _rowvec(tlse, plan, "tlse"), stream))
 
 
 def attn_fwd(plan, q, k, v, o, lse=None, stream: int = 0) -> None:
     """Masked attention forward without tangents (AJ_TANGENT_NONE plans): O and lse only."""
-    ts = [_tensor(x) for x in (q, k, v, o)]
-    _check(lib().attn_fwd(plan, *[ctypes.byref(x) for x in ts], None if lse is None else lse.data_ptr(), stream))
+    ts = [_tensor(x, plan, n, kk) for x, n, kk in zip((q, k, v, o), ("q", "k", "v", "o"), (False, True, True, False))]
+    _check(lib().attn_fwd(plan, *[ctypes.byref(x) for x in ts], _rowvec(lse, plan, "lse"), stream))
+
+
+_BWD_NAMES = ("q", "k", "v", "o", "dout", "dq", "dk", "dv")
+_BWD_KEYS = (False, True, True, False, False, False, True, True)
 
 
 def attn_bwd(plan, q, k, v, o, lse, dout, dq, dk, dv, stream: int = 0) -> None:
     """Primal backward: device tensors; lse is the forward's fp32 [B,H,Nq]; writes dq, dk, dv."""
-    a = [_tensor(x) for x in (q, k, v, o)]
-    b = [_tensor(x) for x in (dout, dq, dk, dv)]
-    _check(lib().attn_bwd(plan, *[ctypes.byref(x) for x in a], lse.data_ptr(), *[ctypes.byref(x) for x in b], stream))
+    ts = [_tensor(x, plan, n, kk) for x, n, kk in zip((q, k, v, o, dout, dq, dk, dv), _BWD_NAMES, _BWD_KEYS)]
+    if lse is None:
+        raise ValueError("attn_bwd needs the forward's lse")
+    _check(lib().attn_bwd(plan, *[ctypes.byref(x) for x in ts[:4]], _rowvec(lse, plan, "lse"),
+                          *[ctypes.byref(x) for x in ts[4:]], stream))
+
+
+def _host(t, plan, name, keys):
+    _tensor(t, plan, name, keys, cuda=False)
+    if not t.is_contiguous():
+        raise ValueError(f"{name}: the host-buffer calls expect contiguous tensors")
+    return t.data_ptr()
 
 
 def attn_jvp_fwd_host(plan, q, k, v, tq, tk, tv, o, to, lse=None, stream: int = 0) -> None:
     """Host tensors (contiguous [B,H,N,d], ideally pinned); copies + kernel are enqueued on `stream`.
     tq, tk, tv, to may be None on AJ_TANGENT_NONE plans."""
-    for x in (q, k, v, tq, tk, tv, o, to):
-        if x is not None and (x.is_cuda or not x.is_contiguous()):
-            raise ValueError("attn_jvp_fwd_host expects contiguous host tensors")
-    _check(lib().attn_jvp_fwd_host(plan, *[None if x is None else x.data_ptr() for x in (q, k, v, tq, tk, tv, o, to)],
-                                   None if lse is None else lse.data_ptr(), stream))
+    ptrs = [None if x is None else _host(x, plan, n, kk) for x, n, kk in zip((q, k, v, tq, tk, tv, o, to), _FWD_NAMES, _FWD_KEYS)]
+    _check(lib().attn_jvp_fwd_host(plan, *ptrs, _rowvec(lse, plan, "lse", cuda=False), stream))
+
+
+def attn_bwd_host(plan, q, k, v, o, lse, dout, dq, dk, dv, stream: int = 0) -> None:
+    """attn_bwd on host tensors (contiguous, ideally pinned): copies + the three kernels are enqueued on `stream`."""
+    ptrs = [_host(x, plan, n, kk) for x, n, kk in zip((q, k, v, o, dout, dq, dk, dv), _BWD_NAMES, _BWD_KEYS)]
+    if lse is None:
+        raise ValueError("attn_bwd_host needs the forward's lse")
+    _check(lib().attn_bwd_host(plan, *ptrs[:4], _rowvec(lse, plan, "lse", cuda=False), *ptrs[4:], stream))

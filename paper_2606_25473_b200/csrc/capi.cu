@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -30,15 +31,31 @@ struct aj_plan {
         uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
         int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
         int32_t num_pairs = 0;
-    } full, head, bwd_q, bwd_k;   // bwd_*: SIMT-tiled schedules of the primal backward (rows x key ranges, keys x row ranges)
+    } full, head;                 // forward
+    // primal backward: query tiles x key ranges (dQ) and key tiles x row ranges (dK, dV) for all B x H heads, and for ONE
+    // head (attn_bwd_host)
+    DevSchedule bwd_q, bwd_k, bwd_q_head, bwd_k_head;
     float *d_delta = nullptr;     // [B, H, Nq] workspace of attn_bwd
-    // attn_jvp_fwd_host: device staging buffers, copy streams, one event per head and direction
-    void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    void *d_out[2] = {nullptr, nullptr};
+    // attn_jvp_fwd_host / attn_bwd_host: device staging buffers, copy streams, one event per head and direction
+    void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // q k v tq tk tv
+    void *d_out[2] = {nullptr, nullptr};                                      // o to
+    void *d_bwd[4] = {nullptr, nullptr, nullptr, nullptr};                    // dout dq dk dv
     float *d_lse = nullptr;
     cudaStream_t s_in = nullptr, s_out = nullptr;
     std::vector<cudaEvent_t> ev_in, ev_k;
     cudaEvent_t ev_begin = nullptr, ev_end = nullptr;
+    // TMA descriptors the plan has encoded, one per tensor slot of a call site (the plan owns them): a slot is
+    // re-encoded only when the tensor view it was encoded for changes.  `mu` guards the cache (the forward takes a const plan
+    // and may be called from several host threads).
+    struct MapSlot {
+        const void *ptr = nullptr;
+        int64_t sb = 0, sh = 0, sn = 0, rows = 0;
+        int32_t box = 0, B = 0, H = 0;
+        CUtensorMap map;
+    };
+    mutable std::mutex mu;
+    mutable std::vector<MapSlot> maps;
+    mutable int64_t map_encodes = 0, map_hits = 0;
 };
 
 namespace {
@@ -144,26 +161,43 @@ aj_status install_schedule(aj_plan *p, int32_t kernel, int32_t tiling) {
     free_schedule(p->head);
     free_schedule(p->bwd_q);      // their tile sizes follow the kernel family
     free_schedule(p->bwd_k);
+    free_schedule(p->bwd_q_head);
+    free_schedule(p->bwd_k_head);
     p->kernel = kernel; p->tiling = tiling;
     return AJ_OK;
 }
 
-aj_status check_tensor(const aj_tensor *t, const char *name, int d, int elem_bytes) {
+// `output`: the kernels write every element once, so heads / batches must not alias.  Inputs may be broadcast over heads or
+// batches with a zero stride on the plain-FMA kernels; the TMA tensor maps of the tcgen05 kernels cannot express it
+// (`tma` = the call will build tensor maps).
+aj_status check_tensor(const aj_tensor *t, const char *name, const aj_problem &p, bool output, bool tma) {
     if (!t || !t->ptr) return fail(AJ_ERR_INVALID_ARG, std::string(name) + " is NULL");
     if ((uintptr_t)t->ptr % 16 != 0) return fail(AJ_ERR_INVALID_ARG, std::string(name) + ": pointer must be 16-byte aligned");
-    if (t->stride_n < d || t->stride_n % 8 || t->stride_h % 8 || t->stride_b % 8 || t->stride_h < 0 || t->stride_b < 0)
+    if (t->stride_n < p.d || t->stride_n % 8 || t->stride_h % 8 || t->stride_b % 8 || t->stride_h < 0 || t->stride_b < 0)
         return fail(AJ_ERR_INVALID_ARG, std::string(name) + ": strides must be multiples of 8 elements with stride_n >= d");
-    (void)elem_bytes;
+    const bool bcast = (p.H > 1 && t->stride_h == 0) || (p.B > 1 && t->stride_b == 0);
+    if (bcast && output) return fail(AJ_ERR_INVALID_ARG, std::string(name) + ": an output tensor must not alias heads or batches (zero stride)");
+    if (bcast && tma) return fail(AJ_ERR_UNSUPPORTED, std::string(name) + ": zero head / batch strides (broadcast inputs) are not supported by the tcgen05 kernels");
     return AJ_OK;
 }
 
-aj_status encode_map(CUtensorMap *map, const aj_tensor &t, const aj_problem &p, int64_t n_rows, int box_rows) {
+aj_status check_device(const aj_plan *p) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev != p->device)
+        return fail(AJ_ERR_INVALID_ARG, "the current CUDA device (" + std::to_string(dev) + ") is not the plan's device (" + std::to_string(p->device) + ")");
+    return AJ_OK;
+}
+
+aj_status encode_map_raw(CUtensorMap *map, const aj_tensor &t, const aj_problem &p, int64_t n_rows, int box_rows) {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    // dims innermost first: d, N, H, B.  A size-1 dimension still needs a legal (16-byte multiple) stride.
+    // dims innermost first: d, N, H, B.  A size-1 dimension still needs a legal (non-zero, 16-byte multiple) stride, which is
+    // never used to address anything; a zero stride over a dimension > 1 was rejected by check_tensor.
     cuuint64_t dims[4] = {(cuuint64_t)p.d, (cuuint64_t)n_rows, (cuuint64_t)p.H, (cuuint64_t)p.B};
-    auto bytes = [](int64_t elems) { return (cuuint64_t)std::max<int64_t>(elems, 8) * 2; };
-    cuuint64_t strides[3] = {bytes(t.stride_n), bytes(t.stride_h), bytes(t.stride_b)};
+    auto bytes = [](int64_t elems, int dim) { return (cuuint64_t)(dim == 1 ? std::max<int64_t>(elems, 8) : elems) * 2; };
+    cuuint64_t strides[3] = {bytes(t.stride_n, 0), bytes(t.stride_h, p.H), bytes(t.stride_b, p.B)};
     cuuint32_t box[4] = {64, (cuuint32_t)box_rows, 1, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, t.ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -171,6 +205,26 @@ aj_status encode_map(CUtensorMap *map, const aj_tensor &t, const aj_problem &p, 
     if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r));
     return AJ_OK;
 }
+
+// The tensor map of `t` for call-site slot `slot`: from the plan's cache if the slot was encoded for the same view.
+aj_status encode_map(const aj_plan *plan, int slot, CUtensorMap *map, const aj_tensor &t, const aj_problem &p, int64_t n_rows, int box_rows) {
+    std::lock_guard<std::mutex> lock(plan->mu);
+    if ((size_t)slot >= plan->maps.size()) plan->maps.resize(slot + 1);
+    aj_plan::MapSlot &m = plan->maps[slot];
+    if (m.ptr == t.ptr && m.sb == t.stride_b && m.sh == t.stride_h && m.sn == t.stride_n && m.rows == n_rows && m.box == box_rows &&
+        m.B == p.B && m.H == p.H) {
+        *map = m.map;
+        ++plan->map_hits;
+        return AJ_OK;
+    }
+    if (aj_status st = encode_map_raw(&m.map, t, p, n_rows, box_rows)) { m.ptr = nullptr; return st; }
+    m.ptr = t.ptr; m.sb = t.stride_b; m.sh = t.stride_h; m.sn = t.stride_n; m.rows = n_rows; m.box = box_rows; m.B = p.B; m.H = p.H;
+    *map = m.map;
+    ++plan->map_encodes;
+    return AJ_OK;
+}
+// call-site slots of the cache
+enum { SLOT_FWD = 0, SLOT_BWD = 8, SLOT_HEAD = 16, SLOTS_PER_HEAD = 16 };   // per head: 6 forward + 8 backward maps
 
 }  // namespace
 
@@ -227,10 +281,13 @@ aj_status attn_jvp_plan_destroy(aj_plan *p) {
     free_schedule(p->head);
     free_schedule(p->bwd_q);
     free_schedule(p->bwd_k);
+    free_schedule(p->bwd_q_head);
+    free_schedule(p->bwd_k_head);
     cudaFree(p->d_delta);
     cudaFree(p->d_counters);
     for (void *x : p->d_in) cudaFree(x);
     for (void *x : p->d_out) cudaFree(x);
+    for (void *x : p->d_bwd) cudaFree(x);
     cudaFree(p->d_lse);
     for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
     for (cudaEvent_t e : p->ev_k) cudaEventDestroy(e);
@@ -259,6 +316,8 @@ aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
     if (kernel == AJ_KERNEL_AUTO) kernel = auto_kernel(p->problem);
     if (kernel != AJ_KERNEL_SIMT && !is_umma(kernel)) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
     if (is_umma(kernel) && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernels need bf16 and d = 128");
+    if (kernel == AJ_KERNEL_UMMA && p->mask.tangent_zero == AJ_TANGENT_NONE)
+        return fail(AJ_ERR_UNSUPPORTED, "the single-CTA tcgen05 kernel has no tangent-free mode (AJ_TANGENT_NONE plans run the CTA-pair or the SIMT kernel)");
     if (kernel == p->kernel) return AJ_OK;
     return install_schedule(p, kernel, default_tiling(kernel));
 }
@@ -291,29 +350,28 @@ aj_status attn_jvp_plan_device_status(aj_plan *p, int32_t *code) {
 namespace {
 
 // One kernel launch over the tasks of `ds`, which were built for a [B, H] problem (the plan's, or B = H = 1 with the
-// tensor views already moved to the head they address).
+// tensor views already moved to the head they address).  `slot`: first of the six tensor-map cache slots of the call site.
 aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int32_t B, int32_t H, const aj_tensor *const ts[8],
-                          float *lse, cudaStream_t stream) {
+                          float *lse, float *tlse, cudaStream_t stream, int slot) {
     aj_problem pr = p->problem;
     pr.B = B; pr.H = H;
     if (ds.num_tasks == 0) return AJ_OK;
     cudaError_t e;
-    // AJ_TANGENT_NONE plans may leave tq, tk, tv, to NULL: every task is primal-only and never touches them (the tensor
-    // maps of the absent tangents alias the primals so that they stay valid)
-    const bool no_tangents = !ts[3] || !ts[4] || !ts[5] || !ts[7];
-    if (no_tangents && p->kernel != AJ_KERNEL_UMMA_PAIR)
-        return fail(AJ_ERR_UNSUPPORTED, "NULL tangents need the CTA-pair tcgen05 kernel (bf16, d = 128)");
+    // AJ_TANGENT_NONE plans: every kernel ignores tq, tk, tv (they may be NULL), writes tO = 0 where `to` is given and
+    // tlse = 0 (the tensor maps of the absent tangents alias the primals so that they stay valid)
+    const bool none = p->mask.tangent_zero == AJ_TANGENT_NONE;
     if (is_umma(p->kernel)) {
         aj::UmmaParams prm;
         std::memset(&prm, 0, sizeof(prm));
         aj_status st;
-        if ((st = encode_map(&prm.tm_q, *ts[0], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&prm.tm_tq, *(ts[3] ? ts[3] : ts[0]), pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&prm.tm_k, *ts[1], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tk, *(ts[4] ? ts[4] : ts[1]), pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_v, *ts[2], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&prm.tm_tv, *(ts[5] ? ts[5] : ts[2]), pr, pr.Nk, aj::UMMA_TILE_K))) return st;
-        prm.o = *ts[6]; prm.lse = lse;
+        const aj_tensor *tq = (none || !ts[3]) ? ts[0] : ts[3], *tk = (none || !ts[4]) ? ts[1] : ts[4], *tv = (none || !ts[5]) ? ts[2] : ts[5];
+        if ((st = encode_map(p, slot + 0, &prm.tm_q, *ts[0], pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(p, slot + 1, &prm.tm_tq, *tq, pr, pr.Nq, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(p, slot + 2, &prm.tm_k, *ts[1], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(p, slot + 3, &prm.tm_tk, *tk, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(p, slot + 4, &prm.tm_v, *ts[2], pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(p, slot + 5, &prm.tm_tv, *tv, pr, pr.Nk, aj::UMMA_TILE_K))) return st;
+        prm.o = *ts[6]; prm.lse = lse; prm.tlse = tlse;
         if (ts[7]) prm.to = *ts[7];
         prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke; prm.rows = ds.d_rows; prm.counters = p->d_counters;
         prm.num_tasks = ds.num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
@@ -323,8 +381,12 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
                                              : aj::launch_umma(prm, std::min(p->num_sms, ds.num_tasks), stream);
     } else {
         aj::SimtParams prm;
-        prm.q = *ts[0]; prm.k = *ts[1]; prm.v = *ts[2]; prm.tq = *ts[3]; prm.tk = *ts[4]; prm.tv = *ts[5]; prm.o = *ts[6]; prm.to = *ts[7];
-        prm.lse = lse; prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke;
+        std::memset(&prm, 0, sizeof(prm));
+        prm.q = *ts[0]; prm.k = *ts[1]; prm.v = *ts[2]; prm.o = *ts[6];
+        if (!none) { prm.tq = *ts[3]; prm.tk = *ts[4]; prm.tv = *ts[5]; }
+        if (ts[7]) prm.to = *ts[7];
+        prm.no_tangents = none ? 1 : 0;
+        prm.lse = lse; prm.tlse = tlse; prm.tasks = ds.d_tasks; prm.k_begin = ds.d_kb; prm.k_end = ds.d_ke;
         prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
         e = aj::launch_simt(prm, pr.dtype, pr.d, ds.num_tasks, stream);
     }
@@ -336,22 +398,29 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
 
 extern "C" {
 
-aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
-                       const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
-                       void *cuda_stream) {
+aj_status attn_jvp_fwd_tl(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
+                          const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
+                          float *tlse, void *cuda_stream) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (aj_status st = check_device(p)) return st;
     const aj_problem &pr = p->problem;
-    const int eb = pr.dtype == AJ_BF16 ? 2 : 4;
     const aj_tensor *ts[8] = {q, k, v, tq, tk, tv, o, to};
     const char *names[8] = {"q", "k", "v", "tq", "tk", "tv", "o", "to"};
     const bool may_omit = p->mask.tangent_zero == AJ_TANGENT_NONE;
     for (int i = 0; i < 8; ++i) {
         const bool tangent = (i >= 3 && i <= 5) || i == 7;
         if (tangent && may_omit && !ts[i]) continue;
-        if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
+        if (aj_status st = check_tensor(ts[i], names[i], pr, i >= 6, is_umma(p->kernel))) return st;
     }
     if (lse && (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: pointer must be 4-byte aligned");
-    return launch_schedule(p, p->full, pr.B, pr.H, ts, lse, (cudaStream_t)cuda_stream);
+    if (tlse && (uintptr_t)tlse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "tlse: pointer must be 4-byte aligned");
+    return launch_schedule(p, p->full, pr.B, pr.H, ts, lse, tlse, (cudaStream_t)cuda_stream, SLOT_FWD);
+}
+
+aj_status attn_jvp_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *tq,
+                       const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o, const aj_tensor *to, float *lse,
+                       void *cuda_stream) {
+    return attn_jvp_fwd_tl(p, q, k, v, tq, tk, tv, o, to, lse, nullptr, cuda_stream);
 }
 
 aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o, float *lse,
@@ -361,44 +430,46 @@ aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, con
     return attn_jvp_fwd(p, q, k, v, nullptr, nullptr, nullptr, o, nullptr, lse, cuda_stream);
 }
 
-aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o, const float *lse,
-                   const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv, void *cuda_stream) {
-    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
-    const aj_problem &pr = p->problem;
-    const int eb = pr.dtype == AJ_BF16 ? 2 : 4;
-    const aj_tensor *ts[8] = {q, k, v, o, dout, dq, dk, dv};
-    const char *names[8] = {"q", "k", "v", "o", "dout", "dq", "dk", "dv"};
-    for (int i = 0; i < 8; ++i)
-        if (aj_status st = check_tensor(ts[i], names[i], pr.d, eb)) return st;
-    if (!lse || (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: NULL or misaligned");
-    // bf16, d = 128 (unless the plan was forced to the SIMT kernels): tcgen05 passes; otherwise plain-FMA kernels
-    const bool umma = umma_covers(pr) && p->kernel != AJ_KERNEL_SIMT;
+}  // extern "C"
+
+namespace {
+
+// The backward schedules of `prob` (the plan's problem, or one head of it): query tiles x key ranges (dQ) and key tiles x
+// row ranges (dK, dV; the transposed mask), tiled for the kernel family that will run; built and uploaded on first use.
+aj_status ensure_bwd_schedules(aj_plan *p, const aj_problem &prob, bool umma, aj_plan::DevSchedule &bq, aj_plan::DevSchedule &bk) {
     const int tile_s = umma ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q, tile_m = umma ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
-    // first use: the two schedules (query tiles x key ranges; key tiles x row ranges) and the delta workspace
-    if (!p->bwd_q.sched) {
+    if (!bq.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_tiled(&p->problem, &p->mask, tile_s, tile_m, AJ_TILING_PER_GROUP, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_q, umma ? p->num_sms : 0)) return st;
+        if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tile_s, tile_m, AJ_TILING_PER_GROUP, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, bq, umma ? p->num_sms : 0)) return st;
     }
-    if (!p->bwd_k.sched) {
+    if (!bk.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_transposed(&p->problem, &p->mask, tile_s, tile_m, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, p->bwd_k, umma ? p->num_sms : 0)) return st;
+        if (aj_status st = attn_jvp_schedule_create_transposed(&prob, &p->mask, tile_s, tile_m, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, bk, umma ? p->num_sms : 0)) return st;
     }
-    if (!p->d_delta) {
-        cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
-        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
-    }
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    return AJ_OK;
+}
+
+// bf16, d = 128 (unless the plan was forced to the SIMT kernels): tcgen05 passes; otherwise plain-FMA kernels
+bool bwd_uses_umma(const aj_plan *p) { return umma_covers(p->problem) && p->kernel != AJ_KERNEL_SIMT; }
+
+// The three kernels of one backward call over the tasks of (bq, bk), which were built for a [B, H] problem.
+// ts = {q, k, v, o, dout, dq, dk, dv}; lse, delta: [B, H, Nq] of that problem; `slot`: first of eight tensor-map slots.
+aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_plan::DevSchedule &bk, int32_t B, int32_t H,
+                     const aj_tensor *const ts[8], const float *lse, float *delta, cudaStream_t stream, int slot) {
+    aj_problem pr = p->problem;
+    pr.B = B; pr.H = H;
+    const aj_tensor *q = ts[0], *k = ts[1], *v = ts[2], *o = ts[3], *dout = ts[4], *dq = ts[5], *dk = ts[6], *dv = ts[7];
     aj::BwdParams prm;
     prm.q = *q; prm.k = *k; prm.v = *v; prm.o = *o; prm.dout = *dout; prm.dq = *dq; prm.dk = *dk; prm.dv = *dv;
-    prm.lse = lse; prm.delta = p->d_delta;
-    prm.q_tasks = p->bwd_q.d_tasks; prm.q_kb = p->bwd_q.d_kb; prm.q_ke = p->bwd_q.d_ke;
-    prm.k_tasks = p->bwd_k.d_tasks; prm.k_rb = p->bwd_k.d_kb; prm.k_re = p->bwd_k.d_ke;
+    prm.lse = lse; prm.delta = delta;
+    prm.q_tasks = bq.d_tasks; prm.q_kb = bq.d_kb; prm.q_ke = bq.d_ke;
+    prm.k_tasks = bk.d_tasks; prm.k_rb = bk.d_kb; prm.k_re = bk.d_ke;
     prm.B = pr.B; prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
     cudaError_t e;
-    if (!umma) {
-        e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, p->bwd_q.num_tasks, p->bwd_k.num_tasks, stream);
+    if (!bwd_uses_umma(p)) {
+        e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, bq.num_tasks, bk.num_tasks, stream);
         if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
         return AJ_OK;
     }
@@ -406,21 +477,21 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     if (e != cudaSuccess) return cuda_fail(e, "backward delta kernel launch");
     for (int pass = 0; pass < 2; ++pass) {
         const bool keys = pass == 1;
-        const aj_plan::DevSchedule &ds = keys ? p->bwd_k : p->bwd_q;
+        const aj_plan::DevSchedule &ds = keys ? bk : bq;
         aj::BwdUmmaParams up;
         std::memset(&up, 0, sizeof(up));
         aj_status st;
         // stationary operands (128-row boxes) and streamed operands (64-row boxes) of the pass
         const aj_tensor *a1 = keys ? k : q, *a2 = keys ? v : dout, *b1 = keys ? q : k, *b2 = keys ? dout : v;
         const int64_t na = keys ? pr.Nk : pr.Nq, nb = keys ? pr.Nq : pr.Nk;
-        if ((st = encode_map(&up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(&up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(&up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
+        if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
+        if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
         up.a1 = *a1; up.a2 = *a2; up.Na = (int32_t)na;
         up.out1 = keys ? *dk : *dq;
         up.out2 = *dv;
-        up.lse = lse; up.delta = p->d_delta;
+        up.lse = lse; up.delta = delta;
         up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.err = p->d_counters + 2;
         up.cta_off = ds.d_pair_off; up.cta_ids = ds.d_pair_ids;
         up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
@@ -431,9 +502,128 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     return AJ_OK;
 }
 
+// device staging of the host-buffer calls: `n` buffers of `bytes` each, allocated on first use
+aj_status ensure_staging(void **bufs, int n, const size_t *bytes) {
+    for (int i = 0; i < n; ++i)
+        if (!bufs[i]) {
+            cudaError_t e = cudaMalloc(&bufs[i], bytes[i]);
+            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for staging") : cuda_fail(e, "staging allocation");
+        }
+    return AJ_OK;
+}
+
+aj_status ensure_copy_streams(aj_plan *p) {
+    if (p->s_in) return AJ_OK;
+    const int nheads = p->problem.B * p->problem.H;
+    cudaError_t e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_begin, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_end, cudaEventDisableTiming);
+    p->ev_in.assign(nheads, nullptr); p->ev_k.assign(nheads, nullptr);
+    for (int i = 0; i < nheads && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_k[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "copy streams / events");
+    return AJ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o, const float *lse,
+                   const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv, void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (aj_status st = check_device(p)) return st;
+    const aj_problem &pr = p->problem;
+    const aj_tensor *ts[8] = {q, k, v, o, dout, dq, dk, dv};
+    const char *names[8] = {"q", "k", "v", "o", "dout", "dq", "dk", "dv"};
+    const bool umma = bwd_uses_umma(p);
+    for (int i = 0; i < 8; ++i)
+        if (aj_status st = check_tensor(ts[i], names[i], pr, i >= 5, umma)) return st;
+    if (!lse || (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: NULL or misaligned");
+    // first use: the two schedules and the delta workspace (synchronous host work and allocations)
+    if (aj_status st = ensure_bwd_schedules(p, p->problem, umma, p->bwd_q, p->bwd_k)) return st;
+    if (!p->d_delta) {
+        cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
+    }
+    return launch_bwd(p, p->bwd_q, p->bwd_k, pr.B, pr.H, ts, lse, p->d_delta, (cudaStream_t)cuda_stream, SLOT_BWD);
+}
+
+aj_status attn_bwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *o, const float *lse,
+                        const void *dout, void *dq, void *dk, void *dv, void *cuda_stream) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (aj_status st = check_device(p)) return st;
+    if (!q || !k || !v || !o || !lse || !dout || !dq || !dk || !dv) return fail(AJ_ERR_INVALID_ARG, "a host pointer is NULL");
+    const aj_problem &pr = p->problem;
+    const size_t eb = pr.dtype == AJ_BF16 ? 2 : 4;
+    const int nheads = pr.B * pr.H;
+    const size_t hq = (size_t)pr.Nq * pr.d * eb, hk = (size_t)pr.Nk * pr.d * eb;     // one head of a tensor
+    const size_t nq_bytes = hq * nheads, nk_bytes = hk * nheads, lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    {   // staging: q k v (shared with the forward) | o | dout dq dk dv | lse | delta
+        const size_t in_bytes[3] = {nq_bytes, nk_bytes, nk_bytes}, bwd_bytes[4] = {nq_bytes, nq_bytes, nk_bytes, nk_bytes};
+        if (aj_status st = ensure_staging(p->d_in, 3, in_bytes)) return st;
+        if (aj_status st = ensure_staging(p->d_out, 1, &nq_bytes)) return st;
+        if (aj_status st = ensure_staging(p->d_bwd, 4, bwd_bytes)) return st;
+        if (aj_status st = ensure_staging((void **)&p->d_lse, 1, &lse_bytes)) return st;
+        if (aj_status st = ensure_staging((void **)&p->d_delta, 1, &lse_bytes)) return st;
+    }
+    if (aj_status st = ensure_copy_streams(p)) return st;
+    aj_problem one = p->problem;
+    one.B = 1; one.H = 1;
+    if (aj_status st = ensure_bwd_schedules(p, one, bwd_uses_umma(p), p->bwd_q_head, p->bwd_k_head)) return st;
+    // Same pipeline as attn_jvp_fwd_host: head i's q, k, v, o, dout, lse go up on the copy-in stream, its three kernels run on
+    // the caller's stream as soon as they have landed, its dq, dk, dv come back on the copy-out stream.
+    cudaError_t e = cudaEventRecord(p->ev_begin, stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_in, p->ev_begin, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_begin, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
+    const void *src[5] = {q, k, v, o, dout};
+    void *dst[5] = {p->d_in[0], p->d_in[1], p->d_in[2], p->d_out[0], p->d_bwd[0]};
+    void *res_d[3] = {p->d_bwd[1], p->d_bwd[2], p->d_bwd[3]};
+    void *res_h[3] = {dq, dk, dv};
+    for (int hd = 0; hd < nheads; ++hd) {
+        for (int i = 0; i < 5 && e == cudaSuccess; ++i) {
+            const size_t hb = (i == 1 || i == 2) ? hk : hq;
+            e = cudaMemcpyAsync((char *)dst[i] + hd * hb, (const char *)src[i] + hd * hb, hb, cudaMemcpyHostToDevice, p->s_in);
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(p->d_lse + (size_t)hd * pr.Nq, lse + (size_t)hd * pr.Nq, pr.Nq * sizeof(float), cudaMemcpyHostToDevice, p->s_in);
+        if (e == cudaSuccess) e = cudaEventRecord(p->ev_in[hd], p->s_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_in[hd], 0);
+        if (e != cudaSuccess) return cuda_fail(e, "host-to-device copy");
+        aj_tensor t[8];
+        const aj_tensor *ts[8];
+        void *base[8] = {p->d_in[0], p->d_in[1], p->d_in[2], p->d_out[0], p->d_bwd[0], p->d_bwd[1], p->d_bwd[2], p->d_bwd[3]};
+        for (int i = 0; i < 8; ++i) {
+            const bool is_k = i == 1 || i == 2 || i >= 6;
+            const int64_t n = is_k ? pr.Nk : pr.Nq;
+            t[i].ptr = (char *)base[i] + hd * (is_k ? hk : hq);
+            t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = n * pr.d;
+            ts[i] = &t[i];
+        }
+        if (aj_status st = launch_bwd(p, p->bwd_q_head, p->bwd_k_head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq,
+                                      p->d_delta + (size_t)hd * pr.Nq, stream, SLOT_HEAD + hd * SLOTS_PER_HEAD + 8)) return st;
+        e = cudaEventRecord(p->ev_k[hd], stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
+        for (int i = 0; i < 3 && e == cudaSuccess; ++i) {
+            const size_t hb = i == 0 ? hq : hk;
+            e = cudaMemcpyAsync((char *)res_h[i] + hd * hb, (char *)res_d[i] + hd * hb, hb, cudaMemcpyDeviceToHost, p->s_out);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "device-to-host copy");
+    }
+    e = cudaEventRecord(p->ev_end, p->s_out);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_end, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
+    return AJ_OK;
+}
+
 aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void *v, const void *tq, const void *tk,
                             const void *tv, void *o, void *to, float *lse, void *cuda_stream) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (aj_status st = check_device(p)) return st;
     const void *in[6] = {q, k, v, tq, tk, tv};
     const bool no_tangents = p->mask.tangent_zero == AJ_TANGENT_NONE && !tq && !tk && !tv && !to;   // forward only
     for (int i = 0; i < (no_tangents ? 3 : 6); ++i) if (!in[i]) return fail(AJ_ERR_INVALID_ARG, "a host input pointer is NULL");
@@ -445,25 +635,14 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
     const size_t nq_bytes = hq_bytes * nheads, nk_bytes = hk_bytes * nheads;
     const size_t lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
-    cudaError_t e = cudaSuccess;
-    for (int i = 0; i < (no_tangents ? 3 : 6) && e == cudaSuccess; ++i)
-        if (!p->d_in[i]) e = cudaMalloc(&p->d_in[i], (i == 0 || i == 3) ? nq_bytes : nk_bytes);
-    for (int i = 0; i < (no_tangents ? 1 : 2) && e == cudaSuccess; ++i)
-        if (!p->d_out[i]) e = cudaMalloc(&p->d_out[i], nq_bytes);
-    if (e == cudaSuccess && !p->d_lse) e = cudaMalloc(&p->d_lse, lse_bytes);
-    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for staging") : cuda_fail(e, "staging allocation");
-    if (!p->s_in) {
-        e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking);
-        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_begin, cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_end, cudaEventDisableTiming);
-        p->ev_in.assign(nheads, nullptr); p->ev_k.assign(nheads, nullptr);
-        for (int i = 0; i < nheads && e == cudaSuccess; ++i) {
-            e = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_k[i], cudaEventDisableTiming);
-        }
-        if (e != cudaSuccess) return cuda_fail(e, "copy streams / events");
+    {
+        const size_t in_bytes[6] = {nq_bytes, nk_bytes, nk_bytes, nq_bytes, nk_bytes, nk_bytes}, out_bytes[2] = {nq_bytes, nq_bytes};
+        if (aj_status st = ensure_staging(p->d_in, no_tangents ? 3 : 6, in_bytes)) return st;
+        if (aj_status st = ensure_staging(p->d_out, no_tangents ? 1 : 2, out_bytes)) return st;
+        if (aj_status st = ensure_staging((void **)&p->d_lse, 1, &lse_bytes)) return st;
     }
+    if (aj_status st = ensure_copy_streams(p)) return st;
+    cudaError_t e = cudaSuccess;
     if (!p->head.sched) {
         aj_problem one = p->problem;
         one.B = 1; one.H = 1;
@@ -493,7 +672,7 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
             t[i].stride_n = pr.d; t[i].stride_h = n * pr.d; t[i].stride_b = n * pr.d;
             ts[i] = (no_tangents && ((i >= 3 && i <= 5) || i == 7)) ? nullptr : &t[i];
         }
-        if (aj_status st = launch_schedule(p, p->head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq, stream)) return st;
+        if (aj_status st = launch_schedule(p, p->head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq, nullptr, stream, SLOT_HEAD + hd * SLOTS_PER_HEAD)) return st;
         e = cudaEventRecord(p->ev_k[hd], stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync((char *)o + hd * hq_bytes, (char *)p->d_out[0] + hd * hq_bytes, hq_bytes, cudaMemcpyDeviceToHost, p->s_out);
@@ -506,6 +685,14 @@ aj_status attn_jvp_fwd_host(aj_plan *p, const void *q, const void *k, const void
     e = cudaEventRecord(p->ev_end, p->s_out);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_end, 0);
     if (e != cudaSuccess) return cuda_fail(e, "stream ordering");
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_tensor_map_stats(const aj_plan *p, int64_t *encodes, int64_t *hits) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    std::lock_guard<std::mutex> lock(p->mu);
+    if (encodes) *encodes = p->map_encodes;
+    if (hits) *hits = p->map_hits;
     return AJ_OK;
 }
 

@@ -38,7 +38,8 @@ __device__ __forceinline__ float warp_sum(float x) {
     return x;
 }
 
-template <typename T, int D>
+// PRIMAL: a plan without tangents (AJ_TANGENT_NONE): tq, tk, tv are never read (they may be NULL), tO = 0, tlse = 0.
+template <typename T, int D, bool PRIMAL>
 __global__ void __launch_bounds__(NWARPS * 32)
 attn_jvp_simt_kernel(SimtParams prm) {
     constexpr int DP = D + 1;        // padded row: lane-per-key reads hit distinct banks
@@ -54,18 +55,18 @@ attn_jvp_simt_kernel(SimtParams prm) {
     const aj_task task = prm.tasks[blockIdx.x];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const T *q = (const T *)prm.q.ptr + task.b * prm.q.stride_b + task.h * prm.q.stride_h;
-    const T *tq = (const T *)prm.tq.ptr + task.b * prm.tq.stride_b + task.h * prm.tq.stride_h;
+    const T *tq = PRIMAL ? nullptr : (const T *)prm.tq.ptr + task.b * prm.tq.stride_b + task.h * prm.tq.stride_h;
     const T *k = (const T *)prm.k.ptr + task.b * prm.k.stride_b + task.h * prm.k.stride_h;
-    const T *tk = (const T *)prm.tk.ptr + task.b * prm.tk.stride_b + task.h * prm.tk.stride_h;
+    const T *tk = PRIMAL ? nullptr : (const T *)prm.tk.ptr + task.b * prm.tk.stride_b + task.h * prm.tk.stride_h;
     const T *v = (const T *)prm.v.ptr + task.b * prm.v.stride_b + task.h * prm.v.stride_h;
-    const T *tv = (const T *)prm.tv.ptr + task.b * prm.tv.stride_b + task.h * prm.tv.stride_h;
+    const T *tv = PRIMAL ? nullptr : (const T *)prm.tv.ptr + task.b * prm.tv.stride_b + task.h * prm.tv.stride_h;
 
     // Alg. 1 line "Load Q_i, tQ_i"; rows past the group end are zero and never stored.
     for (int i = threadIdx.x; i < TQ * D; i += blockDim.x) {
         int r = i / D, c = i % D;
         bool ok = r < task.q_rows;
         sQ[i] = ok ? to_f32(q[(int64_t)(task.q_begin + r) * prm.q.stride_n + c]) : 0.f;
-        sTQ[i] = ok ? to_f32(tq[(int64_t)(task.q_begin + r) * prm.tq.stride_n + c]) : 0.f;
+        sTQ[i] = (ok && !PRIMAL) ? to_f32(tq[(int64_t)(task.q_begin + r) * prm.tq.stride_n + c]) : 0.f;
     }
 
     float m[ROWS_PER_WARP], l[ROWS_PER_WARP], rs[ROWS_PER_WARP];
@@ -86,9 +87,9 @@ attn_jvp_simt_kernel(SimtParams prm) {
                 bool ok = kt + r < k1;
                 int64_t row = kt + r;
                 sK[r * DP + c] = ok ? to_f32(k[row * prm.k.stride_n + c]) : 0.f;
-                sTK[r * DP + c] = ok ? to_f32(tk[row * prm.tk.stride_n + c]) : 0.f;
+                sTK[r * DP + c] = (ok && !PRIMAL) ? to_f32(tk[row * prm.tk.stride_n + c]) : 0.f;
                 sV[r * DP + c] = ok ? to_f32(v[row * prm.v.stride_n + c]) : 0.f;
-                sTV[r * DP + c] = ok ? to_f32(tv[row * prm.tv.stride_n + c]) : 0.f;
+                sTV[r * DP + c] = (ok && !PRIMAL) ? to_f32(tv[row * prm.tv.stride_n + c]) : 0.f;
             }
             __syncthreads();
             const bool valid = kt + lane < k1;               // tile-valid mask B_ij
@@ -132,7 +133,7 @@ attn_jvp_simt_kernel(SimtParams prm) {
 
     // Epilogue.  A task with no keys writes O = 0, tO = 0, lse = -inf (R9).
     T *o = (T *)prm.o.ptr + task.b * prm.o.stride_b + task.h * prm.o.stride_h;
-    T *to = (T *)prm.to.ptr + task.b * prm.to.stride_b + task.h * prm.to.stride_h;
+    T *to = prm.to.ptr ? (T *)prm.to.ptr + task.b * prm.to.stride_b + task.h * prm.to.stride_h : nullptr;
 #pragma unroll
     for (int i = 0; i < ROWS_PER_WARP; ++i) {
         const int r = warp * ROWS_PER_WARP + i;
@@ -146,20 +147,26 @@ attn_jvp_simt_kernel(SimtParams prm) {
             const float on = accO[i][j] * inv;
             const float tn = accT[i][j] * inv - rl * on;             // Eq. 45
             o[row * prm.o.stride_n + lane + 32 * j] = from_f32<T>(on);
-            to[row * prm.to.stride_n + lane + 32 * j] = from_f32<T>(tn);
+            if (to) to[row * prm.to.stride_n + lane + 32 * j] = from_f32<T>(PRIMAL ? 0.f : tn);
         }
         if (prm.lse && lane == 0)
             prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + row] = empty ? -CUDART_INF_F : m[i] + logf(l[i]);
+        if (prm.tlse && lane == 0)                                    // tangent of lse: r / l
+            prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + row] = PRIMAL ? 0.f : rl;
     }
 }
 
+template <typename T, int D, bool PRIMAL>
+cudaError_t launch_p(const SimtParams &prm, int num_tasks, cudaStream_t stream) {
+    const size_t smem = sizeof(float) * (2 * TQ * D + 4 * TK * (D + 1));
+    static std::atomic<uint64_t> configured{0};
+    if (cudaError_t e = ensure_dynamic_smem(attn_jvp_simt_kernel<T, D, PRIMAL>, (int)smem, configured)) return e;
+    attn_jvp_simt_kernel<T, D, PRIMAL><<<num_tasks, NWARPS * 32, smem, stream>>>(prm);
+    return cudaGetLastError();
+}
 template <typename T, int D>
 cudaError_t launch_t(const SimtParams &prm, int num_tasks, cudaStream_t stream) {
-    const size_t smem = sizeof(float) * (2 * TQ * D + 4 * TK * (D + 1));
-    cudaError_t e = cudaFuncSetAttribute(attn_jvp_simt_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attn_jvp_simt_kernel<T, D><<<num_tasks, NWARPS * 32, smem, stream>>>(prm);
-    return cudaGetLastError();
+    return prm.no_tangents ? launch_p<T, D, true>(prm, num_tasks, stream) : launch_p<T, D, false>(prm, num_tasks, stream);
 }
 
 }  // namespace

@@ -397,13 +397,9 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
 
 cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream) {
     if (grid <= 0 || prm.num_tasks <= 0) return cudaSuccess;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(attn_bwd_umma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(attn_bwd_umma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<uint64_t> configured[2];
+    if (cudaError_t e = keys ? ensure_dynamic_smem(attn_bwd_umma_kernel<true>, (int)SMEM_TOTAL, configured[1])
+                             : ensure_dynamic_smem(attn_bwd_umma_kernel<false>, (int)SMEM_TOTAL, configured[0])) return e;
     if (keys) attn_bwd_umma_kernel<true><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
     else attn_bwd_umma_kernel<false><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
     return cudaGetLastError();

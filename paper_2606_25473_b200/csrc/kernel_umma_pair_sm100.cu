@@ -623,6 +623,7 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
                     for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; if (tp) ((uint4 *)tp)[c] = z; }
                     if (prm.lse) prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = -INFINITY;
+                    if (prm.tlse) prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = 0.f;
                 }
                 continue;
             }
@@ -685,6 +686,9 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             }
             if (store && prm.lse)
                 prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = l > 0.f ? (m_ref + log2f(l)) * 0.6931471805599453f : -INFINITY;
+            // tangent of lse: sum_b p_ab tS_ab = r / l; a primal-only task has tS = 0 throughout
+            if (store && prm.tlse)
+                prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = primal ? 0.f : rl;
             tc_fence_before();
         }
     }
@@ -706,12 +710,8 @@ size_t umma_pair_smem_bytes() { return SMEM_TOTAL; }
 
 cudaError_t launch_umma_pair(const UmmaParams &prm, int num_pairs, cudaStream_t stream) {
     if (num_pairs <= 0) return cudaSuccess;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(attn_jvp_umma_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<uint64_t> configured{0};
+    if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_pair_kernel, (int)SMEM_TOTAL, configured)) return e;
     attn_jvp_umma_pair_kernel<<<2 * num_pairs, NTHREADS, SMEM_TOTAL, stream>>>(prm);
     return cudaGetLastError();
 }

@@ -387,6 +387,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
                     for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; ((uint4 *)tp)[c] = z; }
                     if (prm.lse) prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = -INFINITY;
+                    if (prm.tlse) prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = 0.f;
                 }
                 continue;
             }
@@ -426,6 +427,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             }
             if (store && prm.lse)
                 prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = l > 0.f ? (m_ref + log2f(l)) * 0.6931471805599453f : -INFINITY;
+            if (store && prm.tlse) prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = rl;   // r / l
             tc_fence_before();
             g += n;
         }
@@ -445,12 +447,8 @@ size_t umma_smem_bytes() { return SMEM_TOTAL; }
 
 cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(attn_jvp_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_TOTAL);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<uint64_t> configured{0};
+    if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel, (int)SMEM_TOTAL, configured)) return e;
     attn_jvp_umma_kernel<<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
     return cudaGetLastError();
 }

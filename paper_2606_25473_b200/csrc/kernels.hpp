@@ -3,9 +3,25 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "attn_jvp.h"
 
 namespace aj {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the (kernel, device) pair: `done` is one bit per device ordinal
+// of a kernel's launcher (ordinals >= 64 set the attribute on every launch).  Safe from several host threads.
+template <typename K>
+inline cudaError_t ensure_dynamic_smem(K *kernel, int bytes, std::atomic<uint64_t> &done) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const uint64_t bit = dev < 64 ? (1ull << dev) : 0ull;
+    if (bit && (done.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess && bit) done.fetch_or(bit, std::memory_order_release);
+    return e;
+}
 
 constexpr int SIMT_TILE_Q = 16;
 constexpr int SIMT_TILE_K = 32;
@@ -14,8 +30,10 @@ constexpr int UMMA_TILE_K = 64;   // B_c: keys per streamed tile
 constexpr int UMMA_PAIR_TILE_Q = 256;  // query rows per task of the CTA-pair kernel (UMMA M = 256 over two SMs)
 
 struct SimtParams {
-    aj_tensor q, k, v, tq, tk, tv, o, to;
+    aj_tensor q, k, v, tq, tk, tv, o, to;   // no_tangents: tq, tk, tv are never read; to.ptr may be NULL
     float *lse;
+    float *tlse;                            // [B, H, Nq] tangent of lse (r / l) or NULL
+    int32_t no_tangents;                    // AJ_TANGENT_NONE plans: plain masked attention, tO = 0, tlse = 0
     const aj_task *tasks;
     const int32_t *k_begin, *k_end;
     int32_t H, Nq;
@@ -62,6 +80,7 @@ struct UmmaParams {
     CUtensorMap tm_k, tm_tk, tm_v, tm_tv;  // box {64, 64, 1, 1} over [B, H, Nk, d], SWIZZLE_128B
     aj_tensor o, to;
     float *lse;
+    float *tlse;                // [B, H, Nq] tangent of lse (r / l) or NULL
     const aj_task *tasks;
     const int32_t *k_begin, *k_end;   // schedule entries: keys [k_begin[e], k_end[e]) ...
     const uint32_t *rows;             // ... seen by tile rows [rows[e] & 0xffff, rows[e] >> 16)

@@ -3,76 +3,182 @@
 PAPER.md:318: before attention every rank holds the sequence shard `[B, H, N/P, d]`; one all-to-all turns it into the
 head shard `[B, H/P, N, d]`; attention runs locally on full sequences (the mask descriptor is unchanged); a second
 all-to-all brings the outputs back.  PAPER.md:358-360: with the JVP the tangents ride along, so six tensors go in
-(Q, K, V, tQ, tK, tV) and two come out (O, tO).  Here the six (two) tensors are packed into ONE buffer and exchanged
-with ONE `all_to_all_single` per direction (NCCL over NVLink / NVSwitch on GPUs; gloo in the CPU tests).
+(Q, K, V, tQ, tK, tV) and two come out (O, tO).  The primal backward (PAPER.md:247, :945) sends dO in and dQ, dK, dV out;
+Q, K, V, O and lse stay head-sharded on the rank between the two calls.
 
-Only plumbing lives here (packing, the collective, unpacking): the attention itself is the `local_op` the caller
-passes, in production `local_attn_jvp(plan)` = the C-ABI call on this rank's `H/P` heads.
+How the exchange is organised here
+  * The rank's H/P heads are cut into `head_groups` groups.  Per group and direction ALL tensors travel in ONE
+    `all_to_all_single` (NCCL over NVLink / NVSwitch on GPUs; gloo in the CPU tests).
+  * The groups are pipelined: the collective of group g + 1 is issued (async) before the kernel of group g is enqueued, and
+    the outputs of group g go back while group g + 1 computes, so that the exchange hides under the kernel except for the
+    first group's way in and the last group's way out.
+  * Packing is one strided copy per tensor into the send buffer and one per tensor out of the receive buffer (no stacked
+    intermediate), with the index arithmetic in `pack_*` / `unpack_*` below -- the same functions the single-process
+    emulation of the tests drives, so that what the tests check is what production runs.
+
+Only plumbing lives here (packing, the collective, stream ordering): the attention itself is the `local_op` the caller
+passes, in production `local_attn_jvp(plan)` / `local_attn_bwd(plan)` = the C-ABI calls on one head group.
 """
 from __future__ import annotations
 
-from typing import Callable, Optional, Sequence, Tuple
+from typing import Callable, List, Optional, Sequence, Tuple
 
 import torch
 import torch.distributed as dist
 
 
-def _exchange(buf: torch.Tensor, group) -> torch.Tensor:
-    """buf [P, ...]: chunk j goes to rank j; returns [P, ...] with chunk i received from rank i."""
-    out = torch.empty_like(buf)
-    dist.all_to_all_single(out, buf, group=group)
-    return out
-
-
-def seq_to_head_shard(xs: Sequence[torch.Tensor], group=None) -> Tuple[torch.Tensor, ...]:
-    """T tensors `[B, H, N/P, d]` (this rank's tokens, all heads) -> T tensors `[B, H/P, N, d]` (all tokens, this rank's
-    heads), one collective.  Rank r owns tokens [r N/P, (r+1) N/P) and heads [r H/P, (r+1) H/P)."""
-    P = dist.get_world_size(group)
+# ---------------------------------------------------------------------------------------------- index arithmetic
+def pack_seq_shard(xs: Sequence[torch.Tensor], P: int, g: int, G: int) -> torch.Tensor:
+    """This rank's T tensors `[B, H, n, d]` (its n = N/P tokens, all H heads) -> the send buffer of head group g:
+    `[P, T, B, hg, n, d]`, chunk j = heads `[j H/P + g hg, j H/P + (g + 1) hg)` (rank j's group g), hg = H/(P G)."""
     B, H, n, d = xs[0].shape
-    if H % P:
-        raise ValueError(f"H = {H} is not divisible by the context-parallel size {P}")
-    T = len(xs)
-    # [T, B, P, H/P, n, d] -> [P, T, B, H/P, n, d]: chunk j = the heads of rank j
-    send = torch.stack(list(xs)).view(T, B, P, H // P, n, d).permute(2, 0, 1, 3, 4, 5).contiguous()
-    recv = _exchange(send, group)                       # chunk i = rank i's tokens of my heads
-    full = recv.permute(1, 2, 3, 0, 4, 5).reshape(T, B, H // P, P * n, d)
-    return tuple(full[t] for t in range(T))
+    if H % (P * G):
+        raise ValueError(f"H = {H} is not divisible by context-parallel size {P} x head groups {G}")
+    h, hg = H // P, H // (P * G)
+    send = xs[0].new_empty((P, len(xs), B, hg, n, d))
+    for t, x in enumerate(xs):
+        send[:, t].copy_(x.unflatten(1, (P, h))[:, :, g * hg:(g + 1) * hg].permute(1, 0, 2, 3, 4))
+    return send
 
 
-def head_to_seq_shard(ys: Sequence[torch.Tensor], group=None) -> Tuple[torch.Tensor, ...]:
-    """The inverse: T tensors `[B, H/P, N, d]` -> T tensors `[B, H, N/P, d]`, one collective."""
-    P = dist.get_world_size(group)
-    B, h, N, d = ys[0].shape
+def unpack_head_shard(recv: torch.Tensor) -> Tuple[torch.Tensor, ...]:
+    """The receive buffer `[P, T, B, hg, n, d]` (chunk i = rank i's tokens of my heads) -> T tensors `[B, hg, P n, d]`
+    (all tokens; rank i owns tokens `[i n, (i + 1) n)`)."""
+    P, T, B, hg, n, d = recv.shape
+    outs = []
+    for t in range(T):
+        full = recv.new_empty((B, hg, P * n, d))
+        full.view(B, hg, P, n, d).copy_(recv[:, t].permute(1, 2, 0, 3, 4))
+        outs.append(full)
+    return tuple(outs)
+
+
+def pack_head_shard(ys: Sequence[torch.Tensor], P: int) -> torch.Tensor:
+    """T tensors `[B, hg, N, d]` (all tokens of my heads) -> the send buffer `[P, T, B, hg, n, d]`, chunk j = rank j's tokens."""
+    B, hg, N, d = ys[0].shape
     if N % P:
         raise ValueError(f"N = {N} is not divisible by the context-parallel size {P}")
-    T = len(ys)
-    # [T, B, h, P, n, d] -> [P, T, B, h, n, d]: chunk j = the tokens of rank j
-    send = torch.stack(list(ys)).view(T, B, h, P, N // P, d).permute(3, 0, 1, 2, 4, 5).contiguous()
-    recv = _exchange(send, group)                       # chunk i = my tokens of rank i's heads
-    local = recv.permute(1, 2, 0, 3, 4, 5).reshape(T, B, P * h, N // P, d)
-    return tuple(local[t] for t in range(T))
+    n = N // P
+    send = ys[0].new_empty((P, len(ys), B, hg, n, d))
+    for t, y in enumerate(ys):
+        send[:, t].copy_(y.unflatten(2, (P, n)).permute(2, 0, 1, 3, 4))
+    return send
 
 
-LocalOp = Callable[[torch.Tensor, torch.Tensor, torch.Tensor, torch.Tensor, torch.Tensor, torch.Tensor],
-                   Tuple[torch.Tensor, torch.Tensor, Optional[torch.Tensor]]]
+def unpack_seq_shard(recv: torch.Tensor, outs: Sequence[torch.Tensor], g: int, G: int) -> None:
+    """The receive buffer `[P, T, B, hg, n, d]` (chunk i = my tokens of rank i's head group g) -> written into head group g
+    of the T output tensors `[B, H, n, d]`."""
+    P, T, B, hg, n, d = recv.shape
+    h = hg * G
+    for t, out in enumerate(outs):
+        out.unflatten(1, (P, h))[:, :, g * hg:(g + 1) * hg].copy_(recv[:, t].permute(1, 0, 2, 3, 4))
 
 
-def ulysses_attn_jvp(local_op: LocalOp, q, k, v, tq, tk, tv, group=None):
-    """q, k, v, tq, tk, tv: this rank's `[B, H, N/P, d]` shards.  -> (o, to) `[B, H, N/P, d]`, lse `[B, H/P, N]` or None
-    (lse stays head-sharded: it is consumed by the primal backward on the same rank)."""
-    hq, hk, hv, htq, htk, htv = seq_to_head_shard((q, k, v, tq, tk, tv), group)
-    o, to, lse = local_op(hq, hk, hv, htq, htk, htv)
-    o_l, to_l = head_to_seq_shard((o, to), group)
-    return o_l, to_l, lse
+# ---------------------------------------------------------------------------------------------- the collective
+class _Done:
+    def wait(self):
+        return True
 
 
+def _exchange(send: torch.Tensor, group, async_op: bool):
+    """send [P, ...]: chunk j goes to rank j.  -> (recv [P, ...] with chunk i from rank i, work handle)."""
+    recv = torch.empty_like(send)
+    work = dist.all_to_all_single(recv, send, group=group, async_op=async_op)
+    return recv, (work if async_op and work is not None else _Done())
+
+
+LocalOp = Callable[..., Tuple[torch.Tensor, ...]]
+
+
+def _pipeline(ins: Sequence[torch.Tensor], n_out: int, local_op: LocalOp, group, head_groups: int, out_like: Sequence[int]):
+    """Shared by the forward and the backward: `ins` = this rank's `[B, H, n, d]` tensors; per head group: exchange in,
+    `local_op(g, *head_sharded_inputs)` -> n_out head-sharded `[B, hg, N, d]` tensors (+ anything it wants to keep, which
+    is returned per group), exchange out.  out_like[i] = index of the input whose shape output i has.
+    -> (outs `[B, H, n, d]`, [extras of group g])."""
+    P = dist.get_world_size(group)
+    G = head_groups
+    outs = [torch.empty(ins[i].shape, dtype=ins[i].dtype, device=ins[i].device) for i in out_like]
+    extras: List = [None] * G
+    recv_in, work_in = _exchange(pack_seq_shard(ins, P, 0, G), group, True)
+    pending_out = None                                    # (recv, work, g) of the previous group's way back
+    for g in range(G):
+        nxt = _exchange(pack_seq_shard(ins, P, g + 1, G), group, True) if g + 1 < G else None   # in flight under kernel g
+        work_in.wait()
+        res = local_op(g, *unpack_head_shard(recv_in))
+        extras[g] = res[n_out:]
+        back = _exchange(pack_head_shard(res[:n_out], P), group, True)                            # in flight under kernel g + 1
+        if pending_out is not None:
+            pending_out[1].wait()
+            unpack_seq_shard(pending_out[0], outs, pending_out[2], G)
+        pending_out = (back[0], back[1], g)
+        if nxt is not None:
+            recv_in, work_in = nxt
+    pending_out[1].wait()
+    unpack_seq_shard(pending_out[0], outs, pending_out[2], G)
+    return outs, extras
+
+
+def ulysses_attn_jvp(local_op: LocalOp, q, k, v, tq, tk, tv, group=None, head_groups: int = 1):
+    """q, k, v, tq, tk, tv: this rank's `[B, H, N/P, d]` shards.  local_op(g, q, k, v, tq, tk, tv) -> (o, to, lse) on the
+    head shard of group g.  -> (o, to) `[B, H, N/P, d]`, and `saved` = per head group (q, k, v, o, lse) head-sharded, which
+    is what the primal backward on this rank consumes (lse never leaves the rank)."""
+    def op(g, hq, hk, hv, htq, htk, htv):
+        o, to, lse = local_op(g, hq, hk, hv, htq, htk, htv)
+        return o, to, (hq, hk, hv, o, lse)
+    (o_l, to_l), extras = _pipeline((q, k, v, tq, tk, tv), 2, op, group, head_groups, (0, 0))
+    return o_l, to_l, [e[0] for e in extras]
+
+
+def ulysses_attn_bwd(local_bwd: LocalOp, saved, dout, group=None, head_groups: int = 1):
+    """dout: this rank's `[B, H, N/P, d]` shard of dO; `saved` from ulysses_attn_jvp (same head_groups).
+    local_bwd(g, q, k, v, o, lse, dout) -> (dq, dk, dv) on the head shard.  -> dq, dk, dv `[B, H, N/P, d]`."""
+    def op(g, hdo):
+        hq, hk, hv, o, lse = saved[g]
+        return local_bwd(g, hq, hk, hv, o, lse, hdo)
+    (dq, dk, dv), _ = _pipeline((dout,), 3, op, group, head_groups, (0, 0, 0))
+    return dq, dk, dv
+
+
+# ---------------------------------------------------------------------------------------------- production local ops
 def local_attn_jvp(plan, stream: int = 0) -> LocalOp:
-    """The production local op: `attn_jvp_fwd` of a plan created for (B, H/P heads, N, N) on this rank's GPU."""
+    """`attn_jvp_fwd` of a plan created for (B, H / (P G) heads, N, N) on this rank's GPU; every head group reuses it."""
     from . import binding as aj
 
-    def op(q, k, v, tq, tk, tv):
+    def op(g, q, k, v, tq, tk, tv):
         o, to = torch.empty_like(q), torch.empty_like(q)
         lse = torch.empty(q.shape[:3], dtype=torch.float32, device=q.device)
         aj.attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse, stream)
         return o, to, lse
     return op
+
+
+def local_attn_bwd(plan, stream: int = 0) -> LocalOp:
+    """`attn_bwd` of the same plan."""
+    from . import binding as aj
+
+    def op(g, q, k, v, o, lse, dout):
+        dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(k)
+        aj.attn_bwd(plan, q, k, v, o, lse, dout, dq, dk, dv, stream)
+        return dq, dk, dv
+    return op
+
+
+# ---------------------------------------------------------------------------------------------- single-process emulation
+def emulate_ranks(P: int, shards: Sequence[Sequence[torch.Tensor]], n_out: int, local_op: LocalOp, head_groups: int = 1,
+                  out_like: Optional[Sequence[int]] = None):
+    """P virtual ranks in ONE process (tests; one GPU): shards[r] = rank r's `[B, H, n, d]` tensors.  Runs the same
+    pack / unpack functions as `_pipeline`, with the all-to-all replaced by its definition (recv_r[i] = send_i[r]).
+    -> outs[r] = rank r's n_out output shards."""
+    G = head_groups
+    out_like = out_like or [0] * n_out
+    outs = [[torch.empty(shards[r][i].shape, dtype=shards[r][i].dtype, device=shards[r][i].device) for i in out_like] for r in range(P)]
+    for g in range(G):
+        sends = [pack_seq_shard(shards[r], P, g, G) for r in range(P)]
+        backs = []
+        for r in range(P):
+            recv = torch.stack([sends[i][r] for i in range(P)])
+            res = local_op(r, g, *unpack_head_shard(recv))
+            backs.append(pack_head_shard(res[:n_out], P))
+        for r in range(P):
+            unpack_seq_shard(torch.stack([backs[i][r] for i in range(P)]), outs[r], g, G)
+    return outs

@@ -87,29 +87,46 @@ def compare(w: Workload, gpu, ref, tol=None):
     return errs
 
 
-def sample_rows(w: Workload, per_head_groups: int = 4, random_per_group: int = 2, tile_q: int = 128):
-    """Deterministic row subset for full-size configs: for every (b, h) a rotating choice of query groups
-    (every group is hit by some head), and inside each group its first and last row, the rows on both sides
-    of the first and the last query-tile boundary, and seeded random rows."""
+def query_groups(w: Workload):
+    """The mask's query groups as [(q_begin, q_end)] from the block structure (test-side accounting)."""
     C, n = w.block_len, w.num_blocks
     if w.mask == "full":
-        groups = [(0, w.num_queries)]
-    elif w.mask == "block_causal":
-        groups = [(i * C, (i + 1) * C) for i in range(n)]
-    else:
-        groups = [(i * C, (i + 1) * C) for i in range(2 * n)]
-    rng = np.random.default_rng(1234)
+        return [(0, w.num_queries)]
+    if w.mask == "block_causal":
+        return [(i * C, (i + 1) * C) for i in range(n)]
+    return [(i * C, (i + 1) * C) for i in range(2 * n)]
+
+
+def sample_rows(w: Workload, random_per_group: int = 16, max_boundaries: int = 64, heads=None, seed: int = 1234):
+    """SURVEY.md 8(c) "GPU-vs-oracle protocol" for the full-size configs: for EVERY (b, h) (or those in `heads`) and EVERY
+    query group -- its first and last row, the rows on both sides of every query-tile boundary that falls inside it (the
+    global 256- and 128-row grids of the packed tilings and the group-relative 128-row grid of per-group tiling; at most
+    `max_boundaries` of them per group and grid, seeded choice, when a group holds more), and `random_per_group` seeded
+    random rows.  -> {(b, h): sorted unique int64 rows}.  Asserts that every group is hit on every head."""
+    groups = query_groups(w)
     out = {}
-    idx = 0
     for b in range(w.B):
         for h in range(w.H):
-            rows = []
-            for j in range(min(per_head_groups, len(groups))):
-                q0, q1 = groups[(idx + j * max(1, len(groups) // per_head_groups)) % len(groups)]
-                last_tile = q0 + ((q1 - q0 - 1) // tile_q) * tile_q
-                cand = [q0, q1 - 1, q0 + tile_q - 1, q0 + tile_q, last_tile - 1, last_tile]
-                cand += list(rng.integers(q0, q1, size=random_per_group))
-                rows += [int(r) for r in cand if q0 <= r < q1]
+            if heads is not None and (b, h) not in heads:
+                continue
+            rng = np.random.default_rng([seed, b, h])
+            rows, hit = [], set()
+            for g, (q0, q1) in enumerate(groups):
+                cand = [q0, q1 - 1]
+                for grid, origin in ((256, 0), (128, 0), (128, q0)):
+                    first = origin + ((q0 - origin) // grid + 1) * grid
+                    bnd = np.arange(first, q1, grid)
+                    if len(bnd) > max_boundaries:
+                        bnd = rng.choice(bnd, size=max_boundaries, replace=False)
+                    for t in bnd:
+                        cand += [int(t) - 1, int(t)]
+                # at least `random_per_group` random rows, and enough of them that about 2 % of a large group is compared
+                n_rand = max(random_per_group, min(1024, int(0.02 * (q1 - q0)) - len(cand)))
+                cand += [int(r) for r in rng.integers(q0, q1, size=n_rand)]
+                cand = [r for r in cand if q0 <= r < q1]
+                assert len(cand) >= min(random_per_group, q1 - q0)
+                rows += cand
+                hit.add(g)
+            assert hit == set(range(len(groups))), "every query group must be sampled on every head"
             out[(b, h)] = np.unique(np.asarray(rows, dtype=np.int64))
-            idx += 1
     return out

@@ -198,24 +198,126 @@ def test_backward_strided_views_and_argument_errors():
     aj.attn_jvp_plan_destroy(plan)
 
 
-def test_backward_full_size_config2_one_head_sampled():
-    """BASELINE.json configs[1] shape (H = 1 to keep the fp32 backward and the oracle to seconds): sampled query rows
-    and keys of every block, against the oracle (whose pass over all rows supplies lse and delta)."""
-    base = WORKLOADS["wan13b_tf_framewise"]
-    w = Workload("wan13b_tf_framewise_H1", 1, 1, base.d, base.mask, base.frame_len, base.num_frames, base.chunk_frames,
-                 base.dtype, base.tangent_std, base.seed)
+# ---------------------------------------------------------------------------------------- full size (what bench.py times)
+FULL_SIZE_BACKWARD = ["wan13b_tf_framewise_bwd"]            # EXTRA_WORKLOADS whose step is attn_bwd
+
+
+def _block_samples(w, rng, per_block=6):
+    """first, last, both sides of the 128- / 256-row tile boundaries next to the block's ends, and random tokens of every block"""
+    C, n = w.block_len, w.num_blocks
+    idx = []
+    for blk in range(2 * n if w.mask == "teacher_forcing" else n):
+        q0, q1 = blk * C, (blk + 1) * C
+        first256, last256 = (q0 // 256 + 1) * 256, ((q1 - 1) // 256) * 256
+        cand = [q0, q1 - 1, first256 - 1, first256, last256 - 1, last256, q0 + 127, q0 + 128]
+        cand += list(rng.integers(q0, q1, size=per_block))
+        idx += [int(r) for r in cand if q0 <= r < q1]
+    return np.unique(np.asarray(idx, dtype=np.int64))
+
+
+@pytest.mark.parametrize("name", FULL_SIZE_BACKWARD)
+def test_backward_full_size_all_heads_launch_sampled(name):
+    """The launch bench.py times for the backward workload: all H = 12 heads in one attn_bwd call (host-assigned head-major
+    task lists), compared on three heads -- the first, a middle one and the LAST one the lists schedule -- at sampled query
+    rows and keys of every block (the oracle's pass over all rows of a head supplies lse and delta)."""
+    from paper_2606_25473_b200.workloads import EXTRA_WORKLOADS
+    w = EXTRA_WORKLOADS[name]
+    assert w.backward and w.H == 12
     x = make_inputs(w)
     dout = _dout(w)
     got = run_fwd_bwd(w, x, dout)
-    rng = np.random.default_rng(5)
-    C, n = w.block_len, w.num_blocks
-    idx = []
-    for blk in range(2 * n):                                  # first, last and two random tokens of every block
-        idx += [blk * C, (blk + 1) * C - 1] + list(rng.integers(blk * C, (blk + 1) * C, size=2))
-    idx = np.unique(np.asarray(idx, dtype=np.int64))
-    errs = check(w, x, dout, got, rows=idx, keys=idx)
-    print(f"{w.name}: {len(idx)} rows/keys, errs={errs}")
     for t in got:
         assert torch.isfinite(t.float()).all()
-    half = w.N // 2
+    heads = [(0, 0), (0, 5), (0, w.H - 1)]
+    for i, bh in enumerate(heads):
+        idx = _block_samples(w, np.random.default_rng(50 + i))
+        errs = check(w, x, dout, got, heads=[bh], rows=idx, keys=idx)
+        print(f"{w.name} head {bh}: {len(idx)} rows and keys, errs={errs}")
+    half, C, n = w.N // 2, w.block_len, w.num_blocks
     assert torch.count_nonzero(got[1][:, :, half + (n - 1) * C:]) > 0      # the last noisy block's keys are seen by itself
+
+
+def test_backward_config2_one_full_head_every_element():
+    """One full head of config 2 through the 12-head launch: every row of dQ and every key of dK, dV of head (0, 11)."""
+    from paper_2606_25473_b200.workloads import EXTRA_WORKLOADS
+    w = EXTRA_WORKLOADS["wan13b_tf_framewise_bwd"]
+    x = make_inputs(w)
+    dout = _dout(w)
+    got = run_fwd_bwd(w, x, dout)
+    errs = check(w, x, dout, got, heads=[(0, w.H - 1)])
+    print(f"{w.name} head (0, {w.H - 1}), every element: {errs}")
+
+
+@pytest.mark.parametrize("w", [SMALL[4], SMALL[0]], ids=lambda w: w.name)
+def test_bwd_host_matches_device_path(w):
+    # attn_bwd_host: per-head copies and launches on three streams; same bits as the one-launch device path
+    x = make_inputs(w, pin=True)
+    dout = _dout(w).pin_memory()
+    plan = make_plan(w)
+    q, k, v, tq, tk, tv = [t.cuda() for t in x]
+    o, to = torch.empty_like(q), torch.empty_like(q)
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    aj.attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse, 0)
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(k)
+    aj.attn_bwd(plan, q, k, v, o, lse, dout.cuda(), dq, dk, dv, 0)
+    torch.cuda.synchronize()
+    h_o, h_lse = o.cpu().pin_memory(), lse.cpu().pin_memory()
+    h = [torch.full_like(x[0], float("nan")).pin_memory(), torch.full_like(x[1], float("nan")).pin_memory(),
+         torch.full_like(x[1], float("nan")).pin_memory()]
+    for _ in range(2):                                  # the second call reuses staging buffers, schedules and tensor maps
+        aj.attn_bwd_host(plan, x[0], x[1], x[2], h_o, h_lse, dout, *h, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for a, b in zip(h, (dq, dk, dv)):
+            assert torch.equal(a, b.cpu())
+        for t in h:
+            t.fill_(float("nan"))
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+
+
+def test_forward_and_backward_replay_from_a_cuda_graph():
+    """SURVEY.md 8(b) "no hidden stream sync" / PAPER.md:534 (CUDA Graphs): after one eager call (attn_bwd builds its
+    schedules on first use) attn_jvp_fwd + attn_bwd are captured into a graph; two replays on fresh inputs give the bits of
+    the eager calls; the plan's tensor-map cache encodes nothing in steady state."""
+    w = SMALL[4]
+    x = make_inputs(w)
+    dout = _dout(w)
+    plan = make_plan(w)
+    q, k, v, tq, tk, tv = [t.cuda() for t in x]
+    dO = dout.cuda()
+    o, to = torch.empty_like(q), torch.empty_like(q)
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(k)
+    side = torch.cuda.Stream()
+
+    def step(stream):
+        aj.attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse, stream)
+        aj.attn_bwd(plan, q, k, v, o, lse, dO, dq, dk, dv, stream)
+
+    with torch.cuda.stream(side):
+        step(side.cuda_stream)
+    side.synchronize()
+    eager = [t.clone() for t in (o, to, lse, dq, dk, dv)]
+    enc0, hits0 = aj.attn_jvp_plan_tensor_map_stats(plan)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        step(side.cuda_stream)
+    enc1, hits1 = aj.attn_jvp_plan_tensor_map_stats(plan)
+    assert enc1 == enc0 and hits1 == hits0 + 14          # 6 forward + 8 backward maps, all from the plan's cache
+    for _ in range(2):
+        for t in (o, to, lse, dq, dk, dv):
+            t.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        for a, b in zip((o, to, lse, dq, dk, dv), eager):
+            assert torch.equal(a, b)
+    # new data in the same buffers: the replay follows it
+    q.copy_((x[0].float() * 0.5).to(q.dtype))
+    graph.replay()
+    torch.cuda.synchronize()
+    ref = [t.clone() for t in (o, dq)]
+    step(0)
+    torch.cuda.synchronize()
+    assert torch.equal(ref[0], o) and torch.equal(ref[1], dq)
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)

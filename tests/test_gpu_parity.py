@@ -10,7 +10,7 @@ import torch
 
 import oracle
 from gpu_common import TOL, compare, make_plan, run_gpu, run_oracle, sample_rows
-from helpers import widen, max_norm_err
+from helpers import oracle_mask, widen, max_norm_err
 from paper_2606_25473_b200 import binding as aj
 from paper_2606_25473_b200 import build as aj_build
 from paper_2606_25473_b200.workloads import WORKLOADS, Workload, make_inputs, scaled_down
@@ -261,6 +261,72 @@ def test_fwd_host_matches_device_path(w):
     aj.attn_jvp_plan_destroy(plan)
 
 
+def test_broadcast_heads_zero_stride():
+    """A K/V shared by all heads (`expand` over H: stride_h = 0).  The SIMT kernels honour it; the tcgen05 kernels cannot
+    express it in a TMA tensor map and say so (AJ_ERR_UNSUPPORTED) instead of reading heads 16 bytes apart; an output with
+    aliased heads is always an error."""
+    w = Workload("bcast", 1, 3, 128, "block_causal", 80, 3, 1, "bf16", 0.1, seed=8)
+    x = make_inputs(w)
+    for i in (1, 2, 4, 5):
+        x[i] = x[i][:, :1].expand(-1, w.H, -1, -1)             # every head sees head 0's K, V, tK, tV
+    dev = [t.cuda() for t in x]
+    dev = [dev[0], dev[1][:, :1].expand(-1, w.H, -1, -1), dev[2][:, :1].expand(-1, w.H, -1, -1), dev[3],
+           dev[4][:, :1].expand(-1, w.H, -1, -1), dev[5][:, :1].expand(-1, w.H, -1, -1)]
+    assert dev[1].stride(1) == 0
+    o, to = torch.full_like(dev[0], float("nan")), torch.full_like(dev[0], float("nan"))
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    plan = make_plan(w)
+    with pytest.raises(aj.AttnJvpError) as e:
+        aj.attn_jvp_fwd(plan, *dev, o, to, lse, 0)
+    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_SIMT)
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, 0)
+    torch.cuda.synchronize()
+    compare(w, (o.cpu(), to.cpu(), lse.cpu()), run_oracle(w, [t.contiguous() for t in x]))
+    with pytest.raises(aj.AttnJvpError) as e:                      # aliased output heads
+        aj.attn_jvp_fwd(plan, *dev, o[:, :1].expand(-1, w.H, -1, -1), to, lse, 0)
+    assert e.value.status == aj.AJ_ERR_INVALID_ARG
+    aj.attn_jvp_plan_destroy(plan)
+
+
+def test_binding_rejects_tensors_that_do_not_match_the_plan():
+    w = SMALL_UMMA[4]
+    plan = make_plan(w)
+    dev = [t.cuda() for t in make_inputs(w)]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    with pytest.raises(ValueError):                                # wrong N
+        aj.attn_jvp_fwd(plan, dev[0][:, :, :-8], *dev[1:], o, to, lse, 0)
+    with pytest.raises(ValueError):                                # wrong dtype
+        aj.attn_jvp_fwd(plan, dev[0].float(), *dev[1:], o, to, lse, 0)
+    with pytest.raises(ValueError):                                # host tensor on the device call
+        aj.attn_jvp_fwd(plan, dev[0].cpu(), *dev[1:], o, to, lse, 0)
+    with pytest.raises(ValueError):                                # lse of the wrong dtype
+        aj.attn_jvp_fwd(plan, *dev, o, to, lse.double(), 0)
+    with pytest.raises(ValueError):                                # lse too short
+        aj.attn_jvp_fwd(plan, *dev, o, to, lse[:, :, :-1].contiguous(), 0)
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, 0)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+
+
+def test_tensor_maps_are_cached_by_the_plan():
+    w = SMALL_UMMA[0]
+    plan = make_plan(w)
+    dev = [t.cuda() for t in make_inputs(w)]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    assert aj.attn_jvp_plan_tensor_map_stats(plan) == (0, 0)
+    aj.attn_jvp_fwd(plan, *dev, o, to, None, 0)
+    assert aj.attn_jvp_plan_tensor_map_stats(plan) == (6, 0)
+    aj.attn_jvp_fwd(plan, *dev, o, to, None, 0)
+    assert aj.attn_jvp_plan_tensor_map_stats(plan) == (6, 6)
+    q2 = dev[0].clone()                                             # one argument moves: one map is re-encoded
+    aj.attn_jvp_fwd(plan, q2, *dev[1:], o, to, None, 0)
+    assert aj.attn_jvp_plan_tensor_map_stats(plan) == (7, 11)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+
+
 def test_fwd_argument_errors():
     w = SMALL_UMMA[4]
     plan = make_plan(w)
@@ -271,7 +337,7 @@ def test_fwd_argument_errors():
         aj.attn_jvp_fwd(plan, bad, *dev[1:], o, to, None, 0)
     assert e.value.status == aj.AJ_ERR_INVALID_ARG
     with pytest.raises(aj.AttnJvpError) as e:                      # stride_n < d
-        aj.attn_jvp_fwd(plan, dev[0].as_strided(dev[0].shape, (0, 0, 64, 1)), *dev[1:], o, to, None, 0)
+        aj.attn_jvp_fwd(plan, dev[0].as_strided(dev[0].shape, (w.N * 64, w.N * 64, 64, 1)), *dev[1:], o, to, None, 0)
     assert e.value.status == aj.AJ_ERR_INVALID_ARG
     assert aj.lib().attn_jvp_fwd(plan, None, None, None, None, None, None, None, None, None, None) == aj.AJ_ERR_INVALID_ARG
     with pytest.raises(aj.AttnJvpError) as e:                      # the tcgen05 kernel does not cover fp32
@@ -292,6 +358,8 @@ FULL = ["wan13b_tf_framewise", "wan13b_tf_chunkwise", "block_causal_b2", "dit_la
 @pytest.mark.parametrize("name,kernel", [(n, aj.AJ_KERNEL_AUTO) for n in FULL] + [("wan13b_tf_framewise", aj.AJ_KERNEL_UMMA)],
                          ids=lambda v: v if isinstance(v, str) else {0: "default", 2: "single"}[v])
 def test_full_size_config_sampled_rows(name, kernel):
+    """The launch configuration bench.py times, against the oracle on the SURVEY.md 8(c) row protocol: every head, every
+    query group (first / last row, both sides of every tile boundary, 16 random rows)."""
     w = WORKLOADS[name]
     x = make_inputs(w)
     plan = make_plan(w, kernel)
@@ -300,34 +368,153 @@ def test_full_size_config_sampled_rows(name, kernel):
     assert pairs == w.unmasked_pairs_per_head
     gpu = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_destroy(plan)
-    per_head = 2 if w.N > 100000 else 3
-    rows = sample_rows(w, per_head_groups=per_head, random_per_group=2, tile_q=256 if kernel == aj.AJ_KERNEL_AUTO else 128)
+    rows = sample_rows(w)
+    assert set(rows) == {(b, h) for b in range(w.B) for h in range(w.H)}
     errs = compare(w, gpu, run_oracle(w, x, rows))
-    print(f"{name}: rows/head={len(next(iter(rows.values())))} errs={errs}")
-    # properties that hold at any size: every output written and finite, lse within [min s, max s + ln N]
+    nrows = sum(len(r) for r in rows.values())
+    print(f"{name}: {nrows} rows = {100.0 * nrows / (w.B * w.H * w.num_queries):.2f} % of all rows, errs={errs}")
+    # properties that hold at any size: every output written and finite
     for t in gpu:
         assert torch.isfinite(t.float()).all()
 
 
-# ---------------------------------------------------------------------------------------- Ulysses wrapper on one GPU
-def test_ulysses_wrapper_with_the_cuda_local_op_world_size_1():
-    """The N4 plumbing with the production local op (NCCL, one rank = one GPU: the exchanges are identities here; the
-    multi-rank layout is covered by the gloo test): same bits as the direct call."""
+def test_config2_one_full_head_every_row():
+    """one full head of config 2 -- all 65,520 rows of head (0, 5) of the 12-head launch bench.py times,
+    O, tO, lse and the lse tangent, element by element."""
+    w = WORKLOADS["wan13b_tf_framewise"]
+    x = make_inputs(w)
+    plan = make_plan(w)
+    dev = [t.cuda() for t in x]
+    o, to = torch.full_like(dev[0], float("nan")), torch.full_like(dev[0], float("nan"))
+    lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")
+    tlse = torch.full_like(lse, float("nan"))
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, torch.cuda.current_stream().cuda_stream, tlse=tlse)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    h = 5
+    ro, rto, rlse, rtl = oracle.attn_jvp_head(oracle.teacher_forcing_mask(w.block_len, w.num_blocks),
+                                              *[widen(t[0, h]) for t in x], 1.0 / np.sqrt(w.d), with_tlse=True)
+    errs = dict(o=max_norm_err(o[0, h].cpu().double().numpy(), ro), to=max_norm_err(to[0, h].cpu().double().numpy(), rto),
+                lse=max_norm_err(lse[0, h].cpu().double().numpy(), rlse), tlse=max_norm_err(tlse[0, h].cpu().double().numpy(), rtl))
+    print(f"config 2, head {h}, all {w.N} rows: {errs}")
+    assert errs["o"] <= 1e-2 and errs["to"] <= 1e-2 and errs["lse"] <= 1e-3 and errs["tlse"] <= 1e-2, errs
+
+
+# ---------------------------------------------------------------------------------------- the lse tangent (attn_jvp_fwd_tl)
+@pytest.mark.parametrize("kernel", [aj.AJ_KERNEL_UMMA_PAIR, aj.AJ_KERNEL_UMMA, aj.AJ_KERNEL_SIMT], ids=["pair", "single", "simt"])
+@pytest.mark.parametrize("w", [SMALL_UMMA[0], SMALL_UMMA[2], SMALL_UMMA[3]], ids=lambda w: w.name)
+def test_lse_tangent_every_row(w, kernel):
+    # tlse = sum_b p_ab tS_ab = r / l (PAPER.md:870-876), unit-variance tangents so that it is not small
+    w = Workload(w.name, w.B, w.H, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, 1.0, w.seed)
+    x = make_inputs(w)
+    plan = make_plan(w, kernel)
+    dev = [t.cuda() for t in x]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    tlse = torch.full_like(lse, float("nan"))
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, 0, tlse=tlse)
+    o2, to2, lse2 = torch.empty_like(o), torch.empty_like(o), torch.empty_like(lse)
+    aj.attn_jvp_fwd(plan, *dev, o2, to2, lse2, 0)                   # without tlse: the same bits everywhere else
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+    assert torch.equal(o, o2) and torch.equal(to, to2) and torch.equal(lse, lse2)
+    om = oracle_mask(w)
+    got, want = [], []
+    for b in range(w.B):
+        for h in range(w.H):
+            want.append(oracle.attn_jvp_head(om, *[widen(t[b, h]) for t in x], 1.0 / np.sqrt(w.d), with_tlse=True)[3])
+            got.append(tlse[b, h].cpu().double().numpy())
+    err = max_norm_err(np.concatenate(got), np.concatenate(want))
+    assert err <= (1e-2 if w.dtype == "bf16" else 1e-4), err
+
+
+def test_lse_tangent_is_zero_where_tangents_are_structurally_zero():
+    w = Workload("tl_cleanzero", 1, 2, 128, "teacher_forcing", 300, 3, 1, "bf16", 1.0, 3, True)
+    x = make_inputs(w)
+    plan = make_plan(w)                                             # AJ_TANGENT_CLEAN_ZERO from the workload
+    dev = [t.cuda() for t in x]
+    o, to = torch.empty_like(dev[0]), torch.empty_like(dev[0])
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+    tlse = torch.full_like(lse, float("nan"))
+    aj.attn_jvp_fwd(plan, *dev, o, to, lse, 0, tlse=tlse)
+    torch.cuda.synchronize()
+    aj.attn_jvp_plan_destroy(plan)
+    assert torch.count_nonzero(tlse[:, :, :w.N // 2]) == 0          # clean rows: primal-only tasks
+    om = oracle_mask(w)
+    for h in range(w.H):
+        rtl = oracle.attn_jvp_head(om, *[widen(t[0, h]) for t in x], 1.0 / np.sqrt(w.d), with_tlse=True)[3]
+        assert max_norm_err(tlse[0, h].cpu().double().numpy(), rtl) <= 1e-2
+
+
+# ---------------------------------------------------------------------------------------- Ulysses (SURVEY.md 8(f) N4)
+@pytest.mark.parametrize("P,G", [(2, 1), (2, 2), (4, 1)])
+def test_ulysses_sequence_shards_with_the_cuda_local_op_against_the_oracle(P, G):
+    """P virtual ranks in one process, each holding the token shard [B, H, N/P, d]: the production pack / unpack index
+    arithmetic with the all-to-all replaced by its definition, the CUDA call as the local op on every head shard (forward
+    + JVP, then the primal backward), and the reassembled result against the UNDISTRIBUTED oracle."""
+    from paper_2606_25473_b200 import ulysses
+    w = Workload("uly_tf", 1, 4, 128, "teacher_forcing", 120, 2, 1, "bf16", 0.1, seed=21)      # N = 480, H = 4
+    x = make_inputs(w)
+    g = torch.Generator().manual_seed(22)
+    dout = torch.randn(x[0].shape, generator=g).to(torch.bfloat16)
+    hg = w.H // (P * G)
+    wl = Workload("uly_local", w.B, hg, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std)
+    plan = make_plan(wl)                                       # one plan for every head group: (B, H / (P G) heads, N, N)
+    fwd, bwd = ulysses.local_attn_jvp(plan), ulysses.local_attn_bwd(plan)
+    n = w.N // P
+    dev = [t.cuda() for t in x] + [dout.cuda()]
+    shards = [[t[:, :, r * n:(r + 1) * n].contiguous() for t in dev] for r in range(P)]
+    saved = {}
+
+    def fwd_op(r, grp, q, k, v, tq, tk, tv):
+        o, to, lse = fwd(grp, q, k, v, tq, tk, tv)
+        saved[(r, grp)] = (q, k, v, o, lse)
+        return o, to
+
+    outs = ulysses.emulate_ranks(P, [s[:6] for s in shards], 2, fwd_op, G)
+    grads = ulysses.emulate_ranks(P, [s[6:] for s in shards], 3, lambda r, grp, do: bwd(grp, *saved[(r, grp)], do), G)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    o = torch.cat([outs[r][0] for r in range(P)], dim=2).cpu()
+    to = torch.cat([outs[r][1] for r in range(P)], dim=2).cpu()
+    lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32)
+    h = w.H // P
+    for (r, grp), sv in saved.items():
+        lse[:, r * h + grp * hg:r * h + (grp + 1) * hg] = sv[4].cpu()
+    compare(w, (o, to, lse), run_oracle(w, x))
+    om = oracle_mask(w)
+    for i, name in enumerate(("dq", "dk", "dv")):
+        got = torch.cat([grads[r][i] for r in range(P)], dim=2).cpu()
+        for hh in range(w.H):
+            ref = oracle.attn_bwd_head(om, widen(x[0][0, hh]), widen(x[1][0, hh]), widen(x[2][0, hh]), widen(dout[0, hh]),
+                                       1.0 / np.sqrt(w.d))[i]
+            assert max_norm_err(got[0, hh].double().numpy(), ref) <= 1e-2, (name, hh)
+
+
+def test_ulysses_pipeline_with_nccl_world_size_1():
+    """The production pipeline (async all_to_all_single per head group on NCCL, here one rank = one GPU, so the exchanges
+    are identities): same bits as the direct call on all heads."""
     import torch.distributed as dist
     from paper_2606_25473_b200 import ulysses
     w = SMALL_UMMA[0]
     x = make_inputs(w)
     plan = make_plan(w)
     ref = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    wl = Workload("uly_local1", w.B, 1, w.d, w.mask, w.frame_len, w.num_frames, w.chunk_frames, w.dtype, w.tangent_std)
+    plan = make_plan(wl)
     own = not dist.is_initialized()
     if own:
         dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29517", rank=0, world_size=1)
     try:
-        o, to, lse = ulysses.ulysses_attn_jvp(ulysses.local_attn_jvp(plan, torch.cuda.current_stream().cuda_stream),
-                                              *[t.cuda() for t in x])
+        o, to, saved = ulysses.ulysses_attn_jvp(ulysses.local_attn_jvp(plan, torch.cuda.current_stream().cuda_stream),
+                                                *[t.cuda() for t in x], head_groups=w.H)
         torch.cuda.synchronize()
     finally:
         if own:
             dist.destroy_process_group()
     aj.attn_jvp_plan_destroy(plan)
+    lse = torch.cat([s[4] for s in saved], dim=1)
     assert torch.equal(o.cpu(), ref[0]) and torch.equal(to.cpu(), ref[1]) and torch.equal(lse.cpu(), ref[2])

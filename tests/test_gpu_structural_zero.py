@@ -179,27 +179,75 @@ def test_null_tangents_are_rejected_unless_the_plan_says_none():
     assert e.value.status == aj.AJ_ERR_INVALID_ARG
     aj.attn_jvp_plan_destroy(plan)
     plan = make_plan(w, tangent_zero=aj.AJ_TANGENT_NONE)
-    aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA)            # only the CTA-pair kernel runs without tangents
-    with pytest.raises(aj.AttnJvpError) as e:
-        aj.attn_fwd(plan, x[0], x[1], x[2], o, None, 0)
+    with pytest.raises(aj.AttnJvpError) as e:                      # the single-CTA tcgen05 kernel has no tangent-free mode
+        aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA)
     assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_UMMA_PAIR      # and the plan is unchanged
     aj.attn_jvp_plan_destroy(plan)
     torch.cuda.synchronize()
 
 
+@pytest.mark.parametrize("dtype,d", [("fp32", 64), ("fp32", 128), ("bf16", 64), ("bf16", 128)])
+def test_tangent_none_means_the_same_on_every_kernel(dtype, d):
+    """AJ_TANGENT_NONE plans: tq, tk, tv are never read (NULL or garbage alike), a non-NULL `to` is zero-filled, O and lse
+    are plain masked attention -- on the SIMT kernel (fp32, d = 64) as on the CTA-pair kernel; then attn_bwd on the
+    same plan (the non-JVP stages)."""
+    w = Workload(f"none_{dtype}_{d}", 1, 2, d, "block_causal", 70, 3, 1, dtype, 0.0, 17, False, True)
+    x = make_inputs(w)
+    plan = make_plan(w)
+    want = aj.AJ_KERNEL_UMMA_PAIR if (dtype == "bf16" and d == 128) else aj.AJ_KERNEL_SIMT
+    assert aj.attn_jvp_plan_kernel(plan)[0] == want
+    q, k, v = [t.cuda() for t in x[:3]]
+    junk = torch.full_like(q, float("nan"))
+    o1, o2, to2 = torch.empty_like(q), torch.empty_like(q), torch.full_like(q, float("nan"))
+    lse1, lse2 = [torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda") for _ in range(2)]
+    tl = torch.full_like(lse1, float("nan"))
+    aj.attn_fwd(plan, q, k, v, o1, lse1, 0)
+    aj.attn_jvp_fwd(plan, q, k, v, junk, junk, junk, o2, to2, lse2, 0, tlse=tl)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2) and torch.equal(lse1, lse2)
+    assert torch.count_nonzero(to2) == 0 and torch.count_nonzero(tl) == 0
+    om = oracle.block_causal_mask(w.block_len, w.num_blocks)
+    z = np.zeros((w.N, d), np.float32)
+    tol = 1e-2 if dtype == "bf16" else 1e-4
+    g = torch.Generator().manual_seed(5)
+    dout = torch.randn(q.shape, generator=g).to(q.dtype)
+    dq, dk, dv = [torch.full_like(q, float("nan")) for _ in range(3)]
+    aj.attn_bwd(plan, q, k, v, o1, lse1, dout.cuda(), dq, dk, dv, 0)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    for h in range(w.H):
+        ro, _, rlse = oracle.attn_jvp_head(om, widen(x[0][0, h]), widen(x[1][0, h]), widen(x[2][0, h]), z, z, z, 1.0 / np.sqrt(d))
+        assert max_norm_err(o1[0, h].cpu().double().numpy(), ro) <= tol
+        assert max_norm_err(lse1[0, h].cpu().double().numpy(), rlse) <= (1e-3 if dtype == "bf16" else 1e-4)
+        rq, rk, rv = oracle.attn_bwd_head(om, widen(x[0][0, h]), widen(x[1][0, h]), widen(x[2][0, h]), widen(dout[0, h]), 1.0 / np.sqrt(d))
+        for got, ref in ((dq, rq), (dk, rk), (dv, rv)):
+            assert max_norm_err(got[0, h].cpu().double().numpy(), ref) <= tol
+
+
 # ---------------------------------------------------------------------------------------- full size (what bench.py times)
-@pytest.mark.parametrize("name", list(EXTRA_WORKLOADS))
+FORWARD_EXTRAS = [n for n, w in EXTRA_WORKLOADS.items() if not w.backward]
+
+
+def test_backward_extras_are_covered_by_the_backward_tests():
+    # a workload whose step is attn_bwd is compared through attn_bwd (tests/test_gpu_backward.py), never through the forward
+    import test_gpu_backward
+    assert {n for n, w in EXTRA_WORKLOADS.items() if w.backward} == set(test_gpu_backward.FULL_SIZE_BACKWARD)
+
+
+@pytest.mark.parametrize("name", FORWARD_EXTRAS)
 def test_extra_workloads_full_size_sampled_rows(name):
+    """SURVEY.md 8(c) row protocol (every head, every query group) on the 8(f) forward workloads bench.py times."""
     w = EXTRA_WORKLOADS[name]
     x = make_inputs(w)
     plan = make_plan(w)
     gpu = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_destroy(plan)
-    rows = sample_rows(w, per_head_groups=3, random_per_group=2, tile_q=256)
-    if w.B * w.H > 24:                       # keep the oracle's share to seconds: every fourth (b, h)
-        rows = {bh: r for i, (bh, r) in enumerate(rows.items()) if i % 4 == 0}
+    rows = sample_rows(w)
     errs = compare(w, gpu, run_oracle(w, x, rows))
-    print(f"{name}: errs={errs}")
+    nrows = sum(len(r) for r in rows.values())
+    print(f"{name}: {nrows} rows = {100.0 * nrows / (w.B * w.H * w.num_queries):.2f} % of all rows, errs={errs}")
     if w.clean_tangent_zero:
         assert torch.count_nonzero(gpu[1][:, :, :w.N // 2]) == 0
     for t in gpu:
