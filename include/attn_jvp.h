@@ -160,6 +160,10 @@ aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mas
  * tile_rows.  attn_jvp_schedule_get / _info read it like any schedule, with the roles swapped. */
 aj_status attn_jvp_schedule_create_transposed(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
                                               int32_t tile_rows, aj_schedule **out);
+/* Same with an explicit aj_tiling of the KEY axis (PACKED: key tiles on a global grid of tile_keys keys; a tile that
+ * straddles key intervals streams the union of their row ranges, each entry carrying the interval of tile keys it sees). */
+aj_status attn_jvp_schedule_create_transposed_tiled(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
+                                                    int32_t tile_rows, int32_t tiling, aj_schedule **out);
 aj_status attn_jvp_schedule_destroy(aj_schedule *sched);
 /* Any out pointer may be NULL. unmasked_pairs_per_head = sum over groups of rows * allowed keys. */
 aj_status attn_jvp_schedule_info(const aj_schedule *sched, int32_t *num_groups, int32_t *num_ranges,

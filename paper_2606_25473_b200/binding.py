@@ -59,7 +59,7 @@ SYMBOLS = [
     "attn_jvp_schedule_create_transposed", "attn_jvp_schedule_entry_flags", "attn_jvp_schedule_pair_classes", "attn_jvp_plan_pair_classes", "attn_fwd", "attn_bwd",
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
-    "attn_jvp_fwd_tl", "attn_bwd_host", "attn_jvp_plan_tensor_map_stats",
+    "attn_jvp_fwd_tl", "attn_bwd_host", "attn_jvp_plan_tensor_map_stats", "attn_jvp_schedule_create_transposed_tiled",
 ]
 
 _lib = None
@@ -77,6 +77,7 @@ def lib():
         l.attn_jvp_schedule_create.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_create_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_create_transposed.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, ctypes.POINTER(vp)]
+        l.attn_jvp_schedule_create_transposed_tiled.argtypes = [ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc), i32, i32, i32, ctypes.POINTER(vp)]
         l.attn_jvp_schedule_entries.argtypes = [vp, _I32P, _I32P, _I32P, _I32P, _I32P]
         l.attn_jvp_schedule_assign.argtypes = [vp, i32, _I32P, _I32P]
         l.attn_jvp_schedule_entry_flags.argtypes = [vp, _I32P]
@@ -179,6 +180,12 @@ def attn_jvp_schedule_create_tiled(problem: aj_problem, mask: aj_mask_desc, tile
 def attn_jvp_schedule_create_transposed(problem: aj_problem, mask: aj_mask_desc, tile_keys: int, tile_rows: int) -> ctypes.c_void_p:
     out = ctypes.c_void_p()
     _check(lib().attn_jvp_schedule_create_transposed(ctypes.byref(problem), ctypes.byref(mask), tile_keys, tile_rows, ctypes.byref(out)))
+    return out
+
+
+def attn_jvp_schedule_create_transposed_tiled(problem: aj_problem, mask: aj_mask_desc, tile_keys: int, tile_rows: int, tiling: int) -> ctypes.c_void_p:
+    out = ctypes.c_void_p()
+    _check(lib().attn_jvp_schedule_create_transposed_tiled(ctypes.byref(problem), ctypes.byref(mask), tile_keys, tile_rows, tiling, ctypes.byref(out)))
     return out
 
 

@@ -434,41 +434,72 @@ aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, con
 
 namespace {
 
+// Which kernels the backward runs: plain FMA (fp32, d = 64, or a plan forced to SIMT), the single-CTA tcgen05 kernel (a plan
+// forced to AJ_KERNEL_UMMA, or a problem too large for the pair kernel's 1-D {lse, delta} map), or CTA pairs (default).
+enum BwdFamily { BWD_SIMT = 0, BWD_UMMA = 1, BWD_PAIR = 2 };
+BwdFamily bwd_family(const aj_plan *p) {
+    if (!umma_covers(p->problem) || p->kernel == AJ_KERNEL_SIMT) return BWD_SIMT;
+    if (p->kernel == AJ_KERNEL_UMMA) return BWD_UMMA;
+    const int64_t ld_floats = 2 * (int64_t)p->problem.B * p->problem.H * p->problem.Nq;
+    return ld_floats + 256 < (int64_t)1 << 31 ? BWD_PAIR : BWD_UMMA;
+}
+
 // The backward schedules of `prob` (the plan's problem, or one head of it): query tiles x key ranges (dQ) and key tiles x
 // row ranges (dK, dV; the transposed mask), tiled for the kernel family that will run; built and uploaded on first use.
-aj_status ensure_bwd_schedules(aj_plan *p, const aj_problem &prob, bool umma, aj_plan::DevSchedule &bq, aj_plan::DevSchedule &bk) {
-    const int tile_s = umma ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q, tile_m = umma ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
+// The tangent promises of the mask do not concern the backward: its schedules are built from the DENSE descriptor.
+aj_status ensure_bwd_schedules(aj_plan *p, const aj_problem &prob, BwdFamily fam, aj_plan::DevSchedule &bq, aj_plan::DevSchedule &bk) {
+    const int tile_s = fam == BWD_PAIR ? aj::UMMA_PAIR_TILE_Q : fam == BWD_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
+    const int tile_m = fam == BWD_SIMT ? aj::SIMT_TILE_K : aj::UMMA_TILE_K;
+    const int32_t tiling = fam == BWD_PAIR ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP;
+    const int32_t kernel = fam == BWD_PAIR ? AJ_KERNEL_UMMA_PAIR : AJ_KERNEL_SIMT;     // what upload_schedule lays the lists out for
+    const int workers = fam == BWD_UMMA ? p->num_sms : 0;                               // single-CTA kernel: one list per SM
+    aj_mask_desc dense = p->mask;
+    dense.tangent_zero = AJ_TANGENT_DENSE;
+    dense.q_tangent_zero = dense.k_tangent_zero = nullptr;
     if (!bq.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tile_s, tile_m, AJ_TILING_PER_GROUP, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, bq, umma ? p->num_sms : 0)) return st;
+        if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &dense, tile_s, tile_m, tiling, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, kernel, bq, workers)) return st;
     }
     if (!bk.sched) {
         aj_schedule *s = nullptr;
-        if (aj_status st = attn_jvp_schedule_create_transposed(&prob, &p->mask, tile_s, tile_m, &s)) return st;
-        if (aj_status st = upload_schedule(p, s, AJ_KERNEL_SIMT, bk, umma ? p->num_sms : 0)) return st;
+        if (aj_status st = attn_jvp_schedule_create_transposed_tiled(&prob, &dense, tile_s, tile_m, tiling, &s)) return st;
+        if (aj_status st = upload_schedule(p, s, kernel, bk, workers)) return st;
     }
     return AJ_OK;
 }
 
-// bf16, d = 128 (unless the plan was forced to the SIMT kernels): tcgen05 passes; otherwise plain-FMA kernels
-bool bwd_uses_umma(const aj_plan *p) { return umma_covers(p->problem) && p->kernel != AJ_KERNEL_SIMT; }
+aj_status encode_ld_map(CUtensorMap *map, const float *ld, int64_t floats) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    cuuint64_t dims[1] = {(cuuint64_t)floats};
+    cuuint64_t strides[1] = {0};
+    cuuint32_t box[1] = {128}, estr[1] = {1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 1, (void *)ld, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (lse / delta map) failed with CUresult " + std::to_string((int)r));
+    return AJ_OK;
+}
 
-// The three kernels of one backward call over the tasks of (bq, bk), which were built for a [B, H] problem.
-// ts = {q, k, v, o, dout, dq, dk, dv}; lse, delta: [B, H, Nq] of that problem; `slot`: first of eight tensor-map slots.
+// The kernels of one backward call over the tasks of (bq, bk), which were built for a [B, H] problem.
+// ts = {q, k, v, o, dout, dq, dk, dv}; lse: [B, H, Nq] of that problem; work: [B, H, Nq] floats (delta) for the SIMT and
+// single-CTA kernels, 2 x that ({lse log2e, delta} pairs) for the CTA-pair kernels; `slot`: first of eight tensor-map slots.
 aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_plan::DevSchedule &bk, int32_t B, int32_t H,
-                     const aj_tensor *const ts[8], const float *lse, float *delta, cudaStream_t stream, int slot) {
+                     const aj_tensor *const ts[8], const float *lse, float *work, cudaStream_t stream, int slot) {
     aj_problem pr = p->problem;
     pr.B = B; pr.H = H;
+    const BwdFamily fam = bwd_family(p);
     const aj_tensor *q = ts[0], *k = ts[1], *v = ts[2], *o = ts[3], *dout = ts[4], *dq = ts[5], *dk = ts[6], *dv = ts[7];
     aj::BwdParams prm;
     prm.q = *q; prm.k = *k; prm.v = *v; prm.o = *o; prm.dout = *dout; prm.dq = *dq; prm.dk = *dk; prm.dv = *dv;
-    prm.lse = lse; prm.delta = delta;
+    prm.lse = lse;
+    prm.delta = fam == BWD_PAIR ? nullptr : work;
+    prm.ld = fam == BWD_PAIR ? (float2 *)work : nullptr;
     prm.q_tasks = bq.d_tasks; prm.q_kb = bq.d_kb; prm.q_ke = bq.d_ke;
     prm.k_tasks = bk.d_tasks; prm.k_rb = bk.d_kb; prm.k_re = bk.d_ke;
     prm.B = pr.B; prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
     cudaError_t e;
-    if (!bwd_uses_umma(p)) {
+    if (fam == BWD_SIMT) {
         e = aj::launch_bwd_simt(prm, pr.dtype, pr.d, bq.num_tasks, bk.num_tasks, stream);
         if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
         return AJ_OK;
@@ -478,25 +509,46 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
     for (int pass = 0; pass < 2; ++pass) {
         const bool keys = pass == 1;
         const aj_plan::DevSchedule &ds = keys ? bk : bq;
-        aj::BwdUmmaParams up;
-        std::memset(&up, 0, sizeof(up));
-        aj_status st;
         // stationary operands (128-row boxes) and streamed operands (64-row boxes) of the pass
         const aj_tensor *a1 = keys ? k : q, *a2 = keys ? v : dout, *b1 = keys ? q : k, *b2 = keys ? dout : v;
         const int64_t na = keys ? pr.Nk : pr.Nq, nb = keys ? pr.Nq : pr.Nk;
-        if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
-        if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
-        if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
-        up.a1 = *a1; up.a2 = *a2; up.Na = (int32_t)na;
-        up.out1 = keys ? *dk : *dq;
-        up.out2 = *dv;
-        up.lse = lse; up.delta = delta;
-        up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.err = p->d_counters + 2;
-        up.cta_off = ds.d_pair_off; up.cta_ids = ds.d_pair_ids;
-        up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
-        up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
-        e = aj::launch_bwd_umma(up, keys, ds.num_pairs, stream);
+        aj_status st;
+        if (fam == BWD_PAIR) {
+            aj::BwdPairParams up;
+            std::memset(&up, 0, sizeof(up));
+            if (keys) {
+                if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
+                if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
+                if ((st = encode_ld_map(&up.tm_ld, work, 2 * (int64_t)pr.B * pr.H * pr.Nq))) return st;
+            }
+            if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
+            if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+            up.a1 = *a1; up.a2 = *a2;
+            up.out1 = keys ? *dk : *dq;
+            up.out2 = *dv;
+            up.ld = (const float2 *)work;
+            up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.rows = ds.d_rows; up.err = p->d_counters + 2;
+            up.pair_off = ds.d_pair_off; up.pair_ids = ds.d_pair_ids;
+            up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
+            up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
+            e = aj::launch_bwd_umma_pair(up, keys, ds.num_pairs, stream);
+        } else {
+            aj::BwdUmmaParams up;
+            std::memset(&up, 0, sizeof(up));
+            if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
+            if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
+            if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
+            if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+            up.a1 = *a1; up.a2 = *a2; up.Na = (int32_t)na;
+            up.out1 = keys ? *dk : *dq;
+            up.out2 = *dv;
+            up.lse = lse; up.delta = work;
+            up.tasks = ds.d_tasks; up.r_begin = ds.d_kb; up.r_end = ds.d_ke; up.err = p->d_counters + 2;
+            up.cta_off = ds.d_pair_off; up.cta_ids = ds.d_pair_ids;
+            up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
+            up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
+            e = aj::launch_bwd_umma(up, keys, ds.num_pairs, stream);
+        }
         if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
     }
     return AJ_OK;
@@ -539,14 +591,14 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     const aj_problem &pr = p->problem;
     const aj_tensor *ts[8] = {q, k, v, o, dout, dq, dk, dv};
     const char *names[8] = {"q", "k", "v", "o", "dout", "dq", "dk", "dv"};
-    const bool umma = bwd_uses_umma(p);
+    const BwdFamily fam = bwd_family(p);
     for (int i = 0; i < 8; ++i)
-        if (aj_status st = check_tensor(ts[i], names[i], pr, i >= 5, umma)) return st;
+        if (aj_status st = check_tensor(ts[i], names[i], pr, i >= 5, fam != BWD_SIMT)) return st;
     if (!lse || (uintptr_t)lse % 4 != 0) return fail(AJ_ERR_INVALID_ARG, "lse: NULL or misaligned");
     // first use: the two schedules and the delta workspace (synchronous host work and allocations)
-    if (aj_status st = ensure_bwd_schedules(p, p->problem, umma, p->bwd_q, p->bwd_k)) return st;
+    if (aj_status st = ensure_bwd_schedules(p, p->problem, fam, p->bwd_q, p->bwd_k)) return st;
     if (!p->d_delta) {
-        cudaError_t e = cudaMalloc(&p->d_delta, (size_t)pr.B * pr.H * pr.Nq * sizeof(float));
+        cudaError_t e = cudaMalloc(&p->d_delta, 2 * (size_t)pr.B * pr.H * pr.Nq * sizeof(float));   // delta, or {lse log2e, delta}
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
     }
     return launch_bwd(p, p->bwd_q, p->bwd_k, pr.B, pr.H, ts, lse, p->d_delta, (cudaStream_t)cuda_stream, SLOT_BWD);
@@ -562,19 +614,20 @@ aj_status attn_bwd_host(aj_plan *p, const void *q, const void *k, const void *v,
     const int nheads = pr.B * pr.H;
     const size_t hq = (size_t)pr.Nq * pr.d * eb, hk = (size_t)pr.Nk * pr.d * eb;     // one head of a tensor
     const size_t nq_bytes = hq * nheads, nk_bytes = hk * nheads, lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
+    const size_t work_bytes = 2 * lse_bytes;
     cudaStream_t stream = (cudaStream_t)cuda_stream;
-    {   // staging: q k v (shared with the forward) | o | dout dq dk dv | lse | delta
+    {   // staging: q k v (shared with the forward) | o | dout dq dk dv | lse | delta / {lse log2e, delta}
         const size_t in_bytes[3] = {nq_bytes, nk_bytes, nk_bytes}, bwd_bytes[4] = {nq_bytes, nq_bytes, nk_bytes, nk_bytes};
         if (aj_status st = ensure_staging(p->d_in, 3, in_bytes)) return st;
         if (aj_status st = ensure_staging(p->d_out, 1, &nq_bytes)) return st;
         if (aj_status st = ensure_staging(p->d_bwd, 4, bwd_bytes)) return st;
         if (aj_status st = ensure_staging((void **)&p->d_lse, 1, &lse_bytes)) return st;
-        if (aj_status st = ensure_staging((void **)&p->d_delta, 1, &lse_bytes)) return st;
+        if (aj_status st = ensure_staging((void **)&p->d_delta, 1, &work_bytes)) return st;
     }
     if (aj_status st = ensure_copy_streams(p)) return st;
     aj_problem one = p->problem;
     one.B = 1; one.H = 1;
-    if (aj_status st = ensure_bwd_schedules(p, one, bwd_uses_umma(p), p->bwd_q_head, p->bwd_k_head)) return st;
+    if (aj_status st = ensure_bwd_schedules(p, one, bwd_family(p), p->bwd_q_head, p->bwd_k_head)) return st;
     // Same pipeline as attn_jvp_fwd_host: head i's q, k, v, o, dout, lse go up on the copy-in stream, its three kernels run on
     // the caller's stream as soon as they have landed, its dq, dk, dv come back on the copy-out stream.
     cudaError_t e = cudaEventRecord(p->ev_begin, stream);
@@ -605,7 +658,7 @@ aj_status attn_bwd_host(aj_plan *p, const void *q, const void *k, const void *v,
             ts[i] = &t[i];
         }
         if (aj_status st = launch_bwd(p, p->bwd_q_head, p->bwd_k_head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq,
-                                      p->d_delta + (size_t)hd * pr.Nq, stream, SLOT_HEAD + hd * SLOTS_PER_HEAD + 8)) return st;
+                                      p->d_delta + 2 * (size_t)hd * pr.Nq, stream, SLOT_HEAD + hd * SLOTS_PER_HEAD + 8)) return st;
         e = cudaEventRecord(p->ev_k[hd], stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
         for (int i = 0; i < 3 && e == cudaSuccess; ++i) {

@@ -46,7 +46,10 @@ __global__ void __launch_bounds__(128) attn_bwd_delta_kernel(BwdParams prm) {
     for (int c = lane; c < D; c += 32) acc = fmaf(ld32(o[c]), ld32(g[c]), acc);
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
-    if (lane == 0) prm.delta[row] = acc;
+    if (lane == 0) {
+        if (prm.delta) prm.delta[row] = acc;
+        if (prm.ld) prm.ld[row] = make_float2(prm.lse[row] * 1.4426950408889634f, acc);   // what the CTA-pair passes consume
+    }
 }
 
 // KEYS = false: stationary = query rows (Q, dO, lse, delta), streamed = keys (K, V); writes dQ.

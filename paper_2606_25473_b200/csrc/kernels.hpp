@@ -47,7 +47,8 @@ cudaError_t launch_simt(const SimtParams &prm, int dtype, int d, int num_tasks, 
 struct BwdParams {
     aj_tensor q, k, v, o, dout, dq, dk, dv;
     const float *lse;                 // [B, H, Nq] from the forward
-    float *delta;                     // [B, H, Nq] workspace: <dO_a, O_a>
+    float *delta;                     // [B, H, Nq] workspace: <dO_a, O_a> (may be NULL when `ld` is given)
+    float2 *ld;                       // [B, H, Nq] workspace of the CTA-pair kernels: {lse * log2(e), delta} (or NULL)
     const aj_task *q_tasks; const int32_t *q_kb, *q_ke;   // query tiles and their key ranges
     const aj_task *k_tasks; const int32_t *k_rb, *k_re;   // key tiles and their row ranges
     int32_t B, H, Nq;
@@ -71,6 +72,24 @@ struct BwdUmmaParams {
     float scale, scale_log2;
 };
 cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream);
+
+// Primal backward on CTA pairs (kernel_umma_bwd_pair_sm100.cu; bf16, d = 128): tcgen05.mma.cta_group::2, 256 stationary rows
+// per pair, packed tiling (entries carry row intervals).  a1, a2: stationary operands (box {64, 128}; KEYS pass only);
+// b1, b2: streamed (box {64, 64}); ld: 1-D map over the {lse log2e, delta} workspace as plain floats (box 128; KEYS pass).
+struct BwdPairParams {
+    CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2, tm_ld;
+    aj_tensor out1, out2;             // dQ | dK, dV
+    aj_tensor a1, a2;                 // dQ pass: Q and dO as plain views (their rows go to TMEM, not to shared memory)
+    const float2 *ld;                 // [B, H, Nq] {lse log2e, delta}
+    const aj_task *tasks;
+    const int32_t *r_begin, *r_end;   // schedule entries: streamed rows [r_begin[e], r_end[e]) ...
+    const uint32_t *rows;             // ... seen by stationary tile rows [rows[e] & 0xffff, (rows[e] >> 16) & 0x7fff)
+    const int32_t *pair_off, *pair_ids;
+    int32_t *err;                     // abort code word of the plan
+    int32_t num_tasks, H, Nq;
+    float scale, scale_log2;
+};
+cudaError_t launch_bwd_umma_pair(const BwdPairParams &prm, bool keys, int num_pairs, cudaStream_t stream);
 // delta kernel of kernel_simt_bwd.cu alone (shared by both backward paths)
 cudaError_t launch_bwd_delta(const BwdParams &prm, int dtype, int d, cudaStream_t stream);
 

@@ -411,11 +411,17 @@ aj_status attn_jvp_schedule_create_tiled(const aj_problem *problem, const aj_mas
 
 aj_status attn_jvp_schedule_create_transposed(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
                                               int32_t tile_rows, aj_schedule **out) {
+    return attn_jvp_schedule_create_transposed_tiled(problem, mask, tile_keys, tile_rows, AJ_TILING_PER_GROUP, out);
+}
+
+aj_status attn_jvp_schedule_create_transposed_tiled(const aj_problem *problem, const aj_mask_desc *mask, int32_t tile_keys,
+                                                    int32_t tile_rows, int32_t tiling, aj_schedule **out) {
     if (!out) return aj::fail(AJ_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
     if (aj_status st = aj::check_problem(problem)) return st;
     if (!mask) return aj::fail(AJ_ERR_INVALID_ARG, "mask is NULL");
     if (tile_keys <= 0 || tile_rows <= 0 || tile_keys > 32767) return aj::fail(AJ_ERR_INVALID_ARG, "tile sizes must be > 0 (tile_keys < 32768)");
+    if (tiling != AJ_TILING_PER_GROUP && tiling != AJ_TILING_PACKED) return aj::fail(AJ_ERR_INVALID_ARG, "unknown tiling");
     aj_schedule *s = new (std::nothrow) aj_schedule();
     if (!s) return aj::fail(AJ_ERR_OOM, "out of host memory");
     try {
@@ -424,9 +430,10 @@ aj_status attn_jvp_schedule_create_transposed(const aj_problem *problem, const a
         if (st != AJ_OK) { delete s; return st; }
         s->problem = *problem;
         std::swap(s->problem.Nq, s->problem.Nk);           // the tasks' "query rows" are keys
-        s->tile_q = tile_keys; s->tile_k = tile_rows; s->tiling = AJ_TILING_PER_GROUP;
+        s->tile_q = tile_keys; s->tile_k = tile_rows; s->tiling = tiling;
         aj::transpose_lowered(*problem, low, s->low);
-        aj::build_tasks(s->problem, s->low, tile_keys, tile_rows, s->entries, s->tasks);
+        if (tiling == AJ_TILING_PACKED) aj::build_tasks_packed(s->problem, s->low, tile_keys, tile_rows, s->entries, s->tasks);
+        else aj::build_tasks(s->problem, s->low, tile_keys, tile_rows, s->entries, s->tasks);
     } catch (const std::bad_alloc &) {
         delete s;
         return aj::fail(AJ_ERR_OOM, "out of host memory");

@@ -107,6 +107,34 @@ def test_backward_small_every_element(w):
         assert max(errs.values()) < 2e-5
 
 
+BF16_D128 = [w for w in SMALL if w.dtype == "bf16" and w.d == 128]
+
+
+@pytest.mark.parametrize("w", BF16_D128, ids=lambda w: w.name)
+def test_backward_single_cta_tcgen05_kernel_every_element(w):
+    # a plan forced to AJ_KERNEL_UMMA runs the single-CTA backward (128 stationary rows per CTA, per-group tiling); the default
+    # (test_backward_small_every_element) is the CTA-pair backward (256 rows per SM pair, packed tiling)
+    x = make_inputs(w)
+    dout = _dout(w)
+    got = run_fwd_bwd(w, x, dout, kernel=aj.AJ_KERNEL_UMMA)
+    check(w, x, dout, got)
+    pair = run_fwd_bwd(w, x, dout)
+    for u, v in zip(got, pair):
+        assert max_norm_err(u.double().numpy(), v.double().numpy()) <= 1e-2
+
+
+def test_backward_pair_kernel_many_tasks_per_pair_and_long_streams():
+    # more 256-row tasks than SM pairs (148 + tasks on 74 pairs: every pair runs several tasks back to back, with the
+    # accumulators, the TMEM A operands and the {lse, delta} stages reused), long streams with odd tile counts
+    w = Workload("bwd_bc_bf16_many", 2, 4, 128, "block_causal", 1000, 5, 1, "bf16", 0.1, seed=31)
+    x = make_inputs(w)
+    dout = _dout(w)
+    got = run_fwd_bwd(w, x, dout)
+    check(w, x, dout, got, heads=[(0, 0), (1, 3)])
+    for t in got:
+        assert torch.isfinite(t.float()).all()
+
+
 def test_backward_bf16_tcgen05_and_simt_paths_agree():
     w = SMALL[4]
     x = make_inputs(w)

@@ -459,3 +459,46 @@ def test_transposed_schedule_of_generic_ranges_with_unseen_keys(oracle):
     want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
     for tk, tr in [(8, 4), (16, 8), (3, 5)]:
         _check_transposed(want, prob, mask, tk, tr)
+
+
+# ---------------------------------------------------------------------------------------------- transposed + packed (CTA-pair backward)
+def _transposed_packed(prob, mask, tile_keys, tile_rows):
+    s = aj.attn_jvp_schedule_create_transposed_tiled(prob, mask, tile_keys, tile_rows, aj.AJ_TILING_PACKED)
+    info = aj.attn_jvp_schedule_info(s)
+    got = aj.attn_jvp_schedule_get(s)
+    ent = aj.attn_jvp_schedule_entries(s)
+    aj.attn_jvp_schedule_destroy(s)
+    return info, got, ent
+
+
+@pytest.mark.parametrize("mask,L,F,cf", [
+    ("teacher_forcing", 16, 3, 1), ("teacher_forcing", 10, 6, 3), ("teacher_forcing", 7, 4, 2),
+    ("block_causal", 16, 3, 1), ("block_causal", 9, 6, 2), ("full", 13, 5, 1), ("teacher_forcing", 3, 5, 1)])
+@pytest.mark.parametrize("tile_keys,tile_rows", [(16, 32), (8, 4), (256, 64), (5, 3)])
+def test_transposed_packed_tiles_cover_the_transposed_mask_exactly_once(oracle, mask, L, F, cf, tile_keys, tile_rows):
+    # key tiles on a global grid; an entry = query rows [k_begin, k_end) seen by the tile's keys [row_begin, row_end)
+    w = Workload("t", 1, 2, 64, mask, L, F, cf, "fp32", 1.0)
+    prob = aj.make_problem(w.B, w.H, w.N, w.N, w.d, aj.AJ_FP32)
+    m, keep = aj.make_mask(_kind(w), L, F, cf)
+    info, got, ent = _transposed_packed(prob, m, tile_keys, tile_rows)
+    want = oracle.dense_mask(oracle_mask(w), w.N, w.N)
+    _check_packed(want.T, w.N, info, got, ent, tile_keys, tile_rows, heads=2)
+
+
+def test_transposed_packed_generic_ranges_with_unseen_keys_and_nq_ne_nk(oracle):
+    groups = [(4, 9, [(0, 5), (5, 9), (30, 40)]), (9, 13, [(2, 3)]), (13, 20, [(30, 40), (44, 48)]), (33, 40, [])]
+    prob = aj.make_problem(1, 1, 40, 48, 64, aj.AJ_FP32)
+    mask, keep = aj.make_mask(aj.AJ_MASK_RANGES, groups=groups)
+    want = oracle.dense_mask(oracle.ranges_mask(groups), 40, 48)
+    for tk, tr in [(8, 4), (16, 8), (64, 64), (3, 5)]:
+        info, got, ent = _transposed_packed(prob, mask, tk, tr)
+        _check_packed(want.T, 48, info, got, ent, tk, tr)
+
+
+def test_transposed_packed_ignores_tangent_promises():
+    # the backward has no tangents: a CLEAN_ZERO descriptor lowered with the promise stripped flags no task
+    w = Workload("t", 1, 1, 128, "teacher_forcing", 300, 3, 1, "bf16", 0.1)
+    prob = aj.make_problem(1, 1, w.N, w.N, w.d, aj.AJ_BF16)
+    m, keep = aj.make_mask(aj.AJ_MASK_TEACHER_FORCING, w.frame_len, w.num_frames, 1, tangent_zero=aj.AJ_TANGENT_DENSE)
+    info, got, ent = _transposed_packed(prob, m, 256, 64)
+    assert all(t.flags == 0 for t in got["tasks"])
