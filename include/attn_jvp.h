@@ -73,8 +73,11 @@ typedef enum { AJ_TANGENT_DENSE = 0, AJ_TANGENT_CLEAN_ZERO = 1, AJ_TANGENT_NONE 
 
 /* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA_PAIR when (bf16, d = 128), else SIMT.
  * UMMA: one CTA per 128-row query tile (tcgen05.mma.cta_group::1).  UMMA_PAIR: a CTA pair per 256-row query tile
- * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile). */
-typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2, AJ_KERNEL_UMMA_PAIR = 3 } aj_kernel;
+ * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile).
+ * UMMA_PAIR sends the tasks that need no tangent at all (AJ_TASK_PRIMAL_ONLY: everything under AJ_TANGENT_NONE, the clean
+ * rows under AJ_TANGENT_CLEAN_ZERO) to a second kernel specialised for them (two softmax warpgroups, S triple-buffered), in
+ * a launch of its own before the general one; UMMA_PAIR_ONE keeps every task in the one general CTA-pair kernel. */
+typedef enum { AJ_KERNEL_AUTO = 0, AJ_KERNEL_SIMT = 1, AJ_KERNEL_UMMA = 2, AJ_KERNEL_UMMA_PAIR = 3, AJ_KERNEL_UMMA_PAIR_ONE = 4 } aj_kernel;
 
 /*
  * Mask descriptor = the paper's problem statement.  Structured kinds: a block is

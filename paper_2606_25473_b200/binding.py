@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_PKG, "libattn_jvp.so")
 AJ_OK, AJ_ERR_INVALID_ARG, AJ_ERR_UNSUPPORTED, AJ_ERR_CUDA, AJ_ERR_OOM = 0, -1, -2, -3, -4
 AJ_BF16, AJ_FP32 = 0, 1
 AJ_MASK_FULL, AJ_MASK_BLOCK_CAUSAL, AJ_MASK_TEACHER_FORCING, AJ_MASK_RANGES = 0, 1, 2, 3
-AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA, AJ_KERNEL_UMMA_PAIR = 0, 1, 2, 3
+AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA, AJ_KERNEL_UMMA_PAIR, AJ_KERNEL_UMMA_PAIR_ONE = 0, 1, 2, 3, 4
 AJ_TILING_PER_GROUP, AJ_TILING_PACKED = 0, 1
 AJ_TANGENT_DENSE, AJ_TANGENT_CLEAN_ZERO, AJ_TANGENT_NONE = 0, 1, 2
 AJ_TASK_PRIMAL_ONLY = 1

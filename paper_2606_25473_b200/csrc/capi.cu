@@ -31,6 +31,10 @@ struct aj_plan {
         uint32_t *d_rows = nullptr;   // per entry: row_begin | row_end << 16
         int32_t *d_pair_off = nullptr, *d_pair_ids = nullptr;   // CTA-pair kernel: host-assigned task lists
         int32_t num_pairs = 0;
+        // AJ_KERNEL_UMMA_PAIR: the primal-only tasks have lists of their own (run by the forward-only kernel) and are absent
+        // from the lists above
+        int32_t *d_prim_off = nullptr, *d_prim_ids = nullptr;
+        int32_t num_prim_pairs = 0;
     } full, head;                 // forward
     // primal backward: query tiles x key ranges (dQ) and key tiles x row ranges (dK, dV) for all B x H heads, and for ONE
     // head (attn_bwd_host)
@@ -85,14 +89,15 @@ aj_status cuda_fail(cudaError_t e, const char *what) {
 
 void free_schedule(aj_plan::DevSchedule &ds) {
     cudaFree(ds.d_tasks); cudaFree(ds.d_kb); cudaFree(ds.d_ke); cudaFree(ds.d_rows);
-    cudaFree(ds.d_pair_off); cudaFree(ds.d_pair_ids);
+    cudaFree(ds.d_pair_off); cudaFree(ds.d_pair_ids); cudaFree(ds.d_prim_off); cudaFree(ds.d_prim_ids);
     attn_jvp_schedule_destroy(ds.sched);
     ds = aj_plan::DevSchedule();
 }
 
 bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && p.d == 128; }
 
-bool is_umma(int32_t kernel) { return kernel == AJ_KERNEL_UMMA || kernel == AJ_KERNEL_UMMA_PAIR; }
+bool is_pair(int32_t kernel) { return kernel == AJ_KERNEL_UMMA_PAIR || kernel == AJ_KERNEL_UMMA_PAIR_ONE; }
+bool is_umma(int32_t kernel) { return kernel == AJ_KERNEL_UMMA || is_pair(kernel); }
 int32_t auto_kernel(const aj_problem &p) { return umma_covers(p) ? AJ_KERNEL_UMMA_PAIR : AJ_KERNEL_SIMT; }
 
 // The tcgen05 kernels tile queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
@@ -104,9 +109,9 @@ int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACK
 aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers = 0);
 
 aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int32_t tiling, aj_plan::DevSchedule &ds) {
-    const int tq = kernel == AJ_KERNEL_UMMA_PAIR ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
+    const int tq = is_pair(kernel) ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
     const int tk = is_umma(kernel) ? aj::UMMA_TILE_K : aj::SIMT_TILE_K;
-    if (kernel == AJ_KERNEL_UMMA_PAIR && tiling != AJ_TILING_PACKED)
+    if (is_pair(kernel) && tiling != AJ_TILING_PACKED)
         return fail(AJ_ERR_UNSUPPORTED, "the CTA-pair tcgen05 kernel only supports packed tiling");
     if (kernel == AJ_KERNEL_SIMT && tiling != AJ_TILING_PER_GROUP)
         return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
@@ -122,20 +127,36 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r)   // row_begin | row_end << 16 (both < 32768) | key-tangents-zero << 31
         rows[r] = (uint32_t)s->entries.row_begin[r] | ((uint32_t)s->entries.row_end[r] << 16) | (s->entries.k_tz[r] ? 0x80000000u : 0u);
-    std::vector<int32_t> pair_off, pair_ids;
-    int num_pairs = 0;
-    if (kernel == AJ_KERNEL_UMMA_PAIR || workers > 0) {
-        num_pairs = (int)std::min<size_t>(workers > 0 ? workers : std::max(p->num_sms / 2, 1), std::max<size_t>(nt, 1));
-        aj::assign_workers(s->tasks, s->entries, s->tile_k, num_pairs, pair_off, pair_ids);
+    std::vector<int32_t> pair_off, pair_ids, prim_off, prim_ids;
+    int num_pairs = 0, num_prim_pairs = 0;
+    // tasks [ids] of the schedule onto `want` workers (fewer if there are fewer tasks); ids refer to s->tasks
+    auto assign = [&](const std::vector<int32_t> &ids, int want, std::vector<int32_t> &off, std::vector<int32_t> &out) {
+        std::vector<aj_task> sub;
+        for (int32_t t : ids) sub.push_back(s->tasks[t]);
+        const int n = (int)std::min<size_t>(std::max(want, 1), std::max<size_t>(sub.size(), 1));
+        aj::assign_workers(sub, s->entries, s->tile_k, n, off, out);
+        for (int32_t &t : out) t = ids[t];
+        return n;
+    };
+    if (is_pair(kernel) || workers > 0) {
+        const int want = workers > 0 ? workers : std::max(p->num_sms / 2, 1);
+        std::vector<int32_t> general, primal;
+        for (size_t t = 0; t < nt; ++t)
+            ((kernel == AJ_KERNEL_UMMA_PAIR && (s->tasks[t].flags & AJ_TASK_PRIMAL_ONLY)) ? primal : general).push_back((int32_t)t);
+        num_pairs = assign(general, want, pair_off, pair_ids);
+        if (general.empty()) num_pairs = 0;
+        if (!primal.empty()) num_prim_pairs = assign(primal, want, prim_off, prim_ids);
     }
     aj_task *d_tasks = nullptr;
-    int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr;
+    int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr, *d_prim_off = nullptr, *d_prim_ids = nullptr;
     uint32_t *d_rows = nullptr;
     cudaError_t e = cudaMalloc(&d_tasks, std::max<size_t>(nt, 1) * sizeof(aj_task));
-    if (e == cudaSuccess && num_pairs) e = cudaMalloc(&d_pair_off, pair_off.size() * sizeof(int32_t));
-    if (e == cudaSuccess && num_pairs) e = cudaMalloc(&d_pair_ids, std::max<size_t>(pair_ids.size(), 1) * sizeof(int32_t));
-    if (e == cudaSuccess && num_pairs) e = cudaMemcpy(d_pair_off, pair_off.data(), pair_off.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && num_pairs && !pair_ids.empty()) e = cudaMemcpy(d_pair_ids, pair_ids.data(), pair_ids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    auto up = [&](const std::vector<int32_t> &h, int32_t **d) {
+        if (e == cudaSuccess) e = cudaMalloc(d, std::max<size_t>(h.size(), 1) * sizeof(int32_t));
+        if (e == cudaSuccess && !h.empty()) e = cudaMemcpy(*d, h.data(), h.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    };
+    if (num_pairs) { up(pair_off, &d_pair_off); up(pair_ids, &d_pair_ids); }
+    if (num_prim_pairs) { up(prim_off, &d_prim_off); up(prim_ids, &d_prim_ids); }
     if (e == cudaSuccess) e = cudaMalloc(&d_kb, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_ke, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_rows, std::max<size_t>(nr, 1) * sizeof(uint32_t));
@@ -145,6 +166,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     if (e == cudaSuccess && nr) e = cudaMemcpy(d_rows, rows.data(), nr * sizeof(uint32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke); cudaFree(d_rows); cudaFree(d_pair_off); cudaFree(d_pair_ids);
+        cudaFree(d_prim_off); cudaFree(d_prim_ids);
         attn_jvp_schedule_destroy(s);
         return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
     }
@@ -152,6 +174,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     ds.sched = s; ds.num_tasks = (int32_t)nt;
     ds.d_tasks = d_tasks; ds.d_kb = d_kb; ds.d_ke = d_ke; ds.d_rows = d_rows;
     ds.d_pair_off = d_pair_off; ds.d_pair_ids = d_pair_ids; ds.num_pairs = num_pairs;
+    ds.d_prim_off = d_prim_off; ds.d_prim_ids = d_prim_ids; ds.num_prim_pairs = num_prim_pairs;
     return AJ_OK;
 }
 
@@ -332,7 +355,7 @@ aj_status attn_jvp_plan_set_tiling(aj_plan *p, int32_t tiling) {
 aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launches) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
     if (kernel) *kernel = p->kernel;
-    if (launches) *launches = p->full.num_tasks > 0 ? 1 : 0;
+    if (launches) *launches = p->full.num_tasks == 0 ? 0 : is_pair(p->kernel) ? (p->full.num_pairs > 0) + (p->full.num_prim_pairs > 0) : 1;
     return AJ_OK;
 }
 
@@ -377,8 +400,17 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
         prm.num_tasks = ds.num_tasks; prm.H = pr.H; prm.Nq = pr.Nq;
         prm.scale = pr.scale; prm.scale_log2 = pr.scale * 1.4426950408889634f;
         prm.pair_off = ds.d_pair_off; prm.pair_ids = ds.d_pair_ids;
-        e = p->kernel == AJ_KERNEL_UMMA_PAIR ? aj::launch_umma_pair(prm, ds.num_pairs, stream)
-                                             : aj::launch_umma(prm, std::min(p->num_sms, ds.num_tasks), stream);
+        if (is_pair(p->kernel)) {
+            e = cudaSuccess;
+            if (ds.num_prim_pairs > 0) {                 // the tasks without tangents: the forward-only kernel, lists of their own
+                aj::UmmaParams pp = prm;
+                pp.pair_off = ds.d_prim_off; pp.pair_ids = ds.d_prim_ids;
+                e = aj::launch_umma_pair_fwd(pp, ds.num_prim_pairs, stream);
+            }
+            if (e == cudaSuccess && ds.num_pairs > 0) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);
+        } else {
+            e = aj::launch_umma(prm, std::min(p->num_sms, ds.num_tasks), stream);
+        }
     } else {
         aj::SimtParams prm;
         std::memset(&prm, 0, sizeof(prm));
@@ -474,7 +506,7 @@ aj_status encode_ld_map(CUtensorMap *map, const float *ld, int64_t floats) {
     if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
     cuuint64_t dims[1] = {(cuuint64_t)floats};
     cuuint64_t strides[1] = {0};
-    cuuint32_t box[1] = {128}, estr[1] = {1};
+    cuuint32_t box[1] = {132}, estr[1] = {1};   // 66 rows of {lse log2e, delta}: see LD_BOX_FLOATS in the kernel
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 1, (void *)ld, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (lse / delta map) failed with CUresult " + std::to_string((int)r));

@@ -54,8 +54,11 @@ constexpr uint32_t A_BYTES = BR * D * 2;           // 32 KB
 constexpr uint32_t AHALF_BYTES = BR * 64 * 2;      // one 64-column swizzle block of a stationary operand: 16 KB
 constexpr uint32_t BLK_BYTES = BC * 64 * 2;        // 8 KB: 64 streamed rows x 64 columns, 128-byte swizzled rows
 constexpr uint32_t SLOT_BYTES = 4 * BLK_BYTES;     // 32 KB
-constexpr int LD_STAGES = 4;                       // KEYS: {lse log2e, delta} of both tiles of a pair-step, 2 x 64 x 8 B
-constexpr uint32_t LD_TILE_BYTES = BC * 8;         // 512 B
+constexpr int LD_STAGES = 4;                       // KEYS: {lse log2e, delta} of both tiles of a pair-step
+// A TMA tile must start on a 16-byte boundary of global memory, a row's float2 only guarantees 8: the load starts at the
+// even row at or below the tile's first row and brings 66 rows; `ld_shift` tells the readers whether to skip one.
+constexpr uint32_t LD_BOX_FLOATS = 2 * (BC + 2);   // 132 floats = 528 B
+constexpr uint32_t LD_TILE_BYTES = 640;            // 528 rounded up to 128 B
 constexpr uint32_t LD_STAGE_BYTES = 2 * LD_TILE_BYTES;
 constexpr int NTHREADS = 384;
 
@@ -98,6 +101,8 @@ struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
     int abort_flag;
+    int ld_shift[LD_STAGES][2];   // KEYS: 1 if the stage's tile starts at an odd row of the {lse, delta} array (written by the
+                                  // producer before it arms LD_FULL[stage], read after the wait)
 };
 static_assert(sizeof(Shared) <= 512, "struct Shared outgrew its reservation");
 
@@ -200,9 +205,12 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         // {lse log2e, delta} of the 64 streamed rows of both tiles.  Stage nstep & 3 was last read in pair-step
                         // nstep - 4, whose Z hand-over precedes (through the MMA issue order) the release of the slot just waited for.
                         const uint32_t st = nstep & (LD_STAGES - 1), lbar = bars + 8 * (BAR_LD_FULL + st);
-                        mbar_expect_tx(lbar, LD_STAGE_BYTES);
-                        tma_load_1d(sLd + st * LD_STAGE_BYTES, &prm.tm_ld, lbar, (int)(2 * (ld_base + t0.key_row)));
-                        tma_load_1d(sLd + st * LD_STAGE_BYTES + LD_TILE_BYTES, &prm.tm_ld, lbar, (int)(2 * (ld_base + t1.key_row)));
+                        const int64_t r0 = ld_base + t0.key_row, r1 = ld_base + t1.key_row;
+                        ((volatile int *)sh->ld_shift[st])[0] = (int)(r0 & 1);
+                        ((volatile int *)sh->ld_shift[st])[1] = (int)(r1 & 1);
+                        mbar_expect_tx(lbar, 2 * LD_BOX_FLOATS * 4);
+                        tma_load_1d(sLd + st * LD_STAGE_BYTES, &prm.tm_ld, lbar, (int)(2 * (r0 & ~(int64_t)1)));
+                        tma_load_1d(sLd + st * LD_STAGE_BYTES + LD_TILE_BYTES, &prm.tm_ld, lbar, (int)(2 * (r1 & ~(int64_t)1)));
                     }
                     {   // this CTA's column half of the MN-major operands of both tiles
                         const uint32_t slot = ring % NSTAGE;
@@ -382,11 +390,16 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     const int v1 = 2 * p + 1 < n ? cur.tile() : 0;
                     valid = wg ? v1 : v0;
                 }
-                const float4 *stg = nullptr;
-                if (KEYS) {
-                    const uint32_t st = c_step & (LD_STAGES - 1);
-                    stg = reinterpret_cast<const float4 *>(ld_gen + st * LD_STAGE_BYTES + wg * LD_TILE_BYTES);
-                }
+                const uint8_t *stg_base = nullptr;
+                if (KEYS) stg_base = ld_gen + (c_step & (LD_STAGES - 1)) * LD_STAGE_BYTES + wg * LD_TILE_BYTES;
+                // {lse log2e, delta} of streamed rows c, c + 1 of the tile (c even): one 16-byte read when the tile starts at an
+                // even row of the array, two 8-byte reads otherwise
+                bool odd = false;
+                auto ld2 = [&](int c) -> float4 {
+                    if (!odd) return reinterpret_cast<const float4 *>(stg_base)[c >> 1];
+                    const float2 a = reinterpret_cast<const float2 *>(stg_base)[c + 1], b = reinterpret_cast<const float2 *>(stg_base)[c + 2];
+                    return make_float4(a.x, a.y, b.x, b.y);
+                };
                 wait(BAR_X_FULL, c_step & 1);
                 tc_fence_after();
                 // ---- W = exp2(X s log2e - lse log2e) = p_ab (PAPER.md:842-844 with the forward's L, :945), fp32 in registers
@@ -396,11 +409,14 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     uint32_t xu[32];
                     tmem_ld32(tX + 32 * hb, xu);
                     tc_wait_ld(xu);
-                    if (KEYS && hb == 0) wait(BAR_LD_FULL + (c_step & (LD_STAGES - 1)), (c_step / LD_STAGES) & 1);
+                    if (KEYS && hb == 0) {
+                        wait(BAR_LD_FULL + (c_step & (LD_STAGES - 1)), (c_step / LD_STAGES) & 1);
+                        odd = ((volatile int *)sh->ld_shift[c_step & (LD_STAGES - 1)])[wg] != 0;
+                    }
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
                         uint64_t nl = myl_2;
-                        if (KEYS) { const float4 f = stg[(32 * hb + c) >> 1]; nl = pack2(-f.x, -f.z); }
+                        if (KEYS) { const float4 f = ld2(32 * hb + c); nl = pack2(-f.x, -f.z); }
                         const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl);
                         float x0, x1;
                         unpack2(x, x0, x1);
@@ -439,7 +455,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
                         uint64_t nd = myd_2;
-                        if (KEYS) { const float4 f = stg[(32 * hb + c) >> 1]; nd = pack2(-f.y, -f.w); }
+                        if (KEYS) { const float4 f = ld2(32 * hb + c); nd = pack2(-f.y, -f.w); }
                         const int cc = 32 * hb + c;
                         const uint64_t z = fmul2(pack2(w[cc], w[cc + 1]), fadd2(pack2(yu[c], yu[c + 1]), nd));
                         float z0, z1;

@@ -117,4 +117,8 @@ cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream);
 size_t umma_pair_smem_bytes();
 cudaError_t launch_umma_pair(const UmmaParams &prm, int num_pairs, cudaStream_t stream);
 
+// bf16, d = 128, CTA pairs, primal-only tasks alone (no tangents: S and P~ V): two softmax warpgroups on alternate pair-steps,
+// S triple-buffered in TMEM (kernel_umma_pair_fwd_sm100.cu).  prm.pair_off / pair_ids must list primal-only tasks only.
+cudaError_t launch_umma_pair_fwd(const UmmaParams &prm, int num_pairs, cudaStream_t stream);
+
 }  // namespace aj

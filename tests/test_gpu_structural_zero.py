@@ -40,13 +40,17 @@ CLEAN_ZERO = [
 ]
 
 
+@pytest.mark.parametrize("kernel", [aj.AJ_KERNEL_UMMA_PAIR, aj.AJ_KERNEL_UMMA_PAIR_ONE], ids=["split", "one"])
 @pytest.mark.parametrize("w", CLEAN_ZERO, ids=lambda w: w.name)
-def test_clean_zero_every_row(w):
+def test_clean_zero_every_row(w, kernel):
+    # "split" (default): the primal-only tasks run in the forward-only kernel (two softmax warpgroups), the rest in the general
+    # CTA-pair kernel; "one": every task in the general kernel
     x = make_inputs(w)
     half = w.N // 2
     assert all(torch.count_nonzero(t[:, :, :half]) == 0 for t in x[3:]) and all(torch.count_nonzero(t[:, :, half:]) > 0 for t in x[3:])
-    plan = make_plan(w)
-    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA_PAIR, 1)
+    plan = make_plan(w, kernel)
+    k_id, launches = aj.attn_jvp_plan_kernel(plan)
+    assert k_id == kernel and launches == (1 if kernel == aj.AJ_KERNEL_UMMA_PAIR_ONE else 2 if w.N // 2 >= 256 else launches)
     classes = aj.attn_jvp_plan_pair_classes(plan)
     n, C = w.num_blocks, w.block_len
     assert classes == [n * (n + 1) // 2 * C * C, n * (n - 1) // 2 * C * C, n * C * C]
@@ -74,7 +78,38 @@ def test_clean_zero_rescales_mid_stream():
     ramp = torch.linspace(0.2, 9.0, w.N // 2).repeat(2).view(1, 1, w.N, 1)
     x[1] = (x[1].float() * ramp).to(torch.bfloat16)
     x[0] = (x[0].float() * 3.0).to(torch.bfloat16)
-    compare(w, run_gpu(w, x), run_oracle(w, x))
+    ref = run_oracle(w, x)
+    compare(w, run_gpu(w, x), ref)
+    compare(w, run_gpu(w, x, kernel=aj.AJ_KERNEL_UMMA_PAIR_ONE), ref)
+
+
+def test_forward_only_kernel_rescales_across_the_two_warpgroups():
+    # AJ_TANGENT_NONE, one long key stream per task (14 pair-steps and more): the reference max keeps moving by more than the
+    # lazy threshold, so it is handed from one softmax warpgroup to the other again and again and both rescale their share of l
+    Nq, Nk = 600, 1900
+    g = torch.Generator().manual_seed(77)
+    q = (torch.randn((1, 2, Nq, 128), generator=g) * 3.0).to(torch.bfloat16)
+    k = (torch.randn((1, 2, Nk, 128), generator=g) * torch.linspace(0.2, 9.0, Nk).view(1, 1, Nk, 1)).to(torch.bfloat16)
+    v = torch.randn((1, 2, Nk, 128), generator=g).to(torch.bfloat16)
+    prob = aj.make_problem(1, 2, Nq, Nk, 128, aj.AJ_BF16)
+    mask, keep = aj.make_mask(aj.AJ_MASK_FULL, tangent_zero=aj.AJ_TANGENT_NONE)
+    outs = {}
+    for kernel in (aj.AJ_KERNEL_UMMA_PAIR, aj.AJ_KERNEL_UMMA_PAIR_ONE):
+        plan = aj.attn_jvp_plan_create(prob, mask)
+        aj.attn_jvp_plan_set_kernel(plan, kernel)
+        o = torch.full((1, 2, Nq, 128), float("nan"), dtype=torch.bfloat16, device="cuda")
+        lse = torch.full((1, 2, Nq), float("nan"), dtype=torch.float32, device="cuda")
+        aj.attn_fwd(plan, q.cuda(), k.cuda(), v.cuda(), o, lse, 0)
+        torch.cuda.synchronize()
+        assert aj.attn_jvp_plan_device_status(plan) == 0
+        aj.attn_jvp_plan_destroy(plan)
+        outs[kernel] = (o.cpu(), lse.cpu())
+    zq, zk = np.zeros((Nq, 128), np.float32), np.zeros((Nk, 128), np.float32)
+    for h in range(2):
+        ro, _, rlse = oracle.attn_jvp_head(oracle.full_mask(), widen(q[0, h]), widen(k[0, h]), widen(v[0, h]), zq, zk, zk, 1.0 / np.sqrt(128))
+        for o, lse in outs.values():
+            assert max_norm_err(o[0, h].double().numpy(), ro) <= 1e-2
+            assert max_norm_err(lse[0, h].double().numpy(), rlse) <= 1e-3
 
 
 def test_ranges_mask_with_zero_flags_matches_oracle():
