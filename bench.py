@@ -372,7 +372,8 @@ def run_cuda(args, w: Workload):
         aj.attn_jvp_fwd(sp, *sx, so, sto, sl, stream.cuda_stream)
         aj.attn_bwd(sp, sx[0], sx[1], sx[2], so, sl, sx[3], *sg, stream.cuda_stream)
         torch.cuda.synchronize()
-        ts_f, ts_b = [], []
+        import ctypes
+        ts_f, ts_b, ts_c = [], [], []
         for i in range(1000):
             t0 = time.perf_counter_ns()
             aj.attn_jvp_fwd(sp, *sx, so, sto, sl, stream.cuda_stream)
@@ -382,11 +383,24 @@ def run_cuda(args, w: Workload):
             ts_f.append((t1 - t0) / 1e3); ts_b.append((t2 - t1) / 1e3)
             if i % 100 == 99:
                 torch.cuda.synchronize()
+        # the C ABI alone: arguments marshalled once, 1000 calls of the exported function itself
+        views = [aj.aj_tensor(t.data_ptr(), t.stride(0), t.stride(1), t.stride(2)) for t in (*sx, so, sto)]
+        refs = [ctypes.byref(v) for v in views]
+        fn, lse_p, st_p = aj.lib().attn_jvp_fwd, ctypes.c_void_p(sl.data_ptr()), ctypes.c_void_p(stream.cuda_stream)
+        for i in range(1000):
+            t0 = time.perf_counter_ns()
+            fn(sp, *refs, lse_p, st_p)
+            ts_c.append((time.perf_counter_ns() - t0) / 1e3)
+            if i % 100 == 99:
+                torch.cuda.synchronize()
         enc, hits = aj.attn_jvp_plan_tensor_map_stats(sp)
         aj.attn_jvp_plan_destroy(sp)
-        overhead_us = {"attn_jvp_fwd": statistics.median(ts_f), "attn_bwd": statistics.median(ts_b),
-                       "how": "median host time of 1000 calls through the ctypes binding (marshalling included) on a "
-                              "2-head, 512-token problem of the same kernels", "tensor_maps_encoded": enc, "tensor_map_cache_hits": hits}
+        overhead_us = {"attn_jvp_fwd_c_abi": statistics.median(ts_c), "attn_jvp_fwd_python_binding": statistics.median(ts_f),
+                       "attn_bwd_python_binding": statistics.median(ts_b),
+                       "how": "median host time of 1000 calls on a 2-head, 512-token problem of the same kernels: the exported C "
+                              "function with arguments marshalled once (ctypes foreign-call cost included), and the Python "
+                              "binding (argument checks and marshalling per call)",
+                       "tensor_maps_encoded": enc, "tensor_map_cache_hits": hits}
 
     # ---- parity of what was just timed: the device outputs of head (0, 0) against the oracle rows of the cpu_baseline leg
     parity = None
@@ -422,7 +436,7 @@ def run_cuda(args, w: Workload):
         "ms_per_step": total_ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "config": workload_config(w),
         "tokens_per_s": world * w.B * w.num_queries / (total_ms_all / K * 1e-3),
-        "kernel": {1: "simt_fp32", 2: "tcgen05_umma", 3: "tcgen05_umma_cta_pair"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
+        "kernel": {1: "simt_fp32", 2: "tcgen05_umma", 3: "tcgen05_umma_cta_pair", 4: "tcgen05_umma_cta_pair_one_launch"}[kernel], "num_tasks": num_tasks, "plan_create_ms": plan_ms,
         "ms_per_launch": {"mean": avg_launch_ms, "median": statistics.median(per_launch), "min": min(per_launch)},
         "e2e": {"value": e2e_flops_all / (e2e_ms_all * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_all / K,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -433,15 +447,29 @@ def run_cuda(args, w: Workload):
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": f"{peak_src} bf16_tflops (burst cuBLAS GEMM)",
                      "frac_of_sustained": achieved / sustained, "frac_of_nominal_2250": achieved / 2250.0,
-                     "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 3: "attn_jvp_umma_pair_kernel"}[kernel],
+                     "kernel": {1: "attn_jvp_simt_kernel", 2: "attn_jvp_umma_kernel", 4: "attn_jvp_umma_pair_kernel",
+                                3: ("attn_fwd_umma_pair_kernel" if w.no_tangents else
+                                    "attn_fwd_umma_pair_kernel (primal-only tasks) + attn_jvp_umma_pair_kernel" if w.clean_tangent_zero
+                                    else "attn_jvp_umma_pair_kernel")}[kernel],
                      "flops_per_launch": flops},
     }
+    if kernel == 1:
+        # plain-FMA kernels (fp32 inputs, or bf16 with d = 64): bound by fp32 FMA issue, not by the tensor pipe.  Peak from the
+        # unit counts and the maximum SM clock: SMs x 128 fp32 lanes x 2 flop x f.
+        props = torch.cuda.get_device_properties(local)
+        f_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+        alu_peak = props.multi_processor_count * 128 * 2 * f_max * 1e6 / 1e12
+        line["roofline"].update(bound="alu", peak=alu_peak, frac=achieved / alu_peak,
+                                peak_source=f"derived: {props.multi_processor_count} SMs x 128 fp32 lanes x 2 flop x {f_max:.0f} MHz",
+                                note="counted flop are the six length-d contractions only; the kernel also spends FMA issue slots "
+                                     "on the softmax and on shared-memory address arithmetic")
+        del line["roofline"]["frac_of_sustained"], line["roofline"]["frac_of_nominal_2250"]
     if w.backward:
         # three kernels per step, timed together: delta (HBM-bound, small), the dQ pass and the dK/dV pass of the tcgen05
         # backward kernel (bf16, d = 128).  The 10*d convention counts the minimal five contractions;
         # the two-pass kernel executes seven (S and dP are recomputed in the second pass).
-        line["kernel"] = "tcgen05_backward_two_pass" if (w.dtype == "bf16" and w.d == 128) else "simt_fp32_backward"
-        line["roofline"].update(kernel="attn_bwd_umma_kernel<false> (dQ) + attn_bwd_umma_kernel<true> (dK, dV) + attn_bwd_delta_kernel",
+        line["kernel"] = "tcgen05_backward_two_pass_cta_pairs" if (w.dtype == "bf16" and w.d == 128) else "simt_fp32_backward"
+        line["roofline"].update(kernel="attn_bwd_umma_pair_kernel<false> (dQ) + attn_bwd_umma_pair_kernel<true> (dK, dV) + attn_bwd_delta_kernel",
                                 executed_over_counted_contractions=7.0 / 5.0)
     if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12

@@ -59,6 +59,9 @@ struct aj_plan {
     };
     mutable std::mutex mu;
     mutable std::vector<MapSlot> maps;
+    mutable CUtensorMap ld_map;                 // 1-D map over the backward's {lse log2e, delta} workspace
+    mutable const float *ld_map_ptr = nullptr;
+    mutable int64_t ld_map_floats = 0;
     mutable int64_t map_encodes = 0, map_hits = 0;
 };
 
@@ -501,7 +504,9 @@ aj_status ensure_bwd_schedules(aj_plan *p, const aj_problem &prob, BwdFamily fam
     return AJ_OK;
 }
 
-aj_status encode_ld_map(CUtensorMap *map, const float *ld, int64_t floats) {
+aj_status encode_ld_map(const aj_plan *plan, CUtensorMap *map, const float *ld, int64_t floats) {
+    std::lock_guard<std::mutex> lock(plan->mu);
+    if (plan->ld_map_ptr == ld && plan->ld_map_floats == floats) { *map = plan->ld_map; ++plan->map_hits; return AJ_OK; }
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
     cuuint64_t dims[1] = {(cuuint64_t)floats};
@@ -510,6 +515,8 @@ aj_status encode_ld_map(CUtensorMap *map, const float *ld, int64_t floats) {
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 1, (void *)ld, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (lse / delta map) failed with CUresult " + std::to_string((int)r));
+    plan->ld_map = *map; plan->ld_map_ptr = ld; plan->ld_map_floats = floats;
+    ++plan->map_encodes;
     return AJ_OK;
 }
 
@@ -551,7 +558,7 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
             if (keys) {
                 if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
                 if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
-                if ((st = encode_ld_map(&up.tm_ld, work, 2 * (int64_t)pr.B * pr.H * pr.Nq))) return st;
+                if ((st = encode_ld_map(p, &up.tm_ld, work, 2 * (int64_t)pr.B * pr.H * pr.Nq))) return st;
             }
             if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
             if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;

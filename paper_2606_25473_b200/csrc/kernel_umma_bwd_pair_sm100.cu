@@ -61,6 +61,10 @@ constexpr uint32_t LD_BOX_FLOATS = 2 * (BC + 2);   // 132 floats = 528 B
 constexpr uint32_t LD_TILE_BYTES = 640;            // 528 rounded up to 128 B
 constexpr uint32_t LD_STAGE_BYTES = 2 * LD_TILE_BYTES;
 constexpr int NTHREADS = 384;
+#ifndef AJ_BWD_POLY_EXP
+#define AJ_BWD_POLY_EXP 0
+#endif
+constexpr bool POLY_EXP = AJ_BWD_POLY_EXP != 0;      // every other column pair's exponential on the FMA pipe (measured: DESIGN.md 6d)
 
 template <bool KEYS> struct Cfg {
     static constexpr int NSTAGE = KEYS ? 4 : 6;                          // ring slots of 32 KB
@@ -418,10 +422,14 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         uint64_t nl = myl_2;
                         if (KEYS) { const float4 f = ld2(32 * hb + c); nl = pack2(-f.x, -f.z); }
                         const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl);
-                        float x0, x1;
-                        unpack2(x, x0, x1);
-                        w[32 * hb + c] = ex2(x0);
-                        w[32 * hb + c + 1] = ex2(x1);
+                        if (POLY_EXP && ((c >> 1) & 1)) {      // every other column pair on the FMA pipe instead of the MUFU pipe
+                            unpack2(ex2_poly2(x), w[32 * hb + c], w[32 * hb + c + 1]);
+                        } else {
+                            float x0, x1;
+                            unpack2(x, x0, x1);
+                            w[32 * hb + c] = ex2(x0);
+                            w[32 * hb + c + 1] = ex2(x1);
+                        }
                     }
                 }
                 if (!KEYS) {                                   // X(p) is in registers: X(p+1) may overwrite it

@@ -13,8 +13,12 @@
 //   step overlap the load / max / store phases of the next.  A row's lazy reference max (PAPER.md:916-927 applied only when
 //   the tile max exceeds it by 2^8) is handed from the warp that decided it for step g to its twin in the other warpgroup
 //   through shared memory and a 64-thread named barrier; each warpgroup sums its own share of l and the two are combined
-//   (rescaled to the final reference) in the epilogue.  S is read from TMEM twice (max pass, exponential pass) in 32-column
-//   chunks, which keeps the role under the 168 registers that 384 threads allow.
+//   (rescaled to the final reference) in the epilogue.  Tile j0 of a step is read from TMEM twice (max pass, exponential
+//   pass) and tile j1 once (it stays in registers across the reference-max decision), which keeps the role under the 168
+//   registers that 384 threads allow with three TMEM round trips per step; tile j1 is handed to the MMA warp first.
+//   Every other column pair takes its exponential from the FMA pipe (ptx::ex2_poly2): at d = 128 a tangent-free pair-step is
+//   1024 clk of tensor work against 128 x 128 exponentials = 1024 clk of the 16-lane/clk MUFU pipe, so the MUFU pipe alone
+//   would cap the kernel at the tensor roofline with no slack at all.
 // Roles per CTA: warp 0 TMA producer, warp 1 MMA issuer (leader CTA), warp 2 TMEM allocator, warps 4-11 softmax / epilogue.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -50,6 +54,10 @@ constexpr int NTHREADS = 384;
 
 constexpr uint32_t TM_O = 0, TM_S = 128;           // S buffer b at TM_S + 128 b; P~(j_i) over the first 32 columns of its tile's 64
 constexpr float RESCALE_THRESHOLD = 8.0f;          // log2 units
+#ifndef AJ_FWD_POLY_EXP
+#define AJ_FWD_POLY_EXP 0
+#endif
+constexpr bool POLY_EXP = AJ_FWD_POLY_EXP != 0;      // every other column pair's exponential on the FMA pipe (measured: DESIGN.md 6c)
 constexpr float M_UNSET = -1.0e30f;
 
 enum {
@@ -212,10 +220,11 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     wait(BAR_KV_FULL + vslot, (item / NSTAGE) & 1);
                     const uint32_t v_lo = (((sRing + vslot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
 #pragma unroll
-                    for (int i = 0; i < 2; ++i) {
+                    for (int ii = 0; ii < 2; ++ii) {
+                        const int i = 1 - ii;                        // the softmax hands over tile j1 first (it keeps S(j1) in registers)
                         const uint32_t vi_lo = v_lo + ((i * BLK_BYTES) >> 4);
                         const uint32_t tP = tmem + TM_S + 128 * buf + i * BC;
-                        const uint32_t acc = (p > 0 || i > 0) ? 1u : 0u;
+                        const uint32_t acc = (p > 0 || ii > 0) ? 1u : 0u;
                         wait(BAR_P_FULL + 2 * buf + i, (g / NSBUF) & 1);
                         tc_fence_after();
                         if (leader) {
@@ -267,22 +276,28 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 const uint32_t tS = tmem + lane_base + TM_S + 128 * buf;
                 wait(BAR_S_FULL + buf, (g / NSBUF) & 1);
                 tc_fence_after();
-                // ---- pass 1: the pair-step's row max over the columns this row may see
+                // ---- pass 1: the pair-step's row max over the columns this row may see.  Tile j0 is read for its
+                // max alone and read again in pass 2; tile j1 stays in registers (64 + 64 values would not fit beside the rest).
                 float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+                auto load_tile = [&](int i, uint32_t (&a)[32], uint32_t (&b)[32]) {
+                    tmem_ld32(tS + 64 * i, a);
+                    tmem_ld32(tS + 64 * i + 32, b);
+                    tc_wait_ld(a, b);
+                    if (valid[i] < BC) {                            // outside the entry's keys / row interval: S = -inf (P~ = 0)
 #pragma unroll
-                for (int ch = 0; ch < 4; ++ch) {
-                    uint32_t su[32];
-                    tmem_ld32(tS + 32 * ch, su);
-                    tc_wait_ld(su);
-                    const int v = valid[ch >> 1] - 32 * (ch & 1);      // columns of this chunk the row sees
-                    if (v >= 32) {
-#pragma unroll
-                        for (int c = 0; c < 32; ++c) mx[c & 3] = fmaxf(mx[c & 3], __uint_as_float(su[c]));
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 32; ++c) if (c < v) mx[c & 3] = fmaxf(mx[c & 3], __uint_as_float(su[c]));
+                        for (int c = 0; c < 32; ++c) { if (c >= valid[i]) a[c] = 0xff800000u; if (c + 32 >= valid[i]) b[c] = 0xff800000u; }
                     }
+                };
+                uint32_t s1a[32], s1b[32];
+                {
+                    uint32_t s0a[32], s0b[32];
+                    load_tile(0, s0a, s0b);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) { mx[c & 1] = fmaxf(mx[c & 1], __uint_as_float(s0a[c])); mx[2 + (c & 1)] = fmaxf(mx[2 + (c & 1)], __uint_as_float(s0b[c])); }
                 }
+                load_tile(1, s1a, s1b);
+#pragma unroll
+                for (int c = 0; c < 32; ++c) { mx[c & 1] = fmaxf(mx[c & 1], __uint_as_float(s1a[c])); mx[2 + (c & 1)] = fmaxf(mx[2 + (c & 1)], __uint_as_float(s1b[c])); }
                 const float cand = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * sl2;
                 // ---- the reference max: taken over from the twin warp (step g - 1), moved only if this step's max exceeds it by 2^8
                 if (p > 0) {
@@ -325,36 +340,41 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     sh->mref[g & 1][row] = m_ref;
                     named_bar_arrive(1 + 2 * q4 + (int)(g & 1), 64);
                 }
-                // ---- pass 2: P~ = exp2(S s log2e - m_ref); l += rowsum; bf16 P~ over the tile's first 32 columns
+                // ---- pass 2: P~ = exp2(S s log2e - m_ref); l += rowsum; bf16 P~ over the tile's first 32 columns.
+                // Every other column pair takes its exponential from the FMA pipe (ex2_poly2) instead of the MUFU pipe; tiles with
+                // masked columns use the MUFU alone (exp2(-inf) = 0 exactly).
                 const uint64_t negm2 = pack2(-m_ref, -m_ref);
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
+                auto exp_tile = [&](int i, const uint32_t (&a)[32], const uint32_t (&b)[32]) {
                     uint32_t pk[32];
+                    const bool whole = valid[i] == BC;
 #pragma unroll
-                    for (int hb = 0; hb < 2; ++hb) {
-                        uint32_t su[32];
-                        tmem_ld32(tS + 64 * i + 32 * hb, su);
-                        tc_wait_ld(su);
-                        const int v = valid[i] - 32 * hb;
-                        if (v < 32) {
-#pragma unroll
-                            for (int c = 0; c < 32; ++c) if (c >= v) su[c] = 0xff800000u;      // -inf: P~ = 0
-                        }
-#pragma unroll
-                        for (int c = 0; c < 32; c += 2) {
-                            const uint64_t x = ffma2(pack2(su[c], su[c + 1]), sl2_2, negm2);
+                    for (int c = 0; c < 64; c += 2) {
+                        const uint32_t u0 = c < 32 ? a[c & 31] : b[c & 31], u1 = c < 32 ? a[(c + 1) & 31] : b[(c + 1) & 31];
+                        const uint64_t x = ffma2(pack2(u0, u1), sl2_2, negm2);
+                        uint64_t e;
+                        if (POLY_EXP && ((c >> 1) & 1) && whole) {
+                            e = ex2_poly2(x);
+                        } else {
                             float x0, x1;
                             unpack2(x, x0, x1);
-                            const float p0 = ex2(x0), p1 = ex2(x1);
-                            l2[(c >> 1) & 1] = fadd2(l2[(c >> 1) & 1], pack2(p0, p1));
-                            pk[16 * hb + (c >> 1)] = pack_bf16(p0, p1);
+                            e = pack2(ex2(x0), ex2(x1));
                         }
+                        l2[(c >> 1) & 1] = fadd2(l2[(c >> 1) & 1], e);
+                        float p0, p1;
+                        unpack2(e, p0, p1);
+                        pk[c >> 1] = pack_bf16(p0, p1);
                     }
                     tmem_st32(tS + 64 * i, pk);
                     tc_wait_st();
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * (BAR_P_FULL + 2 * buf + i));
+                };
+                exp_tile(1, s1a, s1b);                              // from registers
+                {
+                    uint32_t s0a[32], s0b[32];
+                    load_tile(0, s0a, s0b);
+                    exp_tile(0, s0a, s0b);
                 }
             }
             // ---- epilogue: O / l, lse = m + log l; each warpgroup writes one 64-column half ----
