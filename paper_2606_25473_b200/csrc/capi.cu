@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -39,7 +40,9 @@ struct aj_plan {
     // primal backward: query tiles x key ranges (dQ) and key tiles x row ranges (dK, dV) for all B x H heads, and for ONE
     // head (attn_bwd_host)
     DevSchedule bwd_q, bwd_k, bwd_q_head, bwd_k_head;
-    float *d_delta = nullptr;     // [B, H, Nq] workspace of attn_bwd
+    float *d_delta = nullptr;     // workspace of attn_bwd (bwd_alloc_bytes)
+    int32_t bwd_poly_exp = 0;     // AJ_BWD_POLY_EXP env (A/B runs): half of the backward's exponentials on the FMA pipe
+    int32_t bwd_dq_form = 0;      // dQ pass of the CTA-pair backward: 0 = tile ping-pong, 1 = pair-step form (AJ_BWD_DQ_FORM env, for A/B runs)
     // attn_jvp_fwd_host / attn_bwd_host: device staging buffers, copy streams, one event per head and direction
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // q k v tq tk tv
     void *d_out[2] = {nullptr, nullptr};                                      // o to
@@ -59,9 +62,9 @@ struct aj_plan {
     };
     mutable std::mutex mu;
     mutable std::vector<MapSlot> maps;
-    mutable CUtensorMap ld_map;                 // 1-D map over the backward's {lse log2e, delta} workspace
-    mutable const float *ld_map_ptr = nullptr;
-    mutable int64_t ld_map_floats = 0;
+    mutable CUtensorMap aug_map[2];             // 2-D maps over the backward's augmentation rows (-lse/s, -delta)
+    mutable const void *aug_map_ptr = nullptr;
+    mutable int64_t aug_map_rows = 0;
     mutable int64_t map_encodes = 0, map_hits = 0;
 };
 
@@ -291,6 +294,8 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         e = cudaMalloc(&p->d_counters, 4 * sizeof(int32_t));
         if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
+        if (const char *f = std::getenv("AJ_BWD_DQ_FORM")) p->bwd_dq_form = std::atoi(f) == 1 ? 1 : 0;
+        if (const char *f = std::getenv("AJ_BWD_POLY_EXP")) p->bwd_poly_exp = std::atoi(f) == 1 ? 1 : 0;
         const int32_t kernel = auto_kernel(p->problem);
         st = install_schedule(p, kernel, default_tiling(kernel));
     } catch (const std::bad_alloc &) {
@@ -470,13 +475,12 @@ aj_status attn_fwd(const aj_plan *p, const aj_tensor *q, const aj_tensor *k, con
 namespace {
 
 // Which kernels the backward runs: plain FMA (fp32, d = 64, or a plan forced to SIMT), the single-CTA tcgen05 kernel (a plan
-// forced to AJ_KERNEL_UMMA, or a problem too large for the pair kernel's 1-D {lse, delta} map), or CTA pairs (default).
+// forced to AJ_KERNEL_UMMA), or CTA pairs (default).
 enum BwdFamily { BWD_SIMT = 0, BWD_UMMA = 1, BWD_PAIR = 2 };
 BwdFamily bwd_family(const aj_plan *p) {
     if (!umma_covers(p->problem) || p->kernel == AJ_KERNEL_SIMT) return BWD_SIMT;
     if (p->kernel == AJ_KERNEL_UMMA) return BWD_UMMA;
-    const int64_t ld_floats = 2 * (int64_t)p->problem.B * p->problem.H * p->problem.Nq;
-    return ld_floats + 256 < (int64_t)1 << 31 ? BWD_PAIR : BWD_UMMA;
+    return BWD_PAIR;
 }
 
 // The backward schedules of `prob` (the plan's problem, or one head of it): query tiles x key ranges (dQ) and key tiles x
@@ -504,25 +508,41 @@ aj_status ensure_bwd_schedules(aj_plan *p, const aj_problem &prob, BwdFamily fam
     return AJ_OK;
 }
 
-aj_status encode_ld_map(const aj_plan *plan, CUtensorMap *map, const float *ld, int64_t floats) {
+// Backward workspace of `rows` = B * H * Nq query rows: [delta: rows floats] for the SIMT and single-CTA kernels; for the CTA
+// pairs [{lse log2e, delta}: rows float2, padded to 16 B][aug rows of -lse/s: rows x 32 B][aug rows of -delta: rows x 32 B].
+size_t bwd_ld_bytes(int64_t rows) { return ((size_t)rows * 8 + 15) & ~(size_t)15; }
+size_t bwd_work_bytes(int64_t rows) { return bwd_ld_bytes(rows) + (size_t)rows * 64; }
+// what a plan allocates: enough for one call over all heads and for B * H per-head calls (attn_bwd_host)
+size_t bwd_alloc_bytes(const aj_problem &pr) {
+    return std::max(bwd_work_bytes((int64_t)pr.B * pr.H * pr.Nq), bwd_work_bytes(pr.Nq) * (size_t)pr.B * pr.H);
+}
+
+// 2-D maps over the two aug arrays ([rows][16] bf16 each, box {16, 64}); cached in the plan by workspace pointer
+aj_status encode_aug_maps(const aj_plan *plan, CUtensorMap *m1, CUtensorMap *m2, const void *aug, int64_t rows) {
     std::lock_guard<std::mutex> lock(plan->mu);
-    if (plan->ld_map_ptr == ld && plan->ld_map_floats == floats) { *map = plan->ld_map; ++plan->map_hits; return AJ_OK; }
-    EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    cuuint64_t dims[1] = {(cuuint64_t)floats};
-    cuuint64_t strides[1] = {0};
-    cuuint32_t box[1] = {132}, estr[1] = {1};   // 66 rows of {lse log2e, delta}: see LD_BOX_FLOATS in the kernel
-    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 1, (void *)ld, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (lse / delta map) failed with CUresult " + std::to_string((int)r));
-    plan->ld_map = *map; plan->ld_map_ptr = ld; plan->ld_map_floats = floats;
-    ++plan->map_encodes;
+    if (plan->aug_map_ptr != aug || plan->aug_map_rows != rows) {
+        EncodeTiledFn fn = encode_tiled_fn();
+        if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+        for (int i = 0; i < 2; ++i) {
+            cuuint64_t dims[2] = {16, (cuuint64_t)rows};
+            cuuint64_t strides[1] = {32};
+            cuuint32_t box[2] = {16, 64}, estr[2] = {1, 1};
+            CUresult r = fn(&plan->aug_map[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (char *)aug + (size_t)i * rows * 32, dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) { plan->aug_map_ptr = nullptr; return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (augmentation rows) failed with CUresult " + std::to_string((int)r)); }
+        }
+        plan->aug_map_ptr = aug; plan->aug_map_rows = rows;
+        plan->map_encodes += 2;
+    } else {
+        plan->map_hits += 2;
+    }
+    *m1 = plan->aug_map[0]; *m2 = plan->aug_map[1];
     return AJ_OK;
 }
 
 // The kernels of one backward call over the tasks of (bq, bk), which were built for a [B, H] problem.
-// ts = {q, k, v, o, dout, dq, dk, dv}; lse: [B, H, Nq] of that problem; work: [B, H, Nq] floats (delta) for the SIMT and
-// single-CTA kernels, 2 x that ({lse log2e, delta} pairs) for the CTA-pair kernels; `slot`: first of eight tensor-map slots.
+// ts = {q, k, v, o, dout, dq, dk, dv}; lse: [B, H, Nq] of that problem; work: bwd_work_bytes(B * H * Nq) bytes;
+// `slot`: first of eight tensor-map slots.
 aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_plan::DevSchedule &bk, int32_t B, int32_t H,
                      const aj_tensor *const ts[8], const float *lse, float *work, cudaStream_t stream, int slot) {
     aj_problem pr = p->problem;
@@ -533,7 +553,10 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
     prm.q = *q; prm.k = *k; prm.v = *v; prm.o = *o; prm.dout = *dout; prm.dq = *dq; prm.dk = *dk; prm.dv = *dv;
     prm.lse = lse;
     prm.delta = fam == BWD_PAIR ? nullptr : work;
+    const int64_t rows = (int64_t)pr.B * pr.H * pr.Nq;
+    void *aug = (char *)work + bwd_ld_bytes(rows);
     prm.ld = fam == BWD_PAIR ? (float2 *)work : nullptr;
+    prm.aug = fam == BWD_PAIR ? (uint4 *)aug : nullptr;
     prm.q_tasks = bq.d_tasks; prm.q_kb = bq.d_kb; prm.q_ke = bq.d_ke;
     prm.k_tasks = bk.d_tasks; prm.k_rb = bk.d_kb; prm.k_re = bk.d_ke;
     prm.B = pr.B; prm.H = pr.H; prm.Nq = pr.Nq; prm.scale = pr.scale;
@@ -558,10 +581,16 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
             if (keys) {
                 if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
                 if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
-                if ((st = encode_ld_map(p, &up.tm_ld, work, 2 * (int64_t)pr.B * pr.H * pr.Nq))) return st;
+                if ((st = encode_aug_maps(p, &up.tm_aug1, &up.tm_aug2, aug, rows))) return st;
             }
             if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
             if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
+            if (!keys) {   // the dQ pass stages half a streamed tile (32 rows) per CTA for X and Y: cache slots of the unused a1, a2
+                if ((st = encode_map(p, slot + 0, &up.tm_b1h, *b1, pr, nb, aj::UMMA_TILE_K / 2))) return st;
+                if ((st = encode_map(p, slot + 1, &up.tm_b2h, *b2, pr, nb, aj::UMMA_TILE_K / 2))) return st;
+                up.dq_form = p->bwd_dq_form;
+            }
+            up.poly_exp = p->bwd_poly_exp;
             up.a1 = *a1; up.a2 = *a2;
             up.out1 = keys ? *dk : *dq;
             up.out2 = *dv;
@@ -637,7 +666,7 @@ aj_status attn_bwd(aj_plan *p, const aj_tensor *q, const aj_tensor *k, const aj_
     // first use: the two schedules and the delta workspace (synchronous host work and allocations)
     if (aj_status st = ensure_bwd_schedules(p, p->problem, fam, p->bwd_q, p->bwd_k)) return st;
     if (!p->d_delta) {
-        cudaError_t e = cudaMalloc(&p->d_delta, 2 * (size_t)pr.B * pr.H * pr.Nq * sizeof(float));   // delta, or {lse log2e, delta}
+        cudaError_t e = cudaMalloc(&p->d_delta, bwd_alloc_bytes(pr));
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the backward workspace") : cuda_fail(e, "workspace allocation");
     }
     return launch_bwd(p, p->bwd_q, p->bwd_k, pr.B, pr.H, ts, lse, p->d_delta, (cudaStream_t)cuda_stream, SLOT_BWD);
@@ -653,7 +682,7 @@ aj_status attn_bwd_host(aj_plan *p, const void *q, const void *k, const void *v,
     const int nheads = pr.B * pr.H;
     const size_t hq = (size_t)pr.Nq * pr.d * eb, hk = (size_t)pr.Nk * pr.d * eb;     // one head of a tensor
     const size_t nq_bytes = hq * nheads, nk_bytes = hk * nheads, lse_bytes = (size_t)nheads * pr.Nq * sizeof(float);
-    const size_t work_bytes = 2 * lse_bytes;
+    const size_t head_work = bwd_work_bytes(pr.Nq), work_bytes = bwd_alloc_bytes(pr);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     {   // staging: q k v (shared with the forward) | o | dout dq dk dv | lse | delta / {lse log2e, delta}
         const size_t in_bytes[3] = {nq_bytes, nk_bytes, nk_bytes}, bwd_bytes[4] = {nq_bytes, nq_bytes, nk_bytes, nk_bytes};
@@ -697,7 +726,7 @@ aj_status attn_bwd_host(aj_plan *p, const void *q, const void *k, const void *v,
             ts[i] = &t[i];
         }
         if (aj_status st = launch_bwd(p, p->bwd_q_head, p->bwd_k_head, 1, 1, ts, p->d_lse + (size_t)hd * pr.Nq,
-                                      p->d_delta + 2 * (size_t)hd * pr.Nq, stream, SLOT_HEAD + hd * SLOTS_PER_HEAD + 8)) return st;
+                                      (float *)((char *)p->d_delta + hd * head_work), stream, SLOT_HEAD + hd * SLOTS_PER_HEAD + 8)) return st;
         e = cudaEventRecord(p->ev_k[hd], stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_out, p->ev_k[hd], 0);
         for (int i = 0; i < 3 && e == cudaSuccess; ++i) {

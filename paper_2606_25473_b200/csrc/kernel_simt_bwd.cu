@@ -48,7 +48,22 @@ __global__ void __launch_bounds__(128) attn_bwd_delta_kernel(BwdParams prm) {
     for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
     if (lane == 0) {
         if (prm.delta) prm.delta[row] = acc;
-        if (prm.ld) prm.ld[row] = make_float2(prm.lse[row] * 1.4426950408889634f, acc);   // what the CTA-pair passes consume
+        if (prm.ld) prm.ld[row] = make_float2(prm.lse[row] * 1.4426950408889634f, acc);   // what the CTA-pair dQ pass consumes
+        if (prm.aug) {
+            // the 16 extra K columns of the CTA-pair dK/dV pass: v = h + l in bf16 (16 mantissa bits), stored halved in BOTH
+            // 16-byte halves of the row (the constant A operand has ones at the same four positions): sum = v
+            const float lse = prm.lse[row];
+            const float v[2] = {lse == -CUDART_INF_F ? 0.f : -lse / prm.scale, -acc};   // rows without keys are never unmasked
+            for (int i = 0; i < 2; ++i) {
+                const __nv_bfloat16 h = __float2bfloat16_rn(v[i]);
+                const __nv_bfloat16 l = __float2bfloat16_rn(v[i] - __bfloat162float(h));
+                const __nv_bfloat16 h2 = __float2bfloat16_rn(0.5f * __bfloat162float(h)), l2 = __float2bfloat16_rn(0.5f * __bfloat162float(l));
+                const uint32_t w = (uint32_t)__bfloat16_as_ushort(h2) | ((uint32_t)__bfloat16_as_ushort(l2) << 16);
+                uint4 *dst = prm.aug + ((int64_t)i * total + row) * 2;
+                dst[0] = make_uint4(w, 0u, 0u, 0u);
+                dst[1] = make_uint4(w, 0u, 0u, 0u);
+            }
+        }
     }
 }
 

@@ -9,20 +9,24 @@
 //   pair-step = TWO 64-row STREAMED tiles j0, j1 of the task's stream (CTA c stages tile j_c for the K-major operands and
 //               the column half [64 c, 64 c + 64) of both tiles for the MN-major operands)
 //     [X(j0) | X(j1)] = A1 [B1(j0) ; B1(j1)]^T,   [Y(j0) | Y(j1)] = A2 [B2(j0) ; B2(j1)]^T        2 x 8 x (M256 N128 K16)
-//     W = exp2(X s log2e - lse log2e),   Z = W o (Y - delta)       two exp / dS warpgroups, one streamed tile each,
-//                                                                    thread = stationary row = TMEM lane
+//     W = exp2(X s log2e - lse log2e),   Z = W o (Y - delta)       two exp / dS warpgroups, 32 of a tile's 64 columns each,
+//                                                                    tile j0 first; thread = stationary row = TMEM lane
 //     per tile: acc1 += Z B1  (and acc2 += W B2)                    4 (+ 4) x (M256 N128 K16), A = bf16 Z / W in TMEM
 //   KEYS = false (dQ):     stationary = query rows (A1 = Q, A2 = dO), streamed = keys (B1 = K, B2 = V); acc1 = dQ / s; lse and
 //                          delta belong to the thread's own row.  Q and dO rows live in TMEM as bf16 A operands (written by
 //                          the exp / dS warps once per task), so the X / Y MMAs read only B from shared memory.
 //   KEYS = true (dK, dV):  stationary = keys (A1 = K, A2 = V in shared memory), streamed = query rows (B1 = Q, B2 = dO):
-//                          X = S^T, Y = dP^T, acc1 = dK / s, acc2 = dV; lse and delta belong to the COLUMNS: the delta kernel
-//                          leaves them interleaved as float2 {lse log2e, delta}, and the producer brings 64 of them per tile
-//                          into shared memory with a 1-D TMA load.  Tasks come from the transposed mask (keys x row ranges).
+//                          X = S^T, Y = dP^T, acc1 = dK / s, acc2 = dV; lse and delta belong to the COLUMNS, and they are
+//                          folded INTO the two contractions: one extra K step (16 of the bf16 K dimension) multiplies a
+//                          constant block of ones (A) with 16 extra columns per streamed row (B) that the delta kernel
+//                          wrote: -lse/s (resp. -delta) split into bf16 hi + lo, so that the tensor pipe delivers
+//                          X = <k, q> - lse/s and Y = <v, dO> - delta and the exp / dS warps read nothing per column
+//                          (a shared-memory copy of lse / delta read by every thread cost 41 % of the shared-memory port
+//                          and doubled the role's instruction count).  Tasks come from the transposed mask.
 // S and dP are computed in both passes (7 contractions for the minimal 5): a single pass would need dK, dV, S^T, dP^T and a
 // 128-column dQ partial = 640 TMEM columns and a cross-CTA reduction of dQ; DESIGN.md section 6d.
 // TMEM (512 columns per CTA):  acc1 128 | acc2 128 (KEYS) or bf16 A1 64 + A2 64 (dQ pass) | X(j0) X(j1) 128 | Y(j0) Y(j1) 128;
-// bf16 W / Z overwrite the first 32 columns of their tile's X / Y.  X / Y are single-buffered; as in the forward the overlap
+// bf16 W / Z of a tile's streamed rows [32 h, 32 h + 32) overwrite columns [32 h, 32 h + 16) of the tile's X / Y.  X / Y are single-buffered; as in the forward the overlap
 // comes from the issue order on the in-order tensor pipe:
 //   KEYS:  W(j0) B2, W(j1) B2, X(p+1) [overwrites W], Z(j0) B1, Z(j1) B1, Y(p+1) [overwrites Z]
 //   dQ:    X(p+1) [once the exp warps have LOADED X(p): X_FREE], Z(j0) B1, Z(j1) B1, Y(p+1)
@@ -54,12 +58,14 @@ constexpr uint32_t A_BYTES = BR * D * 2;           // 32 KB
 constexpr uint32_t AHALF_BYTES = BR * 64 * 2;      // one 64-column swizzle block of a stationary operand: 16 KB
 constexpr uint32_t BLK_BYTES = BC * 64 * 2;        // 8 KB: 64 streamed rows x 64 columns, 128-byte swizzled rows
 constexpr uint32_t SLOT_BYTES = 4 * BLK_BYTES;     // 32 KB
-constexpr int LD_STAGES = 4;                       // KEYS: {lse log2e, delta} of both tiles of a pair-step
-// A TMA tile must start on a 16-byte boundary of global memory, a row's float2 only guarantees 8: the load starts at the
-// even row at or below the tile's first row and brings 66 rows; `ld_shift` tells the readers whether to skip one.
-constexpr uint32_t LD_BOX_FLOATS = 2 * (BC + 2);   // 132 floats = 528 B
-constexpr uint32_t LD_TILE_BYTES = 640;            // 528 rounded up to 128 B
-constexpr uint32_t LD_STAGE_BYTES = 2 * LD_TILE_BYTES;
+// KEYS: the K-augmentation operands.  A row of an aug array is 16 bf16 = 32 B: [h/2, l/2, 0 x 6, h/2, l/2, 0 x 6] with
+// h + l = the folded value (both 16-byte halves alike, so no swizzle pattern can matter); the constant A block is 128 rows of
+// [1, 1, 0 x 6, 1, 1, 0 x 6].  Both are read through K-major descriptors of the 32-byte-swizzle kind: rows 32 B apart, 8-row
+// groups 256 B apart.
+constexpr uint32_t AUG_TILE_BYTES = BC * 32;       // 2 KB: 64 streamed rows
+constexpr uint32_t AUG_STAGE_BYTES = 2 * AUG_TILE_BYTES;   // q-aug and dO-aug of this CTA's tile
+constexpr int AUG_STAGES = 2;                      // one per ring slot that can hold a {B1, B2} tile (slots 0 and 2 of 4)
+constexpr uint32_t ONES_BYTES = BR * 32;           // 4 KB
 constexpr int NTHREADS = 384;
 #ifndef AJ_BWD_POLY_EXP
 #define AJ_BWD_POLY_EXP 0
@@ -69,8 +75,8 @@ constexpr bool POLY_EXP = AJ_BWD_POLY_EXP != 0;      // every other column pair'
 template <bool KEYS> struct Cfg {
     static constexpr int NSTAGE = KEYS ? 4 : 6;                          // ring slots of 32 KB
     static constexpr uint32_t A_SMEM = KEYS ? 2 * A_BYTES : 0;           // stationary operands in shared memory (KEYS only)
-    static constexpr uint32_t LD_SMEM = KEYS ? LD_STAGES * LD_STAGE_BYTES : 0;
-    static constexpr uint32_t SMEM_TILES = A_SMEM + NSTAGE * SLOT_BYTES + LD_SMEM;
+    static constexpr uint32_t AUG_SMEM = KEYS ? AUG_STAGES * AUG_STAGE_BYTES + ONES_BYTES : 0;
+    static constexpr uint32_t SMEM_TILES = A_SMEM + NSTAGE * SLOT_BYTES + AUG_SMEM;
     static constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 512 /*barriers*/;
 };
 
@@ -88,8 +94,7 @@ enum {
     BAR_W_FULL,                             // leader, x2 (tile): W stored by the tile's warpgroup in both CTAs (KEYS)
     BAR_Z_FULL = BAR_W_FULL + 2,            // leader, x2
     BAR_ACC_DONE = BAR_Z_FULL + 2,          // both: every MMA into acc1 / acc2 of the pair-step is complete
-    BAR_LD_FULL,                            // own CTA, x LD_STAGES: the pair-step's {lse, delta} landed (KEYS)
-    NUM_BARS = BAR_LD_FULL + LD_STAGES
+    NUM_BARS
 };
 
 // Instruction descriptor, kind::f16: D fp32, A and B bf16, N >> 3 at bit 17, M >> 4 at bit 24 (M = 256 over the pair).
@@ -100,20 +105,20 @@ constexpr uint32_t IDESC_XY = make_idesc(2 * BC, false);   // 256 x 128 x 16, B 
 constexpr uint32_t IDESC_ACC = make_idesc(D, true);        // 256 x 128 x 16, A from TMEM, B MN-major (64 columns per CTA)
 constexpr uint32_t DESC_HI = desc_hi(1024);                // 8-row groups are 1024 B apart
 constexpr uint32_t LBO_CANON = desc_lo_lbo(16);            // single 64-column block per operand: LBO unused
+constexpr uint32_t DESC_HI_SW32 = ((256u >> 4) & 0x3FFF) | (1u << 14) | (6u << 29);   // 32-byte swizzle kind, 8-row groups 256 B apart
 
 struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
     int abort_flag;
-    int ld_shift[LD_STAGES][2];   // KEYS: 1 if the stage's tile starts at an odd row of the {lse, delta} array (written by the
-                                  // producer before it arms LD_FULL[stage], read after the wait)
 };
 static_assert(sizeof(Shared) <= 512, "struct Shared outgrew its reservation");
 
-// 1-D TMA load ({lse log2e, delta} pairs as plain floats) completing on a barrier of THIS CTA
-__device__ __forceinline__ void tma_load_1d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0) {
-    asm volatile("cp.async.bulk.tensor.1d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3}], [%2];"
-                 ::"r"(dst), "l"(map), "r"(bar), "r"(c0) : "memory");
+// 2-D TMA load (rows of an aug array) whose completion bytes go to a barrier of either CTA of the pair
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap *map, uint32_t cluster_bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(cluster_bar), "r"(c0), "r"(c1) : "memory");
 }
 
 template <bool KEYS>
@@ -125,8 +130,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t tiles = (raw + 1023u) & ~1023u;       // 1024-byte alignment for the 128-byte swizzle
     Shared *sh = reinterpret_cast<Shared *>(smem_raw + (tiles - raw) + C::SMEM_TILES);
-    const uint32_t sA1 = tiles, sA2 = tiles + A_BYTES, sRing = tiles + C::A_SMEM, sLd = sRing + NSTAGE * SLOT_BYTES;
-    const uint8_t *ld_gen = smem_raw + (tiles - raw) + C::A_SMEM + NSTAGE * SLOT_BYTES;   // generic address of sLd
+    const uint32_t sA1 = tiles, sA2 = tiles + A_BYTES, sRing = tiles + C::A_SMEM, sAug = sRing + NSTAGE * SLOT_BYTES;
+    const uint32_t sOnes = sAug + AUG_STAGES * AUG_STAGE_BYTES;
     const uint32_t bars = smem_u32(sh->bars);
     const PairWaiter wait{bars, &sh->abort_flag, prm.err, KEYS ? 300 : 200};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -143,14 +148,20 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         mbar_init(bars + 8 * BAR_Y_FULL, 1);
         mbar_init(bars + 8 * BAR_X_FREE, 16);
         for (int i = 0; i < 2; ++i) {
-            mbar_init(bars + 8 * (BAR_W_FULL + i), 8);    // the tile's warpgroup: 4 warps in each CTA
-            mbar_init(bars + 8 * (BAR_Z_FULL + i), 8);
+            mbar_init(bars + 8 * (BAR_W_FULL + i), 16);   // all 8 exp / dS warps of each CTA (32 of the tile's columns per warpgroup)
+            mbar_init(bars + 8 * (BAR_Z_FULL + i), 16);
         }
         mbar_init(bars + 8 * BAR_ACC_DONE, 1);
-        for (int i = 0; i < LD_STAGES; ++i) mbar_init(bars + 8 * (BAR_LD_FULL + i), 1);
         sh->abort_flag = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (KEYS && threadIdx.x >= 128 && threadIdx.x < 128 + BR) {
+        // the constant A operand of the augmentation step: row r = [1, 1, 0 x 6, 1, 1, 0 x 6] (bf16 1.0 = 0x3f80)
+        uint8_t *ones = smem_raw + (tiles - raw) + C::A_SMEM + NSTAGE * SLOT_BYTES + AUG_STAGES * AUG_STAGE_BYTES + (threadIdx.x - 128) * 32;
+        reinterpret_cast<uint4 *>(ones)[0] = make_uint4(0x3f803f80u, 0u, 0u, 0u);
+        reinterpret_cast<uint4 *>(ones)[1] = make_uint4(0x3f803f80u, 0u, 0u, 0u);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // read by the tensor pipe (async proxy)
     }
     if (warp == 2) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh->tmem_base)), "r"(512u) : "memory");
@@ -167,8 +178,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         // ================================================= TMA producer (both CTAs) ================================
         if (lane == 0) {
             prefetch_tmap(&prm.tm_b1); prefetch_tmap(&prm.tm_b2);
-            if (KEYS) { prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_ld); }
-            uint32_t ring = 0, na = 0, nstep = 0;
+            if (KEYS) { prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_aug1); prefetch_tmap(&prm.tm_aug2); }
+            uint32_t ring = 0, na = 0;
             for (int it = list_begin; it < list_end; ++it) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
@@ -188,7 +199,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                 TileCursor cur;
                 cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
                 const int np = (n + 1) >> 1;
-                for (int p = 0; p < np; ++p, ++nstep) {
+                for (int p = 0; p < np; ++p) {
                     const Tile t0 = cur.get();
                     cur.next();
                     Tile t1 = t0;                          // odd tail: the second tile is a fully masked copy of the first
@@ -197,24 +208,18 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         const uint32_t slot = ring % NSTAGE;
                         wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                         const uint32_t dst = sRing + slot * SLOT_BYTES, full = lead_bars + 8 * (BAR_KV_FULL + slot);
-                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES);
+                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES + (KEYS ? 2 * AUG_STAGE_BYTES : 0));
                         const int row = rank ? t1.key_row : t0.key_row;
                         tma_load_4d_pair(dst, &prm.tm_b1, full, 0, row, task.h, task.b);
                         tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_b1, full, 64, row, task.h, task.b);
                         tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_b2, full, 0, row, task.h, task.b);
                         tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_b2, full, 64, row, task.h, task.b);
+                        if (KEYS) {   // the 16 extra K columns of the tile's rows: -lse/s for X, -delta for Y (slots 0 and 2 hold such tiles)
+                            const uint32_t adst = sAug + (slot >> 1) * AUG_STAGE_BYTES;
+                            tma_load_2d_pair(adst, &prm.tm_aug1, full, 0, (int)(ld_base + row));
+                            tma_load_2d_pair(adst + AUG_TILE_BYTES, &prm.tm_aug2, full, 0, (int)(ld_base + row));
+                        }
                         ++ring;
-                    }
-                    if (KEYS) {
-                        // {lse log2e, delta} of the 64 streamed rows of both tiles.  Stage nstep & 3 was last read in pair-step
-                        // nstep - 4, whose Z hand-over precedes (through the MMA issue order) the release of the slot just waited for.
-                        const uint32_t st = nstep & (LD_STAGES - 1), lbar = bars + 8 * (BAR_LD_FULL + st);
-                        const int64_t r0 = ld_base + t0.key_row, r1 = ld_base + t1.key_row;
-                        ((volatile int *)sh->ld_shift[st])[0] = (int)(r0 & 1);
-                        ((volatile int *)sh->ld_shift[st])[1] = (int)(r1 & 1);
-                        mbar_expect_tx(lbar, 2 * LD_BOX_FLOATS * 4);
-                        tma_load_1d(sLd + st * LD_STAGE_BYTES, &prm.tm_ld, lbar, (int)(2 * (r0 & ~(int64_t)1)));
-                        tma_load_1d(sLd + st * LD_STAGE_BYTES + LD_TILE_BYTES, &prm.tm_ld, lbar, (int)(2 * (r1 & ~(int64_t)1)));
                     }
                     {   // this CTA's column half of the MN-major operands of both tiles
                         const uint32_t slot = ring % NSTAGE;
@@ -243,6 +248,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         if (rank == 0) {
             const bool leader = elect_one();
             const uint32_t a1_lo = ((sA1 >> 4) & 0x3FFF) | LBO_CANON, a2_lo = ((sA2 >> 4) & 0x3FFF) | LBO_CANON;
+            const uint32_t ones_lo = ((sOnes >> 4) & 0x3FFF) | LBO_CANON;
+            auto aug_lo = [&](uint32_t slot) { return (((sAug + (slot >> 1) * AUG_STAGE_BYTES) >> 4) & 0x3FFF) | LBO_CANON; };
             uint32_t ring = 0, na = 0, c_step = 0;        // ring items consumed; tasks; pair-steps (barrier phases)
             for (int it = list_begin; it < list_end; ++it) {
                 const aj_task &tk = prm.tasks[prm.pair_ids[it]];
@@ -266,6 +273,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                             if (KEYS) mma_ss_pair(tmem + TM_X, a1_lo + aoff, DESC_HI, b_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                             else mma_ts_pair(tmem + TM_X, tmem + TM_A1 + ks * 8, b_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                         }
+                        if (KEYS)                                   // X -= lse / s of the column's query row (augmentation step)
+                            mma_ss_pair(tmem + TM_X, ones_lo, DESC_HI_SW32, aug_lo(xslot), DESC_HI_SW32, IDESC_XY, 1u);
                         tc_commit_pair(bars + 8 * BAR_X_FULL, 3);
                     }
                     __syncwarp();
@@ -281,6 +290,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                             if (KEYS) mma_ss_pair(tmem + TM_Y, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                             else mma_ts_pair(tmem + TM_Y, tmem + TM_A2 + ks * 8, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                         }
+                        if (KEYS)                                   // Y -= delta of the column's query row
+                            mma_ss_pair(tmem + TM_Y, ones_lo, DESC_HI_SW32, aug_lo(xslot) + (AUG_TILE_BYTES >> 4), DESC_HI_SW32, IDESC_XY, 1u);
                         tc_commit_pair(bars + 8 * BAR_Y_FULL, 3);
                         tc_commit_pair(bars + 8 * (BAR_KV_EMPTY + xslot), 3);
                         if (last && KEYS) tc_commit_pair(bars + 8 * BAR_A_EMPTY, 3);   // every X / Y of this task has been issued
@@ -306,7 +317,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                             if (leader) {
 #pragma unroll
                                 for (int ks = 0; ks < BC / 16; ++ks)    // acc2 += W B2   (dV += P^T dO)
-                                    mma_ts_pair(tmem + TM_ACC2, tW + ks * 8, b2i_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (uint32_t)(i > 0) | (ks > 0));
+                                    mma_ts_pair(tmem + TM_ACC2, tW + (ks >> 1) * 32 + (ks & 1) * 8, b2i_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (uint32_t)(i > 0) | (ks > 0));
                             }
                             __syncwarp();
                         }
@@ -325,7 +336,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         if (leader) {
 #pragma unroll
                             for (int ks = 0; ks < BC / 16; ++ks)        // acc1 += Z B1   (dQ += dS K | dK += dS^T Q)
-                                mma_ts_pair(tmem + TM_ACC1, tZ + ks * 8, b1i_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (uint32_t)(i > 0) | (ks > 0));
+                                mma_ts_pair(tmem + TM_ACC1, tZ + (ks >> 1) * 32 + (ks & 1) * 8, b1i_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, acc | (uint32_t)(i > 0) | (ks > 0));
                         }
                         __syncwarp();
                     }
@@ -346,8 +357,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const float sl2 = prm.scale_log2;
         const uint64_t sl2_2 = pack2(sl2, sl2);
-        const uint32_t w_full = lead_bars + 8 * (BAR_W_FULL + wg), z_full = lead_bars + 8 * (BAR_Z_FULL + wg);
-        const uint32_t tX = tmem + lane_base + TM_X + wg * BC, tY = tmem + lane_base + TM_Y + wg * BC;
+        const bool poly = prm.poly_exp != 0;
+        const uint32_t tX = tmem + lane_base + TM_X + 32 * wg, tY = tmem + lane_base + TM_Y + 32 * wg;   // + 64 i for tile j_i
         uint32_t c_step = 0;
         for (int it = list_begin; it < list_end; ++it) {
             if (sh->abort_flag) break;
@@ -384,52 +395,55 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
             cur.init(prm.r_begin, prm.r_end, prm.rows, task.range_begin, task.range_count, prow);
             const int np = (n + 1) >> 1;
             for (int p = 0; p < np; ++p, ++c_step) {
-                // streamed rows of this warpgroup's tile that this stationary row may see (inside the entry's range and its
-                // row interval; PAPER.md:909-914 from the side of the pass)
-                int valid;
+                // streamed rows of the two tiles that this stationary row may see (inside the entry's range and its row interval;
+                // PAPER.md:909-914 from the side of the pass)
+                int valid[2];
                 if (cur.pair_inside()) {
-                    valid = cur.pair();
+                    valid[0] = valid[1] = cur.pair();
                 } else {
-                    const int v0 = cur.tile();
-                    const int v1 = 2 * p + 1 < n ? cur.tile() : 0;
-                    valid = wg ? v1 : v0;
+                    valid[0] = cur.tile();
+                    valid[1] = 2 * p + 1 < n ? cur.tile() : 0;
                 }
-                const uint8_t *stg_base = nullptr;
-                if (KEYS) stg_base = ld_gen + (c_step & (LD_STAGES - 1)) * LD_STAGE_BYTES + wg * LD_TILE_BYTES;
-                // {lse log2e, delta} of streamed rows c, c + 1 of the tile (c even): one 16-byte read when the tile starts at an
-                // even row of the array, two 8-byte reads otherwise
-                bool odd = false;
-                auto ld2 = [&](int c) -> float4 {
-                    if (!odd) return reinterpret_cast<const float4 *>(stg_base)[c >> 1];
-                    const float2 a = reinterpret_cast<const float2 *>(stg_base)[c + 1], b = reinterpret_cast<const float2 *>(stg_base)[c + 2];
-                    return make_float4(a.x, a.y, b.x, b.y);
-                };
+                // Each warpgroup takes the streamed rows (columns) [32 wg, 32 wg + 32) of BOTH tiles, tile j0 first: W(j0) and
+                // Z(j0) are complete after half of the pair-step's exponentials, so the MMAs of tile j0 start while tile j1 is
+                // still being computed (with a warpgroup per tile both tiles became ready together, late).  The bf16 W / Z of a
+                // warpgroup overwrite the first 16 of the 32 fp32 columns it has just read.
                 wait(BAR_X_FULL, c_step & 1);
                 tc_fence_after();
                 // ---- W = exp2(X s log2e - lse log2e) = p_ab (PAPER.md:842-844 with the forward's L, :945), fp32 in registers
-                float w[BC];
+                float w[2][32];
 #pragma unroll
-                for (int hb = 0; hb < 2; ++hb) {
+                for (int i = 0; i < 2; ++i) {
                     uint32_t xu[32];
-                    tmem_ld32(tX + 32 * hb, xu);
+                    tmem_ld32(tX + BC * i, xu);
                     tc_wait_ld(xu);
-                    if (KEYS && hb == 0) {
-                        wait(BAR_LD_FULL + (c_step & (LD_STAGES - 1)), (c_step / LD_STAGES) & 1);
-                        odd = ((volatile int *)sh->ld_shift[c_step & (LD_STAGES - 1)])[wg] != 0;
-                    }
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
-                        uint64_t nl = myl_2;
-                        if (KEYS) { const float4 f = ld2(32 * hb + c); nl = pack2(-f.x, -f.z); }
-                        const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, nl);
-                        if (POLY_EXP && ((c >> 1) & 1)) {      // every other column pair on the FMA pipe instead of the MUFU pipe
-                            unpack2(ex2_poly2(x), w[32 * hb + c], w[32 * hb + c + 1]);
+                        // dQ pass: this thread's row's -lse log2e; KEYS: -lse / s of the column is already inside X
+                        const uint64_t x = KEYS ? fmul2(pack2(xu[c], xu[c + 1]), sl2_2) : ffma2(pack2(xu[c], xu[c + 1]), sl2_2, myl_2);
+                        if ((POLY_EXP || poly) && ((c >> 1) & 1)) {      // every other column pair on the FMA pipe instead of the MUFU pipe
+                            unpack2(ex2_poly2(x), w[i][c], w[i][c + 1]);
                         } else {
                             float x0, x1;
                             unpack2(x, x0, x1);
-                            w[32 * hb + c] = ex2(x0);
-                            w[32 * hb + c + 1] = ex2(x1);
+                            w[i][c] = ex2(x0);
+                            w[i][c + 1] = ex2(x1);
                         }
+                    }
+                    const int v = valid[i] - 32 * wg;          // of this warpgroup's 32 columns, the first v are seen
+                    if (v < 32) {                              // outside the range / the row interval: p = 0 (selected after the
+#pragma unroll                                                 // exponential: the masked operands may be anything, even inf - inf)
+                        for (int c = 0; c < 32; ++c) if (c >= v) w[i][c] = 0.f;
+                    }
+                    if (KEYS) {
+                        uint32_t wk[16];
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) wk[c] = pack_bf16(w[i][2 * c], w[i][2 * c + 1]);
+                        tmem_st16(tX + BC * i, wk);
+                        tc_wait_st();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * (BAR_W_FULL + i));
                     }
                 }
                 if (!KEYS) {                                   // X(p) is in registers: X(p+1) may overwrite it
@@ -437,46 +451,33 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * BAR_X_FREE);
                 }
-                if (valid < BC) {                              // outside the range / the row interval: p = 0 (selected after the
-#pragma unroll                                                 // exponential: the masked operands may be anything, even inf - inf)
-                    for (int c = 0; c < BC; ++c) if (c >= valid) w[c] = 0.f;
-                }
-                if (KEYS) {
-                    uint32_t wk[32];
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) wk[c] = pack_bf16(w[2 * c], w[2 * c + 1]);
-                    tmem_st32(tX, wk);
-                    tc_wait_st();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(w_full);
-                }
                 // ---- Z = W o (Y - delta) = dS / s
                 wait(BAR_Y_FULL, c_step & 1);
                 tc_fence_after();
-                uint32_t zk[32];
 #pragma unroll
-                for (int hb = 0; hb < 2; ++hb) {
-                    uint32_t yu[32];
-                    tmem_ld32(tY + 32 * hb, yu);
+                for (int i = 0; i < 2; ++i) {
+                    uint32_t yu[32], zk[16];
+                    tmem_ld32(tY + BC * i, yu);
                     tc_wait_ld(yu);
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
-                        uint64_t nd = myd_2;
-                        if (KEYS) { const float4 f = ld2(32 * hb + c); nd = pack2(-f.y, -f.w); }
-                        const int cc = 32 * hb + c;
-                        const uint64_t z = fmul2(pack2(w[cc], w[cc + 1]), fadd2(pack2(yu[c], yu[c + 1]), nd));
+                        const uint64_t y = KEYS ? pack2(yu[c], yu[c + 1]) : fadd2(pack2(yu[c], yu[c + 1]), myd_2);   // KEYS: -delta is inside Y
+                        const uint64_t z = fmul2(pack2(w[i][c], w[i][c + 1]), y);
                         float z0, z1;
                         unpack2(z, z0, z1);
-                        if (valid < BC) { if (cc >= valid) z0 = 0.f; if (cc + 1 >= valid) z1 = 0.f; }
-                        zk[cc >> 1] = pack_bf16(z0, z1);
+                        zk[c >> 1] = pack_bf16(z0, z1);
                     }
+                    const int v = valid[i] - 32 * wg;
+                    if (v < 32) {                              // masked columns: Z = 0 whatever Y held (a branch, not 32 selects)
+#pragma unroll
+                        for (int k = 0; k < 16; ++k) zk[k] = 2 * k >= v ? 0u : (2 * k + 1 >= v ? (zk[k] & 0xffffu) : zk[k]);
+                    }
+                    tmem_st16(tY + BC * i, zk);
+                    tc_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * (BAR_Z_FULL + i));
                 }
-                tmem_st32(tY, zk);
-                tc_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(z_full);
             }
             // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one 64-column half ----
             __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
@@ -530,6 +531,285 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
     }
 }
 
+
+// ======================================================================================================================
+// dQ pass, second form ("tile ping-pong"): the same computation as attn_bwd_umma_pair_kernel<false>, with the streamed tiles
+// taken ONE AT A TIME and the two exp / dS warpgroups on ALTERNATE tiles.  The A operands of X and Y sit in TMEM, so their
+// MMAs do not need N = 128 to stay off the shared-memory port; with N = 64 (cta_group::2: each CTA stages 32 rows of the
+// tile's K and V) X(j) | Y(j) of tile j occupy one 64 + 64 column buffer and the two buffers alternate:
+//     issue order   X(j+1), Y(j+1) [buffer (j+1) & 1]   then   acc1 += Z(j) K(j) [buffer j & 1]
+// A warpgroup has two tile periods (2 x 768 clk of tensor work) to turn X, Y of its tile into Z, and nothing on the tensor
+// pipe waits for it except its own tile's last MMA.  In the pair-step form the chain Y(p) -> Z(p) -> Z(p) K -> Y(p+1) is
+// serial (X and Y are single-buffered at 128 + 128 columns) and the pipe idles a third of the time (ncu: 65 %).
+// TMEM: acc1 128 | bf16 Q 64 + dO 64 | X(b0) X(b1) 128 | Y(b0) Y(b1) 128.  Ring: 8 slots of 24 KB per tile and CTA:
+// [K rows 32c..32c+32: h0 | h1 | V rows likewise: h0 | h1 (4 KB each, K-major) | K(j) columns 64c..64c+64 (8 KB, MN-major)].
+constexpr int DQ_NSTAGE = 8;
+constexpr uint32_t DQ_HBLK = 32 * 64 * 2;              // 4 KB: 32 streamed rows x 64 columns
+constexpr uint32_t DQ_SLOT = 4 * DQ_HBLK + BLK_BYTES;  // 24 KB
+constexpr uint32_t DQ_SMEM_TILES = DQ_NSTAGE * DQ_SLOT;
+constexpr uint32_t DQ_SMEM_TOTAL = DQ_SMEM_TILES + 1024 + 512;
+constexpr uint32_t IDESC_XY64 = make_idesc(BC, false);     // 256 x 64 x 16, B K-major (32 streamed rows per CTA)
+enum {
+    DQ_A_FULL = 0,                              // leader: 16 warps stored their Q / dO rows to TMEM
+    DQ_KV_FULL,                                 // leader, x DQ_NSTAGE
+    DQ_KV_EMPTY = DQ_KV_FULL + DQ_NSTAGE,       // both
+    DQ_XY_FULL = DQ_KV_EMPTY + DQ_NSTAGE,       // both, x2 (buffer)
+    DQ_Z_FULL = DQ_XY_FULL + 2,                 // leader, x2: Z stored by the tile's warpgroup in both CTAs
+    DQ_ACC_DONE = DQ_Z_FULL + 2,                // both, x2 (buffer): every MMA up to and including the tile's Z K is complete
+    DQ_NUM_BARS = DQ_ACC_DONE + 2
+};
+static_assert(DQ_NUM_BARS <= NUM_BARS + 16, "barrier array");
+struct DqShared {
+    uint64_t bars[DQ_NUM_BARS];
+    uint32_t tmem_base;
+    int abort_flag;
+};
+static_assert(sizeof(DqShared) <= 512, "struct DqShared outgrew its reservation");
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+attn_bwd_dq_pair_kernel(const __grid_constant__ BwdPairParams prm) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t tiles = (raw + 1023u) & ~1023u;
+    DqShared *sh = reinterpret_cast<DqShared *>(smem_raw + (tiles - raw) + DQ_SMEM_TILES);
+    const uint32_t sRing = tiles;
+    const uint32_t bars = smem_u32(sh->bars);
+    const PairWaiter wait{bars, &sh->abort_flag, prm.err, 250};
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const uint32_t lead_bars = mapa(bars, 0);
+    const int pair = blockIdx.x >> 1;
+    const int list_begin = prm.pair_off[pair], list_end = prm.pair_off[pair + 1];
+
+    if (threadIdx.x == 0) {
+        mbar_init(bars + 8 * DQ_A_FULL, 16);
+        for (int i = 0; i < DQ_NSTAGE; ++i) { mbar_init(bars + 8 * (DQ_KV_FULL + i), 1); mbar_init(bars + 8 * (DQ_KV_EMPTY + i), 1); }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bars + 8 * (DQ_XY_FULL + b), 1);
+            mbar_init(bars + 8 * (DQ_Z_FULL + b), 8);
+            mbar_init(bars + 8 * (DQ_ACC_DONE + b), 1);
+        }
+        sh->abort_flag = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sh->tmem_base)), "r"(512u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_arrive();
+    cluster_wait();
+    tc_fence_after();
+    const uint32_t tmem = sh->tmem_base;
+
+    if (warp == 0) {
+        // ================================================= TMA producer (both CTAs) ================================
+        if (lane == 0) {
+            prefetch_tmap(&prm.tm_b1); prefetch_tmap(&prm.tm_b2); prefetch_tmap(&prm.tm_b1h); prefetch_tmap(&prm.tm_b2h);
+            uint32_t ring = 0;
+            for (int it = list_begin; it < list_end; ++it) {
+                const aj_task task = prm.tasks[prm.pair_ids[it]];
+                const int n = task.num_kv_tiles;
+                if (n == 0 || sh->abort_flag) continue;
+                TileCursor cur;
+                cur.init(prm.r_begin, prm.r_end, task.range_begin, task.range_count);
+                for (int j = 0; j < n; ++j, cur.next(), ++ring) {
+                    const Tile t = cur.get();
+                    const uint32_t slot = ring % DQ_NSTAGE;
+                    wait(DQ_KV_EMPTY + slot, ((ring / DQ_NSTAGE) & 1) ^ 1);
+                    const uint32_t dst = sRing + slot * DQ_SLOT, full = lead_bars + 8 * (DQ_KV_FULL + slot);
+                    if (rank == 0) mbar_expect_tx(bars + 8 * (DQ_KV_FULL + slot), 2 * DQ_SLOT);
+                    const int row = t.key_row + 32 * (int)rank;     // this CTA's 32 of the tile's 64 keys (B operand split by N)
+                    tma_load_4d_pair(dst, &prm.tm_b1h, full, 0, row, task.h, task.b);
+                    tma_load_4d_pair(dst + DQ_HBLK, &prm.tm_b1h, full, 64, row, task.h, task.b);
+                    tma_load_4d_pair(dst + 2 * DQ_HBLK, &prm.tm_b2h, full, 0, row, task.h, task.b);
+                    tma_load_4d_pair(dst + 3 * DQ_HBLK, &prm.tm_b2h, full, 64, row, task.h, task.b);
+                    tma_load_4d_pair(dst + 4 * DQ_HBLK, &prm.tm_b1, full, 64 * (int)rank, t.key_row, task.h, task.b);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================================================= MMA issuer (leader CTA) ==================================
+        if (rank == 0) {
+            const bool leader = elect_one();
+            uint32_t ring = 0, na = 0;                    // ring = tiles before this task = global tile index base
+            for (int it = list_begin; it < list_end; ++it) {
+                const aj_task &tk = prm.tasks[prm.pair_ids[it]];
+                const int n = (int)warp_uniform((uint32_t)tk.num_kv_tiles | (sh->abort_flag ? 0x80000000u : 0u));
+                if (n <= 0) continue;
+                wait(DQ_A_FULL, na & 1);
+                ++na;
+                tc_fence_after();
+                auto issue_xy = [&](uint32_t g) {         // X(g) = Q K(g)^T, Y(g) = dO V(g)^T into buffer g & 1
+                    const uint32_t slot = g % DQ_NSTAGE, b = g & 1;
+                    wait(DQ_KV_FULL + slot, (g / DQ_NSTAGE) & 1);
+                    tc_fence_after();
+                    const uint32_t k_lo = (((sRing + slot * DQ_SLOT) >> 4) & 0x3FFF) | LBO_CANON, v_lo = k_lo + ((2 * DQ_HBLK) >> 4);
+                    if (leader) {
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t boff = ((ks >> 2) * DQ_HBLK + (ks & 3) * 32) >> 4;
+                            mma_ts_pair(tmem + TM_X + BC * b, tmem + TM_A1 + ks * 8, k_lo + boff, DESC_HI, IDESC_XY64, ks > 0);
+                        }
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t boff = ((ks >> 2) * DQ_HBLK + (ks & 3) * 32) >> 4;
+                            mma_ts_pair(tmem + TM_Y + BC * b, tmem + TM_A2 + ks * 8, v_lo + boff, DESC_HI, IDESC_XY64, ks > 0);
+                        }
+                        tc_commit_pair(bars + 8 * (DQ_XY_FULL + b), 3);
+                    }
+                    __syncwarp();
+                };
+                issue_xy(ring);
+                for (int j = 0; j < n; ++j) {
+                    const uint32_t g = ring + (uint32_t)j, slot = g % DQ_NSTAGE, b = g & 1;
+                    if (j + 1 < n) issue_xy(g + 1);
+                    const uint32_t m_lo = (((sRing + slot * DQ_SLOT + 4 * DQ_HBLK) >> 4) & 0x3FFF) | LBO_CANON;
+                    wait(DQ_Z_FULL + b, (g >> 1) & 1);
+                    tc_fence_after();
+                    if (leader) {
+#pragma unroll
+                        for (int ks = 0; ks < BC / 16; ++ks)        // acc1 += Z K   (dQ += dS K)
+                            mma_ts_pair(tmem + TM_ACC1, tmem + TM_Y + BC * b + ks * 8, m_lo + ks * (2048 >> 4), DESC_HI, IDESC_ACC, (uint32_t)(j > 0) | (ks > 0));
+                        tc_commit_pair(bars + 8 * (DQ_KV_EMPTY + slot), 3);
+                        tc_commit_pair(bars + 8 * (DQ_ACC_DONE + b), 3);
+                    }
+                    __syncwarp();
+                }
+                ring += (uint32_t)n;
+            }
+        }
+    } else if (warp >= 4) {
+        // ================================================= exp / dS / epilogue (both CTAs) ==========================
+        const int wg = (warp - 4) >> 2;                            // takes the tiles whose global index has this parity
+        const int row = (threadIdx.x - 128) & (BR - 1);
+        const int prow = row + BR * (int)rank;
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const float sl2 = prm.scale_log2;
+        const uint64_t sl2_2 = pack2(sl2, sl2);
+        const uint32_t z_full = lead_bars + 8 * (DQ_Z_FULL + wg);
+        const uint32_t tX = tmem + lane_base + TM_X + BC * wg, tY = tmem + lane_base + TM_Y + BC * wg;
+        uint32_t g0 = 0;                                           // tiles before this task
+        for (int it = list_begin; it < list_end; ++it) {
+            if (sh->abort_flag) break;
+            const aj_task task = prm.tasks[prm.pair_ids[it]];
+            const int n = task.num_kv_tiles;
+            const bool store = prow < task.q_rows;
+            const int64_t grow = task.q_begin + prow;
+            uint64_t myl_2 = 0ull, myd_2 = 0ull;
+            if (n > 0) {
+                float2 my = make_float2(0.f, 0.f);
+                if (store) my = prm.ld[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow];
+                myl_2 = pack2(-my.x, -my.x); myd_2 = pack2(-my.y, -my.y);
+                // this thread's row of Q (warpgroup 0) or dO (warpgroup 1) as a bf16 A operand in TMEM
+                const aj_tensor &src = wg ? prm.a2 : prm.a1;
+                const uint4 *rowp = (const uint4 *)((const __nv_bfloat16 *)src.ptr + task.b * src.stride_b + task.h * src.stride_h + grow * src.stride_n);
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+                    uint32_t ra[32];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const uint4 u = store ? rowp[half * 8 + i] : make_uint4(0, 0, 0, 0);
+                        ra[4 * i] = u.x; ra[4 * i + 1] = u.y; ra[4 * i + 2] = u.z; ra[4 * i + 3] = u.w;
+                    }
+                    tmem_st32(tmem + lane_base + (wg ? TM_A2 : TM_A1) + 32 * half, ra);
+                }
+                tc_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * DQ_A_FULL);
+            }
+            RowCursor cur;
+            cur.init(prm.r_begin, prm.r_end, prm.rows, task.range_begin, task.range_count, prow);
+            for (int j = 0; j < n; ++j) {
+                const uint32_t g = g0 + (uint32_t)j;
+                const int valid = cur.tile();                      // keys of the tile this row may see
+                if ((int)(g & 1) != wg) continue;                  // the other warpgroup's tile
+                wait(DQ_XY_FULL + wg, (g >> 1) & 1);
+                tc_fence_after();
+                uint32_t zk[32];
+#pragma unroll
+                for (int hb = 0; hb < 2; ++hb) {
+                    uint32_t xu[32], yu[32];
+                    tmem_ld32(tX + 32 * hb, xu);
+                    tmem_ld32(tY + 32 * hb, yu);
+                    tc_wait_ld(xu, yu);
+#pragma unroll
+                    for (int c = 0; c < 32; c += 2) {
+                        // W = exp2(S s log2e - lse log2e) = p_ab;  Z = W (dP - delta) = dS / s
+                        const uint64_t x = ffma2(pack2(xu[c], xu[c + 1]), sl2_2, myl_2);
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        const uint64_t z = fmul2(pack2(ex2(x0), ex2(x1)), fadd2(pack2(yu[c], yu[c + 1]), myd_2));
+                        float z0, z1;
+                        unpack2(z, z0, z1);
+                        zk[(32 * hb + c) >> 1] = pack_bf16(z0, z1);
+                    }
+                }
+                if (valid < BC) {                              // masked columns: Z = 0, selected after the exponential (a branch, not 64 selects)
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) zk[k] = 2 * k >= valid ? 0u : (2 * k + 1 >= valid ? (zk[k] & 0xffffu) : zk[k]);
+                }
+                tmem_st32(tY, zk);
+                tc_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(z_full);
+            }
+            // ---- epilogue: acc1 * s -> dQ; each warpgroup writes one 64-column half ----
+            __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
+            if (n == 0) {
+                if (store) {
+                    const uint4 z = make_uint4(0, 0, 0, 0);
+                    for (int c = 8 * wg; c < 8 * wg + 8; ++c) ((uint4 *)o1)[c] = z;
+                }
+                continue;
+            }
+            // The warpgroup of the last tile saw X, Y of that tile, which the in-order pipe produced after the Z K of the tile
+            // three before (the previous phase of this buffer's barrier is the tile two before): after the named barrier both
+            // warpgroups know that the barrier is at most one phase away.
+            named_bar_sync(3, 256);
+            {
+                const uint32_t gl = g0 + (uint32_t)n - 1;
+                wait(DQ_ACC_DONE + (gl & 1), (gl >> 1) & 1);
+                tc_fence_after();
+            }
+            g0 += (uint32_t)n;
+#pragma unroll 1
+            for (int cb = 64 * wg; cb < 64 * wg + 64; cb += 32) {
+                uint32_t a1[32];
+                tmem_ld32(tmem + lane_base + TM_ACC1 + cb, a1);
+                tc_wait_ld(a1);
+                if (store) {
+#pragma unroll
+                    for (int v4 = 0; v4 < 4; ++v4) {
+                        uint32_t w1[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const int c = v4 * 8 + 2 * e;
+                            w1[e] = pack_bf16(__uint_as_float(a1[c]) * prm.scale, __uint_as_float(a1[c + 1]) * prm.scale);
+                        }
+                        *(uint4 *)(o1 + cb + v4 * 8) = make_uint4(w1[0], w1[1], w1[2], w1[3]);
+                    }
+                }
+            }
+            tc_fence_before();
+            named_bar_sync(4, 256);          // the accumulator and the A columns are free only when both warpgroups are done
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_arrive();
+    cluster_wait();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_bwd_umma_pair(const BwdPairParams &prm, bool keys, int num_pairs, cudaStream_t stream) {
@@ -538,9 +818,13 @@ cudaError_t launch_bwd_umma_pair(const BwdPairParams &prm, bool keys, int num_pa
     if (keys) {
         if (cudaError_t e = ensure_dynamic_smem(attn_bwd_umma_pair_kernel<true>, (int)Cfg<true>::SMEM_TOTAL, configured[1])) return e;
         attn_bwd_umma_pair_kernel<true><<<2 * num_pairs, NTHREADS, Cfg<true>::SMEM_TOTAL, stream>>>(prm);
-    } else {
+    } else if (prm.dq_form == 1) {      // pair-step form of the dQ pass (kept for comparison: DESIGN.md section 6d)
         if (cudaError_t e = ensure_dynamic_smem(attn_bwd_umma_pair_kernel<false>, (int)Cfg<false>::SMEM_TOTAL, configured[0])) return e;
         attn_bwd_umma_pair_kernel<false><<<2 * num_pairs, NTHREADS, Cfg<false>::SMEM_TOTAL, stream>>>(prm);
+    } else {
+        static std::atomic<uint64_t> configured_dq{0};
+        if (cudaError_t e = ensure_dynamic_smem(attn_bwd_dq_pair_kernel, (int)DQ_SMEM_TOTAL, configured_dq)) return e;
+        attn_bwd_dq_pair_kernel<<<2 * num_pairs, NTHREADS, DQ_SMEM_TOTAL, stream>>>(prm);
     }
     return cudaGetLastError();
 }

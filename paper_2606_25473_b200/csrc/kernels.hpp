@@ -49,6 +49,7 @@ struct BwdParams {
     const float *lse;                 // [B, H, Nq] from the forward
     float *delta;                     // [B, H, Nq] workspace: <dO_a, O_a> (may be NULL when `ld` is given)
     float2 *ld;                       // [B, H, Nq] workspace of the CTA-pair kernels: {lse * log2(e), delta} (or NULL)
+    uint4 *aug;                       // [2][B, H, Nq] rows of 32 B = 2 x uint4: the 16 extra K columns -lse/s and -delta (or NULL)
     const aj_task *q_tasks; const int32_t *q_kb, *q_ke;   // query tiles and their key ranges
     const aj_task *k_tasks; const int32_t *k_rb, *k_re;   // key tiles and their row ranges
     int32_t B, H, Nq;
@@ -75,9 +76,13 @@ cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaS
 
 // Primal backward on CTA pairs (kernel_umma_bwd_pair_sm100.cu; bf16, d = 128): tcgen05.mma.cta_group::2, 256 stationary rows
 // per pair, packed tiling (entries carry row intervals).  a1, a2: stationary operands (box {64, 128}; KEYS pass only);
-// b1, b2: streamed (box {64, 64}); ld: 1-D map over the {lse log2e, delta} workspace as plain floats (box 128; KEYS pass).
+// b1, b2: streamed (box {64, 64}); aug1, aug2: 2-D maps over the augmentation rows (16 bf16 each) of -lse/s and -delta, box
+// {16, 64} (KEYS pass).
 struct BwdPairParams {
-    CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2, tm_ld;
+    CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2, tm_aug1, tm_aug2;
+    CUtensorMap tm_b1h, tm_b2h;       // dQ pass, tile ping-pong form: streamed operands with box {64, 32} (half a tile per CTA)
+    int32_t dq_form;                  // dQ pass: 0 = tile ping-pong (default), 1 = pair-step form
+    int32_t poly_exp;                 // pair-step kernels: every other column pair's exponential on the FMA pipe (A/B switch)
     aj_tensor out1, out2;             // dQ | dK, dV
     aj_tensor a1, a2;                 // dQ pass: Q and dO as plain views (their rows go to TMEM, not to shared memory)
     const float2 *ld;                 // [B, H, Nq] {lse log2e, delta}
