@@ -412,11 +412,13 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                 tc_fence_after();
                 // ---- W = exp2(X s log2e - lse log2e) = p_ab (PAPER.md:842-844 with the forward's L, :945), fp32 in registers
                 float w[2][32];
+                uint32_t xu2[2][32];
+                tmem_ld32(tX, xu2[0]);                         // both tiles in flight: one TMEM round trip per phase
+                tmem_ld32(tX + BC, xu2[1]);
+                tc_wait_ld(xu2[0], xu2[1]);
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
-                    uint32_t xu[32];
-                    tmem_ld32(tX + BC * i, xu);
-                    tc_wait_ld(xu);
+                    const uint32_t (&xu)[32] = xu2[i];
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
                         // dQ pass: this thread's row's -lse log2e; KEYS: -lse / s of the column is already inside X
@@ -454,11 +456,14 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                 // ---- Z = W o (Y - delta) = dS / s
                 wait(BAR_Y_FULL, c_step & 1);
                 tc_fence_after();
+                uint32_t yu2[2][32];
+                tmem_ld32(tY, yu2[0]);
+                tmem_ld32(tY + BC, yu2[1]);
+                tc_wait_ld(yu2[0], yu2[1]);
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
-                    uint32_t yu[32], zk[16];
-                    tmem_ld32(tY + BC * i, yu);
-                    tc_wait_ld(yu);
+                    const uint32_t (&yu)[32] = yu2[i];
+                    uint32_t zk[16];
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
                         const uint64_t y = KEYS ? pack2(yu[c], yu[c + 1]) : fadd2(pack2(yu[c], yu[c + 1]), myd_2);   // KEYS: -delta is inside Y
@@ -730,12 +735,17 @@ attn_bwd_dq_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                 wait(DQ_XY_FULL + wg, (g >> 1) & 1);
                 tc_fence_after();
                 uint32_t zk[32];
+                uint32_t xh[2][32], yh[2][32];
+                tmem_ld32(tX, xh[0]);
+                tmem_ld32(tY, yh[0]);
+                tc_wait_ld(xh[0], yh[0]);
+                tmem_ld32(tX + 32, xh[1]);                       // the second half is in flight under the first half's arithmetic
+                tmem_ld32(tY + 32, yh[1]);
 #pragma unroll
                 for (int hb = 0; hb < 2; ++hb) {
-                    uint32_t xu[32], yu[32];
-                    tmem_ld32(tX + 32 * hb, xu);
-                    tmem_ld32(tY + 32 * hb, yu);
-                    tc_wait_ld(xu, yu);
+                    if (hb == 1) tc_wait_ld(xh[1], yh[1]);
+                    const uint32_t (&xu)[32] = xh[hb];
+                    const uint32_t (&yu)[32] = yh[hb];
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
                         // W = exp2(S s log2e - lse log2e) = p_ab;  Z = W (dP - delta) = dS / s
