@@ -37,26 +37,32 @@ namespace {
 
 constexpr int BR = UMMA_TILE_Q;        // 128 query rows
 constexpr int BC = UMMA_TILE_K;        // 64 keys per tile
-constexpr int D = 128;
-constexpr int NSTAGE = 5;              // ring slots of 32 KB ({K,tK} or {V,tV} of one tile)
-constexpr uint32_t Q_BYTES = BR * D * 2;           // 32 KB
 constexpr uint32_t QHALF_BYTES = BR * 64 * 2;      // one 64-column swizzle block of Q: 16 KB
-constexpr uint32_t KV_BYTES = BC * D * 2;          // 16 KB
-constexpr uint32_t KVHALF_BYTES = BC * 64 * 2;     // 8 KB
-constexpr uint32_t SLOT_BYTES = 2 * KV_BYTES;      // 32 KB
-constexpr uint32_t SMEM_TILES = 2 * Q_BYTES + NSTAGE * SLOT_BYTES;  // 224 KB
-constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr uint32_t KVHALF_BYTES = BC * 64 * 2;     // one 64-column swizzle block of a streamed tile: 8 KB
+// Head dimension D = 128 (two 64-column swizzle blocks per operand row) or 64 (one): the same kernel, with the K loops, the
+// accumulator widths and the slot layouts following D.
+template <int D> struct Cfg {
+    static_assert(D == 64 || D == 128, "d must be 64 or 128");
+    static constexpr int NSTAGE = D == 128 ? 5 : 10;                    // ring slots ({K,tK} or {V,tV} of one tile)
+    static constexpr uint32_t Q_BYTES = BR * D * 2;                      // 32 KB | 16 KB
+    static constexpr uint32_t KV_BYTES = BC * D * 2;                     // 16 KB | 8 KB
+    static constexpr uint32_t SLOT_BYTES = 2 * KV_BYTES;                 // 32 KB | 16 KB
+    static constexpr uint32_t SMEM_TILES = 2 * Q_BYTES + NSTAGE * SLOT_BYTES;   // 224 KB | 192 KB
+    static constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 256 /*barriers*/;
+    static constexpr uint32_t TM_T = D;                                  // O [0, D) | T [D, 2 D)
+};
+constexpr int MAX_STAGE = 10;
 constexpr int NTHREADS = 256;
 
-constexpr uint32_t TM_O = 0, TM_T = 128, TM_S0 = 256, TM_TS0 = 320, TM_SBUF = 128;  // S1 = S0 + 128, ...
+constexpr uint32_t TM_O = 0, TM_S0 = 256, TM_TS0 = 320, TM_SBUF = 128;  // S1 = S0 + 128, ...
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units
 constexpr float M_UNSET = -1.0e30f;        // reference max of a row that has not met an unmasked key yet (finite on purpose)
 
 // Barrier indices inside the shared barrier array.
 enum {
     BAR_Q_FULL = 0, BAR_Q_EMPTY,
-    BAR_KV_FULL, BAR_KV_EMPTY = BAR_KV_FULL + NSTAGE,
-    BAR_S_FULL = BAR_KV_EMPTY + NSTAGE, BAR_P_FULL = BAR_S_FULL + 2, BAR_H_FULL = BAR_P_FULL + 2, BAR_PV_DONE = BAR_H_FULL + 2,
+    BAR_KV_FULL, BAR_KV_EMPTY = BAR_KV_FULL + MAX_STAGE,
+    BAR_S_FULL = BAR_KV_EMPTY + MAX_STAGE, BAR_P_FULL = BAR_S_FULL + 2, BAR_H_FULL = BAR_P_FULL + 2, BAR_PV_DONE = BAR_H_FULL + 2,
     BAR_TASK_FULL = BAR_PV_DONE + 2, BAR_TASK_EMPTY = BAR_TASK_FULL + 2, NUM_BARS = BAR_TASK_EMPTY + 2
 };
 
@@ -64,13 +70,12 @@ using namespace ptx;
 
 // Instruction descriptor for kind::f16: D fp32 (bits 4-5 = 1), A and B bf16 (bits 7-9, 10-12 = 1), B major (bit 16),
 // N >> 3 (bits 17-22), M >> 4 (bits 24-28).
-constexpr uint32_t make_idesc(int n, bool b_mn_major) {
+__host__ __device__ constexpr uint32_t make_idesc(int n, bool b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BR >> 4) << 24);
 }
 constexpr uint32_t IDESC_QK2 = make_idesc(2 * BC, false);  // 128 x 128 x 16: [S | tS] = Q [K ; tK]^T, A and B K-major
 constexpr uint32_t IDESC_QK1 = make_idesc(BC, false);      // 128 x  64 x 16: tS += tQ K^T
-constexpr uint32_t IDESC_PV2 = make_idesc(2 * D, true);    // 128 x 256 x 16: [O | T] += P~ [V | tV], A from TMEM, B MN-major
-constexpr uint32_t IDESC_PV1 = make_idesc(D, true);        // 128 x 128 x 16: T += H~ V
+// [O | T] += P~ [V | tV] is 128 x 2 D x 16 and T += H~ V is 128 x D x 16 (A from TMEM, B MN-major): make_idesc(2 * D | D, true)
 constexpr uint32_t DESC_HI = desc_hi(1024);                // 8-row (K-major) / 8-key (MN-major) groups are 1024 B apart
 constexpr uint32_t LBO_K = desc_lo_lbo(16);                // K-major with 128 B swizzle: unused, canonical value
 constexpr uint32_t LBO_V = desc_lo_lbo(KVHALF_BYTES);      // MN-major: 64-column blocks [V h0 | V h1 | tV h0 | tV h1] 8 KB apart
@@ -99,8 +104,13 @@ struct Shared {
     int abort_flag;
 };
 
+template <int D>
 __global__ void __launch_bounds__(NTHREADS, 1)
 attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
+    using C = Cfg<D>;
+    constexpr int NSTAGE = C::NSTAGE;
+    constexpr uint32_t Q_BYTES = C::Q_BYTES, SLOT_BYTES = C::SLOT_BYTES, SMEM_TILES = C::SMEM_TILES, TM_T = C::TM_T;
+    constexpr uint32_t IDESC_PV2 = make_idesc(2 * D, true), IDESC_PV1 = make_idesc(D, true);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t tiles = (raw + 1023u) & ~1023u;       // 1024-byte alignment for the 128-byte swizzle
@@ -156,13 +166,14 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 wait(BAR_Q_EMPTY, (nq & 1) ^ 1);
                 mbar_expect_tx(bars + 8 * BAR_Q_FULL, 2 * Q_BYTES);
                 tma_load_4d(sQ, &prm.tm_q, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
-                tma_load_4d(sQ + QHALF_BYTES, &prm.tm_q, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
+                if (D == 128) tma_load_4d(sQ + QHALF_BYTES, &prm.tm_q, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
                 tma_load_4d(sTQ, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
-                tma_load_4d(sTQ + QHALF_BYTES, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
+                if (D == 128) tma_load_4d(sTQ + QHALF_BYTES, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
                 ++nq;
                 // ring order = MMA consumption order: KtK(0), KtK(1), VtV(0), KtK(2), VtV(1), ...
                 // {K,tK} slot: [K h0 | tK h0 | K h1 | tK h1] so that [K ; tK] is one 128-row B operand per 64-column half;
                 // {V,tV} slot: [V h0 | V h1 | tV h0 | tV h1] so that [V | tV] is one 256-column B operand.   (8 KB each)
+                // D = 64: [K | tK] and [V | tV], one block per tensor.
                 TileCursor ck, cv;
                 ck.init(prm.k_begin, prm.k_end, task.range_begin, task.range_count);
                 cv = ck;
@@ -174,12 +185,13 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     mbar_expect_tx(full, SLOT_BYTES);
                     TileCursor &c = is_k ? ck : cv;
                     const CUtensorMap *m0 = is_k ? &prm.tm_k : &prm.tm_v, *m1 = is_k ? &prm.tm_tk : &prm.tm_tv;
-                    const uint32_t o_m0h1 = is_k ? 2 * KVHALF_BYTES : KVHALF_BYTES, o_m1h0 = is_k ? KVHALF_BYTES : 2 * KVHALF_BYTES;
+                    const uint32_t o_m0h1 = is_k ? 2 * KVHALF_BYTES : KVHALF_BYTES;
+                    const uint32_t o_m1h0 = D == 64 ? KVHALF_BYTES : is_k ? KVHALF_BYTES : 2 * KVHALF_BYTES;
                     const int row = c.key_row();
                     tma_load_4d(dst, m0, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + o_m0h1, m0, full, 64, row, task.h, task.b);
+                    if (D == 128) tma_load_4d(dst + o_m0h1, m0, full, 64, row, task.h, task.b);
                     tma_load_4d(dst + o_m1h0, m1, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + 3 * KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
+                    if (D == 128) tma_load_4d(dst + 3 * KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
                     c.next();
                     ++ring;
                 };
@@ -443,13 +455,20 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
 
 }  // namespace
 
-size_t umma_smem_bytes() { return SMEM_TOTAL; }
+size_t umma_smem_bytes() { return Cfg<128>::SMEM_TOTAL; }
 
-cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream) {
+cudaError_t launch_umma(const UmmaParams &prm, int d, int grid, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    static std::atomic<uint64_t> configured{0};
-    if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel, (int)SMEM_TOTAL, configured)) return e;
-    attn_jvp_umma_kernel<<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
+    static std::atomic<uint64_t> configured[2];
+    if (d == 64) {
+        if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel<64>, (int)Cfg<64>::SMEM_TOTAL, configured[0])) return e;
+        attn_jvp_umma_kernel<64><<<grid, NTHREADS, Cfg<64>::SMEM_TOTAL, stream>>>(prm);
+    } else if (d == 128) {
+        if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel<128>, (int)Cfg<128>::SMEM_TOTAL, configured[1])) return e;
+        attn_jvp_umma_kernel<128><<<grid, NTHREADS, Cfg<128>::SMEM_TOTAL, stream>>>(prm);
+    } else {
+        return cudaErrorInvalidValue;
+    }
     return cudaGetLastError();
 }
 

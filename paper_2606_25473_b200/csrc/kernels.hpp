@@ -98,7 +98,7 @@ cudaError_t launch_bwd_umma_pair(const BwdPairParams &prm, bool keys, int num_pa
 // delta kernel of kernel_simt_bwd.cu alone (shared by both backward paths)
 cudaError_t launch_bwd_delta(const BwdParams &prm, int dtype, int d, cudaStream_t stream);
 
-// bf16, d = 128, tcgen05 + TMEM + TMA (kernel_umma_sm100.cu)
+// bf16, d = 128 or 64, tcgen05 + TMEM + TMA (kernel_umma_sm100.cu; the CTA-pair kernels below take d = 128 only)
 struct UmmaParams {
     CUtensorMap tm_q, tm_tq;    // box {64, 128, 1, 1} over [B, H, Nq, d], SWIZZLE_128B
     CUtensorMap tm_k, tm_tk, tm_v, tm_tv;  // box {64, 64, 1, 1} over [B, H, Nk, d], SWIZZLE_128B
@@ -116,7 +116,7 @@ struct UmmaParams {
 };
 
 size_t umma_smem_bytes();
-cudaError_t launch_umma(const UmmaParams &prm, int grid, cudaStream_t stream);
+cudaError_t launch_umma(const UmmaParams &prm, int d, int grid, cudaStream_t stream);
 
 // bf16, d = 128, CTA pairs: tcgen05.mma.cta_group::2 with M = 256 (kernel_umma_pair_sm100.cu)
 size_t umma_pair_smem_bytes();

@@ -95,9 +95,11 @@ EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     # N2: the primal backward of configs[1]
     Workload("wan13b_tf_framewise_bwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
     # The plain-FMA (SIMT) correctness paths at a size that gives a throughput figure: fp32 inputs (the 1e-4 path of configs[0])
-    # and bf16 with d = 64 (no tcgen05 kernel).  Same teacher-forcing structure, 2 x 4 frames of 512 tokens.
+    # and bf16 with d = 64 (single-CTA tcgen05 kernel).  Same teacher-forcing structure, 2 x 4 frames of 512 tokens.
     Workload("mid_tf_fp32_d64", 1, 4, 64, "teacher_forcing", 512, 4, 1, "fp32", 1.0),
     Workload("mid_tf_bf16_d64", 1, 4, 64, "teacher_forcing", 512, 4, 1, "bf16", 0.1),
+    # bf16 with d = 64 on the single-CTA tcgen05 kernel at a size that fills the chip: configs[1]'s mask and length, 24 heads
+    Workload("wan13b_tf_framewise_d64", 1, 24, 64, "teacher_forcing", 1560, 21, 1, "bf16", 0.1),
 ]}
 
 

@@ -132,6 +132,67 @@ def test_umma_growing_scores_force_rescales_late_in_the_stream(kernel):
     compare(w, run_gpu(w, x, kernel=kernel), run_oracle(w, x))
 
 
+# ---------------------------------------------------------------------------------------- tcgen05 path, bf16 with d = 64
+SMALL_UMMA_D64 = [
+    Workload("d64_tf_frame_L200", 1, 2, 64, "teacher_forcing", 200, 3, 1, "bf16", 0.1, seed=20),
+    Workload("d64_tf_chunk_L100", 1, 2, 64, "teacher_forcing", 100, 6, 3, "bf16", 0.1, seed=21),
+    Workload("d64_bc_L137_B2", 2, 2, 64, "block_causal", 137, 4, 1, "bf16", 0.1, seed=22),
+    Workload("d64_full_N517", 1, 3, 64, "full", 517, 1, 1, "bf16", 0.1, seed=23),
+    Workload("d64_tf_L8", 1, 1, 64, "teacher_forcing", 8, 2, 1, "bf16", 0.1, seed=24),          # all tiles partial
+    Workload("d64_tf_L64x5", 1, 1, 64, "teacher_forcing", 64, 5, 1, "bf16", 0.1, seed=25),      # exact key tiles
+    Workload("d64_tf_L1560_F2", 1, 1, 64, "teacher_forcing", 1560, 2, 1, "bf16", 0.1, seed=26),  # the real frame length
+]
+
+
+@pytest.mark.parametrize("w", SMALL_UMMA_D64, ids=lambda w: w.name)
+def test_umma_d64_small_every_row(w):
+    # bf16 with d = 64 runs the single-CTA tcgen05 kernel (one 64-column swizzle block per operand row) by default
+    x = make_inputs(w)
+    ref = run_oracle(w, x)
+    plan = make_plan(w)
+    assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA, 1)
+    with pytest.raises(aj.AttnJvpError) as e:                      # the CTA-pair kernels take d = 128 only
+        aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA_PAIR)
+    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    packed = run_gpu(w, x, plan=plan)
+    packed2 = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_set_tiling(plan, aj.AJ_TILING_PER_GROUP)
+    per_group = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_SIMT)           # the plain-FMA kernel as an on-GPU cross-check
+    simt = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    compare(w, packed, ref)
+    compare(w, per_group, ref)
+    compare(w, simt, ref)
+    for a, b in zip(packed, packed2):
+        assert torch.equal(a, b)
+
+
+def test_umma_d64_peaked_and_growing_scores_rescale_mid_stream():
+    w = Workload("d64_full_growing", 1, 2, 64, "full", 1100, 1, 1, "bf16", 0.5, seed=27)
+    x = make_inputs(w)
+    ramp = torch.linspace(0.2, 9.0, w.N).view(1, 1, w.N, 1)
+    x[1] = (x[1].float() * ramp).to(torch.bfloat16)
+    x[0] = (x[0].float() * 3.0).to(torch.bfloat16)
+    compare(w, run_gpu(w, x), run_oracle(w, x))
+    w = Workload("d64_tf_peaked", 1, 2, 64, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=28)    # unit-variance tangents
+    x = make_inputs(w)
+    x[0] = (x[0].float() * 4.0).to(torch.bfloat16)
+    compare(w, run_gpu(w, x), run_oracle(w, x))
+
+
+def test_umma_d64_tangent_free_plans_stay_on_the_plain_fma_kernel():
+    w = Workload("d64_fwd_only", 1, 2, 64, "teacher_forcing", 100, 3, 1, "bf16", 0.0, 0, False, True)
+    plan = make_plan(w)
+    assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_SIMT
+    with pytest.raises(aj.AttnJvpError) as e:
+        aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA)
+    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
+    x = make_inputs(w)
+    compare(w, run_gpu(w, x, plan=plan), run_oracle(w, x))
+    aj.attn_jvp_plan_destroy(plan)
+
+
 def test_umma_zero_tangents_give_exact_zero():
     w = SMALL_UMMA[0]
     x = make_inputs(w)
