@@ -468,8 +468,12 @@ def run_cuda(args, w: Workload):
         # three kernels per step, timed together: delta (HBM-bound, small), the dQ pass and the dK/dV pass of the tcgen05
         # backward kernel (bf16, d = 128).  The 10*d convention counts the minimal five contractions;
         # the two-pass kernel executes seven (S and dP are recomputed in the second pass).
-        line["kernel"] = "tcgen05_backward_two_pass_cta_pairs" if (w.dtype == "bf16" and w.d == 128) else "simt_fp32_backward"
-        line["roofline"].update(kernel="attn_bwd_umma_pair_kernel<false> (dQ) + attn_bwd_umma_pair_kernel<true> (dK, dV) + attn_bwd_delta_kernel",
+        pair = w.dtype == "bf16" and w.d == 128
+        line["kernel"] = ("tcgen05_backward_two_pass_cta_pairs" if pair else
+                          "tcgen05_backward_two_pass_single_cta" if kernel == 2 else "simt_fp32_backward")
+        line["roofline"].update(kernel=("attn_bwd_dq_pair_kernel (dQ) + attn_bwd_umma_pair_kernel<true> (dK, dV) + attn_bwd_delta_kernel" if pair else
+                                        "attn_bwd_umma_kernel<false> (dQ) + attn_bwd_umma_kernel<true> (dK, dV) + attn_bwd_delta_kernel" if kernel == 2
+                                        else "attn_bwd_simt_kernel + attn_bwd_delta_kernel"),
                                 executed_over_counted_contractions=7.0 / 5.0)
     if w.clean_tangent_zero and not w.no_tangents:     # what the same call would be credited under the dense 12*d convention (speed-up over dense)
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12

@@ -488,8 +488,8 @@ namespace {
 // forced to AJ_KERNEL_UMMA), or CTA pairs (default).
 enum BwdFamily { BWD_SIMT = 0, BWD_UMMA = 1, BWD_PAIR = 2 };
 BwdFamily bwd_family(const aj_plan *p) {
-    if (!pair_covers(p->problem) || p->kernel == AJ_KERNEL_SIMT) return BWD_SIMT;   // the tcgen05 backward kernels take d = 128 only
-    if (p->kernel == AJ_KERNEL_UMMA) return BWD_UMMA;
+    if (!umma_covers(p->problem) || p->kernel == AJ_KERNEL_SIMT) return BWD_SIMT;
+    if (p->kernel == AJ_KERNEL_UMMA || !pair_covers(p->problem)) return BWD_UMMA;    // bf16 d = 64: the single-CTA kernels
     return BWD_PAIR;
 }
 
@@ -625,7 +625,7 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
             up.cta_off = ds.d_pair_off; up.cta_ids = ds.d_pair_ids;
             up.num_tasks = ds.num_tasks; up.H = pr.H; up.Nq = pr.Nq;
             up.scale = pr.scale; up.scale_log2 = pr.scale * 1.4426950408889634f;
-            e = aj::launch_bwd_umma(up, keys, ds.num_pairs, stream);
+            e = aj::launch_bwd_umma(up, pr.d, keys, ds.num_pairs, stream);
         }
         if (e != cudaSuccess) return cuda_fail(e, "backward kernel launch");
     }

@@ -35,15 +35,22 @@ using namespace ptx;
 
 constexpr int BR = UMMA_TILE_Q;        // 128 stationary rows
 constexpr int BC = UMMA_TILE_K;        // 64 streamed rows per tile
-constexpr int D = 128;
-constexpr int NSTAGE_MAX = 4;          // ring slots of 32 KB: [B1 h0 | B1 h1 | B2 h0 | B2 h1] (6 slots in the dQ pass, whose
-                                       // stationary operands live in TMEM, measured no faster: 13.05 M against 12.69 M cycles)
-constexpr uint32_t A_BYTES = BR * D * 2;           // 32 KB
+constexpr int NSTAGE_MAX = 8;
 constexpr uint32_t AHALF_BYTES = BR * 64 * 2;      // one 64-column swizzle block of a stationary operand: 16 KB
 constexpr uint32_t BHALF_BYTES = BC * 64 * 2;      // 8 KB
-constexpr uint32_t SLOT_BYTES = 4 * BHALF_BYTES;   // 32 KB
-constexpr uint32_t SMEM_TILES = 2 * A_BYTES + 4 * SLOT_BYTES;  // 192 KB
-constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 2048 /*struct Shared*/;
+// Head dimension D = 128 (two 64-column swizzle blocks per operand row) or 64 (one block; the accumulators use the first 64
+// of their 128 TMEM columns).
+template <int D> struct Cfg {
+    static_assert(D == 64 || D == 128, "d must be 64 or 128");
+    static constexpr int NB = D / 64;                                    // swizzle blocks per operand row
+    static constexpr int NSTAGE = D == 128 ? 4 : 8;   // ring slots [B1 h0 | B1 h1 | B2 h0 | B2 h1] of 32 KB | [B1 | B2] of 16 KB (6 slots of
+                                                      // 32 KB in the dQ pass, whose stationary operands live in TMEM, measured no faster:
+                                                      // 13.05 M against 12.69 M cycles)
+    static constexpr uint32_t A_BYTES = BR * D * 2;                      // 32 KB | 16 KB
+    static constexpr uint32_t SLOT_BYTES = 2 * NB * BHALF_BYTES;         // 32 KB | 16 KB
+    static constexpr uint32_t SMEM_TILES = 2 * A_BYTES + NSTAGE * SLOT_BYTES;   // 192 KB | 160 KB
+    static constexpr uint32_t SMEM_TOTAL = SMEM_TILES + 1024 /*align*/ + 2048 /*struct Shared*/;
+};
 constexpr int NTHREADS = 384;               // warps 0-3: TMA / MMA / TMEM alloc / idle; warps 4-7 and 8-11: exp / dS warpgroups 0, 1
 
 constexpr uint32_t TM_ACC1 = 0, TM_ACC2 = 128, TM_X0 = 256, TM_Y0 = 320, TM_BUF = 128;   // X1 = X0 + 128, Y1 = Y0 + 128
@@ -61,11 +68,11 @@ enum {
     NUM_BARS = BAR_ACC_DONE + 2
 };
 
-constexpr uint32_t make_idesc(int n, bool b_mn_major) {
+__host__ __device__ constexpr uint32_t make_idesc(int n, bool b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BR >> 4) << 24);
 }
 constexpr uint32_t IDESC_XY = make_idesc(BC, false);     // 128 x  64 x 16, A and B K-major
-constexpr uint32_t IDESC_ACC = make_idesc(D, true);      // 128 x 128 x 16, A from TMEM, B MN-major
+// acc += Z B1 / W B2 is 128 x D x 16, A from TMEM, B MN-major: make_idesc(D, true)
 constexpr uint32_t DESC_HI = desc_hi(1024);
 constexpr uint32_t LBO_K = desc_lo_lbo(16);              // K-major with 128 B swizzle: unused, canonical value
 constexpr uint32_t LBO_MN = desc_lo_lbo(BHALF_BYTES);    // MN-major: the two 64-column blocks of a streamed operand are 8 KB apart
@@ -94,14 +101,18 @@ struct TileCursor {
     }
 };
 
-template <bool KEYS>
+template <bool KEYS, int D>
 __global__ void __launch_bounds__(NTHREADS, 1)
 attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
+    using C = Cfg<D>;
+    constexpr int NB = C::NB;
+    constexpr uint32_t A_BYTES = C::A_BYTES, SLOT_BYTES = C::SLOT_BYTES, SMEM_TILES = C::SMEM_TILES;
+    constexpr uint32_t IDESC_ACC = make_idesc(D, true);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t tiles = (raw + 1023u) & ~1023u;
     Shared *sh = reinterpret_cast<Shared *>(smem_raw + (tiles - raw) + SMEM_TILES);
-    constexpr int NSTAGE = NSTAGE_MAX;
+    constexpr int NSTAGE = C::NSTAGE;
     const uint32_t sA1 = tiles, sA2 = tiles + A_BYTES, sRing = tiles + 2 * A_BYTES;
     const uint32_t bars = smem_u32(sh->bars);
     const Waiter wait{bars, &sh->abort_flag, prm.err};
@@ -142,9 +153,9 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                     const uint32_t afull = bars + 8 * BAR_A_FULL;
                     mbar_expect_tx(afull, 2 * A_BYTES);
                     tma_load_4d(sA1, &prm.tm_a1, afull, 0, task.q_begin, task.h, task.b);
-                    tma_load_4d(sA1 + AHALF_BYTES, &prm.tm_a1, afull, 64, task.q_begin, task.h, task.b);
+                    if (NB == 2) tma_load_4d(sA1 + AHALF_BYTES, &prm.tm_a1, afull, 64, task.q_begin, task.h, task.b);
                     tma_load_4d(sA2, &prm.tm_a2, afull, 0, task.q_begin, task.h, task.b);
-                    tma_load_4d(sA2 + AHALF_BYTES, &prm.tm_a2, afull, 64, task.q_begin, task.h, task.b);
+                    if (NB == 2) tma_load_4d(sA2 + AHALF_BYTES, &prm.tm_a2, afull, 64, task.q_begin, task.h, task.b);
                     ++na;
                 }
                 TileCursor cur;
@@ -156,9 +167,9 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                     mbar_expect_tx(full, SLOT_BYTES);
                     const int row = cur.row();
                     tma_load_4d(dst, &prm.tm_b1, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + BHALF_BYTES, &prm.tm_b1, full, 64, row, task.h, task.b);
-                    tma_load_4d(dst + 2 * BHALF_BYTES, &prm.tm_b2, full, 0, row, task.h, task.b);
-                    tma_load_4d(dst + 3 * BHALF_BYTES, &prm.tm_b2, full, 64, row, task.h, task.b);
+                    if (NB == 2) tma_load_4d(dst + BHALF_BYTES, &prm.tm_b1, full, 64, row, task.h, task.b);
+                    tma_load_4d(dst + NB * BHALF_BYTES, &prm.tm_b2, full, 0, row, task.h, task.b);
+                    if (NB == 2) tma_load_4d(dst + 3 * BHALF_BYTES, &prm.tm_b2, full, 64, row, task.h, task.b);
                 }
             }
         }
@@ -172,7 +183,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
             const uint32_t slot = item % NSTAGE;
             wait(BAR_B_FULL + slot, (item / NSTAGE) & 1);
             tc_fence_after();
-            const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_K, b2_lo = b1_lo + ((2 * BHALF_BYTES) >> 4);
+            const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_K, b2_lo = b1_lo + ((NB * BHALF_BYTES) >> 4);
             const uint32_t tX = tmem + TM_X0 + (gj & 1) * TM_BUF, tY = tmem + TM_Y0 + (gj & 1) * TM_BUF;
             if (leader) {
 #pragma unroll
@@ -203,7 +214,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 if (j + 1 < n) issue_xy(gj + 1, item + 1);
                 else if (leader) tc_commit(bars + 8 * BAR_A_EMPTY);      // every X, Y of this task has been issued
                 // streamed tile as MN-major B operand: row r at r*128 bytes inside each 64-column block, 16-row K steps 2 KB apart
-                const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_MN, b2_lo = b1_lo + ((2 * BHALF_BYTES) >> 4);
+                const uint32_t b1_lo = (((sRing + slot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_MN, b2_lo = b1_lo + ((NB * BHALF_BYTES) >> 4);
                 const uint32_t tW = tmem + TM_X0 + b * TM_BUF, tZ = tmem + TM_Y0 + b * TM_BUF;
                 const uint32_t acc = j > 0 ? 1u : 0u;
                 wait(BAR_W_FULL + b, (gj >> 1) & 1);
@@ -255,7 +266,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 const aj_tensor &src = wg ? prm.a2 : prm.a1;
                 const uint4 *rowp = (const uint4 *)((const __nv_bfloat16 *)src.ptr + task.b * src.stride_b + task.h * src.stride_h + grow * src.stride_n);
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {
+                for (int half = 0; half < NB; ++half) {
                     uint32_t ra[32];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
@@ -343,13 +354,13 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bars + 8 * (BAR_W_FULL + b));
             }
-            // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one 64-column half ----
+            // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one half of the D columns ----
             __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
             __nv_bfloat16 *o2 = KEYS ? (__nv_bfloat16 *)prm.out2.ptr + task.b * prm.out2.stride_b + task.h * prm.out2.stride_h + grow * prm.out2.stride_n : nullptr;
             if (n == 0) {                                           // a row without keys / a key no row sees: zeros
                 if (store) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
-                    for (int c = 8 * wg; c < 8 * wg + 8; ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
+                    for (int c = (D / 16) * wg; c < (D / 16) * (wg + 1); ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
                 }
                 continue;
             }
@@ -360,7 +371,7 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
             tc_fence_after();
             g += n;
 #pragma unroll 1
-            for (int cb = 64 * wg; cb < 64 * wg + 64; cb += 32) {
+            for (int cb = (D / 2) * wg; cb < (D / 2) * (wg + 1); cb += 32) {
                 uint32_t a1[32], a2[32];
                 tmem_ld32(tmem + lane_base + TM_ACC1 + cb, a1);
                 if (KEYS) tmem_ld32(tmem + lane_base + TM_ACC2 + cb, a2);
@@ -393,16 +404,21 @@ attn_bwd_umma_kernel(const __grid_constant__ BwdUmmaParams prm) {
     }
 }
 
+template <bool KEYS, int D>
+cudaError_t launch_one(const BwdUmmaParams &prm, int grid, cudaStream_t stream, std::atomic<uint64_t> &configured) {
+    if (cudaError_t e = ensure_dynamic_smem(attn_bwd_umma_kernel<KEYS, D>, (int)Cfg<D>::SMEM_TOTAL, configured)) return e;
+    attn_bwd_umma_kernel<KEYS, D><<<grid, NTHREADS, Cfg<D>::SMEM_TOTAL, stream>>>(prm);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
-cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream) {
+cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, int d, bool keys, int grid, cudaStream_t stream) {
     if (grid <= 0 || prm.num_tasks <= 0) return cudaSuccess;
-    static std::atomic<uint64_t> configured[2];
-    if (cudaError_t e = keys ? ensure_dynamic_smem(attn_bwd_umma_kernel<true>, (int)SMEM_TOTAL, configured[1])
-                             : ensure_dynamic_smem(attn_bwd_umma_kernel<false>, (int)SMEM_TOTAL, configured[0])) return e;
-    if (keys) attn_bwd_umma_kernel<true><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
-    else attn_bwd_umma_kernel<false><<<grid, NTHREADS, SMEM_TOTAL, stream>>>(prm);
-    return cudaGetLastError();
+    static std::atomic<uint64_t> configured[4];
+    if (d == 128) return keys ? launch_one<true, 128>(prm, grid, stream, configured[1]) : launch_one<false, 128>(prm, grid, stream, configured[0]);
+    if (d == 64) return keys ? launch_one<true, 64>(prm, grid, stream, configured[3]) : launch_one<false, 64>(prm, grid, stream, configured[2]);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace aj

@@ -57,7 +57,7 @@ struct BwdParams {
 };
 cudaError_t launch_bwd_simt(const BwdParams &prm, int dtype, int d, int num_q_tasks, int num_k_tasks, cudaStream_t stream);
 
-// Primal backward on tcgen05 (kernel_umma_bwd_sm100.cu; bf16, d = 128): one pass with query tiles stationary (dQ),
+// Primal backward on tcgen05 (kernel_umma_bwd_sm100.cu; bf16, d = 128 or 64): one pass with query tiles stationary (dQ),
 // one with key tiles stationary (dK, dV).  a1, a2: stationary operands (box {64, 128}); b1, b2: streamed (box {64, 64}).
 struct BwdUmmaParams {
     CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2;
@@ -72,7 +72,7 @@ struct BwdUmmaParams {
     int32_t num_tasks, H, Nq;
     float scale, scale_log2;
 };
-cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, bool keys, int grid, cudaStream_t stream);
+cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, int d, bool keys, int grid, cudaStream_t stream);
 
 // Primal backward on CTA pairs (kernel_umma_bwd_pair_sm100.cu; bf16, d = 128): tcgen05.mma.cta_group::2, 256 stationary rows
 // per pair, packed tiling (entries carry row intervals).  a1, a2: stationary operands (box {64, 128}; KEYS pass only);

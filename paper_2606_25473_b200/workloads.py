@@ -100,6 +100,7 @@ EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     Workload("mid_tf_bf16_d64", 1, 4, 64, "teacher_forcing", 512, 4, 1, "bf16", 0.1),
     # bf16 with d = 64 on the single-CTA tcgen05 kernel at a size that fills the chip: configs[1]'s mask and length, 24 heads
     Workload("wan13b_tf_framewise_d64", 1, 24, 64, "teacher_forcing", 1560, 21, 1, "bf16", 0.1),
+    Workload("wan13b_tf_framewise_d64_bwd", 1, 24, 64, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
 ]}
 
 

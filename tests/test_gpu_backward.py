@@ -123,6 +123,37 @@ def test_backward_single_cta_tcgen05_kernel_every_element(w):
         assert max_norm_err(u.double().numpy(), v.double().numpy()) <= 1e-2
 
 
+BF16_D64 = [
+    Workload("bwd_d64_tf_L200", 1, 2, 64, "teacher_forcing", 200, 3, 1, "bf16", 0.1, seed=40),
+    Workload("bwd_d64_tf_chunk_L100", 1, 2, 64, "teacher_forcing", 100, 6, 3, "bf16", 0.1, seed=41),
+    Workload("bwd_d64_bc_L137_B2", 2, 2, 64, "block_causal", 137, 4, 1, "bf16", 0.1, seed=42),
+    Workload("bwd_d64_full_N517", 1, 3, 64, "full", 517, 1, 1, "bf16", 0.1, seed=43),
+    Workload("bwd_d64_tf_L8", 1, 1, 64, "teacher_forcing", 8, 2, 1, "bf16", 0.1, seed=44),
+    Workload("bwd_d64_tf_L1560_F2", 1, 1, 64, "teacher_forcing", 1560, 2, 1, "bf16", 0.1, seed=45),
+    Workload("bwd_d64_tf_unit", 1, 2, 64, "teacher_forcing", 300, 3, 1, "bf16", 1.0, seed=46),
+]
+
+
+@pytest.mark.parametrize("w", BF16_D64, ids=lambda w: w.name)
+def test_backward_bf16_d64_runs_the_single_cta_tcgen05_kernels_every_element(w):
+    # bf16 with d = 64: forward and backward on the single-CTA tcgen05 kernels (one 64-column swizzle block per operand row);
+    # the plain-FMA kernels on the same plan as an on-GPU cross-check
+    x = make_inputs(w)
+    dout = _dout(w)
+    plan = make_plan(w)
+    assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_UMMA
+    got = run_fwd_bwd(w, x, dout, plan)
+    got2 = run_fwd_bwd(w, x, dout, plan)
+    aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_SIMT)
+    simt = run_fwd_bwd(w, x, dout, plan)
+    aj.attn_jvp_plan_destroy(plan)
+    check(w, x, dout, got)
+    check(w, x, dout, simt)
+    for a, b in zip(got, got2):
+        assert torch.equal(a, b)
+    assert any(not torch.equal(a, b) for a, b in zip(got, simt)), "the forced plain-FMA run must be a different kernel"
+
+
 def test_backward_pair_kernel_many_tasks_per_pair_and_long_streams():
     # more 256-row tasks than SM pairs (148 + tasks on 74 pairs: every pair runs several tasks back to back, with the
     # accumulators, the TMEM A operands and the {lse, delta} stages reused), long streams with odd tile counts
@@ -227,7 +258,7 @@ def test_backward_strided_views_and_argument_errors():
 
 
 # ---------------------------------------------------------------------------------------- full size (what bench.py times)
-FULL_SIZE_BACKWARD = ["wan13b_tf_framewise_bwd"]            # EXTRA_WORKLOADS whose step is attn_bwd
+FULL_SIZE_BACKWARD = ["wan13b_tf_framewise_bwd", "wan13b_tf_framewise_d64_bwd"]     # EXTRA_WORKLOADS whose step is attn_bwd
 
 
 def _block_samples(w, rng, per_block=6):
@@ -245,18 +276,18 @@ def _block_samples(w, rng, per_block=6):
 
 @pytest.mark.parametrize("name", FULL_SIZE_BACKWARD)
 def test_backward_full_size_all_heads_launch_sampled(name):
-    """The launch bench.py times for the backward workload: all H = 12 heads in one attn_bwd call (host-assigned head-major
+    """The launch bench.py times for the backward workload: all heads in one attn_bwd call (host-assigned head-major
     task lists), compared on three heads -- the first, a middle one and the LAST one the lists schedule -- at sampled query
     rows and keys of every block (the oracle's pass over all rows of a head supplies lse and delta)."""
     from paper_2606_25473_b200.workloads import EXTRA_WORKLOADS
     w = EXTRA_WORKLOADS[name]
-    assert w.backward and w.H == 12
+    assert w.backward and w.H >= 12
     x = make_inputs(w)
     dout = _dout(w)
     got = run_fwd_bwd(w, x, dout)
     for t in got:
         assert torch.isfinite(t.float()).all()
-    heads = [(0, 0), (0, 5), (0, w.H - 1)]
+    heads = [(0, 0), (0, w.H // 2 - 1), (0, w.H - 1)]
     for i, bh in enumerate(heads):
         idx = _block_samples(w, np.random.default_rng(50 + i))
         errs = check(w, x, dout, got, heads=[bh], rows=idx, keys=idx)
