@@ -17,10 +17,11 @@
  *  - The caller owns every tensor.  "device" pointers are CUDA device memory of the current
  *    device; "host" pointers are ordinary (preferably pinned) host memory.
  *  - Tensors are [B, H, N, d] with d contiguous; strides are in ELEMENTS (aj_tensor).
- *  - Supported: d in {64, 128}; dtype AJ_BF16 with d = 128 is the performance path (tcgen05 / TMEM / TMA kernels on
- *    CTA pairs).  Everything else -- AJ_FP32 (any supported d; plain fp32 FMA for the 1e-4 tolerance, R14) and
- *    AJ_BF16 with d = 64 -- runs the plain-FMA SIMT kernels: a CORRECTNESS path two to three orders of magnitude slower
- *    (a few TFLOP/s; DESIGN.md section 7 has the measured figure), which attn_jvp_plan_kernel reports as AJ_KERNEL_SIMT.
+ *  - Supported: d in {64, 128}.  dtype AJ_BF16 runs tcgen05 / TMEM / TMA kernels: d = 128 on CTA pairs (the performance
+ *    path, AJ_KERNEL_UMMA_PAIR), d = 64 on the single-CTA kernels (AJ_KERNEL_UMMA: forward, tangent-free forward and
+ *    backward; about two thirds of the d = 128 throughput).  AJ_FP32 (any supported d) runs the
+ *    plain-FMA SIMT kernels (plain fp32 FMA for the 1e-4 tolerance, R14): a CORRECTNESS path two to three orders
+ *    of magnitude slower (a few TFLOP/s), which attn_jvp_plan_kernel reports as AJ_KERNEL_SIMT.
  *    Anything else returns AJ_ERR_UNSUPPORTED.  There is no CPU fallback.
  *  - Inputs must be finite: masked-out tail keys are multiplied by an exact 0 (R15).
  *  - The CUDA device that is current when a plan is created owns the plan: every later call with that plan must be made
@@ -205,9 +206,9 @@ aj_status attn_jvp_plan_destroy(aj_plan *plan);
 aj_status attn_jvp_plan_info(const aj_plan *plan, int64_t *unmasked_pairs_per_head, int32_t *num_tasks);
 /* attn_jvp_schedule_pair_classes of the plan's mask. */
 aj_status attn_jvp_plan_pair_classes(const aj_plan *plan, int64_t pairs[3]);
-/* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  AJ_KERNEL_UMMA on a
- * problem it does not cover returns AJ_ERR_UNSUPPORTED and leaves the plan unchanged; the single-CTA kernel also has no
- * tangent-free mode (AJ_ERR_UNSUPPORTED on AJ_TANGENT_NONE plans). */
+/* Force a kernel (debugging / comparison).  Rebuilds and re-uploads the schedule.  A kernel on a problem it does not
+ * cover (a tcgen05 kernel on fp32 inputs, a CTA-pair kernel on d = 64) returns AJ_ERR_UNSUPPORTED and leaves the plan
+ * unchanged. */
 aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
 /* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernels, PER_GROUP for the SIMT kernel; the SIMT
  * kernel supports only PER_GROUP and the CTA-pair kernel only PACKED (AJ_ERR_UNSUPPORTED otherwise).  Rebuilds and re-uploads the schedule; results do not change. */
@@ -223,7 +224,7 @@ aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *la
  * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
  * A plan must not be used by two streams at the same time (it owns a device work counter).
  * Plans whose mask says AJ_TANGENT_NONE never read tq, tk, tv (they may be NULL), fill a non-NULL `to` with zeros and
- * write O and lse only -- on every kernel that runs them (CTA-pair tcgen05, SIMT).
+ * write O and lse only -- on every kernel (CTA-pair and single-CTA tcgen05, SIMT).
  */
 aj_status attn_jvp_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v,
                        const aj_tensor *tq, const aj_tensor *tk, const aj_tensor *tv, const aj_tensor *o,
@@ -254,8 +255,9 @@ aj_status attn_fwd(const aj_plan *plan, const aj_tensor *q, const aj_tensor *k, 
  * keys and keys no row sees).  Enqueues three kernels on `cuda_stream` (delta = <dO, O>; a pass with query tiles
  * stationary for dQ; a pass with key tiles stationary, on the transposed schedule, for dK and dV -- no atomics); the
  * first call on a plan also builds and uploads the two backward schedules (synchronous host work) and allocates a
- * [B,H,Nq] fp32 workspace.  bf16 with d = 128: tcgen05 / TMEM / TMA kernel (bf16 P and dS operands, fp32 accumulation);
- * anything else, or a plan forced to AJ_KERNEL_SIMT: plain fp32 FMA kernels.
+ * [B,H,Nq] fp32 workspace.  bf16: tcgen05 / TMEM / TMA kernels (bf16 P and dS operands, fp32 accumulation; d = 128 on CTA
+ * pairs, d = 64 and plans forced to AJ_KERNEL_UMMA on single CTAs); fp32 inputs, or a plan forced to AJ_KERNEL_SIMT: plain
+ * fp32 FMA kernels.
  */
 aj_status attn_bwd(aj_plan *plan, const aj_tensor *q, const aj_tensor *k, const aj_tensor *v, const aj_tensor *o,
                    const float *lse, const aj_tensor *dout, const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv,

@@ -107,13 +107,8 @@ bool umma_covers(const aj_problem &p) { return p.dtype == AJ_BF16 && (p.d == 128
 
 bool is_pair(int32_t kernel) { return kernel == AJ_KERNEL_UMMA_PAIR || kernel == AJ_KERNEL_UMMA_PAIR_ONE; }
 bool is_umma(int32_t kernel) { return kernel == AJ_KERNEL_UMMA || is_pair(kernel); }
-// bf16 d = 64 with tangents: the single-CTA tcgen05 kernel (it has no tangent-free mode: AJ_TANGENT_NONE plans of d = 64 stay
-// on the plain-FMA kernel)
-int32_t auto_kernel(const aj_problem &p, const aj_mask_desc &m) {
-    if (pair_covers(p)) return AJ_KERNEL_UMMA_PAIR;
-    if (umma_covers(p) && m.tangent_zero != AJ_TANGENT_NONE) return AJ_KERNEL_UMMA;
-    return AJ_KERNEL_SIMT;
-}
+// bf16 d = 64: the single-CTA tcgen05 kernels
+int32_t auto_kernel(const aj_problem &p) { return pair_covers(p) ? AJ_KERNEL_UMMA_PAIR : umma_covers(p) ? AJ_KERNEL_UMMA : AJ_KERNEL_SIMT; }
 
 // The tcgen05 kernels tile queries on a global grid (no rows wasted at group ends); the SIMT kernel per group.
 int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACKED : AJ_TILING_PER_GROUP; }
@@ -305,7 +300,7 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
         if (const char *f = std::getenv("AJ_BWD_DQ_FORM")) p->bwd_dq_form = std::atoi(f) == 1 ? 1 : 0;
         if (const char *f = std::getenv("AJ_BWD_POLY_EXP")) p->bwd_poly_exp = std::atoi(f) == 1 ? 1 : 0;
-        const int32_t kernel = auto_kernel(p->problem, p->mask);
+        const int32_t kernel = auto_kernel(p->problem);
         st = install_schedule(p, kernel, default_tiling(kernel));
     } catch (const std::bad_alloc &) {
         st = fail(AJ_ERR_OOM, "out of host memory");
@@ -353,12 +348,10 @@ aj_status attn_jvp_plan_pair_classes(const aj_plan *p, int64_t pairs[3]) {
 
 aj_status attn_jvp_plan_set_kernel(aj_plan *p, int32_t kernel) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
-    if (kernel == AJ_KERNEL_AUTO) kernel = auto_kernel(p->problem, p->mask);
+    if (kernel == AJ_KERNEL_AUTO) kernel = auto_kernel(p->problem);
     if (kernel != AJ_KERNEL_SIMT && !is_umma(kernel)) return fail(AJ_ERR_INVALID_ARG, "unknown kernel");
     if (is_umma(kernel) && !umma_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the tcgen05 kernels need bf16 inputs");
     if (is_pair(kernel) && !pair_covers(p->problem)) return fail(AJ_ERR_UNSUPPORTED, "the CTA-pair tcgen05 kernels need d = 128 (bf16 d = 64 runs AJ_KERNEL_UMMA)");
-    if (kernel == AJ_KERNEL_UMMA && p->mask.tangent_zero == AJ_TANGENT_NONE)
-        return fail(AJ_ERR_UNSUPPORTED, "the single-CTA tcgen05 kernel has no tangent-free mode (AJ_TANGENT_NONE plans run the CTA-pair or the SIMT kernel)");
     if (kernel == p->kernel) return AJ_OK;
     return install_schedule(p, kernel, default_tiling(kernel));
 }
@@ -427,7 +420,7 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
             }
             if (e == cudaSuccess && ds.num_pairs > 0) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);
         } else {
-            e = aj::launch_umma(prm, pr.d, std::min(p->num_sms, ds.num_tasks), stream);
+            e = aj::launch_umma(prm, pr.d, none, std::min(p->num_sms, ds.num_tasks), stream);
         }
     } else {
         aj::SimtParams prm;

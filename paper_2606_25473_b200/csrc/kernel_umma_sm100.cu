@@ -104,7 +104,9 @@ struct Shared {
     int abort_flag;
 };
 
-template <int D>
+// PRIMAL: AJ_TANGENT_NONE plans -- plain masked attention (S and P~ V only): tQ, tK, tV are never loaded, the tS / T columns
+// and the H~ hand-over are unused, tO = 0 and tlse = 0 are written where the caller gave the pointers.
+template <int D, bool PRIMAL>
 __global__ void __launch_bounds__(NTHREADS, 1)
 attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
     using C = Cfg<D>;
@@ -164,11 +166,11 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 if (task.num_kv_tiles == 0) continue;
                 // Q_i, tQ_i: two 64-column swizzle blocks each
                 wait(BAR_Q_EMPTY, (nq & 1) ^ 1);
-                mbar_expect_tx(bars + 8 * BAR_Q_FULL, 2 * Q_BYTES);
+                mbar_expect_tx(bars + 8 * BAR_Q_FULL, PRIMAL ? Q_BYTES : 2 * Q_BYTES);
                 tma_load_4d(sQ, &prm.tm_q, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
                 if (D == 128) tma_load_4d(sQ + QHALF_BYTES, &prm.tm_q, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
-                tma_load_4d(sTQ, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
-                if (D == 128) tma_load_4d(sTQ + QHALF_BYTES, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
+                if (!PRIMAL) tma_load_4d(sTQ, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 0, task.q_begin, task.h, task.b);
+                if (!PRIMAL && D == 128) tma_load_4d(sTQ + QHALF_BYTES, &prm.tm_tq, bars + 8 * BAR_Q_FULL, 64, task.q_begin, task.h, task.b);
                 ++nq;
                 // ring order = MMA consumption order: KtK(0), KtK(1), VtV(0), KtK(2), VtV(1), ...
                 // {K,tK} slot: [K h0 | tK h0 | K h1 | tK h1] so that [K ; tK] is one 128-row B operand per 64-column half;
@@ -182,7 +184,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     const uint32_t slot = ring % NSTAGE;
                     wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                     const uint32_t dst = sRing + slot * SLOT_BYTES, full = bars + 8 * (BAR_KV_FULL + slot);
-                    mbar_expect_tx(full, SLOT_BYTES);
+                    mbar_expect_tx(full, PRIMAL ? SLOT_BYTES / 2 : SLOT_BYTES);
                     TileCursor &c = is_k ? ck : cv;
                     const CUtensorMap *m0 = is_k ? &prm.tm_k : &prm.tm_v, *m1 = is_k ? &prm.tm_tk : &prm.tm_tv;
                     const uint32_t o_m0h1 = is_k ? 2 * KVHALF_BYTES : KVHALF_BYTES;
@@ -190,8 +192,8 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     const int row = c.key_row();
                     tma_load_4d(dst, m0, full, 0, row, task.h, task.b);
                     if (D == 128) tma_load_4d(dst + o_m0h1, m0, full, 64, row, task.h, task.b);
-                    tma_load_4d(dst + o_m1h0, m1, full, 0, row, task.h, task.b);
-                    if (D == 128) tma_load_4d(dst + 3 * KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
+                    if (!PRIMAL) tma_load_4d(dst + o_m1h0, m1, full, 0, row, task.h, task.b);
+                    if (!PRIMAL && D == 128) tma_load_4d(dst + 3 * KVHALF_BYTES, m1, full, 64, row, task.h, task.b);
                     c.next();
                     ++ring;
                 };
@@ -223,8 +225,12 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 for (int ks = 0; ks < D / 16; ++ks) {
                     const uint32_t qoff = ((ks >> 2) * QHALF_BYTES + (ks & 3) * 32) >> 4;
                     const uint32_t koff = ((ks >> 2) * 2 * KVHALF_BYTES + (ks & 3) * 32) >> 4;
-                    mma_ss(tS_, q_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK2, ks > 0);   // [S | tS] = Q [K ; tK]^T
-                    mma_ss(tTS_, tq_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK1, 1);      // tS += tQ K^T
+                    if (PRIMAL) {
+                        mma_ss(tS_, q_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK1, ks > 0);   // S = Q K^T
+                    } else {
+                        mma_ss(tS_, q_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK2, ks > 0);   // [S | tS] = Q [K ; tK]^T
+                        mma_ss(tTS_, tq_lo + qoff, DESC_HI, k_lo + koff, DESC_HI, IDESC_QK1, 1);      // tS += tQ K^T
+                    }
                 }
                 tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
                 tc_commit(bars + 8 * (BAR_S_FULL + (gj & 1)));
@@ -258,16 +264,18 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 tc_fence_after();
                 if (leader) {
 #pragma unroll
-                    for (int ks = 0; ks < BC / 16; ++ks)    // [O | T] += P~ [V | tV]
-                        mma_ts(tmem + TM_O, tP + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV2, acc | (ks > 0));
+                    for (int ks = 0; ks < BC / 16; ++ks)    // [O | T] += P~ [V | tV]; PRIMAL: O += P~ V
+                        mma_ts(tmem + TM_O, tP + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, PRIMAL ? IDESC_PV1 : IDESC_PV2, acc | (ks > 0));
                 }
                 __syncwarp();
-                wait(BAR_H_FULL + b, (gj >> 1) & 1);
-                tc_fence_after();
+                if (!PRIMAL) {
+                    wait(BAR_H_FULL + b, (gj >> 1) & 1);
+                    tc_fence_after();
+                }
                 if (leader) {
 #pragma unroll
                     for (int ks = 0; ks < BC / 16; ++ks)    // T += H~ V
-                        mma_ts(tmem + TM_T, tH + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV1, 1);
+                        if (!PRIMAL) mma_ts(tmem + TM_T, tH + ks * 8, v_lo + ks * (2048 >> 4), DESC_HI, IDESC_PV1, 1);
                     tc_commit(bars + 8 * (BAR_KV_EMPTY + slot));
                     tc_commit(bars + 8 * (BAR_PV_DONE + b));
                 }
@@ -311,8 +319,10 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 tmem_ld32(tS_, su[0]);
                 tmem_ld32(tS_ + 32, su[1]);
                 tc_wait_ld(su[0], su[1]);
-                tmem_ld32(tTS_, tu[0]);                            // in flight while P~ is computed
-                tmem_ld32(tTS_ + 32, tu[1]);
+                if (!PRIMAL) {
+                    tmem_ld32(tTS_, tu[0]);                        // in flight while P~ is computed
+                    tmem_ld32(tTS_ + 32, tu[1]);
+                }
                 // tile-valid mask: S = -inf past the entry's last key and on rows outside its row interval
                 const int valid = (row >= row_lo && row < row_hi) ? cur.valid() : 0;
                 if (valid < BC) {
@@ -337,7 +347,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                         tc_fence_after();
                         const float f = (need && !fresh) ? ex2(m_ref - cand) : 1.f;
 #pragma unroll 1
-                        for (int cb = 0; cb < 256; cb += 32) {
+                        for (int cb = 0; cb < (PRIMAL ? D : 2 * D); cb += 32) {
                             uint32_t a[32];
                             tmem_ld32(tmem + lane_base + cb, a);
                             tc_wait_ld(a);
@@ -371,6 +381,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                 tc_fence_before();
                 mbar_arrive(bars + 8 * (BAR_P_FULL + b));
                 // H~ = P~ o (s * tS); r += rowsum.  Masked columns have P~ = 0, so H~ = 0.
+                if (PRIMAL) continue;
                 tc_wait_ld(tu[0], tu[1]);
                 {
                     uint32_t hk[32];
@@ -397,7 +408,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             if (n == 0) {                                         // no key: O = 0, tO = 0, lse = -inf (R9)
                 if (store) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
-                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; ((uint4 *)tp)[c] = z; }
+                    for (int c = 0; c < D / 8; ++c) { ((uint4 *)op)[c] = z; if (prm.to.ptr) ((uint4 *)tp)[c] = z; }
                     if (prm.lse) prm.lse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = -INFINITY;
                     if (prm.tlse) prm.tlse[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow] = 0.f;
                 }
@@ -417,8 +428,14 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             for (int cb = 0; cb < D; cb += 32) {
                 uint32_t ao[32], at[32];
                 tmem_ld32(tmem + lane_base + TM_O + cb, ao);
-                tmem_ld32(tmem + lane_base + TM_T + cb, at);
-                tc_wait_ld(ao, at);
+                if (PRIMAL) {
+                    tc_wait_ld(ao);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) at[c] = 0u;
+                } else {
+                    tmem_ld32(tmem + lane_base + TM_T + cb, at);
+                    tc_wait_ld(ao, at);
+                }
                 if (store) {
 #pragma unroll
                     for (int v4 = 0; v4 < 4; ++v4) {
@@ -433,7 +450,7 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                             wt[e] = pack_bf16(t0, t1);
                         }
                         *(uint4 *)(op + cb + v4 * 8) = make_uint4(wo[0], wo[1], wo[2], wo[3]);
-                        *(uint4 *)(tp + cb + v4 * 8) = make_uint4(wt[0], wt[1], wt[2], wt[3]);
+                        if (!PRIMAL || prm.to.ptr) *(uint4 *)(tp + cb + v4 * 8) = make_uint4(wt[0], wt[1], wt[2], wt[3]);
                     }
                 }
             }
@@ -457,19 +474,19 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
 
 size_t umma_smem_bytes() { return Cfg<128>::SMEM_TOTAL; }
 
-cudaError_t launch_umma(const UmmaParams &prm, int d, int grid, cudaStream_t stream) {
+cudaError_t launch_umma(const UmmaParams &prm, int d, bool primal, int grid, cudaStream_t stream) {
     if (grid <= 0) return cudaSuccess;
-    static std::atomic<uint64_t> configured[2];
-    if (d == 64) {
-        if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel<64>, (int)Cfg<64>::SMEM_TOTAL, configured[0])) return e;
-        attn_jvp_umma_kernel<64><<<grid, NTHREADS, Cfg<64>::SMEM_TOTAL, stream>>>(prm);
-    } else if (d == 128) {
-        if (cudaError_t e = ensure_dynamic_smem(attn_jvp_umma_kernel<128>, (int)Cfg<128>::SMEM_TOTAL, configured[1])) return e;
-        attn_jvp_umma_kernel<128><<<grid, NTHREADS, Cfg<128>::SMEM_TOTAL, stream>>>(prm);
-    } else {
-        return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
+    static std::atomic<uint64_t> configured[4];
+    auto run = [&](auto kernel, uint32_t smem, std::atomic<uint64_t> &done) -> cudaError_t {
+        if (cudaError_t e = ensure_dynamic_smem(kernel, (int)smem, done)) return e;
+        kernel<<<grid, NTHREADS, smem, stream>>>(prm);
+        return cudaGetLastError();
+    };
+    if (d == 64) return primal ? run(attn_jvp_umma_kernel<64, true>, Cfg<64>::SMEM_TOTAL, configured[1])
+                               : run(attn_jvp_umma_kernel<64, false>, Cfg<64>::SMEM_TOTAL, configured[0]);
+    if (d == 128) return primal ? run(attn_jvp_umma_kernel<128, true>, Cfg<128>::SMEM_TOTAL, configured[3])
+                                : run(attn_jvp_umma_kernel<128, false>, Cfg<128>::SMEM_TOTAL, configured[2]);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace aj

@@ -116,7 +116,8 @@ struct UmmaParams {
 };
 
 size_t umma_smem_bytes();
-cudaError_t launch_umma(const UmmaParams &prm, int d, int grid, cudaStream_t stream);
+// primal: AJ_TANGENT_NONE plans (tq, tk, tv maps unused; tO = 0, tlse = 0)
+cudaError_t launch_umma(const UmmaParams &prm, int d, bool primal, int grid, cudaStream_t stream);
 
 // bf16, d = 128, CTA pairs: tcgen05.mma.cta_group::2 with M = 256 (kernel_umma_pair_sm100.cu)
 size_t umma_pair_smem_bytes();

@@ -181,16 +181,21 @@ def test_umma_d64_peaked_and_growing_scores_rescale_mid_stream():
     compare(w, run_gpu(w, x), run_oracle(w, x))
 
 
-def test_umma_d64_tangent_free_plans_stay_on_the_plain_fma_kernel():
-    w = Workload("d64_fwd_only", 1, 2, 64, "teacher_forcing", 100, 3, 1, "bf16", 0.0, 0, False, True)
-    plan = make_plan(w)
-    assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_SIMT
-    with pytest.raises(aj.AttnJvpError) as e:
-        aj.attn_jvp_plan_set_kernel(plan, aj.AJ_KERNEL_UMMA)
-    assert e.value.status == aj.AJ_ERR_UNSUPPORTED
-    x = make_inputs(w)
-    compare(w, run_gpu(w, x, plan=plan), run_oracle(w, x))
-    aj.attn_jvp_plan_destroy(plan)
+@pytest.mark.parametrize("d", [64, 128])
+def test_single_cta_kernel_tangent_free_mode(d):
+    # AJ_TANGENT_NONE on the single-CTA tcgen05 kernel (the default for bf16 d = 64; forced for d = 128): S and P~ V only
+    for w in (Workload(f"fwd_only_tf_d{d}", 1, 2, d, "teacher_forcing", 200, 3, 1, "bf16", 0.0, 30, False, True),
+              Workload(f"fwd_only_prefix_d{d}", 2, 2, d, "full", 150, 4, 1, "bf16", 0.0, 31, False, True, 150)):   # Nq != Nk
+        plan = make_plan(w, aj.AJ_KERNEL_UMMA)
+        assert aj.attn_jvp_plan_kernel(plan) == (aj.AJ_KERNEL_UMMA, 1)
+        x = make_inputs(w)
+        got = run_gpu(w, x, plan=plan)
+        aj.attn_jvp_plan_destroy(plan)
+        compare(w, got, run_oracle(w, x))
+        if d == 64:
+            plan = make_plan(w)
+            assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_UMMA
+            aj.attn_jvp_plan_destroy(plan)
 
 
 def test_umma_zero_tangents_give_exact_zero():
