@@ -127,7 +127,8 @@ aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int
         return fail(AJ_ERR_UNSUPPORTED, "the SIMT kernel only supports per-group tiling");
     aj_schedule *s = nullptr;
     if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tq, tk, tiling, &s)) return st;
-    return upload_schedule(p, s, kernel, ds);
+    // the single-CTA tcgen05 kernel: one host-assigned, head-major task list per SM (the CTA-pair kernels get one per SM pair)
+    return upload_schedule(p, s, kernel, ds, kernel == AJ_KERNEL_UMMA ? p->num_sms : 0);
 }
 
 // Uploads `s` (owned by `ds` afterwards; destroyed on failure, `ds` then unchanged).
@@ -420,7 +421,7 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
             }
             if (e == cudaSuccess && ds.num_pairs > 0) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);
         } else {
-            e = aj::launch_umma(prm, pr.d, none, std::min(p->num_sms, ds.num_tasks), stream);
+            e = aj::launch_umma(prm, pr.d, none, ds.num_pairs, stream);
         }
     } else {
         aj::SimtParams prm;

@@ -153,16 +153,18 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
             prefetch_tmap(&prm.tm_q); prefetch_tmap(&prm.tm_tq); prefetch_tmap(&prm.tm_k);
             prefetch_tmap(&prm.tm_tk); prefetch_tmap(&prm.tm_v); prefetch_tmap(&prm.tm_tv);
             uint32_t ring = 0, nq = 0;
-            int task_id = blockIdx.x;
+            // this CTA's task list, assigned by the host head by head (assign_workers): all CTAs stream the same head's K, tK, V, tV
+            // through L2 at the same time (a longest-first queue over ALL heads re-read them from DRAM 9.6 x: ncu, d = 64, 24 heads)
+            int it = prm.pair_off[blockIdx.x];
+            const int it_end = prm.pair_off[blockIdx.x + 1];
             for (uint32_t t = 0;; ++t) {
                 const int ts = t & 1;
                 wait(BAR_TASK_EMPTY + ts, ((t >> 1) & 1) ^ 1);
-                if (sh->abort_flag) task_id = prm.num_tasks;
+                const int task_id = (it < it_end && !sh->abort_flag) ? prm.pair_ids[it++] : prm.num_tasks;
                 sh->task_id[ts] = task_id;
                 mbar_arrive(bars + 8 * (BAR_TASK_FULL + ts));
                 if (task_id >= prm.num_tasks) break;
                 const aj_task task = prm.tasks[task_id];
-                task_id = atomicAdd(&prm.counters[0], 1) + gridDim.x;
                 if (task.num_kv_tiles == 0) continue;
                 // Q_i, tQ_i: two 64-column swizzle blocks each
                 wait(BAR_Q_EMPTY, (nq & 1) ^ 1);
@@ -203,9 +205,6 @@ attn_jvp_umma_kernel(const __grid_constant__ UmmaParams prm) {
                     push(false);
                 }
             }
-            // the last CTA to run out of work re-arms the counters for the next launch
-            const int done = atomicAdd(&prm.counters[1], 1);
-            if (done == (int)gridDim.x - 1) { prm.counters[0] = 0; prm.counters[1] = 0; __threadfence(); }
         }
     } else if (warp == 1) {
         // ================================================= MMA issuer ============================================
