@@ -222,7 +222,9 @@ aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *la
  * without waiting.  q, tq: [B,H,Nq,d]; k, v, tk, tv: [B,H,Nk,d]; o, to: [B,H,Nq,d] in the problem dtype;
  * lse: contiguous fp32 [B,H,Nq] (may be NULL).  All DEVICE memory; inputs are only read.  Pointers must be
  * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
- * A plan must not be used by two streams at the same time (it owns a device work counter).
+ * The forward calls keep no per-call device state in the plan: one plan may be enqueued on several streams at the same time
+ * (the tensor-map cache is guarded by a mutex).  attn_bwd and the host-buffer calls own a workspace / staging buffers in
+ * the plan: one such call at a time per plan.
  * Plans whose mask says AJ_TANGENT_NONE never read tq, tk, tv (they may be NULL), fill a non-NULL `to` with zeros and
  * write O and lse only -- on every kernel (CTA-pair and single-CTA tcgen05, SIMT).
  */

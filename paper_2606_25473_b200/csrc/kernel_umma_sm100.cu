@@ -10,8 +10,8 @@
 // T (both get the same rescale and are only ever summed); the reference max m_ref is only moved when the tile
 // max exceeds it by 2^8 (lazy rescale; P~ <= 256), which leaves Eq. 45 unchanged; exp is base 2.
 //
-// CTA = 8 warps, persistent, one CTA per SM:
-//   warp 0      TMA producer (one lane): task fetch, Q/tQ tile, ring of {K,tK} / {V,tV} half-stages
+// CTA = 8 warps, persistent, one CTA per SM, each with its own host-assigned task list (head-major: assign_workers):
+//   warp 0      TMA producer (one lane): next task of the list, Q/tQ tile, ring of {K,tK} / {V,tV} half-stages
 //   warp 1      MMA issuer (whole warp runs the loop so every descriptor stays in uniform registers, one elected
 //               lane issues): QK(j+1) is issued before PV(j) so the tensor pipe never waits on softmax
 //   warp 2      TMEM allocator

@@ -108,8 +108,8 @@ struct UmmaParams {
     const aj_task *tasks;
     const int32_t *k_begin, *k_end;   // schedule entries: keys [k_begin[e], k_end[e]) ...
     const uint32_t *rows;             // ... seen by tile rows [rows[e] & 0xffff, rows[e] >> 16)
-    int32_t *counters;          // [0] next task, [1] CTAs finished (both 0 between launches), [2] abort code
-    const int32_t *pair_off, *pair_ids;   // CTA-pair kernel: pair p runs tasks pair_ids[pair_off[p] .. pair_off[p+1])
+    int32_t *counters;          // [2] abort code ([0], [1] unused)
+    const int32_t *pair_off, *pair_ids;   // worker w (an SM pair; an SM of the single-CTA kernel) runs tasks pair_ids[pair_off[w] .. pair_off[w+1])
     int32_t num_tasks, H, Nq;
     float scale_log2;           // s * log2(e)
     float scale;                // s

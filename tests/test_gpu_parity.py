@@ -86,7 +86,7 @@ def test_umma_small_every_row(w, kernel):
     plan = make_plan(w, kernel)
     assert aj.attn_jvp_plan_kernel(plan) == (kernel, 1)
     gpu = run_gpu(w, x, plan=plan)
-    gpu2 = run_gpu(w, x, plan=plan)            # the plan re-arms its work counter: a second launch must agree
+    gpu2 = run_gpu(w, x, plan=plan)            # a second launch on the same plan must agree
     aj.attn_jvp_plan_destroy(plan)
     compare(w, gpu, run_oracle(w, x))
     for a, b in zip(gpu, gpu2):
@@ -196,6 +196,39 @@ def test_single_cta_kernel_tangent_free_mode(d):
             plan = make_plan(w)
             assert aj.attn_jvp_plan_kernel(plan)[0] == aj.AJ_KERNEL_UMMA
             aj.attn_jvp_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("kernel", UMMA_KERNELS, ids=KERNEL_IDS.get)
+def test_one_plan_on_two_streams_at_once(kernel):
+    # the forward keeps no per-call device state in the plan (task lists are read-only): two launches of the same plan in flight
+    # on two streams, on different inputs, give the bits of the same launches run one after the other
+    w = Workload("two_streams", 1, 4, 128, "teacher_forcing", 700, 3, 1, "bf16", 0.1, seed=41)
+    w2 = Workload("two_streams_b", 1, 4, 128, "teacher_forcing", 700, 3, 1, "bf16", 0.1, seed=42)
+    xa, xb = [t.cuda() for t in make_inputs(w)], [t.cuda() for t in make_inputs(w2)]
+    plan = make_plan(w, kernel)
+    outs = []
+    for x in (xa, xb):                                   # sequential reference
+        o, to = torch.empty_like(x[0]), torch.empty_like(x[0])
+        lse = torch.empty((w.B, w.H, w.N), dtype=torch.float32, device="cuda")
+        aj.attn_jvp_fwd(plan, *x, o, to, lse, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        outs.append((o, to, lse))
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    conc = []
+    for x, st in ((xa, s1), (xb, s2)):
+        o, to = torch.full_like(x[0], float("nan")), torch.full_like(x[0], float("nan"))
+        lse = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")
+        conc.append((o, to, lse))
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for (x, st), out in zip(((xa, s1), (xb, s2)), conc):
+            aj.attn_jvp_fwd(plan, *x, *out, st.cuda_stream)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    for ref, got in zip(outs, conc):
+        for a, b in zip(ref, got):
+            assert torch.equal(a, b)
 
 
 def test_umma_zero_tangents_give_exact_zero():
