@@ -36,6 +36,9 @@ struct aj_plan {
         // from the lists above
         int32_t *d_prim_off = nullptr, *d_prim_ids = nullptr;
         int32_t num_prim_pairs = 0;
+        // task-slot rendezvous of the CTA-pair forward kernel (UmmaParams::slot_sync): counters and targets, one per task slot
+        int32_t *d_slot_sync = nullptr, *d_slot_expect = nullptr;
+        int32_t num_slots = 0;
     } full, head;                 // forward
     // primal backward: query tiles x key ranges (dQ) and key tiles x row ranges (dK, dV) for all B x H heads, and for ONE
     // head (attn_bwd_host)
@@ -96,6 +99,7 @@ aj_status cuda_fail(cudaError_t e, const char *what) {
 void free_schedule(aj_plan::DevSchedule &ds) {
     cudaFree(ds.d_tasks); cudaFree(ds.d_kb); cudaFree(ds.d_ke); cudaFree(ds.d_rows);
     cudaFree(ds.d_pair_off); cudaFree(ds.d_pair_ids); cudaFree(ds.d_prim_off); cudaFree(ds.d_prim_ids);
+    cudaFree(ds.d_slot_sync); cudaFree(ds.d_slot_expect);
     attn_jvp_schedule_destroy(ds.sched);
     ds = aj_plan::DevSchedule();
 }
@@ -158,7 +162,25 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
         if (general.empty()) num_pairs = 0;
         if (!primal.empty()) num_prim_pairs = assign(primal, want, prim_off, prim_ids);
     }
+    // Task-slot rendezvous (kernel_umma_pair_sm100.cu): only where it costs nothing and pays -- every task of the launch has the same
+    // cost (so the pairs would start each slot together anyway), the lists are long enough for the drift to build up, and one
+    // task's key stream is larger than what L2 keeps (K, tK, V, tV rows of 2 d bytes each).
+    std::vector<int32_t> slot_expect;
+    if (is_pair(kernel) && workers == 0 && num_pairs > 1 && num_prim_pairs == 0 && !pair_ids.empty()) {
+        const aj_task &t0 = s->tasks[pair_ids[0]];
+        bool uniform = t0.num_kv_tiles > 0;
+        for (int32_t t : pair_ids) uniform = uniform && s->tasks[t].num_kv_tiles == t0.num_kv_tiles && s->tasks[t].flags == t0.flags;
+        int max_len = 0;
+        for (int w = 0; w < num_pairs; ++w) max_len = std::max(max_len, pair_off[w + 1] - pair_off[w]);
+        const double stream_bytes = (double)t0.num_kv_tiles * s->tile_k * 4.0 * p->problem.d * 2.0;
+        if (uniform && max_len >= 16 && stream_bytes > 48e6) {
+            slot_expect.assign(max_len, 0);
+            for (int w = 0; w < num_pairs; ++w)
+                for (int i = 0; i < pair_off[w + 1] - pair_off[w]; ++i) ++slot_expect[i];
+        }
+    }
     aj_task *d_tasks = nullptr;
+    int32_t *d_slot_sync = nullptr, *d_slot_expect = nullptr;
     int32_t *d_kb = nullptr, *d_ke = nullptr, *d_pair_off = nullptr, *d_pair_ids = nullptr, *d_prim_off = nullptr, *d_prim_ids = nullptr;
     uint32_t *d_rows = nullptr;
     cudaError_t e = cudaMalloc(&d_tasks, std::max<size_t>(nt, 1) * sizeof(aj_task));
@@ -168,6 +190,10 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     };
     if (num_pairs) { up(pair_off, &d_pair_off); up(pair_ids, &d_pair_ids); }
     if (num_prim_pairs) { up(prim_off, &d_prim_off); up(prim_ids, &d_prim_ids); }
+    if (!slot_expect.empty()) {
+        up(slot_expect, &d_slot_expect);
+        if (e == cudaSuccess) e = cudaMalloc(&d_slot_sync, slot_expect.size() * sizeof(int32_t));
+    }
     if (e == cudaSuccess) e = cudaMalloc(&d_kb, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_ke, std::max<size_t>(nr, 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&d_rows, std::max<size_t>(nr, 1) * sizeof(uint32_t));
@@ -177,7 +203,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     if (e == cudaSuccess && nr) e = cudaMemcpy(d_rows, rows.data(), nr * sizeof(uint32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         cudaFree(d_tasks); cudaFree(d_kb); cudaFree(d_ke); cudaFree(d_rows); cudaFree(d_pair_off); cudaFree(d_pair_ids);
-        cudaFree(d_prim_off); cudaFree(d_prim_ids);
+        cudaFree(d_prim_off); cudaFree(d_prim_ids); cudaFree(d_slot_sync); cudaFree(d_slot_expect);
         attn_jvp_schedule_destroy(s);
         return e == cudaErrorMemoryAllocation ? fail(AJ_ERR_OOM, "out of device memory for the schedule") : cuda_fail(e, "schedule upload");
     }
@@ -186,6 +212,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     ds.d_tasks = d_tasks; ds.d_kb = d_kb; ds.d_ke = d_ke; ds.d_rows = d_rows;
     ds.d_pair_off = d_pair_off; ds.d_pair_ids = d_pair_ids; ds.num_pairs = num_pairs;
     ds.d_prim_off = d_prim_off; ds.d_prim_ids = d_prim_ids; ds.num_prim_pairs = num_prim_pairs;
+    ds.d_slot_sync = d_slot_sync; ds.d_slot_expect = d_slot_expect; ds.num_slots = (int32_t)slot_expect.size();
     return AJ_OK;
 }
 
@@ -419,7 +446,13 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
                 pp.pair_off = ds.d_prim_off; pp.pair_ids = ds.d_prim_ids;
                 e = aj::launch_umma_pair_fwd(pp, ds.num_prim_pairs, stream);
             }
-            if (e == cudaSuccess && ds.num_pairs > 0) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);
+            if (e == cudaSuccess && ds.num_pairs > 0) {
+                if (ds.num_slots > 0 && !std::getenv("AJ_NO_SLOT_SYNC")) {       // (the environment switch is for A/B runs)
+                    prm.slot_sync = ds.d_slot_sync; prm.slot_expect = ds.d_slot_expect;
+                    e = cudaMemsetAsync(ds.d_slot_sync, 0, ds.num_slots * sizeof(int32_t), stream);
+                }
+                if (e == cudaSuccess) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);
+            }
         } else {
             e = aj::launch_umma(prm, pr.d, none, ds.num_pairs, stream);
         }

@@ -225,6 +225,18 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
+                if (prm.slot_sync) {
+                    // Task-slot rendezvous of the producers (uniform-cost schedules only): the pairs start every slot together, so they
+                    // stream the same keys of the same head at the same time and L2 serves all but one of them.  Without it the pairs
+                    // drift apart by a fraction of a per cent per task, and after a few dozen slots every pair streams from DRAM on its
+                    // own (full mask, N = 115,200, 24 heads: 379 GB of DRAM reads per launch for 5.7 GB of inputs).  Bounded: after
+                    // ~0.1 ms the pair goes on alone (the rendezvous is a performance hint, never a correctness condition).
+                    const int slot_i = it - list_begin;
+                    if (rank == 0) atomicAdd(prm.slot_sync + slot_i, 1);
+                    const int want = prm.slot_expect[slot_i];
+                    const long long t0 = clock64();
+                    while (*(volatile int32_t *)(prm.slot_sync + slot_i) < want && clock64() - t0 < 200000) __nanosleep(64);
+                }
                 const bool primal = (task.flags & AJ_TASK_PRIMAL_ONLY) != 0;
                 // Q_i, tQ_i: this CTA's 128 rows, two 64-column swizzle blocks each (no tQ if it is zero)
                 wait(BAR_Q_EMPTY, (nq & 1) ^ 1);

@@ -110,6 +110,11 @@ struct UmmaParams {
     const uint32_t *rows;             // ... seen by tile rows [rows[e] & 0xffff, rows[e] >> 16)
     int32_t *counters;          // [2] abort code ([0], [1] unused)
     const int32_t *pair_off, *pair_ids;   // worker w (an SM pair; an SM of the single-CTA kernel) runs tasks pair_ids[pair_off[w] .. pair_off[w+1])
+    // CTA-pair forward kernel, uniform-cost schedules whose per-head key stream does not fit in L2 (full masks of long sequences):
+    // pair w enters the i-th task of its list only when slot_sync[i] has reached slot_expect[i] (all pairs that have an i-th task
+    // have arrived), so that the pairs keep streaming the same keys at the same time; NULL = off.  Zeroed before every launch.
+    int32_t *slot_sync;
+    const int32_t *slot_expect;
     int32_t num_tasks, H, Nq;
     float scale_log2;           // s * log2(e)
     float scale;                // s
