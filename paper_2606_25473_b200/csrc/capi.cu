@@ -38,7 +38,7 @@ struct aj_plan {
         int32_t num_prim_pairs = 0;
         // task-slot rendezvous of the CTA-pair forward kernel (UmmaParams::slot_sync): counters and targets, one per task slot
         int32_t *d_slot_sync = nullptr, *d_slot_expect = nullptr;
-        int32_t num_slots = 0;
+        int32_t num_slots = 0, sync_per_head = 0;
     } full, head;                 // forward
     // primal backward: query tiles x key ranges (dQ) and key tiles x row ranges (dK, dV) for all B x H heads, and for ONE
     // head (attn_bwd_host)
@@ -145,11 +145,12 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     std::vector<int32_t> pair_off, pair_ids, prim_off, prim_ids;
     int num_pairs = 0, num_prim_pairs = 0;
     // tasks [ids] of the schedule onto `want` workers (fewer if there are fewer tasks); ids refer to s->tasks
-    auto assign = [&](const std::vector<int32_t> &ids, int want, std::vector<int32_t> &off, std::vector<int32_t> &out) {
+    bool head_sync = false;            // the pairs meet before every head (CTA-pair forward kernel, see below)
+    auto assign = [&](const std::vector<int32_t> &ids, int want, std::vector<int32_t> &off, std::vector<int32_t> &out, bool sync) {
         std::vector<aj_task> sub;
         for (int32_t t : ids) sub.push_back(s->tasks[t]);
         const int n = (int)std::min<size_t>(std::max(want, 1), std::max<size_t>(sub.size(), 1));
-        aj::assign_workers(sub, s->entries, s->tile_k, n, off, out);
+        aj::assign_workers(sub, s->entries, s->tile_k, n, off, out, sync);
         for (int32_t &t : out) t = ids[t];
         return n;
     };
@@ -158,9 +159,19 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
         std::vector<int32_t> general, primal;
         for (size_t t = 0; t < nt; ++t)
             ((kernel == AJ_KERNEL_UMMA_PAIR && (s->tasks[t].flags & AJ_TASK_PRIMAL_ONLY)) ? primal : general).push_back((int32_t)t);
-        num_pairs = assign(general, want, pair_off, pair_ids);
+        // Per-head rendezvous (kernel_umma_pair_sm100.cu, UmmaParams::slot_sync with sync_per_head): for the forward CTA-pair kernel when
+        // the tasks of a launch differ in cost (equal ones get the task-slot rendezvous below) and the longest key stream of a task
+        // is larger than what L2 keeps for all pairs (K, tK, V, tV rows of 2 d bytes each).  AJ_HEAD_SYNC=1 / 0 forces it on / off
+        // (tests, A/B runs).
+        if (is_pair(kernel) && workers == 0 && !general.empty()) {
+            int32_t tmin = INT32_MAX, tmax = 0;
+            for (int32_t t : general) { tmin = std::min(tmin, s->tasks[t].num_kv_tiles); tmax = std::max(tmax, s->tasks[t].num_kv_tiles); }
+            head_sync = tmin != tmax && (double)tmax * s->tile_k * 4.0 * p->problem.d * 2.0 > 48e6;
+            if (const char *f = std::getenv("AJ_HEAD_SYNC")) head_sync = std::atoi(f) != 0 && tmax > 0;
+        }
+        num_pairs = assign(general, want, pair_off, pair_ids, head_sync);
         if (general.empty()) num_pairs = 0;
-        if (!primal.empty()) num_prim_pairs = assign(primal, want, prim_off, prim_ids);
+        if (!primal.empty()) num_prim_pairs = assign(primal, want, prim_off, prim_ids, false);
     }
     // Task-slot rendezvous (kernel_umma_pair_sm100.cu): only where it costs nothing and pays -- every task of the launch has the same
     // cost (so the pairs would start each slot together anyway), the lists are long enough for the drift to build up, and one
@@ -178,6 +189,20 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
             for (int w = 0; w < num_pairs; ++w)
                 for (int i = 0; i < pair_off[w + 1] - pair_off[w]; ++i) ++slot_expect[i];
         }
+    }
+    int32_t sync_per_head = 0;
+    if (head_sync && num_pairs > 1) {       // tasks of different cost: the pairs meet before every head; target = the pairs that have a task in it
+        slot_expect.assign((size_t)s->problem.B * s->problem.H, 0);
+        for (int w = 0; w < num_pairs; ++w) {
+            int prev = -1;
+            for (int i = pair_off[w]; i < pair_off[w + 1]; ++i) {
+                const aj_task &t = s->tasks[pair_ids[i]];
+                if (t.num_kv_tiles == 0) continue;
+                const int hd = t.b * s->problem.H + t.h;
+                if (hd != prev) { ++slot_expect[hd]; prev = hd; }
+            }
+        }
+        sync_per_head = 1;
     }
     aj_task *d_tasks = nullptr;
     int32_t *d_slot_sync = nullptr, *d_slot_expect = nullptr;
@@ -213,6 +238,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     ds.d_pair_off = d_pair_off; ds.d_pair_ids = d_pair_ids; ds.num_pairs = num_pairs;
     ds.d_prim_off = d_prim_off; ds.d_prim_ids = d_prim_ids; ds.num_prim_pairs = num_prim_pairs;
     ds.d_slot_sync = d_slot_sync; ds.d_slot_expect = d_slot_expect; ds.num_slots = (int32_t)slot_expect.size();
+    ds.sync_per_head = sync_per_head;
     return AJ_OK;
 }
 
@@ -448,7 +474,7 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
             }
             if (e == cudaSuccess && ds.num_pairs > 0) {
                 if (ds.num_slots > 0 && !std::getenv("AJ_NO_SLOT_SYNC")) {       // (the environment switch is for A/B runs)
-                    prm.slot_sync = ds.d_slot_sync; prm.slot_expect = ds.d_slot_expect;
+                    prm.slot_sync = ds.d_slot_sync; prm.slot_expect = ds.d_slot_expect; prm.sync_per_head = ds.sync_per_head;
                     e = cudaMemsetAsync(ds.d_slot_sync, 0, ds.num_slots * sizeof(int32_t), stream);
                 }
                 if (e == cudaSuccess) e = aj::launch_umma_pair(prm, ds.num_pairs, stream);

@@ -46,7 +46,7 @@ void build_tasks_packed(const aj_problem &p, const Lowered &low, int32_t tile_q,
 // Static list scheduling of tasks onto persistent workers (the CTA pairs of the cta_group::2 kernel): off has
 // num_workers + 1 entries, worker w runs tasks ids[off[w] .. off[w+1]) in that order.
 void assign_workers(const std::vector<aj_task> &tasks, const Entries &ent, int32_t tile_k, int num_workers,
-                    std::vector<int32_t> &off, std::vector<int32_t> &ids);
+                    std::vector<int32_t> &off, std::vector<int32_t> &ids, bool head_sync = false);
 
 }  // namespace aj
 

@@ -221,6 +221,7 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             prefetch_tmap(&prm.tm_q); prefetch_tmap(&prm.tm_tq); prefetch_tmap(&prm.tm_k);
             prefetch_tmap(&prm.tm_tk); prefetch_tmap(&prm.tm_v); prefetch_tmap(&prm.tm_tv);
             uint32_t ring = 0, nq = 0;
+            int sync_prev = -1;
             for (int it = list_begin; it < list_end; ++it) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
@@ -231,11 +232,18 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     // drift apart by a fraction of a per cent per task, and after a few dozen slots every pair streams from DRAM on its
                     // own (full mask, N = 115,200, 24 heads: 379 GB of DRAM reads per launch for 5.7 GB of inputs).  Bounded: after
                     // ~0.1 ms the pair goes on alone (the rendezvous is a performance hint, never a correctness condition).
-                    const int slot_i = it - list_begin;
-                    if (rank == 0) atomicAdd(prm.slot_sync + slot_i, 1);
-                    const int want = prm.slot_expect[slot_i];
-                    const long long t0 = clock64();
-                    while (*(volatile int32_t *)(prm.slot_sync + slot_i) < want && clock64() - t0 < 200000) __nanosleep(64);
+                    // Per-head mode (tasks of different cost): the pairs meet when they enter a head -- the lists are built for that
+                    // (assign_workers levels the workers at every head), so the wait is the imbalance inside one head, about one
+                    // short task; the bound is correspondingly longer.
+                    const int slot_i = prm.sync_per_head ? task.b * prm.H + task.h : it - list_begin;
+                    if (!prm.sync_per_head || slot_i != sync_prev) {
+                        if (rank == 0) atomicAdd(prm.slot_sync + slot_i, 1);
+                        const int want = prm.slot_expect[slot_i];
+                        const long long t0 = clock64();
+                        const long long limit = prm.sync_per_head ? 4000000 : 200000;
+                        while (*(volatile int32_t *)(prm.slot_sync + slot_i) < want && clock64() - t0 < limit) __nanosleep(64);
+                        sync_prev = slot_i;
+                    }
                 }
                 const bool primal = (task.flags & AJ_TASK_PRIMAL_ONLY) != 0;
                 // Q_i, tQ_i: this CTA's 128 rows, two 64-column swizzle blocks each (no tQ if it is zero)

@@ -115,6 +115,7 @@ struct UmmaParams {
     // have arrived), so that the pairs keep streaming the same keys at the same time; NULL = off.  Zeroed before every launch.
     int32_t *slot_sync;
     const int32_t *slot_expect;
+    int32_t sync_per_head;      // 0: the counters are per task slot; 1: per (b, h), and the pairs meet when they enter a new head
     int32_t num_tasks, H, Nq;
     float scale_log2;           // s * log2(e)
     float scale;                // s

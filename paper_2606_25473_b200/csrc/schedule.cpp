@@ -334,8 +334,12 @@ static int64_t task_cost(const aj_task &t, const Entries &ent, int32_t tile_k) {
 // All pairs therefore stream the K/V of the same head at the same time (one
 // head's K, tK, V, tV stay in L2), heads overlap only at their boundaries, and because the last head ends with its
 // shortest tasks the pairs finish within about one short task of each other.
+//
+// `head_sync`: the lists of a launch whose workers meet before every head (UmmaParams::slot_sync in per-head mode): every head
+// starts from a level field (all workers free at the time the last one is), so that the wait at the rendezvous is only the
+// imbalance inside one head -- about one of its shortest tasks -- instead of whatever the heads before have piled up.
 void assign_workers(const std::vector<aj_task> &tasks, const Entries &ent, int32_t tile_k, int num_pairs,
-                    std::vector<int32_t> &off, std::vector<int32_t> &ids) {
+                    std::vector<int32_t> &off, std::vector<int32_t> &ids, bool head_sync) {
     std::vector<int64_t> cost(tasks.size());
     for (size_t t = 0; t < tasks.size(); ++t) cost[t] = task_cost(tasks[t], ent, tile_k);
     std::vector<int32_t> order(tasks.size());
@@ -350,7 +354,16 @@ void assign_workers(const std::vector<aj_task> &tasks, const Entries &ent, int32
     std::vector<std::pair<int64_t, int>> heap;            // (-busy-until, -pair): max-heap picks the pair free first
     for (int i = 0; i < num_pairs; ++i) heap.emplace_back(0, -i);
     std::make_heap(heap.begin(), heap.end());
+    int cur_b = -1, cur_h = -1;
     for (int32_t t : order) {
+        if (head_sync && (tasks[t].b != cur_b || tasks[t].h != cur_h)) {
+            // the workers meet before every head (the kernel's rendezvous): all of them start it at the time the last one is free
+            int64_t latest = 0;
+            for (auto &w : heap) latest = std::min(latest, w.first);
+            for (auto &w : heap) w.first = latest;
+            std::make_heap(heap.begin(), heap.end());
+            cur_b = tasks[t].b; cur_h = tasks[t].h;
+        }
         std::pop_heap(heap.begin(), heap.end());
         auto &top = heap.back();
         lists[-top.second].push_back(t);

@@ -231,6 +231,27 @@ def test_one_plan_on_two_streams_at_once(kernel):
             assert torch.equal(a, b)
 
 
+def test_per_head_rendezvous_forced_on_a_small_problem(monkeypatch):
+    # Long-sequence launches whose tasks differ in cost make the SM pairs meet before every head (UmmaParams::slot_sync in
+    # per-head mode; configs[4] turns it on by itself, and its full-mask control the per-slot mode).  AJ_HEAD_SYNC=1 forces the
+    # mode on a problem the oracle finishes in seconds: more tasks than pairs, eight heads, same results as without it.
+    w = Workload("head_sync", 2, 4, 128, "block_causal", 1000, 5, 1, "bf16", 0.1, seed=51)
+    x = make_inputs(w)
+    plain = run_gpu(w, x)
+    monkeypatch.setenv("AJ_HEAD_SYNC", "1")
+    plan = make_plan(w)
+    synced = run_gpu(w, x, plan=plan)
+    synced2 = run_gpu(w, x, plan=plan)
+    aj.attn_jvp_plan_destroy(plan)
+    monkeypatch.delenv("AJ_HEAD_SYNC")
+    rows = {(0, 0): np.arange(0, w.N, 7), (1, 3): np.arange(3, w.N, 11)}
+    compare(w, synced, run_oracle(w, x, rows))
+    for a, b in zip(synced, synced2):
+        assert torch.equal(a, b)
+    for a, b in zip(synced, plain):                       # the lists differ (levelled at every head), the arithmetic per task does not
+        assert torch.equal(a, b)
+
+
 def test_umma_zero_tangents_give_exact_zero():
     w = SMALL_UMMA[0]
     x = make_inputs(w)
