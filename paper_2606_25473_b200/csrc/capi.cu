@@ -120,7 +120,7 @@ int32_t default_tiling(int32_t kernel) { return is_umma(kernel) ? AJ_TILING_PACK
 
 // Build the schedule of `prob` (the plan's problem, or one head of it) for `kernel` / `tiling` and upload it into `ds`
 // (left unchanged on failure).
-aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers = 0);
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers = 0, bool rendezvous = false);
 
 aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int32_t tiling, aj_plan::DevSchedule &ds) {
     const int tq = is_pair(kernel) ? aj::UMMA_PAIR_TILE_Q : kernel == AJ_KERNEL_UMMA ? aj::UMMA_TILE_Q : aj::SIMT_TILE_Q;
@@ -132,12 +132,13 @@ aj_status build_schedule(aj_plan *p, const aj_problem &prob, int32_t kernel, int
     aj_schedule *s = nullptr;
     if (aj_status st = attn_jvp_schedule_create_tiled(&prob, &p->mask, tq, tk, tiling, &s)) return st;
     // the single-CTA tcgen05 kernel: one host-assigned, head-major task list per SM (the CTA-pair kernels get one per SM pair)
-    return upload_schedule(p, s, kernel, ds, kernel == AJ_KERNEL_UMMA ? p->num_sms : 0);
+    return upload_schedule(p, s, kernel, ds, kernel == AJ_KERNEL_UMMA ? p->num_sms : 0, /*rendezvous=*/true);
 }
 
 // Uploads `s` (owned by `ds` afterwards; destroyed on failure, `ds` then unchanged).
 // workers > 0: also assign the tasks to that many persistent workers (head-major lists, see assign_workers).
-aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers) {
+// rendezvous: the schedule is for the forward CTA-pair kernel, whose producers can meet per task slot / per head (long sequences).
+aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::DevSchedule &ds, int workers, bool rendezvous) {
     const size_t nt = s->tasks.size(), nr = s->entries.size();
     std::vector<uint32_t> rows(nr);
     for (size_t r = 0; r < nr; ++r)   // row_begin | row_end << 16 (both < 32768) | key-tangents-zero << 31
@@ -163,7 +164,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
         // the tasks of a launch differ in cost (equal ones get the task-slot rendezvous below) and the longest key stream of a task
         // is larger than what L2 keeps for all pairs (K, tK, V, tV rows of 2 d bytes each).  AJ_HEAD_SYNC=1 / 0 forces it on / off
         // (tests, A/B runs).
-        if (is_pair(kernel) && workers == 0 && !general.empty()) {
+        if (rendezvous && is_pair(kernel) && workers == 0 && !general.empty()) {
             int32_t tmin = INT32_MAX, tmax = 0;
             for (int32_t t : general) { tmin = std::min(tmin, s->tasks[t].num_kv_tiles); tmax = std::max(tmax, s->tasks[t].num_kv_tiles); }
             head_sync = tmin != tmax && (double)tmax * s->tile_k * 4.0 * p->problem.d * 2.0 > 48e6;
@@ -177,7 +178,7 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     // cost (so the pairs would start each slot together anyway), the lists are long enough for the drift to build up, and one
     // task's key stream is larger than what L2 keeps (K, tK, V, tV rows of 2 d bytes each).
     std::vector<int32_t> slot_expect;
-    if (is_pair(kernel) && workers == 0 && num_pairs > 1 && num_prim_pairs == 0 && !pair_ids.empty()) {
+    if (rendezvous && is_pair(kernel) && workers == 0 && num_pairs > 1 && num_prim_pairs == 0 && !pair_ids.empty()) {
         const aj_task &t0 = s->tasks[pair_ids[0]];
         bool uniform = t0.num_kv_tiles > 0;
         for (int32_t t : pair_ids) uniform = uniform && s->tasks[t].num_kv_tiles == t0.num_kv_tiles && s->tasks[t].flags == t0.flags;
