@@ -13,13 +13,16 @@
 //   step overlap the load / max / store phases of the next.  A row's lazy reference max (PAPER.md:916-927 applied only when
 //   the tile max exceeds it by 2^8) is handed from the warp that decided it for step g to its twin in the other warpgroup
 //   through shared memory and a 64-thread named barrier; each warpgroup sums its own share of l and the two are combined
-//   (rescaled to the final reference) in the epilogue.  Tile j0 of a step is read from TMEM twice (max pass, exponential
-//   pass) and tile j1 once (it stays in registers across the reference-max decision), which keeps the role under the 168
-//   registers that 384 threads allow with three TMEM round trips per step; tile j1 is handed to the MMA warp first.
+//   (rescaled to the final reference) in the epilogue.  The softmax warps run under a raised register budget (setmaxnreg:
+//   208 registers, the producer / MMA / allocator warps give theirs back: 80), so all 128 scores of a pair-step come into
+//   registers in ONE TMEM round trip and stay there across the reference-max decision (168 registers forced three round trips:
+//   5.98 -> 5.66 ms on configs[1]'s mask); the branch holds no function call (PairWaiterInline), or ptxas would spill everything
+//   live across it; tile j1 is handed to the MMA warp first.
 //   Every other column pair takes its exponential from the FMA pipe (ptx::ex2_poly2): at d = 128 a tangent-free pair-step is
 //   1024 clk of tensor work against 128 x 128 exponentials = 1024 clk of the 16-lane/clk MUFU pipe, so the MUFU pipe alone
 //   would cap the kernel at the tensor roofline with no slack at all.
-// Roles per CTA: warp 0 TMA producer, warp 1 MMA issuer (leader CTA), warp 2 TMEM allocator, warps 4-11 softmax / epilogue.
+// Roles per CTA: warp 0 TMA producer, warp 1 MMA issuer (leader CTA), warp 2 TMEM allocator (80 registers), warps 4-11 softmax /
+// epilogue (208 registers).
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -36,6 +39,7 @@ namespace {
 using namespace ptx;
 using pairk::BC;
 using pairk::PairWaiter;
+using pairk::PairWaiterInline;
 using pairk::RowCursor;
 using pairk::Tile;
 using pairk::TileCursor;
@@ -44,6 +48,8 @@ constexpr int BR = 128;                // query rows per CTA (UMMA M = 256 over 
 constexpr int D = 128;
 constexpr int NSTAGE = 10;             // ring slots of 16 KB: {K of this CTA's tile} and {this CTA's half of V(j0), V(j1)} alternate
 constexpr int NSBUF = 3;               // S buffers in TMEM
+// Register budget per role (setmaxnreg, whole warpgroups: warps 0-3 / 4-7 / 8-11): 128 x 80 + 256 x 208 = 63,488 of the SM's 65,536.
+constexpr int REG_MISC = 80, REG_ROLE = 208;
 constexpr uint32_t Q_BYTES = BR * D * 2;           // 32 KB
 constexpr uint32_t QHALF_BYTES = BR * 64 * 2;      // 16 KB: one 64-column swizzle block of Q
 constexpr uint32_t BLK_BYTES = BC * 64 * 2;        // 8 KB: 64 keys x 64 columns, 128-byte swizzled rows
@@ -133,6 +139,10 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
     tc_fence_after();
     const uint32_t tmem = sh->tmem_base;
 
+    // Each branch below is dominated by its own setmaxnreg, which is what lets ptxas allocate it against that budget; the softmax
+    // branch contains no function call (PairWaiterInline), or everything live across the call would be spilled.
+    if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_MISC));
     if (warp == 0) {
         // ================================================= TMA producer (both CTAs) ================================
         if (lane == 0) {
@@ -244,7 +254,10 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 g0 += (uint32_t)np;
             }
         }
-    } else if (warp >= 4) {
+    }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_ROLE));
+        const PairWaiterInline wait{bars, &sh->abort_flag, prm.counters + 2, 400};
         // ================================================= softmax / epilogue (both CTAs, two warpgroups) ==========
         const int wg = (warp - 4) >> 2;                          // takes the pair-steps whose global index has this parity
         const int q4 = warp & 3;                                 // lane quarter of TMEM = warp index inside the warpgroup
@@ -276,28 +289,29 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 const uint32_t tS = tmem + lane_base + TM_S + 128 * buf;
                 wait(BAR_S_FULL + buf, (g / NSBUF) & 1);
                 tc_fence_after();
-                // ---- pass 1: the pair-step's row max over the columns this row may see.  Tile j0 is read for its
-                // max alone and read again in pass 2; tile j1 stays in registers (64 + 64 values would not fit beside the rest).
+                // ---- pass 1: the pair-step's row max over the columns this row may see.  All 128 scores of the
+                // step come into registers in ONE TMEM round trip (four loads in flight) and stay there for pass 2.
                 float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-                auto load_tile = [&](int i, uint32_t (&a)[32], uint32_t (&b)[32]) {
-                    tmem_ld32(tS + 64 * i, a);
-                    tmem_ld32(tS + 64 * i + 32, b);
-                    tc_wait_ld(a, b);
-                    if (valid[i] < BC) {                            // outside the entry's keys / row interval: S = -inf (P~ = 0)
+                uint32_t s0a[32], s0b[32], s1a[32], s1b[32];
+                tmem_ld32(tS, s0a);
+                tmem_ld32(tS + 32, s0b);
+                tmem_ld32(tS + 64, s1a);
+                tmem_ld32(tS + 96, s1b);
+                tc_wait_ld(s0a, s0b);
+                tc_wait_ld(s1a, s1b);
+                if (valid[0] < BC) {                            // outside the entry's keys / row interval: S = -inf (P~ = 0)
 #pragma unroll
-                        for (int c = 0; c < 32; ++c) { if (c >= valid[i]) a[c] = 0xff800000u; if (c + 32 >= valid[i]) b[c] = 0xff800000u; }
-                    }
-                };
-                uint32_t s1a[32], s1b[32];
-                {
-                    uint32_t s0a[32], s0b[32];
-                    load_tile(0, s0a, s0b);
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) { mx[c & 1] = fmaxf(mx[c & 1], __uint_as_float(s0a[c])); mx[2 + (c & 1)] = fmaxf(mx[2 + (c & 1)], __uint_as_float(s0b[c])); }
+                    for (int c = 0; c < 32; ++c) { if (c >= valid[0]) s0a[c] = 0xff800000u; if (c + 32 >= valid[0]) s0b[c] = 0xff800000u; }
                 }
-                load_tile(1, s1a, s1b);
+                if (valid[1] < BC) {
 #pragma unroll
-                for (int c = 0; c < 32; ++c) { mx[c & 1] = fmaxf(mx[c & 1], __uint_as_float(s1a[c])); mx[2 + (c & 1)] = fmaxf(mx[2 + (c & 1)], __uint_as_float(s1b[c])); }
+                    for (int c = 0; c < 32; ++c) { if (c >= valid[1]) s1a[c] = 0xff800000u; if (c + 32 >= valid[1]) s1b[c] = 0xff800000u; }
+                }
+#pragma unroll
+                for (int c = 0; c < 32; ++c) {
+                    mx[0] = fmaxf(mx[0], __uint_as_float(s0a[c])); mx[1] = fmaxf(mx[1], __uint_as_float(s0b[c]));
+                    mx[2] = fmaxf(mx[2], __uint_as_float(s1a[c])); mx[3] = fmaxf(mx[3], __uint_as_float(s1b[c]));
+                }
                 const float cand = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * sl2;
                 // ---- the reference max: taken over from the twin warp (step g - 1), moved only if this step's max exceeds it by 2^8
                 if (p > 0) {
@@ -370,12 +384,8 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * (BAR_P_FULL + 2 * buf + i));
                 };
-                exp_tile(1, s1a, s1b);                              // from registers
-                {
-                    uint32_t s0a[32], s0b[32];
-                    load_tile(0, s0a, s0b);
-                    exp_tile(0, s0a, s0b);
-                }
+                exp_tile(1, s1a, s1b);                              // tile j1 is handed to the MMA warp first
+                exp_tile(0, s0a, s0b);
             }
             // ---- epilogue: O / l, lse = m + log l; each warpgroup writes one 64-column half ----
             const bool store = prow < task.q_rows;

@@ -43,6 +43,27 @@ struct PairWaiter {
     }
 };
 
+// The same bounded wait without a function call and without printf, for roles that run under a raised register budget
+// (setmaxnreg): a call in such a region makes ptxas spill everything that is live across it.
+struct PairWaiterInline {
+    uint32_t bars;
+    volatile int *abort_flag;
+    int32_t *err;
+    int code_base;
+    __device__ __forceinline__ void operator()(int idx, uint32_t parity) const {
+        const uint32_t bar = bars + 8u * idx;
+        if (ptx::mbar_try_wait(bar, parity)) return;
+        const long long t0 = clock64();
+        uint32_t spins = 0;
+        while (!ptx::mbar_try_wait(bar, parity)) {
+            if ((++spins & 0x3f) == 0) {
+                if (*abort_flag) return;
+                if (clock64() - t0 > 4000000000LL) { *abort_flag = 1; atomicExch(err, code_base + idx); return; }
+            }
+        }
+    }
+};
+
 // One 64-row tile of a task's stream.
 struct Tile { int key_row, valid, entry; };
 // Walks the streamed tiles of a task in order: schedule entries [rb, rb + rc), each cut into BC-row tiles from its start.
