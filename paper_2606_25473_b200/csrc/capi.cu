@@ -45,6 +45,7 @@ struct aj_plan {
     DevSchedule bwd_q, bwd_k, bwd_q_head, bwd_k_head;
     float *d_delta = nullptr;     // workspace of attn_bwd (bwd_alloc_bytes)
     int32_t bwd_poly_exp = 0;     // AJ_BWD_POLY_EXP env (A/B runs): half of the backward's exponentials on the FMA pipe
+    int32_t no_slot_sync = 0;     // AJ_NO_SLOT_SYNC env (A/B runs): launch without the task-slot / per-head rendezvous
     int32_t bwd_dq_form = 0;      // dQ pass of the CTA-pair backward: 0 = tile ping-pong, 1 = pair-step form (AJ_BWD_DQ_FORM env, for A/B runs)
     // attn_jvp_fwd_host / attn_bwd_host: device staging buffers, copy streams, one event per head and direction
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // q k v tq tk tv
@@ -354,6 +355,7 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
         if (const char *f = std::getenv("AJ_BWD_DQ_FORM")) p->bwd_dq_form = std::atoi(f) == 1 ? 1 : 0;
+        if (const char *f = std::getenv("AJ_NO_SLOT_SYNC")) p->no_slot_sync = std::atoi(f) != 0 ? 1 : 0;
         if (const char *f = std::getenv("AJ_BWD_POLY_EXP")) p->bwd_poly_exp = std::atoi(f) == 1 ? 1 : 0;
         const int32_t kernel = auto_kernel(p->problem);
         st = install_schedule(p, kernel, default_tiling(kernel));
@@ -474,7 +476,7 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
                 e = aj::launch_umma_pair_fwd(pp, ds.num_prim_pairs, stream);
             }
             if (e == cudaSuccess && ds.num_pairs > 0) {
-                if (ds.num_slots > 0 && !std::getenv("AJ_NO_SLOT_SYNC")) {       // (the environment switch is for A/B runs)
+                if (ds.num_slots > 0 && !p->no_slot_sync) {
                     prm.slot_sync = ds.d_slot_sync; prm.slot_expect = ds.d_slot_expect; prm.sync_per_head = ds.sync_per_head;
                     e = cudaMemsetAsync(ds.d_slot_sync, 0, ds.num_slots * sizeof(int32_t), stream);
                 }
