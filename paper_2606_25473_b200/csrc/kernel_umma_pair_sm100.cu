@@ -222,11 +222,13 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             prefetch_tmap(&prm.tm_tk); prefetch_tmap(&prm.tm_v); prefetch_tmap(&prm.tm_tv);
             uint32_t ring = 0, nq = 0;
             int sync_prev = -1;
+            bool sync_on = true;
+            int sync_fail = 0;
             for (int it = list_begin; it < list_end; ++it) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
-                if (prm.slot_sync) {
+                if (prm.slot_sync && sync_on) {
                     // Task-slot rendezvous of the producers (uniform-cost schedules only): the pairs start every slot together, so they
                     // stream the same keys of the same head at the same time and L2 serves all but one of them.  Without it the pairs
                     // drift apart by a fraction of a per cent per task, and after a few dozen slots every pair streams from DRAM on its
@@ -240,8 +242,11 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                         if (rank == 0) atomicAdd(prm.slot_sync + slot_i, 1);
                         const int want = prm.slot_expect[slot_i];
                         const long long t0 = clock64();
-                        const long long limit = prm.sync_per_head ? 4000000 : 200000;
+                        const long long limit = prm.sync_per_head ? 1500000 : 400000;
                         while (*(volatile int32_t *)(prm.slot_sync + slot_i) < want && clock64() - t0 < limit) __nanosleep(64);
+                        // Rendezvous that keep timing out mean that the pairs are not all running (other kernels hold SMs, or two launches
+                        // share the counters): after three in a row this pair stops waiting for the rest of the launch.
+                        if (*(volatile int32_t *)(prm.slot_sync + slot_i) < want) { if (++sync_fail >= 3) sync_on = false; } else sync_fail = 0;
                         sync_prev = slot_i;
                     }
                 }
