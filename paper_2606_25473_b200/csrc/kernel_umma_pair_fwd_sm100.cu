@@ -276,18 +276,35 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
             RowCursor cur;
             cur.init(prm.k_begin, prm.k_end, prm.rows, task.range_begin, task.range_count, prow);
             const int np = (n + 1) >> 1;
-            for (int p = 0; p < np; ++p) {
-                const uint32_t g = g0 + (uint32_t)p, buf = g % NSBUF;
+            // This warpgroup's pair-steps are those whose global index g0 + p has its parity: p = first, first + 2, ...  The loop visits
+            // only them (the bookkeeping of a visited step is ~50 scalar instructions with half a dozen branches, ~300 clk on a warp
+            // that has nothing else to issue: visiting the twin's steps as well cost 600 clk per own step); the twin's step that follows
+            // is consumed from the cursor together with the own one.  S buffer and barrier phase advance by two steps at a time.
+            const int first = (int)((g0 ^ (uint32_t)wg) & 1u);
+            auto skip_step = [&](int q) {                        // consume pair-step q of the stream without using it
+                if (cur.pair_inside()) cur.pair();
+                else { cur.tile(); if (2 * q + 1 < n) cur.tile(); }
+            };
+            if (first == 1 && np > 0) skip_step(0);
+            uint32_t buf = (g0 + (uint32_t)first) % NSBUF, sph = ((g0 + (uint32_t)first) / NSBUF) & 1;
+            for (int p = first; p < np; p += 2) {
+                const uint32_t g = g0 + (uint32_t)p;
                 int valid[2];
-                if (cur.pair_inside()) {
-                    valid[0] = valid[1] = cur.pair();
+                if (cur.rem >= 4 * BC) {                         // the own step and the twin's next one lie inside the current entry
+                    valid[0] = valid[1] = cur.sees ? BC : 0;
+                    cur.rem -= 4 * BC;
+                    if (cur.rem <= 0) cur.advance();
                 } else {
-                    valid[0] = cur.tile();
-                    valid[1] = 2 * p + 1 < n ? cur.tile() : 0;
+                    if (cur.pair_inside()) {
+                        valid[0] = valid[1] = cur.pair();
+                    } else {
+                        valid[0] = cur.tile();
+                        valid[1] = 2 * p + 1 < n ? cur.tile() : 0;
+                    }
+                    if (p + 1 < np) skip_step(p + 1);
                 }
-                if ((int)(g & 1) != wg) continue;                // the other warpgroup's pair-step
                 const uint32_t tS = tmem + lane_base + TM_S + 128 * buf;
-                wait(BAR_S_FULL + buf, (g / NSBUF) & 1);
+                wait(BAR_S_FULL + buf, sph);
                 tc_fence_after();
                 // ---- pass 1: the pair-step's row max over the columns this row may see.  All 128 scores of the
                 // step come into registers in ONE TMEM round trip (four loads in flight) and stay there for pass 2.
@@ -386,6 +403,8 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                 };
                 exp_tile(1, s1a, s1b);                              // tile j1 is handed to the MMA warp first
                 exp_tile(0, s0a, s0b);
+                buf += 2;                                           // two pair-steps on: S buffer (g + 2) % 3 and its barrier phase
+                if (buf >= NSBUF) { buf -= NSBUF; sph ^= 1; }
             }
             // ---- epilogue: O / l, lse = m + log l; each warpgroup writes one 64-column half ----
             const bool store = prow < task.q_rows;
