@@ -288,6 +288,37 @@ aj_status attn_jvp_fwd_host(aj_plan *plan, const void *q, const void *k, const v
 aj_status attn_bwd_host(aj_plan *plan, const void *q, const void *k, const void *v, const void *o, const float *lse,
                         const void *dout, void *dq, void *dk, void *dv, void *cuda_stream);
 
+/*
+ * attn_bwd for callers that cannot allocate device memory: no plan, no cudaMalloc / cudaFree, no allocating library call, on
+ * the first call or any later one.  It exists for host programs in which a library-side allocation is not an option -- a
+ * process whose own memory pool claimed the GPU at start-up (a raw cudaMalloc then fails, or takes memory the pool counts as
+ * its own), and step loops with a latency budget, where an allocation can hold up every stream of the device.  Such a caller
+ * could not even create a plan, so the mask is passed as its descriptor and evaluated inside the kernels.
+ *
+ * Computes exactly what attn_bwd computes (PAPER.md:247 Eq. 19, :945), with the plain-FMA fp32 kernels (both dtypes, d in
+ * {64, 128}; a few TFLOP/s: a correctness-grade path, not the tcgen05 one).  problem / mask as for attn_jvp_plan_create; mask
+ * kinds FULL (Nq != Nk allowed), BLOCK_CAUSAL and TEACHER_FORCING; AJ_MASK_RANGES returns AJ_ERR_UNSUPPORTED (its lists would
+ * need device memory), and the mask's tangent_zero field is ignored (the backward has no tangents).  Tensors, lse, alignment
+ * rules and `cuda_stream` as for attn_bwd; all DEVICE memory of the current device, owned by the caller; every element of
+ * dq, dk, dv is written.  Enqueues three kernels and returns without waiting.
+ *
+ * Scratch.  The one intermediate, delta_a = <dO_a, O_a> per query row, lives in a fixed array inside the library's device
+ * image: AJ_STATIC_SCRATCH_MAX_ROWS floats (4 MiB) on every GPU that loads the library, held until the process exits.
+ *  - Limit: B * H * Nq <= AJ_STATIC_SCRATCH_MAX_ROWS, else AJ_ERR_INVALID_ARG with a message that names both numbers
+ *    (BASELINE.json's config 2, 12 heads x 65,520 rows, fits; larger launches go head group by head group).
+ *  - Every call on a device uses the SAME array.  Each call writes the rows it will read before reading them, so nothing has
+ *    to be cleared between calls and stale contents are harmless; but two calls that can overlap on the GPU (different
+ *    streams, or different host threads without ordering between their streams) race on it and give wrong gradients.
+ *    Calls on one stream, or on streams ordered by events, are safe.
+ *  - The first call made with a given device current looks up the array's address on that device and raises the kernels'
+ *    shared-memory limit (no allocation, but possibly the lazy load of the device image): make that first call ahead of
+ *    time, outside any stream capture.  Later calls on that device only check arguments and launch.
+ */
+#define AJ_STATIC_SCRATCH_MAX_ROWS 1048576
+aj_status attn_bwd_static(const aj_problem *problem, const aj_mask_desc *mask, const aj_tensor *q, const aj_tensor *k,
+                          const aj_tensor *v, const aj_tensor *o, const float *lse, const aj_tensor *dout,
+                          const aj_tensor *dq, const aj_tensor *dk, const aj_tensor *dv, void *cuda_stream);
+
 /* How many TMA tensor maps the plan has encoded so far and how many calls found theirs in the plan's cache (either
  * pointer may be NULL).  Steady-state calls on unchanged tensors encode nothing. */
 aj_status attn_jvp_plan_tensor_map_stats(const aj_plan *plan, int64_t *encodes, int64_t *hits);

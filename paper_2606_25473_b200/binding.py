@@ -19,6 +19,7 @@ AJ_KERNEL_AUTO, AJ_KERNEL_SIMT, AJ_KERNEL_UMMA, AJ_KERNEL_UMMA_PAIR, AJ_KERNEL_U
 AJ_TILING_PER_GROUP, AJ_TILING_PACKED = 0, 1
 AJ_TANGENT_DENSE, AJ_TANGENT_CLEAN_ZERO, AJ_TANGENT_NONE = 0, 1, 2
 AJ_TASK_PRIMAL_ONLY = 1
+AJ_STATIC_SCRATCH_MAX_ROWS = 1048576
 
 _I32P = ctypes.POINTER(ctypes.c_int32)
 
@@ -60,6 +61,7 @@ SYMBOLS = [
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
     "attn_jvp_fwd_tl", "attn_bwd_host", "attn_jvp_plan_tensor_map_stats", "attn_jvp_schedule_create_transposed_tiled",
+    "attn_bwd_static",
 ]
 
 _lib = None
@@ -100,6 +102,8 @@ def lib():
         l.attn_jvp_fwd_tl.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp, vp]
         l.attn_bwd_host.argtypes = [vp] * 11
         l.attn_jvp_plan_tensor_map_stats.argtypes = [vp, i64p, i64p]
+        l.attn_bwd_static.argtypes = ([ctypes.POINTER(aj_problem), ctypes.POINTER(aj_mask_desc)] + [ctypes.POINTER(aj_tensor)] * 4 + [vp] +
+                                      [ctypes.POINTER(aj_tensor)] * 4 + [vp])
         for name in SYMBOLS:
             getattr(l, name).restype = ctypes.c_int
         l.attn_jvp_last_error.restype = ctypes.c_char_p
@@ -395,3 +399,21 @@ def attn_bwd_host(plan, q, k, v, o, lse, dout, dq, dk, dv, stream: int = 0) -> N
     if lse is None:
         raise ValueError("attn_bwd_host needs the forward's lse")
     _check(lib().attn_bwd_host(plan, *ptrs[:4], _rowvec(lse, plan, "lse", cuda=False), *ptrs[4:], stream))
+
+
+def attn_bwd_static(problem: aj_problem, mask: aj_mask_desc, q, k, v, o, lse, dout, dq, dk, dv, stream: int = 0) -> None:
+    """attn_bwd without a plan and without any device allocation, for processes that cannot call cudaMalloc (their own pool
+    owns the GPU's memory) or must not (an allocation can stall every stream of the device).  Device tensors as for attn_bwd;
+    the mask descriptor is evaluated inside the kernels (FULL, BLOCK_CAUSAL, TEACHER_FORCING).  The per-row scratch is a
+    fixed array in the library: B * H * Nq <= AJ_STATIC_SCRATCH_MAX_ROWS, and calls that overlap on the GPU race on it."""
+    import torch
+    want_q, want_k = (problem.B, problem.H, problem.Nq, problem.d), (problem.B, problem.H, problem.Nk, problem.d)
+    ts = []
+    for x, n, kk in zip((q, k, v, o, dout, dq, dk, dv), _BWD_NAMES, _BWD_KEYS):
+        if tuple(x.shape) != (want_k if kk else want_q) or x.dtype != _torch_dtype(problem.dtype) or not x.is_cuda:
+            raise ValueError(f"{n}: expected a CUDA {_torch_dtype(problem.dtype)} tensor of shape {want_k if kk else want_q}")
+        ts.append(_tensor(x, None, n, kk))
+    if lse is None or lse.dtype != torch.float32 or not lse.is_contiguous() or not lse.is_cuda or tuple(lse.shape) != want_q[:3]:
+        raise ValueError("lse: expected the forward's contiguous fp32 CUDA tensor [B, H, Nq]")
+    _check(lib().attn_bwd_static(ctypes.byref(problem), ctypes.byref(mask), *[ctypes.byref(x) for x in ts[:4]], lse.data_ptr(),
+                                 *[ctypes.byref(x) for x in ts[4:]], stream))
