@@ -140,25 +140,33 @@ def ulysses_attn_bwd(local_bwd: LocalOp, saved, dout, group=None, head_groups: i
 
 
 # ---------------------------------------------------------------------------------------------- production local ops
-def local_attn_jvp(plan, stream: int = 0) -> LocalOp:
-    """`attn_jvp_fwd` of a plan created for (B, H / (P G) heads, N, N) on this rank's GPU; every head group reuses it."""
+def _launch_stream(stream: Optional[int], device) -> int:
+    """The cudaStream_t the kernel goes on.  None = torch's CURRENT stream of `device` at the moment of the call: the packing
+    copies, the allocations and the collective's wait() in `_pipeline` are all ordered on that stream, so the kernel must be
+    too (under `with torch.cuda.stream(s)` the legacy default stream 0 is ordered against none of them)."""
+    return torch.cuda.current_stream(device).cuda_stream if stream is None else stream
+
+
+def local_attn_jvp(plan, stream: Optional[int] = None) -> LocalOp:
+    """`attn_jvp_fwd` of a plan created for (B, H / (P G) heads, N, N) on this rank's GPU; every head group reuses it.
+    stream: a cudaStream_t handle, or None for torch's current stream when the op runs."""
     from . import binding as aj
 
     def op(g, q, k, v, tq, tk, tv):
         o, to = torch.empty_like(q), torch.empty_like(q)
         lse = torch.empty(q.shape[:3], dtype=torch.float32, device=q.device)
-        aj.attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse, stream)
+        aj.attn_jvp_fwd(plan, q, k, v, tq, tk, tv, o, to, lse, _launch_stream(stream, q.device))
         return o, to, lse
     return op
 
 
-def local_attn_bwd(plan, stream: int = 0) -> LocalOp:
-    """`attn_bwd` of the same plan."""
+def local_attn_bwd(plan, stream: Optional[int] = None) -> LocalOp:
+    """`attn_bwd` of the same plan (stream as in local_attn_jvp)."""
     from . import binding as aj
 
     def op(g, q, k, v, o, lse, dout):
         dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(k)
-        aj.attn_bwd(plan, q, k, v, o, lse, dout, dq, dk, dv, stream)
+        aj.attn_bwd(plan, q, k, v, o, lse, dout, dq, dk, dv, _launch_stream(stream, q.device))
         return dq, dk, dv
     return op
 
