@@ -296,6 +296,24 @@ def test_backward_full_size_all_heads_launch_sampled(name):
     assert torch.count_nonzero(got[1][:, :, half + (n - 1) * C:]) > 0      # the last noisy block's keys are seen by itself
 
 
+@pytest.mark.parametrize("name", ["wan13b_tf_chunkwise", "block_causal_b2"])
+def test_backward_full_size_other_masks_sampled(name):
+    """The transposed packed schedules of the chunk-wise mask (4680-row blocks) and of B = 2 block-causal at full size, all heads
+    in one attn_bwd call: two heads (the first, and the last head of the last batch) at sampled rows and keys of every block."""
+    import dataclasses
+    from paper_2606_25473_b200.workloads import WORKLOADS
+    w = dataclasses.replace(WORKLOADS[name], name=name + "_bwd", backward=True)
+    x = make_inputs(w)
+    dout = _dout(w)
+    got = run_fwd_bwd(w, x, dout)
+    for t in got:
+        assert torch.isfinite(t.float()).all()
+    for i, bh in enumerate([(0, 0), (w.B - 1, w.H - 1)]):
+        idx = _block_samples(w, np.random.default_rng(60 + i), per_block=4)
+        errs = check(w, x, dout, got, heads=[bh], rows=idx, keys=idx)
+        print(f"{w.name} head {bh}: {len(idx)} rows and keys, errs={errs}")
+
+
 def test_backward_config2_one_full_head_every_element():
     """One full head of config 2 through the 12-head launch: every row of dQ and every key of dK, dV of head (0, 11)."""
     from paper_2606_25473_b200.workloads import EXTRA_WORKLOADS
@@ -323,13 +341,19 @@ def test_bwd_host_matches_device_path(w):
     h_o, h_lse = o.cpu().pin_memory(), lse.cpu().pin_memory()
     h = [torch.full_like(x[0], float("nan")).pin_memory(), torch.full_like(x[1], float("nan")).pin_memory(),
          torch.full_like(x[1], float("nan")).pin_memory()]
-    for _ in range(2):                                  # the second call reuses staging buffers, schedules and tensor maps
+    encodes = []
+    for _ in range(3):                                  # later calls reuse staging buffers, schedules and tensor maps
         aj.attn_bwd_host(plan, x[0], x[1], x[2], h_o, h_lse, dout, *h, torch.cuda.current_stream().cuda_stream)
         torch.cuda.synchronize()
         for a, b in zip(h, (dq, dk, dv)):
             assert torch.equal(a, b.cpu())
         for t in h:
             t.fill_(float("nan"))
+        encodes.append(aj.attn_jvp_plan_tensor_map_stats(plan)[0])
+        aj.attn_bwd(plan, q, k, v, o, lse, dout.cuda(), dq, dk, dv, 0)     # alternating with the device call evicts nothing either
+        torch.cuda.synchronize()
+    # steady state encodes nothing, including the per-head augmentation-row maps of the CTA-pair dK/dV pass
+    assert encodes[1] == encodes[0] and encodes[2] == encodes[0] == aj.attn_jvp_plan_tensor_map_stats(plan)[0], encodes
     assert aj.attn_jvp_plan_device_status(plan) == 0
     aj.attn_jvp_plan_destroy(plan)
 
