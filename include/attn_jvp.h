@@ -19,7 +19,8 @@
  *  - Tensors are [B, H, N, d] with d contiguous; strides are in ELEMENTS (aj_tensor).
  *  - Supported: d in {64, 128}.  dtype AJ_BF16 runs tcgen05 / TMEM / TMA kernels: d = 128 on CTA pairs (the performance
  *    path, AJ_KERNEL_UMMA_PAIR), d = 64 on the single-CTA kernels (AJ_KERNEL_UMMA: forward, tangent-free forward and
- *    backward; about two thirds of the d = 128 throughput).  AJ_FP32 (any supported d) runs the
+ *    backward; the forward + JVP reaches about 0.6 of the bf16 tensor peak there and the backward about 0.3, against 0.9 and
+ *    0.5 at d = 128).  AJ_FP32 (any supported d) runs the
  *    plain-FMA SIMT kernels (plain fp32 FMA for the 1e-4 tolerance, R14): a CORRECTNESS path two to three orders
  *    of magnitude slower (a few TFLOP/s), which attn_jvp_plan_kernel reports as AJ_KERNEL_SIMT.
  *    Anything else returns AJ_ERR_UNSUPPORTED.  There is no CPU fallback.
@@ -72,7 +73,7 @@ typedef enum {
  *              (a non-NULL `to` is filled with zeros).  This is the cached-prefix forward of PAPER.md:324-328. */
 typedef enum { AJ_TANGENT_DENSE = 0, AJ_TANGENT_CLEAN_ZERO = 1, AJ_TANGENT_NONE = 2 } aj_tangent_zero;
 
-/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA_PAIR when (bf16, d = 128), else SIMT.
+/* Kernel selection (attn_jvp_plan_set_kernel). AUTO = UMMA_PAIR when (bf16, d = 128), UMMA when (bf16, d = 64), else SIMT.
  * UMMA: one CTA per 128-row query tile (tcgen05.mma.cta_group::1).  UMMA_PAIR: a CTA pair per 256-row query tile
  * (tcgen05.mma.cta_group::2, M = 256; the two SMs share every K/V tile).
  * UMMA_PAIR sends the tasks that need no tangent at all (AJ_TASK_PRIMAL_ONLY: everything under AJ_TANGENT_NONE, the clean
@@ -213,6 +214,41 @@ aj_status attn_jvp_plan_set_kernel(aj_plan *plan, int32_t kernel);
 /* Force a query tiling (aj_tiling).  Default: PACKED for the tcgen05 kernels, PER_GROUP for the SIMT kernel; the SIMT
  * kernel supports only PER_GROUP and the CTA-pair kernel only PACKED (AJ_ERR_UNSUPPORTED otherwise).  Rebuilds and re-uploads the schedule; results do not change. */
 aj_status attn_jvp_plan_set_tiling(aj_plan *plan, int32_t tiling);
+/*
+ * Rendezvous of the CTA-pair forward kernel's workers (AJ_KERNEL_UMMA_PAIR / _ONE).  On long sequences every SM pair streams
+ * the keys of its task on its own schedule; the pairs drift apart and each ends up reading K, tK, V, tV from DRAM instead of
+ * sharing them through L2 (N = 115,200, 24 heads, full mask: 379 GB read per launch for 5.7 GB of inputs).  With a rendezvous
+ * the producers of all pairs meet -- at every task slot of their lists (PER_SLOT: for schedules whose tasks cost the same), or
+ * whenever they enter a new head (PER_HEAD: tasks of different cost; the lists are then levelled at every head) -- through
+ * plan-owned counters that a cudaMemsetAsync on the call's stream clears before every launch.  The wait is bounded (a pair
+ * that waits in vain three times stops waiting for the rest of the launch): a performance hint, never a correctness condition;
+ * results are bit-identical in every mode.
+ *   AUTO      (default) the library turns a mode on where it pays: the longest key stream of a task exceeds what L2 keeps for
+ *             all pairs (48 MB) and the schedule has the shape the mode needs.
+ *   OFF / PER_SLOT / PER_HEAD  force it.  PER_SLOT is ignored on plans with primal-only task lists (AJ_TANGENT_CLEAN_ZERO);
+ *             both are ignored by kernels other than the CTA-pair forward.  attn_jvp_plan_rendezvous reports what is in effect.
+ * Rebuilds and re-uploads the forward schedule (synchronous).  ONE LAUNCH AT A TIME while a mode is in effect: two launches of
+ * the same plan that overlap on the GPU (two streams) share the counters -- the second launch's memset clears what the first
+ * is counting -- so pairs wait for their time-outs (up to 3 x 1.5 M clk each) and the L2 sharing is lost.  Results stay
+ * right.  Callers that overlap launches of one plan should set OFF or use one plan per stream.
+ */
+typedef enum { AJ_RENDEZVOUS_AUTO = 0, AJ_RENDEZVOUS_OFF = 1, AJ_RENDEZVOUS_PER_SLOT = 2, AJ_RENDEZVOUS_PER_HEAD = 3 } aj_rendezvous;
+aj_status attn_jvp_plan_set_rendezvous(aj_plan *plan, int32_t mode);
+/* *in_effect = AJ_RENDEZVOUS_OFF, PER_SLOT or PER_HEAD: what attn_jvp_fwd on this plan does now. */
+aj_status attn_jvp_plan_rendezvous(const aj_plan *plan, int32_t *in_effect);
+/*
+ * Worker budget of the CTA-pair kernels (forward, forward-only, backward): they are persistent, one CTA pair per SM pair
+ * with a host-assigned task list each, and by default take every pair of the device (74 on a B200).  A caller that runs
+ * something else beside them -- the NCCL kernels of the Ulysses all-to-all of the next head group, a
+ * copy kernel -- can leave it room: num_pairs > 0 builds the lists for that many pairs (the grid and the rendezvous targets
+ * follow), 0 restores the default.  Without a budget a pair whose SMs are held by another kernel starts its whole list
+ * late, and the launch ends when that pair does.  Results do not depend on the budget.  Rebuilds and re-uploads the forward
+ * schedule (synchronous); the backward schedules are rebuilt on the next attn_bwd.  Ignored by the single-CTA and SIMT kernels.
+ */
+aj_status attn_jvp_plan_set_workers(aj_plan *plan, int32_t num_pairs);
+/* How many CTA pairs attn_jvp_fwd launches for the general kernel and for the forward-only kernel of the primal-only tasks
+ * (either pointer may be NULL; 0 when that kernel is not launched). */
+aj_status attn_jvp_plan_workers(const aj_plan *plan, int32_t *num_pairs, int32_t *num_primal_pairs);
 /* Which kernel attn_jvp_fwd will launch (aj_kernel, never AUTO) and how many kernel launches one
  * attn_jvp_fwd call makes. */
 aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *launches_per_call);
@@ -222,9 +258,10 @@ aj_status attn_jvp_plan_kernel(const aj_plan *plan, int32_t *kernel, int32_t *la
  * without waiting.  q, tq: [B,H,Nq,d]; k, v, tk, tv: [B,H,Nk,d]; o, to: [B,H,Nq,d] in the problem dtype;
  * lse: contiguous fp32 [B,H,Nq] (may be NULL).  All DEVICE memory; inputs are only read.  Pointers must be
  * 16-byte aligned and strides multiples of 8 elements, stride_n >= d (else AJ_ERR_INVALID_ARG).
- * The forward calls keep no per-call device state in the plan: one plan may be enqueued on several streams at the same time
- * (the tensor-map cache is guarded by a mutex).  attn_bwd and the host-buffer calls own a workspace / staging buffers in
- * the plan: one such call at a time per plan.
+ * The forward calls keep no per-call device state in the plan, except the rendezvous counters of long-sequence plans
+ * (attn_jvp_plan_set_rendezvous: one launch at a time while a mode is in effect): otherwise one plan may be enqueued on several
+ * streams at the same time (the tensor-map cache is guarded by a mutex).  attn_bwd and the host-buffer calls own a workspace /
+ * staging buffers in the plan: one such call at a time per plan.
  * Plans whose mask says AJ_TANGENT_NONE never read tq, tk, tv (they may be NULL), fill a non-NULL `to` with zeros and
  * write O and lse only -- on every kernel (CTA-pair and single-CTA tcgen05, SIMT).
  */

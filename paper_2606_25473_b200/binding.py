@@ -20,6 +20,7 @@ AJ_TILING_PER_GROUP, AJ_TILING_PACKED = 0, 1
 AJ_TANGENT_DENSE, AJ_TANGENT_CLEAN_ZERO, AJ_TANGENT_NONE = 0, 1, 2
 AJ_TASK_PRIMAL_ONLY = 1
 AJ_STATIC_SCRATCH_MAX_ROWS = 1048576
+AJ_RENDEZVOUS_AUTO, AJ_RENDEZVOUS_OFF, AJ_RENDEZVOUS_PER_SLOT, AJ_RENDEZVOUS_PER_HEAD = 0, 1, 2, 3
 
 _I32P = ctypes.POINTER(ctypes.c_int32)
 
@@ -61,7 +62,8 @@ SYMBOLS = [
     "attn_jvp_plan_create", "attn_jvp_plan_destroy", "attn_jvp_plan_info", "attn_jvp_plan_set_kernel", "attn_jvp_plan_set_tiling",
     "attn_jvp_plan_kernel", "attn_jvp_plan_device_status", "attn_jvp_fwd", "attn_jvp_fwd_host", "attn_jvp_last_error", "attn_jvp_version",
     "attn_jvp_fwd_tl", "attn_bwd_host", "attn_jvp_plan_tensor_map_stats", "attn_jvp_schedule_create_transposed_tiled",
-    "attn_bwd_static",
+    "attn_bwd_static", "attn_jvp_plan_set_rendezvous", "attn_jvp_plan_rendezvous",
+    "attn_jvp_plan_set_workers", "attn_jvp_plan_workers",
 ]
 
 _lib = None
@@ -96,6 +98,10 @@ def lib():
         l.attn_jvp_plan_set_kernel.argtypes = [vp, i32]
         l.attn_jvp_plan_set_tiling.argtypes = [vp, i32]
         l.attn_jvp_plan_kernel.argtypes = [vp, _I32P, _I32P]
+        l.attn_jvp_plan_set_rendezvous.argtypes = [vp, i32]
+        l.attn_jvp_plan_rendezvous.argtypes = [vp, _I32P]
+        l.attn_jvp_plan_set_workers.argtypes = [vp, i32]
+        l.attn_jvp_plan_workers.argtypes = [vp, _I32P, _I32P]
         l.attn_jvp_plan_device_status.argtypes = [vp, _I32P]
         l.attn_jvp_fwd.argtypes = [vp] + [ctypes.POINTER(aj_tensor)] * 8 + [vp, vp]
         l.attn_jvp_fwd_host.argtypes = [vp] * 11
@@ -293,6 +299,29 @@ def attn_jvp_plan_set_kernel(plan, kernel: int) -> None:
 
 def attn_jvp_plan_set_tiling(plan, tiling: int) -> None:
     _check(lib().attn_jvp_plan_set_tiling(plan, tiling))
+
+
+def attn_jvp_plan_set_rendezvous(plan, mode: int) -> None:
+    _check(lib().attn_jvp_plan_set_rendezvous(plan, mode))
+
+
+def attn_jvp_plan_rendezvous(plan) -> int:
+    """-> the rendezvous mode in effect (AJ_RENDEZVOUS_OFF, PER_SLOT or PER_HEAD)"""
+    a = ctypes.c_int32()
+    _check(lib().attn_jvp_plan_rendezvous(plan, ctypes.byref(a)))
+    return a.value
+
+
+def attn_jvp_plan_set_workers(plan, num_pairs: int) -> None:
+    """Budget of SM pairs for the CTA-pair kernels (0 = all)."""
+    _check(lib().attn_jvp_plan_set_workers(plan, num_pairs))
+
+
+def attn_jvp_plan_workers(plan):
+    """-> (CTA pairs of the general kernel, CTA pairs of the forward-only kernel)"""
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib().attn_jvp_plan_workers(plan, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def attn_jvp_plan_kernel(plan):

@@ -4,11 +4,11 @@
 
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
 #include <string>
+#include <unordered_map>
 
 #include "internal.hpp"
 #include "kernels.hpp"
@@ -44,9 +44,8 @@ struct aj_plan {
     // head (attn_bwd_host)
     DevSchedule bwd_q, bwd_k, bwd_q_head, bwd_k_head;
     float *d_delta = nullptr;     // workspace of attn_bwd (bwd_alloc_bytes)
-    int32_t bwd_poly_exp = 0;     // AJ_BWD_POLY_EXP env (A/B runs): half of the backward's exponentials on the FMA pipe
-    int32_t no_slot_sync = 0;     // AJ_NO_SLOT_SYNC env (A/B runs): launch without the task-slot / per-head rendezvous
-    int32_t bwd_dq_form = 0;      // dQ pass of the CTA-pair backward: 0 = tile ping-pong, 1 = pair-step form (AJ_BWD_DQ_FORM env, for A/B runs)
+    int32_t rendezvous = AJ_RENDEZVOUS_AUTO;   // attn_jvp_plan_set_rendezvous: what the forward schedules are built for
+    int32_t max_pairs = 0;                     // attn_jvp_plan_set_workers: SM pairs the CTA-pair kernels may occupy (0 = all)
     // attn_jvp_fwd_host / attn_bwd_host: device staging buffers, copy streams, one event per head and direction
     void *d_in[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // q k v tq tk tv
     void *d_out[2] = {nullptr, nullptr};                                      // o to
@@ -66,9 +65,14 @@ struct aj_plan {
     };
     mutable std::mutex mu;
     mutable std::vector<MapSlot> maps;
-    mutable CUtensorMap aug_map[2];             // 2-D maps over the backward's augmentation rows (-lse/s, -delta)
-    mutable const void *aug_map_ptr = nullptr;
-    mutable int64_t aug_map_rows = 0;
+    // 2-D maps over the backward's augmentation rows (-lse/s, -delta), one entry per call site (keyed by its first map slot:
+    // attn_bwd has one, attn_bwd_host one per head, whose workspace pointers differ)
+    struct AugSlot {
+        const void *ptr = nullptr;
+        int64_t rows = 0;
+        CUtensorMap map[2];
+    };
+    mutable std::unordered_map<int, AugSlot> aug_maps;
     mutable int64_t map_encodes = 0, map_hits = 0;
 };
 
@@ -157,19 +161,20 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
         return n;
     };
     if (is_pair(kernel) || workers > 0) {
-        const int want = workers > 0 ? workers : std::max(p->num_sms / 2, 1);
+        const int all_pairs = std::max(p->num_sms / 2, 1);
+        const int want = workers > 0 ? workers : p->max_pairs > 0 ? std::min(p->max_pairs, all_pairs) : all_pairs;
         std::vector<int32_t> general, primal;
         for (size_t t = 0; t < nt; ++t)
             ((kernel == AJ_KERNEL_UMMA_PAIR && (s->tasks[t].flags & AJ_TASK_PRIMAL_ONLY)) ? primal : general).push_back((int32_t)t);
         // Per-head rendezvous (kernel_umma_pair_sm100.cu, UmmaParams::slot_sync with sync_per_head): for the forward CTA-pair kernel when
         // the tasks of a launch differ in cost (equal ones get the task-slot rendezvous below) and the longest key stream of a task
-        // is larger than what L2 keeps for all pairs (K, tK, V, tV rows of 2 d bytes each).  AJ_HEAD_SYNC=1 / 0 forces it on / off
-        // (tests, A/B runs).
+        // is larger than what L2 keeps for all pairs (K, tK, V, tV rows of 2 d bytes each).  attn_jvp_plan_set_rendezvous forces
+        // it on (PER_HEAD) or off (OFF, PER_SLOT).
         if (rendezvous && is_pair(kernel) && workers == 0 && !general.empty()) {
             int32_t tmin = INT32_MAX, tmax = 0;
             for (int32_t t : general) { tmin = std::min(tmin, s->tasks[t].num_kv_tiles); tmax = std::max(tmax, s->tasks[t].num_kv_tiles); }
             head_sync = tmin != tmax && (double)tmax * s->tile_k * 4.0 * p->problem.d * 2.0 > 48e6;
-            if (const char *f = std::getenv("AJ_HEAD_SYNC")) head_sync = std::atoi(f) != 0 && tmax > 0;
+            if (p->rendezvous != AJ_RENDEZVOUS_AUTO) head_sync = p->rendezvous == AJ_RENDEZVOUS_PER_HEAD && tmax > 0;
         }
         num_pairs = assign(general, want, pair_off, pair_ids, head_sync);
         if (general.empty()) num_pairs = 0;
@@ -177,19 +182,22 @@ aj_status upload_schedule(aj_plan *p, aj_schedule *s, int32_t kernel, aj_plan::D
     }
     // Task-slot rendezvous (kernel_umma_pair_sm100.cu): only where it costs nothing and pays -- every task of the launch has the same
     // cost (so the pairs would start each slot together anyway), the lists are long enough for the drift to build up, and one
-    // task's key stream is larger than what L2 keeps (K, tK, V, tV rows of 2 d bytes each).
+    // task's key stream is larger than what L2 keeps (K, tK, V, tV rows of 2 d bytes each).  AJ_RENDEZVOUS_PER_SLOT asks for it
+    // on any schedule of the CTA-pair forward kernel that has no primal-only lists (the wait is bounded, so it is always safe).
     std::vector<int32_t> slot_expect;
-    if (rendezvous && is_pair(kernel) && workers == 0 && num_pairs > 1 && num_prim_pairs == 0 && !pair_ids.empty()) {
+    if (rendezvous && is_pair(kernel) && workers == 0 && num_pairs > 1 && num_prim_pairs == 0 && !pair_ids.empty() &&
+        (p->rendezvous == AJ_RENDEZVOUS_AUTO || p->rendezvous == AJ_RENDEZVOUS_PER_SLOT)) {
         const aj_task &t0 = s->tasks[pair_ids[0]];
         bool uniform = t0.num_kv_tiles > 0;
         for (int32_t t : pair_ids) uniform = uniform && s->tasks[t].num_kv_tiles == t0.num_kv_tiles && s->tasks[t].flags == t0.flags;
         int max_len = 0;
         for (int w = 0; w < num_pairs; ++w) max_len = std::max(max_len, pair_off[w + 1] - pair_off[w]);
         const double stream_bytes = (double)t0.num_kv_tiles * s->tile_k * 4.0 * p->problem.d * 2.0;
-        if (uniform && max_len >= 16 && stream_bytes > 48e6) {
-            slot_expect.assign(max_len, 0);
-            for (int w = 0; w < num_pairs; ++w)
-                for (int i = 0; i < pair_off[w + 1] - pair_off[w]; ++i) ++slot_expect[i];
+        if (p->rendezvous == AJ_RENDEZVOUS_PER_SLOT || (uniform && max_len >= 16 && stream_bytes > 48e6)) {
+            slot_expect.assign(max_len, 0);                    // target of slot i: the pairs whose i-th task streams any keys
+            for (int w = 0; w < num_pairs; ++w)                // (the producer skips key-less tasks without arriving)
+                for (int i = 0; i < pair_off[w + 1] - pair_off[w]; ++i)
+                    if (s->tasks[pair_ids[pair_off[w] + i]].num_kv_tiles > 0) ++slot_expect[i];
         }
     }
     int32_t sync_per_head = 0;
@@ -354,9 +362,6 @@ aj_status attn_jvp_plan_create(const aj_problem *problem, const aj_mask_desc *ma
         e = cudaMalloc(&p->d_counters, 4 * sizeof(int32_t));
         if (e == cudaSuccess) e = cudaMemset(p->d_counters, 0, 4 * sizeof(int32_t));
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "counter allocation"); }
-        if (const char *f = std::getenv("AJ_BWD_DQ_FORM")) p->bwd_dq_form = std::atoi(f) == 1 ? 1 : 0;
-        if (const char *f = std::getenv("AJ_NO_SLOT_SYNC")) p->no_slot_sync = std::atoi(f) != 0 ? 1 : 0;
-        if (const char *f = std::getenv("AJ_BWD_POLY_EXP")) p->bwd_poly_exp = std::atoi(f) == 1 ? 1 : 0;
         const int32_t kernel = auto_kernel(p->problem);
         st = install_schedule(p, kernel, default_tiling(kernel));
     } catch (const std::bad_alloc &) {
@@ -420,6 +425,41 @@ aj_status attn_jvp_plan_set_tiling(aj_plan *p, int32_t tiling) {
     return install_schedule(p, p->kernel, tiling);
 }
 
+aj_status attn_jvp_plan_set_rendezvous(aj_plan *p, int32_t mode) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (mode != AJ_RENDEZVOUS_AUTO && mode != AJ_RENDEZVOUS_OFF && mode != AJ_RENDEZVOUS_PER_SLOT && mode != AJ_RENDEZVOUS_PER_HEAD)
+        return fail(AJ_ERR_INVALID_ARG, "unknown rendezvous mode");
+    if (mode == p->rendezvous) return AJ_OK;
+    const int32_t old = p->rendezvous;
+    p->rendezvous = mode;
+    if (aj_status st = install_schedule(p, p->kernel, p->tiling)) { p->rendezvous = old; return st; }
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_set_workers(aj_plan *p, int32_t num_pairs) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (num_pairs < 0) return fail(AJ_ERR_INVALID_ARG, "num_pairs must be >= 0 (0 = every SM pair of the device)");
+    if (num_pairs == p->max_pairs) return AJ_OK;
+    const int32_t old = p->max_pairs;
+    p->max_pairs = num_pairs;
+    // forward lists now; the backward lists are rebuilt on the next attn_bwd (install_schedule drops them)
+    if (aj_status st = install_schedule(p, p->kernel, p->tiling)) { p->max_pairs = old; return st; }
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_workers(const aj_plan *p, int32_t *num_pairs, int32_t *num_primal_pairs) {
+    if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
+    if (num_pairs) *num_pairs = p->full.num_pairs;
+    if (num_primal_pairs) *num_primal_pairs = p->full.num_prim_pairs;
+    return AJ_OK;
+}
+
+aj_status attn_jvp_plan_rendezvous(const aj_plan *p, int32_t *in_effect) {
+    if (!p || !in_effect) return fail(AJ_ERR_INVALID_ARG, "plan or in_effect is NULL");
+    *in_effect = p->full.num_slots == 0 ? AJ_RENDEZVOUS_OFF : p->full.sync_per_head ? AJ_RENDEZVOUS_PER_HEAD : AJ_RENDEZVOUS_PER_SLOT;
+    return AJ_OK;
+}
+
 aj_status attn_jvp_plan_kernel(const aj_plan *p, int32_t *kernel, int32_t *launches) {
     if (!p) return fail(AJ_ERR_INVALID_ARG, "plan is NULL");
     if (kernel) *kernel = p->kernel;
@@ -476,7 +516,7 @@ aj_status launch_schedule(const aj_plan *p, const aj_plan::DevSchedule &ds, int3
                 e = aj::launch_umma_pair_fwd(pp, ds.num_prim_pairs, stream);
             }
             if (e == cudaSuccess && ds.num_pairs > 0) {
-                if (ds.num_slots > 0 && !p->no_slot_sync) {
+                if (ds.num_slots > 0) {
                     prm.slot_sync = ds.d_slot_sync; prm.slot_expect = ds.d_slot_expect; prm.sync_per_head = ds.sync_per_head;
                     e = cudaMemsetAsync(ds.d_slot_sync, 0, ds.num_slots * sizeof(int32_t), stream);
                 }
@@ -583,26 +623,27 @@ size_t bwd_alloc_bytes(const aj_problem &pr) {
     return std::max(bwd_work_bytes((int64_t)pr.B * pr.H * pr.Nq), bwd_work_bytes(pr.Nq) * (size_t)pr.B * pr.H);
 }
 
-// 2-D maps over the two aug arrays ([rows][16] bf16 each, box {16, 64}); cached in the plan by workspace pointer
-aj_status encode_aug_maps(const aj_plan *plan, CUtensorMap *m1, CUtensorMap *m2, const void *aug, int64_t rows) {
+// 2-D maps over the two aug arrays ([rows][16] bf16 each, box {16, 64}); cached in the plan per call site `slot`
+aj_status encode_aug_maps(const aj_plan *plan, int slot, CUtensorMap *m1, CUtensorMap *m2, const void *aug, int64_t rows) {
     std::lock_guard<std::mutex> lock(plan->mu);
-    if (plan->aug_map_ptr != aug || plan->aug_map_rows != rows) {
+    aj_plan::AugSlot &a = plan->aug_maps[slot];
+    if (a.ptr != aug || a.rows != rows) {
         EncodeTiledFn fn = encode_tiled_fn();
         if (!fn) return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
         for (int i = 0; i < 2; ++i) {
             cuuint64_t dims[2] = {16, (cuuint64_t)rows};
             cuuint64_t strides[1] = {32};
             cuuint32_t box[2] = {16, 64}, estr[2] = {1, 1};
-            CUresult r = fn(&plan->aug_map[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (char *)aug + (size_t)i * rows * 32, dims, strides, box, estr,
+            CUresult r = fn(&a.map[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (char *)aug + (size_t)i * rows * 32, dims, strides, box, estr,
                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            if (r != CUDA_SUCCESS) { plan->aug_map_ptr = nullptr; return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (augmentation rows) failed with CUresult " + std::to_string((int)r)); }
+            if (r != CUDA_SUCCESS) { a.ptr = nullptr; return fail(AJ_ERR_CUDA, "cuTensorMapEncodeTiled (augmentation rows) failed with CUresult " + std::to_string((int)r)); }
         }
-        plan->aug_map_ptr = aug; plan->aug_map_rows = rows;
+        a.ptr = aug; a.rows = rows;
         plan->map_encodes += 2;
     } else {
         plan->map_hits += 2;
     }
-    *m1 = plan->aug_map[0]; *m2 = plan->aug_map[1];
+    *m1 = a.map[0]; *m2 = a.map[1];
     return AJ_OK;
 }
 
@@ -647,16 +688,14 @@ aj_status launch_bwd(const aj_plan *p, const aj_plan::DevSchedule &bq, const aj_
             if (keys) {
                 if ((st = encode_map(p, slot + 4 * pass + 0, &up.tm_a1, *a1, pr, na, aj::UMMA_TILE_Q))) return st;
                 if ((st = encode_map(p, slot + 4 * pass + 1, &up.tm_a2, *a2, pr, na, aj::UMMA_TILE_Q))) return st;
-                if ((st = encode_aug_maps(p, &up.tm_aug1, &up.tm_aug2, aug, rows))) return st;
+                if ((st = encode_aug_maps(p, slot, &up.tm_aug1, &up.tm_aug2, aug, rows))) return st;
             }
             if ((st = encode_map(p, slot + 4 * pass + 2, &up.tm_b1, *b1, pr, nb, aj::UMMA_TILE_K))) return st;
             if ((st = encode_map(p, slot + 4 * pass + 3, &up.tm_b2, *b2, pr, nb, aj::UMMA_TILE_K))) return st;
             if (!keys) {   // the dQ pass stages half a streamed tile (32 rows) per CTA for X and Y: cache slots of the unused a1, a2
                 if ((st = encode_map(p, slot + 0, &up.tm_b1h, *b1, pr, nb, aj::UMMA_TILE_K / 2))) return st;
                 if ((st = encode_map(p, slot + 1, &up.tm_b2h, *b2, pr, nb, aj::UMMA_TILE_K / 2))) return st;
-                up.dq_form = p->bwd_dq_form;
             }
-            up.poly_exp = p->bwd_poly_exp;
             up.a1 = *a1; up.a2 = *a2;
             up.out1 = keys ? *dk : *dq;
             up.out2 = *dv;

@@ -67,10 +67,6 @@ constexpr uint32_t AUG_STAGE_BYTES = 2 * AUG_TILE_BYTES;   // q-aug and dO-aug o
 constexpr int AUG_STAGES = 2;                      // one per ring slot that can hold a {B1, B2} tile (slots 0 and 2 of 4)
 constexpr uint32_t ONES_BYTES = BR * 32;           // 4 KB
 constexpr int NTHREADS = 384;
-#ifndef AJ_BWD_POLY_EXP
-#define AJ_BWD_POLY_EXP 0
-#endif
-constexpr bool POLY_EXP = AJ_BWD_POLY_EXP != 0;      // every other column pair's exponential on the FMA pipe (measured: DESIGN.md 6d)
 
 template <bool KEYS> struct Cfg {
     static constexpr int NSTAGE = KEYS ? 4 : 6;                          // ring slots of 32 KB
@@ -357,7 +353,6 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const float sl2 = prm.scale_log2;
         const uint64_t sl2_2 = pack2(sl2, sl2);
-        const bool poly = prm.poly_exp != 0;
         const uint32_t tX = tmem + lane_base + TM_X + 32 * wg, tY = tmem + lane_base + TM_Y + 32 * wg;   // + 64 i for tile j_i
         uint32_t c_step = 0;
         for (int it = list_begin; it < list_end; ++it) {
@@ -423,14 +418,10 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     for (int c = 0; c < 32; c += 2) {
                         // dQ pass: this thread's row's -lse log2e; KEYS: -lse / s of the column is already inside X
                         const uint64_t x = KEYS ? fmul2(pack2(xu[c], xu[c + 1]), sl2_2) : ffma2(pack2(xu[c], xu[c + 1]), sl2_2, myl_2);
-                        if ((POLY_EXP || poly) && ((c >> 1) & 1)) {      // every other column pair on the FMA pipe instead of the MUFU pipe
-                            unpack2(ex2_poly2(x), w[i][c], w[i][c + 1]);
-                        } else {
-                            float x0, x1;
-                            unpack2(x, x0, x1);
-                            w[i][c] = ex2(x0);
-                            w[i][c + 1] = ex2(x1);
-                        }
+                        float x0, x1;                          // (half of these on the FMA pipe was measured slower: DESIGN.md 6d)
+                        unpack2(x, x0, x1);
+                        w[i][c] = ex2(x0);
+                        w[i][c + 1] = ex2(x1);
                     }
                     const int v = valid[i] - 32 * wg;          // of this warpgroup's 32 columns, the first v are seen
                     if (v < 32) {                              // outside the range / the row interval: p = 0 (selected after the
@@ -828,10 +819,7 @@ cudaError_t launch_bwd_umma_pair(const BwdPairParams &prm, bool keys, int num_pa
     if (keys) {
         if (cudaError_t e = ensure_dynamic_smem(attn_bwd_umma_pair_kernel<true>, (int)Cfg<true>::SMEM_TOTAL, configured[1])) return e;
         attn_bwd_umma_pair_kernel<true><<<2 * num_pairs, NTHREADS, Cfg<true>::SMEM_TOTAL, stream>>>(prm);
-    } else if (prm.dq_form == 1) {      // pair-step form of the dQ pass (kept for comparison: DESIGN.md section 6d)
-        if (cudaError_t e = ensure_dynamic_smem(attn_bwd_umma_pair_kernel<false>, (int)Cfg<false>::SMEM_TOTAL, configured[0])) return e;
-        attn_bwd_umma_pair_kernel<false><<<2 * num_pairs, NTHREADS, Cfg<false>::SMEM_TOTAL, stream>>>(prm);
-    } else {
+    } else {                            // (the pair-step form of this pass, attn_bwd_umma_pair_kernel<false>, was measured slower: DESIGN.md 6d)
         static std::atomic<uint64_t> configured_dq{0};
         if (cudaError_t e = ensure_dynamic_smem(attn_bwd_dq_pair_kernel, (int)DQ_SMEM_TOTAL, configured_dq)) return e;
         attn_bwd_dq_pair_kernel<<<2 * num_pairs, NTHREADS, DQ_SMEM_TOTAL, stream>>>(prm);

@@ -18,9 +18,10 @@
 //   registers in ONE TMEM round trip and stay there across the reference-max decision (168 registers forced three round trips:
 //   5.98 -> 5.66 ms on configs[1]'s mask); the branch holds no function call (PairWaiterInline), or ptxas would spill everything
 //   live across it; tile j1 is handed to the MMA warp first.
-//   Every other column pair takes its exponential from the FMA pipe (ptx::ex2_poly2): at d = 128 a tangent-free pair-step is
-//   1024 clk of tensor work against 128 x 128 exponentials = 1024 clk of the 16-lane/clk MUFU pipe, so the MUFU pipe alone
-//   would cap the kernel at the tensor roofline with no slack at all.
+//   All exponentials run on the MUFU pipe.  At d = 128 a tangent-free pair-step is 1024 clk of tensor work against
+//   128 x 128 exponentials = 1024 clk of the 16-lane/clk MUFU pipe, so that pipe has no slack; moving every other column pair to
+//   a polynomial on the FMA pipe was built and measured SLOWER (8.42 against 5.95 ms: the softmax warps are issue-bound, and
+//   the polynomial costs ten instructions for the MUFU's one) and is not in the product.
 // Roles per CTA: warp 0 TMA producer, warp 1 MMA issuer (leader CTA), warp 2 TMEM allocator (80 registers), warps 4-11 softmax /
 // epilogue (208 registers).
 #include <cuda_bf16.h>
@@ -60,10 +61,6 @@ constexpr int NTHREADS = 384;
 
 constexpr uint32_t TM_O = 0, TM_S = 128;           // S buffer b at TM_S + 128 b; P~(j_i) over the first 32 columns of its tile's 64
 constexpr float RESCALE_THRESHOLD = 8.0f;          // log2 units
-#ifndef AJ_FWD_POLY_EXP
-#define AJ_FWD_POLY_EXP 0
-#endif
-constexpr bool POLY_EXP = AJ_FWD_POLY_EXP != 0;      // every other column pair's exponential on the FMA pipe (measured: DESIGN.md 6c)
 constexpr float M_UNSET = -1.0e30f;
 
 enum {
@@ -378,24 +375,17 @@ attn_fwd_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
                     named_bar_arrive(1 + 2 * q4 + (int)(g & 1), 64);
                 }
                 // ---- pass 2: P~ = exp2(S s log2e - m_ref); l += rowsum; bf16 P~ over the tile's first 32 columns.
-                // Every other column pair takes its exponential from the FMA pipe (ex2_poly2) instead of the MUFU pipe; tiles with
-                // masked columns use the MUFU alone (exp2(-inf) = 0 exactly).
+                // Masked columns hold -inf: exp2(-inf) = 0 exactly.
                 const uint64_t negm2 = pack2(-m_ref, -m_ref);
                 auto exp_tile = [&](int i, const uint32_t (&a)[32], const uint32_t (&b)[32]) {
                     uint32_t pk[32];
-                    const bool whole = valid[i] == BC;
 #pragma unroll
                     for (int c = 0; c < 64; c += 2) {
                         const uint32_t u0 = c < 32 ? a[c & 31] : b[c & 31], u1 = c < 32 ? a[(c + 1) & 31] : b[(c + 1) & 31];
                         const uint64_t x = ffma2(pack2(u0, u1), sl2_2, negm2);
-                        uint64_t e;
-                        if (POLY_EXP && ((c >> 1) & 1) && whole) {
-                            e = ex2_poly2(x);
-                        } else {
-                            float x0, x1;
-                            unpack2(x, x0, x1);
-                            e = pack2(ex2(x0), ex2(x1));
-                        }
+                        float x0, x1;
+                        unpack2(x, x0, x1);
+                        const uint64_t e = pack2(ex2(x0), ex2(x1));
                         l2[(c >> 1) & 1] = fadd2(l2[(c >> 1) & 1], e);
                         float p0, p1;
                         unpack2(e, p0, p1);

@@ -32,6 +32,7 @@
 #include <cstdio>
 
 #include "kernels.hpp"
+#include "pair_common.cuh"
 #include "umma_ptx.cuh"
 
 namespace aj {
@@ -39,9 +40,13 @@ namespace aj {
 namespace {
 
 using namespace ptx;
+using pairk::PairWaiter;
+using pairk::RowCursor;
+using pairk::Tile;
+using pairk::TileCursor;
 
 constexpr int BR = 128;                // query rows per CTA (UMMA M = 256 over the pair)
-constexpr int BC = UMMA_TILE_K;        // 64 keys per tile
+using pairk::BC;                       // 64 keys per tile
 constexpr int D = 128;
 constexpr int NSTAGE = 5;              // ring slots of 32 KB
 constexpr uint32_t Q_BYTES = BR * D * 2;           // 32 KB
@@ -78,94 +83,6 @@ constexpr uint32_t IDESC_PV = make_idesc(D, true);         // 256 x 128 x 16, B 
 constexpr uint32_t DESC_HI = desc_hi(1024);                // 8-row / 8-key groups are 1024 B apart
 constexpr uint32_t LBO_CANON = desc_lo_lbo(16);            // single 64-column block per operand: LBO unused
 
-__device__ __noinline__ void pair_wait_slow(uint32_t bar, int idx, uint32_t parity, volatile int *abort_flag, int32_t *err) {
-    const long long t0 = clock64();
-    uint32_t spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0x3f) == 0) {
-            if (*abort_flag) return;
-            if (clock64() - t0 > 4000000000LL) {
-                printf("attn_jvp umma pair: timeout block %d thread %d barrier %d parity %u\n", blockIdx.x, threadIdx.x, idx, parity);
-                *abort_flag = 1;
-                atomicExch(err, 100 + idx);
-                return;
-            }
-        }
-    }
-}
-struct PairWaiter {
-    uint32_t bars;
-    volatile int *abort_flag;
-    int32_t *err;
-    __device__ __forceinline__ void operator()(int idx, uint32_t parity) const {
-        const uint32_t bar = bars + 8u * idx;
-        if (mbar_try_wait(bar, parity)) return;
-        if (mbar_try_wait(bar, parity)) return;
-        pair_wait_slow(bar, idx, parity, abort_flag, err);
-    }
-};
-
-// One 64-key tile of a task's key stream.
-struct Tile { int key_row, valid, entry; };
-// Walks the key tiles of a task in order: schedule entries [rb, rb + rc), each cut into BC-key tiles from its start.
-struct TileCursor {
-    const int32_t *kb, *ke;
-    int r, rend, k, kend;
-    __device__ void init(const int32_t *k_begin, const int32_t *k_end, int rb, int rc) {
-        kb = k_begin; ke = k_end; r = rb; rend = rb + rc;
-        if (r < rend) { k = kb[r]; kend = ke[r]; } else { k = 0; kend = 0; }
-    }
-    __device__ Tile get() const { return Tile{k, min(BC, kend - k), r}; }
-    __device__ void next() {
-        k += BC;
-        if (k >= kend) { ++r; if (r < rend) { k = kb[r]; kend = ke[r]; } }
-    }
-};
-
-// The softmax role's view of a task's key stream: how many columns of the next tile this thread's row sees
-// (inside the entry's key range and the entry's row interval).  The next entry is fetched when the
-// current one is entered, so that crossing into it costs no memory latency.
-struct RowCursor {
-    const int32_t *kb, *ke;
-    const uint32_t *rows;
-    int r, rend, prow;
-    int rem;             // keys left in the current entry
-    bool sees;           // this row is inside the current entry's row interval
-    int nkb, nke;        // the next entry as loaded (decoded only when it is entered, so the loads stay in flight)
-    uint32_t nrr;
-    __device__ __forceinline__ void fetch_next() {
-        if (r + 1 < rend) { nkb = kb[r + 1]; nke = ke[r + 1]; nrr = rows[r + 1]; }
-        else { nkb = 0; nke = 0; nrr = 0; }
-    }
-    __device__ __forceinline__ void advance() {
-        ++r;
-        rem = nke - nkb;
-        sees = prow >= (int)(nrr & 0xffffu) && prow < (int)((nrr >> 16) & 0x7fffu);
-        fetch_next();
-    }
-    __device__ __forceinline__ void init(const int32_t *k_begin, const int32_t *k_end, const uint32_t *row_iv, int rb, int rc, int row) {
-        kb = k_begin; ke = k_end; rows = row_iv; r = rb - 2; rend = rb + rc; prow = row;
-        nkb = 0; nke = 0; nrr = 0;
-        advance();           // r = rb - 1: fetches entry rb
-        advance();           // r = rb: current = entry rb, next = entry rb + 1
-    }
-    // columns of the next tile this row sees; consumes the tile
-    __device__ __forceinline__ int tile() {
-        const int v = sees ? min(BC, rem) : 0;
-        rem -= BC;
-        if (rem <= 0) advance();
-        return v;
-    }
-    // both tiles of a pair-step that lies inside the current entry
-    __device__ __forceinline__ bool pair_inside() const { return rem >= 2 * BC; }
-    __device__ __forceinline__ int pair() {
-        const int v = sees ? BC : 0;
-        rem -= 2 * BC;
-        if (rem <= 0) advance();
-        return v;
-    }
-};
-
 struct Shared {
     uint64_t bars[NUM_BARS];
     uint32_t tmem_base;
@@ -182,7 +99,7 @@ attn_jvp_umma_pair_kernel(const __grid_constant__ UmmaParams prm) {
     Shared *sh = reinterpret_cast<Shared *>(smem_raw + (tiles - raw) + SMEM_TILES);
     const uint32_t sQ = tiles, sTQ = tiles + Q_BYTES, sRing = tiles + 2 * Q_BYTES;
     const uint32_t bars = smem_u32(sh->bars);
-    const PairWaiter wait{bars, &sh->abort_flag, prm.counters + 2};
+    const PairWaiter wait{bars, &sh->abort_flag, prm.counters + 2, 100};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();              // 0 = leader (issues the MMAs, owns the "full" barriers)
     const uint32_t lead_bars = mapa(bars, 0);             // the leader's barrier array in the cluster window

@@ -81,8 +81,6 @@ cudaError_t launch_bwd_umma(const BwdUmmaParams &prm, int d, bool keys, int grid
 struct BwdPairParams {
     CUtensorMap tm_a1, tm_a2, tm_b1, tm_b2, tm_aug1, tm_aug2;
     CUtensorMap tm_b1h, tm_b2h;       // dQ pass, tile ping-pong form: streamed operands with box {64, 32} (half a tile per CTA)
-    int32_t dq_form;                  // dQ pass: 0 = tile ping-pong (default), 1 = pair-step form
-    int32_t poly_exp;                 // pair-step kernels: every other column pair's exponential on the FMA pipe (A/B switch)
     aj_tensor out1, out2;             // dQ | dK, dV
     aj_tensor a1, a2;                 // dQ pass: Q and dO as plain views (their rows go to TMEM, not to shared memory)
     const float2 *ld;                 // [B, H, Nq] {lse log2e, delta}

@@ -218,27 +218,6 @@ __device__ __forceinline__ float ex2(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// 2^x for two values on the FMA / ALU pipes, no MUFU (the 16-lane/clk MUFU pipe is what bounds the softmax of a tangent-free
-// attention step on sm_100: 128 x 128 exponentials against 1024 clk of tensor work).  x = n + f with n = round(x) taken from
-// the low mantissa bits of x + 1.5 * 2^23, f in [-0.5, 0.5]; 2^f by a degree-3 minimax polynomial (max relative error
-// 7.5e-5, far below the bf16 rounding of every consumer of the result); 2^n by adding n to the exponent field.
-// Inputs below -126 are clamped (result ~1e-38 instead of 0); inputs must be < 128 and not NaN.
-__device__ __forceinline__ uint64_t ex2_poly2(uint64_t x2) {
-    float x0, x1;
-    unpack2(x2, x0, x1);
-    x2 = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
-    const uint64_t magic = pack2(12582912.f, 12582912.f), nmagic = pack2(-12582912.f, -12582912.f), neg1 = pack2(-1.f, -1.f);
-    const uint64_t t = fadd2(x2, magic);                    // low mantissa bits = n (two's complement)
-    const uint64_t f = ffma2(fadd2(t, nmagic), neg1, x2);   // x - n
-    uint64_t p = ffma2(f, pack2(0.055170975625514984f, 0.055170975625514984f), pack2(0.2426094263792038f, 0.2426094263792038f));
-    p = ffma2(p, f, pack2(0.6932609677314758f, 0.6932609677314758f));
-    p = ffma2(p, f, pack2(0.9999281764030457f, 0.9999281764030457f));
-    uint32_t t0, t1, p0, p1;
-    asm("mov.b64 {%0, %1}, %2;" : "=r"(t0), "=r"(t1) : "l"(t));
-    asm("mov.b64 {%0, %1}, %2;" : "=r"(p0), "=r"(p1) : "l"(p));
-    return pack2(p0 + (t0 << 23), p1 + (t1 << 23));
-}
-
 // bf16x2 with `lo` in bits [0,16) and `hi` in bits [16,32), round to nearest even
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     uint32_t r;

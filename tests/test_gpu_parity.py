@@ -231,25 +231,74 @@ def test_one_plan_on_two_streams_at_once(kernel):
             assert torch.equal(a, b)
 
 
-def test_per_head_rendezvous_forced_on_a_small_problem(monkeypatch):
-    # Long-sequence launches whose tasks differ in cost make the SM pairs meet before every head (UmmaParams::slot_sync in
-    # per-head mode; configs[4] turns it on by itself, and its full-mask control the per-slot mode).  AJ_HEAD_SYNC=1 forces the
-    # mode on a problem the oracle finishes in seconds: more tasks than pairs, eight heads, same results as without it.
+@pytest.mark.parametrize("mode", ["per_head", "per_slot"])
+def test_rendezvous_forced_on_a_small_problem(mode):
+    # Long-sequence launches make the SM pairs meet -- before every head when their tasks differ in cost (configs[4] turns that
+    # on by itself), at every task slot when they cost the same (its full-mask control).  attn_jvp_plan_set_rendezvous forces
+    # either mode on a problem the oracle finishes in seconds: more tasks than pairs, eight heads, same results as without it.
     w = Workload("head_sync", 2, 4, 128, "block_causal", 1000, 5, 1, "bf16", 0.1, seed=51)
     x = make_inputs(w)
-    plain = run_gpu(w, x)
-    monkeypatch.setenv("AJ_HEAD_SYNC", "1")
     plan = make_plan(w)
+    assert aj.attn_jvp_plan_rendezvous(plan) == aj.AJ_RENDEZVOUS_OFF          # AUTO leaves it off on short key streams
+    plain = run_gpu(w, x, plan=plan)
+    want = aj.AJ_RENDEZVOUS_PER_HEAD if mode == "per_head" else aj.AJ_RENDEZVOUS_PER_SLOT
+    aj.attn_jvp_plan_set_rendezvous(plan, want)
+    assert aj.attn_jvp_plan_rendezvous(plan) == want
     synced = run_gpu(w, x, plan=plan)
     synced2 = run_gpu(w, x, plan=plan)
+    # two launches of the plan in flight at once share the counters: allowed to be slow, not to be wrong (attn_jvp.h)
+    dev = [t.cuda() for t in x]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    conc = [[torch.full_like(dev[0], float("nan")), torch.full_like(dev[0], float("nan")),
+             torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32, device="cuda")] for _ in streams]
+    torch.cuda.synchronize()
+    for st, out in zip(streams, conc):
+        aj.attn_jvp_fwd(plan, *dev, *out, st.cuda_stream)
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_set_rendezvous(plan, aj.AJ_RENDEZVOUS_OFF)
+    assert aj.attn_jvp_plan_rendezvous(plan) == aj.AJ_RENDEZVOUS_OFF
+    off = run_gpu(w, x, plan=plan)
     aj.attn_jvp_plan_destroy(plan)
-    monkeypatch.delenv("AJ_HEAD_SYNC")
     rows = {(0, 0): np.arange(0, w.N, 7), (1, 3): np.arange(3, w.N, 11)}
     compare(w, synced, run_oracle(w, x, rows))
-    for a, b in zip(synced, synced2):
-        assert torch.equal(a, b)
-    for a, b in zip(synced, plain):                       # the lists differ (levelled at every head), the arithmetic per task does not
-        assert torch.equal(a, b)
+    for other in (synced2, plain, off, [t.cpu() for t in conc[0]], [t.cpu() for t in conc[1]]):
+        for a, b in zip(synced, other):                   # the lists may differ (levelled at every head), the arithmetic per task does not
+            assert torch.equal(a, b)
+
+
+def test_worker_budget_leaves_sm_pairs_free_and_keeps_the_bits():
+    # attn_jvp_plan_set_workers: task lists for fewer SM pairs (room for a collective's kernels beside the persistent grid).
+    # Forward + JVP (general and forward-only kernel of a clean-zero plan) and the backward: same bits under every budget.
+    w = Workload("budget", 1, 4, 128, "teacher_forcing", 700, 4, 1, "bf16", 0.1, seed=61, clean_tangent_zero=True)
+    x = make_inputs(w)
+    g = torch.Generator().manual_seed(62)
+    dout = torch.randn(x[0].shape, generator=g).to(torch.bfloat16).cuda()
+    plan = make_plan(w)
+    full_pairs = aj.attn_jvp_plan_workers(plan)
+    assert full_pairs[0] > 8 and full_pairs[1] > 8
+
+    def run():
+        o, to, lse = [t.cuda() for t in run_gpu(w, x, plan=plan)]
+        dev = [t.cuda() for t in x]
+        grads = [torch.full_like(dev[0], float("nan")) for _ in range(3)]
+        aj.attn_bwd(plan, dev[0], dev[1], dev[2], o, lse, dout, *grads, 0)
+        torch.cuda.synchronize()
+        assert aj.attn_jvp_plan_device_status(plan) == 0
+        return [o, to, lse] + grads
+
+    ref = run()
+    for budget in (8, 1, 66):
+        aj.attn_jvp_plan_set_workers(plan, budget)
+        pairs = aj.attn_jvp_plan_workers(plan)
+        assert pairs[0] == min(budget, full_pairs[0]) and pairs[1] == min(budget, full_pairs[1])
+        for a, b in zip(run(), ref):
+            assert torch.equal(a, b)
+    aj.attn_jvp_plan_set_workers(plan, 0)
+    assert aj.attn_jvp_plan_workers(plan) == full_pairs
+    aj.attn_jvp_plan_destroy(plan)
+    rows = {(0, h): np.arange(h, w.N, 13) for h in range(w.H)}
+    compare(w, [t.cpu() for t in ref[:3]], run_oracle(w, x, rows))
 
 
 def test_umma_zero_tangents_give_exact_zero():
@@ -611,6 +660,34 @@ def test_ulysses_sequence_shards_with_the_cuda_local_op_against_the_oracle(P, G)
             ref = oracle.attn_bwd_head(om, widen(x[0][0, hh]), widen(x[1][0, hh]), widen(x[2][0, hh]), widen(dout[0, hh]),
                                        1.0 / np.sqrt(w.d))[i]
             assert max_norm_err(got[0, hh].double().numpy(), ref) <= 1e-2, (name, hh)
+
+
+def test_ulysses_local_ops_follow_torchs_current_stream():
+    """local_attn_jvp / local_attn_bwd without a stream argument launch on torch's current stream AT CALL TIME: under
+    `with torch.cuda.stream(s)` the inputs are produced on s (here behind a long sleep), so a kernel on the legacy default
+    stream would read them before they exist.  Same bits as the synchronous run."""
+    from paper_2606_25473_b200 import ulysses
+    w = SMALL_UMMA[0]
+    x = make_inputs(w)
+    g = torch.Generator().manual_seed(23)
+    dout = torch.randn(x[0].shape, generator=g).to(w.torch_dtype)
+    plan = make_plan(w)
+    fwd, bwd = ulysses.local_attn_jvp(plan), ulysses.local_attn_bwd(plan)
+    dev = [t.cuda() for t in x] + [dout.cuda()]
+    o, to, lse = fwd(0, *dev[:6])
+    ref = (o, to, lse) + bwd(0, dev[0], dev[1], dev[2], o, lse, dev[6])
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        torch.cuda._sleep(200_000_000)                       # ~0.1 s: everything below on s is still pending when enqueued
+        late = [torch.zeros_like(t).copy_(t, non_blocking=True) for t in dev]
+        o, to, lse = fwd(0, *late[:6])
+        got = (o, to, lse) + bwd(0, late[0], late[1], late[2], o, lse, late[6])
+    torch.cuda.synchronize()
+    assert aj.attn_jvp_plan_device_status(plan) == 0
+    aj.attn_jvp_plan_destroy(plan)
+    for a, b in zip(got, ref):
+        assert torch.equal(a, b)
 
 
 def test_ulysses_pipeline_with_nccl_world_size_1():
