@@ -146,8 +146,9 @@ class ClockSampler:
             # "under load" = samples in the upper half of the power range (skips idle samples at the edges)
             thr = 0.5 * (max(power) + min(power))
             loaded = [c for c, p in zip(sm, power) if p >= thr] or sm
+            loaded_p = [p for p in power if p >= thr] or power
             res.update(sm_mhz=statistics.median(loaded), sm_max_mhz=max(smax), reasons=sorted(reasons),
-                       samples=len(sm), power_w_max=max(power))
+                       samples=len(sm), power_w_max=max(power), power_w_loaded=sum(loaded_p) / len(loaded_p))
         return res
 
 
@@ -173,6 +174,39 @@ def time_oracle_sample(w: Workload, inputs, budget_s: float, seed: int = 0):
     dt = time.perf_counter() - t0
     flops = 12.0 * w.d * float(allowed_keys_per_row(w, rows).sum())
     return flops / dt / 1e12, dt, nrows, oracle.num_threads(), (rows,) + tuple(ref)
+
+
+def rows_seeing_key(w: Workload, keys: np.ndarray) -> np.ndarray:
+    """How many query rows see each key, from the block structure (accounting only, for the CPU backward sample)."""
+    C, n = w.block_len, w.num_blocks
+    if w.mask == "full":
+        return np.full(keys.shape, w.num_queries, dtype=np.int64)
+    if w.mask == "block_causal":
+        return (n - keys // C) * C
+    half = w.N // 2
+    j = (keys % half) // C
+    return np.where(keys < half, (n - j) * C + (n - 1 - j) * C, C)   # clean key: clean blocks >= j and noisy blocks > j
+
+
+def time_oracle_bwd_sample(w: Workload, q, k, v, dout, n_sample: int, seed: int = 0):
+    """The backward oracle as it stands on head (0, 0): its pass over ALL query rows (lse and delta, which every key needs)
+    plus dQ of `n_sample` seeded rows and dK, dV of `n_sample` seeded keys.
+    -> (TFLOP/s over the contractions the oracle executed, seconds, cores, (rows, keys, dq, dk, dv))."""
+    import oracle
+    oracle.build()
+    om = {"teacher_forcing": oracle.teacher_forcing_mask, "block_causal": oracle.block_causal_mask}.get(w.mask)
+    om = om(w.block_len, w.num_blocks) if om else oracle.full_mask()
+    rng = np.random.default_rng(seed)
+    rows = np.unique(rng.integers(0, w.num_queries, size=n_sample))
+    keys = np.unique(rng.integers(0, w.N, size=n_sample))
+    args = [x[0, 0].float().numpy() for x in (q, k, v, dout)]
+    t0 = time.perf_counter()
+    dq, dk, dv = oracle.attn_bwd_head(om, *args, 1.0 / float(np.sqrt(w.d)), rows, keys)
+    dt = time.perf_counter() - t0
+    # executed: S and dP for every pair of the head (2 contractions), dQ for the sampled rows (1), S, dP, dK, dV for the sampled keys (4)
+    flops = 2.0 * w.d * (2.0 * w.unmasked_pairs_per_head + float(allowed_keys_per_row(w, rows).sum()) +
+                         4.0 * float(rows_seeing_key(w, keys).sum()))
+    return flops / dt / 1e12, dt, oracle.num_threads(), (rows, keys, dq, dk, dv)
 
 
 def run_reference(args, w: Workload):
@@ -214,8 +248,19 @@ def workload_config(w: Workload):
                                 "4*d per unmasked pair (S and P V only)" if w.no_tangents else
                                 "2*d per contraction actually needed per unmasked pair (2, 4 or 6 of them: zero clean tangents)"
                                 if w.clean_tangent_zero else "12*d per unmasked pair"),
-            "l2": "no flush: the six inputs (%.2f GB) are larger than the 126 MB L2" %
-                  (6 * w.B * w.H * w.N * w.d * (2 if w.dtype == "bf16" else 4) / 1e9)}
+            "l2": ("no flush: the inputs (%.2f GB) are larger than the 126 MB L2" % (input_bytes(w) / 1e9) if not needs_l2_flush(w) else
+                   "flushed: a 256 MB buffer is overwritten between timed launches (the inputs, %.3f GB, would stay in the 126 MB L2); "
+                   "every launch is timed by its own event pair" % (input_bytes(w) / 1e9))}
+
+
+def input_bytes(w: Workload) -> int:
+    eb = 2 if w.dtype == "bf16" else 4
+    per_q, per_k = w.B * w.H * w.num_queries * w.d * eb, w.B * w.H * w.N * w.d * eb
+    return (1 if w.no_tangents else 2) * (per_q + 2 * per_k)
+
+
+def needs_l2_flush(w: Workload) -> bool:
+    return input_bytes(w) < 2 * 126e6
 
 
 # ----------------------------------------------------------------------------------------------- distributed glue
@@ -325,17 +370,43 @@ def run_cuda(args, w: Workload):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if needs_l2_flush(w) else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    ev_b = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
     torch.cuda.synchronize()
     ev[0].record(stream)
     for i in range(K):
+        if flush is not None:          # small inputs: evict them from L2, then time this launch alone
+            flush.zero_()
+        ev_b[i].record(stream)
         step_device()
         ev[i + 1].record(stream)
     torch.cuda.synchronize()
     barrier(inited)
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = ev[0].elapsed_time(ev[K])
-    per_launch = [ev[i].elapsed_time(ev[i + 1]) for i in range(K)]
+    per_launch = [ev_b[i].elapsed_time(ev[i + 1]) for i in range(K)]
+    total_ms = ev[0].elapsed_time(ev[K]) if flush is None else sum(per_launch)
+    del flush
+
+    # ---- energy per launch: board power (nvidia-smi, 100 ms samples) over a loop of at least 2.5 s of back-to-back launches
+    energy = None
+    if rank == 0 and world == 1 and not args.no_energy:
+        n_loop = max(K, int(2.5e3 / max(total_ms / K, 1e-3)) + 1)
+        ps = ClockSampler(local)
+        ps.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n_loop):
+            step_device()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        pw = ps.stop()
+        loop_ms = e0.elapsed_time(e1)
+        if pw.get("power_w_loaded"):
+            joule = pw["power_w_loaded"] * loop_ms * 1e-3 / n_loop
+            energy = {"energy_j_per_launch": joule, "pj_per_counted_flop": joule / flops * 1e12, "mean_board_power_w": pw["power_w_loaded"],
+                      "sm_mhz": pw["sm_mhz"], "launches": n_loop, "loop_s": loop_ms * 1e-3, "ms_per_launch": loop_ms / n_loop,
+                      "how": "mean of nvidia-smi power.draw samples in the upper half of the power range x loop time / launches"}
     total_ms_all, flops_all = aggregate(total_ms, flops * K, inited, dev)
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the six inputs + kernel + D2H of O, tO, lse
@@ -420,6 +491,24 @@ def run_cuda(args, w: Workload):
                   "to": None if w.no_tangents else nerr(to[0, 0][rsel], rto), "metric": "max|gpu - oracle| / max|oracle|",
                   "tolerance": {"o": 1e-2, "to": 1e-2, "lse": 1e-3} if w.dtype == "bf16" else {"o": 1e-4, "to": 1e-4, "lse": 1e-4}}
         parity["ok"] = all(parity[k] is None or parity[k] <= parity["tolerance"][k] for k in ("o", "to", "lse"))
+    bwd_leg = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and w.backward:
+        # the gradients that were just timed, head (0, 0), against the backward oracle on sampled rows and keys
+        step_device()
+        torch.cuda.synchronize()
+        tf, dt, cores, (rows, keys, rdq, rdk, rdv) = time_oracle_bwd_sample(w, h_bwd[0], h_bwd[1], h_bwd[2], h_bwd[4], args.bwd_parity_samples)
+        bwd_leg = (tf, dt, cores, len(rows), len(keys))
+        rsel, ksel = torch.from_numpy(rows).to(dev), torch.from_numpy(keys).to(dev)
+
+        def nerr(got, ref):
+            den = float(np.max(np.abs(ref)))
+            return float(np.max(np.abs(got.double().cpu().numpy() - ref)) / (den if den > 0 else 1.0))
+
+        tol = 1e-2 if w.dtype == "bf16" else 1e-4
+        parity = {"rows": int(len(rows)), "keys": int(len(keys)), "head": [0, 0], "dq": nerr(dq[0, 0][rsel], rdq),
+                  "dk": nerr(dk[0, 0][ksel], rdk), "dv": nerr(dv[0, 0][ksel], rdv), "metric": "max|gpu - oracle| / max|oracle|",
+                  "tolerance": {"dq": tol, "dk": tol, "dv": tol}}
+        parity["ok"] = all(parity[k] <= tol for k in ("dq", "dk", "dv"))
 
     aj.attn_jvp_plan_destroy(plan)
     if rank != 0:
@@ -479,6 +568,8 @@ def run_cuda(args, w: Workload):
         line["equivalent_dense_tflops"] = 12.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (avg_launch_ms * 1e-3) / 1e12
     if overhead_us is not None:
         line["launch_overhead_us"] = overhead_us
+    if energy is not None:
+        line["energy"] = energy
     if parity is not None:
         line["parity"] = parity
     if cpu_leg is not None:                                          # (the timed oracle leg is the forward oracle)
@@ -486,6 +577,20 @@ def run_cuda(args, w: Workload):
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{nrows} uniformly sampled query rows of head (0,0), all their allowed "
                                           f"keys, {dt:.1f} s", "extrapolated_full_config_s": flops / (tf * 1e12)}
+    if bwd_leg is not None:
+        tf, dt, cores, nr, nk_s = bwd_leg
+        line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"head (0,0): the backward oracle's pass over all {w.num_queries} query rows (lse, delta), dQ of "
+                                          f"{nr} sampled rows, dK and dV of {nk_s} sampled keys, {dt:.1f} s",
+                                "flop_convention": "2*d per contraction the oracle executed (S and dP per pair of the head; dQ per "
+                                                   "sampled row; S, dP, dK, dV per sampled key)",
+                                "extrapolated_full_config_s": 14.0 * w.d * w.unmasked_pairs_per_head * w.B * w.H / (tf * 1e12)}
+    if parity is not None and not parity["ok"]:
+        # a fast wrong kernel must not score: no value, and a failing exit status
+        line["value"] = None
+        line["invalid"] = "the timed outputs are outside the tolerance against the oracle (see parity)"
+        print(json.dumps(line), flush=True)
+        raise SystemExit(3)
     print(json.dumps(line), flush=True)
 
 
@@ -602,6 +707,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(WORKLOADS) + list(EXTRA_WORKLOADS))
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-energy", action="store_true", help="skip the 2.5 s power loop")
+    ap.add_argument("--bwd-parity-samples", type=int, default=512, help="backward workloads: query rows / keys of head (0,0) held against the oracle")
     ap.add_argument("--ulysses", action="store_true", help="sequence-sharded ranks with the all-to-all on both sides of the kernel")
     ap.add_argument("--head-groups", type=int, default=2, help="--ulysses: head groups per rank (exchange / kernel pipelining)")
     args = ap.parse_args()

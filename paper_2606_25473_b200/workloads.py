@@ -92,6 +92,13 @@ EXTRA_WORKLOADS: Dict[str, Workload] = {w.name: w for w in [
     # (PAPER.md:180), and the rollout shape: one chunk of queries against the cached prefix plus itself.
     Workload("wan13b_tf_framewise_fwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.0, 0, False, True),
     Workload("wan13b_chunk_vs_prefix_fwd", 8, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
+    # ... at the batch size the paper's inference uses (PAPER.md:410 "batch size 1"; :326 one block at a time against the cached
+    # prefix): a frame (1560 queries) or a 3-frame chunk (4680) against 21 frames of keys, all 12 heads and one rank's 3 heads
+    # behind a P = 4 Ulysses split.  7 / 19 query tiles per head: fewer tasks than SM pairs (no split of a task's key stream yet).
+    Workload("wan13b_frame_vs_prefix_fwd_b1", 1, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 1560),
+    Workload("wan13b_chunk_vs_prefix_fwd_b1", 1, 12, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
+    Workload("wan13b_frame_vs_prefix_fwd_b1_h3", 1, 3, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 1560),
+    Workload("wan13b_chunk_vs_prefix_fwd_b1_h3", 1, 3, 128, "full", 1560, 21, 1, "bf16", 0.0, 0, False, True, 3 * 1560),
     # N2: the primal backward of configs[1]
     Workload("wan13b_tf_framewise_bwd", 1, 12, 128, "teacher_forcing", 1560, 21, 1, "bf16", 0.1, 0, False, False, 0, True),
     # The plain-FMA (SIMT) correctness paths at a size that gives a throughput figure: fp32 inputs (the 1e-4 path of configs[0])

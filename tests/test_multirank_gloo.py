@@ -115,8 +115,27 @@ for grp in range(G):
         for j in range(P):
             sel[j * h + grp * hg:j * h + (grp + 1) * hg] = True
         assert torch.equal(outs[t][:, sel], shard[t][:, sel]) and torch.count_nonzero(outs[t][:, ~sel]) == 0
+# the zero-copy chunk lists: every [n, d] block lands where the kernel reads it, and comes back where the caller reads it
+for grp in range(G):
+    heads = [torch.full((B, hg, N, d), float("nan")) for _ in range(6)]
+    ulysses._exchange_p2p(ulysses.p2p_chunks_in(shard[:6], heads, P, rank, grp, G), rank, None).wait()
+    for t in range(6):
+        assert torch.equal(heads[t], full[t][:, rank * h + grp * hg:rank * h + (grp + 1) * hg])
+    outs = [torch.zeros_like(x) for x in shard[:6]]
+    ulysses._exchange_p2p(ulysses.p2p_chunks_out(heads, outs, P, rank, grp, G), rank, None).wait()
+    for t in range(6):
+        sel = torch.zeros(H, dtype=torch.bool)
+        for j in range(P):
+            sel[j * h + grp * hg:j * h + (grp + 1) * hg] = True
+        assert torch.equal(outs[t][:, sel], shard[t][:, sel]) and torch.count_nonzero(outs[t][:, ~sel]) == 0
+# both exchange modes give the same bits
+o2, to2, saved2 = ulysses.ulysses_attn_jvp(local_op, *shard[:6], head_groups=G, mode="packed")
+dq2, dk2, dv2 = ulysses.ulysses_attn_bwd(local_bwd, saved2, shard[6], head_groups=G, mode="packed")
+calls.clear()
 o, to, saved = ulysses.ulysses_attn_jvp(local_op, *shard[:6], head_groups=G)
 dq, dk, dv = ulysses.ulysses_attn_bwd(local_bwd, saved, shard[6], head_groups=G)
+for a, b in zip((o, to, dq, dk, dv), (o2, to2, dq2, dk2, dv2)):
+    assert torch.equal(a, b)
 sl = slice(rank * n, (rank + 1) * n)
 ro, rto, rlse = oracle.attn_jvp(om, *[t.numpy() for t in full[:6]], 1.0 / np.sqrt(d))     # the undistributed result
 err = dict(o=float(np.abs(o.numpy() - ro[:, :, sl]).max()), to=float(np.abs(to.numpy() - rto[:, :, sl]).max()))
