@@ -7,8 +7,13 @@ all-to-all brings the outputs back.  PAPER.md:358-360: with the JVP the tangents
 Q, K, V, O and lse stay head-sharded on the rank between the two calls.
 
 How the exchange is organised here
-  * The rank's H/P heads are cut into `head_groups` groups.  Per group and direction ALL tensors travel in ONE
-    `all_to_all_single` (NCCL over NVLink / NVSwitch on GPUs; gloo in the CPU tests).
+  * The rank's H/P heads are cut into `head_groups` groups.  Per group and direction ALL tensors travel in ONE group of
+    point-to-point transfers (`mode="p2p"`, the default: `dist.batch_isend_irecv` = one ncclGroupStart / End on GPUs) whose
+    chunks are the `[n, d]` blocks themselves -- sent from the `[B, H, n, d]` shard in place and received at rows
+    `[i n, (i + 1) n)` of the `[B, hg, N, d]` tensor the kernel reads (and back: sent from the kernel's output in place,
+    received in the `[B, H, n, d]` result).  No send buffer, no receive buffer, no pack or unpack pass; the rank's own chunk
+    is one strided copy.  `mode="packed"` is the earlier form: ONE `all_to_all_single` per group and direction around
+    `pack_*` / `unpack_*` copies (four extra passes over the data).
   * The groups are pipelined: the collective of group g + 1 is issued (async) before the kernel of group g is enqueued, and
     the outputs of group g go back while group g + 1 computes, so that the exchange hides under the kernel except for the
     first group's way in and the last group's way out.
@@ -87,14 +92,110 @@ def _exchange(send: torch.Tensor, group, async_op: bool):
     return recv, (work if async_op and work is not None else _Done())
 
 
+# ---------------------------------------------------------------------------------------------- zero-copy point-to-point exchange
+def p2p_chunks_in(ins: Sequence[torch.Tensor], heads: Sequence[torch.Tensor], P: int, r: int, g: int, G: int):
+    """The way in for head group g on rank r.  ins: T tensors `[B, H, n, d]` (my tokens, all heads); heads: T tensors
+    `[B, hg, P n, d]` (all tokens of my group-g heads).  -> [(peer, send_view, recv_view)] in the order both ends enumerate:
+    send_view = my tokens of peer's head (a contiguous `[n, d]` block of `ins`), recv_view = peer's tokens of my head (rows
+    `[peer n, (peer + 1) n)` of `heads`, contiguous).  peer == r: the same two views, to be copied locally."""
+    B, H, n, d = ins[0].shape
+    if H % (P * G):
+        raise ValueError(f"H = {H} is not divisible by context-parallel size {P} x head groups {G}")
+    h, hg = H // P, H // (P * G)
+    out = []
+    for j in range(P):
+        for t in range(len(ins)):
+            for b in range(B):
+                for i in range(hg):
+                    out.append((j, ins[t][b, j * h + g * hg + i], heads[t][b, i, j * n:(j + 1) * n]))
+    return out
+
+
+def p2p_chunks_out(res: Sequence[torch.Tensor], outs: Sequence[torch.Tensor], P: int, r: int, g: int, G: int):
+    """The way back: res = T tensors `[B, hg, P n, d]` (the local op's results on my group-g heads), outs = T tensors
+    `[B, H, n, d]` (my tokens, all heads).  send_view = peer's tokens of my head, recv_view = my tokens of peer's head."""
+    B, hg, N, d = res[0].shape
+    n, h = N // P, hg * G
+    out = []
+    for j in range(P):
+        for t in range(len(res)):
+            for b in range(B):
+                for i in range(hg):
+                    out.append((j, res[t][b, i, j * n:(j + 1) * n], outs[t][b, j * h + g * hg + i]))
+    return out
+
+
+class _Works:
+    def __init__(self, works):
+        self.works = works
+
+    def wait(self):
+        for w in self.works:
+            w.wait()
+        return True
+
+
+def _exchange_p2p(chunks, r: int, group):
+    """Issues every transfer of `chunks` as one batch (async); the rank's own chunks are copied in place.  -> work handle."""
+    ops = []
+    seq = {}                               # per peer: position of the chunk in that peer's sub-list (the same number at both ends)
+    for peer, send, recv in chunks:
+        if peer == r:
+            recv.copy_(send)
+        else:
+            k = seq[peer] = seq.get(peer, -1) + 1
+            dst = peer if group is None else dist.get_global_rank(group, peer)
+            ops.append(dist.P2POp(dist.isend, send, dst, group=group, tag=k))
+            ops.append(dist.P2POp(dist.irecv, recv, dst, group=group, tag=k))
+    return _Works(dist.batch_isend_irecv(ops)) if ops else _Done()
+
+
 LocalOp = Callable[..., Tuple[torch.Tensor, ...]]
 
 
-def _pipeline(ins: Sequence[torch.Tensor], n_out: int, local_op: LocalOp, group, head_groups: int, out_like: Sequence[int]):
+def _pipeline_p2p(ins: Sequence[torch.Tensor], n_out: int, local_op: LocalOp, group, head_groups: int, out_like: Sequence[int]):
+    """`_pipeline` with the zero-copy exchange: the transfers of group g + 1 are in flight under the kernel of group g, the
+    results of group g travel back under the kernel of group g + 1.  The head-sharded tensors are fresh allocations per call
+    (no pass over memory): the forward hands them to the caller as `saved`, which must outlive later calls."""
+    P, r, G = dist.get_world_size(group), dist.get_rank(group), head_groups
+    ins = [x if x.is_contiguous() else x.contiguous() for x in ins]
+    B, H, n, d = ins[0].shape
+    hg = H // (P * G)
+    outs = [torch.empty(ins[i].shape, dtype=ins[i].dtype, device=ins[i].device) for i in out_like]
+    extras: List = [None] * G
+
+    def way_in(g):
+        heads = [x.new_empty((B, hg, P * n, d)) for x in ins]
+        return heads, _exchange_p2p(p2p_chunks_in(ins, heads, P, r, g, G), r, group)
+
+    heads, work_in = way_in(0)
+    pending = []                                            # way-back transfers in flight (their source tensors kept alive)
+    for g in range(G):
+        nxt = way_in(g + 1) if g + 1 < G else None
+        work_in.wait()
+        res = local_op(g, *heads)
+        extras[g] = res[n_out:]
+        back = [t if t.is_contiguous() else t.contiguous() for t in res[:n_out]]
+        for wk, _ in pending:
+            wk.wait()
+        pending = [(_exchange_p2p(p2p_chunks_out(back, outs, P, r, g, G), r, group), back)]
+        if nxt is not None:
+            heads, work_in = nxt
+    for wk, _ in pending:
+        wk.wait()
+    return outs, extras
+
+
+def _pipeline(ins: Sequence[torch.Tensor], n_out: int, local_op: LocalOp, group, head_groups: int, out_like: Sequence[int],
+              mode: str = "p2p"):
     """Shared by the forward and the backward: `ins` = this rank's `[B, H, n, d]` tensors; per head group: exchange in,
     `local_op(g, *head_sharded_inputs)` -> n_out head-sharded `[B, hg, N, d]` tensors (+ anything it wants to keep, which
     is returned per group), exchange out.  out_like[i] = index of the input whose shape output i has.
     -> (outs `[B, H, n, d]`, [extras of group g])."""
+    if mode == "p2p":
+        return _pipeline_p2p(ins, n_out, local_op, group, head_groups, out_like)
+    if mode != "packed":
+        raise ValueError(f"unknown exchange mode {mode!r}")
     P = dist.get_world_size(group)
     G = head_groups
     outs = [torch.empty(ins[i].shape, dtype=ins[i].dtype, device=ins[i].device) for i in out_like]
@@ -118,24 +219,24 @@ def _pipeline(ins: Sequence[torch.Tensor], n_out: int, local_op: LocalOp, group,
     return outs, extras
 
 
-def ulysses_attn_jvp(local_op: LocalOp, q, k, v, tq, tk, tv, group=None, head_groups: int = 1):
+def ulysses_attn_jvp(local_op: LocalOp, q, k, v, tq, tk, tv, group=None, head_groups: int = 1, mode: str = "p2p"):
     """q, k, v, tq, tk, tv: this rank's `[B, H, N/P, d]` shards.  local_op(g, q, k, v, tq, tk, tv) -> (o, to, lse) on the
     head shard of group g.  -> (o, to) `[B, H, N/P, d]`, and `saved` = per head group (q, k, v, o, lse) head-sharded, which
     is what the primal backward on this rank consumes (lse never leaves the rank)."""
     def op(g, hq, hk, hv, htq, htk, htv):
         o, to, lse = local_op(g, hq, hk, hv, htq, htk, htv)
         return o, to, (hq, hk, hv, o, lse)
-    (o_l, to_l), extras = _pipeline((q, k, v, tq, tk, tv), 2, op, group, head_groups, (0, 0))
+    (o_l, to_l), extras = _pipeline((q, k, v, tq, tk, tv), 2, op, group, head_groups, (0, 0), mode)
     return o_l, to_l, [e[0] for e in extras]
 
 
-def ulysses_attn_bwd(local_bwd: LocalOp, saved, dout, group=None, head_groups: int = 1):
+def ulysses_attn_bwd(local_bwd: LocalOp, saved, dout, group=None, head_groups: int = 1, mode: str = "p2p"):
     """dout: this rank's `[B, H, N/P, d]` shard of dO; `saved` from ulysses_attn_jvp (same head_groups).
     local_bwd(g, q, k, v, o, lse, dout) -> (dq, dk, dv) on the head shard.  -> dq, dk, dv `[B, H, N/P, d]`."""
     def op(g, hdo):
         hq, hk, hv, o, lse = saved[g]
         return local_bwd(g, hq, hk, hv, o, lse, hdo)
-    (dq, dk, dv), _ = _pipeline((dout,), 3, op, group, head_groups, (0, 0, 0))
+    (dq, dk, dv), _ = _pipeline((dout,), 3, op, group, head_groups, (0, 0, 0), mode)
     return dq, dk, dv
 
 
@@ -172,14 +273,35 @@ def local_attn_bwd(plan, stream: Optional[int] = None) -> LocalOp:
 
 
 # ---------------------------------------------------------------------------------------------- single-process emulation
+def _deliver(plans):
+    """plans[r] = rank r's chunk list: the k-th chunk rank i sends to rank j lands in the k-th chunk rank j receives from rank i."""
+    P = len(plans)
+    for i in range(P):
+        for j in range(P):
+            sends = [c[1] for c in plans[i] if c[0] == j]
+            recvs = [c[2] for c in plans[j] if c[0] == i]
+            assert len(sends) == len(recvs)
+            for s_, r_ in zip(sends, recvs):
+                r_.copy_(s_)
+
+
 def emulate_ranks(P: int, shards: Sequence[Sequence[torch.Tensor]], n_out: int, local_op: LocalOp, head_groups: int = 1,
-                  out_like: Optional[Sequence[int]] = None):
-    """P virtual ranks in ONE process (tests; one GPU): shards[r] = rank r's `[B, H, n, d]` tensors.  Runs the same
-    pack / unpack functions as `_pipeline`, with the all-to-all replaced by its definition (recv_r[i] = send_i[r]).
-    -> outs[r] = rank r's n_out output shards."""
+                  out_like: Optional[Sequence[int]] = None, mode: str = "p2p"):
+    """P virtual ranks in ONE process (tests; one GPU): shards[r] = rank r's `[B, H, n, d]` tensors.  Runs the same index
+    arithmetic as `_pipeline` (`p2p_chunks_*`, or `pack_*` / `unpack_*` for mode="packed"), with the transfers replaced by
+    their definition.  -> outs[r] = rank r's n_out output shards."""
     G = head_groups
     out_like = out_like or [0] * n_out
     outs = [[torch.empty(shards[r][i].shape, dtype=shards[r][i].dtype, device=shards[r][i].device) for i in out_like] for r in range(P)]
+    if mode == "p2p":
+        B, H, n, d = shards[0][0].shape
+        hg = H // (P * G)
+        for g in range(G):
+            heads = [[x.new_empty((B, hg, P * n, d)) for x in shards[r]] for r in range(P)]
+            _deliver([p2p_chunks_in(shards[r], heads[r], P, r, g, G) for r in range(P)])
+            res = [local_op(r, g, *heads[r])[:n_out] for r in range(P)]
+            _deliver([p2p_chunks_out([t.contiguous() for t in res[r]], outs[r], P, r, g, G) for r in range(P)])
+        return outs
     for g in range(G):
         sends = [pack_seq_shard(shards[r], P, g, G) for r in range(P)]
         backs = []
