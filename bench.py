@@ -669,8 +669,8 @@ def run_ulysses(args, w: Workload):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    step_ms = timed(lambda: ulysses.ulysses_attn_jvp(local_op, *shard, head_groups=G))
-    comm_ms = timed(lambda: ulysses.ulysses_attn_jvp(noop, *shard, head_groups=G))
+    step_ms = timed(lambda: ulysses.ulysses_attn_jvp(local_op, *shard, head_groups=G, mode=args.exchange))
+    comm_ms = timed(lambda: ulysses.ulysses_attn_jvp(noop, *shard, head_groups=G, mode=args.exchange))
     kernel_ms = None
     if cuda:
         hs = [torch.empty((w.B, hg, w.N, w.d), dtype=w.torch_dtype, device=dev).normal_() for _ in range(6)]
@@ -682,7 +682,7 @@ def run_ulysses(args, w: Workload):
         peaks, peak_src = load_peaks()
         line = {"metric": METRIC, "value": flops / (step_ms * 1e-3) / 1e12 if cuda else None, "unit": UNIT, "n_gpus": world,
                 "steps": K, "warmup": W, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-                "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "mode": "ulysses",
+                "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "mode": "ulysses", "exchange": args.exchange,
                 "config": dict(workload_config(w), parallelism=f"ulysses cp{P}, {G} head group(s) per rank",
                                tokens_per_rank=n, heads_per_rank=w.H // P),
                 "comm_ms": comm_ms, "kernel_ms": kernel_ms, "a2a_bytes_in_per_rank": bytes_in, "a2a_bytes_out_per_rank": bytes_out,
@@ -693,7 +693,7 @@ def run_ulysses(args, w: Workload):
             peak = float(peaks.get("bf16_tflops", FALLBACK_PEAKS["bf16_tflops"])) * world
             line["roofline"] = {"bound": "tensor", "achieved": line["value"], "peak": peak, "unit": "TFLOP/s",
                                 "frac": line["value"] / peak, "traffic": None, "peak_source": f"{peak_src} bf16_tflops x {world} GPUs",
-                                "kernel": "attn_jvp_umma_pair_kernel + all_to_all_single"}
+                                "kernel": "attn_jvp_umma_pair_kernel + " + ("batch_isend_irecv (zero-copy chunks)" if args.exchange == "p2p" else "all_to_all_single (packed)")}
         print(json.dumps(line), flush=True)
     dist.destroy_process_group()
 
@@ -711,6 +711,8 @@ def main():
     ap.add_argument("--bwd-parity-samples", type=int, default=512, help="backward workloads: query rows / keys of head (0,0) held against the oracle")
     ap.add_argument("--ulysses", action="store_true", help="sequence-sharded ranks with the all-to-all on both sides of the kernel")
     ap.add_argument("--head-groups", type=int, default=2, help="--ulysses: head groups per rank (exchange / kernel pipelining)")
+    ap.add_argument("--exchange", default="p2p", choices=["p2p", "packed"],
+                    help="--ulysses: zero-copy grouped point-to-point transfers (default) or the packed all_to_all_single")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     w = {**WORKLOADS, **EXTRA_WORKLOADS}[args.workload]
