@@ -12,9 +12,9 @@
 //     W = exp2(X s log2e - lse log2e),   Z = W o (Y - delta)       two exp / dS warpgroups, 32 of a tile's 64 columns each,
 //                                                                    tile j0 first; thread = stationary row = TMEM lane
 //     per tile: acc1 += Z B1  (and acc2 += W B2)                    4 (+ 4) x (M256 N128 K16), A = bf16 Z / W in TMEM
-//   KEYS = false (dQ):     stationary = query rows (A1 = Q, A2 = dO), streamed = keys (B1 = K, B2 = V); acc1 = dQ / s; lse and
-//                          delta belong to the thread's own row.  Q and dO rows live in TMEM as bf16 A operands (written by
-//                          the exp / dS warps once per task), so the X / Y MMAs read only B from shared memory.
+//   dQ:                    attn_bwd_dq_pair_kernel below (tile ping-pong; stationary = query rows, Q and dO rows as bf16 A
+//                          operands in TMEM).  A pair-step form of it used to be the KEYS = false instantiation of this
+//                          template; it was measured slower and has been removed.
 //   KEYS = true (dK, dV):  stationary = keys (A1 = K, A2 = V in shared memory), streamed = query rows (B1 = Q, B2 = dO):
 //                          X = S^T, Y = dP^T, acc1 = dK / s, acc2 = dV; lse and delta belong to the COLUMNS, and they are
 //                          folded INTO the two contractions: one extra K step (16 of the bf16 K dimension) multiplies a
@@ -117,9 +117,10 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap
         ::"r"(dst), "l"(map), "r"(cluster_bar), "r"(c0), "r"(c1) : "memory");
 }
 
-template <bool KEYS>
+template <bool KEYS>   // only KEYS = true exists (the dQ pass has its own kernel below); the parameter keeps the kernel's name
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
+    static_assert(KEYS, "the pair-step form of the dQ pass was removed (measured slower: DESIGN.md 6d); dQ runs attn_bwd_dq_pair_kernel");
     using C = Cfg<KEYS>;
     constexpr int NSTAGE = C::NSTAGE;
     extern __shared__ uint8_t smem_raw[];
@@ -129,7 +130,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
     const uint32_t sA1 = tiles, sA2 = tiles + A_BYTES, sRing = tiles + C::A_SMEM, sAug = sRing + NSTAGE * SLOT_BYTES;
     const uint32_t sOnes = sAug + AUG_STAGES * AUG_STAGE_BYTES;
     const uint32_t bars = smem_u32(sh->bars);
-    const PairWaiter wait{bars, &sh->abort_flag, prm.err, KEYS ? 300 : 200};
+    const PairWaiter wait{bars, &sh->abort_flag, prm.err, 300};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();              // 0 = leader (issues the MMAs, owns the "full" barriers)
     const uint32_t lead_bars = mapa(bars, 0);
@@ -137,7 +138,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
     const int list_begin = prm.pair_off[pair], list_end = prm.pair_off[pair + 1];
 
     if (threadIdx.x == 0) {
-        mbar_init(bars + 8 * BAR_A_FULL, KEYS ? 1 : 16);
+        mbar_init(bars + 8 * BAR_A_FULL, 1);
         mbar_init(bars + 8 * BAR_A_EMPTY, 1);
         for (int i = 0; i < MAX_STAGE; ++i) { mbar_init(bars + 8 * (BAR_KV_FULL + i), 1); mbar_init(bars + 8 * (BAR_KV_EMPTY + i), 1); }
         mbar_init(bars + 8 * BAR_X_FULL, 1);
@@ -152,7 +153,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
-    if (KEYS && threadIdx.x >= 128 && threadIdx.x < 128 + BR) {
+    if (threadIdx.x >= 128 && threadIdx.x < 128 + BR) {
         // the constant A operand of the augmentation step: row r = [1, 1, 0 x 6, 1, 1, 0 x 6] (bf16 1.0 = 0x3f80)
         uint8_t *ones = smem_raw + (tiles - raw) + C::A_SMEM + NSTAGE * SLOT_BYTES + AUG_STAGES * AUG_STAGE_BYTES + (threadIdx.x - 128) * 32;
         reinterpret_cast<uint4 *>(ones)[0] = make_uint4(0x3f803f80u, 0u, 0u, 0u);
@@ -174,13 +175,13 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
         // ================================================= TMA producer (both CTAs) ================================
         if (lane == 0) {
             prefetch_tmap(&prm.tm_b1); prefetch_tmap(&prm.tm_b2);
-            if (KEYS) { prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_aug1); prefetch_tmap(&prm.tm_aug2); }
+            prefetch_tmap(&prm.tm_a1); prefetch_tmap(&prm.tm_a2); prefetch_tmap(&prm.tm_aug1); prefetch_tmap(&prm.tm_aug2);
             uint32_t ring = 0, na = 0;
             for (int it = list_begin; it < list_end; ++it) {
                 const aj_task task = prm.tasks[prm.pair_ids[it]];
                 const int n = task.num_kv_tiles;
                 if (n == 0 || sh->abort_flag) continue;
-                if (KEYS) {   // this CTA's 128 stationary rows of K and V, two 64-column swizzle blocks each
+                {   // this CTA's 128 stationary rows of K and V, two 64-column swizzle blocks each
                     wait(BAR_A_EMPTY, (na & 1) ^ 1);
                     const uint32_t afull = lead_bars + 8 * BAR_A_FULL;
                     if (rank == 0) mbar_expect_tx(bars + 8 * BAR_A_FULL, 4 * A_BYTES);
@@ -204,13 +205,13 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         const uint32_t slot = ring % NSTAGE;
                         wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                         const uint32_t dst = sRing + slot * SLOT_BYTES, full = lead_bars + 8 * (BAR_KV_FULL + slot);
-                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES + (KEYS ? 2 * AUG_STAGE_BYTES : 0));
+                        if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES + 2 * AUG_STAGE_BYTES);
                         const int row = rank ? t1.key_row : t0.key_row;
                         tma_load_4d_pair(dst, &prm.tm_b1, full, 0, row, task.h, task.b);
                         tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_b1, full, 64, row, task.h, task.b);
                         tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_b2, full, 0, row, task.h, task.b);
                         tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_b2, full, 64, row, task.h, task.b);
-                        if (KEYS) {   // the 16 extra K columns of the tile's rows: -lse/s for X, -delta for Y (slots 0 and 2 hold such tiles)
+                        {   // the 16 extra K columns of the tile's rows: -lse/s for X, -delta for Y (slots 0 and 2 hold such tiles)
                             const uint32_t adst = sAug + (slot >> 1) * AUG_STAGE_BYTES;
                             tma_load_2d_pair(adst, &prm.tm_aug1, full, 0, (int)(ld_base + row));
                             tma_load_2d_pair(adst + AUG_TILE_BYTES, &prm.tm_aug2, full, 0, (int)(ld_base + row));
@@ -222,16 +223,12 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         wait(BAR_KV_EMPTY + slot, ((ring / NSTAGE) & 1) ^ 1);
                         const uint32_t dst = sRing + slot * SLOT_BYTES, full = lead_bars + 8 * (BAR_KV_FULL + slot);
                         const int col = 64 * (int)rank;
-                        if (KEYS) {   // [B1(j0) | B2(j0) | B1(j1) | B2(j1)]
+                        {   // [B1(j0) | B2(j0) | B1(j1) | B2(j1)]
                             if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), 2 * SLOT_BYTES);
                             tma_load_4d_pair(dst, &prm.tm_b1, full, col, t0.key_row, task.h, task.b);
                             tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_b2, full, col, t0.key_row, task.h, task.b);
                             tma_load_4d_pair(dst + 2 * BLK_BYTES, &prm.tm_b1, full, col, t1.key_row, task.h, task.b);
                             tma_load_4d_pair(dst + 3 * BLK_BYTES, &prm.tm_b2, full, col, t1.key_row, task.h, task.b);
-                        } else {      // [B1(j0) | B1(j1)]
-                            if (rank == 0) mbar_expect_tx(bars + 8 * (BAR_KV_FULL + slot), SLOT_BYTES);
-                            tma_load_4d_pair(dst, &prm.tm_b1, full, col, t0.key_row, task.h, task.b);
-                            tma_load_4d_pair(dst + BLK_BYTES, &prm.tm_b1, full, col, t1.key_row, task.h, task.b);
                         }
                         ++ring;
                     }
@@ -266,10 +263,9 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         for (int ks = 0; ks < D / 16; ++ks) {       // [X(j0) | X(j1)] = A1 [B1(j0) ; B1(j1)]^T
                             const uint32_t aoff = ((ks >> 2) * AHALF_BYTES + (ks & 3) * 32) >> 4;
                             const uint32_t boff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
-                            if (KEYS) mma_ss_pair(tmem + TM_X, a1_lo + aoff, DESC_HI, b_lo + boff, DESC_HI, IDESC_XY, ks > 0);
-                            else mma_ts_pair(tmem + TM_X, tmem + TM_A1 + ks * 8, b_lo + boff, DESC_HI, IDESC_XY, ks > 0);
+                            mma_ss_pair(tmem + TM_X, a1_lo + aoff, DESC_HI, b_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                         }
-                        if (KEYS)                                   // X -= lse / s of the column's query row (augmentation step)
+                        // X -= lse / s of the column's query row (augmentation step)
                             mma_ss_pair(tmem + TM_X, ones_lo, DESC_HI_SW32, aug_lo(xslot), DESC_HI_SW32, IDESC_XY, 1u);
                         tc_commit_pair(bars + 8 * BAR_X_FULL, 3);
                     }
@@ -283,14 +279,13 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         for (int ks = 0; ks < D / 16; ++ks) {       // [Y(j0) | Y(j1)] = A2 [B2(j0) ; B2(j1)]^T
                             const uint32_t aoff = ((ks >> 2) * AHALF_BYTES + (ks & 3) * 32) >> 4;
                             const uint32_t boff = ((ks >> 2) * BLK_BYTES + (ks & 3) * 32) >> 4;
-                            if (KEYS) mma_ss_pair(tmem + TM_Y, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);
-                            else mma_ts_pair(tmem + TM_Y, tmem + TM_A2 + ks * 8, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);
+                            mma_ss_pair(tmem + TM_Y, a2_lo + aoff, DESC_HI, b2_lo + boff, DESC_HI, IDESC_XY, ks > 0);
                         }
-                        if (KEYS)                                   // Y -= delta of the column's query row
+                        // Y -= delta of the column's query row
                             mma_ss_pair(tmem + TM_Y, ones_lo, DESC_HI_SW32, aug_lo(xslot) + (AUG_TILE_BYTES >> 4), DESC_HI_SW32, IDESC_XY, 1u);
                         tc_commit_pair(bars + 8 * BAR_Y_FULL, 3);
                         tc_commit_pair(bars + 8 * (BAR_KV_EMPTY + xslot), 3);
-                        if (last && KEYS) tc_commit_pair(bars + 8 * BAR_A_EMPTY, 3);   // every X / Y of this task has been issued
+                        if (last) tc_commit_pair(bars + 8 * BAR_A_EMPTY, 3);   // every X / Y of this task has been issued
                     }
                     __syncwarp();
                 };
@@ -303,7 +298,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     // MN-major operands, this CTA's 64 columns: streamed row r at r * 128 B, 16-row K steps 2 KB apart
                     const uint32_t m_lo = (((sRing + mslot * SLOT_BYTES) >> 4) & 0x3FFF) | LBO_CANON;
                     const uint32_t acc = p > 0 ? 1u : 0u;
-                    if (KEYS) {
+                    {
 #pragma unroll
                         for (int i = 0; i < 2; ++i) {
                             const uint32_t b2i_lo = m_lo + (((2 * i + 1) * BLK_BYTES) >> 4);
@@ -318,14 +313,10 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                             __syncwarp();
                         }
                         if (p + 1 < np) issue_x();                  // overwrites W(p): the pipe executes in order
-                    } else if (p + 1 < np) {
-                        wait(BAR_X_FREE, c_step & 1);               // the exp / dS warps hold X(p) in registers
-                        tc_fence_after();
-                        issue_x();
                     }
 #pragma unroll
                     for (int i = 0; i < 2; ++i) {
-                        const uint32_t b1i_lo = m_lo + (((KEYS ? 2 * i : i) * BLK_BYTES) >> 4);
+                        const uint32_t b1i_lo = m_lo + (((2 * i) * BLK_BYTES) >> 4);
                         const uint32_t tZ = tmem + TM_Y + i * BC;
                         wait(BAR_Z_FULL + i, c_step & 1);
                         tc_fence_after();
@@ -361,31 +352,6 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
             const int n = task.num_kv_tiles;
             const bool store = prow < task.q_rows;
             const int64_t grow = task.q_begin + prow;
-            // ---- dQ pass: this thread's own {lse log2e, delta}; its row of Q (warpgroup 0) or dO (warpgroup 1) as a bf16 A
-            // operand in TMEM (16 elements = 8 columns per MMA K step).  The previous task's MMAs are complete (its epilogue
-            // waited for them) and both warpgroups have left that epilogue (named barrier).
-            uint64_t myl_2 = 0ull, myd_2 = 0ull;
-            if (!KEYS && n > 0) {
-                float2 my = make_float2(0.f, 0.f);
-                if (store) my = prm.ld[((int64_t)task.b * prm.H + task.h) * prm.Nq + grow];
-                myl_2 = pack2(-my.x, -my.x); myd_2 = pack2(-my.y, -my.y);
-                const aj_tensor &src = wg ? prm.a2 : prm.a1;
-                const uint4 *rowp = (const uint4 *)((const __nv_bfloat16 *)src.ptr + task.b * src.stride_b + task.h * src.stride_h + grow * src.stride_n);
-#pragma unroll
-                for (int half = 0; half < 2; ++half) {
-                    uint32_t ra[32];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const uint4 u = store ? rowp[half * 8 + i] : make_uint4(0, 0, 0, 0);
-                        ra[4 * i] = u.x; ra[4 * i + 1] = u.y; ra[4 * i + 2] = u.z; ra[4 * i + 3] = u.w;
-                    }
-                    tmem_st32(tmem + lane_base + (wg ? TM_A2 : TM_A1) + 32 * half, ra);
-                }
-                tc_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * BAR_A_FULL);
-            }
             RowCursor cur;
             cur.init(prm.r_begin, prm.r_end, prm.rows, task.range_begin, task.range_count, prow);
             const int np = (n + 1) >> 1;
@@ -416,8 +382,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     const uint32_t (&xu)[32] = xu2[i];
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
-                        // dQ pass: this thread's row's -lse log2e; KEYS: -lse / s of the column is already inside X
-                        const uint64_t x = KEYS ? fmul2(pack2(xu[c], xu[c + 1]), sl2_2) : ffma2(pack2(xu[c], xu[c + 1]), sl2_2, myl_2);
+                        const uint64_t x = fmul2(pack2(xu[c], xu[c + 1]), sl2_2);      // -lse / s of the column is already inside X
                         float x0, x1;                          // (half of these on the FMA pipe was measured slower: DESIGN.md 6d)
                         unpack2(x, x0, x1);
                         w[i][c] = ex2(x0);
@@ -428,7 +393,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
 #pragma unroll                                                 // exponential: the masked operands may be anything, even inf - inf)
                         for (int c = 0; c < 32; ++c) if (c >= v) w[i][c] = 0.f;
                     }
-                    if (KEYS) {
+                    {                                          // bf16 W = P^T, the A operand of dV += P^T dO
                         uint32_t wk[16];
 #pragma unroll
                         for (int c = 0; c < 16; ++c) wk[c] = pack_bf16(w[i][2 * c], w[i][2 * c + 1]);
@@ -438,11 +403,6 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         __syncwarp();
                         if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * (BAR_W_FULL + i));
                     }
-                }
-                if (!KEYS) {                                   // X(p) is in registers: X(p+1) may overwrite it
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(lead_bars + 8 * BAR_X_FREE);
                 }
                 // ---- Z = W o (Y - delta) = dS / s
                 wait(BAR_Y_FULL, c_step & 1);
@@ -457,7 +417,7 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                     uint32_t zk[16];
 #pragma unroll
                     for (int c = 0; c < 32; c += 2) {
-                        const uint64_t y = KEYS ? pack2(yu[c], yu[c + 1]) : fadd2(pack2(yu[c], yu[c + 1]), myd_2);   // KEYS: -delta is inside Y
+                        const uint64_t y = pack2(yu[c], yu[c + 1]);                 // -delta is inside Y
                         const uint64_t z = fmul2(pack2(w[i][c], w[i][c + 1]), y);
                         float z0, z1;
                         unpack2(z, z0, z1);
@@ -477,11 +437,11 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
             }
             // ---- epilogue: acc1 * s -> dQ | dK, acc2 -> dV; each warpgroup writes one 64-column half ----
             __nv_bfloat16 *o1 = (__nv_bfloat16 *)prm.out1.ptr + task.b * prm.out1.stride_b + task.h * prm.out1.stride_h + grow * prm.out1.stride_n;
-            __nv_bfloat16 *o2 = KEYS ? (__nv_bfloat16 *)prm.out2.ptr + task.b * prm.out2.stride_b + task.h * prm.out2.stride_h + grow * prm.out2.stride_n : nullptr;
+            __nv_bfloat16 *o2 = (__nv_bfloat16 *)prm.out2.ptr + task.b * prm.out2.stride_b + task.h * prm.out2.stride_h + grow * prm.out2.stride_n;
             if (n == 0) {                                           // a row without keys / a key no row sees: zeros
                 if (store) {
                     const uint4 z = make_uint4(0, 0, 0, 0);
-                    for (int c = 8 * wg; c < 8 * wg + 8; ++c) { ((uint4 *)o1)[c] = z; if (KEYS) ((uint4 *)o2)[c] = z; }
+                    for (int c = 8 * wg; c < 8 * wg + 8; ++c) { ((uint4 *)o1)[c] = z; ((uint4 *)o2)[c] = z; }
                 }
                 continue;
             }
@@ -494,8 +454,8 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
             for (int cb = 64 * wg; cb < 64 * wg + 64; cb += 32) {
                 uint32_t a1[32], a2[32];
                 tmem_ld32(tmem + lane_base + TM_ACC1 + cb, a1);
-                if (KEYS) tmem_ld32(tmem + lane_base + TM_ACC2 + cb, a2);
-                if (KEYS) tc_wait_ld(a1, a2); else tc_wait_ld(a1);
+                tmem_ld32(tmem + lane_base + TM_ACC2 + cb, a2);
+                tc_wait_ld(a1, a2);
                 if (store) {
 #pragma unroll
                     for (int v4 = 0; v4 < 4; ++v4) {
@@ -504,10 +464,10 @@ attn_bwd_umma_pair_kernel(const __grid_constant__ BwdPairParams prm) {
                         for (int e = 0; e < 4; ++e) {
                             const int c = v4 * 8 + 2 * e;
                             w1[e] = pack_bf16(__uint_as_float(a1[c]) * prm.scale, __uint_as_float(a1[c + 1]) * prm.scale);
-                            if (KEYS) w2[e] = pack_bf16(__uint_as_float(a2[c]), __uint_as_float(a2[c + 1]));
+                            w2[e] = pack_bf16(__uint_as_float(a2[c]), __uint_as_float(a2[c + 1]));
                         }
                         *(uint4 *)(o1 + cb + v4 * 8) = make_uint4(w1[0], w1[1], w1[2], w1[3]);
-                        if (KEYS) *(uint4 *)(o2 + cb + v4 * 8) = make_uint4(w2[0], w2[1], w2[2], w2[3]);
+                        *(uint4 *)(o2 + cb + v4 * 8) = make_uint4(w2[0], w2[1], w2[2], w2[3]);
                     }
                 }
             }
